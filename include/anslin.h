@@ -1,0 +1,174 @@
+/*
+ * anslin.h — C ABI of libanslin: tile-level rANS weight compression fused into tcgen05 GEMM on B200.
+ *
+ * Follows the problem statement of arxiv/paper_2606_15789 (P = /root/reference/PAPER.md):
+ *   offline: compress each projection matrix into tile-aligned, independently decodable rANS
+ *            substreams with one shared per-matrix codebook and a 4-byte offset per tile
+ *            (P:l.149 §IV-A, P:l.165-169 §V-B, Eq.3 P:l.440);
+ *   run time: decode tiles on the SMs straight into shared memory and feed the tensor cores
+ *            (P:l.181-252 Alg V.1, P:l.260-287 Alg V.2, P:l.301-304 Alg V.3), or decode only.
+ *
+ * Conventions (all entry points):
+ *   - return value: anslin_status (0 = ANSLIN_OK); no exceptions, no abort, nothing printed.
+ *   - "host" pointers are CPU memory, "dev" pointers are CUDA device memory of the current device.
+ *   - the CALLER owns every buffer; the library allocates no device memory and keeps no global
+ *     state.  Handles (anslin_weight) are small host objects released with anslin_close.
+ *   - kernels are enqueued on the caller's stream and run asynchronously; asynchronous faults
+ *     surface at the caller's next synchronisation.  No hidden synchronisation.
+ *   - device pointers must be 16-byte aligned (else ANSLIN_ERR_INVALID_ARG).
+ *   - shapes: n_out % 128 == 0 and k_in % tile_k == 0 (else ANSLIN_ERR_UNSUPPORTED); m >= 1.
+ *   - orientation: W is [n_out x k_in] row-major (torch Linear.weight), X is [m x k_in] row-major
+ *     with leading dimension ldx (elements), Y is [m x n_out] row-major float32 with ldy.
+ *   - there is no CPU fallback: the device entry points fail with ANSLIN_ERR_CUDA when no sm_100
+ *     device / driver is usable.
+ *
+ * The byte layout of a container is specified in DESIGN.md §"Container".
+ */
+#ifndef ANSLIN_H
+#define ANSLIN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  ANSLIN_OK = 0,
+  ANSLIN_ERR_INVALID_ARG = 1,
+  ANSLIN_ERR_UNSUPPORTED = 2,
+  ANSLIN_ERR_BUFFER_TOO_SMALL = 3,
+  ANSLIN_ERR_CORRUPT = 4,
+  ANSLIN_ERR_CUDA = 5
+} anslin_status;
+
+/* Numeric format of W (P:l.80, l.341; BASELINE.json configs 1-5). */
+typedef enum {
+  ANSLIN_FMT_BF16 = 0,     /* w_host: uint16 bit patterns; coded symbol = exponent byte, sign+mantissa raw */
+  ANSLIN_FMT_FP8_E4M3 = 1, /* w_host: e4m3fn bytes; coded symbol = the byte; per-tensor scale in desc.w_scale */
+  ANSLIN_FMT_INT8 = 2,     /* w_host: int8; coded symbol = the byte; scales_host = fp16[n_out] (SQ8-style) */
+  ANSLIN_FMT_INT4_AWQ = 3  /* w_host: uint8[n_out][k_in/2], low nibble = even k; coded symbol = packed byte;
+                              scales_host/zeros_host = fp16[n_out][k_in/group_size]; w = (q - z) * s */
+} anslin_format;
+
+/* Element type of X. */
+typedef enum {
+  ANSLIN_DT_F32 = 0, ANSLIN_DT_F16 = 1, ANSLIN_DT_BF16 = 2, ANSLIN_DT_I8 = 3, ANSLIN_DT_FP8_E4M3 = 4
+} anslin_dtype;
+
+/* Container flag bits. */
+#define ANSLIN_FLAG_STATE_PAYLOAD 1u /* bf16: each lane's rANS start state carries its last two raw-plane
+                                        bytes ("arbitrary initial states", P:l.167; A4) */
+
+/* What the caller states about W. */
+typedef struct {
+  uint32_t format;      /* anslin_format */
+  uint32_t n_out, k_in; /* W is [n_out x k_in] */
+  uint32_t tile_k;      /* K extent of one tile in weights; 0 = format default (bf16 64, fp8/int8/int4 256);
+                           tile rows are always 128 (= tcgen05 MMA M); 32 interleaved streams per tile */
+  uint32_t group_size;  /* int4: quantisation group along K (multiple of 16); else 0 */
+  uint32_t flags;       /* ANSLIN_FLAG_* */
+  float    w_scale;     /* fp8: per-tensor dequant scale applied to Y; other formats: ignored (1.0) */
+  uint32_t reserved;
+} anslin_desc;
+
+/* Size accounting filled by the encoder (P:l.444 reports payload and metadata separately). Bits. */
+typedef struct {
+  uint64_t n_weights;
+  uint64_t payload_bits;      /* rANS words */
+  uint64_t state_bits;        /* 32 x 32-bit lane states per tile */
+  uint64_t pad_bits;          /* 16-byte record padding */
+  uint64_t offset_table_bits; /* 4 B per tile (+1 sentinel): Eq.3 first term */
+  uint64_t freq_table_bits;   /* 256 x u16 */
+  uint64_t raw_bits;          /* bf16 sign+mantissa plane */
+  uint64_t side_bits;         /* scales / zeros (reported separately from bits/weight) */
+  uint64_t total_bytes;
+  double entropy_bits_per_symbol; /* H of the coded-symbol histogram (P:l.70) */
+  double xent_bits_per_symbol;    /* cross entropy under the 12-bit table */
+  double raw_entropy_bits_per_symbol; /* bf16 raw plane's own order-0 entropy, else 0 */
+  double bits_per_weight;         /* 8 * (total_bytes - side bytes) / n_weights */
+} anslin_stats;
+
+/* Worst-case container size in bytes for `desc` (0 if desc is invalid). Host only. */
+size_t anslin_encode_bound(const anslin_desc *desc);
+
+/*
+ * Offline CPU encoder and tile packer (P:l.165-169): histogram over the whole matrix, 12-bit
+ * normalisation, per-tile 32-lane interleaved rANS with 16-bit words and 32-bit states.
+ *   w_host, scales_host, zeros_host: host, read only (see anslin_format for shapes).
+ *   container_out: host, capacity bytes; *bytes_out = bytes written.  stats_or_null: host.
+ * Errors: INVALID_ARG (null/desc), UNSUPPORTED (shape/format), BUFFER_TOO_SMALL.
+ */
+int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *scales_host,
+                       const void *zeros_host, void *container_out, size_t capacity,
+                       size_t *bytes_out, anslin_stats *stats_or_null);
+
+/* Host handle over a container whose bytes the caller has placed in device memory. */
+typedef struct anslin_weight anslin_weight;
+
+/*
+ * Validate a container and bind it to its device copy.
+ *   container_host: host copy (at least header + freq + offset sections; `bytes` = how many are
+ *   readable); container_dev: device copy of the WHOLE container (16-byte aligned), may be NULL
+ *   for host-only inspection.  Checks magic/version/shape/section bounds, that the frequency table
+ *   sums to 2^12 and that tile offsets are monotone and in range -> ANSLIN_ERR_CORRUPT otherwise
+ *   (so that no kernel can be steered out of bounds by a damaged table).
+ */
+int anslin_open(const void *container_host, size_t bytes, const void *container_dev, anslin_weight **out);
+int anslin_close(anslin_weight *w);
+/* Copy of the descriptor the container was encoded with (tile_k resolved). */
+int anslin_describe(const anslin_weight *w, anslin_desc *out);
+
+/*
+ * Decode only, to HBM (the paper's unfused stage, Fig. 9 P:l.410): writes W row-major in its
+ * original dtype/packing to w_out_dev (capacity >= n_out*k_in*bytes_per_weight).
+ * `stream` is a cudaStream_t passed as void*.
+ */
+int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void *stream);
+
+/* Scratch bytes anslin_gemm needs for batch m (split-K partials + counters). */
+size_t anslin_gemm_workspace_bytes(const anslin_weight *w, int32_t m);
+
+/*
+ * Fused decode + GEMM, Y = X . W^T (Alg V.1): only compressed bytes of W cross HBM.
+ *   x_dev: [m x k_in], dtype per format: bf16 -> BF16, int4 -> F16, int8 -> I8, fp8 -> FP8_E4M3.
+ *   x_scale_dev: int8/fp8: f32[m] per-token scales; else NULL.
+ *   y_dev: f32 [m x n_out]; int8: acc * x_scale[m] * w_scale[n]; fp8: acc * x_scale[m] * desc.w_scale.
+ *   1 <= m <= 256.
+ */
+int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m,
+                const void *x_scale_dev, void *y_dev, int64_t ldy, void *workspace_dev,
+                size_t workspace_bytes, void *stream);
+
+/*
+ * Grouped fused decode-GEMM over MoE experts (BASELINE config 5): rows of X already sorted by
+ * expert and contiguous; expert e owns rows_per_expert_host[e] rows (0 = inactive, skipped).
+ * All experts share one shape/format.  Y rows are in the same order as X rows.
+ */
+int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts,
+                        const int32_t *rows_per_expert_host, const void *x_dev, uint32_t x_dtype,
+                        int64_t ldx, const void *x_scale_dev, void *y_dev, int64_t ldy,
+                        void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/*
+ * Uncompressed comparator: the same tcgen05 pipeline with TMA loads of raw W instead of decoder
+ * warps ("uncompressed cuBLAS-free dense GEMM", BASELINE.json north_star).  w_dev: row-major W
+ * in the operand dtype (bf16 / fp16 / int8 / e4m3; int4 is not supported here).
+ */
+size_t anslin_dense_workspace_bytes(uint32_t n_out, uint32_t k_in, int32_t m);
+int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32_t k_in,
+                      const void *w_scale_dev /* int8: fp16[n_out]; else NULL */, float w_scale,
+                      const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m,
+                      const void *x_scale_dev, void *y_dev, int64_t ldy, void *workspace_dev,
+                      size_t workspace_bytes, void *stream);
+
+/* Number of kernels the last device call on this thread enqueued (for bench.py's gpu_launches). */
+int anslin_last_launch_count(void);
+
+const char *anslin_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ANSLIN_H */

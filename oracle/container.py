@@ -74,7 +74,7 @@ def tile_order(fmt: int, tile_k: int):
     i = t*32 + lane.  The tile is cut along K into units of 32 operand bytes per row
     (16 bf16/fp16 weights, 32 fp8/int8 weights); unit u is decoded completely before unit u+1.
     Inside a unit there are 8 chunk rounds g; in round g lane l owns the 16-byte operand chunk
-    j = g*32 + l  ->  row j div 2, half j mod 2, and produces its spc symbols in steps
+    (row (g mod 4)*32 + l, half g div 4) and produces its spc symbols in steps
     t = (u*8 + g)*spc + e, e = 0..spc-1.
     """
     spc = SPC[fmt]
@@ -89,9 +89,8 @@ def tile_order(fmt: int, tile_k: int):
             for e in range(spc):
                 t = (u * 8 + g) * spc + e
                 for lane in range(LANES):
-                    j = g * 32 + lane
-                    rows[t * LANES + lane] = j // 2
-                    cols[t * LANES + lane] = u * 2 * spc + (j % 2) * spc + e
+                    rows[t * LANES + lane] = (g % 4) * 32 + lane
+                    cols[t * LANES + lane] = u * 2 * spc + (g // 4) * spc + e
     return rows, cols
 
 

@@ -1,0 +1,168 @@
+"""Thin ctypes binding of libanslin.so (include/anslin.h): argument marshalling only.
+
+Every step of the hot path runs inside the library's kernels; torch is used by CALLERS for device
+memory and streams.  There is no fallback: if the shared object is missing or a call fails, an
+exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libanslin.so")
+
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ = 0, 1, 2, 3
+DT_F32, DT_F16, DT_BF16, DT_I8, DT_FP8_E4M3 = 0, 1, 2, 3, 4
+FLAG_STATE_PAYLOAD = 1
+X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_INT4_AWQ: DT_F16}
+
+EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_close", "anslin_describe",
+           "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm", "anslin_gemm_grouped",
+           "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_last_launch_count", "anslin_status_string"]
+
+
+class AnslinError(RuntimeError):
+    pass
+
+
+class Desc(ctypes.Structure):
+    _fields_ = [("format", ctypes.c_uint32), ("n_out", ctypes.c_uint32), ("k_in", ctypes.c_uint32),
+                ("tile_k", ctypes.c_uint32), ("group_size", ctypes.c_uint32), ("flags", ctypes.c_uint32),
+                ("w_scale", ctypes.c_float), ("reserved", ctypes.c_uint32)]
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_uint64) for n in ("n_weights", "payload_bits", "state_bits", "pad_bits", "offset_table_bits",
+                                               "freq_table_bits", "raw_bits", "side_bits", "total_bytes")] + \
+               [(n, ctypes.c_double) for n in ("entropy_bits_per_symbol", "xent_bits_per_symbol",
+                                               "raw_entropy_bits_per_symbol", "bits_per_weight")]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise AnslinError("libanslin.so is not built (run `python -m paper_2606_15789_b200.build`); there is no fallback")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, sz, i32, u32, i64 = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_uint32, ctypes.c_int64
+        L.anslin_encode_bound.argtypes = [ctypes.POINTER(Desc)]; L.anslin_encode_bound.restype = sz
+        L.anslin_encode_host.argtypes = [ctypes.POINTER(Desc), vp, vp, vp, vp, sz, ctypes.POINTER(sz), ctypes.POINTER(Stats)]
+        L.anslin_open.argtypes = [vp, sz, vp, ctypes.POINTER(vp)]
+        L.anslin_close.argtypes = [vp]
+        L.anslin_describe.argtypes = [vp, ctypes.POINTER(Desc)]
+        L.anslin_decode.argtypes = [vp, vp, sz, vp]
+        L.anslin_gemm_workspace_bytes.argtypes = [vp, i32]; L.anslin_gemm_workspace_bytes.restype = sz
+        L.anslin_gemm.argtypes = [vp, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
+        L.anslin_gemm_grouped.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(i32), vp, u32, i64, vp, vp, i64, vp, sz, vp]
+        L.anslin_dense_workspace_bytes.argtypes = [u32, u32, i32]; L.anslin_dense_workspace_bytes.restype = sz
+        L.anslin_dense_gemm.argtypes = [u32, vp, u32, u32, vp, ctypes.c_float, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
+        L.anslin_last_launch_count.restype = ctypes.c_int
+        L.anslin_status_string.argtypes = [ctypes.c_int]; L.anslin_status_string.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise AnslinError("%s failed: %s (status %d)" % (what, lib().anslin_status_string(rc).decode(), rc))
+
+
+def _hp(a):
+    return None if a is None else ctypes.c_void_p(a.ctypes.data)
+
+
+def anslin_encode_host(fmt: int, w: np.ndarray, n_out: int, k_in: int, tile_k: int = 0, flags: int = 0,
+                       scales: np.ndarray | None = None, zeros: np.ndarray | None = None, group_size: int = 0,
+                       w_scale: float = 1.0):
+    """Returns (container as np.uint8 array, stats dict)."""
+    d = Desc(fmt, n_out, k_in, tile_k, group_size, flags, w_scale, 0)
+    cap = lib().anslin_encode_bound(ctypes.byref(d))
+    if cap == 0:
+        raise AnslinError("anslin_encode_bound: unsupported shape or format")
+    w = np.ascontiguousarray(w)
+    scales = None if scales is None else np.ascontiguousarray(scales, dtype=np.float16)
+    zeros = None if zeros is None else np.ascontiguousarray(zeros, dtype=np.float16)
+    out = np.empty(cap, dtype=np.uint8)
+    n = ctypes.c_size_t(0)
+    st = Stats()
+    _check(lib().anslin_encode_host(ctypes.byref(d), _hp(w), _hp(scales), _hp(zeros), _hp(out), cap, ctypes.byref(n),
+                                    ctypes.byref(st)), "anslin_encode_host")
+    return out[:n.value].copy(), st.as_dict()
+
+
+class Weight:
+    """Host handle (anslin_weight*) bound to a device copy of the container."""
+
+    def __init__(self, container_host: np.ndarray, container_dev_ptr: int | None):
+        self._h = ctypes.c_void_p()
+        c = np.ascontiguousarray(container_host, dtype=np.uint8)
+        _check(lib().anslin_open(_hp(c), c.size, ctypes.c_void_p(container_dev_ptr or 0), ctypes.byref(self._h)), "anslin_open")
+        d = Desc()
+        _check(lib().anslin_describe(self._h, ctypes.byref(d)), "anslin_describe")
+        self.desc = d
+        self.nbytes = c.size
+
+    @property
+    def handle(self):
+        return self._h
+
+    def close(self):
+        if self._h:
+            lib().anslin_close(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def anslin_decode(w: Weight, out_ptr: int, capacity: int, stream: int = 0):
+    _check(lib().anslin_decode(w.handle, ctypes.c_void_p(out_ptr), capacity, ctypes.c_void_p(stream)), "anslin_decode")
+
+
+def anslin_gemm_workspace_bytes(w: Weight, m: int) -> int:
+    return int(lib().anslin_gemm_workspace_bytes(w.handle, m))
+
+
+def anslin_gemm(w: Weight, x_ptr: int, x_dtype: int, ldx: int, m: int, x_scale_ptr: int | None, y_ptr: int, ldy: int,
+                ws_ptr: int, ws_bytes: int, stream: int = 0):
+    _check(lib().anslin_gemm(w.handle, ctypes.c_void_p(x_ptr), x_dtype, ldx, m, ctypes.c_void_p(x_scale_ptr or 0),
+                             ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.c_void_p(stream)), "anslin_gemm")
+
+
+def anslin_gemm_grouped(experts, rows_per_expert, x_ptr: int, x_dtype: int, ldx: int, x_scale_ptr: int | None, y_ptr: int,
+                        ldy: int, ws_ptr: int, ws_bytes: int, stream: int = 0):
+    n = len(experts)
+    arr = (ctypes.c_void_p * n)(*[e.handle for e in experts])
+    rows = (ctypes.c_int32 * n)(*[int(r) for r in rows_per_expert])
+    _check(lib().anslin_gemm_grouped(arr, n, rows, ctypes.c_void_p(x_ptr), x_dtype, ldx, ctypes.c_void_p(x_scale_ptr or 0),
+                                     ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.c_void_p(stream)),
+           "anslin_gemm_grouped")
+
+
+def anslin_dense_workspace_bytes(n_out: int, k_in: int, m: int) -> int:
+    return int(lib().anslin_dense_workspace_bytes(n_out, k_in, m))
+
+
+def anslin_dense_gemm(fmt: int, w_ptr: int, n_out: int, k_in: int, w_scale_ptr: int | None, w_scale: float, x_ptr: int,
+                      x_dtype: int, ldx: int, m: int, x_scale_ptr: int | None, y_ptr: int, ldy: int, ws_ptr: int, ws_bytes: int,
+                      stream: int = 0):
+    _check(lib().anslin_dense_gemm(fmt, ctypes.c_void_p(w_ptr), n_out, k_in, ctypes.c_void_p(w_scale_ptr or 0), w_scale,
+                                   ctypes.c_void_p(x_ptr), x_dtype, ldx, m, ctypes.c_void_p(x_scale_ptr or 0),
+                                   ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.c_void_p(stream)),
+           "anslin_dense_gemm")
+
+
+def anslin_last_launch_count() -> int:
+    return int(lib().anslin_last_launch_count())

@@ -1,0 +1,58 @@
+// Internal definitions shared by the product's host encoder and device kernels (NOT by oracle/).
+// Container byte layout: DESIGN.md §"Container".
+#pragma once
+#include <stdint.h>
+#include <stddef.h>
+#include "../../include/anslin.h"
+
+#ifdef __CUDACC__
+#define ANSLIN_HD __host__ __device__
+#else
+#define ANSLIN_HD
+#endif
+
+namespace anslin {
+
+constexpr uint32_t kMagic = 0x4C534E41u;  // "ANSL"
+constexpr uint32_t kVersion = 1;
+constexpr int kTileN = 128;      // weight rows per tile = tcgen05 MMA M
+constexpr int kLanes = 32;       // interleaved rANS streams per tile (P:l.192)
+constexpr int kProbBits = 12;    // b (P:l.442)
+constexpr int kWordBits = 16;    // w
+constexpr int kStateLoLog2 = 16; // L = 2^16
+constexpr uint32_t kL = 1u << kStateLoLog2;
+constexpr uint32_t kM = 1u << kProbBits;
+constexpr int kHeaderBytes = 128;
+constexpr int kUnitBytes = 4096; // one operand unit = 128 rows x 32 B (one tcgen05.mma K step)
+
+struct Header {  // 128 bytes, little endian
+  uint32_t magic, version, format, n_out, k_in, tile_n, tile_k, streams, prob_bits, word_bits,
+      state_lo_log2, group_size, flags, n_tiles;
+  float w_scale;
+  uint32_t reserved0;
+  uint64_t off_freq, off_offsets, off_records, off_raw, off_scales, off_zeros, total_bytes, reserved1;
+};
+static_assert(sizeof(Header) == kHeaderBytes, "header must be 128 bytes");
+
+// symbols per 16-byte operand chunk
+ANSLIN_HD constexpr int spc_of(uint32_t fmt) {
+  return fmt == ANSLIN_FMT_BF16 ? 8 : fmt == ANSLIN_FMT_INT4_AWQ ? 4 : 16;
+}
+ANSLIN_HD constexpr int weights_per_symbol(uint32_t fmt) { return fmt == ANSLIN_FMT_INT4_AWQ ? 2 : 1; }
+// weights along K covered by one operand unit (32 bytes of bf16/fp16 = 16, of fp8/int8 = 32)
+ANSLIN_HD constexpr int unit_k_of(uint32_t fmt) {
+  return (fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT4_AWQ) ? 16 : 32;
+}
+constexpr uint32_t default_tile_k(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 ? 64 : 256; }
+// bytes per stored weight element of row-major W (int4: half a byte -> handled by callers)
+ANSLIN_HD constexpr size_t raw_tile_bytes(uint32_t tile_k, uint32_t flags) {
+  return size_t(kTileN) * tile_k - ((flags & ANSLIN_FLAG_STATE_PAYLOAD) ? 64 : 0);
+}
+inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
+
+}  // namespace anslin
+
+struct anslin_weight {
+  anslin::Header h;
+  const uint8_t *dev;  // device copy of the whole container (may be null)
+};

@@ -1,0 +1,235 @@
+// Warp-cooperative rANS tile decoder (Alg V.2, P:l.260-287), sm_100a.
+//
+// One warp decodes one tile: lane l owns stream l (P:l.192 "each warp lane maintains its own rANS
+// state").  Per step and lane:  slot = x & 4095;  e = T[slot] (shared-memory table, P:l.271);
+// x = f*(x>>12) + bias;  if x < 2^16: x = x<<16 | next word.  The words of a tile are interleaved
+// in decoder read order, so the renormalising lanes of a step read CONSECUTIVE 16-bit words
+// (P:l.256 "renormalization loads are naturally coalesced"): ballot + popc prefix picks the word.
+// The compressed words are streamed HBM -> shared memory through a per-warp 1 KiB ring with
+// 16-byte cp.async (32 lanes x 16 B = 512 B per fill), two fills in flight.
+//
+// Table entry (4 B, Eq.3's "2^b x 4 B", P:l.440):  sym[7:0] | f[19:8] | bias[31:20].
+#pragma once
+#include <cuda_fp16.h>
+#include <stdint.h>
+#include "anslin_internal.h"
+
+namespace anslin {
+
+constexpr int kRingBytes = 1024;      // per decoder warp
+constexpr int kRingChunkWords = 256;  // 512 B per fill
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t lanemask_lt() {
+  uint32_t m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds16(uint32_t a) {
+  uint16_t v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ uint4 ldg128_stream(const void *p) {
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+
+// Expand the 256 x u16 frequency table of the container into the 4096-entry slot table in shared
+// memory (Alg V.1 l.6 "Copy global decode table T into shared memory", P:l.212).  All threads of
+// the CTA must call; `cum` is 257 u32 of scratch.  Ends with __syncthreads().
+__device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, const uint16_t *freq_g) {
+  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
+  if (warp == 0) {  // exclusive prefix sum of 256 frequencies: 8 per lane + warp scan
+    uint32_t f[8], s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { f[i] = freq_g[lane * 8 + i]; s += f[i]; }
+    uint32_t inc = s;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
+      if (lane >= d) inc += o;
+    }
+    uint32_t run = inc - s;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { cum[lane * 8 + i] = run; run += f[i]; }
+    if (lane == 31) cum[256] = run;
+  }
+  __syncthreads();
+  for (int s = warp; s < 256; s += nwarp) {
+    const uint32_t c0 = cum[s], f = cum[s + 1] - c0;
+    for (uint32_t k = lane; k < f; k += 32) tab[c0 + k] = uint32_t(s) | (f << 8) | (k << 20);
+  }
+  __syncthreads();
+}
+
+// Per-warp stream state over one tile record.
+struct WarpStream {
+  uint32_t x;        // this lane's rANS state
+  uint32_t pos;      // words consumed so far (warp uniform)
+  uint32_t ready;    // words landed in the ring (warp uniform)
+  uint32_t issued;   // ring fills issued (warp uniform)
+  uint32_t limit;    // readable bytes from words_g (clamp for the over-read at the container end)
+  uint32_t ring;     // shared-space address of this warp's ring
+  const uint8_t *words_g;
+};
+
+__device__ __forceinline__ void stream_fill(WarpStream &s, int lane) {
+  const uint32_t off = s.issued * 512u + uint32_t(lane) * 16u;
+  cp_async16(s.ring + ((s.issued & 1u) * 512u) + uint32_t(lane) * 16u, s.words_g + off, off + 16u <= s.limit ? 16u : 0u);
+  cp_async_commit();
+  ++s.issued;
+}
+
+// rec = start of the tile record in HBM (16-byte aligned); end = one past the last readable byte.
+__device__ __forceinline__ void stream_open(WarpStream &s, const uint8_t *rec, const uint8_t *end, uint32_t ring, int lane) {
+  cp_async_wait_all();  // fills of the previous tile may still be in flight into this ring
+  __syncwarp();
+  s.x = reinterpret_cast<const uint32_t *>(rec)[lane];
+  s.words_g = rec + 4 * kLanes;
+  const size_t room = size_t(end - s.words_g);
+  s.limit = room > 0xFFFFFFF0ull ? 0xFFFFFFF0u : uint32_t(room);
+  s.pos = 0; s.ready = 0; s.issued = 0; s.ring = ring;
+  stream_fill(s, lane);
+  stream_fill(s, lane);
+}
+
+// One decode step of Alg V.2 for all 32 lanes; returns the table entry (symbol in bits 7:0).
+__device__ __forceinline__ uint32_t decode_step(WarpStream &s, uint32_t tab_s, int lane, uint32_t lt) {
+  if (s.pos + 32u > s.ready) {  // the 32-word window of this step must be resident
+    cp_async_wait_all();
+    __syncwarp();
+    s.ready += kRingChunkWords;
+  }
+  const uint32_t e = lds32(tab_s + ((s.x & (kM - 1)) << 2));
+  uint32_t x = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
+  const bool need = x < kL;
+  const uint32_t mask = __ballot_sync(0xffffffffu, need);
+  if (need) {
+    const uint32_t idx = s.pos + __popc(mask & lt);
+    x = (x << 16) | lds16(s.ring + ((idx << 1) & (kRingBytes - 1)));
+  }
+  s.x = x;
+  s.pos += __popc(mask);
+  if (s.pos >= (s.issued - 1u) * kRingChunkWords) {  // the older ring half is dead: refill it
+    __syncwarp();
+    stream_fill(s, lane);
+  }
+  return e;
+}
+
+// bf16: merge 4 exponent bytes (E) with 4 raw bytes (R = mantissa<<1 | sign) into 4 bf16 values.
+__device__ __forceinline__ uint2 bf16_merge4(uint32_t E, uint32_t R) {
+  const uint32_t p0 = __byte_perm(R, E, 0x5140), p1 = __byte_perm(R, E, 0x7362);
+  uint2 o;
+  o.x = ((p0 >> 1) & 0x7FFF7FFFu) | ((p0 << 15) & 0x80008000u);
+  o.y = ((p1 >> 1) & 0x7FFF7FFFu) | ((p1 << 15) & 0x80008000u);
+  return o;
+}
+
+// int4 (AWQ-style): one packed byte (low nibble = even k) -> two fp16 weights (q - z) * s.
+// 0x6400 | q is the fp16 number 1024 + q, so (1024+q) - (1024+z) is exact and the product rounds once.
+__device__ __forceinline__ uint32_t awq_dequant2(uint32_t byte, __half2 zoff, __half2 sc) {
+  const uint32_t v = (byte & 0x0Fu) | ((byte & 0xF0u) << 12) | 0x64006400u;
+  __half2 h = *reinterpret_cast<const __half2 *>(&v);
+  h = __hmul2(__hsub2(h, zoff), sc);
+  return *reinterpret_cast<const uint32_t *>(&h);
+}
+
+// Raw-plane (bf16 sign+mantissa) reader: 16 steps of one lane = one 16-byte vector.
+template <bool kPayload>
+struct RawReader {
+  const uint8_t *tile_raw;
+  int V;  // vectors per tile
+  __device__ __forceinline__ uint4 load(int v, int lane) const {
+    if (!kPayload || v < V - 1) return ldg128_stream(tile_raw + size_t(v) * 512 + lane * 16);
+    // last vector with the state-payload flag: 7 sub-rows of 32 x 2 bytes; bytes 14,15 come from the end state
+    uint32_t h[7];
+#pragma unroll
+    for (int i = 0; i < 7; ++i)
+      h[i] = reinterpret_cast<const uint16_t *>(tile_raw + size_t(v) * 512)[i * 32 + lane];
+    uint4 r;
+    r.x = h[0] | (h[1] << 16); r.y = h[2] | (h[3] << 16); r.z = h[4] | (h[5] << 16); r.w = h[6];
+    return r;
+  }
+};
+
+// Decode one operand unit (128 rows x 32 operand bytes = 256 chunks of 16 B) of a tile.
+//   FMT: container format.  Emit: functor with
+//     void chunk(int g, int lane, uint4 v)   operand-format 16-byte chunk of round g (all formats), or
+//     void packed(int g, int lane, uint32_t b) for int4 when Emit::kOperand == false (4 packed bytes).
+//   u: unit index inside the tile (selects the raw vectors / scale group).
+template <uint32_t FMT, bool kPayload, class Emit>
+__device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab_s, int lane, uint32_t lt, int u,
+                                            const RawReader<kPayload> &raw, uint4 &raw_next,
+                                            const uint32_t *sz_row /* int4: &sz[group][n0] */, Emit &emit) {
+  constexpr int SPC = spc_of(FMT);
+  if constexpr (FMT == ANSLIN_FMT_BF16) {
+#pragma unroll 1
+    for (int g2 = 0; g2 < 4; ++g2) {  // two rounds share one 16-byte raw vector
+      const int v = u * 4 + g2;
+      uint4 rv = raw_next;
+      if (v + 1 < raw.V) raw_next = raw.load(v + 1, lane);
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        uint32_t E0 = 0, E1 = 0;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) E0 = __byte_perm(E0, decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
+#pragma unroll
+        for (int e = 0; e < 4; ++e) E1 = __byte_perm(E1, decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
+        if (kPayload && v == raw.V - 1 && h == 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
+          const uint32_t p = s.x - kL;
+          rv.w = (rv.w & 0xFFFFu) | (p << 16);
+        }
+        const uint2 a = bf16_merge4(E0, h ? rv.z : rv.x), b = bf16_merge4(E1, h ? rv.w : rv.y);
+        emit.chunk(g2 * 2 + h, lane, make_uint4(a.x, a.y, b.x, b.y));
+      }
+    }
+  } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
+#pragma unroll 1
+    for (int g = 0; g < 8; ++g) {
+      uint32_t B = 0;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) B = __byte_perm(B, decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
+      if constexpr (Emit::kOperand) {
+        const uint32_t szv = __ldg(sz_row + (g & 3) * 32 + lane);
+        const __half2 sz = *reinterpret_cast<const __half2 *>(&szv);
+        const __half2 sc = __half2half2(__low2half(sz));
+        const __half2 zoff = __hadd2(__half2half2(__high2half(sz)), __float2half2_rn(1024.f));
+        emit.chunk(g, lane, make_uint4(awq_dequant2(B & 0xFF, zoff, sc), awq_dequant2((B >> 8) & 0xFF, zoff, sc),
+                                       awq_dequant2((B >> 16) & 0xFF, zoff, sc), awq_dequant2(B >> 24, zoff, sc)));
+      } else {
+        emit.packed(g, lane, B);
+      }
+    }
+  } else {  // fp8 / int8: the byte is the operand
+#pragma unroll 1
+    for (int g = 0; g < 8; ++g) {
+      uint32_t q[4] = {0, 0, 0, 0};
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) q[j] = __byte_perm(q[j], decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
+      emit.chunk(g, lane, make_uint4(q[0], q[1], q[2], q[3]));
+    }
+  }
+  (void)SPC;
+}
+
+}  // namespace anslin

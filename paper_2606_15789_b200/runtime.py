@@ -1,0 +1,94 @@
+"""Device-memory plumbing around the C ABI: torch owns HBM buffers and streams, nothing else.
+
+No arithmetic of the method happens here; every call forwards to libanslin through binding.py.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import binding as B
+
+_TORCH_X = {B.FMT_BF16: torch.bfloat16, B.FMT_INT4_AWQ: torch.float16, B.FMT_INT8: torch.int8,
+            B.FMT_FP8_E4M3: torch.uint8}
+
+
+def _stream() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def x_to_device(fmt: int, x: np.ndarray) -> torch.Tensor:
+    """numpy activations in the format's X dtype (bf16 as uint16 bits, fp16, int8, e4m3 bytes) -> cuda tensor."""
+    t = torch.from_numpy(np.ascontiguousarray(x))
+    if fmt == B.FMT_BF16:
+        t = t.view(torch.int16).view(torch.bfloat16)
+    return t.cuda()
+
+
+class DeviceWeight:
+    """A compressed weight matrix resident in HBM + its anslin_weight handle."""
+
+    def __init__(self, container: np.ndarray, device: str = "cuda"):
+        if not torch.cuda.is_available():
+            raise B.AnslinError("no CUDA device: anslin has no CPU fallback")
+        self.container_host = np.ascontiguousarray(container, dtype=np.uint8)
+        self.container_dev = torch.from_numpy(self.container_host).to(device)
+        self.weight = B.Weight(self.container_host, self.container_dev.data_ptr())
+        d = self.weight.desc
+        self.fmt, self.n_out, self.k_in = d.format, d.n_out, d.k_in
+        self._ws = None
+
+    def close(self):
+        self.weight.close()
+
+    def decode(self) -> torch.Tensor:
+        """anslin_decode -> row-major W in its original dtype/packing (bf16 as int16 bit patterns)."""
+        if self.fmt == B.FMT_BF16:
+            out = torch.empty((self.n_out, self.k_in), dtype=torch.int16, device=self.container_dev.device)
+        elif self.fmt == B.FMT_INT4_AWQ:
+            out = torch.empty((self.n_out, self.k_in // 2), dtype=torch.uint8, device=self.container_dev.device)
+        else:
+            out = torch.empty((self.n_out, self.k_in), dtype=torch.uint8, device=self.container_dev.device)
+        B.anslin_decode(self.weight, out.data_ptr(), out.numel() * out.element_size(), _stream())
+        return out
+
+    def workspace(self, m: int) -> torch.Tensor:
+        need = B.anslin_gemm_workspace_bytes(self.weight, m)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = torch.empty(need, dtype=torch.uint8, device=self.container_dev.device)
+        return self._ws
+
+    def gemm(self, x: torch.Tensor, x_scale: torch.Tensor | None = None, y: torch.Tensor | None = None) -> torch.Tensor:
+        """anslin_gemm: Y[m x n_out] f32 = X . W^T with W decoded on the fly."""
+        m = x.shape[0]
+        if y is None:
+            y = torch.empty((m, self.n_out), dtype=torch.float32, device=x.device)
+        ws = self.workspace(m)
+        B.anslin_gemm(self.weight, x.data_ptr(), B.X_DTYPE[self.fmt], x.stride(0), m,
+                      None if x_scale is None else x_scale.data_ptr(), y.data_ptr(), y.stride(0), ws.data_ptr(), ws.numel(), _stream())
+        return y
+
+
+def gemm_grouped(experts, rows_per_expert, x: torch.Tensor, x_scale: torch.Tensor | None, y: torch.Tensor | None = None):
+    m = x.shape[0]
+    if y is None:
+        y = torch.empty((m, experts[0].n_out), dtype=torch.float32, device=x.device)
+    ws = experts[0].workspace(int(max(max(rows_per_expert), 1)))
+    B.anslin_gemm_grouped([e.weight for e in experts], rows_per_expert, x.data_ptr(), B.X_DTYPE[experts[0].fmt], x.stride(0),
+                          None if x_scale is None else x_scale.data_ptr(), y.data_ptr(), y.stride(0), ws.data_ptr(), ws.numel(), _stream())
+    return y
+
+
+def dense_gemm(fmt: int, w: torch.Tensor, x: torch.Tensor, w_scale_vec: torch.Tensor | None = None, w_scale: float = 1.0,
+               x_scale: torch.Tensor | None = None, y: torch.Tensor | None = None, ws: torch.Tensor | None = None):
+    """Uncompressed comparator (anslin_dense_gemm): w is row-major W in the operand dtype."""
+    n_out, k_in = w.shape
+    m = x.shape[0]
+    if y is None:
+        y = torch.empty((m, n_out), dtype=torch.float32, device=x.device)
+    if ws is None:
+        ws = torch.empty(B.anslin_dense_workspace_bytes(n_out, k_in, m), dtype=torch.uint8, device=x.device)
+    B.anslin_dense_gemm(fmt, w.data_ptr(), n_out, k_in, None if w_scale_vec is None else w_scale_vec.data_ptr(), w_scale,
+                        x.data_ptr(), B.X_DTYPE[fmt], x.stride(0), m, None if x_scale is None else x_scale.data_ptr(),
+                        y.data_ptr(), y.stride(0), ws.data_ptr(), ws.numel(), _stream())
+    return y

@@ -1,0 +1,205 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element.
+
+Bars (BASELINE.json north_star): decoded weights bit-exact; GEMM max|d| <= 1e-2 * sum_k|x*w| per
+element and relative Frobenius error <= 1e-3 (fp32 accumulate vs float64 oracle).
+"""
+import numpy as np
+import pytest
+
+from oracle import container as oc, gemm as og
+from paper_2606_15789_b200 import binding as B
+from paper_2606_15789_b200 import build as libbuild
+from paper_2606_15789_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    libbuild.build()
+
+
+def _rt():
+    from paper_2606_15789_b200 import runtime
+    return runtime
+
+
+def check_gemm(y_gpu, y_ref, a_ref):
+    y = y_gpu.astype(np.float64)
+    assert np.all(np.isfinite(y))
+    err = np.abs(y - y_ref)
+    assert np.all(err <= 1e-2 * a_ref + 1e-30), "per-element bound: worst ratio %g" % float(np.max(err / (a_ref + 1e-30)))
+    fro = np.linalg.norm(y - y_ref) / max(np.linalg.norm(y_ref), 1e-30)
+    assert fro <= 1e-3, "relative Frobenius error %g" % fro
+
+
+# ------------------------------------------------------------------ decode (a4-a7, a11)
+def _decode_cases():
+    wf = inputs.weights_f32(384, 640, seed=41, jitter=True)
+    yield "bf16-t64", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 640, dict(tile_k=64)
+    yield "bf16-t64-payload", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 640, dict(tile_k=64, flags=1)
+    yield "bf16-t128-payload", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 640, dict(tile_k=128, flags=1)
+    wf2 = inputs.weights_f32(256, 768, seed=42, jitter=True)
+    q8, s8 = inputs.quant_sq8_weights(wf2)
+    yield "int8", B.FMT_INT8, q8, 768, dict(tile_k=256, scales=s8)
+    f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(256, 768, seed=43, std=0.015, outliers=False))
+    yield "fp8", B.FMT_FP8_E4M3, f8, 768, dict(tile_k=128, w_scale=sc)
+    p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(256, 768, seed=44, outliers=False), 128)
+    yield "int4", B.FMT_INT4_AWQ, p4, 768, dict(tile_k=256, scales=s4, zeros=z4, group_size=128)
+    yield "bf16-constant", B.FMT_BF16, np.full((128, 64), 0xBF80, dtype=np.uint16), 64, dict(tile_k=64)
+
+
+@pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_decode_cases()), ids=[c[0] for c in _decode_cases()])
+@pytest.mark.parametrize("encoder", ["library", "oracle"])
+def test_decode_bit_exact(name, fmt, w, k_in, kw, encoder):
+    """decode(encode(W)) == W bit for bit (P:l.26, l.46, l.486), for containers from both encoders."""
+    if encoder == "library":
+        buf, _ = B.anslin_encode_host(fmt, w, w.shape[0], k_in, **kw)
+    else:
+        buf, _ = oc.encode(fmt, w, k_in, **kw)
+    dw = _rt().DeviceWeight(buf)
+    out = dw.decode().cpu().numpy()
+    assert np.array_equal(out.view(np.uint8).reshape(w.shape[0], -1), np.ascontiguousarray(w).view(np.uint8).reshape(w.shape[0], -1))
+    dw.close()
+
+
+def test_decode_config1_full():
+    w, _ = inputs.config1()
+    for flags in (0, 1):
+        buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=64, flags=flags)
+        dw = _rt().DeviceWeight(buf)
+        assert np.array_equal(dw.decode().cpu().numpy().view(np.uint16), w)
+        dw.close()
+
+
+# ------------------------------------------------------------------ fused GEMM (a4-a10)
+@pytest.mark.parametrize("m", [1, 8, 16, 47, 75])
+@pytest.mark.parametrize("flags", [0, 1])
+def test_gemm_bf16(m, flags):
+    rt = _rt()
+    n, k = 640, 1024      # 5 stripes x 16 k-tiles: spans several CTAs and split-K segments
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=51, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=52))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=flags)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    y_ref, a_ref = og.gemm_bf16(x, w)
+    check_gemm(y, y_ref, a_ref)
+    dw.close()
+
+
+def test_gemm_config1_and_unit_vector():
+    """BASELINE config 1 (W 1024x1024 bf16, X 8x1024) and the e_k special case: Y = column k of W exactly."""
+    rt = _rt()
+    w, x = inputs.config1()
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=64, flags=1)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    check_gemm(y, *og.gemm_bf16(x, w))
+    wf = og.bf16_bits_to_f64(w)
+    for kk in (0, 7, 15, 16, 63, 64, 1000, 1023):
+        e = np.zeros((1, 1024), dtype=np.float32); e[0, kk] = 1.0
+        y = dw.gemm(rt.x_to_device(B.FMT_BF16, inputs.f32_to_bf16_bits(e))).cpu().numpy()
+        assert np.array_equal(y[0].astype(np.float64), wf[:, kk]), "column %d" % kk
+    dw.close()
+
+
+@pytest.mark.parametrize("m", [1, 32, 75])
+def test_gemm_int8(m):
+    rt = _rt()
+    import torch
+    n, k = 384, 1536
+    q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=61, jitter=True))
+    xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=62))
+    buf, _ = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=256, scales=s)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
+    y_ref, a_ref, acc = og.gemm_int8(xq, xs, q, s)
+    check_gemm(y, y_ref, a_ref)
+    # integer sums are exact: undoing the (float) scales must round to the oracle's int64 sums
+    back = np.rint(y.astype(np.float64) / (xs.astype(np.float64)[:, None] * s.astype(np.float64)[None, :]))
+    small = np.abs(acc) < (1 << 22)
+    assert np.array_equal(back[small], acc[small].astype(np.float64))
+    dw.close()
+
+
+@pytest.mark.parametrize("m", [1, 20, 64])
+def test_gemm_fp8(m):
+    rt = _rt()
+    import torch
+    n, k = 256, 1536
+    f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=71, std=0.015, outliers=False))
+    x8, xs = inputs.quant_fp8_acts(inputs.acts_f32(m, k, seed=72))
+    buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
+    check_gemm(y, *og.gemm_fp8(x8, xs, f8, sc))
+    dw.close()
+
+
+@pytest.mark.parametrize("m", [1, 16, 64])
+def test_gemm_int4(m):
+    rt = _rt()
+    n, k = 256, 1024
+    p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=81, outliers=False), 128)
+    x = inputs.acts_f32(m, k, seed=82).astype(np.float16)
+    buf, _ = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=256, scales=s4, zeros=z4, group_size=128)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
+    check_gemm(y, *og.gemm_int4(x, p4, s4, z4, 128))
+    dw.close()
+
+
+def test_gemm_grouped_fp8():
+    """BASELINE config 5 in miniature: 8 experts, top-2 routing, rows sorted by expert."""
+    rt = _rt()
+    import torch
+    n, k, E, tokens = 256, 768, 8, 20
+    rows, tok = inputs.route_top2(tokens, E, seed=91)
+    x8_tok, xs_tok = inputs.quant_fp8_acts(inputs.acts_f32(tokens, k, seed=92))
+    x8, xs = x8_tok[tok], xs_tok[tok]
+    experts, refs = [], []
+    for e in range(E):
+        f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=100 + e, std=0.015, outliers=False))
+        buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc)
+        experts.append(rt.DeviceWeight(buf))
+        refs.append((f8, sc))
+    y = rt.gemm_grouped(experts, rows, rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
+    r0 = 0
+    for e in range(E):
+        r1 = r0 + int(rows[e])
+        if r1 > r0:
+            check_gemm(y[r0:r1], *og.gemm_fp8(x8[r0:r1], xs[r0:r1], refs[e][0], refs[e][1]))
+        r0 = r1
+    for d in experts:
+        d.close()
+
+
+# ------------------------------------------------------------------ dense comparator
+@pytest.mark.parametrize("m", [1, 16, 75])
+def test_dense_gemm_bf16(m):
+    rt = _rt()
+    import torch
+    n, k = 640, 1024
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=51, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=52))
+    wd = torch.from_numpy(w.view(np.int16)).cuda()
+    y = rt.dense_gemm(B.FMT_BF16, wd, rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    check_gemm(y, *og.gemm_bf16(x, w))
+
+
+def test_dense_gemm_int8_fp8():
+    rt = _rt()
+    import torch
+    n, k, m = 256, 1536, 32
+    q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=61, jitter=True))
+    xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=62))
+    y = rt.dense_gemm(B.FMT_INT8, torch.from_numpy(q).cuda(), rt.x_to_device(B.FMT_INT8, xq),
+                      w_scale_vec=torch.from_numpy(s).cuda(), x_scale=torch.from_numpy(xs).cuda()).cpu().numpy()
+    y_ref, a_ref, _ = og.gemm_int8(xq, xs, q, s)
+    check_gemm(y, y_ref, a_ref)
+    f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=71, std=0.015, outliers=False))
+    x8, xs8 = inputs.quant_fp8_acts(inputs.acts_f32(m, k, seed=72))
+    y = rt.dense_gemm(B.FMT_FP8_E4M3, torch.from_numpy(f8).cuda(), rt.x_to_device(B.FMT_FP8_E4M3, x8), w_scale=sc,
+                      x_scale=torch.from_numpy(xs8).cuda()).cpu().numpy()
+    check_gemm(y, *og.gemm_fp8(x8, xs8, f8, sc))

@@ -1,0 +1,138 @@
+"""CPU tests of the product's host side through the C ABI: symbol export, anslin_encode_host vs the
+oracle (cross-decode both ways), size accounting, validation in anslin_open.  No GPU calls."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import container as oc
+from paper_2606_15789_b200 import binding as B
+from paper_2606_15789_b200 import build as libbuild
+from paper_2606_15789_b200 import inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    libbuild.build()
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "anslin.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(anslin_[a-z_0-9]+)\s*\(", hdr))
+    assert names == set(B.EXPORTS)
+    L = ctypes.CDLL(B.LIB_PATH)
+    for n in names:
+        assert hasattr(L, n), n
+    assert B.lib().anslin_status_string(4) == b"corrupt container"
+
+
+def _cases():
+    wf = inputs.weights_f32(256, 512, seed=31, jitter=True)
+    yield "bf16", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=64)
+    yield "bf16-payload", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=64, flags=1)
+    yield "bf16-tile128", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=128, flags=1)
+    q8, s8 = inputs.quant_sq8_weights(wf)
+    yield "int8", oc.FMT_INT8, q8, 512, dict(tile_k=256, scales=s8)
+    f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(128, 512, seed=32, std=0.015, outliers=False))
+    yield "fp8", oc.FMT_FP8_E4M3, f8, 512, dict(tile_k=128, w_scale=sc)
+    p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(128, 512, seed=33, outliers=False), 128)
+    yield "int4", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=256, scales=s4, zeros=z4, group_size=128)
+
+
+@pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_cases()), ids=[c[0] for c in _cases()])
+def test_cross_decode_and_stats(name, fmt, w, k_in, kw):
+    n_out = w.shape[0]
+    buf, st = B.anslin_encode_host(fmt, w, n_out, k_in, **kw)
+    # the oracle decodes the library's container bit-exactly (P:l.26 strict losslessness)
+    h, w2, side = oc.decode(buf)
+    assert np.array_equal(w2.view(np.uint8), np.ascontiguousarray(w).view(np.uint8))
+    if "scales" in kw:
+        assert np.array_equal(side["scales"], kw["scales"])
+    if "zeros" in kw:
+        assert np.array_equal(side["zeros"], kw["zeros"])
+    # the library accepts the oracle's container (header-only open; no device pointer)
+    obuf, ost = oc.encode(fmt, w, k_in, **kw)
+    hw = B.Weight(obuf, None)
+    assert (hw.desc.n_out, hw.desc.k_in, hw.desc.tile_k, hw.desc.flags) == (n_out, k_in, kw["tile_k"], kw.get("flags", 0))
+    hw.close()
+    B.Weight(buf, None).close()
+    # both encoders are legal rANS coders over (possibly different) legal tables: sizes agree closely
+    assert st["total_bytes"] == buf.size
+    assert abs(st["bits_per_weight"] - ost["bits_per_weight"]) < 0.01
+    assert st["entropy_bits_per_symbol"] == pytest.approx(ost["entropy_bits_per_symbol"], abs=1e-9)
+    assert st["xent_bits_per_symbol"] >= st["entropy_bits_per_symbol"]
+    wps = 2 if fmt == oc.FMT_INT4_AWQ else 1
+    assert st["bits_per_weight"] >= (st["entropy_bits_per_symbol"] + st["raw_entropy_bits_per_symbol"]) / wps
+    total_bits = (st["payload_bits"] + st["state_bits"] + st["pad_bits"] + st["raw_bits"] + st["side_bits"])
+    assert total_bits <= 8 * buf.size <= total_bits + st["offset_table_bits"] + st["freq_table_bits"] + 8 * (128 + 5 * 16)
+
+
+def test_config1_gap_through_the_abi():
+    """BASELINE target: bits/weight within 0.1 of the empirical entropy on config 1."""
+    w, _ = inputs.config1()
+    _, st = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=64, flags=B.FLAG_STATE_PAYLOAD)
+    gap = st["bits_per_weight"] - (st["entropy_bits_per_symbol"] + st["raw_entropy_bits_per_symbol"])
+    assert 0.0 <= gap <= 0.1
+
+
+def test_unsupported_and_invalid_arguments():
+    w = np.zeros((128, 64), dtype=np.uint16)
+    with pytest.raises(B.AnslinError):
+        B.anslin_encode_host(B.FMT_BF16, w, 100, 64)           # n_out not a multiple of 128
+    with pytest.raises(B.AnslinError):
+        B.anslin_encode_host(B.FMT_BF16, w, 128, 96)           # k_in not a multiple of tile_k
+    with pytest.raises(B.AnslinError):
+        B.anslin_encode_host(B.FMT_INT8, w, 128, 256, flags=1)  # payload flag is bf16-only
+    d = B.Desc(B.FMT_INT8, 128, 256, 0, 0, 0, 1.0, 0)
+    out = np.zeros(B.lib().anslin_encode_bound(ctypes.byref(d)), dtype=np.uint8)
+    n = ctypes.c_size_t(0)
+    rc = B.lib().anslin_encode_host(ctypes.byref(d), out.ctypes.data, None, None, out.ctypes.data, out.size, ctypes.byref(n), None)
+    assert rc == 1                                              # int8 without scales: INVALID_ARG
+    wq = np.zeros((128, 256), dtype=np.int8)
+    sc = np.ones(128, dtype=np.float16)
+    rc = B.lib().anslin_encode_host(ctypes.byref(d), wq.ctypes.data, sc.ctypes.data, None, out.ctypes.data, 64, ctypes.byref(n), None)
+    assert rc == 3 and n.value > 64                             # BUFFER_TOO_SMALL reports the needed size
+
+
+def test_open_rejects_corrupt_containers():
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(128, 128, seed=34))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 128, 128, tile_k=64)
+    h = oc.Header.unpack(buf)
+
+    def status(b):
+        out = ctypes.c_void_p()
+        rc = B.lib().anslin_open(b.ctypes.data, b.size, None, ctypes.byref(out))
+        if rc == 0:
+            B.lib().anslin_close(out)
+        return rc
+
+    assert status(buf) == 0
+    bad = buf.copy(); bad[0] ^= 1
+    assert status(bad) == 4                                     # magic
+    bad = buf.copy(); bad[h.off_freq] ^= 1
+    assert status(bad) == 4                                     # table no longer sums to 4096
+    bad = buf.copy(); bad[h.off_offsets + 4:h.off_offsets + 8] = 255
+    assert status(bad) == 4                                     # tile offset out of range
+    bad = buf.copy(); bad[12:16] = np.frombuffer(np.uint32(256).tobytes(), dtype=np.uint8)
+    assert status(bad) == 4                                     # n_out inconsistent with n_tiles
+    assert status(buf[:64].copy()) == 1                         # shorter than a header: INVALID_ARG
+
+
+def test_gemm_entry_points_fail_loudly_without_a_device():
+    """No CPU fallback: on a box without a GPU the device entry points return an error status."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(128, 128, seed=35))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 128, 128)
+    hw = B.Weight(buf, None)
+    with pytest.raises(B.AnslinError):
+        B.anslin_decode(hw, 0, 0)
+    with pytest.raises(B.AnslinError):
+        B.anslin_gemm(hw, 16, B.DT_BF16, 128, 1, None, 16, 128, 16, 1 << 20)
+    hw.close()
