@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py — fused rANS-decode GEMM throughput on BASELINE.json config 2 (Qwen-14B-shaped bf16 layer).
+
+One "step" = one pass of the hot path over the layer: anslin_gemm (table residency, compressed tile
+fetch, warp-cooperative rANS decode, operand store, X TMA, tcgen05 MMA, epilogue) for the seven
+projections q,k,v,o,gate,up,down at batch M (default 75, the paper's Qwen-14B max batch, P:l.378).
+Prints ONE JSON line (contract in the task statement).  `--impl reference` times the CPU oracle.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fused_ans_decode_gemm_tflops"
+UNIT = "TFLOP/s"
+WORKLOAD = "config2: Qwen-14B-shaped decoder layer, bf16, q/k/v/o/gate/up/down, synthetic N(0,0.02^2)+jitter+outliers"
+
+
+def layer_weights(seed0: int = 1):
+    from paper_2606_15789_b200 import inputs
+    out = []
+    for i, (name, n, k) in enumerate(inputs.QWEN14B_LAYER):
+        w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=seed0 + i, jitter=True))
+        out.append((name, n, k, w))
+    return out
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("bf16_tflops", 1590.0)), "measured"
+    return 6650.0, 1590.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm)}
+
+
+def cpu_oracle_leg(layer, containers, m: int, names=("q", "k", "down")):
+    """The oracle as it stands, timed on the host cores over a bounded sample of the workload:
+    full container decode (plain C rANS, single thread) + float64 GEMM of the named projections."""
+    from oracle import container as oc, gemm as og
+    from paper_2606_15789_b200 import inputs
+    try:
+        from threadpoolctl import threadpool_info
+        blas = max([i.get("num_threads", 1) for i in threadpool_info()] or [1])
+    except Exception:
+        blas = 1
+    flops, t0 = 0.0, time.perf_counter()
+    for (name, n, k, w), buf in zip(layer, containers):
+        if name not in names:
+            continue
+        _, w_dec, _ = oc.decode(buf)
+        x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=7))
+        og.gemm_bf16(x, w_dec)
+        flops += 2.0 * m * n * k
+    dt = time.perf_counter() - t0
+    return {"value": flops / dt / 1e12, "unit": UNIT, "cores": int(blas), "kind": "oracle", "seconds": round(dt, 2),
+            "sample": "projections %s of the layer at M=%d: oracle container decode (1 thread) + float64 GEMM (%d BLAS threads)"
+                      % ("/".join(names), m, blas)}
+
+
+def run_reference(args):
+    from paper_2606_15789_b200 import binding as B, build as libbuild
+    libbuild.build()
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    layer = [t for t in layer_weights() if t[0] in ("k",)]       # bounded sample: the k projection (1024x5120)
+    containers = [B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=1)[0] for (_, n, k, w) in layer]
+    for _ in range(args.warmup):
+        cpu_oracle_leg(layer, containers, args.m, names=("k",))
+    t0 = time.perf_counter()
+    vals = [cpu_oracle_leg(layer, containers, args.m, names=("k",)) for _ in range(args.steps)]
+    dt = time.perf_counter() - t0
+    flops = args.steps * 2.0 * args.m * 1024 * 5120
+    v = flops / dt / 1e12
+    cb = dict(vals[-1]); cb["value"] = v
+    cb["sample"] = "each step = oracle decode + float64 GEMM of the k projection (1024x5120) at M=%d" % args.m
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                      "config": {"workload": WORKLOAD, "batch_m": args.m}, "cpu_baseline": cb,
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="anslin")
+    ap.add_argument("--m", type=int, default=75)
+    ap.add_argument("--no-extras", action="store_true", help="skip per-M table, dense comparator, decode-only and CPU legs")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2606_15789_b200 import binding as B, build as libbuild, inputs, runtime as rt
+    libbuild.build()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: anslin has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    # ---- offline stage (untimed): synthesize, compress, upload
+    layer = layer_weights()
+    containers, stats = [], []
+    for (_, n, k, w) in layer:
+        buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=B.FLAG_STATE_PAYLOAD)
+        containers.append(buf); stats.append(st)
+    dws = [rt.DeviceWeight(c) for c in containers]
+    m = args.m
+    xs_host = [torch.from_numpy(inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=500 + i + 97 * rank)).view(np.int16)).pin_memory()
+               for i, (_, n, k, _) in enumerate(layer)]
+    xs = [t.cuda().view(torch.bfloat16) for t in xs_host]
+    ys = [torch.empty((m, n), dtype=torch.float32, device="cuda") for (_, n, k, _) in layer]
+    ys_host = [torch.empty((m, n), dtype=torch.float32).pin_memory() for (_, n, k, _) in layer]
+    flops_step = sum(2.0 * m * n * k for (_, n, k, _) in layer)
+    comp_bytes = sum(c.size for c in containers)
+    algo_bytes = [c.size + m * k * 2 + m * n * 4 for c, (_, n, k, _) in zip(containers, layer)]
+    n_weights = sum(n * k for (_, n, k, _) in layer)
+
+    def step(record=None):
+        launches = 0
+        for i, dw in enumerate(dws):
+            if record is not None:
+                record[i][0].record()
+            dw.gemm(xs[i], None, ys[i])
+            launches += B.anslin_last_launch_count()
+            if record is not None:
+                record[i][1].record()
+        return launches
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in dws] for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    e0.record()
+    for s in range(args.steps):
+        launches += step(evs[s])
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+    ms_step = ms / args.steps
+    value = world * flops_step / (ms_step * 1e-3) / 1e12
+    kern_ms = [[a.elapsed_time(b) for (a, b) in row] for row in evs]
+    kern_ms_mean = np.mean(np.array(kern_ms), axis=0)             # per projection
+    hbm_peak, tc_peak, peak_kind = peaks()
+    achieved = sum(algo_bytes) / (float(np.sum(kern_ms_mean)) * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get("fused_gemm_bytes_per_launch_mean")
+
+    # ---- e2e: the same step through the C ABI with HOST buffers (pinned X in, Y out) inside the timed region
+    def step_e2e():
+        for i, dw in enumerate(dws):
+            xd = xs[i]
+            xd.view(torch.int16).copy_(xs_host[i], non_blocking=True)
+            dw.gemm(xd, None, ys[i])
+            ys_host[i].copy_(ys[i], non_blocking=True)
+    for _ in range(3):
+        step_e2e()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step_e2e()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e = {"value": world * flops_step * args.steps / e2e_s / 1e12, "unit": UNIT,
+           "h2d_bytes_per_step": int(sum(m * k * 2 for (_, n, k, _) in layer)),
+           "d2h_bytes_per_step": int(sum(m * n * 4 for (_, n, k, _) in layer))}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+           "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+           "data": "synthetic",
+           "config": {"workload": WORKLOAD, "batch_m": m, "tile": "128x64", "streams": 32, "prob_bits": 12,
+                      "l2_policy": "inputs larger than L2: %.0f MB of compressed weights stream per step" % (comp_bytes / 1e6),
+                      "parallelism": "replicas, one batch per GPU" if world > 1 else "1 GPU"},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+           "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                        "traffic": traffic, "peak_kind": "of " + peak_kind,
+                        "kernel": "fused_gemm_kernel<bf16,payload> (7 launches/step; bytes = container + X + Y)"},
+           "compressed_gbs": world * comp_bytes / (ms_step * 1e-3) / 1e9,
+           "decoded_weights_gbs": world * n_weights * 2 / (ms_step * 1e-3) / 1e9,
+           "bits_per_weight": 8.0 * comp_bytes / n_weights,
+           "h_sym_bits_per_weight": float(np.sum([(s["entropy_bits_per_symbol"] + s["raw_entropy_bits_per_symbol"]) * s["n_weights"]
+                                                  for s in stats]) / n_weights),
+           "per_projection_us": {name: round(1e3 * float(t), 2) for (name, _, _, _), t in zip(layer, kern_ms_mean)}}
+
+    if rank == 0 and not args.no_extras:
+        # per-M table (BASELINE config 2: M in {1,16,47,75}), dense comparator, decode-only; then the CPU oracle leg
+        extra = {}
+        for mm in (1, 16, 47, 75):
+            xm = [x[:mm].contiguous() for x in xs]
+            ym = [torch.empty((mm, n), dtype=torch.float32, device="cuda") for (_, n, k, _) in layer]
+            for _ in range(3):
+                for i, dw in enumerate(dws):
+                    dw.gemm(xm[i], None, ym[i])
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); a.record()
+            for _ in range(5):
+                for i, dw in enumerate(dws):
+                    dw.gemm(xm[i], None, ym[i])
+            b.record(); torch.cuda.synchronize()
+            t = a.elapsed_time(b) / 5
+            fl = sum(2.0 * mm * n * k for (_, n, k, _) in layer)
+            extra["M=%d" % mm] = {"ms": round(t, 4), "tflops": round(fl / (t * 1e-3) / 1e12, 3),
+                                  "compressed_gbs": round(comp_bytes / (t * 1e-3) / 1e9, 1)}
+        out["per_m"] = extra
+        wd = [torch.from_numpy(w.view(np.int16)).cuda() for (_, _, _, w) in layer]
+        wsd = [torch.empty(B.anslin_dense_workspace_bytes(n, k, m), dtype=torch.uint8, device="cuda") for (_, n, k, _) in layer]
+        for _ in range(3):
+            for i in range(len(layer)):
+                rt.dense_gemm(B.FMT_BF16, wd[i], xs[i], y=ys[i], ws=wsd[i])
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); a.record()
+        for _ in range(5):
+            for i in range(len(layer)):
+                rt.dense_gemm(B.FMT_BF16, wd[i], xs[i], y=ys[i], ws=wsd[i])
+        b.record(); torch.cuda.synchronize()
+        t = a.elapsed_time(b) / 5
+        out["dense_uncompressed"] = {"ms": round(t, 4), "tflops": round(flops_step / (t * 1e-3) / 1e12, 3),
+                                     "hbm_gbs": round(n_weights * 2 / (t * 1e-3) / 1e9, 1)}
+        del wd
+        a.record()
+        for _ in range(3):
+            for dw in dws:
+                dw.decode()
+        b.record(); torch.cuda.synchronize()
+        t = a.elapsed_time(b) / 3
+        out["decode_only"] = {"ms": round(t, 4), "decoded_gbs": round(n_weights * 2 / (t * 1e-3) / 1e9, 1),
+                              "gsym_per_s": round(n_weights / (t * 1e-3) / 1e9, 1)}
+        out["cpu_baseline"] = cpu_oracle_leg(layer, containers, m)
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -6,7 +6,8 @@
 // in decoder read order, so the renormalising lanes of a step read CONSECUTIVE 16-bit words
 // (P:l.256 "renormalization loads are naturally coalesced"): ballot + popc prefix picks the word.
 // The compressed words are streamed HBM -> shared memory through a per-warp 1 KiB ring with
-// 16-byte cp.async (32 lanes x 16 B = 512 B per fill), two fills in flight.
+// 16-byte cp.async (16 lanes x 16 B = 256 B per fill, 768..1024 B of look-ahead); the ring
+// bookkeeping runs once per FOUR decode steps.
 //
 // Table entry (4 B, Eq.3's "2^b x 4 B", P:l.440):  sym[7:0] | f[19:8] | bias[31:20].
 #pragma once
@@ -16,19 +17,14 @@
 
 namespace anslin {
 
-constexpr int kRingBytes = 1024;      // per decoder warp
-constexpr int kRingChunkWords = 256;  // 512 B per fill
+constexpr uint32_t kRingBytes = 1024;  // per decoder warp; the ring must be 1 KiB aligned
+constexpr uint32_t kFillBytes = 256;
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ uint32_t lanemask_lt() {
   uint32_t m;
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
   return m;
-}
-__device__ __forceinline__ uint32_t lds32(uint32_t a) {
-  uint32_t v;
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
-  return v;
 }
 __device__ __forceinline__ uint32_t lds16(uint32_t a) {
   uint16_t v;
@@ -38,11 +34,23 @@ __device__ __forceinline__ uint32_t lds16(uint32_t a) {
 __device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src, uint32_t src_bytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+// 16-byte cp.async, executed only when `on` != 0; copies src_bytes (16 or 0 = zero fill) bytes.
+__device__ __forceinline__ void cp_async16_if(uint32_t on, uint32_t dst, const void *src, uint32_t src_bytes) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p cp.async.cg.shared.global [%1], [%2], 16, %3;\n\t}" ::"r"(on), "r"(dst),
+      "l"(src), "r"(src_bytes)
+      : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit_if(uint32_t on) {
+  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p cp.async.commit_group;\n\t}" ::"r"(on) : "memory");
+}
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
+__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  return v;
+}
 __device__ __forceinline__ uint4 ldg128_stream(const void *p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
@@ -81,20 +89,20 @@ __device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, c
 
 // Per-warp stream state over one tile record.
 struct WarpStream {
-  uint32_t x;        // this lane's rANS state
-  uint32_t pos;      // words consumed so far (warp uniform)
-  uint32_t ready;    // words landed in the ring (warp uniform)
-  uint32_t issued;   // ring fills issued (warp uniform)
-  uint32_t limit;    // readable bytes from words_g (clamp for the over-read at the container end)
-  uint32_t ring;     // shared-space address of this warp's ring
+  uint32_t x;       // this lane's rANS state
+  uint32_t posb;    // BYTES of words consumed so far (warp uniform)
+  uint32_t filled;  // bytes of words whose ring fill has been issued (warp uniform, multiple of 256)
+  uint32_t limit;   // readable bytes from words_g (clamp for the over-read at the container end)
+  uint32_t ring;    // shared-space address of this warp's 1 KiB-aligned ring
   const uint8_t *words_g;
 };
 
-__device__ __forceinline__ void stream_fill(WarpStream &s, int lane) {
-  const uint32_t off = s.issued * 512u + uint32_t(lane) * 16u;
-  cp_async16(s.ring + ((s.issued & 1u) * 512u) + uint32_t(lane) * 16u, s.words_g + off, off + 16u <= s.limit ? 16u : 0u);
-  cp_async_commit();
-  ++s.issued;
+// Issue the next 256-byte ring fill iff `on` (lanes 0..15 copy 16 B each).
+__device__ __forceinline__ void stream_fill_if(WarpStream &s, uint32_t on, int lane) {
+  const uint32_t off = s.filled + (uint32_t(lane) << 4);
+  cp_async16_if(on & uint32_t(lane < 16), s.ring | (off & (kRingBytes - 1)), s.words_g + off, off + 16u <= s.limit ? 16u : 0u);
+  cp_async_commit_if(on);
+  s.filled += on ? kFillBytes : 0u;
 }
 
 // rec = start of the tile record in HBM (16-byte aligned); end = one past the last readable byte.
@@ -105,33 +113,51 @@ __device__ __forceinline__ void stream_open(WarpStream &s, const uint8_t *rec, c
   s.words_g = rec + 4 * kLanes;
   const size_t room = size_t(end - s.words_g);
   s.limit = room > 0xFFFFFFF0ull ? 0xFFFFFFF0u : uint32_t(room);
-  s.pos = 0; s.ready = 0; s.issued = 0; s.ring = ring;
-  stream_fill(s, lane);
-  stream_fill(s, lane);
+  s.posb = 0; s.filled = 0; s.ring = ring;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) stream_fill_if(s, 1u, lane);
+}
+
+// Ring upkeep for the next FOUR decode steps (they consume at most 256 B): refill the dead quarter
+// behind the read position and make sure everything up to posb + 512 has landed.  Invariant:
+// 768 <= filled - posb <= 1024 after the call, at most ONE fill pending => landed >= posb + 512
+// >= the 256 + 62 bytes the four steps can touch.  A fill writes ring bytes
+// [filled, filled + 256) - 1024 < posb, i.e. only words already consumed.
+__device__ __forceinline__ void stream_upkeep4(WarpStream &s, int lane) {
+  stream_fill_if(s, uint32_t(s.filled - s.posb < 768u), lane);
+  cp_async_wait_1();
+  __syncwarp();
 }
 
 // One decode step of Alg V.2 for all 32 lanes; returns the table entry (symbol in bits 7:0).
-__device__ __forceinline__ uint32_t decode_step(WarpStream &s, uint32_t tab_s, int lane, uint32_t lt) {
-  if (s.pos + 32u > s.ready) {  // the 32-word window of this step must be resident
-    cp_async_wait_all();
-    __syncwarp();
-    s.ready += kRingChunkWords;
-  }
-  const uint32_t e = lds32(tab_s + ((s.x & (kM - 1)) << 2));
-  uint32_t x = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
-  const bool need = x < kL;
+__device__ __forceinline__ uint32_t decode_step(WarpStream &s, uint32_t tab_s, uint32_t lt) {
+  uint32_t ea;
+  asm("mad.lo.u32 %0, %1, 4, %2;" : "=r"(ea) : "r"(s.x & (kM - 1)), "r"(tab_s));
+  const uint32_t e = lds32(ea);
+  const uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
+  const bool need = xn < kL;
   const uint32_t mask = __ballot_sync(0xffffffffu, need);
-  if (need) {
-    const uint32_t idx = s.pos + __popc(mask & lt);
-    x = (x << 16) | lds16(s.ring + ((idx << 1) & (kRingBytes - 1)));
-  }
-  s.x = x;
-  s.pos += __popc(mask);
-  if (s.pos >= (s.issued - 1u) * kRingChunkWords) {  // the older ring half is dead: refill it
-    __syncwarp();
-    stream_fill(s, lane);
-  }
+  // every lane loads (the window is resident); only renormalising lanes use the word
+  const uint32_t w = lds16(s.ring | ((s.posb + 2u * __popc(mask & lt)) & (kRingBytes - 1)));
+  s.x = need ? __byte_perm(w, xn, 0x5410) : xn;  // (xn << 16) | w
+  s.posb += 2u * __popc(mask);
   return e;
+}
+
+// Insert the symbol byte of table entry e at byte position `pos` of acc.
+template <int pos>
+__device__ __forceinline__ uint32_t put_sym(uint32_t acc, uint32_t e) {
+  return __byte_perm(acc, e, (0x3210 & ~(0xF << (4 * pos))) | (4 << (4 * pos)));
+}
+// Four decode steps -> four symbol bytes (one ring upkeep).
+__device__ __forceinline__ uint32_t decode4(WarpStream &s, uint32_t tab, int lane, uint32_t lt) {
+  uint32_t q = 0;
+  stream_upkeep4(s, lane);
+  q = put_sym<0>(q, decode_step(s, tab, lt));
+  q = put_sym<1>(q, decode_step(s, tab, lt));
+  q = put_sym<2>(q, decode_step(s, tab, lt));
+  q = put_sym<3>(q, decode_step(s, tab, lt));
+  return q;
 }
 
 // bf16: merge 4 exponent bytes (E) with 4 raw bytes (R = mantissa<<1 | sign) into 4 bf16 values.
@@ -176,23 +202,19 @@ struct RawReader {
 //     void packed(int g, int lane, uint32_t b) for int4 when Emit::kOperand == false (4 packed bytes).
 //   u: unit index inside the tile (selects the raw vectors / scale group).
 template <uint32_t FMT, bool kPayload, class Emit>
-__device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab_s, int lane, uint32_t lt, int u,
-                                            const RawReader<kPayload> &raw, uint4 &raw_next,
+__device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab, int lane, uint32_t lt, int u,
+                                            const RawReader<kPayload> &raw, uint4 &raw_next, uint4 &raw_next2,
                                             const uint32_t *sz_row /* int4: &sz[group][n0] */, Emit &emit) {
-  constexpr int SPC = spc_of(FMT);
   if constexpr (FMT == ANSLIN_FMT_BF16) {
 #pragma unroll 1
-    for (int g2 = 0; g2 < 4; ++g2) {  // two rounds share one 16-byte raw vector
+    for (int g2 = 0; g2 < 4; ++g2) {  // two rounds share one 16-byte raw vector; vectors are fetched two ahead
       const int v = u * 4 + g2;
       uint4 rv = raw_next;
-      if (v + 1 < raw.V) raw_next = raw.load(v + 1, lane);
+      raw_next = raw_next2;
+      if (v + 2 < raw.V) raw_next2 = raw.load(v + 2, lane);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        uint32_t E0 = 0, E1 = 0;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) E0 = __byte_perm(E0, decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
-#pragma unroll
-        for (int e = 0; e < 4; ++e) E1 = __byte_perm(E1, decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
+        const uint32_t E0 = decode4(s, tab, lane, lt), E1 = decode4(s, tab, lane, lt);
         if (kPayload && v == raw.V - 1 && h == 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
           const uint32_t p = s.x - kL;
           rv.w = (rv.w & 0xFFFFu) | (p << 16);
@@ -204,9 +226,7 @@ __device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab_s, int l
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll 1
     for (int g = 0; g < 8; ++g) {
-      uint32_t B = 0;
-#pragma unroll
-      for (int e = 0; e < 4; ++e) B = __byte_perm(B, decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
+      const uint32_t B = decode4(s, tab, lane, lt);
       if constexpr (Emit::kOperand) {
         const uint32_t szv = __ldg(sz_row + (g & 3) * 32 + lane);
         const __half2 sz = *reinterpret_cast<const __half2 *>(&szv);
@@ -221,15 +241,11 @@ __device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab_s, int l
   } else {  // fp8 / int8: the byte is the operand
 #pragma unroll 1
     for (int g = 0; g < 8; ++g) {
-      uint32_t q[4] = {0, 0, 0, 0};
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-#pragma unroll
-        for (int e = 0; e < 4; ++e) q[j] = __byte_perm(q[j], decode_step(s, tab_s, lane, lt), 0x3210 & ~(0xF << (4 * e)) | (4 << (4 * e)));
-      emit.chunk(g, lane, make_uint4(q[0], q[1], q[2], q[3]));
+      const uint32_t q0 = decode4(s, tab, lane, lt), q1 = decode4(s, tab, lane, lt);
+      const uint32_t q2 = decode4(s, tab, lane, lt), q3 = decode4(s, tab, lane, lt);
+      emit.chunk(g, lane, make_uint4(q0, q1, q2, q3));
     }
   }
-  (void)SPC;
 }
 
 }  // namespace anslin

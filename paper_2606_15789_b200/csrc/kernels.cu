@@ -15,6 +15,7 @@
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
 #include <stdint.h>
+#include <stdio.h>
 #include <stdlib.h>
 
 #include "anslin_internal.h"
@@ -166,10 +167,10 @@ template <uint32_t FMT, bool PAYLOAD>
 __global__ void __launch_bounds__(kDecWarps * 32) decode_kernel(ContainerView cv, uint8_t *out) {
   __shared__ __align__(16) uint32_t tab[kM];
   __shared__ uint32_t cum[260];
-  __shared__ __align__(16) uint8_t rings[kDecWarps][kRingBytes];
+  __shared__ __align__(1024) uint8_t rings[kDecWarps][kRingBytes];
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t lt = lanemask_lt(), tab_s = smem_u32(tab), ring_s = smem_u32(rings[warp]);
+  const uint32_t lt = lanemask_lt(), ring_s = smem_u32(rings[warp]);
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
   const size_t row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.k_in) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.k_in) / 2 : size_t(cv.k_in);
   const size_t tile_row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.tile_k) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.tile_k) / 2 : size_t(cv.tile_k);
@@ -184,11 +185,11 @@ __global__ void __launch_bounds__(kDecWarps * 32) decode_kernel(ContainerView cv
     RawReader<PAYLOAD> raw;
     raw.tile_raw = cv.base + cv.off_raw + size_t(t) * rtb;
     raw.V = int(cv.units) * 4;
-    uint4 raw_next = make_uint4(0, 0, 0, 0);
-    if (FMT == ANSLIN_FMT_BF16) raw_next = raw.load(0, lane);
+    uint4 raw_next = make_uint4(0, 0, 0, 0), raw_next2 = raw_next;
+    if (FMT == ANSLIN_FMT_BF16) { raw_next = raw.load(0, lane); raw_next2 = raw.load(1, lane); }
     for (uint32_t u = 0; u < cv.units; ++u) {
       emit.u = int(u);
-      decode_unit<FMT, PAYLOAD>(s, tab_s, lane, lt, int(u), raw, raw_next, nullptr, emit);
+      decode_unit<FMT, PAYLOAD>(s, smem_u32(tab), lane, lt, int(u), raw, raw_next, raw_next2, nullptr, emit);
     }
   }
   cp_async_wait_all();
@@ -254,6 +255,109 @@ __device__ __forceinline__ uint32_t acc_add(uint32_t a, uint32_t b) {
   else return __float_as_uint(__uint_as_float(a) + __uint_as_float(b));
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// Epilogue (a10), shared by the fused and the dense kernel.  Warps 0..3: TMEM -> registers -> Y for
+// whole stripes, or -> split-K partial + deterministic fix-up (the LAST CTA to finish a stripe sums
+// all partials in CTA order, 16-byte loads, up to 8 contributors in flight per thread).
+// ------------------------------------------------------------------------------------------------
+struct EpiParams {
+  const float *x_scale;     // int8 / fp8: f32[m]
+  const __half *w_scale_h;  // int8: fp16[n_out]
+  float w_scale;            // fp8
+  float *y;
+  int64_t ldy;
+  uint32_t *partials, *counters;
+  uint32_t m, mpad;
+};
+
+__device__ __forceinline__ uint4 ldcg128(const uint32_t *p) {
+  uint4 r;
+  asm volatile("ld.global.cg.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+
+template <uint32_t FMT>
+__device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_base, uint32_t tfull_s, uint32_t tempty_s,
+                                             volatile uint32_t *flag, uint32_t t_begin, uint32_t t_end, uint32_t KT, uint32_t G,
+                                             uint32_t T, int warp, int lane) {
+  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
+  const uint32_t row = uint32_t(warp * 32 + lane);
+  uint32_t si = 0;
+  for (uint32_t t = t_begin; t < t_end; ++si) {
+    const uint32_t stripe = t / KT, ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
+    const bool whole = (ka == 0 && nt == KT);
+    const uint32_t n = stripe * kTileN + row;
+    float ws = 1.0f;
+    if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n]);
+    if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
+    mbar_wait(tfull_s + 8 * ab, (si >> 1) & 1u);
+    tc_fence_after();
+    const uint32_t pslot = blockIdx.x * 2u + (t == t_begin ? 0u : 1u);
+    uint32_t *part = p.partials + size_t(pslot) * p.mpad * kTileN;
+    for (uint32_t c0 = 0; c0 < p.mpad; c0 += 16) {
+      uint32_t v[16];
+      tmem_ld16(tmem_base + ((uint32_t(warp) * 32u) << 16) + ab * p.mpad + c0, v);
+#pragma unroll
+      for (int j = 0; j < 16; ++j) {
+        const uint32_t mm = c0 + j;
+        if (mm < p.m) {
+          if (whole) p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(v[j], kScaled ? p.x_scale[mm] : 1.0f, ws);
+          else part[size_t(mm) * kTileN + row] = v[j];
+        }
+      }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(tempty_s + 8 * ab);
+    if (!whole) {
+      const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
+      __threadfence();
+      named_bar_sync(1, kEpiWarps * 32);
+      if (threadIdx.x == 0) *flag = (atomicAdd(&p.counters[stripe], 1u) == c_last - c_first) ? 1u : 0u;
+      named_bar_sync(1, kEpiWarps * 32);
+      if (*flag) {
+        __threadfence();
+        // thread -> 4 consecutive output channels (one 16-byte load per contributor), warp -> batch rows mm = warp, warp+4, ..
+        const uint32_t r4 = uint32_t(lane) * 4u, n4 = stripe * kTileN + r4;
+        float ws4[4] = {ws, ws, ws, ws};
+        if (FMT == ANSLIN_FMT_INT8)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) ws4[j] = __half2float(p.w_scale_h[n4 + j]);
+        for (uint32_t mm = uint32_t(warp); mm < p.m; mm += kEpiWarps) {
+          uint32_t acc[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
+          for (uint32_t cb = c_first; cb <= c_last; cb += 8) {
+            uint4 v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const uint32_t c = cb + j;
+              v[j] = make_uint4(0, 0, 0, 0);
+              if (c <= c_last) {
+                const uint32_t ps = c * 2u + (cta_first_tile(c, G, T) / KT == stripe ? 0u : 1u);
+                v[j] = ldcg128(p.partials + (size_t(ps) * p.mpad + mm) * kTileN + r4);
+              }
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {  // fixed CTA order -> bit-reproducible sums
+              acc[0] = acc_add<FMT>(acc[0], v[j].x); acc[1] = acc_add<FMT>(acc[1], v[j].y);
+              acc[2] = acc_add<FMT>(acc[2], v[j].z); acc[3] = acc_add<FMT>(acc[3], v[j].w);
+            }
+          }
+          const float xs = kScaled ? p.x_scale[mm] : 1.0f;
+          float *yo = p.y + size_t(mm) * p.ldy + n4;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) yo[j] = finalize<FMT>(acc[j], xs, ws4[j]);
+        }
+        if (threadIdx.x == 0) p.counters[stripe] = 0;
+      }
+      named_bar_sync(1, kEpiWarps * 32);  // flag is reused by the next segment
+    }
+    t += nt;
+  }
+}
+
 template <uint32_t FMT, bool PAYLOAD>
 __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ CUtensorMap tmx, GemmParams p) {
   using TR = FmtTraits<FMT>;
@@ -262,22 +366,26 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   uint8_t *smem = smem_raw + (smem0 - smem_u32(smem_raw));
   // carve-up
   const uint32_t slots_s = smem0;
-  const uint32_t tab_off = p.U * p.slot_bytes;
+  const uint32_t ring_off = (p.U * p.slot_bytes + 1023u) & ~1023u;   // rings are 1 KiB aligned
+  const uint32_t tab_off = ring_off + p.D * kRingBytes;
   uint32_t *tab = reinterpret_cast<uint32_t *>(smem + tab_off);
   uint32_t *cum = reinterpret_cast<uint32_t *>(smem + tab_off + 16384);
-  const uint32_t ring_off = tab_off + 16384 + 1056;
-  const uint32_t bar_off = ring_off + p.D * kRingBytes;
+  const uint32_t bar_off = tab_off + 16384 + 1056;
   const uint32_t full_s = smem0 + bar_off, empty_s = full_s + 8 * kMaxSlots, tfull_s = empty_s + 8 * kMaxSlots,
                  tempty_s = tfull_s + 16, tmemptr_s = tempty_s + 16, flag_s = tmemptr_s + 8;
   volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 32);
   volatile uint32_t *flag = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 40);
+  // lapw[slot] = number of ring laps whose producer has ACQUIRED the slot.  A decoder warp may run
+  // more than one lap ahead of a slot's barrier (idle rounds, segment changes), where an mbarrier
+  // parity wait would alias; it first waits for its predecessor lap to be acquired.
+  volatile uint32_t *lapw = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 64);
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const ContainerView &cv = p.cv;
   const uint32_t G = gridDim.x, T = cv.n_tiles, KT = cv.KT;
 
   if (threadIdx.x == 0) {
-    for (uint32_t i = 0; i < p.U; ++i) { mbar_init(full_s + 8 * i, 2); mbar_init(empty_s + 8 * i, 1); }
+    for (uint32_t i = 0; i < p.U; ++i) { mbar_init(full_s + 8 * i, 2); mbar_init(empty_s + 8 * i, 1); lapw[i] = 0; }
     for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); }
     fence_mbar_init();
   }
@@ -294,50 +402,55 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     // ===================== decoder warps: Alg V.2 into the operand ring =====================
     const uint32_t d = uint32_t(warp - kFirstDecWarp);
     if (d < p.D) {
-      const uint32_t lt = lanemask_lt(), tab_s = smem_u32(tab), ring_s = smem0 + ring_off + d * kRingBytes;
+      const uint32_t lt = lanemask_lt(), ring_s = smem0 + ring_off + d * kRingBytes;
       const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
       const size_t rtb = raw_tile_bytes(cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
       const uint32_t xbytes = p.mpad * 32u;
-      uint32_t seq_base = 0;
-      for (uint32_t t = t_begin; t < t_end;) {
-        const uint32_t stripe = t / KT, ka = t % KT, nt = min(KT - ka, t_end - t);
-        for (uint32_t i = d; i < nt; i += p.D) {
-          const uint32_t r = i / p.D, cnt_r = min(p.D, nt - r * p.D), gt = t + i;
-          WarpStream s;
-          stream_open(s, cv.base + cv.off_records + size_t(offs[gt]) * 16, cv.base + cv.total, ring_s, lane);
-          RawReader<PAYLOAD> raw;
-          raw.tile_raw = cv.base + cv.off_raw + size_t(gt) * rtb;
-          raw.V = int(units) * 4;
-          uint4 raw_next = make_uint4(0, 0, 0, 0);
-          if (FMT == ANSLIN_FMT_BF16) raw_next = raw.load(0, lane);
-          for (uint32_t u = 0; u < units; ++u) {
-            const uint32_t seq = seq_base + r * units * p.D + u * cnt_r + d;
-            const uint32_t slot = seq % p.U, par = (seq / p.U) & 1u;
-            const uint32_t slot_a = slots_s + slot * p.slot_bytes;
-            mbar_wait(empty_s + 8 * slot, par ^ 1u);
-            const int k_elem = int((ka + i) * cv.tile_k + u * unit_k_of(FMT));
-            if (lane == 0) {
-              mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
-              if (p.layout == kLayoutSW32) {
-                tma_load_2d(slot_a + kUnitBytes, &tmx, k_elem, 0, full_s + 8 * slot);
-              } else {  // two 16-byte-wide boxes = two K-adjacent columns of 8x16B core matrices
-                tma_load_2d(slot_a + kUnitBytes, &tmx, k_elem, 0, full_s + 8 * slot);
-                tma_load_2d(slot_a + kUnitBytes + p.mpad * 16u, &tmx, k_elem + unit_k_of(FMT) / 2, 0, full_s + 8 * slot);
-              }
+      // Tiles of this CTA are dealt to the decoder warps round-robin over the CTA's WHOLE range
+      // (tile i -> warp i mod D, round i div D).  The MMA warp consumes units segment by segment
+      // (one accumulator per stripe segment); inside a segment the order is (round, unit, tile).
+      for (uint32_t i = d; i < t_end - t_begin; i += p.D) {
+        const uint32_t gt = t_begin + i, stripe = gt / KT, kt = gt % KT;
+        const uint32_t seg_a = max(t_begin, stripe * KT) - t_begin;            // segment = [seg_a, seg_b) in CTA-local tiles
+        const uint32_t seg_b = min(t_end, stripe * KT + KT) - t_begin;
+        const uint32_t rho = i / p.D;
+        const uint32_t grp_a = max(seg_a, rho * p.D), grp_b = min(seg_b, rho * p.D + p.D);   // this round's tiles of the segment
+        const uint32_t seq0 = (seg_a + (grp_a - seg_a)) * units, cnt = grp_b - grp_a, idx = i - grp_a;
+        WarpStream s;
+        stream_open(s, cv.base + cv.off_records + size_t(offs[gt]) * 16, cv.base + cv.total, ring_s, lane);
+        RawReader<PAYLOAD> raw;
+        raw.tile_raw = cv.base + cv.off_raw + size_t(gt) * rtb;
+        raw.V = int(units) * 4;
+        uint4 raw_next = make_uint4(0, 0, 0, 0), raw_next2 = raw_next;
+        if (FMT == ANSLIN_FMT_BF16) { raw_next = raw.load(0, lane); raw_next2 = raw.load(1, lane); }
+        for (uint32_t u = 0; u < units; ++u) {
+          const uint32_t seq = seq0 + u * cnt + idx;
+          const uint32_t slot = seq % p.U, lap = seq / p.U;
+          const uint32_t slot_a = slots_s + slot * p.slot_bytes;
+          for (uint32_t spins = 0; lapw[slot] < lap;)
+            if (++spins > (1u << 28)) __trap();
+          mbar_wait(empty_s + 8 * slot, (lap & 1u) ^ 1u);
+          if (lane == 0) lapw[slot] = lap + 1u;
+          const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
+          if (lane == 0) {
+            mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
+            if (p.layout == kLayoutSW32) {
+              tma_load_2d(slot_a + kUnitBytes, &tmx, k_elem, 0, full_s + 8 * slot);
+            } else {  // two 16-byte-wide boxes = two K-adjacent columns of 8x16B core matrices
+              tma_load_2d(slot_a + kUnitBytes, &tmx, k_elem, 0, full_s + 8 * slot);
+              tma_load_2d(slot_a + kUnitBytes + p.mpad * 16u, &tmx, k_elem + unit_k_of(FMT) / 2, 0, full_s + 8 * slot);
             }
-            SmemEmit emit{slot_a, p.layout};
-            const uint32_t *sz_row = nullptr;
-            if (FMT == ANSLIN_FMT_INT4_AWQ)
-              sz_row = reinterpret_cast<const uint32_t *>(cv.base + cv.off_scales) +
-                       size_t(uint32_t(k_elem) / cv.group) * cv.n_out + size_t(stripe) * kTileN;
-            decode_unit<FMT, PAYLOAD>(s, tab_s, lane, lt, int(u), raw, raw_next, sz_row, emit);
-            fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
-            __syncwarp();
-            if (lane == 0) mbar_arrive(full_s + 8 * slot);
           }
+          SmemEmit emit{slot_a, p.layout};
+          const uint32_t *sz_row = nullptr;
+          if (FMT == ANSLIN_FMT_INT4_AWQ)
+            sz_row = reinterpret_cast<const uint32_t *>(cv.base + cv.off_scales) +
+                     size_t(uint32_t(k_elem) / cv.group) * cv.n_out + size_t(stripe) * kTileN;
+          decode_unit<FMT, PAYLOAD>(s, smem0 + tab_off, lane, lt, int(u), raw, raw_next, raw_next2, sz_row, emit);
+          fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
+          __syncwarp();
+          if (lane == 0) mbar_arrive(full_s + 8 * slot);
         }
-        seq_base += nt * units;
-        t += nt;
       }
       cp_async_wait_all();
     }
@@ -373,63 +486,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       t += nt;
     }
   } else {
-    // ===================== epilogue warps 0..3: TMEM -> registers -> Y / split-K partials =====================
-    const uint32_t row = uint32_t(warp * 32 + lane);
-    uint32_t si = 0;
-    for (uint32_t t = t_begin; t < t_end; ++si) {
-      const uint32_t stripe = t / KT, ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
-      const bool whole = (ka == 0 && nt == KT);
-      const uint32_t n = stripe * kTileN + row;
-      float ws = 1.0f;
-      if (FMT == ANSLIN_FMT_INT8) ws = __half2float(reinterpret_cast<const __half *>(cv.base + cv.off_scales)[n]);
-      if (FMT == ANSLIN_FMT_FP8_E4M3) ws = cv.w_scale;
-      mbar_wait(tfull_s + 8 * ab, (si >> 1) & 1u);
-      tc_fence_after();
-      const uint32_t pslot = blockIdx.x * 2u + (t == t_begin ? 0u : 1u);
-      uint32_t *part = p.partials + size_t(pslot) * p.mpad * kTileN;
-      for (uint32_t c0 = 0; c0 < p.mpad; c0 += 16) {
-        uint32_t v[16];
-        tmem_ld16(tmem_base + ((uint32_t(warp) * 32u) << 16) + ab * p.mpad + c0, v);
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const uint32_t mm = c0 + j;
-          if (mm < p.m) {
-            if (whole) {
-              const float xs = (FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3) ? p.x_scale[mm] : 1.0f;
-              p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(v[j], xs, ws);
-            } else {
-              part[size_t(mm) * kTileN + row] = v[j];
-            }
-          }
-        }
-      }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(tempty_s + 8 * ab);
-      if (!whole) {
-        // Deterministic split-K fix-up: the LAST CTA to finish a stripe sums all partials in CTA order.
-        const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
-        __threadfence();
-        named_bar_sync(1, kEpiWarps * 32);
-        if (threadIdx.x == 0) *flag = (atomicAdd(&p.counters[stripe], 1u) == c_last - c_first) ? 1u : 0u;
-        named_bar_sync(1, kEpiWarps * 32);
-        if (*flag) {
-          __threadfence();
-          for (uint32_t mm = 0; mm < p.m; ++mm) {
-            uint32_t acc = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-            for (uint32_t c = c_first; c <= c_last; ++c) {
-              const uint32_t ps = c * 2u + (cta_first_tile(c, G, T) / KT == stripe ? 0u : 1u);
-              acc = acc_add<FMT>(acc, __ldcg(p.partials + (size_t(ps) * p.mpad + mm) * kTileN + row));
-            }
-            const float xs = (FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3) ? p.x_scale[mm] : 1.0f;
-            p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(acc, xs, ws);
-          }
-          if (threadIdx.x == 0) p.counters[stripe] = 0;
-        }
-        named_bar_sync(1, kEpiWarps * 32);  // flag is reused by the next segment
-      }
-      t += nt;
-    }
+    // ===================== epilogue warps 0..3 =====================
+    EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, p.y, p.ldy, p.partials,
+                 p.counters, p.m, p.mpad};
+    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, flag, t_begin, t_end, KT, G, T, warp, lane);
   }
   tc_fence_before();
   __syncthreads();
@@ -516,61 +576,8 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
     }
     (void)UK;
   } else {
-    const uint32_t row = uint32_t(warp * 32 + lane);
-    uint32_t si = 0;
-    for (uint32_t t = t_begin; t < t_end; ++si) {
-      const uint32_t stripe = t / KT, ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
-      const bool whole = (ka == 0 && nt == KT);
-      const uint32_t n = stripe * kTileN + row;
-      float ws = 1.0f;
-      if (FMT == ANSLIN_FMT_INT8) ws = __half2float(reinterpret_cast<const __half *>(p.w_scale_h)[n]);
-      if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
-      mbar_wait(tfull_s + 8 * ab, (si >> 1) & 1u);
-      tc_fence_after();
-      const uint32_t pslot = blockIdx.x * 2u + (t == t_begin ? 0u : 1u);
-      uint32_t *part = p.partials + size_t(pslot) * p.mpad * kTileN;
-      for (uint32_t c0 = 0; c0 < p.mpad; c0 += 16) {
-        uint32_t v[16];
-        tmem_ld16(tmem_base + ((uint32_t(warp) * 32u) << 16) + ab * p.mpad + c0, v);
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const uint32_t mm = c0 + j;
-          if (mm < p.m) {
-            if (whole) {
-              const float xs = (FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3) ? p.x_scale[mm] : 1.0f;
-              p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(v[j], xs, ws);
-            } else {
-              part[size_t(mm) * kTileN + row] = v[j];
-            }
-          }
-        }
-      }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(tempty_s + 8 * ab);
-      if (!whole) {
-        const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
-        __threadfence();
-        named_bar_sync(1, kEpiWarps * 32);
-        if (threadIdx.x == 0) *flag = (atomicAdd(&p.counters[stripe], 1u) == c_last - c_first) ? 1u : 0u;
-        named_bar_sync(1, kEpiWarps * 32);
-        if (*flag) {
-          __threadfence();
-          for (uint32_t mm = 0; mm < p.m; ++mm) {
-            uint32_t acc = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-            for (uint32_t c = c_first; c <= c_last; ++c) {
-              const uint32_t ps = c * 2u + (cta_first_tile(c, G, T) / KT == stripe ? 0u : 1u);
-              acc = acc_add<FMT>(acc, __ldcg(p.partials + (size_t(ps) * p.mpad + mm) * kTileN + row));
-            }
-            const float xs = (FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3) ? p.x_scale[mm] : 1.0f;
-            p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(acc, xs, ws);
-          }
-          if (threadIdx.x == 0) p.counters[stripe] = 0;
-        }
-        named_bar_sync(1, kEpiWarps * 32);
-      }
-      t += nt;
-    }
+    EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.m, p.mpad};
+    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, flag, t_begin, t_end, KT, G, T, warp, lane);
   }
   tc_fence_before();
   __syncthreads();
@@ -624,7 +631,12 @@ uint32_t tmem_cols_of(uint32_t mpad) {
   return c;
 }
 constexpr size_t kSmemMax = 232448;  // 227 KiB opt-in per CTA
-uint32_t grid_of(uint32_t n_tiles) { return uint32_t(std::min<uint64_t>(n_tiles, uint64_t(std::max(1, num_sms())))); }
+// Persistent grid: one CTA per SM, but never fewer than `min_tiles` tiles per CTA (a CTA's decoder
+// warps work on that many tiles concurrently, and fewer CTAs per stripe = fewer split-K partials).
+uint32_t grid_of(uint32_t n_tiles, uint32_t min_tiles) {
+  const uint64_t by_work = std::max<uint64_t>(1, n_tiles / min_tiles);
+  return uint32_t(std::min<uint64_t>(by_work, uint64_t(std::max(1, num_sms()))));
+}
 
 struct Workspace { size_t counters_off, partials_off, total; };
 Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
@@ -647,6 +659,11 @@ int launch_fused(const anslin_weight *w, const CUtensorMap &tmx, GemmParams &p, 
   kern<<<grid, kGemmThreads, smem, st>>>(tmx, p);
   ++g_launches;
   (void)w;
+  if (getenv("ANSLIN_DEBUG")) {  // debugging aid only: synchronous error report
+    cudaError_t e = cudaStreamSynchronize(st);
+    fprintf(stderr, "[anslin] fused grid=%u smem=%zu D=%u U=%u mpad=%u tiles=%u: %s\n", grid, smem, p.D, p.U, p.mpad,
+            p.cv.n_tiles, cudaGetErrorString(e));
+  }
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 
@@ -675,9 +692,9 @@ int gemm_one(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_
   p.ldy = ldy;
   const char *lay = getenv("ANSLIN_LAYOUT");  // debug: "none" selects the unswizzled core-matrix layout
   p.layout = (lay && lay[0] == 'n') ? kLayoutNone : kLayoutSW32;
-  const uint32_t grid = grid_of(h.n_tiles), stripes = h.n_out / kTileN;
+  const uint32_t grid = grid_of(h.n_tiles, 12), stripes = h.n_out / kTileN;
   // ring sizing: D decoder warps (1 KiB compressed-word ring each) and U operand slots
-  const size_t fixed = 1024 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 64;
+  const size_t fixed = 1024 /*align slack*/ + 1024 /*ring alignment*/ + 16384 + 1056 + 16 * kMaxSlots + 64 + 4 * kMaxSlots;
   uint32_t D = kMaxDecWarps, U = 0;
   const char *denv = getenv("ANSLIN_DECODER_WARPS");
   if (denv && atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
@@ -715,7 +732,9 @@ int gemm_one(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_
 
 template <uint32_t FMT, bool PAYLOAD>
 int launch_decode(const ContainerView &cv, void *out, cudaStream_t st) {
-  const uint32_t ctas = std::min<uint32_t>((cv.n_tiles + kDecWarps - 1) / kDecWarps, uint32_t(std::max(1, num_sms())) * 6u);
+  uint32_t per_sm = 4;
+  if (const char *e = getenv("ANSLIN_DECODE_CTAS_PER_SM")) per_sm = uint32_t(std::max(1, atoi(e)));  // debug knob
+  const uint32_t ctas = std::min<uint32_t>((cv.n_tiles + kDecWarps - 1) / kDecWarps, uint32_t(std::max(1, num_sms())) * per_sm);
   decode_kernel<FMT, PAYLOAD><<<ctas, kDecWarps * 32, 0, st>>>(cv, static_cast<uint8_t *>(out));
   ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
@@ -829,7 +848,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   const size_t fixed = 1024 + 16 * kMaxSlots + 64;
   p.S = uint32_t(std::min<size_t>((kSmemMax - fixed) / p.stage_bytes, 12));
   const size_t smem = fixed + size_t(p.S) * p.stage_bytes;
-  const uint32_t stripes = n_out / kTileN, T = stripes * p.KB, grid = grid_of(T);
+  const uint32_t stripes = n_out / kTileN, T = stripes * p.KB, grid = grid_of(T, 8);
   const Workspace ws = workspace_layout(stripes, grid, p.mpad);
   if (workspace_bytes < ws.total) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   p.counters = reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(workspace_dev) + ws.counters_off);
