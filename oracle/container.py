@@ -29,6 +29,7 @@ PROB_BITS = 12        # b (P:l.442 "default b = 12")
 WORD_BITS = 16        # w   (reading A3)
 STATE_LO_LOG2 = 16    # L = 2^16 (reading A3)
 HEADER_BYTES = 128
+TAIL_BYTES = 4096      # readable bytes that must follow the records section
 
 # symbols per 16-byte operand chunk, and default tile_k (in weights) per format
 SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4}
@@ -236,6 +237,7 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     off_raw = _align(off_records + len(rec_bytes))
     off_scales = _align(off_raw + len(raw_bytes))
     total = _align(off_scales + len(side))
+    total = max(total, _align(off_records + len(rec_bytes) + TAIL_BYTES))   # tail rule
     hdr = Header(fmt, n_out, k_in, TILE_N, tile_k, LANES, PROB_BITS, WORD_BITS, STATE_LO_LOG2, group_size, flags,
                  n_tiles, float(w_scale), off_freq, off_offsets, off_records, off_raw if raw_bytes else 0,
                  off_scales if side else 0, 0, total)

@@ -23,6 +23,7 @@ constexpr int kStateLoLog2 = 16; // L = 2^16
 constexpr uint32_t kL = 1u << kStateLoLog2;
 constexpr uint32_t kM = 1u << kProbBits;
 constexpr int kHeaderBytes = 128;
+constexpr int kTailBytes = 4096; // readable bytes guaranteed after the records section (ring read-ahead)
 constexpr int kUnitBytes = 4096; // one operand unit = 128 rows x 32 B (one tcgen05.mma K step)
 
 struct Header {  // 128 bytes, little endian

@@ -5,9 +5,9 @@
 // x = f*(x>>12) + bias;  if x < 2^16: x = x<<16 | next word.  The words of a tile are interleaved
 // in decoder read order, so the renormalising lanes of a step read CONSECUTIVE 16-bit words
 // (P:l.256 "renormalization loads are naturally coalesced"): ballot + popc prefix picks the word.
-// The compressed words are streamed HBM -> shared memory through a per-warp 1 KiB ring with
-// 16-byte cp.async (16 lanes x 16 B = 256 B per fill, 768..1024 B of look-ahead); the ring
-// bookkeeping runs once per FOUR decode steps.
+// The compressed words are streamed HBM -> shared memory through a per-warp 2 KiB ring with
+// 16-byte cp.async (32 lanes x 16 B = 512 B per fill, 1.5-2 KiB of look-ahead); the ring
+// bookkeeping runs once per EIGHT decode steps.
 //
 // Table entry (4 B, Eq.3's "2^b x 4 B", P:l.440):  sym[7:0] | f[19:8] | bias[31:20].
 #pragma once
@@ -17,8 +17,11 @@
 
 namespace anslin {
 
-constexpr uint32_t kRingBytes = 1024;  // per decoder warp; the ring must be 1 KiB aligned
-constexpr uint32_t kFillBytes = 256;
+constexpr uint32_t kRingBytes = 2048;  // per decoder warp; the ring must be 2 KiB aligned
+constexpr uint32_t kFillBytes = 512;   // 32 lanes x 16 B per fill
+// The ring reads ahead of the record it decodes: the container guarantees this many readable bytes
+// after the records section (tail rule), so fills need no bounds check.
+static_assert(2 * kRingBytes <= uint32_t(kTailBytes), "ring read-ahead must fit the container tail rule");
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ uint32_t lanemask_lt() {
@@ -91,40 +94,37 @@ __device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, c
 struct WarpStream {
   uint32_t x;       // this lane's rANS state
   uint32_t posb;    // BYTES of words consumed so far (warp uniform)
-  uint32_t filled;  // bytes of words whose ring fill has been issued (warp uniform, multiple of 256)
-  uint32_t limit;   // readable bytes from words_g (clamp for the over-read at the container end)
-  uint32_t ring;    // shared-space address of this warp's 1 KiB-aligned ring
-  const uint8_t *words_g;
+  uint32_t filled;  // bytes of words whose ring fill has been issued (warp uniform, multiple of 512)
+  uint32_t ring;    // shared-space address of this warp's 2 KiB-aligned ring
+  const uint8_t *src;  // this lane's next fill source = words + filled + 16*lane
 };
 
-// Issue the next 256-byte ring fill iff `on` (lanes 0..15 copy 16 B each).
+// Issue the next 512-byte ring fill iff `on` (every lane copies 16 B).
 __device__ __forceinline__ void stream_fill_if(WarpStream &s, uint32_t on, int lane) {
-  const uint32_t off = s.filled + (uint32_t(lane) << 4);
-  cp_async16_if(on & uint32_t(lane < 16), s.ring | (off & (kRingBytes - 1)), s.words_g + off, off + 16u <= s.limit ? 16u : 0u);
+  cp_async16_if(on, s.ring | ((s.filled + (uint32_t(lane) << 4)) & (kRingBytes - 1)), s.src, 16u);
   cp_async_commit_if(on);
   s.filled += on ? kFillBytes : 0u;
+  s.src += on ? kFillBytes : 0u;
 }
 
-// rec = start of the tile record in HBM (16-byte aligned); end = one past the last readable byte.
-__device__ __forceinline__ void stream_open(WarpStream &s, const uint8_t *rec, const uint8_t *end, uint32_t ring, int lane) {
+// rec = start of the tile record in HBM (16-byte aligned).
+__device__ __forceinline__ void stream_open(WarpStream &s, const uint8_t *rec, uint32_t ring, int lane) {
   cp_async_wait_all();  // fills of the previous tile may still be in flight into this ring
   __syncwarp();
   s.x = reinterpret_cast<const uint32_t *>(rec)[lane];
-  s.words_g = rec + 4 * kLanes;
-  const size_t room = size_t(end - s.words_g);
-  s.limit = room > 0xFFFFFFF0ull ? 0xFFFFFFF0u : uint32_t(room);
+  s.src = rec + 4 * kLanes + 16 * lane;
   s.posb = 0; s.filled = 0; s.ring = ring;
 #pragma unroll
   for (int i = 0; i < 4; ++i) stream_fill_if(s, 1u, lane);
 }
 
-// Ring upkeep for the next FOUR decode steps (they consume at most 256 B): refill the dead quarter
-// behind the read position and make sure everything up to posb + 512 has landed.  Invariant:
-// 768 <= filled - posb <= 1024 after the call, at most ONE fill pending => landed >= posb + 512
-// >= the 256 + 62 bytes the four steps can touch.  A fill writes ring bytes
-// [filled, filled + 256) - 1024 < posb, i.e. only words already consumed.
-__device__ __forceinline__ void stream_upkeep4(WarpStream &s, int lane) {
-  stream_fill_if(s, uint32_t(s.filled - s.posb < 768u), lane);
+// Ring upkeep for the next EIGHT decode steps (they consume at most 512 B): refill the dead quarter
+// behind the read position and make sure everything up to posb + 1024 has landed.  Invariant:
+// 1536 <= filled - posb <= 2048 after the call, at most ONE fill pending => landed >= posb + 1024
+// >= the 512 + 62 bytes eight steps can touch.  A fill writes ring bytes
+// [filled, filled + 512) - 2048 < posb, i.e. only words already consumed.
+__device__ __forceinline__ void stream_upkeep8(WarpStream &s, int lane) {
+  stream_fill_if(s, uint32_t(s.filled - s.posb < 1536u), lane);
   cp_async_wait_1();
   __syncwarp();
 }
@@ -149,10 +149,9 @@ template <int pos>
 __device__ __forceinline__ uint32_t put_sym(uint32_t acc, uint32_t e) {
   return __byte_perm(acc, e, (0x3210 & ~(0xF << (4 * pos))) | (4 << (4 * pos)));
 }
-// Four decode steps -> four symbol bytes (one ring upkeep).
-__device__ __forceinline__ uint32_t decode4(WarpStream &s, uint32_t tab, int lane, uint32_t lt) {
+// Four decode steps -> four symbol bytes.
+__device__ __forceinline__ uint32_t decode4(WarpStream &s, uint32_t tab, uint32_t lt) {
   uint32_t q = 0;
-  stream_upkeep4(s, lane);
   q = put_sym<0>(q, decode_step(s, tab, lt));
   q = put_sym<1>(q, decode_step(s, tab, lt));
   q = put_sym<2>(q, decode_step(s, tab, lt));
@@ -214,7 +213,8 @@ __device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab, int lan
       if (v + 2 < raw.V) raw_next2 = raw.load(v + 2, lane);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        const uint32_t E0 = decode4(s, tab, lane, lt), E1 = decode4(s, tab, lane, lt);
+        stream_upkeep8(s, lane);
+        const uint32_t E0 = decode4(s, tab, lt), E1 = decode4(s, tab, lt);
         if (kPayload && v == raw.V - 1 && h == 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
           const uint32_t p = s.x - kL;
           rv.w = (rv.w & 0xFFFFu) | (p << 16);
@@ -226,7 +226,8 @@ __device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab, int lan
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll 1
     for (int g = 0; g < 8; ++g) {
-      const uint32_t B = decode4(s, tab, lane, lt);
+      if ((g & 1) == 0) stream_upkeep8(s, lane);
+      const uint32_t B = decode4(s, tab, lt);
       if constexpr (Emit::kOperand) {
         const uint32_t szv = __ldg(sz_row + (g & 3) * 32 + lane);
         const __half2 sz = *reinterpret_cast<const __half2 *>(&szv);
@@ -241,8 +242,10 @@ __device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab, int lan
   } else {  // fp8 / int8: the byte is the operand
 #pragma unroll 1
     for (int g = 0; g < 8; ++g) {
-      const uint32_t q0 = decode4(s, tab, lane, lt), q1 = decode4(s, tab, lane, lt);
-      const uint32_t q2 = decode4(s, tab, lane, lt), q3 = decode4(s, tab, lane, lt);
+      stream_upkeep8(s, lane);
+      const uint32_t q0 = decode4(s, tab, lt), q1 = decode4(s, tab, lt);
+      stream_upkeep8(s, lane);
+      const uint32_t q2 = decode4(s, tab, lt), q3 = decode4(s, tab, lt);
       emit.chunk(g, lane, make_uint4(q0, q1, q2, q3));
     }
   }

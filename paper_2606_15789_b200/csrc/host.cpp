@@ -175,7 +175,7 @@ size_t anslin_encode_bound(const anslin_desc *desc) {
   const size_t rec = align16(4 * kLanes + 2 * (tile_syms * 3 / 4 + 2 * kLanes + 8));
   size_t total = kHeaderBytes + 512 + align16(4 * (g.n_tiles + 1)) + g.n_tiles * rec + 64;
   if (g.fmt == ANSLIN_FMT_BF16) total += g.n_tiles * raw_tile_bytes(g.tile_k, 0) + 16;
-  return total + align16(side_bytes(g)) + 16;
+  return total + align16(side_bytes(g)) + 16 + kTailBytes;
 }
 
 int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *scales_host, const void *zeros_host,
@@ -248,6 +248,9 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   const size_t after_raw = rtb ? h.off_raw + raw_all.size() : h.off_records + rec_total;
   h.off_scales = sb ? align16(after_raw) : 0;
   h.total_bytes = align16(sb ? h.off_scales + sb : after_raw);
+  // tail rule: the decoder's compressed-word ring reads ahead of the record it decodes, so at least
+  // kTailBytes readable bytes follow the records section (zero padding if the sections after it are short)
+  h.total_bytes = std::max<uint64_t>(h.total_bytes, align16(h.off_records + rec_total + kTailBytes));
   *bytes_out = h.total_bytes;
   if (h.total_bytes > capacity) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   if (rec_total / 16 > 0xFFFFFFFFull) return ANSLIN_ERR_UNSUPPORTED;
@@ -346,6 +349,7 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   if (rec_end < h.off_records || rec_end > T) return ANSLIN_ERR_CORRUPT;
   const uint64_t rec_units = (rec_end - h.off_records) / 16;
   if (offs[0] != 0) return ANSLIN_ERR_CORRUPT;
+  if (h.off_records + uint64_t(offs[g.n_tiles]) * 16 + kTailBytes > T) return ANSLIN_ERR_CORRUPT;  // tail rule
   for (size_t t = 0; t < g.n_tiles; ++t) {
     // a record holds at least the 32 lane states and never more than the worst-case tile
     if (offs[t + 1] < offs[t] + 8 || offs[t + 1] > rec_units) return ANSLIN_ERR_CORRUPT;

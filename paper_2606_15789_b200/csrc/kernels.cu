@@ -40,9 +40,13 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 // Bounded wait: a protocol bug traps (launch failure) instead of hanging the GPU.
+// kSleepNs > 0 backs off between probes so that long waits (MMA issuer, epilogue) do not steal issue
+// slots from the decoder warps sharing their scheduler.
+template <int kSleepNs = 0>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   uint32_t done = 0, spins = 0;
   while (true) {
+    if (kSleepNs > 0 && spins > 0) __nanosleep(kSleepNs);
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
@@ -167,17 +171,17 @@ template <uint32_t FMT, bool PAYLOAD>
 __global__ void __launch_bounds__(kDecWarps * 32) decode_kernel(ContainerView cv, uint8_t *out) {
   __shared__ __align__(16) uint32_t tab[kM];
   __shared__ uint32_t cum[260];
-  __shared__ __align__(1024) uint8_t rings[kDecWarps][kRingBytes];
+  __shared__ __align__(16) uint8_t rings[(kDecWarps + 1) * kRingBytes];  // +1: rounded up to ring-size alignment below
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t lt = lanemask_lt(), ring_s = smem_u32(rings[warp]);
+  const uint32_t lt = lanemask_lt(), ring_s = ((smem_u32(rings) + kRingBytes - 1) & ~(kRingBytes - 1)) + uint32_t(warp) * kRingBytes;
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
   const size_t row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.k_in) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.k_in) / 2 : size_t(cv.k_in);
   const size_t tile_row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.tile_k) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.tile_k) / 2 : size_t(cv.tile_k);
   const size_t rtb = raw_tile_bytes(cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
   for (uint32_t t = blockIdx.x * kDecWarps + warp; t < cv.n_tiles; t += gridDim.x * kDecWarps) {
     WarpStream s;
-    stream_open(s, cv.base + cv.off_records + size_t(offs[t]) * 16, cv.base + cv.total, ring_s, lane);
+    stream_open(s, cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s, lane);
     const uint32_t stripe = t / cv.KT, kt = t % cv.KT;
     GlobalEmit<FMT> emit;
     emit.tile_out = out + size_t(stripe) * kTileN * row_bytes + size_t(kt) * tile_row_bytes;
@@ -291,7 +295,7 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     float ws = 1.0f;
     if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n]);
     if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
-    mbar_wait(tfull_s + 8 * ab, (si >> 1) & 1u);
+    mbar_wait<400>(tfull_s + 8 * ab, (si >> 1) & 1u);
     tc_fence_after();
     const uint32_t pslot = blockIdx.x * 2u + (t == t_begin ? 0u : 1u);
     uint32_t *part = p.partials + size_t(pslot) * p.mpad * kTileN;
@@ -362,11 +366,11 @@ template <uint32_t FMT, bool PAYLOAD>
 __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ CUtensorMap tmx, GemmParams p) {
   using TR = FmtTraits<FMT>;
   extern __shared__ uint8_t smem_raw[];
-  const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t smem0 = (smem_u32(smem_raw) + 2047u) & ~2047u;
   uint8_t *smem = smem_raw + (smem0 - smem_u32(smem_raw));
   // carve-up
   const uint32_t slots_s = smem0;
-  const uint32_t ring_off = (p.U * p.slot_bytes + 1023u) & ~1023u;   // rings are 1 KiB aligned
+  const uint32_t ring_off = (p.U * p.slot_bytes + kRingBytes - 1) & ~(kRingBytes - 1);   // rings are ring-size aligned
   const uint32_t tab_off = ring_off + p.D * kRingBytes;
   uint32_t *tab = reinterpret_cast<uint32_t *>(smem + tab_off);
   uint32_t *cum = reinterpret_cast<uint32_t *>(smem + tab_off + 16384);
@@ -417,7 +421,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
         const uint32_t grp_a = max(seg_a, rho * p.D), grp_b = min(seg_b, rho * p.D + p.D);   // this round's tiles of the segment
         const uint32_t seq0 = (seg_a + (grp_a - seg_a)) * units, cnt = grp_b - grp_a, idx = i - grp_a;
         WarpStream s;
-        stream_open(s, cv.base + cv.off_records + size_t(offs[gt]) * 16, cv.base + cv.total, ring_s, lane);
+        stream_open(s, cv.base + cv.off_records + size_t(offs[gt]) * 16, ring_s, lane);
         RawReader<PAYLOAD> raw;
         raw.tile_raw = cv.base + cv.off_raw + size_t(gt) * rtb;
         raw.V = int(units) * 4;
@@ -460,12 +464,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     uint32_t seq = 0, si = 0;
     for (uint32_t t = t_begin; t < t_end; ++si) {
       const uint32_t ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
-      mbar_wait(tempty_s + 8 * ab, ((si >> 1) & 1u) ^ 1u);  // epilogue has drained this accumulator
+      mbar_wait<100>(tempty_s + 8 * ab, ((si >> 1) & 1u) ^ 1u);  // epilogue has drained this accumulator
       tc_fence_after();
       const uint32_t n_units = nt * units;
       for (uint32_t j = 0; j < n_units; ++j, ++seq) {
         const uint32_t slot = seq % p.U, par = (seq / p.U) & 1u;
-        mbar_wait(full_s + 8 * slot, par);
+        mbar_wait<40>(full_s + 8 * slot, par);
         tc_fence_after();
         if (lane == 0) {
           const uint32_t a = slots_s + slot * p.slot_bytes, b = a + kUnitBytes;
@@ -694,10 +698,14 @@ int gemm_one(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_
   p.layout = (lay && lay[0] == 'n') ? kLayoutNone : kLayoutSW32;
   const uint32_t grid = grid_of(h.n_tiles, 12), stripes = h.n_out / kTileN;
   // ring sizing: D decoder warps (1 KiB compressed-word ring each) and U operand slots
-  const size_t fixed = 1024 /*align slack*/ + 1024 /*ring alignment*/ + 16384 + 1056 + 16 * kMaxSlots + 64 + 4 * kMaxSlots;
+  const size_t fixed = 2048 /*align slack*/ + 2048 /*ring alignment*/ + 16384 + 1056 + 16 * kMaxSlots + 64 + 4 * kMaxSlots;
   uint32_t D = kMaxDecWarps, U = 0;
   const char *denv = getenv("ANSLIN_DECODER_WARPS");
   if (denv && atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
+  {  // even rounds: a CTA with tpc tiles needs ceil(tpc/D) tile-times; use the fewest warps that keep that count
+    const uint32_t tpc = (h.n_tiles + grid - 1) / grid, rounds = (tpc + D - 1) / D;
+    D = std::max(1u, (tpc + rounds - 1) / rounds);
+  }
   for (;; --D) {
     const size_t left = kSmemMax - fixed - size_t(D) * kRingBytes;
     U = uint32_t(std::min<size_t>(left / p.slot_bytes, kMaxSlots));

@@ -69,7 +69,7 @@ def test_cross_decode_and_stats(name, fmt, w, k_in, kw):
     wps = 2 if fmt == oc.FMT_INT4_AWQ else 1
     assert st["bits_per_weight"] >= (st["entropy_bits_per_symbol"] + st["raw_entropy_bits_per_symbol"]) / wps
     total_bits = (st["payload_bits"] + st["state_bits"] + st["pad_bits"] + st["raw_bits"] + st["side_bits"])
-    assert total_bits <= 8 * buf.size <= total_bits + st["offset_table_bits"] + st["freq_table_bits"] + 8 * (128 + 5 * 16)
+    assert total_bits <= 8 * buf.size <= total_bits + st["offset_table_bits"] + st["freq_table_bits"] + 8 * (128 + 5 * 16 + 4096)
 
 
 def test_config1_gap_through_the_abi():
