@@ -54,7 +54,7 @@ class ClockSampler:
             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + q, "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "25"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
         except OSError:
             self.proc = None
@@ -63,15 +63,24 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append([t.strip() for t in line.split(",")])
 
-    def stop(self):
+    def wait_first(self, timeout=5.0):
+        t0 = time.time()
+        while self.proc is not None and not self.rows and time.time() - t0 < timeout:
+            time.sleep(0.01)
+
+    def mark(self):
+        return len(self.rows)
+
+    def stop(self, lo=0, hi=None):
+        """Summary over the samples taken between mark() lo and mark() hi (the timed region)."""
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
         self.proc.terminate()
-        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        rows = self.rows[max(lo - 1, 0):(hi + 1 if hi is not None else None)]
+        sm = [float(r[0]) for r in rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        reasons = sorted({names[i] for r in rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
                 "samples": len(sm)}
 
@@ -127,7 +136,7 @@ def run_reference(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=300)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="anslin")
     ap.add_argument("--m", type=int, default=75)
@@ -139,16 +148,13 @@ def main():
     import torch
     from paper_2606_15789_b200 import binding as B, build as libbuild, inputs, runtime as rt
     libbuild.build()
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    from paper_2606_15789_b200.dist import Ranks
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: anslin has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ranks = Ranks("nccl", torch.device("cuda", local))
+    world, rank = ranks.world, ranks.rank
 
     # ---- offline stage (untimed): synthesize, compress, upload
     layer = layer_weights()
@@ -158,7 +164,7 @@ def main():
         containers.append(buf); stats.append(st)
     dws = [rt.DeviceWeight(c) for c in containers]
     m = args.m
-    xs_host = [torch.from_numpy(inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=500 + i + 97 * rank)).view(np.int16)).pin_memory()
+    xs_host = [torch.from_numpy(inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=ranks.batch_seed(500 + i))).view(np.int16)).pin_memory()
                for i, (_, n, k, _) in enumerate(layer)]
     xs = [t.cuda().view(torch.bfloat16) for t in xs_host]
     ys = [torch.empty((m, n), dtype=torch.float32, device="cuda") for (_, n, k, _) in layer]
@@ -181,14 +187,14 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if dist is not None:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize()
 
+    sampler = ClockSampler(local); sampler.start(); sampler.wait_first()
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
-    sampler = ClockSampler(local); sampler.start()
+    mark_lo = sampler.mark()
     evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in dws] for _ in range(args.steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
@@ -197,10 +203,9 @@ def main():
         launches += step(evs[s])
     e1.record()
     barrier()
-    clocks = sampler.stop()
-    ms = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); ms = float(t.item())
+    time.sleep(0.03)
+    clocks = sampler.stop(mark_lo, sampler.mark())
+    ms = ranks.max_over_ranks(e0.elapsed_time(e1))
     ms_step = ms / args.steps
     value = world * flops_step / (ms_step * 1e-3) / 1e12
     kern_ms = [[a.elapsed_time(b) for (a, b) in row] for row in evs]
@@ -226,9 +231,7 @@ def main():
     for _ in range(args.steps):
         step_e2e()
     barrier()
-    e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device="cuda"); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e_s = ranks.max_over_ranks(time.perf_counter() - t0)
     e2e = {"value": world * flops_step * args.steps / e2e_s / 1e12, "unit": UNIT,
            "h2d_bytes_per_step": int(sum(m * k * 2 for (_, n, k, _) in layer)),
            "d2h_bytes_per_step": int(sum(m * n * 4 for (_, n, k, _) in layer))}
@@ -296,8 +299,7 @@ def main():
         out["cpu_baseline"] = cpu_oracle_leg(layer, containers, m)
     if rank == 0:
         print(json.dumps(out))
-    if dist is not None:
-        dist.destroy_process_group()
+    ranks.close()
 
 
 if __name__ == "__main__":

@@ -431,9 +431,11 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           const uint32_t seq = seq0 + u * cnt + idx;
           const uint32_t slot = seq % p.U, lap = seq / p.U;
           const uint32_t slot_a = slots_s + slot * p.slot_bytes;
-          for (uint32_t spins = 0; lapw[slot] < lap;)
-            if (++spins > (1u << 28)) __trap();
-          mbar_wait(empty_s + 8 * slot, (lap & 1u) ^ 1u);
+          for (uint32_t spins = 0; lapw[slot] < lap;) {  // a waiting decoder sleeps: it must not take issue slots
+            __nanosleep(100);
+            if (++spins > (1u << 24)) __trap();
+          }
+          mbar_wait<100>(empty_s + 8 * slot, (lap & 1u) ^ 1u);
           if (lane == 0) lapw[slot] = lap + 1u;
           const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
           if (lane == 0) {
