@@ -66,11 +66,12 @@ typedef struct {
   uint32_t format;      /* anslin_format */
   uint32_t n_out, k_in; /* W is [n_out x k_in] */
   uint32_t tile_k;      /* K extent of one tile in weights; 0 = format default (bf16 64, fp8/int8/int4 256);
-                           tile rows are always 128 (= tcgen05 MMA M); 32 interleaved streams per tile */
+                           32 interleaved streams per tile */
   uint32_t group_size;  /* int4: quantisation group along K (multiple of 16); else 0 */
   uint32_t flags;       /* ANSLIN_FLAG_* */
   float    w_scale;     /* fp8: per-tensor dequant scale applied to Y; other formats: ignored (1.0) */
-  uint32_t reserved;
+  uint32_t tile_n;      /* weight rows per tile: 128 (= tcgen05 MMA M; 0 selects it; BASELINE config 1's 128 x 64)
+                           or 32 (the paper's 32-row tile shape, P:l.444: four tiles share one MMA stripe) */
 } anslin_desc;
 
 /* Size accounting filled by the encoder (P:l.444 reports payload and metadata separately). Bits. */

@@ -23,7 +23,8 @@ MAGIC = 0x4C534E41  # "ANSL"
 VERSION = 1
 FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ = 0, 1, 2, 3
 FLAG_STATE_PAYLOAD = 1
-TILE_N = 128          # weight rows per tile = MMA M
+STRIPE_N = 128        # weight rows per stripe = MMA M; a stripe is cut into tiles of tile_n rows
+TILE_N = 128          # default tile_n (BASELINE config 1: 128 x 64 tiles); 32 is the other supported height
 LANES = 32            # R interleaved streams per tile (P:l.192; BASELINE config 1)
 PROB_BITS = 12        # b (P:l.442 "default b = 12")
 WORD_BITS = 16        # w   (reading A3)
@@ -68,30 +69,33 @@ def desymbolise(fmt: int, coded: np.ndarray, raw):
     return coded
 
 
-def tile_order(fmt: int, tile_k: int):
+def tile_order(fmt: int, tile_k: int, tile_n: int = TILE_N):
     """Tile symbol order (reading A6).  Returns (rows, cols): symbol i of the tile is the coded
-    symbol at (row rows[i], symbol column cols[i]) of the tile's [128 x sym_cols] symbol matrix.
+    symbol at (row rows[i], symbol column cols[i]) of the tile's [tile_n x sym_cols] symbol matrix.
 
     i = t*32 + lane.  The tile is cut along K into units of 32 operand bytes per row
     (16 bf16/fp16 weights, 32 fp8/int8 weights); unit u is decoded completely before unit u+1.
-    Inside a unit there are 8 chunk rounds g; in round g lane l owns the 16-byte operand chunk
-    (row (g mod 4)*32 + l, half g div 4) and produces its spc symbols in steps
-    t = (u*8 + g)*spc + e, e = 0..spc-1.
+    Inside a unit there are G = 2*tile_n/32 chunk rounds g; in round g lane l owns the 16-byte
+    operand chunk (row (g mod tile_n/32)*32 + l, half g div (tile_n/32)) and produces its spc
+    symbols in steps t = (u*G + g)*spc + e, e = 0..spc-1.  (tile_n = 32: lane l simply walks row l.)
     """
+    assert tile_n in (32, 128)
     spc = SPC[fmt]
+    rb = tile_n // 32
+    G = 2 * rb
     sym_cols = tile_k // WEIGHTS_PER_SYMBOL[fmt]
     units = sym_cols // (2 * spc)
     assert units * 2 * spc == sym_cols, "tile_k must be a multiple of the unit width"
-    steps = units * 8 * spc
+    steps = units * G * spc
     rows = np.zeros(steps * LANES, dtype=np.int64)
     cols = np.zeros(steps * LANES, dtype=np.int64)
     for u in range(units):
-        for g in range(8):
+        for g in range(G):
             for e in range(spc):
-                t = (u * 8 + g) * spc + e
+                t = (u * G + g) * spc + e
                 for lane in range(LANES):
-                    rows[t * LANES + lane] = (g % 4) * 32 + lane
-                    cols[t * LANES + lane] = u * 2 * spc + (g // 4) * spc + e
+                    rows[t * LANES + lane] = (g % rb) * 32 + lane
+                    cols[t * LANES + lane] = u * 2 * spc + (g // rb) * spc + e
     return rows, cols
 
 
@@ -133,8 +137,8 @@ class Header:
         return Header(*v[2:15], *v[16:23])
 
 
-def raw_tile_bytes(tile_k: int, flags: int) -> int:
-    n = TILE_N * tile_k
+def raw_tile_bytes(tile_k: int, flags: int, tile_n: int = TILE_N) -> int:
+    n = tile_n * tile_k
     return n - 64 if flags & FLAG_STATE_PAYLOAD else n
 
 
@@ -172,7 +176,7 @@ def _raw_tile_unpack(plane: np.ndarray, steps: int, flags: int, payload):
 
 def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
            scales: np.ndarray | None = None, zeros: np.ndarray | None = None,
-           group_size: int = 0, w_scale: float = 1.0):
+           group_size: int = 0, w_scale: float = 1.0, tile_n: int = TILE_N):
     """Compress one weight matrix.  Returns (container bytes as np.uint8 array, stats dict).
 
     w: bf16 -> uint16 [n_out x k_in]; fp8/int8 -> (u)int8 [n_out x k_in]; int4 -> uint8 [n_out x k_in/2].
@@ -181,13 +185,14 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     tile_k = tile_k or DEFAULT_TILE_K[fmt]
     coded, raw = symbolise(fmt, w)
     n_out = coded.shape[0]
-    assert n_out % TILE_N == 0 and k_in % tile_k == 0
+    assert n_out % STRIPE_N == 0 and k_in % tile_k == 0 and tile_n in (32, 128)
     if flags & FLAG_STATE_PAYLOAD:
         assert fmt == FMT_BF16, "state payload carries raw-plane bytes: bf16 only"
     wps = WEIGHTS_PER_SYMBOL[fmt]
     sym_cols = tile_k // wps
     KT = k_in // tile_k
-    n_tiles = (n_out // TILE_N) * KT
+    Q = STRIPE_N // tile_n                       # tiles per (stripe, k-tile) group; tile index = (stripe*KT + kt)*Q + q
+    n_tiles = (n_out // STRIPE_N) * KT * Q
     L = 1 << STATE_LO_LOG2
 
     # P:l.167 "aggregate the weight statistics across the entire layer to construct a shared codebook"
@@ -197,28 +202,30 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     X = codec.cross_entropy(cnt, f, PROB_BITS)
     tab = codec.Table(f, PROB_BITS)
 
-    rows, cols = tile_order(fmt, tile_k)
+    rows, cols = tile_order(fmt, tile_k, tile_n)
     steps = rows.size // LANES
     records, raws, offsets = [], [], [0]
     state_bits = payload_bits = pad_bits = 0
-    for stripe in range(n_out // TILE_N):
+    for stripe in range(n_out // STRIPE_N):
         for kt in range(KT):
-            blk = coded[stripe * TILE_N:(stripe + 1) * TILE_N, kt * sym_cols:(kt + 1) * sym_cols]
-            sym = blk[rows, cols]
-            x_init = np.full(LANES, L, dtype=np.uint64)
-            if raw is not None:
-                rblk = raw[stripe * TILE_N:(stripe + 1) * TILE_N, kt * sym_cols:(kt + 1) * sym_cols]
-                plane, payload = _raw_tile_pack(rblk[rows, cols].reshape(steps, LANES), flags)
-                raws.append(plane)
-                x_init = x_init + payload
-            states, words = codec.tile_encode(sym, LANES, tab, WORD_BITS, STATE_LO_LOG2, x_init)
-            rec = states.astype("<u4").tobytes() + words.astype("<u2").tobytes()
-            pad = _align(len(rec)) - len(rec)
-            records.append(rec + b"\0" * pad)
-            offsets.append(offsets[-1] + (len(rec) + pad) // 16)
-            state_bits += 32 * LANES
-            payload_bits += 16 * words.size
-            pad_bits += 8 * pad
+            for q in range(Q):
+                r0 = stripe * STRIPE_N + q * tile_n
+                blk = coded[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols]
+                sym = blk[rows, cols]
+                x_init = np.full(LANES, L, dtype=np.uint64)
+                if raw is not None:
+                    rblk = raw[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols]
+                    plane, payload = _raw_tile_pack(rblk[rows, cols].reshape(steps, LANES), flags)
+                    raws.append(plane)
+                    x_init = x_init + payload
+                states, words = codec.tile_encode(sym, LANES, tab, WORD_BITS, STATE_LO_LOG2, x_init)
+                rec = states.astype("<u4").tobytes() + words.astype("<u2").tobytes()
+                pad = _align(len(rec)) - len(rec)
+                records.append(rec + b"\0" * pad)
+                offsets.append(offsets[-1] + (len(rec) + pad) // 16)
+                state_bits += 32 * LANES
+                payload_bits += 16 * words.size
+                pad_bits += 8 * pad
 
     rec_bytes = b"".join(records)
     raw_bytes = np.concatenate(raws).tobytes() if raws else b""
@@ -238,7 +245,7 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     off_scales = _align(off_raw + len(raw_bytes))
     total = _align(off_scales + len(side))
     total = max(total, _align(off_records + len(rec_bytes) + TAIL_BYTES))   # tail rule
-    hdr = Header(fmt, n_out, k_in, TILE_N, tile_k, LANES, PROB_BITS, WORD_BITS, STATE_LO_LOG2, group_size, flags,
+    hdr = Header(fmt, n_out, k_in, tile_n, tile_k, LANES, PROB_BITS, WORD_BITS, STATE_LO_LOG2, group_size, flags,
                  n_tiles, float(w_scale), off_freq, off_offsets, off_records, off_raw if raw_bytes else 0,
                  off_scales if side else 0, 0, total)
     buf = np.zeros(total, dtype=np.uint8)
@@ -269,23 +276,27 @@ def decode(buf: np.ndarray):
     caller's original dtype/packing (bf16 -> uint16 bit patterns)."""
     buf = np.ascontiguousarray(buf, dtype=np.uint8)
     h = Header.unpack(buf)
-    fmt, tile_k = h.fmt, h.tile_k
+    fmt, tile_k, tile_n = h.fmt, h.tile_k, h.tile_n
+    if tile_n not in (32, 128):
+        raise ValueError("unsupported tile_n %d" % tile_n)
+    Q = STRIPE_N // tile_n
     wps = WEIGHTS_PER_SYMBOL[fmt]
     sym_cols = tile_k // wps
     KT = h.k_in // tile_k
     f = np.frombuffer(buf[h.off_freq:h.off_freq + 512].tobytes(), dtype="<u2").astype(np.uint32)
     tab = codec.Table(f, h.prob_bits)
     offsets = np.frombuffer(buf[h.off_offsets:h.off_offsets + 4 * (h.n_tiles + 1)].tobytes(), dtype="<u4").astype(np.int64)
-    rows, cols = tile_order(fmt, tile_k)
+    rows, cols = tile_order(fmt, tile_k, tile_n)
     n_sym = rows.size
     steps = n_sym // LANES
     L = 1 << h.state_lo_log2
     coded = np.zeros((h.n_out, h.k_in // wps), dtype=np.uint8)
     raw = np.zeros_like(coded) if fmt == FMT_BF16 else None
-    rtb = raw_tile_bytes(tile_k, h.flags)
+    rtb = raw_tile_bytes(tile_k, h.flags, tile_n)
     t = 0
-    for stripe in range(h.n_out // TILE_N):
-        for kt in range(KT):
+    for stripe in range(h.n_out // STRIPE_N):
+        for kt, q in ((kt, q) for kt in range(KT) for q in range(Q)):
+            r0 = stripe * STRIPE_N + q * tile_n
             a = h.off_records + 16 * int(offsets[t])
             e = h.off_records + 16 * int(offsets[t + 1])
             states = np.frombuffer(buf[a:a + 4 * LANES].tobytes(), dtype="<u4").astype(np.uint64)
@@ -299,15 +310,15 @@ def decode(buf: np.ndarray):
                 raise ValueError("corrupt tile %d: end state != L" % t)
             if (e - a - 4 * LANES) // 2 - used not in range(0, 8):
                 raise ValueError("corrupt tile %d: %d words stored, %d used" % (t, (e - a - 128) // 2, used))
-            blk = np.zeros((TILE_N, sym_cols), dtype=np.uint8)
+            blk = np.zeros((tile_n, sym_cols), dtype=np.uint8)
             blk[rows, cols] = sym
-            coded[stripe * TILE_N:(stripe + 1) * TILE_N, kt * sym_cols:(kt + 1) * sym_cols] = blk
+            coded[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols] = blk
             if raw is not None:
                 plane = buf[h.off_raw + t * rtb:h.off_raw + (t + 1) * rtb]
                 rl = _raw_tile_unpack(plane, steps, h.flags, payload)
-                rblk = np.zeros((TILE_N, sym_cols), dtype=np.uint8)
+                rblk = np.zeros((tile_n, sym_cols), dtype=np.uint8)
                 rblk[rows, cols] = rl.reshape(-1)
-                raw[stripe * TILE_N:(stripe + 1) * TILE_N, kt * sym_cols:(kt + 1) * sym_cols] = rblk
+                raw[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols] = rblk
             t += 1
     w = desymbolise(fmt, coded, raw)
     side = {}

@@ -31,7 +31,7 @@ class AnslinError(RuntimeError):
 class Desc(ctypes.Structure):
     _fields_ = [("format", ctypes.c_uint32), ("n_out", ctypes.c_uint32), ("k_in", ctypes.c_uint32),
                 ("tile_k", ctypes.c_uint32), ("group_size", ctypes.c_uint32), ("flags", ctypes.c_uint32),
-                ("w_scale", ctypes.c_float), ("reserved", ctypes.c_uint32)]
+                ("w_scale", ctypes.c_float), ("tile_n", ctypes.c_uint32)]
 
 
 class Stats(ctypes.Structure):
@@ -82,9 +82,9 @@ def _hp(a):
 
 def anslin_encode_host(fmt: int, w: np.ndarray, n_out: int, k_in: int, tile_k: int = 0, flags: int = 0,
                        scales: np.ndarray | None = None, zeros: np.ndarray | None = None, group_size: int = 0,
-                       w_scale: float = 1.0):
+                       w_scale: float = 1.0, tile_n: int = 0):
     """Returns (container as np.uint8 array, stats dict)."""
-    d = Desc(fmt, n_out, k_in, tile_k, group_size, flags, w_scale, 0)
+    d = Desc(fmt, n_out, k_in, tile_k, group_size, flags, w_scale, tile_n)
     cap = lib().anslin_encode_bound(ctypes.byref(d))
     if cap == 0:
         raise AnslinError("anslin_encode_bound: unsupported shape or format")

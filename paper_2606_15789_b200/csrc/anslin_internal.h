@@ -15,7 +15,7 @@ namespace anslin {
 
 constexpr uint32_t kMagic = 0x4C534E41u;  // "ANSL"
 constexpr uint32_t kVersion = 1;
-constexpr int kTileN = 128;      // weight rows per tile = tcgen05 MMA M
+constexpr int kTileN = 128;      // weight rows per stripe = tcgen05 MMA M; a stripe is cut into tiles of tile_n = 128 or 32 rows
 constexpr int kLanes = 32;       // interleaved rANS streams per tile (P:l.192)
 constexpr int kProbBits = 12;    // b (P:l.442)
 constexpr int kWordBits = 16;    // w
@@ -46,8 +46,8 @@ ANSLIN_HD constexpr int unit_k_of(uint32_t fmt) {
 }
 constexpr uint32_t default_tile_k(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 ? 64 : 256; }
 // bytes per stored weight element of row-major W (int4: half a byte -> handled by callers)
-ANSLIN_HD constexpr size_t raw_tile_bytes(uint32_t tile_k, uint32_t flags) {
-  return size_t(kTileN) * tile_k - ((flags & ANSLIN_FLAG_STATE_PAYLOAD) ? 64 : 0);
+ANSLIN_HD constexpr size_t raw_tile_bytes(uint32_t tile_n, uint32_t tile_k, uint32_t flags) {
+  return size_t(tile_n) * tile_k - ((flags & ANSLIN_FLAG_STATE_PAYLOAD) ? 64 : 0);
 }
 inline size_t align16(size_t x) { return (x + 15) & ~size_t(15); }
 

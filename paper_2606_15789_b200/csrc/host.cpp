@@ -18,8 +18,8 @@ using namespace anslin;
 namespace {
 
 struct Geometry {
-  uint32_t fmt, n_out, k_in, tile_k, flags, group;
-  int spc, wps, sym_cols /*symbols per tile row*/, units, steps, KT, stripes;
+  uint32_t fmt, n_out, k_in, tile_n, tile_k, flags, group;
+  int spc, wps, sym_cols /*symbols per tile row*/, units, steps, KT, stripes, Q /*tiles per (stripe, k-tile) group*/, rb /*tile_n / 32*/;
   size_t n_tiles, row_syms /*symbols per matrix row*/;
 };
 
@@ -29,6 +29,8 @@ bool make_geometry(const anslin_desc *d, Geometry *g) {
   g->n_out = d->n_out;
   g->k_in = d->k_in;
   g->tile_k = d->tile_k ? d->tile_k : default_tile_k(d->format);
+  g->tile_n = d->tile_n ? d->tile_n : uint32_t(kTileN);
+  if (g->tile_n != 32 && g->tile_n != uint32_t(kTileN)) return false;
   g->flags = d->flags;
   g->group = d->group_size;
   g->spc = spc_of(g->fmt);
@@ -40,10 +42,12 @@ bool make_geometry(const anslin_desc *d, Geometry *g) {
   if (g->fmt == ANSLIN_FMT_INT4_AWQ && (g->group == 0 || g->group % 16 || g->k_in % g->group)) return false;
   g->sym_cols = int(g->tile_k) / g->wps;
   g->units = g->sym_cols / (2 * g->spc);
-  g->steps = g->units * 8 * g->spc;
+  g->rb = int(g->tile_n) / 32;
+  g->Q = kTileN / int(g->tile_n);
+  g->steps = g->units * 2 * g->rb * g->spc;
   g->KT = int(g->k_in / g->tile_k);
   g->stripes = int(g->n_out / kTileN);
-  g->n_tiles = size_t(g->KT) * g->stripes;
+  g->n_tiles = size_t(g->KT) * g->stripes * g->Q;
   g->row_syms = g->k_in / g->wps;
   return true;
 }
@@ -106,18 +110,19 @@ bool normalise(const uint64_t *cnt, uint32_t *f) {
 }
 
 // One tile -> record bytes (32 states + words in decoder read order + pad) and raw plane bytes.
-void encode_tile(const Geometry &g, const void *w, int stripe, int kt, const uint32_t *f, const uint32_t *c,
+void encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *f, const uint32_t *c,
                  std::vector<uint8_t> &rec, uint8_t *raw_out, uint64_t *n_words_out) {
-  const int steps = g.steps, spc = g.spc;
-  const size_t row0 = size_t(stripe) * kTileN, col0 = size_t(kt) * g.sym_cols;
+  const int steps = g.steps, spc = g.spc, G = 2 * g.rb;
+  const size_t grp = tile / g.Q, q = tile % g.Q, stripe = grp / g.KT, kt = grp % g.KT;
+  const size_t row0 = stripe * kTileN + q * g.tile_n, col0 = kt * g.sym_cols;
   std::vector<uint8_t> sym(size_t(steps) * kLanes), raw;
   if (g.fmt == ANSLIN_FMT_BF16) raw.resize(sym.size());
   for (int u = 0; u < g.units; ++u)
-    for (int gq = 0; gq < 8; ++gq)
+    for (int gq = 0; gq < G; ++gq)
       for (int lane = 0; lane < kLanes; ++lane) {
-        size_t row = row0 + size_t((gq & 3) * 32 + lane), col = col0 + size_t(u) * 2 * spc + size_t(gq >> 2) * spc;
+        size_t row = row0 + size_t((gq % g.rb) * 32 + lane), col = col0 + size_t(u) * 2 * spc + size_t(gq / g.rb) * spc;
         for (int e = 0; e < spc; ++e) {
-          size_t t = size_t(u * 8 + gq) * spc + e;
+          size_t t = size_t(u * G + gq) * spc + e;
           sym[t * kLanes + lane] = coded_symbol(g, w, row, col + e);
           if (!raw.empty()) raw[t * kLanes + lane] = raw_byte(g, w, row, col + e);
         }
@@ -174,7 +179,7 @@ size_t anslin_encode_bound(const anslin_desc *desc) {
   // every symbol costs at most 12 bits + one flush word per lane; round generously
   const size_t rec = align16(4 * kLanes + 2 * (tile_syms * 3 / 4 + 2 * kLanes + 8));
   size_t total = kHeaderBytes + 512 + align16(4 * (g.n_tiles + 1)) + g.n_tiles * rec + 64;
-  if (g.fmt == ANSLIN_FMT_BF16) total += g.n_tiles * raw_tile_bytes(g.tile_k, 0) + 16;
+  if (g.fmt == ANSLIN_FMT_BF16) total += g.n_tiles * raw_tile_bytes(g.tile_n, g.tile_k, 0) + 16;
   return total + align16(side_bytes(g)) + 16 + kTailBytes;
 }
 
@@ -216,7 +221,7 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   // Encode tiles in parallel, then lay the records out in tile order.
   std::vector<std::vector<uint8_t>> recs(g.n_tiles);
   std::vector<uint64_t> nwords(g.n_tiles, 0);
-  const size_t rtb = g.fmt == ANSLIN_FMT_BF16 ? raw_tile_bytes(g.tile_k, g.flags) : 0;
+  const size_t rtb = g.fmt == ANSLIN_FMT_BF16 ? raw_tile_bytes(g.tile_n, g.tile_k, g.flags) : 0;
   Header h;
   std::memset(&h, 0, sizeof(h));
   h.off_freq = kHeaderBytes;
@@ -235,8 +240,7 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
         for (;;) {
           size_t t = next.fetch_add(1);
           if (t >= g.n_tiles) break;
-          encode_tile(g, w_host, int(t / g.KT), int(t % g.KT), f, c, recs[t], rtb ? raw_all.data() + t * rtb : nullptr,
-                      &nwords[t]);
+          encode_tile(g, w_host, t, f, c, recs[t], rtb ? raw_all.data() + t * rtb : nullptr, &nwords[t]);
         }
       });
     for (auto &t : th) t.join();
@@ -256,7 +260,7 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   if (rec_total / 16 > 0xFFFFFFFFull) return ANSLIN_ERR_UNSUPPORTED;
 
   h.magic = kMagic; h.version = kVersion; h.format = g.fmt; h.n_out = g.n_out; h.k_in = g.k_in;
-  h.tile_n = kTileN; h.tile_k = g.tile_k; h.streams = kLanes; h.prob_bits = kProbBits; h.word_bits = kWordBits;
+  h.tile_n = g.tile_n; h.tile_k = g.tile_k; h.streams = kLanes; h.prob_bits = kProbBits; h.word_bits = kWordBits;
   h.state_lo_log2 = kStateLoLog2; h.group_size = g.group; h.flags = g.flags; h.n_tiles = uint32_t(g.n_tiles);
   h.w_scale = g.fmt == ANSLIN_FMT_FP8_E4M3 ? desc->w_scale : 1.0f;
 
@@ -326,10 +330,10 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   Header h;
   std::memcpy(&h, container_host, sizeof(h));
   if (h.magic != kMagic || h.version != kVersion) return ANSLIN_ERR_CORRUPT;
-  anslin_desc d{h.format, h.n_out, h.k_in, h.tile_k, h.group_size, h.flags, h.w_scale, 0};
+  anslin_desc d{h.format, h.n_out, h.k_in, h.tile_k, h.group_size, h.flags, h.w_scale, h.tile_n};
   Geometry g;
   if (h.format > ANSLIN_FMT_INT4_AWQ || !make_geometry(&d, &g)) return ANSLIN_ERR_CORRUPT;
-  if (h.tile_n != kTileN || h.streams != kLanes || h.prob_bits != kProbBits || h.word_bits != kWordBits ||
+  if (h.tile_n != g.tile_n || h.streams != kLanes || h.prob_bits != kProbBits || h.word_bits != kWordBits ||
       h.state_lo_log2 != kStateLoLog2 || h.n_tiles != g.n_tiles)
     return ANSLIN_ERR_CORRUPT;
   const uint64_t T = h.total_bytes;
@@ -355,7 +359,7 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
     if (offs[t + 1] < offs[t] + 8 || offs[t + 1] > rec_units) return ANSLIN_ERR_CORRUPT;
     if (uint64_t(offs[t + 1] - offs[t]) * 16 > 128 + uint64_t(g.steps) * kLanes * 2 + 16) return ANSLIN_ERR_CORRUPT;
   }
-  if (g.fmt == ANSLIN_FMT_BF16 && !in(h.off_raw, raw_tile_bytes(g.tile_k, g.flags) * g.n_tiles)) return ANSLIN_ERR_CORRUPT;
+  if (g.fmt == ANSLIN_FMT_BF16 && !in(h.off_raw, raw_tile_bytes(g.tile_n, g.tile_k, g.flags) * g.n_tiles)) return ANSLIN_ERR_CORRUPT;
   if (side_bytes(g) && !in(h.off_scales, side_bytes(g))) return ANSLIN_ERR_CORRUPT;
   anslin_weight *w = new (std::nothrow) anslin_weight;
   if (!w) return ANSLIN_ERR_INVALID_ARG;
@@ -372,7 +376,7 @@ int anslin_close(anslin_weight *w) {
 
 int anslin_describe(const anslin_weight *w, anslin_desc *out) {
   if (!w || !out) return ANSLIN_ERR_INVALID_ARG;
-  *out = anslin_desc{w->h.format, w->h.n_out, w->h.k_in, w->h.tile_k, w->h.group_size, w->h.flags, w->h.w_scale, 0};
+  *out = anslin_desc{w->h.format, w->h.n_out, w->h.k_in, w->h.tile_k, w->h.group_size, w->h.flags, w->h.w_scale, w->h.tile_n};
   return ANSLIN_OK;
 }
 

@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(kDecWarps * 32) decode_kernel(ContainerView cv
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
   const size_t row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.k_in) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.k_in) / 2 : size_t(cv.k_in);
   const size_t tile_row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.tile_k) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.tile_k) / 2 : size_t(cv.tile_k);
-  const size_t rtb = raw_tile_bytes(cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
+  const size_t rtb = raw_tile_bytes(kTileN, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
   for (uint32_t t = blockIdx.x * kDecWarps + warp; t < cv.n_tiles; t += gridDim.x * kDecWarps) {
     WarpStream s;
     stream_open(s, cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s, lane);
@@ -408,7 +408,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     if (d < p.D) {
       const uint32_t lt = lanemask_lt(), ring_s = smem0 + ring_off + d * kRingBytes;
       const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
-      const size_t rtb = raw_tile_bytes(cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
+      const size_t rtb = raw_tile_bytes(kTileN, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
       const uint32_t xbytes = p.mpad * 32u;
       // Tiles of this CTA are dealt to the decoder warps round-robin over the CTA's WHOLE range
       // (tile i -> warp i mod D, round i div D).  The MMA warp consumes units segment by segment
@@ -698,13 +698,15 @@ int gemm_one(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_
   p.ldy = ldy;
   const char *lay = getenv("ANSLIN_LAYOUT");  // debug: "none" selects the unswizzled core-matrix layout
   p.layout = (lay && lay[0] == 'n') ? kLayoutNone : kLayoutSW32;
-  const uint32_t grid = grid_of(h.n_tiles, 12), stripes = h.n_out / kTileN;
+  uint32_t min_tiles = 12;
+  if (const char *e = getenv("ANSLIN_MIN_TILES")) min_tiles = uint32_t(std::max(1, atoi(e)));
+  const uint32_t grid = grid_of(h.n_tiles, min_tiles), stripes = h.n_out / kTileN;
   // ring sizing: D decoder warps (1 KiB compressed-word ring each) and U operand slots
   const size_t fixed = 2048 /*align slack*/ + 2048 /*ring alignment*/ + 16384 + 1056 + 16 * kMaxSlots + 64 + 4 * kMaxSlots;
   uint32_t D = kMaxDecWarps, U = 0;
   const char *denv = getenv("ANSLIN_DECODER_WARPS");
   if (denv && atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
-  {  // even rounds: a CTA with tpc tiles needs ceil(tpc/D) tile-times; use the fewest warps that keep that count
+  if (!getenv("ANSLIN_DMAX")) {  // even rounds: a CTA with tpc tiles needs ceil(tpc/D) tile-times; use the fewest warps that keep that count
     const uint32_t tpc = (h.n_tiles + grid - 1) / grid, rounds = (tpc + D - 1) / D;
     D = std::max(1u, (tpc + rounds - 1) / rounds);
   }

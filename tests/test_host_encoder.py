@@ -36,12 +36,17 @@ def _cases():
     yield "bf16", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=64)
     yield "bf16-payload", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=64, flags=1)
     yield "bf16-tile128", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=128, flags=1)
+    yield "bf16-32x256", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=256, flags=1, tile_n=32)
+    yield "bf16-32x64", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=64, tile_n=32)
     q8, s8 = inputs.quant_sq8_weights(wf)
     yield "int8", oc.FMT_INT8, q8, 512, dict(tile_k=256, scales=s8)
     f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(128, 512, seed=32, std=0.015, outliers=False))
     yield "fp8", oc.FMT_FP8_E4M3, f8, 512, dict(tile_k=128, w_scale=sc)
     p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(128, 512, seed=33, outliers=False), 128)
     yield "int4", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=256, scales=s4, zeros=z4, group_size=128)
+    yield "int8-32x256", oc.FMT_INT8, q8, 512, dict(tile_k=256, scales=s8, tile_n=32)
+    yield "fp8-32x512", oc.FMT_FP8_E4M3, f8, 512, dict(tile_k=512, w_scale=sc, tile_n=32)
+    yield "int4-32x512", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=512, scales=s4, zeros=z4, group_size=128, tile_n=32)
 
 
 @pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_cases()), ids=[c[0] for c in _cases()])
@@ -58,7 +63,8 @@ def test_cross_decode_and_stats(name, fmt, w, k_in, kw):
     # the library accepts the oracle's container (header-only open; no device pointer)
     obuf, ost = oc.encode(fmt, w, k_in, **kw)
     hw = B.Weight(obuf, None)
-    assert (hw.desc.n_out, hw.desc.k_in, hw.desc.tile_k, hw.desc.flags) == (n_out, k_in, kw["tile_k"], kw.get("flags", 0))
+    assert (hw.desc.n_out, hw.desc.k_in, hw.desc.tile_k, hw.desc.flags, hw.desc.tile_n) == \
+        (n_out, k_in, kw["tile_k"], kw.get("flags", 0), kw.get("tile_n", 128))
     hw.close()
     B.Weight(buf, None).close()
     # both encoders are legal rANS coders over (possibly different) legal tables: sizes agree closely

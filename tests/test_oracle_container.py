@@ -37,11 +37,16 @@ def test_symbolise_bf16_is_a_bijection_on_all_65536_codes():
     assert np.array_equal(raw & 1, (bits >> 15).astype(np.uint8))
 
 
-@pytest.mark.parametrize("fmt,tile_k", [(oc.FMT_BF16, 64), (oc.FMT_FP8_E4M3, 256), (oc.FMT_INT8, 128), (oc.FMT_INT4_AWQ, 256)])
-def test_tile_order_is_a_permutation_with_chunk_structure(fmt, tile_k):
-    rows, cols = oc.tile_order(fmt, tile_k)
+@pytest.mark.parametrize("fmt,tile_k,tile_n", [(oc.FMT_BF16, 64, 128), (oc.FMT_FP8_E4M3, 256, 128), (oc.FMT_INT8, 128, 128),
+                                               (oc.FMT_INT4_AWQ, 256, 128), (oc.FMT_BF16, 256, 32), (oc.FMT_INT8, 256, 32),
+                                               (oc.FMT_INT4_AWQ, 512, 32)])
+def test_tile_order_is_a_permutation_with_chunk_structure(fmt, tile_k, tile_n):
+    rows, cols = oc.tile_order(fmt, tile_k, tile_n)
     sym_cols = tile_k // oc.WEIGHTS_PER_SYMBOL[fmt]
-    assert rows.size == 128 * sym_cols
+    assert rows.size == tile_n * sym_cols
+    if tile_n == 32:      # lane l simply walks row l in K order
+        assert np.array_equal(rows.reshape(-1, 32), np.tile(np.arange(32), (sym_cols, 1)))
+        assert np.array_equal(cols.reshape(-1, 32), np.tile(np.arange(sym_cols)[:, None], (1, 32)))
     assert np.unique(rows * sym_cols + cols).size == rows.size
     spc = oc.SPC[fmt]
     # a lane's spc consecutive steps are spc consecutive symbol columns of one row = one 16-byte operand chunk
