@@ -16,7 +16,7 @@
  *   - kernels are enqueued on the caller's stream and run asynchronously; asynchronous faults
  *     surface at the caller's next synchronisation.  No hidden synchronisation.
  *   - device pointers must be 16-byte aligned (else ANSLIN_ERR_INVALID_ARG).
- *   - shapes: n_out % 128 == 0 and k_in % tile_k == 0 (else ANSLIN_ERR_UNSUPPORTED); m >= 1.
+ *   - shapes: n_out % 128 == 0 and k_in % tile_k == 0 (else ANSLIN_ERR_UNSUPPORTED); 1 <= m <= 256.
  *   - orientation: W is [n_out x k_in] row-major (torch Linear.weight), X is [m x k_in] row-major
  *     with leading dimension ldx (elements), Y is [m x n_out] row-major float32 with ldy.
  *   - there is no CPU fallback: the device entry points fail with ANSLIN_ERR_CUDA when no sm_100
@@ -130,6 +130,8 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
 
 /* Scratch bytes anslin_gemm needs for batch m (split-K partials + counters). */
 size_t anslin_gemm_workspace_bytes(const anslin_weight *w, int32_t m);
+/* Scratch bytes anslin_gemm_multi / anslin_gemm_grouped need for these n weights at batch sizes <= m_max. */
+size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, int32_t n, int32_t m_max);
 
 /*
  * Fused decode + GEMM, Y = X . W^T (Alg V.1): only compressed bytes of W cross HBM.
@@ -143,9 +145,24 @@ int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int
                 size_t workspace_bytes, void *stream);
 
 /*
+ * n independent fused decode-GEMMs in ONE persistent launch (projections that share an input, e.g.
+ * q/k/v or gate/up; the building block of anslin_gemm_grouped): Y_i = X_i . W_i^T.  The SMs are shared
+ * out in proportion to n_out*k_in of each problem.  All weights must have the same format, tile_n and
+ * state-payload flag; shapes, tile_k and batch sizes may differ.  Arrays are host arrays of n entries
+ * (device pointers inside); x_scale_dev may be NULL for bf16 / int4.  More than 8 problems are issued
+ * as consecutive launches on the same stream.  Workspace: anslin_gemm_multi_workspace_bytes.
+ */
+int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void *const *x_dev,
+                      uint32_t x_dtype, const int64_t *ldx, const int32_t *m,
+                      const void *const *x_scale_dev, void *const *y_dev, const int64_t *ldy,
+                      void *workspace_dev, size_t workspace_bytes, void *stream);
+
+/*
  * Grouped fused decode-GEMM over MoE experts (BASELINE config 5): rows of X already sorted by
  * expert and contiguous; expert e owns rows_per_expert_host[e] rows (0 = inactive, skipped).
- * All experts share one shape/format.  Y rows are in the same order as X rows.
+ * All experts share one shape/format.  Y rows are in the same order as X rows.  The active experts
+ * run as the problems of one persistent launch (a12; table residency per CTA, one expert per CTA).
+ * Workspace: anslin_gemm_multi_workspace_bytes(experts, n_experts, max rows of one expert).
  */
 int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts,
                         const int32_t *rows_per_expert_host, const void *x_dev, uint32_t x_dtype,

@@ -20,7 +20,8 @@ FLAG_STATE_PAYLOAD = 1
 X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_INT4_AWQ: DT_F16}
 
 EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_close", "anslin_describe",
-           "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm", "anslin_gemm_grouped",
+           "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm_multi_workspace_bytes", "anslin_gemm",
+           "anslin_gemm_multi", "anslin_gemm_grouped",
            "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_last_launch_count", "anslin_status_string"]
 
 
@@ -62,6 +63,10 @@ def lib() -> ctypes.CDLL:
         L.anslin_decode.argtypes = [vp, vp, sz, vp]
         L.anslin_gemm_workspace_bytes.argtypes = [vp, i32]; L.anslin_gemm_workspace_bytes.restype = sz
         L.anslin_gemm.argtypes = [vp, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
+        L.anslin_gemm_multi_workspace_bytes.argtypes = [ctypes.POINTER(vp), i32, i32]
+        L.anslin_gemm_multi_workspace_bytes.restype = sz
+        L.anslin_gemm_multi.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(vp), u32, ctypes.POINTER(i64), ctypes.POINTER(i32),
+                                        ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64), vp, sz, vp]
         L.anslin_gemm_grouped.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(i32), vp, u32, i64, vp, vp, i64, vp, sz, vp]
         L.anslin_dense_workspace_bytes.argtypes = [u32, u32, i32]; L.anslin_dense_workspace_bytes.restype = sz
         L.anslin_dense_gemm.argtypes = [u32, vp, u32, u32, vp, ctypes.c_float, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
@@ -139,6 +144,36 @@ def anslin_gemm(w: Weight, x_ptr: int, x_dtype: int, ldx: int, m: int, x_scale_p
                 ws_ptr: int, ws_bytes: int, stream: int = 0):
     _check(lib().anslin_gemm(w.handle, ctypes.c_void_p(x_ptr), x_dtype, ldx, m, ctypes.c_void_p(x_scale_ptr or 0),
                              ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.c_void_p(stream)), "anslin_gemm")
+
+
+def anslin_gemm_multi_workspace_bytes(weights, m_max: int) -> int:
+    n = len(weights)
+    arr = (ctypes.c_void_p * n)(*[w.handle for w in weights])
+    return int(lib().anslin_gemm_multi_workspace_bytes(arr, n, int(m_max)))
+
+
+class MultiCall:
+    """Marshalled argument arrays of one anslin_gemm_multi call (built once, reusable every step)."""
+
+    def __init__(self, weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes):
+        n = self.n = len(weights)
+        vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
+        self.w = (vp * n)(*[w.handle for w in weights])
+        self.x = (vp * n)(*[int(p) for p in x_ptrs])
+        self.ldx = (i64 * n)(*[int(v) for v in ldxs])
+        self.m = (i32 * n)(*[int(v) for v in ms])
+        self.xs = None if x_scale_ptrs is None else (vp * n)(*[int(p or 0) for p in x_scale_ptrs])
+        self.y = (vp * n)(*[int(p) for p in y_ptrs])
+        self.ldy = (i64 * n)(*[int(v) for v in ldys])
+        self.x_dtype, self.ws_ptr, self.ws_bytes = x_dtype, ctypes.c_void_p(ws_ptr), ws_bytes
+
+    def __call__(self, stream: int = 0):
+        _check(lib().anslin_gemm_multi(self.w, self.n, self.x, self.x_dtype, self.ldx, self.m, self.xs, self.y, self.ldy,
+                                       self.ws_ptr, self.ws_bytes, ctypes.c_void_p(stream)), "anslin_gemm_multi")
+
+
+def anslin_gemm_multi(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes, stream: int = 0):
+    MultiCall(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes)(stream)
 
 
 def anslin_gemm_grouped(experts, rows_per_expert, x_ptr: int, x_dtype: int, ldx: int, x_scale_ptr: int | None, y_ptr: int,

@@ -1,13 +1,18 @@
 // Warp-cooperative rANS tile decoder (Alg V.2, P:l.260-287), sm_100a.
 //
-// One warp decodes one tile: lane l owns stream l (P:l.192 "each warp lane maintains its own rANS
-// state").  Per step and lane:  slot = x & 4095;  e = T[slot] (shared-memory table, P:l.271);
-// x = f*(x>>12) + bias;  if x < 2^16: x = x<<16 | next word.  The words of a tile are interleaved
-// in decoder read order, so the renormalising lanes of a step read CONSECUTIVE 16-bit words
-// (P:l.256 "renormalization loads are naturally coalesced"): ballot + popc prefix picks the word.
-// The compressed words are streamed HBM -> shared memory through a per-warp 2 KiB ring with
-// 16-byte cp.async (32 lanes x 16 B = 512 B per fill, 1.5-2 KiB of look-ahead); the ring
-// bookkeeping runs once per EIGHT decode steps.
+// One warp lane owns one of the 32 interleaved streams of a tile (P:l.192 "each warp lane maintains
+// its own rANS state").  Per step and lane:  slot = x & 4095;  e = T[slot] (shared-memory table,
+// P:l.271);  x = f*(x>>12) + bias;  if x < 2^16: x = x<<16 | next word.  The words of a tile are
+// interleaved in decoder read order, so the renormalising lanes of a step read CONSECUTIVE 16-bit
+// words (P:l.256 "renormalization loads are naturally coalesced"): ballot + popc prefix picks the word.
+//
+// A decode step is a ~140-cycle dependent chain (LDS table -> IMAD -> vote -> popc -> LDS word), so
+// throughput comes from independent chains in flight: a warp decodes J tiles at once, their steps
+// interleaved instruction by instruction (J = 2 for 32-row tiles), and many such warps share an SM.
+//
+// The compressed words stream HBM -> shared memory through a 2 KiB ring per stream (+ a 512-byte
+// mirror of its first block, so that the 8 steps between two upkeeps address the ring linearly)
+// with 16-byte cp.async: 32 lanes x 16 B = one 512-byte block per fill.
 //
 // Table entry (4 B, Eq.3's "2^b x 4 B", P:l.440):  sym[7:0] | f[19:8] | bias[31:20].
 #pragma once
@@ -17,8 +22,10 @@
 
 namespace anslin {
 
-constexpr uint32_t kRingBytes = 2048;  // per decoder warp; the ring must be 2 KiB aligned
-constexpr uint32_t kFillBytes = 512;   // 32 lanes x 16 B per fill
+constexpr uint32_t kRingBytes = 2048;    // per stream
+constexpr uint32_t kFillBytes = 512;     // 32 lanes x 16 B per fill
+constexpr uint32_t kMirrorBytes = 512;   // copy of ring block 0 behind the ring
+constexpr uint32_t kStreamSmem = kRingBytes + kMirrorBytes;
 // The ring reads ahead of the record it decodes: the container guarantees this many readable bytes
 // after the records section (tail rule), so fills need no bounds check.
 static_assert(2 * kRingBytes <= uint32_t(kTailBytes), "ring read-ahead must fit the container tail rule");
@@ -29,31 +36,18 @@ __device__ __forceinline__ uint32_t lanemask_lt() {
   asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
   return m;
 }
-__device__ __forceinline__ uint32_t lds16(uint32_t a) {
-  uint16_t v;
-  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
-  return v;
-}
 __device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
-// 16-byte cp.async, executed only when `on` != 0; copies src_bytes (16 or 0 = zero fill) bytes.
-__device__ __forceinline__ void cp_async16_if(uint32_t on, uint32_t dst, const void *src, uint32_t src_bytes) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p cp.async.cg.shared.global [%1], [%2], 16, %3;\n\t}" ::"r"(on), "r"(dst),
-      "l"(src), "r"(src_bytes)
-      : "memory");
-}
-__device__ __forceinline__ void cp_async_commit_if(uint32_t on) {
-  asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %0, 0;\n\t@p cp.async.commit_group;\n\t}" ::"r"(on) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
-__device__ __forceinline__ uint32_t lds32(uint32_t a) {
+__device__ __forceinline__ uint32_t lds32v(uint32_t a) {
   uint32_t v;
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+  asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
   return v;
 }
+__device__ __forceinline__ void sts32(uint32_t a, uint32_t v) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_1() { asm volatile("cp.async.wait_group 1;" ::: "memory"); }
 __device__ __forceinline__ uint4 ldg128_stream(const void *p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
@@ -61,6 +55,7 @@ __device__ __forceinline__ uint4 ldg128_stream(const void *p) {
                : "l"(p));
   return r;
 }
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // Expand the 256 x u16 frequency table of the container into the 4096-entry slot table in shared
 // memory (Alg V.1 l.6 "Copy global decode table T into shared memory", P:l.212).  All threads of
@@ -90,57 +85,91 @@ __device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, c
   __syncthreads();
 }
 
-// Per-warp stream state over one tile record.
-struct WarpStream {
-  uint32_t x;       // this lane's rANS state
-  uint32_t posb;    // BYTES of words consumed so far (warp uniform)
-  uint32_t filled;  // bytes of words whose ring fill has been issued (warp uniform, multiple of 512)
-  uint32_t ring;    // shared-space address of this warp's 2 KiB-aligned ring
-  const uint8_t *src;  // this lane's next fill source = words + filled + 16*lane
+// One lane's view of one tile's compressed stream.
+struct Stream {
+  uint32_t x;      // this lane's rANS state
+  uint32_t pa;     // shared address of the next unread word (warp uniform; may run into the mirror)
+  uint32_t bal;    // (bytes whose fill has been issued minus bytes consumed) + pa, as of the last upkeep
+  uint32_t fa;     // shared address of this lane's 16-byte slice of the next fill block
+  const uint8_t *src;  // this lane's next fill source = words + issued + 16*lane
 };
 
-// Issue the next 512-byte ring fill iff `on` (every lane copies 16 B).
-__device__ __forceinline__ void stream_fill_if(WarpStream &s, uint32_t on, int lane) {
-  cp_async16_if(on, s.ring | ((s.filled + (uint32_t(lane) << 4)) & (kRingBytes - 1)), s.src, 16u);
-  cp_async_commit_if(on);
-  s.filled += on ? kFillBytes : 0u;
-  s.src += on ? kFillBytes : 0u;
-}
-
-// rec = start of the tile record in HBM (16-byte aligned).
-__device__ __forceinline__ void stream_open(WarpStream &s, const uint8_t *rec, uint32_t ring, int lane) {
-  cp_async_wait_all();  // fills of the previous tile may still be in flight into this ring
-  __syncwarp();
+// rec = start of the tile record in HBM (16-byte aligned); ring = shared address of kStreamSmem bytes.
+// The caller must have drained earlier cp.async groups into this ring (stream_drain) first.
+__device__ __forceinline__ void stream_open(Stream &s, const uint8_t *rec, uint32_t ring, int lane) {
   s.x = reinterpret_cast<const uint32_t *>(rec)[lane];
-  s.src = rec + 4 * kLanes + 16 * lane;
-  s.posb = 0; s.filled = 0; s.ring = ring;
+  const uint8_t *src = rec + 4 * kLanes + 16 * lane;
+  const uint32_t fa = ring + 16u * uint32_t(lane);
 #pragma unroll
-  for (int i = 0; i < 4; ++i) stream_fill_if(s, 1u, lane);
+  for (uint32_t b = 0; b < 3; ++b)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(fa + b * kFillBytes), "l"(src + b * kFillBytes) : "memory");
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(fa + kRingBytes), "l"(src) : "memory");  // mirror of block 0
+  cp_async_commit();
+  s.src = src + 3 * kFillBytes;
+  s.fa = fa + 3 * kFillBytes;
+  s.pa = ring;
+  s.bal = 3 * kFillBytes + ring;
+}
+__device__ __forceinline__ void stream_drain() {
+  cp_async_wait_all();
+  __syncwarp();
 }
 
-// Ring upkeep for the next EIGHT decode steps (they consume at most 512 B): refill the dead quarter
-// behind the read position and make sure everything up to posb + 1024 has landed.  Invariant:
-// 1536 <= filled - posb <= 2048 after the call, at most ONE fill pending => landed >= posb + 1024
-// >= the 512 + 62 bytes eight steps can touch.  A fill writes ring bytes
-// [filled, filled + 512) - 2048 < posb, i.e. only words already consumed.
-__device__ __forceinline__ void stream_upkeep8(WarpStream &s, int lane) {
-  stream_fill_if(s, uint32_t(s.filled - s.posb < 1536u), lane);
+// Ring upkeep of J streams before their next EIGHT decode steps (which consume at most 448 B each:
+// a lane renormalises in at most 7 of 8 steps).  Policy: refill one 512-byte block whenever the
+// issued-but-unread lead has dropped to <= 1024 B.  Invariants on entry: lead >= 641 > 448 and every
+// fill but the one issued by the PREVIOUS upkeep has landed; the single wait_group 1 below (after
+// this upkeep's commit) retires that one, so all `lead` bytes are readable when the steps start.
+// A fill overwrites ring bytes [issued - 2048, issued - 1536) < consumed.  The mirror makes
+// addresses linear for 512 B past the ring end; pa wraps here, once per 8 steps.
+// ring0 = shared address of stream 0's ring; stream j's ring follows at j * kStreamSmem.
+template <int J>
+__device__ __forceinline__ void stream_upkeep8(Stream (&s)[J], uint32_t ring0, int lane) {
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    Stream &t = s[j];
+    const uint32_t lim = ring0 + uint32_t(j) * kStreamSmem + kRingBytes;
+    const uint32_t lead = t.bal - t.pa;
+    if (t.pa >= lim) t.pa -= kRingBytes;
+    t.bal = lead + t.pa;
+    if (lead <= 1024u) {
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(t.fa), "l"(t.src) : "memory");
+      if (t.fa < lim - kRingBytes + kFillBytes)   // block 0 also feeds the mirror
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(t.fa + kRingBytes), "l"(t.src) : "memory");
+      t.fa += kFillBytes;
+      if (t.fa >= lim) t.fa -= kRingBytes;
+      t.src += kFillBytes;
+      t.bal += kFillBytes;
+    }
+  }
+  cp_async_commit();
   cp_async_wait_1();
   __syncwarp();
 }
 
-// One decode step of Alg V.2 for all 32 lanes; returns the table entry (symbol in bits 7:0).
-__device__ __forceinline__ uint32_t decode_step(WarpStream &s, uint32_t tab_s, uint32_t lt) {
-  uint32_t ea;
+// One decode step of Alg V.2 for all 32 lanes of one stream; returns the table entry (symbol in bits 7:0).
+__device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint32_t lt) {
+  uint32_t ea, e;
   asm("mad.lo.u32 %0, %1, 4, %2;" : "=r"(ea) : "r"(s.x & (kM - 1)), "r"(tab_s));
-  const uint32_t e = lds32(ea);
-  const uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
-  const bool need = xn < kL;
-  const uint32_t mask = __ballot_sync(0xffffffffu, need);
-  // every lane loads (the window is resident); only renormalising lanes use the word
-  const uint32_t w = lds16(s.ring | ((s.posb + 2u * __popc(mask & lt)) & (kRingBytes - 1)));
-  s.x = need ? __byte_perm(w, xn, 0x5410) : xn;  // (xn << 16) | w
-  s.posb += 2u * __popc(mask);
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea));
+  uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
+  // renormalisation: the lanes with x < 2^16 read consecutive words, x = (x << 16) | word
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t.reg .u16 h;\n\t.reg .u32 w, m, r, a;\n\t"
+      "setp.lt.u32 p, %0, 65536;\n\t"
+      "vote.sync.ballot.b32 m, p, 0xffffffff;\n\t"
+      "and.b32 r, m, %2;\n\t"
+      "popc.b32 r, r;\n\t"
+      "mad.lo.u32 a, r, 2, %1;\n\t"
+      "@p ld.shared.u16 h, [a];\n\t"
+      "@p cvt.u32.u16 w, h;\n\t"
+      "@p mad.lo.u32 %0, %0, 65536, w;\n\t"
+      "popc.b32 m, m;\n\t"
+      "mad.lo.u32 %1, m, 2, %1;\n\t}"
+      : "+r"(xn), "+r"(s.pa)
+      : "r"(lt)
+      : "memory");
+  s.x = xn;
   return e;
 }
 
@@ -149,17 +178,21 @@ template <int pos>
 __device__ __forceinline__ uint32_t put_sym(uint32_t acc, uint32_t e) {
   return __byte_perm(acc, e, (0x3210 & ~(0xF << (4 * pos))) | (4 << (4 * pos)));
 }
-// Four decode steps -> four symbol bytes.
-__device__ __forceinline__ uint32_t decode4(WarpStream &s, uint32_t tab, uint32_t lt) {
-  uint32_t q = 0;
-  q = put_sym<0>(q, decode_step(s, tab, lt));
-  q = put_sym<1>(q, decode_step(s, tab, lt));
-  q = put_sym<2>(q, decode_step(s, tab, lt));
-  q = put_sym<3>(q, decode_step(s, tab, lt));
-  return q;
+// Four decode steps of each of the J streams, interleaved -> four symbol bytes per stream.
+template <int J>
+__device__ __forceinline__ void decode4(Stream (&s)[J], uint32_t (&q)[J], uint32_t tab, uint32_t lt) {
+#pragma unroll
+  for (int j = 0; j < J; ++j) q[j] = put_sym<0>(0u, decode_step(s[j], tab, lt));
+#pragma unroll
+  for (int j = 0; j < J; ++j) q[j] = put_sym<1>(q[j], decode_step(s[j], tab, lt));
+#pragma unroll
+  for (int j = 0; j < J; ++j) q[j] = put_sym<2>(q[j], decode_step(s[j], tab, lt));
+#pragma unroll
+  for (int j = 0; j < J; ++j) q[j] = put_sym<3>(q[j], decode_step(s[j], tab, lt));
 }
 
-// bf16: merge 4 exponent bytes (E) with 4 raw bytes (R = mantissa<<1 | sign) into 4 bf16 values.
+// bf16: merge 4 exponent bytes (E) with 4 raw bytes (R = mantissa<<1 | sign) into 4 bf16 values:
+// each 16-bit (E<<8 | R) rotated right by one bit.
 __device__ __forceinline__ uint2 bf16_merge4(uint32_t E, uint32_t R) {
   const uint32_t p0 = __byte_perm(R, E, 0x5140), p1 = __byte_perm(R, E, 0x7362);
   uint2 o;
@@ -177,76 +210,108 @@ __device__ __forceinline__ uint32_t awq_dequant2(uint32_t byte, __half2 zoff, __
   return *reinterpret_cast<const uint32_t *>(&h);
 }
 
-// Raw-plane (bf16 sign+mantissa) reader: 16 steps of one lane = one 16-byte vector.
+// Raw-plane (bf16 sign+mantissa) reader of one tile: 16 steps of one lane = one 16-byte vector,
+// fetched one vector ahead into registers, with an L2 prefetch four vectors ahead.
 template <bool kPayload>
 struct RawReader {
-  const uint8_t *tile_raw;
-  int V;  // vectors per tile
-  __device__ __forceinline__ uint4 load(int v, int lane) const {
-    if (!kPayload || v < V - 1) return ldg128_stream(tile_raw + size_t(v) * 512 + lane * 16);
-    // last vector with the state-payload flag: 7 sub-rows of 32 x 2 bytes; bytes 14,15 come from the end state
-    uint32_t h[7];
-#pragma unroll
-    for (int i = 0; i < 7; ++i)
-      h[i] = reinterpret_cast<const uint16_t *>(tile_raw + size_t(v) * 512)[i * 32 + lane];
+  const uint8_t *p;  // this lane's slice of the vector after `next`
+  uint4 next;        // vector v + 1 while vector v is being consumed
+  __device__ __forceinline__ uint4 load(int v, int V, int lane) {
     uint4 r;
-    r.x = h[0] | (h[1] << 16); r.y = h[2] | (h[3] << 16); r.z = h[4] | (h[5] << 16); r.w = h[6];
+    if (!kPayload || v < V - 1) {
+      if (v + 4 < V) prefetch_l2(p + 4 * 512);
+      r = ldg128_stream(p);
+    } else {
+      // last vector with the state-payload flag: 7 sub-rows of 32 x 2 bytes; bytes 14,15 come from the end state
+      const uint16_t *q = reinterpret_cast<const uint16_t *>(p - 16 * lane) + lane;
+      uint32_t h[7];
+#pragma unroll
+      for (int i = 0; i < 7; ++i) h[i] = q[i * 32];
+      r.x = h[0] | (h[1] << 16); r.y = h[2] | (h[3] << 16); r.z = h[4] | (h[5] << 16); r.w = h[6];
+    }
+    p += 512;
+    return r;
+  }
+  __device__ __forceinline__ void open(const uint8_t *tile_raw, int V, int lane) {
+    p = tile_raw + 16 * lane;
+    next = load(0, V, lane);
+  }
+  // returns vector v (already in `next`) and starts fetching v + 1
+  __device__ __forceinline__ uint4 take(int v, int V, int lane) {
+    const uint4 r = next;
+    if (v + 1 < V) next = load(v + 1, V, lane);
     return r;
   }
 };
 
-// Decode one operand unit (128 rows x 32 operand bytes = 256 chunks of 16 B) of a tile.
-//   FMT: container format.  Emit: functor with
-//     void chunk(int g, int lane, uint4 v)   operand-format 16-byte chunk of round g (all formats), or
-//     void packed(int g, int lane, uint32_t b) for int4 when Emit::kOperand == false (4 packed bytes).
-//   u: unit index inside the tile (selects the raw vectors / scale group).
-template <uint32_t FMT, bool kPayload, class Emit>
-__device__ __forceinline__ void decode_unit(WarpStream &s, uint32_t tab, int lane, uint32_t lt, int u,
-                                            const RawReader<kPayload> &raw, uint4 &raw_next, uint4 &raw_next2,
-                                            const uint32_t *sz_row /* int4: &sz[group][n0] */, Emit &emit) {
+// Decode one operand unit (32 operand bytes per row) of J tiles at once.
+//   FMT: container format.  RB = tile_n / 32: the tile has RB row blocks of 32 rows and 2*RB chunk
+//   rounds per unit; in round g lane l owns the 16-byte operand chunk (row (g % RB)*32 + l, half g / RB).
+//   Emit: functor with
+//     void chunk(int j, int g, int lane, uint4 v)    operand-format 16-byte chunk of stream j, round g, or
+//     void packed(int j, int g, int lane, uint32_t b) for int4 when Emit::kOperand == false (4 packed bytes).
+//   ring0: shared address of stream 0's ring (stream j's follows at j * kStreamSmem).
+//   u: unit index inside the tile, V: raw vectors per tile (bf16).  sz[j]: int4: &(scale, zero)[group][first row of tile j].
+template <uint32_t FMT, int RB, int J, bool kPayload, class Emit>
+__device__ __forceinline__ void decode_unit(Stream (&s)[J], uint32_t ring0, uint32_t tab, int lane, uint32_t lt, int u, int V,
+                                            RawReader<kPayload> (&raw)[J], const uint32_t *const (&sz)[J], Emit &emit) {
+  constexpr int G = 2 * RB;
   if constexpr (FMT == ANSLIN_FMT_BF16) {
 #pragma unroll 1
-    for (int g2 = 0; g2 < 4; ++g2) {  // two rounds share one 16-byte raw vector; vectors are fetched two ahead
-      const int v = u * 4 + g2;
-      uint4 rv = raw_next;
-      raw_next = raw_next2;
-      if (v + 2 < raw.V) raw_next2 = raw.load(v + 2, lane);
+    for (int g2 = 0; g2 < RB; ++g2) {  // two chunk rounds share one 16-byte raw vector
+      const int v = u * RB + g2;
+      uint4 rv[J];
+#pragma unroll
+      for (int j = 0; j < J; ++j) rv[j] = raw[j].take(v, V, lane);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        stream_upkeep8(s, lane);
-        const uint32_t E0 = decode4(s, tab, lt), E1 = decode4(s, tab, lt);
-        if (kPayload && v == raw.V - 1 && h == 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
-          const uint32_t p = s.x - kL;
-          rv.w = (rv.w & 0xFFFFu) | (p << 16);
+        stream_upkeep8<J>(s, ring0, lane);
+        uint32_t E0[J], E1[J];
+        decode4<J>(s, E0, tab, lt);
+        decode4<J>(s, E1, tab, lt);
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          if (kPayload && h == 1 && v == V - 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
+            const uint32_t p = s[j].x - kL;
+            rv[j].w = (rv[j].w & 0xFFFFu) | (p << 16);
+          }
+          const uint2 a = bf16_merge4(E0[j], h ? rv[j].z : rv[j].x), b = bf16_merge4(E1[j], h ? rv[j].w : rv[j].y);
+          emit.chunk(j, g2 * 2 + h, lane, make_uint4(a.x, a.y, b.x, b.y));
         }
-        const uint2 a = bf16_merge4(E0, h ? rv.z : rv.x), b = bf16_merge4(E1, h ? rv.w : rv.y);
-        emit.chunk(g2 * 2 + h, lane, make_uint4(a.x, a.y, b.x, b.y));
       }
     }
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll 1
-    for (int g = 0; g < 8; ++g) {
-      if ((g & 1) == 0) stream_upkeep8(s, lane);
-      const uint32_t B = decode4(s, tab, lt);
-      if constexpr (Emit::kOperand) {
-        const uint32_t szv = __ldg(sz_row + (g & 3) * 32 + lane);
-        const __half2 sz = *reinterpret_cast<const __half2 *>(&szv);
-        const __half2 sc = __half2half2(__low2half(sz));
-        const __half2 zoff = __hadd2(__half2half2(__high2half(sz)), __float2half2_rn(1024.f));
-        emit.chunk(g, lane, make_uint4(awq_dequant2(B & 0xFF, zoff, sc), awq_dequant2((B >> 8) & 0xFF, zoff, sc),
-                                       awq_dequant2((B >> 16) & 0xFF, zoff, sc), awq_dequant2(B >> 24, zoff, sc)));
-      } else {
-        emit.packed(g, lane, B);
+    for (int g = 0; g < G; ++g) {
+      if ((g & 1) == 0) stream_upkeep8<J>(s, ring0, lane);
+      uint32_t B[J];
+      decode4<J>(s, B, tab, lt);
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        if constexpr (Emit::kOperand) {
+          const uint32_t szv = __ldg(sz[j] + (g % RB) * 32 + lane);
+          const __half2 szh = *reinterpret_cast<const __half2 *>(&szv);
+          const __half2 sc = __half2half2(__low2half(szh));
+          const __half2 zoff = __hadd2(__half2half2(__high2half(szh)), __float2half2_rn(1024.f));
+          emit.chunk(j, g, lane, make_uint4(awq_dequant2(B[j] & 0xFF, zoff, sc), awq_dequant2((B[j] >> 8) & 0xFF, zoff, sc),
+                                            awq_dequant2((B[j] >> 16) & 0xFF, zoff, sc), awq_dequant2(B[j] >> 24, zoff, sc)));
+        } else {
+          emit.packed(j, g, lane, B[j]);
+        }
       }
     }
   } else {  // fp8 / int8: the byte is the operand
 #pragma unroll 1
-    for (int g = 0; g < 8; ++g) {
-      stream_upkeep8(s, lane);
-      const uint32_t q0 = decode4(s, tab, lt), q1 = decode4(s, tab, lt);
-      stream_upkeep8(s, lane);
-      const uint32_t q2 = decode4(s, tab, lt), q3 = decode4(s, tab, lt);
-      emit.chunk(g, lane, make_uint4(q0, q1, q2, q3));
+    for (int g = 0; g < G; ++g) {
+      uint32_t q0[J], q1[J], q2[J], q3[J];
+      stream_upkeep8<J>(s, ring0, lane);
+      decode4<J>(s, q0, tab, lt);
+      decode4<J>(s, q1, tab, lt);
+      stream_upkeep8<J>(s, ring0, lane);
+      decode4<J>(s, q2, tab, lt);
+      decode4<J>(s, q3, tab, lt);
+#pragma unroll
+      for (int j = 0; j < J; ++j) emit.chunk(j, g, lane, make_uint4(q0[j], q1[j], q2[j], q3[j]));
     }
   }
 }

@@ -17,11 +17,14 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
+#include <string.h>
+#include <algorithm>
 
 #include "anslin_internal.h"
 #include "decode_core.cuh"
 
 using namespace anslin;
+
 
 namespace {
 
@@ -131,7 +134,7 @@ template <> struct FmtTraits<ANSLIN_FMT_INT8> { static constexpr int kind = 2; s
 struct ContainerView {
   const uint8_t *base;
   uint64_t off_freq, off_offsets, off_records, off_raw, off_scales, total;
-  uint32_t n_out, k_in, tile_k, KT, n_tiles, units, group, flags;
+  uint32_t n_out, k_in, tile_n, tile_k, KT, n_tiles, units, group, flags;
   float w_scale;
 };
 
@@ -141,109 +144,95 @@ ContainerView view_of(const anslin_weight *w) {
   v.base = w->dev;
   v.off_freq = h.off_freq; v.off_offsets = h.off_offsets; v.off_records = h.off_records; v.off_raw = h.off_raw;
   v.off_scales = h.off_scales; v.total = h.total_bytes;
-  v.n_out = h.n_out; v.k_in = h.k_in; v.tile_k = h.tile_k; v.KT = h.k_in / h.tile_k; v.n_tiles = h.n_tiles;
+  v.n_out = h.n_out; v.k_in = h.k_in; v.tile_n = h.tile_n; v.tile_k = h.tile_k; v.KT = h.k_in / h.tile_k; v.n_tiles = h.n_tiles;
   v.units = h.tile_k / unit_k_of(h.format); v.group = h.group_size; v.flags = h.flags; v.w_scale = h.w_scale;
   return v;
 }
 
+// A warp decodes J tiles at once (decode_core.cuh).  RB = tile_n / 32; a 128-row MMA unit is filled by
+// NW warps: 32-row tiles: J in {1, 2, 4}, NW = 4 / J; 128-row tiles: J = 1, NW = 1.
+template <int RB, int J> struct TileTraits {
+  static_assert((RB == 1 && (J == 1 || J == 2 || J == 4)) || (RB == 4 && J == 1), "unsupported tile / interleave combination");
+  static constexpr int Q = 4 / RB /*tiles per (stripe, k-tile) group*/, NW = Q / J /*warps per unit*/;
+};
+constexpr int kJ32 = 2;   // tiles a warp interleaves when tiles have 32 rows
+
+__host__ __device__ constexpr size_t row_bytes_of(uint32_t fmt, size_t k) {
+  return fmt == ANSLIN_FMT_BF16 ? k * 2 : fmt == ANSLIN_FMT_INT4_AWQ ? k / 2 : k;
+}
+
 // ------------------------------------------------------------------------------------------------
-// Decode-only kernel (anslin_decode): one warp per tile, output row-major W to HBM.
+// Decode-only kernel (anslin_decode): one warp per J tiles, output row-major W to HBM.
 // ------------------------------------------------------------------------------------------------
-template <uint32_t FMT>
+template <uint32_t FMT, int RB, int J>
 struct GlobalEmit {
   static constexpr bool kOperand = false;
-  uint8_t *tile_out;  // &W[n0][k0] in bytes
-  size_t row_bytes;   // bytes per W row
+  uint8_t *tile_out[J];  // &W[first row of tile j][k0] in bytes
+  size_t row_bytes;      // bytes per W row
   int u;
-  __device__ __forceinline__ void chunk(int g, int lane, uint4 v) const {  // bf16 / fp8 / int8: 16 B of row-major W
-    uint8_t *p = tile_out + size_t((g & 3) * 32 + lane) * row_bytes + size_t(u) * 32 + (g >> 2) * 16;
+  __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {  // bf16 / fp8 / int8: 16 B of row-major W
+    uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 32 + (g / RB) * 16;
     *reinterpret_cast<uint4 *>(p) = v;
   }
-  __device__ __forceinline__ void packed(int g, int lane, uint32_t b) const {  // int4: 4 packed bytes = 8 weights
-    uint8_t *p = tile_out + size_t((g & 3) * 32 + lane) * row_bytes + size_t(u) * 8 + (g >> 2) * 4;
+  __device__ __forceinline__ void packed(int j, int g, int lane, uint32_t b) const {  // int4: 4 packed bytes = 8 weights
+    uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 8 + (g / RB) * 4;
     *reinterpret_cast<uint32_t *>(p) = b;
   }
 };
 
 constexpr int kDecWarps = 8;
 
-template <uint32_t FMT, bool PAYLOAD>
-__global__ void __launch_bounds__(kDecWarps * 32) decode_kernel(ContainerView cv, uint8_t *out) {
-  __shared__ __align__(16) uint32_t tab[kM];
-  __shared__ uint32_t cum[260];
-  __shared__ __align__(16) uint8_t rings[(kDecWarps + 1) * kRingBytes];  // +1: rounded up to ring-size alignment below
+template <uint32_t FMT, int RB, int J, bool PAYLOAD>
+__global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView cv, uint8_t *out) {
+  constexpr int Q = TileTraits<RB, J>::Q;
+  extern __shared__ __align__(16) uint8_t dsm[];
+  uint32_t *tab = reinterpret_cast<uint32_t *>(dsm);
+  uint32_t *cum = tab + kM;
+  uint8_t *rings = dsm + 4 * kM + 1056;
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t lt = lanemask_lt(), ring_s = ((smem_u32(rings) + kRingBytes - 1) & ~(kRingBytes - 1)) + uint32_t(warp) * kRingBytes;
+  const uint32_t lt = lanemask_lt(), ring_s = smem_u32(rings) + uint32_t(warp) * J * kStreamSmem;
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
-  const size_t row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.k_in) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.k_in) / 2 : size_t(cv.k_in);
-  const size_t tile_row_bytes = FMT == ANSLIN_FMT_BF16 ? size_t(cv.tile_k) * 2 : FMT == ANSLIN_FMT_INT4_AWQ ? size_t(cv.tile_k) / 2 : size_t(cv.tile_k);
-  const size_t rtb = raw_tile_bytes(kTileN, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
-  for (uint32_t t = blockIdx.x * kDecWarps + warp; t < cv.n_tiles; t += gridDim.x * kDecWarps) {
-    WarpStream s;
-    stream_open(s, cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s, lane);
-    const uint32_t stripe = t / cv.KT, kt = t % cv.KT;
-    GlobalEmit<FMT> emit;
-    emit.tile_out = out + size_t(stripe) * kTileN * row_bytes + size_t(kt) * tile_row_bytes;
+  const size_t row_bytes = row_bytes_of(FMT, cv.k_in), tile_row_bytes = row_bytes_of(FMT, cv.tile_k);
+  const size_t rtb = raw_tile_bytes(32 * RB, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
+  const int V = int(cv.units) * RB;
+  for (uint32_t job = blockIdx.x * kDecWarps + warp; job < cv.n_tiles / J; job += gridDim.x * kDecWarps) {
+    Stream s[J];
+    RawReader<PAYLOAD> raw[J];
+    const uint32_t *sz[J];
+    GlobalEmit<FMT, RB, J> emit;
     emit.row_bytes = row_bytes;
-    RawReader<PAYLOAD> raw;
-    raw.tile_raw = cv.base + cv.off_raw + size_t(t) * rtb;
-    raw.V = int(cv.units) * 4;
-    uint4 raw_next = make_uint4(0, 0, 0, 0), raw_next2 = raw_next;
-    if (FMT == ANSLIN_FMT_BF16) { raw_next = raw.load(0, lane); raw_next2 = raw.load(1, lane); }
+    stream_drain();
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+      const uint32_t t = job * J + j, grp = t / Q, q = t % Q, stripe = grp / cv.KT, kt = grp % cv.KT;
+      stream_open(s[j], cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s + j * kStreamSmem, lane);
+      emit.tile_out[j] = out + (size_t(stripe) * kTileN + size_t(q) * 32 * RB) * row_bytes + size_t(kt) * tile_row_bytes;
+      if (FMT == ANSLIN_FMT_BF16) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
+      sz[j] = nullptr;
+    }
     for (uint32_t u = 0; u < cv.units; ++u) {
       emit.u = int(u);
-      decode_unit<FMT, PAYLOAD>(s, smem_u32(tab), lane, lt, int(u), raw, raw_next, raw_next2, nullptr, emit);
+      decode_unit<FMT, RB, J, PAYLOAD>(s, ring_s, smem_u32(tab), lane, lt, int(u), V, raw, sz, emit);
     }
   }
   cp_async_wait_all();
 }
 
 // ------------------------------------------------------------------------------------------------
-// Fused decode + GEMM kernel
+// Work split and epilogue helpers shared by the fused and the dense kernel
 // ------------------------------------------------------------------------------------------------
 constexpr int kEpiWarps = 4;
 constexpr int kMmaWarp = 4;
 constexpr int kFirstDecWarp = 5;
-constexpr int kMaxDecWarps = 24;
+constexpr int kMaxDecWarps = 20;
 constexpr int kGemmThreads = 32 * (kFirstDecWarp + kMaxDecWarps);
 constexpr int kMaxSlots = 48;
 
-struct GemmParams {
-  ContainerView cv;
-  const float *x_scale;    // int8 / fp8: f32[m]
-  float *y;
-  int64_t ldy;
-  uint32_t *partials;      // [2*grid][mpad][128] raw accumulator bits
-  uint32_t *counters;      // [stripes]
-  uint32_t m, mpad;
-  uint32_t U, D;           // ring slots, decoder warps
-  uint32_t slot_bytes;     // 4096 + mpad*32
-  uint32_t tmem_cols;
-  uint32_t layout;         // kLayoutSW32 or kLayoutNone (debug alternative)
-};
-
-// Shared-memory unit slot writer: the decoded 16-byte chunk goes where the UMMA K-major canonical
-// layout expects it (P:l.151 "consumed by the GEMM kernel in its required swizzled layout").
-struct SmemEmit {
-  static constexpr bool kOperand = true;
-  uint32_t slot_a;   // shared address of the unit's A operand (4 KiB)
-  uint32_t layout;
-  __device__ __forceinline__ void chunk(int g, int lane, uint4 v) const {
-    const uint32_t row = uint32_t((g & 3) * 32 + lane), c = uint32_t(g >> 2);
-    uint32_t a;
-    if (layout == kLayoutSW32) a = slot_a + row * 32u + ((c ^ ((uint32_t(lane) >> 2) & 1u)) << 4);  // Swizzle<1,4,3>
-    else a = slot_a + c * 2048u + row * 16u;                                                        // 8x16B core matrices
-    sts128(a, v);
-  }
-  __device__ __forceinline__ void packed(int, int, uint32_t) const {}
-};
-
-struct Segment { uint32_t stripe, ka, nt; };
-
-// Work of CTA c: tiles [t0, t1) of the stripe-major tile sequence (stream-K style equal split).
-__device__ __forceinline__ uint32_t cta_first_tile(uint32_t c, uint32_t G, uint32_t T) { return uint32_t(uint64_t(c) * T / G); }
-__device__ __forceinline__ uint32_t cta_of_tile(uint32_t t, uint32_t G, uint32_t T) {  // largest c with first_tile(c) <= t
+// Work of CTA c (of G): groups [first(c), first(c+1)) of the stripe-major sequence of T (stripe, k-tile)
+// groups (stream-K style equal split): a CTA owns at most two partial stripes plus whole stripes.
+__host__ __device__ __forceinline__ uint32_t cta_first_tile(uint32_t c, uint32_t G, uint32_t T) { return uint32_t(uint64_t(c) * T / G); }
+__host__ __device__ __forceinline__ uint32_t cta_of_tile(uint32_t t, uint32_t G, uint32_t T) {  // largest c with first(c) <= t
   return uint32_t((uint64_t(t + 1) * G + T - 1) / T) - 1;
 }
 
@@ -259,21 +248,17 @@ __device__ __forceinline__ uint32_t acc_add(uint32_t a, uint32_t b) {
   else return __float_as_uint(__uint_as_float(a) + __uint_as_float(b));
 }
 
-
-// ------------------------------------------------------------------------------------------------
-// Epilogue (a10), shared by the fused and the dense kernel.  Warps 0..3: TMEM -> registers -> Y for
-// whole stripes, or -> split-K partial + deterministic fix-up (the LAST CTA to finish a stripe sums
-// all partials in CTA order, 16-byte loads, up to 8 contributors in flight per thread).
-// ------------------------------------------------------------------------------------------------
 struct EpiParams {
   const float *x_scale;     // int8 / fp8: f32[m]
   const __half *w_scale_h;  // int8: fp16[n_out]
   float w_scale;            // fp8
   float *y;
   int64_t ldy;
-  uint32_t *partials, *counters;
+  uint32_t *partials, *counters;   // [2*G][mpad][128] raw accumulator bits; [stripes]
   uint32_t m, mpad;
 };
+// A stripe whose last split-K contributor is this CTA (shared memory; at most the first and the last segment).
+struct FinSeg { uint32_t valid, stripe, c_first, c_last; };
 
 __device__ __forceinline__ uint4 ldcg128(const uint32_t *p) {
   uint4 r;
@@ -281,9 +266,11 @@ __device__ __forceinline__ uint4 ldcg128(const uint32_t *p) {
   return r;
 }
 
+// Epilogue (a10), warps 0..3: TMEM -> registers -> Y for whole stripes, or -> split-K partial.  The CTA
+// that contributes LAST to a stripe (global counter) records it in fin[]; splitk_fixup sums it up later.
 template <uint32_t FMT>
 __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_base, uint32_t tfull_s, uint32_t tempty_s,
-                                             volatile uint32_t *flag, uint32_t t_begin, uint32_t t_end, uint32_t KT, uint32_t G,
+                                             FinSeg *fin, uint32_t t_begin, uint32_t t_end, uint32_t KT, uint32_t c, uint32_t G,
                                              uint32_t T, int warp, int lane) {
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
   const uint32_t row = uint32_t(warp * 32 + lane);
@@ -297,8 +284,8 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
     mbar_wait<400>(tfull_s + 8 * ab, (si >> 1) & 1u);
     tc_fence_after();
-    const uint32_t pslot = blockIdx.x * 2u + (t == t_begin ? 0u : 1u);
-    uint32_t *part = p.partials + size_t(pslot) * p.mpad * kTileN;
+    const uint32_t seg = (t == t_begin ? 0u : 1u);
+    uint32_t *part = p.partials + size_t(c * 2u + seg) * p.mpad * kTileN;
     for (uint32_t c0 = 0; c0 < p.mpad; c0 += 16) {
       uint32_t v[16];
       tmem_ld16(tmem_base + ((uint32_t(warp) * 32u) << 16) + ab * p.mpad + c0, v);
@@ -315,144 +302,207 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     __syncwarp();
     if (lane == 0) mbar_arrive(tempty_s + 8 * ab);
     if (!whole) {
-      const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
       __threadfence();
       named_bar_sync(1, kEpiWarps * 32);
-      if (threadIdx.x == 0) *flag = (atomicAdd(&p.counters[stripe], 1u) == c_last - c_first) ? 1u : 0u;
-      named_bar_sync(1, kEpiWarps * 32);
-      if (*flag) {
+      if (threadIdx.x == 0) {
+        const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
+        const bool last = atomicAdd(&p.counters[stripe], 1u) == c_last - c_first;
         __threadfence();
-        // thread -> 4 consecutive output channels (one 16-byte load per contributor), warp -> batch rows mm = warp, warp+4, ..
-        const uint32_t r4 = uint32_t(lane) * 4u, n4 = stripe * kTileN + r4;
-        float ws4[4] = {ws, ws, ws, ws};
-        if (FMT == ANSLIN_FMT_INT8)
-#pragma unroll
-          for (int j = 0; j < 4; ++j) ws4[j] = __half2float(p.w_scale_h[n4 + j]);
-        for (uint32_t mm = uint32_t(warp); mm < p.m; mm += kEpiWarps) {
-          uint32_t acc[4];
-#pragma unroll
-          for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-          for (uint32_t cb = c_first; cb <= c_last; cb += 8) {
-            uint4 v[8];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-              const uint32_t c = cb + j;
-              v[j] = make_uint4(0, 0, 0, 0);
-              if (c <= c_last) {
-                const uint32_t ps = c * 2u + (cta_first_tile(c, G, T) / KT == stripe ? 0u : 1u);
-                v[j] = ldcg128(p.partials + (size_t(ps) * p.mpad + mm) * kTileN + r4);
-              }
-            }
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {  // fixed CTA order -> bit-reproducible sums
-              acc[0] = acc_add<FMT>(acc[0], v[j].x); acc[1] = acc_add<FMT>(acc[1], v[j].y);
-              acc[2] = acc_add<FMT>(acc[2], v[j].z); acc[3] = acc_add<FMT>(acc[3], v[j].w);
-            }
-          }
-          const float xs = kScaled ? p.x_scale[mm] : 1.0f;
-          float *yo = p.y + size_t(mm) * p.ldy + n4;
-#pragma unroll
-          for (int j = 0; j < 4; ++j) yo[j] = finalize<FMT>(acc[j], xs, ws4[j]);
-        }
-        if (threadIdx.x == 0) p.counters[stripe] = 0;
+        fin[seg].stripe = stripe; fin[seg].c_first = c_first; fin[seg].c_last = c_last; fin[seg].valid = last ? 1u : 0u;
       }
-      named_bar_sync(1, kEpiWarps * 32);  // flag is reused by the next segment
     }
     t += nt;
   }
 }
 
-template <uint32_t FMT, bool PAYLOAD>
-__global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ CUtensorMap tmx, GemmParams p) {
+// Deterministic split-K fix-up by ALL threads of the CTA (call after a CTA-wide barrier that follows
+// epilogue_run): for each stripe recorded in fin[], sum the partials of its contributors in CTA order
+// (bit-reproducible), apply the scales and store Y.  One item = one batch row x 4 output channels;
+// 16-byte loads, up to 8 contributors in flight per thread.
+template <uint32_t FMT>
+__device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *fin, uint32_t KT, uint32_t G, uint32_t T) {
+  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
+  for (int seg = 0; seg < 2; ++seg) {
+    if (!fin[seg].valid) continue;
+    const uint32_t stripe = fin[seg].stripe, c_first = fin[seg].c_first, c_last = fin[seg].c_last;
+    for (uint32_t it = threadIdx.x; it < p.m * 32u; it += blockDim.x) {
+      const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u, n4 = stripe * kTileN + r4;
+      uint32_t acc[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
+      for (uint32_t cb = c_first; cb <= c_last; cb += 8) {
+        uint4 v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          const uint32_t cc = cb + j;
+          v[j] = make_uint4(0, 0, 0, 0);
+          if (cc <= c_last) {
+            const uint32_t ps = cc * 2u + (cta_first_tile(cc, G, T) / KT == stripe ? 0u : 1u);
+            v[j] = ldcg128(p.partials + (size_t(ps) * p.mpad + mm) * kTileN + r4);
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {  // fixed CTA order -> bit-reproducible sums
+          acc[0] = acc_add<FMT>(acc[0], v[j].x); acc[1] = acc_add<FMT>(acc[1], v[j].y);
+          acc[2] = acc_add<FMT>(acc[2], v[j].z); acc[3] = acc_add<FMT>(acc[3], v[j].w);
+        }
+      }
+      const float xs = kScaled ? p.x_scale[mm] : 1.0f;
+      float *yo = p.y + size_t(mm) * p.ldy + n4;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        float ws = 1.0f;
+        if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
+        if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
+        yo[j] = finalize<FMT>(acc[j], xs, ws);
+      }
+    }
+    if (threadIdx.x == 0) p.counters[stripe] = 0;   // every contributor has arrived: ready for the next launch
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fused decode + GEMM kernel
+// ------------------------------------------------------------------------------------------------
+constexpr int kMaxProblems = 8;
+// One GEMM of a launch.  A launch is the concatenation of independent sub-grids: problem i owns CTAs
+// [cta0, cta0 + ncta) (grouped MoE experts, or projections that share an input).
+struct Problem {
+  ContainerView cv;
+  const float *x_scale;    // int8 / fp8: f32[m]
+  float *y;
+  int64_t ldy;
+  uint32_t *partials;      // [2*ncta][mpad][128] raw accumulator bits
+  uint32_t *counters;      // [stripes]
+  uint32_t m, mpad, cta0, ncta;
+};
+struct FusedParams {
+  Problem prob[kMaxProblems];
+  uint32_t nprob;
+  uint32_t U, D;           // ring slots, decoder warps
+  uint32_t slot_bytes;     // 4096 + max mpad * 32
+  uint32_t tmem_cols;
+};
+struct TensorMaps { CUtensorMap m[kMaxProblems]; };
+
+// Shared-memory unit slot writer: the decoded 16-byte chunk goes where the UMMA K-major SWIZZLE_32B
+// canonical layout expects it (P:l.151 "consumed by the GEMM kernel in its required swizzled layout").
+template <int RB, int J>
+struct SmemEmit {
+  static constexpr bool kOperand = true;
+  uint32_t slot_a;       // shared address of the unit's A operand (4 KiB)
+  uint32_t row0[J];      // first stripe row of stream j's tile
+  __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {
+    const uint32_t row = row0[j] + uint32_t((g % RB) * 32 + lane), c = uint32_t(g / RB);
+    sts128(slot_a + row * 32u + ((c ^ ((uint32_t(lane) >> 2) & 1u)) << 4), v);  // Swizzle<1,4,3>
+  }
+  __device__ __forceinline__ void packed(int, int, int, uint32_t) const {}
+};
+
+template <uint32_t FMT, int RB, int J, bool PAYLOAD>
+__global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ TensorMaps tms,
+                                                                      const __grid_constant__ FusedParams P) {
   using TR = FmtTraits<FMT>;
+  constexpr int NW = TileTraits<RB, J>::NW, Q = TileTraits<RB, J>::Q;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 2047u) & ~2047u;
   uint8_t *smem = smem_raw + (smem0 - smem_u32(smem_raw));
+  // which problem does this CTA belong to?
+  uint32_t pi = 0;
+  while (pi + 1 < P.nprob && blockIdx.x >= P.prob[pi + 1].cta0) ++pi;
+  const Problem &pr = P.prob[pi];
+  const ContainerView &cv = pr.cv;
+  const uint32_t c = blockIdx.x - pr.cta0, G = pr.ncta, KT = cv.KT, T = (cv.n_out / kTileN) * KT;
+  const uint32_t mpad = pr.mpad, units = cv.units;
   // carve-up
   const uint32_t slots_s = smem0;
-  const uint32_t ring_off = (p.U * p.slot_bytes + kRingBytes - 1) & ~(kRingBytes - 1);   // rings are ring-size aligned
-  const uint32_t tab_off = ring_off + p.D * kRingBytes;
+  const uint32_t ring_off = P.U * P.slot_bytes;
+  const uint32_t tab_off = ring_off + P.D * J * kStreamSmem;
   uint32_t *tab = reinterpret_cast<uint32_t *>(smem + tab_off);
   uint32_t *cum = reinterpret_cast<uint32_t *>(smem + tab_off + 16384);
   const uint32_t bar_off = tab_off + 16384 + 1056;
   const uint32_t full_s = smem0 + bar_off, empty_s = full_s + 8 * kMaxSlots, tfull_s = empty_s + 8 * kMaxSlots,
-                 tempty_s = tfull_s + 16, tmemptr_s = tempty_s + 16, flag_s = tmemptr_s + 8;
+                 tempty_s = tfull_s + 16, tmemptr_s = tempty_s + 16;
   volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 32);
-  volatile uint32_t *flag = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 40);
-  // lapw[slot] = number of ring laps whose producer has ACQUIRED the slot.  A decoder warp may run
+  FinSeg *fin = reinterpret_cast<FinSeg *>(smem + bar_off + 16 * kMaxSlots + 48);
+  // lapw[slot] = number of ring laps whose producers have ACQUIRED the slot.  A decoder warp may run
   // more than one lap ahead of a slot's barrier (idle rounds, segment changes), where an mbarrier
   // parity wait would alias; it first waits for its predecessor lap to be acquired.
-  volatile uint32_t *lapw = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 64);
+  const uint32_t lapw_s = smem0 + bar_off + 16 * kMaxSlots + 80;
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const ContainerView &cv = p.cv;
-  const uint32_t G = gridDim.x, T = cv.n_tiles, KT = cv.KT;
 
   if (threadIdx.x == 0) {
-    for (uint32_t i = 0; i < p.U; ++i) { mbar_init(full_s + 8 * i, 2); mbar_init(empty_s + 8 * i, 1); lapw[i] = 0; }
-    for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); }
+    for (uint32_t i = 0; i < P.U; ++i) { mbar_init(full_s + 8 * i, NW + 1); mbar_init(empty_s + 8 * i, 1); sts32(lapw_s + 4 * i, 0); }
+    for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); fin[i].valid = 0; }
     fence_mbar_init();
   }
-  if (warp == 0) tmem_alloc(tmemptr_s, p.tmem_cols);
+  if (warp == 0) tmem_alloc(tmemptr_s, P.tmem_cols);
   tc_fence_before();
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));  // ends with __syncthreads()
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
 
-  const uint32_t t_begin = cta_first_tile(blockIdx.x, G, T), t_end = cta_first_tile(blockIdx.x + 1, G, T);
-  const uint32_t units = cv.units;
+  const uint32_t t_begin = cta_first_tile(c, G, T), t_end = cta_first_tile(c + 1, G, T);
+  const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, pr.y, pr.ldy,
+                     pr.partials, pr.counters, pr.m, mpad};
 
   if (warp >= kFirstDecWarp) {
     // ===================== decoder warps: Alg V.2 into the operand ring =====================
     const uint32_t d = uint32_t(warp - kFirstDecWarp);
-    if (d < p.D) {
-      const uint32_t lt = lanemask_lt(), ring_s = smem0 + ring_off + d * kRingBytes;
+    if (d < P.D) {
+      const uint32_t PT = P.D / NW, team = d / NW, hw = d % NW;   // teams of NW warps fill one 128-row unit together
+      const uint32_t lt = lanemask_lt(), ring_s = smem0 + ring_off + d * J * kStreamSmem, tab_s = smem0 + tab_off;
       const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
-      const size_t rtb = raw_tile_bytes(kTileN, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
-      const uint32_t xbytes = p.mpad * 32u;
-      // Tiles of this CTA are dealt to the decoder warps round-robin over the CTA's WHOLE range
-      // (tile i -> warp i mod D, round i div D).  The MMA warp consumes units segment by segment
-      // (one accumulator per stripe segment); inside a segment the order is (round, unit, tile).
-      for (uint32_t i = d; i < t_end - t_begin; i += p.D) {
+      const size_t rtb = raw_tile_bytes(32 * RB, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
+      const uint32_t xbytes = mpad * 32u;
+      const int V = int(units) * RB;
+      // Groups of this CTA are dealt to the teams round-robin over the CTA's WHOLE range (group i ->
+      // team i mod PT, round i div PT).  The MMA warp consumes units segment by segment (one
+      // accumulator per stripe segment); inside a segment the order is (round, unit, group).
+      for (uint32_t i = team; i < t_end - t_begin; i += PT) {
         const uint32_t gt = t_begin + i, stripe = gt / KT, kt = gt % KT;
-        const uint32_t seg_a = max(t_begin, stripe * KT) - t_begin;            // segment = [seg_a, seg_b) in CTA-local tiles
+        const uint32_t seg_a = max(t_begin, stripe * KT) - t_begin;            // segment = [seg_a, seg_b) in CTA-local groups
         const uint32_t seg_b = min(t_end, stripe * KT + KT) - t_begin;
-        const uint32_t rho = i / p.D;
-        const uint32_t grp_a = max(seg_a, rho * p.D), grp_b = min(seg_b, rho * p.D + p.D);   // this round's tiles of the segment
-        const uint32_t seq0 = (seg_a + (grp_a - seg_a)) * units, cnt = grp_b - grp_a, idx = i - grp_a;
-        WarpStream s;
-        stream_open(s, cv.base + cv.off_records + size_t(offs[gt]) * 16, ring_s, lane);
-        RawReader<PAYLOAD> raw;
-        raw.tile_raw = cv.base + cv.off_raw + size_t(gt) * rtb;
-        raw.V = int(units) * 4;
-        uint4 raw_next = make_uint4(0, 0, 0, 0), raw_next2 = raw_next;
-        if (FMT == ANSLIN_FMT_BF16) { raw_next = raw.load(0, lane); raw_next2 = raw.load(1, lane); }
+        const uint32_t rho = i / PT;
+        const uint32_t grp_a = max(seg_a, rho * PT), grp_b = min(seg_b, rho * PT + PT);   // this round's groups of the segment
+        const uint32_t seq0 = grp_a * units, cnt = grp_b - grp_a, idx = i - grp_a;
+        Stream s[J];
+        RawReader<PAYLOAD> raw[J];
+        const uint32_t *sz[J];
+        SmemEmit<RB, J> emit;
+        stream_drain();
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          const uint32_t q = hw * J + j, t = gt * Q + q;
+          stream_open(s[j], cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s + j * kStreamSmem, lane);
+          if (FMT == ANSLIN_FMT_BF16) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
+          emit.row0[j] = q * 32u * RB;
+          sz[j] = nullptr;
+        }
         for (uint32_t u = 0; u < units; ++u) {
           const uint32_t seq = seq0 + u * cnt + idx;
-          const uint32_t slot = seq % p.U, lap = seq / p.U;
-          const uint32_t slot_a = slots_s + slot * p.slot_bytes;
-          for (uint32_t spins = 0; lapw[slot] < lap;) {  // a waiting decoder sleeps: it must not take issue slots
-            __nanosleep(100);
+          const uint32_t slot = seq % P.U, lap = seq / P.U;
+          const uint32_t slot_a = slots_s + slot * P.slot_bytes;
+          for (uint32_t spins = 0; lds32v(lapw_s + 4 * slot) < lap;) {  // a waiting decoder sleeps: it must not take issue slots
+            __nanosleep(64);
             if (++spins > (1u << 24)) __trap();
           }
-          mbar_wait<100>(empty_s + 8 * slot, (lap & 1u) ^ 1u);
-          if (lane == 0) lapw[slot] = lap + 1u;
+          mbar_wait<64>(empty_s + 8 * slot, (lap & 1u) ^ 1u);
           const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
-          if (lane == 0) {
+          if (hw == 0 && lane == 0) {
+            sts32(lapw_s + 4 * slot, lap + 1u);
             mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
-            if (p.layout == kLayoutSW32) {
-              tma_load_2d(slot_a + kUnitBytes, &tmx, k_elem, 0, full_s + 8 * slot);
-            } else {  // two 16-byte-wide boxes = two K-adjacent columns of 8x16B core matrices
-              tma_load_2d(slot_a + kUnitBytes, &tmx, k_elem, 0, full_s + 8 * slot);
-              tma_load_2d(slot_a + kUnitBytes + p.mpad * 16u, &tmx, k_elem + unit_k_of(FMT) / 2, 0, full_s + 8 * slot);
-            }
+            tma_load_2d(slot_a + kUnitBytes, &tms.m[pi], k_elem, 0, full_s + 8 * slot);
           }
-          SmemEmit emit{slot_a, p.layout};
-          const uint32_t *sz_row = nullptr;
-          if (FMT == ANSLIN_FMT_INT4_AWQ)
-            sz_row = reinterpret_cast<const uint32_t *>(cv.base + cv.off_scales) +
-                     size_t(uint32_t(k_elem) / cv.group) * cv.n_out + size_t(stripe) * kTileN;
-          decode_unit<FMT, PAYLOAD>(s, smem0 + tab_off, lane, lt, int(u), raw, raw_next, raw_next2, sz_row, emit);
+          emit.slot_a = slot_a;
+          if (FMT == ANSLIN_FMT_INT4_AWQ) {
+#pragma unroll
+            for (int j = 0; j < J; ++j)
+              sz[j] = reinterpret_cast<const uint32_t *>(cv.base + cv.off_scales) + size_t(uint32_t(k_elem) / cv.group) * cv.n_out +
+                      size_t(stripe) * kTileN + emit.row0[j];
+          }
+          decode_unit<FMT, RB, J, PAYLOAD>(s, ring_s, tab_s, lane, lt, int(u), V, raw, sz, emit);
           fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
           __syncwarp();
           if (lane == 0) mbar_arrive(full_s + 8 * slot);
@@ -462,7 +512,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     }
   } else if (warp == kMmaWarp) {
     // ===================== MMA issuer: one thread drives the tensor core =====================
-    const uint32_t idesc = make_idesc(TR::c, TR::ab, TR::ab, 128, p.mpad);
+    const uint32_t idesc = make_idesc(TR::c, TR::ab, TR::ab, 128, mpad);
     uint32_t seq = 0, si = 0;
     for (uint32_t t = t_begin; t < t_end; ++si) {
       const uint32_t ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
@@ -470,20 +520,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       tc_fence_after();
       const uint32_t n_units = nt * units;
       for (uint32_t j = 0; j < n_units; ++j, ++seq) {
-        const uint32_t slot = seq % p.U, par = (seq / p.U) & 1u;
+        const uint32_t slot = seq % P.U, par = (seq / P.U) & 1u;
         mbar_wait<40>(full_s + 8 * slot, par);
         tc_fence_after();
         if (lane == 0) {
-          const uint32_t a = slots_s + slot * p.slot_bytes, b = a + kUnitBytes;
-          uint64_t ad, bd;
-          if (p.layout == kLayoutSW32) {
-            ad = make_smem_desc(a, 16, 256, kLayoutSW32);
-            bd = make_smem_desc(b, 16, 256, kLayoutSW32);
-          } else {
-            ad = make_smem_desc(a, 2048, 128, kLayoutNone);
-            bd = make_smem_desc(b, p.mpad * 16u, 128, kLayoutNone);
-          }
-          umma<TR::kind>(tmem_base + ab * p.mpad, ad, bd, idesc, j > 0 ? 1u : 0u);
+          const uint32_t a = slots_s + slot * P.slot_bytes, b = a + kUnitBytes;
+          umma<TR::kind>(tmem_base + ab * mpad, make_smem_desc(a, 16, 256, kLayoutSW32), make_smem_desc(b, 16, 256, kLayoutSW32),
+                         idesc, j > 0 ? 1u : 0u);
           umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
           if (j + 1 == n_units) umma_commit(tfull_s + 8 * ab);
         }
@@ -493,13 +536,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     }
   } else {
     // ===================== epilogue warps 0..3 =====================
-    EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, p.y, p.ldy, p.partials,
-                 p.counters, p.m, p.mpad};
-    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, flag, t_begin, t_end, KT, G, T, warp, lane);
+    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp, lane);
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem_base, p.tmem_cols);
+  if (warp == 0) tmem_dealloc(tmem_base, P.tmem_cols);
+  splitk_fixup<FMT>(ep, fin, KT, G, T);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -529,12 +571,12 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   const uint32_t full_s = smem0 + bar_off, empty_s = full_s + 8 * kMaxSlots, tfull_s = empty_s + 8 * kMaxSlots,
                  tempty_s = tfull_s + 16, tmemptr_s = tempty_s + 16;
   volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 32);
-  volatile uint32_t *flag = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 40);
+  FinSeg *fin = reinterpret_cast<FinSeg *>(smem + bar_off + 16 * kMaxSlots + 48);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t G = gridDim.x, KT = p.KB, T = (p.n_out / kTileN) * KT;
   if (threadIdx.x == 0) {
     for (uint32_t i = 0; i < p.S; ++i) { mbar_init(full_s + 8 * i, 1); mbar_init(empty_s + 8 * i, 1); }
-    for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); }
+    for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); fin[i].valid = 0; }
     fence_mbar_init();
   }
   if (warp == 0) tmem_alloc(tmemptr_s, p.tmem_cols);
@@ -543,6 +585,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
   const uint32_t t_begin = cta_first_tile(blockIdx.x, G, T), t_end = cta_first_tile(blockIdx.x + 1, G, T);
+  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.m, p.mpad};
 
   if (warp == 5) {
     if (lane == 0) {
@@ -582,12 +625,12 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
     }
     (void)UK;
   } else {
-    EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.m, p.mpad};
-    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, flag, t_begin, t_end, KT, G, T, warp, lane);
+    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, blockIdx.x, G, T, warp, lane);
   }
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(tmem_base, p.tmem_cols);
+  splitk_fixup<FMT>(ep, fin, KT, G, T);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -658,98 +701,168 @@ bool x_dtype_ok(uint32_t fmt, uint32_t dt) {
          (fmt == ANSLIN_FMT_INT8 && dt == ANSLIN_DT_I8) || (fmt == ANSLIN_FMT_FP8_E4M3 && dt == ANSLIN_DT_FP8_E4M3);
 }
 
-template <uint32_t FMT, bool PAYLOAD>
-int launch_fused(const anslin_weight *w, const CUtensorMap &tmx, GemmParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
-  auto kern = fused_gemm_kernel<FMT, PAYLOAD>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
-  kern<<<grid, kGemmThreads, smem, st>>>(tmx, p);
+int sm_budget() { return std::max(1, num_sms()); }
+
+template <uint32_t FMT, int RB, bool PAYLOAD>
+int launch_fused(const TensorMaps &tms, const FusedParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
+  auto kern = fused_gemm_kernel<FMT, RB, (RB == 1 ? kJ32 : 1), PAYLOAD>;
+  static thread_local size_t smem_set = 0;     // per instantiation: raise the dynamic shared memory limit once
+  if (smem > smem_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
+    smem_set = kSmemMax;
+  }
+  kern<<<grid, 32 * (kFirstDecWarp + p.D), smem, st>>>(tms, p);
   ++g_launches;
-  (void)w;
   if (getenv("ANSLIN_DEBUG")) {  // debugging aid only: synchronous error report
     cudaError_t e = cudaStreamSynchronize(st);
-    fprintf(stderr, "[anslin] fused grid=%u smem=%zu D=%u U=%u mpad=%u tiles=%u: %s\n", grid, smem, p.D, p.U, p.mpad,
-            p.cv.n_tiles, cudaGetErrorString(e));
+    fprintf(stderr, "[anslin] fused grid=%u smem=%zu D=%u U=%u nprob=%u: %s\n", grid, smem, p.D, p.U, p.nprob, cudaGetErrorString(e));
   }
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 
-int gemm_one(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m, const void *x_scale_dev,
-             void *y_dev, int64_t ldy, void *workspace_dev, size_t workspace_bytes, cudaStream_t st) {
-  if (!w || !w->dev || !x_dev || !y_dev || !workspace_dev) return ANSLIN_ERR_INVALID_ARG;
-  if (m < 1 || m > 256) return ANSLIN_ERR_UNSUPPORTED;
-  const Header &h = w->h;
-  if (!x_dtype_ok(h.format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
-  if ((reinterpret_cast<uintptr_t>(x_dev) | reinterpret_cast<uintptr_t>(y_dev) | reinterpret_cast<uintptr_t>(workspace_dev)) & 15)
-    return ANSLIN_ERR_INVALID_ARG;
-  const bool scaled = h.format == ANSLIN_FMT_INT8 || h.format == ANSLIN_FMT_FP8_E4M3;
-  if (scaled && !x_scale_dev) return ANSLIN_ERR_INVALID_ARG;
-  const int xb = (h.format == ANSLIN_FMT_BF16 || h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
-  if (ldx < int64_t(h.k_in) || (ldx * xb) % 16 || ldy < int64_t(h.n_out)) return ANSLIN_ERR_INVALID_ARG;
+// One launch over n <= kMaxProblems independent GEMMs that share format and tile geometry.
+int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, uint32_t x_dtype, const int64_t *ldx, const int32_t *ms,
+                const void *const *x_scales, void *const *ys, const int64_t *ldy, void *workspace_dev, size_t workspace_bytes,
+                cudaStream_t st) {
+  if (n < 1 || n > kMaxProblems || !workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) & 15)) return ANSLIN_ERR_INVALID_ARG;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
-
-  GemmParams p;
-  p.cv = view_of(w);
-  p.m = uint32_t(m);
-  p.mpad = mpad_of(m);
-  p.slot_bytes = kUnitBytes + p.mpad * 32u;
-  p.tmem_cols = tmem_cols_of(p.mpad);
-  p.x_scale = static_cast<const float *>(x_scale_dev);
-  p.y = static_cast<float *>(y_dev);
-  p.ldy = ldy;
-  const char *lay = getenv("ANSLIN_LAYOUT");  // debug: "none" selects the unswizzled core-matrix layout
-  p.layout = (lay && lay[0] == 'n') ? kLayoutNone : kLayoutSW32;
-  uint32_t min_tiles = 12;
-  if (const char *e = getenv("ANSLIN_MIN_TILES")) min_tiles = uint32_t(std::max(1, atoi(e)));
-  const uint32_t grid = grid_of(h.n_tiles, min_tiles), stripes = h.n_out / kTileN;
-  // ring sizing: D decoder warps (1 KiB compressed-word ring each) and U operand slots
-  const size_t fixed = 2048 /*align slack*/ + 2048 /*ring alignment*/ + 16384 + 1056 + 16 * kMaxSlots + 64 + 4 * kMaxSlots;
+  const Header &h0 = ws[0]->h;
+  const bool scaled = h0.format == ANSLIN_FMT_INT8 || h0.format == ANSLIN_FMT_FP8_E4M3;
+  const int xb = (h0.format == ANSLIN_FMT_BF16 || h0.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
+  if (!x_dtype_ok(h0.format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
+  uint32_t mpad_max = 16;
+  uint64_t work[kMaxProblems], work_sum = 0;
+  for (int i = 0; i < n; ++i) {
+    const anslin_weight *w = ws[i];
+    if (!w || !w->dev || !xs[i] || !ys[i]) return ANSLIN_ERR_INVALID_ARG;
+    if (ms[i] < 1 || ms[i] > 256) return ANSLIN_ERR_UNSUPPORTED;
+    const Header &h = w->h;
+    if (h.format != h0.format || h.tile_n != h0.tile_n || ((h.flags ^ h0.flags) & ANSLIN_FLAG_STATE_PAYLOAD)) return ANSLIN_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(xs[i]) | reinterpret_cast<uintptr_t>(ys[i])) & 15) return ANSLIN_ERR_INVALID_ARG;
+    if (scaled && !x_scales[i]) return ANSLIN_ERR_INVALID_ARG;
+    if (ldx[i] < int64_t(h.k_in) || (ldx[i] * xb) % 16 || ldy[i] < int64_t(h.n_out)) return ANSLIN_ERR_INVALID_ARG;
+    mpad_max = std::max(mpad_max, mpad_of(ms[i]));
+    work[i] = uint64_t(h.n_out) * h.k_in;
+    work_sum += work[i];
+  }
+  FusedParams p;
+  TensorMaps tms;
+  memset(&p, 0, sizeof(p));
+  p.nprob = uint32_t(n);
+  p.slot_bytes = kUnitBytes + mpad_max * 32u;
+  p.tmem_cols = tmem_cols_of(mpad_max);
+  const int RB = int(h0.tile_n) / 32, J = RB == 1 ? kJ32 : 1, NW = 4 / (RB * J);
+  // shared memory: U operand slots, D*J stream rings, slot table, barriers
+  const size_t fixed = 2048 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 80 + 4 * kMaxSlots + 16;
   uint32_t D = kMaxDecWarps, U = 0;
-  const char *denv = getenv("ANSLIN_DECODER_WARPS");
-  if (denv && atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
-  if (!getenv("ANSLIN_DMAX")) {  // even rounds: a CTA with tpc tiles needs ceil(tpc/D) tile-times; use the fewest warps that keep that count
-    const uint32_t tpc = (h.n_tiles + grid - 1) / grid, rounds = (tpc + D - 1) / D;
-    D = std::max(1u, (tpc + rounds - 1) / rounds);
+  if (const char *denv = getenv("ANSLIN_DECODER_WARPS"))
+    if (atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
+  D -= D % NW;
+  for (; D >= uint32_t(NW); D -= NW) {
+    const size_t rings = size_t(D) * J * kStreamSmem;
+    if (kSmemMax < fixed + rings) continue;
+    U = uint32_t(std::min<size_t>((kSmemMax - fixed - rings) / p.slot_bytes, kMaxSlots));
+    if (U >= D / NW + 2) break;
   }
-  for (;; --D) {
-    const size_t left = kSmemMax - fixed - size_t(D) * kRingBytes;
-    U = uint32_t(std::min<size_t>(left / p.slot_bytes, kMaxSlots));
-    if (U >= D + 2 || D == 1) break;
-  }
-  if (U < 2) return ANSLIN_ERR_UNSUPPORTED;
+  if (D < uint32_t(NW) || U < 3) return ANSLIN_ERR_UNSUPPORTED;
   p.D = D;
   p.U = U;
-  const size_t smem = fixed + size_t(D) * kRingBytes + size_t(U) * p.slot_bytes;
-  const Workspace ws = workspace_layout(stripes, grid, p.mpad);
-  if (workspace_bytes < ws.total) return ANSLIN_ERR_BUFFER_TOO_SMALL;
-  p.counters = reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(workspace_dev) + ws.counters_off);
-  p.partials = reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(workspace_dev) + ws.partials_off);
-  if (cudaMemsetAsync(p.counters, 0, size_t(stripes) * 4, st) != cudaSuccess) return ANSLIN_ERR_CUDA;
-
-  CUtensorMap tmx;
-  const uint32_t uk = unit_k_of(h.format);
-  const bool ok = p.layout == kLayoutSW32
-                      ? make_map_2d(&tmx, x_dev, xb, h.k_in, uint64_t(m), uint64_t(ldx), uk, p.mpad, CU_TENSOR_MAP_SWIZZLE_32B)
-                      : make_map_2d(&tmx, x_dev, xb, h.k_in, uint64_t(m), uint64_t(ldx), uk / 2, p.mpad, CU_TENSOR_MAP_SWIZZLE_NONE);
-  if (!ok) return ANSLIN_ERR_CUDA;
-  const bool pay = h.flags & ANSLIN_FLAG_STATE_PAYLOAD;
-  switch (h.format) {
-    case ANSLIN_FMT_BF16:
-      return pay ? launch_fused<ANSLIN_FMT_BF16, true>(w, tmx, p, grid, smem, st) : launch_fused<ANSLIN_FMT_BF16, false>(w, tmx, p, grid, smem, st);
-    case ANSLIN_FMT_FP8_E4M3: return launch_fused<ANSLIN_FMT_FP8_E4M3, false>(w, tmx, p, grid, smem, st);
-    case ANSLIN_FMT_INT8: return launch_fused<ANSLIN_FMT_INT8, false>(w, tmx, p, grid, smem, st);
-    case ANSLIN_FMT_INT4_AWQ: return launch_fused<ANSLIN_FMT_INT4_AWQ, false>(w, tmx, p, grid, smem, st);
+  const size_t smem = fixed + size_t(D) * J * kStreamSmem + size_t(U) * p.slot_bytes;
+  // CTAs: one per SM in total, shared out in proportion to the problems' sizes (each at least one, at most one per group)
+  const uint32_t S = uint32_t(sm_budget());
+  uint32_t ncta[kMaxProblems], used = 0;
+  for (int i = 0; i < n; ++i) {
+    const Header &h = ws[i]->h;
+    const uint32_t groups = (h.n_out / kTileN) * (h.k_in / h.tile_k);
+    ncta[i] = uint32_t(std::min<uint64_t>(groups, std::max<uint64_t>(1, uint64_t(S) * work[i] / work_sum)));
+    used += ncta[i];
   }
+  for (bool grown = true; used < S && grown;) {  // hand out what rounding left over, largest work per CTA first
+    grown = false;
+    int best = -1;
+    for (int i = 0; i < n; ++i) {
+      const Header &h = ws[i]->h;
+      const uint32_t groups = (h.n_out / kTileN) * (h.k_in / h.tile_k);
+      if (ncta[i] >= groups) continue;
+      if (best < 0 || work[i] * ncta[best] > work[best] * ncta[i]) best = i;
+    }
+    if (best >= 0) { ++ncta[best]; ++used; grown = true; }
+  }
+  // workspace: counters of all problems, then partials carved by the CTAs each problem got
+  size_t off = 0;
+  uint8_t *wsb = static_cast<uint8_t *>(workspace_dev);
+  size_t counters_bytes = 0;
+  for (int i = 0; i < n; ++i) counters_bytes += align16(size_t(ws[i]->h.n_out / kTileN) * 4 + 256);
+  size_t part_off = counters_bytes;
+  uint32_t cta0 = 0;
+  for (int i = 0; i < n; ++i) {
+    const Header &h = ws[i]->h;
+    Problem &q = p.prob[i];
+    q.cv = view_of(ws[i]);
+    q.x_scale = static_cast<const float *>(x_scales ? x_scales[i] : nullptr);
+    q.y = static_cast<float *>(ys[i]);
+    q.ldy = ldy[i];
+    q.m = uint32_t(ms[i]);
+    q.mpad = mpad_of(ms[i]);
+    q.cta0 = cta0;
+    q.ncta = ncta[i];
+    cta0 += ncta[i];
+    q.counters = reinterpret_cast<uint32_t *>(wsb + off);
+    off += align16(size_t(h.n_out / kTileN) * 4 + 256);
+    q.partials = reinterpret_cast<uint32_t *>(wsb + part_off);
+    part_off += size_t(ncta[i]) * 2 * q.mpad * kTileN * 4;
+    const uint32_t uk = unit_k_of(h.format);
+    if (!make_map_2d(&tms.m[i], xs[i], xb, h.k_in, uint64_t(ms[i]), uint64_t(ldx[i]), uk, q.mpad, CU_TENSOR_MAP_SWIZZLE_32B))
+      return ANSLIN_ERR_CUDA;
+  }
+  if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
+  if (cudaMemsetAsync(wsb, 0, counters_bytes, st) != cudaSuccess) return ANSLIN_ERR_CUDA;
+  const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
+  const uint32_t grid = cta0;
+#define ANSLIN_LAUNCH(F, PAY) (RB == 1 ? launch_fused<F, 1, PAY>(tms, p, grid, smem, st) : launch_fused<F, 4, PAY>(tms, p, grid, smem, st))
+  switch (h0.format) {
+    case ANSLIN_FMT_BF16: return pay ? ANSLIN_LAUNCH(ANSLIN_FMT_BF16, true) : ANSLIN_LAUNCH(ANSLIN_FMT_BF16, false);
+    case ANSLIN_FMT_FP8_E4M3: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);
+    case ANSLIN_FMT_INT8: return ANSLIN_LAUNCH(ANSLIN_FMT_INT8, false);
+    case ANSLIN_FMT_INT4_AWQ: return ANSLIN_LAUNCH(ANSLIN_FMT_INT4_AWQ, false);
+  }
+#undef ANSLIN_LAUNCH
   return ANSLIN_ERR_UNSUPPORTED;
 }
 
-template <uint32_t FMT, bool PAYLOAD>
-int launch_decode(const ContainerView &cv, void *out, cudaStream_t st) {
+size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_max) {
+  if (!ws || n < 1 || m_max < 1 || m_max > 256) return 0;
+  size_t counters = 0;
+  for (int i = 0; i < n; ++i) {
+    if (!ws[i]) return 0;
+    counters += align16(size_t(ws[i]->h.n_out / kTileN) * 4 + 256);
+  }
+  // all problems of a launch share one CTA per SM, so their partials never exceed one problem's worst case
+  const size_t per_launch = size_t(std::max(sm_budget(), 148)) * 2 * mpad_of(m_max) * kTileN * 4;
+  return counters + per_launch;
+}
+
+template <uint32_t FMT, int RB, bool PAYLOAD>
+int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   uint32_t per_sm = 4;
   if (const char *e = getenv("ANSLIN_DECODE_CTAS_PER_SM")) per_sm = uint32_t(std::max(1, atoi(e)));  // debug knob
-  const uint32_t ctas = std::min<uint32_t>((cv.n_tiles + kDecWarps - 1) / kDecWarps, uint32_t(std::max(1, num_sms())) * per_sm);
-  decode_kernel<FMT, PAYLOAD><<<ctas, kDecWarps * 32, 0, st>>>(cv, static_cast<uint8_t *>(out));
+  constexpr int J = RB == 1 ? kJ32 : 1;
+  const uint32_t jobs = cv.n_tiles / J;
+  const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
+  auto kern = decode_kernel<FMT, RB, J, PAYLOAD>;
+  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * kStreamSmem;
+  static thread_local bool attr_set = false;   // per instantiation
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
+    attr_set = true;
+  }
+  kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out));
   ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
+}
+template <uint32_t FMT, bool PAYLOAD>
+int launch_decode(const ContainerView &cv, void *out, cudaStream_t st) {
+  return cv.tile_n == 32 ? launch_decode_t<FMT, 1, PAYLOAD>(cv, out, st) : launch_decode_t<FMT, 4, PAYLOAD>(cv, out, st);
 }
 
 template <uint32_t FMT>
@@ -772,8 +885,7 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
   if (!w || !w->dev || !w_out_dev) return ANSLIN_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(w_out_dev) & 15) return ANSLIN_ERR_INVALID_ARG;
   const Header &h = w->h;
-  const size_t need = h.format == ANSLIN_FMT_BF16 ? size_t(h.n_out) * h.k_in * 2
-                      : h.format == ANSLIN_FMT_INT4_AWQ ? size_t(h.n_out) * h.k_in / 2 : size_t(h.n_out) * h.k_in;
+  const size_t need = size_t(h.n_out) * row_bytes_of(h.format, h.k_in);
   if (capacity < need) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
   const ContainerView cv = view_of(w);
@@ -789,37 +901,69 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
   return ANSLIN_ERR_UNSUPPORTED;
 }
 
-size_t anslin_gemm_workspace_bytes(const anslin_weight *w, int32_t m) {
-  if (!w || m < 1 || m > 256) return 0;
-  return workspace_layout(w->h.n_out / kTileN, uint32_t(std::max(1, std::max(num_sms(), 148))), mpad_of(m)).total;
+size_t anslin_gemm_workspace_bytes(const anslin_weight *w, int32_t m) { return multi_workspace_bytes(&w, 1, m); }
+
+size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, int32_t n, int32_t m_max) {
+  return multi_workspace_bytes(weights, n, m_max);
 }
 
 int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m, const void *x_scale_dev,
                 void *y_dev, int64_t ldy, void *workspace_dev, size_t workspace_bytes, void *stream) {
   g_launches = 0;
-  return gemm_one(w, x_dev, x_dtype, ldx, m, x_scale_dev, y_dev, ldy, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
+  if (!w) return ANSLIN_ERR_INVALID_ARG;
+  return gemm_launch(1, &w, &x_dev, x_dtype, &ldx, &m, &x_scale_dev, &y_dev, &ldy, workspace_dev, workspace_bytes,
+                     static_cast<cudaStream_t>(stream));
+}
+
+int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
+                      const int32_t *m, const void *const *x_scale_dev, void *const *y_dev, const int64_t *ldy, void *workspace_dev,
+                      size_t workspace_bytes, void *stream) {
+  g_launches = 0;
+  if (!weights || n < 1 || !x_dev || !ldx || !m || !y_dev || !ldy) return ANSLIN_ERR_INVALID_ARG;
+  const void *no_scales[kMaxProblems] = {nullptr};
+  for (int32_t i0 = 0; i0 < n; i0 += kMaxProblems) {   // more than kMaxProblems: consecutive launches on the same stream
+    const int cnt = std::min<int32_t>(kMaxProblems, n - i0);
+    int rc = gemm_launch(cnt, weights + i0, x_dev + i0, x_dtype, ldx + i0, m + i0, x_scale_dev ? x_scale_dev + i0 : no_scales, y_dev + i0,
+                         ldy + i0, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
+    if (rc != ANSLIN_OK) return rc;
+  }
+  return ANSLIN_OK;
 }
 
 int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts, const int32_t *rows_per_expert_host,
                         const void *x_dev, uint32_t x_dtype, int64_t ldx, const void *x_scale_dev, void *y_dev, int64_t ldy,
                         void *workspace_dev, size_t workspace_bytes, void *stream) {
   g_launches = 0;
-  if (!experts || n_experts < 1 || !rows_per_expert_host) return ANSLIN_ERR_INVALID_ARG;
+  if (!experts || n_experts < 1 || !rows_per_expert_host || !x_dev || !y_dev) return ANSLIN_ERR_INVALID_ARG;
+  // active experts -> problems of one persistent launch (kMaxProblems per launch)
+  const anslin_weight *w[kMaxProblems];
+  const void *xs[kMaxProblems], *xsc[kMaxProblems];
+  void *ys[kMaxProblems];
+  int64_t ldxs[kMaxProblems], ldys[kMaxProblems];
+  int32_t ms[kMaxProblems];
+  int cnt = 0;
   int64_t row = 0;
-  for (int e = 0; e < n_experts; ++e) {
+  for (int e = 0; e <= n_experts; ++e) {
+    if (e == n_experts || cnt == kMaxProblems) {
+      if (cnt > 0) {
+        int rc = gemm_launch(cnt, w, xs, x_dtype, ldxs, ms, xsc, ys, ldys, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
+        if (rc != ANSLIN_OK) return rc;
+      }
+      cnt = 0;
+      if (e == n_experts) break;
+    }
     const int32_t rows = rows_per_expert_host[e];
     if (rows < 0 || !experts[e]) return ANSLIN_ERR_INVALID_ARG;
     if (rows == 0) continue;
     const Header &h = experts[e]->h;
     if (h.format != experts[0]->h.format || h.n_out != experts[0]->h.n_out || h.k_in != experts[0]->h.k_in) return ANSLIN_ERR_INVALID_ARG;
     const int xb = (h.format == ANSLIN_FMT_BF16 || h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
-    const uint8_t *xe = static_cast<const uint8_t *>(x_dev) + size_t(row) * ldx * xb;
-    const float *xs = x_scale_dev ? static_cast<const float *>(x_scale_dev) + row : nullptr;
-    float *ye = static_cast<float *>(y_dev) + size_t(row) * ldy;
-    // Y/X row offsets keep 16-byte alignment only if the row pitch does; require it
-    if ((reinterpret_cast<uintptr_t>(xe) | reinterpret_cast<uintptr_t>(ye)) & 15) return ANSLIN_ERR_INVALID_ARG;
-    int rc = gemm_one(experts[e], xe, x_dtype, ldx, rows, xs, ye, ldy, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
-    if (rc != ANSLIN_OK) return rc;
+    w[cnt] = experts[e];
+    xs[cnt] = static_cast<const uint8_t *>(x_dev) + size_t(row) * ldx * xb;   // row offsets keep 16-byte alignment only if the pitch does
+    xsc[cnt] = x_scale_dev ? static_cast<const float *>(x_scale_dev) + row : nullptr;
+    ys[cnt] = static_cast<float *>(y_dev) + size_t(row) * ldy;
+    ldxs[cnt] = ldx; ldys[cnt] = ldy; ms[cnt] = rows;
+    ++cnt;
     row += rows;
   }
   return ANSLIN_OK;
@@ -857,7 +1001,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   p.KB = k_in / ke;
   p.stage_bytes = 16384 + p.mpad * 128u;
   p.tmem_cols = tmem_cols_of(p.mpad);
-  const size_t fixed = 1024 + 16 * kMaxSlots + 64;
+  const size_t fixed = 1024 + 16 * kMaxSlots + 96;
   p.S = uint32_t(std::min<size_t>((kSmemMax - fixed) / p.stage_bytes, 12));
   const size_t smem = fixed + size_t(p.S) * p.stage_bytes;
   const uint32_t stripes = n_out / kTileN, T = stripes * p.KB, grid = grid_of(T, 8);

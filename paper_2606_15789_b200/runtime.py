@@ -69,11 +69,37 @@ class DeviceWeight:
         return y
 
 
+class MultiGemm:
+    """anslin_gemm_multi over weights that share format and tile geometry: ONE persistent launch for
+    e.g. q/k/v (same X) or gate/up.  Buffers and the marshalled call are built once."""
+
+    def __init__(self, dws, xs, x_scales=None, ys=None):
+        self.dws, self.xs = list(dws), list(xs)
+        dev = self.xs[0].device
+        ms = [int(x.shape[0]) for x in self.xs]
+        self.ys = list(ys) if ys is not None else [torch.empty((m, d.n_out), dtype=torch.float32, device=dev)
+                                                   for m, d in zip(ms, self.dws)]
+        self.x_scales = x_scales
+        need = B.anslin_gemm_multi_workspace_bytes([d.weight for d in self.dws], max(ms))
+        self.ws = torch.empty(need, dtype=torch.uint8, device=dev)
+        self.call = B.MultiCall([d.weight for d in self.dws], [x.data_ptr() for x in self.xs], B.X_DTYPE[self.dws[0].fmt],
+                                [x.stride(0) for x in self.xs], ms,
+                                None if x_scales is None else [s.data_ptr() for s in x_scales],
+                                [y.data_ptr() for y in self.ys], [y.stride(0) for y in self.ys], self.ws.data_ptr(), self.ws.numel())
+
+    def __call__(self):
+        self.call(_stream())
+        return self.ys
+
+
 def gemm_grouped(experts, rows_per_expert, x: torch.Tensor, x_scale: torch.Tensor | None, y: torch.Tensor | None = None):
     m = x.shape[0]
     if y is None:
         y = torch.empty((m, experts[0].n_out), dtype=torch.float32, device=x.device)
-    ws = experts[0].workspace(int(max(max(rows_per_expert), 1)))
+    need = B.anslin_gemm_multi_workspace_bytes([e.weight for e in experts], int(max(max(rows_per_expert), 1)))
+    ws = experts[0]._ws
+    if ws is None or ws.numel() < need:
+        ws = experts[0]._ws = torch.empty(need, dtype=torch.uint8, device=x.device)
     B.anslin_gemm_grouped([e.weight for e in experts], rows_per_expert, x.data_ptr(), B.X_DTYPE[experts[0].fmt], x.stride(0),
                           None if x_scale is None else x_scale.data_ptr(), y.data_ptr(), y.stride(0), ws.data_ptr(), ws.numel(), _stream())
     return y

@@ -47,6 +47,13 @@ def _decode_cases():
     p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(256, 768, seed=44, outliers=False), 128)
     yield "int4", B.FMT_INT4_AWQ, p4, 768, dict(tile_k=256, scales=s4, zeros=z4, group_size=128)
     yield "bf16-constant", B.FMT_BF16, np.full((128, 64), 0xBF80, dtype=np.uint16), 64, dict(tile_k=64)
+    # 32-row tiles (four per MMA stripe), two tiles interleaved per warp
+    yield "bf16-32x128-payload", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 640, dict(tile_k=128, flags=1, tile_n=32)
+    yield "bf16-32x64", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 640, dict(tile_k=64, tile_n=32)
+    yield "int8-32x256", B.FMT_INT8, q8, 768, dict(tile_k=256, scales=s8, tile_n=32)
+    yield "fp8-32x384", B.FMT_FP8_E4M3, f8, 768, dict(tile_k=384, w_scale=sc, tile_n=32)
+    yield "int4-32x256", B.FMT_INT4_AWQ, p4, 768, dict(tile_k=256, scales=s4, zeros=z4, group_size=128, tile_n=32)
+    yield "bf16-constant-32", B.FMT_BF16, np.full((128, 64), 0xBF80, dtype=np.uint16), 64, dict(tile_k=64, tile_n=32)
 
 
 @pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_decode_cases()), ids=[c[0] for c in _decode_cases()])
@@ -73,14 +80,18 @@ def test_decode_config1_full():
 
 
 # ------------------------------------------------------------------ fused GEMM (a4-a10)
+TILES = [(128, 64), (32, 256)]      # (tile_n, bf16 tile_k): BASELINE config 1's 128 x 64 and the 32-row shape bench.py uses
+
+
 @pytest.mark.parametrize("m", [1, 8, 16, 47, 75])
 @pytest.mark.parametrize("flags", [0, 1])
-def test_gemm_bf16(m, flags):
+@pytest.mark.parametrize("tile", TILES, ids=["128x64", "32x256"])
+def test_gemm_bf16(m, flags, tile):
     rt = _rt()
-    n, k = 640, 1024      # 5 stripes x 16 k-tiles: spans several CTAs and split-K segments
+    n, k = 640, 1024      # 5 stripes x 16 (4) k-tiles: spans several CTAs and split-K segments
     w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=51, jitter=True))
     x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=52))
-    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=flags)
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=flags, tile_n=tile[0])
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
     y_ref, a_ref = og.gemm_bf16(x, w)
@@ -88,11 +99,12 @@ def test_gemm_bf16(m, flags):
     dw.close()
 
 
-def test_gemm_config1_and_unit_vector():
+@pytest.mark.parametrize("tile", TILES, ids=["128x64", "32x256"])
+def test_gemm_config1_and_unit_vector(tile):
     """BASELINE config 1 (W 1024x1024 bf16, X 8x1024) and the e_k special case: Y = column k of W exactly."""
     rt = _rt()
     w, x = inputs.config1()
-    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=64, flags=1)
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=tile[1], flags=1, tile_n=tile[0])
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
     check_gemm(y, *og.gemm_bf16(x, w))
@@ -104,14 +116,15 @@ def test_gemm_config1_and_unit_vector():
     dw.close()
 
 
+@pytest.mark.parametrize("tile_n", [128, 32])
 @pytest.mark.parametrize("m", [1, 32, 75])
-def test_gemm_int8(m):
+def test_gemm_int8(m, tile_n):
     rt = _rt()
     import torch
     n, k = 384, 1536
     q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=61, jitter=True))
     xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=62))
-    buf, _ = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=256, scales=s)
+    buf, _ = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=256, scales=s, tile_n=tile_n)
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
     y_ref, a_ref, acc = og.gemm_int8(xq, xs, q, s)
@@ -123,34 +136,38 @@ def test_gemm_int8(m):
     dw.close()
 
 
+@pytest.mark.parametrize("tile_n", [128, 32])
 @pytest.mark.parametrize("m", [1, 20, 64])
-def test_gemm_fp8(m):
+def test_gemm_fp8(m, tile_n):
     rt = _rt()
     import torch
     n, k = 256, 1536
     f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=71, std=0.015, outliers=False))
     x8, xs = inputs.quant_fp8_acts(inputs.acts_f32(m, k, seed=72))
-    buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc)
+    buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc, tile_n=tile_n)
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
     check_gemm(y, *og.gemm_fp8(x8, xs, f8, sc))
     dw.close()
 
 
+@pytest.mark.parametrize("tile_n", [128, 32])
 @pytest.mark.parametrize("m", [1, 16, 64])
-def test_gemm_int4(m):
+def test_gemm_int4(m, tile_n):
     rt = _rt()
     n, k = 256, 1024
     p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=81, outliers=False), 128)
     x = inputs.acts_f32(m, k, seed=82).astype(np.float16)
-    buf, _ = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=256, scales=s4, zeros=z4, group_size=128)
+    buf, _ = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=256 if tile_n == 128 else 512, scales=s4, zeros=z4,
+                                  group_size=128, tile_n=tile_n)
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
     check_gemm(y, *og.gemm_int4(x, p4, s4, z4, 128))
     dw.close()
 
 
-def test_gemm_grouped_fp8():
+@pytest.mark.parametrize("tile_n", [128, 32])
+def test_gemm_grouped_fp8(tile_n):
     """BASELINE config 5 in miniature: 8 experts, top-2 routing, rows sorted by expert."""
     rt = _rt()
     import torch
@@ -161,7 +178,7 @@ def test_gemm_grouped_fp8():
     experts, refs = [], []
     for e in range(E):
         f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=100 + e, std=0.015, outliers=False))
-        buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc)
+        buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc, tile_n=tile_n)
         experts.append(rt.DeviceWeight(buf))
         refs.append((f8, sc))
     y = rt.gemm_grouped(experts, rows, rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
@@ -172,6 +189,27 @@ def test_gemm_grouped_fp8():
             check_gemm(y[r0:r1], *og.gemm_fp8(x8[r0:r1], xs[r0:r1], refs[e][0], refs[e][1]))
         r0 = r1
     for d in experts:
+        d.close()
+
+
+def test_gemm_multi_qkv_shapes():
+    """anslin_gemm_multi: three projections of different shapes that share one input, one launch."""
+    rt = _rt()
+    k, m = 1024, 47
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=95))
+    xd = rt.x_to_device(B.FMT_BF16, x)
+    ws, dws = [], []
+    for i, n in enumerate((640, 128, 256)):
+        w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=96 + i, jitter=True))
+        buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=1, tile_n=32)
+        ws.append(w); dws.append(rt.DeviceWeight(buf))
+    mg = rt.MultiGemm(dws, [xd, xd, xd])
+    ys = [y.cpu().numpy() for y in mg()]
+    for w, y in zip(ws, ys):
+        check_gemm(y, *og.gemm_bf16(x, w))
+    ys2 = [y.cpu().numpy() for y in mg()]
+    assert all(np.array_equal(a, b) for a, b in zip(ys, ys2)), "multi launch must be deterministic"
+    for d in dws:
         d.close()
 
 
@@ -206,15 +244,16 @@ def test_dense_gemm_int8_fp8():
 
 
 # ------------------------------------------------------------------ full-size launch configuration
+@pytest.mark.parametrize("tile", TILES, ids=["128x64", "32x256"])
 @pytest.mark.parametrize("name,n,k,m", [("gate", 13824, 5120, 75), ("down", 5120, 13824, 16), ("k", 1024, 5120, 1)])
-def test_gemm_bf16_full_size_projection(name, n, k, m):
+def test_gemm_bf16_full_size_projection(name, n, k, m, tile):
     """BASELINE config 2 shapes in the launch configuration bench.py times (148 persistent CTAs,
     ~58 tiles per CTA, several ring laps and split-K segments per CTA): decode bit-exact on the
     full tensor, GEMM checked on all M rows x a seeded sample of 1024 output channels."""
     rt = _rt()
     w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=7, jitter=True))
     x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=8))
-    buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=1)
+    buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=1, tile_n=tile[0])
     assert st["bits_per_weight"] - st["entropy_bits_per_symbol"] - st["raw_entropy_bits_per_symbol"] <= 0.1
     dw = rt.DeviceWeight(buf)
     assert np.array_equal(dw.decode().cpu().numpy().view(np.uint16), w)
