@@ -141,6 +141,9 @@ def main():
     ap.add_argument("--impl", default="anslin")
     ap.add_argument("--m", type=int, default=75)
     ap.add_argument("--no-extras", action="store_true", help="skip per-M table, dense comparator, decode-only and CPU legs")
+    ap.add_argument("--tile", default="32x256", help="tile_n x tile_k of the compressed containers (128x64 = BASELINE config 1's shape)")
+    ap.add_argument("--group", default="qkv,o,gateup,down", help="launch grouping of the 7 projections: 'each' = 7 launches, or "
+                    "comma-separated groups out of qkv / q,k,v / gateup / gate,up / o / down (projections that share an input)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -159,30 +162,47 @@ def main():
     # ---- offline stage (untimed): synthesize, compress, upload
     layer = layer_weights()
     containers, stats = [], []
+    tile_n, tile_k = (int(v) for v in args.tile.split("x"))
     for (_, n, k, w) in layer:
-        buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=B.FLAG_STATE_PAYLOAD)
+        buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile_k, flags=B.FLAG_STATE_PAYLOAD, tile_n=tile_n)
         containers.append(buf); stats.append(st)
     dws = [rt.DeviceWeight(c) for c in containers]
     m = args.m
-    xs_host = [torch.from_numpy(inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=ranks.batch_seed(500 + i))).view(np.int16)).pin_memory()
-               for i, (_, n, k, _) in enumerate(layer)]
-    xs = [t.cuda().view(torch.bfloat16) for t in xs_host]
+    # projections that share an input in a decoder layer share the X tensor here too: q/k/v, gate/up
+    share = {"k": "q", "v": "q", "up": "gate"}
+    names = [t[0] for t in layer]
+    x_owner = [names.index(share.get(nm, nm)) for nm in names]
+    xs_host = {i: torch.from_numpy(inputs.f32_to_bf16_bits(inputs.acts_f32(m, layer[i][2], seed=ranks.batch_seed(500 + i))).view(np.int16)).pin_memory()
+               for i in sorted(set(x_owner))}
+    xs_dev = {i: t.cuda().view(torch.bfloat16) for i, t in xs_host.items()}
+    xs = [xs_dev[o] for o in x_owner]
     ys = [torch.empty((m, n), dtype=torch.float32, device="cuda") for (_, n, k, _) in layer]
     ys_host = [torch.empty((m, n), dtype=torch.float32).pin_memory() for (_, n, k, _) in layer]
     flops_step = sum(2.0 * m * n * k for (_, n, k, _) in layer)
     comp_bytes = sum(c.size for c in containers)
-    algo_bytes = [c.size + m * k * 2 + m * n * 4 for c, (_, n, k, _) in zip(containers, layer)]
     n_weights = sum(n * k for (_, n, k, _) in layer)
+    # launch groups: each group is ONE anslin_gemm_multi launch (a single projection = anslin_gemm's launch)
+    alias = {"qkv": ["q", "k", "v"], "gateup": ["gate", "up"]}
+    if args.group == "each":
+        groups = [[i] for i in range(len(layer))]
+    else:
+        groups = [[names.index(nm) for nm in alias.get(g, [g])] for g in args.group.split(",")]
+    assert sorted(i for g in groups for i in g) == list(range(len(layer))), "--group must cover every projection once"
+    calls = [rt.MultiGemm([dws[i] for i in g], [xs[i] for i in g], None, [ys[i] for i in g]) for g in groups]
+    group_names = ["+".join(names[i] for i in g) for g in groups]
+    # algorithmic bytes of a launch: its containers + each distinct X once + its Y
+    algo_bytes = [sum(containers[i].size + m * layer[i][1] * 4 for i in g) + sum(m * layer[o][2] * 2 for o in {x_owner[i] for i in g})
+                  for g in groups]
 
     def step(record=None):
         launches = 0
-        for i, dw in enumerate(dws):
+        for gi, call in enumerate(calls):
             if record is not None:
-                record[i][0].record()
-            dw.gemm(xs[i], None, ys[i])
+                record[gi][0].record()
+            call()
             launches += B.anslin_last_launch_count()
             if record is not None:
-                record[i][1].record()
+                record[gi][1].record()
         return launches
 
     def barrier():
@@ -195,7 +215,7 @@ def main():
         step()
     barrier()
     mark_lo = sampler.mark()
-    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in dws] for _ in range(args.steps)]
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in calls] for _ in range(args.steps)]
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches = 0
     e0.record()
@@ -219,11 +239,12 @@ def main():
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned X in, Y out) inside the timed region
     def step_e2e():
-        for i, dw in enumerate(dws):
-            xd = xs[i]
-            xd.view(torch.int16).copy_(xs_host[i], non_blocking=True)
-            dw.gemm(xd, None, ys[i])
-            ys_host[i].copy_(ys[i], non_blocking=True)
+        for g, call in zip(groups, calls):
+            for o in sorted({x_owner[i] for i in g}):
+                xs_dev[o].view(torch.int16).copy_(xs_host[o], non_blocking=True)
+            call()
+            for i in g:
+                ys_host[i].copy_(ys[i], non_blocking=True)
     for _ in range(3):
         step_e2e()
     barrier()
@@ -233,25 +254,26 @@ def main():
     barrier()
     e2e_s = ranks.max_over_ranks(time.perf_counter() - t0)
     e2e = {"value": world * flops_step * args.steps / e2e_s / 1e12, "unit": UNIT,
-           "h2d_bytes_per_step": int(sum(m * k * 2 for (_, n, k, _) in layer)),
+           "h2d_bytes_per_step": int(sum(t.numel() * 2 for t in xs_host.values())),
            "d2h_bytes_per_step": int(sum(m * n * 4 for (_, n, k, _) in layer))}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
            "data": "synthetic",
-           "config": {"workload": WORKLOAD, "batch_m": m, "tile": "128x64", "streams": 32, "prob_bits": 12,
+           "config": {"workload": WORKLOAD, "batch_m": m, "tile": args.tile, "streams": 32, "prob_bits": 12,
+                      "launch_groups": group_names,
                       "l2_policy": "inputs larger than L2: %.0f MB of compressed weights stream per step" % (comp_bytes / 1e6),
                       "parallelism": "replicas, one batch per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                         "traffic": traffic, "peak_kind": "of " + peak_kind,
-                        "kernel": "fused_gemm_kernel<bf16,payload> (7 launches/step; bytes = container + X + Y)"},
+                        "kernel": "fused_gemm_kernel<bf16,payload> (%d launches/step; bytes = containers + X + Y)" % len(calls)},
            "compressed_gbs": world * comp_bytes / (ms_step * 1e-3) / 1e9,
            "decoded_weights_gbs": world * n_weights * 2 / (ms_step * 1e-3) / 1e9,
            "bits_per_weight": 8.0 * comp_bytes / n_weights,
            "h_sym_bits_per_weight": float(np.sum([(s["entropy_bits_per_symbol"] + s["raw_entropy_bits_per_symbol"]) * s["n_weights"]
                                                   for s in stats]) / n_weights),
-           "per_projection_us": {name: round(1e3 * float(t), 2) for (name, _, _, _), t in zip(layer, kern_ms_mean)}}
+           "per_launch_us": {nm: round(1e3 * float(t), 2) for nm, t in zip(group_names, kern_ms_mean)}}
 
     if rank == 0 and not args.no_extras:
         # per-M table (BASELINE config 2: M in {1,16,47,75}), dense comparator, decode-only; then the CPU oracle leg

@@ -23,7 +23,8 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, *[os.path.join(CSRC, f) for f in SOURCES], "-o", LIB]
+        extra = os.environ.get("ANSLIN_NVCC_EXTRA", "").split()      # developer knob: e.g. -DANSLIN_J32=1
+        cmd = [nvcc, *NVCC_FLAGS, *extra, *[os.path.join(CSRC, f) for f in SOURCES], "-o", LIB]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or r.returncode != 0:
             print(r.stdout + r.stderr)

@@ -161,8 +161,8 @@ __device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint3
       "and.b32 r, m, %2;\n\t"
       "popc.b32 r, r;\n\t"
       "mad.lo.u32 a, r, 2, %1;\n\t"
-      "@p ld.shared.u16 h, [a];\n\t"
-      "@p cvt.u32.u16 w, h;\n\t"
+      "ld.shared.u16 h, [a];\n\t"      // every lane loads (same 64-byte window): keeps w defined on all paths
+      "cvt.u32.u16 w, h;\n\t"
       "@p mad.lo.u32 %0, %0, 65536, w;\n\t"
       "popc.b32 m, m;\n\t"
       "mad.lo.u32 %1, m, 2, %1;\n\t}"

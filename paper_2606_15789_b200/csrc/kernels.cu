@@ -42,23 +42,25 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-// Bounded wait: a protocol bug traps (launch failure) instead of hanging the GPU.
-// kSleepNs > 0 backs off between probes so that long waits (MMA issuer, epilogue) do not steal issue
-// slots from the decoder warps sharing their scheduler.
-template <int kSleepNs = 0>
+#ifndef ANSLIN_WAIT_HINT
+#define ANSLIN_WAIT_HINT 1000000
+#endif
+// Bounded, blocking wait: mbarrier.try_wait suspends the warp in hardware for up to the time hint, so a
+// waiting warp (MMA issuer, epilogue, slot-starved decoder) takes no issue slots from the decoder warps
+// that share its scheduler.  A protocol bug traps (launch failure) instead of hanging the GPU.
+template <int kUnused = 0>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done = 0, spins = 0;
+  uint32_t done = 0, tries = 0;
   while (true) {
-    if (kSleepNs > 0 && spins > 0) __nanosleep(kSleepNs);
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(done)
-        : "r"(bar), "r"(parity)
+        : "r"(bar), "r"(parity), "r"(uint32_t(ANSLIN_WAIT_HINT))
         : "memory");
     if (done) break;
-    if (++spins > (1u << 26)) __trap();
+    if (++tries > (1u << 22)) __trap();
   }
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -105,6 +107,22 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
       : "memory");
   asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
+__device__ __forceinline__ void named_bar_arrive(int id, int nthreads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// non-blocking probe of an mbarrier phase
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return done != 0;
+}
+constexpr int kBarEpiGo = 2;   // named barrier: MMA warp -> epilogue warps, "accumulator is complete"
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -155,7 +173,13 @@ template <int RB, int J> struct TileTraits {
   static_assert((RB == 1 && (J == 1 || J == 2 || J == 4)) || (RB == 4 && J == 1), "unsupported tile / interleave combination");
   static constexpr int Q = 4 / RB /*tiles per (stripe, k-tile) group*/, NW = Q / J /*warps per unit*/;
 };
-constexpr int kJ32 = 2;   // tiles a warp interleaves when tiles have 32 rows
+#ifndef ANSLIN_J32
+#define ANSLIN_J32 2
+#endif
+#ifndef ANSLIN_MAXDEC
+#define ANSLIN_MAXDEC 20
+#endif
+constexpr int kJ32 = ANSLIN_J32;   // tiles a warp interleaves when tiles have 32 rows
 
 __host__ __device__ constexpr size_t row_bytes_of(uint32_t fmt, size_t k) {
   return fmt == ANSLIN_FMT_BF16 ? k * 2 : fmt == ANSLIN_FMT_INT4_AWQ ? k / 2 : k;
@@ -170,10 +194,15 @@ struct GlobalEmit {
   uint8_t *tile_out[J];  // &W[first row of tile j][k0] in bytes
   size_t row_bytes;      // bytes per W row
   int u;
+#ifdef ANSLIN_PROBE_NOSTORE   // developer probe: decode throughput without the HBM stores
+  uint32_t chk = 0;
+  __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) { chk ^= v.x ^ v.y ^ v.z ^ v.w; }
+#else
   __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {  // bf16 / fp8 / int8: 16 B of row-major W
     uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 32 + (g / RB) * 16;
     *reinterpret_cast<uint4 *>(p) = v;
   }
+#endif
   __device__ __forceinline__ void packed(int j, int g, int lane, uint32_t b) const {  // int4: 4 packed bytes = 8 weights
     uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 8 + (g / RB) * 4;
     *reinterpret_cast<uint32_t *>(p) = b;
@@ -215,6 +244,9 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
       emit.u = int(u);
       decode_unit<FMT, RB, J, PAYLOAD>(s, ring_s, smem_u32(tab), lane, lt, int(u), V, raw, sz, emit);
     }
+#ifdef ANSLIN_PROBE_NOSTORE
+    if (emit.chk == 0x12345678u) out[job] = 1;
+#endif
   }
   cp_async_wait_all();
 }
@@ -225,7 +257,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
 constexpr int kEpiWarps = 4;
 constexpr int kMmaWarp = 4;
 constexpr int kFirstDecWarp = 5;
-constexpr int kMaxDecWarps = 20;
+constexpr int kMaxDecWarps = ANSLIN_MAXDEC;
 constexpr int kGemmThreads = 32 * (kFirstDecWarp + kMaxDecWarps);
 constexpr int kMaxSlots = 48;
 
@@ -282,7 +314,9 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     float ws = 1.0f;
     if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n]);
     if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
-    mbar_wait<400>(tfull_s + 8 * ab, (si >> 1) & 1u);
+    // The MMA warp watches the accumulator's mbarrier and releases us through a named barrier: the four
+    // epilogue warps sleep in hardware meanwhile instead of polling next to the decoder warps.
+    named_bar_sync(kBarEpiGo, (kEpiWarps + 1) * 32);
     tc_fence_after();
     const uint32_t seg = (t == t_begin ? 0u : 1u);
     uint32_t *part = p.partials + size_t(c * 2u + seg) * p.mpad * kTileN;
@@ -379,7 +413,7 @@ struct Problem {
 struct FusedParams {
   Problem prob[kMaxProblems];
   uint32_t nprob;
-  uint32_t U, D;           // ring slots, decoder warps
+  uint32_t U, D, B, logB;  // operand slots (= teams * B), decoder warps, slots per team (2 or 4)
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
 };
@@ -394,7 +428,11 @@ struct SmemEmit {
   uint32_t row0[J];      // first stripe row of stream j's tile
   __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {
     const uint32_t row = row0[j] + uint32_t((g % RB) * 32 + lane), c = uint32_t(g / RB);
+#ifndef ANSLIN_DBG_NOSTS
     sts128(slot_a + row * 32u + ((c ^ ((uint32_t(lane) >> 2) & 1u)) << 4), v);  // Swizzle<1,4,3>
+#else
+    if (v.x == 0x12345678u && v.y == 77u) sts128(slot_a, v);
+#endif
   }
   __device__ __forceinline__ void packed(int, int, int, uint32_t) const {}
 };
@@ -425,15 +463,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
                  tempty_s = tfull_s + 16, tmemptr_s = tempty_s + 16;
   volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + bar_off + 16 * kMaxSlots + 32);
   FinSeg *fin = reinterpret_cast<FinSeg *>(smem + bar_off + 16 * kMaxSlots + 48);
-  // lapw[slot] = number of ring laps whose producers have ACQUIRED the slot.  A decoder warp may run
-  // more than one lap ahead of a slot's barrier (idle rounds, segment changes), where an mbarrier
-  // parity wait would alias; it first waits for its predecessor lap to be acquired.
-  const uint32_t lapw_s = smem0 + bar_off + 16 * kMaxSlots + 80;
-
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
   if (threadIdx.x == 0) {
-    for (uint32_t i = 0; i < P.U; ++i) { mbar_init(full_s + 8 * i, NW + 1); mbar_init(empty_s + 8 * i, 1); sts32(lapw_s + 4 * i, 0); }
+    for (uint32_t i = 0; i < P.U; ++i) { mbar_init(full_s + 8 * i, NW + 1); mbar_init(empty_s + 8 * i, 1); }
     for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); fin[i].valid = 0; }
     fence_mbar_init();
   }
@@ -460,13 +493,10 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       // Groups of this CTA are dealt to the teams round-robin over the CTA's WHOLE range (group i ->
       // team i mod PT, round i div PT).  The MMA warp consumes units segment by segment (one
       // accumulator per stripe segment); inside a segment the order is (round, unit, group).
+      uint32_t n_unit = 0;   // units this team has produced so far = (rounds done) * units + u
+#pragma unroll 1
       for (uint32_t i = team; i < t_end - t_begin; i += PT) {
         const uint32_t gt = t_begin + i, stripe = gt / KT, kt = gt % KT;
-        const uint32_t seg_a = max(t_begin, stripe * KT) - t_begin;            // segment = [seg_a, seg_b) in CTA-local groups
-        const uint32_t seg_b = min(t_end, stripe * KT + KT) - t_begin;
-        const uint32_t rho = i / PT;
-        const uint32_t grp_a = max(seg_a, rho * PT), grp_b = min(seg_b, rho * PT + PT);   // this round's groups of the segment
-        const uint32_t seq0 = grp_a * units, cnt = grp_b - grp_a, idx = i - grp_a;
         Stream s[J];
         RawReader<PAYLOAD> raw[J];
         const uint32_t *sz[J];
@@ -480,20 +510,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           emit.row0[j] = q * 32u * RB;
           sz[j] = nullptr;
         }
-        for (uint32_t u = 0; u < units; ++u) {
-          const uint32_t seq = seq0 + u * cnt + idx;
-          const uint32_t slot = seq % P.U, lap = seq / P.U;
+#pragma unroll 1
+        for (uint32_t u = 0; u < units; ++u, ++n_unit) {
+          // team-private slots: unit n of this team lives in slot team*B + n % B (B = P.B buffers per team), so the
+          // only thing a producer ever waits for is the MMA that read ITS OWN slot B units ago.
+          const uint32_t bsel = n_unit & (P.B - 1u), slot = team * P.B + bsel, lap = n_unit >> P.logB;   // B is 2 or 4
           const uint32_t slot_a = slots_s + slot * P.slot_bytes;
-          for (uint32_t spins = 0; lds32v(lapw_s + 4 * slot) < lap;) {  // a waiting decoder sleeps: it must not take issue slots
-            __nanosleep(64);
-            if (++spins > (1u << 24)) __trap();
-          }
-          mbar_wait<64>(empty_s + 8 * slot, (lap & 1u) ^ 1u);
+          mbar_wait(empty_s + 8 * slot, (lap & 1u) ^ 1u);
           const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
           if (hw == 0 && lane == 0) {
-            sts32(lapw_s + 4 * slot, lap + 1u);
+#ifndef ANSLIN_DBG_NOTMA
             mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
             tma_load_2d(slot_a + kUnitBytes, &tms.m[pi], k_elem, 0, full_s + 8 * slot);
+#else
+            mbar_arrive(full_s + 8 * slot);
+#endif
           }
           emit.slot_a = slot_a;
           if (FMT == ANSLIN_FMT_INT4_AWQ) {
@@ -503,7 +534,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
                       size_t(stripe) * kTileN + emit.row0[j];
           }
           decode_unit<FMT, RB, J, PAYLOAD>(s, ring_s, tab_s, lane, lt, int(u), V, raw, sz, emit);
+#ifndef ANSLIN_DBG_NOFENCE
           fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
+#endif
           __syncwarp();
           if (lane == 0) mbar_arrive(full_s + 8 * slot);
         }
@@ -513,27 +546,40 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   } else if (warp == kMmaWarp) {
     // ===================== MMA issuer: one thread drives the tensor core =====================
     const uint32_t idesc = make_idesc(TR::c, TR::ab, TR::ab, 128, mpad);
-    uint32_t seq = 0, si = 0;
+    const uint32_t PT = P.D / NW;
+    uint32_t si = 0, pend = 0, pend_bar = 0, pend_par = 0;   // pend: a committed accumulator not yet handed to the epilogue
     for (uint32_t t = t_begin; t < t_end; ++si) {
       const uint32_t ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
-      mbar_wait<100>(tempty_s + 8 * ab, ((si >> 1) & 1u) ^ 1u);  // epilogue has drained this accumulator
+      mbar_wait(tempty_s + 8 * ab, ((si >> 1) & 1u) ^ 1u);  // epilogue has drained this accumulator
       tc_fence_after();
-      const uint32_t n_units = nt * units;
-      for (uint32_t j = 0; j < n_units; ++j, ++seq) {
-        const uint32_t slot = seq % P.U, par = (seq / P.U) & 1u;
-        mbar_wait<40>(full_s + 8 * slot, par);
-        tc_fence_after();
-        if (lane == 0) {
-          const uint32_t a = slots_s + slot * P.slot_bytes, b = a + kUnitBytes;
-          umma<TR::kind>(tmem_base + ab * mpad, make_smem_desc(a, 16, 256, kLayoutSW32), make_smem_desc(b, 16, 256, kLayoutSW32),
-                         idesc, j > 0 ? 1u : 0u);
-          umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
-          if (j + 1 == n_units) umma_commit(tfull_s + 8 * ab);
+      const uint32_t seg_a = t - t_begin, seg_b = seg_a + nt;   // this stripe segment in CTA-local groups
+      uint32_t first = 1;
+      for (uint32_t rho = seg_a / PT; rho * PT < seg_b; ++rho) {
+        const uint32_t grp_a = max(seg_a, rho * PT), grp_b = min(seg_b, rho * PT + PT);   // this round's groups of the segment
+        for (uint32_t u = 0; u < units; ++u) {
+          const uint32_t n_unit = rho * units + u, bsel = n_unit & (P.B - 1u), par = (n_unit >> P.logB) & 1u;
+          for (uint32_t i = grp_a; i < grp_b; ++i) {
+            const uint32_t slot = (i - rho * PT) * P.B + bsel;
+            if (pend && __all_sync(0xffffffffu, mbar_test(pend_bar, pend_par))) { named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32); pend = 0; }
+            mbar_wait(full_s + 8 * slot, par);
+            tc_fence_after();
+            if (lane == 0) {
+              const uint32_t a = slots_s + slot * P.slot_bytes, b = a + kUnitBytes;
+              umma<TR::kind>(tmem_base + ab * mpad, make_smem_desc(a, 16, 256, kLayoutSW32), make_smem_desc(b, 16, 256, kLayoutSW32),
+                             idesc, first ? 0u : 1u);
+              umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
+              if (rho * PT + PT >= seg_b && u + 1 == units && i + 1 == grp_b) umma_commit(tfull_s + 8 * ab);
+            }
+            first = 0;
+            __syncwarp();
+          }
         }
-        __syncwarp();
       }
+      if (pend) { mbar_wait(pend_bar, pend_par); named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32); }
+      pend = 1; pend_bar = tfull_s + 8 * ab; pend_par = (si >> 1) & 1u;
       t += nt;
     }
+    if (pend) { mbar_wait(pend_bar, pend_par); named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32); }
   } else {
     // ===================== epilogue warps 0..3 =====================
     epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp, lane);
@@ -621,6 +667,8 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
         }
         __syncwarp();
       }
+      mbar_wait(tfull_s + 8 * ab, (si >> 1) & 1u);
+      named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32);
       t += nt;
     }
     (void)UK;
@@ -753,20 +801,26 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   p.tmem_cols = tmem_cols_of(mpad_max);
   const int RB = int(h0.tile_n) / 32, J = RB == 1 ? kJ32 : 1, NW = 4 / (RB * J);
   // shared memory: U operand slots, D*J stream rings, slot table, barriers
-  const size_t fixed = 2048 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 80 + 4 * kMaxSlots + 16;
+  const size_t fixed = 2048 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 96;
   uint32_t D = kMaxDecWarps, U = 0;
   if (const char *denv = getenv("ANSLIN_DECODER_WARPS"))
     if (atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
   D -= D % NW;
-  for (; D >= uint32_t(NW); D -= NW) {
+  uint32_t Bslots = 0;
+  for (; D >= uint32_t(NW); D -= NW) {   // most decoder warps that still leave every team two private operand slots
     const size_t rings = size_t(D) * J * kStreamSmem;
     if (kSmemMax < fixed + rings) continue;
-    U = uint32_t(std::min<size_t>((kSmemMax - fixed - rings) / p.slot_bytes, kMaxSlots));
-    if (U >= D / NW + 2) break;
+    const uint32_t PT = D / NW;
+    Bslots = uint32_t(std::min<size_t>((kSmemMax - fixed - rings) / p.slot_bytes, kMaxSlots) / PT);
+    if (Bslots >= 2) break;
   }
-  if (D < uint32_t(NW) || U < 3) return ANSLIN_ERR_UNSUPPORTED;
+  if (D < uint32_t(NW) || Bslots < 2) return ANSLIN_ERR_UNSUPPORTED;
+  Bslots = Bslots >= 4 ? 4u : 2u;
+  U = (D / NW) * Bslots;
   p.D = D;
   p.U = U;
+  p.B = Bslots;
+  p.logB = Bslots == 4 ? 2u : 1u;
   const size_t smem = fixed + size_t(D) * J * kStreamSmem + size_t(U) * p.slot_bytes;
   // CTAs: one per SM in total, shared out in proportion to the problems' sizes (each at least one, at most one per group)
   const uint32_t S = uint32_t(sm_budget());
