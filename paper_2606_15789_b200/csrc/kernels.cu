@@ -320,6 +320,9 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     tc_fence_after();
     const uint32_t seg = (t == t_begin ? 0u : 1u);
     uint32_t *part = p.partials + size_t(c * 2u + seg) * p.mpad * kTileN;
+#ifdef ANSLIN_DBG_NOEPI
+    if (false)
+#endif
     for (uint32_t c0 = 0; c0 < p.mpad; c0 += 16) {
       uint32_t v[16];
       tmem_ld16(tmem_base + ((uint32_t(warp) * 32u) << 16) + ab * p.mpad + c0, v);
@@ -335,10 +338,13 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(tempty_s + 8 * ab);
+#ifdef ANSLIN_DBG_NOEPI
+    if (false)
+#endif
     if (!whole) {
       __threadfence();
       named_bar_sync(1, kEpiWarps * 32);
-      if (threadIdx.x == 0) {
+      if (warp == 0 && lane == 0) {
         const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
         const bool last = atomicAdd(&p.counters[stripe], 1u) == c_last - c_first;
         __threadfence();
@@ -413,7 +419,7 @@ struct Problem {
 struct FusedParams {
   Problem prob[kMaxProblems];
   uint32_t nprob;
-  uint32_t U, D, B, logB;  // operand slots (= teams * B), decoder warps, slots per team (2 or 4)
+  uint32_t U, D, B;        // operand slots (= teams * B), decoder warps, slots per team (>= 2)
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
 };
@@ -470,7 +476,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); fin[i].valid = 0; }
     fence_mbar_init();
   }
-  if (warp == 0) tmem_alloc(tmemptr_s, P.tmem_cols);
+  if (warp == int(P.D) + kEpiWarps) tmem_alloc(tmemptr_s, P.tmem_cols);
   tc_fence_before();
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));  // ends with __syncthreads()
   tc_fence_after();
@@ -480,10 +486,14 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, pr.y, pr.ldy,
                      pr.partials, pr.counters, pr.m, mpad};
 
-  if (warp >= kFirstDecWarp) {
-    // ===================== decoder warps: Alg V.2 into the operand ring =====================
-    const uint32_t d = uint32_t(warp - kFirstDecWarp);
-    if (d < P.D) {
+  // Warp roles: decoders 0..D-1, epilogue D..D+3 (TMEM lane quadrant = warp % 4), MMA issuer D+4.  The
+  // scheduler favours high warp ids, so the MMA issuer reacts first: a finished unit is consumed and its
+  // slot handed back to the decoders with the least delay.
+  const int epi0 = int(P.D), mma_warp = int(P.D) + kEpiWarps;
+  if (warp < epi0) {
+    // ===================== decoder warps: Alg V.2 into the operand slots =====================
+    const uint32_t d = uint32_t(warp);
+    {
       const uint32_t PT = P.D / NW, team = d / NW, hw = d % NW;   // teams of NW warps fill one 128-row unit together
       const uint32_t lt = lanemask_lt(), ring_s = smem0 + ring_off + d * J * kStreamSmem, tab_s = smem0 + tab_off;
       const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
@@ -493,7 +503,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       // Groups of this CTA are dealt to the teams round-robin over the CTA's WHOLE range (group i ->
       // team i mod PT, round i div PT).  The MMA warp consumes units segment by segment (one
       // accumulator per stripe segment); inside a segment the order is (round, unit, group).
-      uint32_t n_unit = 0;   // units this team has produced so far = (rounds done) * units + u
+      uint32_t bsel = 0, bpar = 1;   // this team's next private slot (unit count mod B) and the parity its empty barrier must have passed
 #pragma unroll 1
       for (uint32_t i = team; i < t_end - t_begin; i += PT) {
         const uint32_t gt = t_begin + i, stripe = gt / KT, kt = gt % KT;
@@ -511,13 +521,17 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           sz[j] = nullptr;
         }
 #pragma unroll 1
-        for (uint32_t u = 0; u < units; ++u, ++n_unit) {
+        for (uint32_t u = 0; u < units; ++u) {
           // team-private slots: unit n of this team lives in slot team*B + n % B (B = P.B buffers per team), so the
           // only thing a producer ever waits for is the MMA that read ITS OWN slot B units ago.
-          const uint32_t bsel = n_unit & (P.B - 1u), slot = team * P.B + bsel, lap = n_unit >> P.logB;   // B is 2 or 4
+          const uint32_t slot = team * P.B + bsel;
           const uint32_t slot_a = slots_s + slot * P.slot_bytes;
-          mbar_wait(empty_s + 8 * slot, (lap & 1u) ^ 1u);
+#ifndef ANSLIN_DBG_DECONLY
+          mbar_wait(empty_s + 8 * slot, bpar);
+#endif
+          if (++bsel == P.B) { bsel = 0; bpar ^= 1u; }
           const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
+#ifndef ANSLIN_DBG_DECONLY
           if (hw == 0 && lane == 0) {
 #ifndef ANSLIN_DBG_NOTMA
             mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
@@ -526,6 +540,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
             mbar_arrive(full_s + 8 * slot);
 #endif
           }
+#endif
           emit.slot_a = slot_a;
           if (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll
@@ -538,55 +553,88 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
 #endif
           __syncwarp();
+#ifndef ANSLIN_DBG_DECONLY
           if (lane == 0) mbar_arrive(full_s + 8 * slot);
+#endif
         }
       }
       cp_async_wait_all();
     }
-  } else if (warp == kMmaWarp) {
+  } else if (warp == mma_warp) {
     // ===================== MMA issuer: one thread drives the tensor core =====================
     const uint32_t idesc = make_idesc(TR::c, TR::ab, TR::ab, 128, mpad);
-    const uint32_t PT = P.D / NW;
-    uint32_t si = 0, pend = 0, pend_bar = 0, pend_par = 0;   // pend: a committed accumulator not yet handed to the epilogue
-    for (uint32_t t = t_begin; t < t_end; ++si) {
-      const uint32_t ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
-      mbar_wait(tempty_s + 8 * ab, ((si >> 1) & 1u) ^ 1u);  // epilogue has drained this accumulator
-      tc_fence_after();
-      const uint32_t seg_a = t - t_begin, seg_b = seg_a + nt;   // this stripe segment in CTA-local groups
-      uint32_t first = 1;
-      for (uint32_t rho = seg_a / PT; rho * PT < seg_b; ++rho) {
-        const uint32_t grp_a = max(seg_a, rho * PT), grp_b = min(seg_b, rho * PT + PT);   // this round's groups of the segment
+    const uint32_t PT = P.D / NW, N = t_end - t_begin;
+    // Consumption order: rounds of PT groups; inside a round, units ascending and groups ascending, with
+    // up to TWO stripe segments of the round interleaved (they own different TMEM accumulators), so the
+    // teams of a round never wait for one another's whole tile at a stripe boundary.  The order is fixed
+    // by the shape alone: accumulation is bit-reproducible.
+    uint32_t n_commit = 0, rel = 0;   // segments whose accumulator has been committed / handed to the epilogue
+    auto release = [&](uint32_t upto, bool block) {   // hand finished accumulators to the epilogue, in segment order
+      while (rel < upto && rel < n_commit) {
+        const uint32_t bar = tfull_s + 8 * (rel & 1u), par = (rel >> 1) & 1u;
+        if (block) mbar_wait(bar, par);
+        else if (!__all_sync(0xffffffffu, mbar_test(bar, par))) break;
+        named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32);
+        ++rel;
+      }
+    };
+    const uint32_t stripe0 = t_begin / KT;
+#ifdef ANSLIN_DBG_DECONLY
+    if (false)
+#endif
+    for (uint32_t rho = 0; rho * PT < N; ++rho) {
+      const uint32_t ga = rho * PT, gb = min(N, ga + PT);
+      for (uint32_t i0 = ga; i0 < gb;) {
+        // run 1 = groups [i0, e1) of segment s1, run 2 = groups [e1, e2) of segment s1 + 1 (may be empty)
+        const uint32_t s1 = (t_begin + i0) / KT - stripe0;
+        const uint32_t e1 = min(gb, (stripe0 + s1 + 1) * KT - t_begin), e2 = min(gb, (stripe0 + s1 + 2) * KT - t_begin);
+        for (uint32_t sg = s1; sg <= s1 + 1; ++sg) {   // segments that START in this window need a drained accumulator
+          const uint32_t first_grp = sg == 0 ? 0u : (stripe0 + sg) * KT - t_begin;
+          if (first_grp < i0 || first_grp >= e2) continue;
+          if (sg >= 2) release(sg - 1, true);
+          mbar_wait(tempty_s + 8 * (sg & 1u), ((sg >> 1) & 1u) ^ 1u);
+          tc_fence_after();
+        }
         for (uint32_t u = 0; u < units; ++u) {
-          const uint32_t n_unit = rho * units + u, bsel = n_unit & (P.B - 1u), par = (n_unit >> P.logB) & 1u;
-          for (uint32_t i = grp_a; i < grp_b; ++i) {
-            const uint32_t slot = (i - rho * PT) * P.B + bsel;
-            if (pend && __all_sync(0xffffffffu, mbar_test(pend_bar, pend_par))) { named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32); pend = 0; }
+          const uint32_t n_unit = rho * units + u, bsel = n_unit % P.B, par = (n_unit / P.B) & 1u;
+          for (uint32_t i = i0; i < e2; ++i) {
+            const uint32_t sg = i < e1 ? s1 : s1 + 1, ab = sg & 1u;
+            const uint32_t seg_first = sg == 0 ? 0u : (stripe0 + sg) * KT - t_begin, seg_last = min(N, (stripe0 + sg + 1) * KT - t_begin) - 1;
+            const uint32_t slot = (i - ga) * P.B + bsel;
+            release(n_commit, false);
             mbar_wait(full_s + 8 * slot, par);
             tc_fence_after();
+            const bool last = (u + 1 == units && i == seg_last);
             if (lane == 0) {
               const uint32_t a = slots_s + slot * P.slot_bytes, b = a + kUnitBytes;
+#ifndef ANSLIN_DBG_NOMMA
               umma<TR::kind>(tmem_base + ab * mpad, make_smem_desc(a, 16, 256, kLayoutSW32), make_smem_desc(b, 16, 256, kLayoutSW32),
-                             idesc, first ? 0u : 1u);
+                             idesc, (u == 0 && i == seg_first) ? 0u : 1u);
               umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
-              if (rho * PT + PT >= seg_b && u + 1 == units && i + 1 == grp_b) umma_commit(tfull_s + 8 * ab);
+              if (last) umma_commit(tfull_s + 8 * ab);
+#else
+              (void)a; (void)b; (void)idesc;
+              mbar_arrive(empty_s + 8 * slot);
+              if (last) mbar_arrive(tfull_s + 8 * ab);
+#endif
             }
-            first = 0;
+            if (last) ++n_commit;
             __syncwarp();
           }
         }
+        i0 = e2;
       }
-      if (pend) { mbar_wait(pend_bar, pend_par); named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32); }
-      pend = 1; pend_bar = tfull_s + 8 * ab; pend_par = (si >> 1) & 1u;
-      t += nt;
     }
-    if (pend) { mbar_wait(pend_bar, pend_par); named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32); }
-  } else {
-    // ===================== epilogue warps 0..3 =====================
-    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp, lane);
+    release(n_commit, true);
+  } else if (warp < mma_warp) {
+    // ===================== epilogue warps =====================
+#ifndef ANSLIN_DBG_DECONLY
+    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp & 3, lane);
+#endif
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 0) tmem_dealloc(tmem_base, P.tmem_cols);
+  if (warp == mma_warp) tmem_dealloc(tmem_base, P.tmem_cols);
   splitk_fixup<FMT>(ep, fin, KT, G, T);
 }
 
@@ -815,12 +863,11 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     if (Bslots >= 2) break;
   }
   if (D < uint32_t(NW) || Bslots < 2) return ANSLIN_ERR_UNSUPPORTED;
-  Bslots = Bslots >= 4 ? 4u : 2u;
+  Bslots = std::min(Bslots, 6u);
   U = (D / NW) * Bslots;
   p.D = D;
   p.U = U;
   p.B = Bslots;
-  p.logB = Bslots == 4 ? 2u : 1u;
   const size_t smem = fixed + size_t(D) * J * kStreamSmem + size_t(U) * p.slot_bytes;
   // CTAs: one per SM in total, shared out in proportion to the problems' sizes (each at least one, at most one per group)
   const uint32_t S = uint32_t(sm_budget());
