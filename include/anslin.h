@@ -61,6 +61,13 @@ typedef enum {
 #define ANSLIN_FLAG_STATE_PAYLOAD 1u /* bf16: each lane's rANS start state carries its last two raw-plane
                                         bytes ("arbitrary initial states", P:l.167; A4) */
 
+#define ANSLIN_FLAG_LANE_STREAMS 2u  /* 32-row tiles only: every lane's 16-bit words are stored as a stream of its own
+                                        (two lanes share a region, one ascending, one descending; 20 bytes of region
+                                        sizes per 256 decode steps) instead of interleaved in read order: the decoder
+                                        needs no ballot / prefix count.  Costs ~0.02 bit/weight.  If a tile cannot be
+                                        represented (region sizes spread over > 255 words) the encoder silently drops
+                                        the flag; anslin_describe reports the flags actually used. */
+
 /* What the caller states about W. */
 typedef struct {
   uint32_t format;      /* anslin_format */

@@ -23,6 +23,8 @@ MAGIC = 0x4C534E41  # "ANSL"
 VERSION = 1
 FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ = 0, 1, 2, 3
 FLAG_STATE_PAYLOAD = 1
+FLAG_LANE_STREAMS = 2   # each lane's words stored as its own stream (tile_n = 32 only), see _lane_record
+SEG_STEPS = 256         # lane-stream records are cut into segments of this many decode steps
 STRIPE_N = 128        # weight rows per stripe = MMA M; a stripe is cut into tiles of tile_n rows
 TILE_N = 128          # default tile_n (BASELINE config 1: 128 x 64 tiles); 32 is the other supported height
 LANES = 32            # R interleaved streams per tile (P:l.192; BASELINE config 1)
@@ -123,10 +125,12 @@ class Header:
     off_zeros: int
     total_bytes: int
 
+    max_seg_bytes: int = 0      # lane-stream layout: shared-memory bytes the largest segment needs when staged
+
     def pack(self) -> bytes:
         return struct.pack("<14IfI8Q", MAGIC, VERSION, self.fmt, self.n_out, self.k_in, self.tile_n, self.tile_k,
                            self.streams, self.prob_bits, self.word_bits, self.state_lo_log2, self.group_size,
-                           self.flags, self.n_tiles, self.w_scale, 0, self.off_freq, self.off_offsets,
+                           self.flags, self.n_tiles, self.w_scale, self.max_seg_bytes, self.off_freq, self.off_offsets,
                            self.off_records, self.off_raw, self.off_scales, self.off_zeros, self.total_bytes, 0)
 
     @staticmethod
@@ -134,7 +138,7 @@ class Header:
         v = struct.unpack("<14IfI8Q", bytes(buf[:HEADER_BYTES]))
         if v[0] != MAGIC or v[1] != VERSION:
             raise ValueError("not an anslin container")
-        return Header(*v[2:15], *v[16:23])
+        return Header(*v[2:15], *v[16:23], max_seg_bytes=v[15])
 
 
 def raw_tile_bytes(tile_k: int, flags: int, tile_n: int = TILE_N) -> int:
@@ -174,6 +178,82 @@ def _raw_tile_unpack(plane: np.ndarray, steps: int, flags: int, payload):
     return vec.transpose(0, 2, 1).reshape(steps, LANES)
 
 
+def _lane_record(sym_tile: np.ndarray, tab, x_init):
+    """Lane-stream record of one tile (FLAG_LANE_STREAMS).  sym_tile: uint8 [steps x 32] in tile order.
+
+    Every lane is an ordinary scalar rANS stream (P:l.192 "each warp lane maintains its own rANS state"); instead
+    of interleaving the lanes' 16-bit words in read order, each lane keeps its words to itself.  The tile is cut
+    into segments of SEG_STEPS decode steps; a word belongs to the segment of the step after which the decoder
+    reads it.  Inside a segment lanes 2p and 2p+1 share region p: lane 2p's words ascending from the region start,
+    lane 2p+1's words descending from the region end (so 16 region sizes locate all 32 streams).
+
+    record = [32 x u32 start states][per segment: u16 base, u16 total words, 16 x u8 (region words - base)]
+             [segment 0 regions 0..15][segment 1 ...] zero-padded to 16 bytes.
+    Returns (record bytes, number of payload words, staged bytes of the largest segment)."""
+    steps = sym_tile.shape[0]
+    assert steps % SEG_STEPS == 0, "lane-stream tiles must have a multiple of %d steps" % SEG_STEPS
+    S = steps // SEG_STEPS
+    states = np.zeros(LANES, dtype=np.uint64)
+    seg_words = [[None] * LANES for _ in range(S)]
+    for lane in range(LANES):
+        col = np.ascontiguousarray(sym_tile[:, lane])
+        st, words = codec.encode_scalar(col, tab, WORD_BITS, STATE_LO_LOG2, int(x_init[lane]))
+        states[lane] = st
+        used_prev = 0
+        for sg in range(S):   # words the decoder has consumed after (sg+1)*SEG_STEPS steps
+            _, _, used = codec.decode_scalar(st, words, (sg + 1) * SEG_STEPS, tab, WORD_BITS, STATE_LO_LOG2)
+            seg_words[sg][lane] = words[used_prev:used]
+            used_prev = used
+        assert used_prev == words.size
+    tables, body, n_words, max_seg = b"", b"", 0, 0
+    for sg in range(S):
+        sizes = [seg_words[sg][2 * p].size + seg_words[sg][2 * p + 1].size for p in range(LANES // 2)]
+        base, total = min(sizes), sum(sizes)
+        if max(sizes) - base > 255 or total > 0xFFFF:
+            raise ValueError("lane-stream layout cannot represent this tile (region sizes spread over more than 255 words)")
+        tables += struct.pack("<HH16B", base, total, *[z - base for z in sizes])
+        for p in range(LANES // 2):
+            body += seg_words[sg][2 * p].astype("<u2").tobytes() + seg_words[sg][2 * p + 1][::-1].astype("<u2").tobytes()
+        n_words += total
+        max_seg = max(max_seg, _align(15 + 2 * total) + 16)
+    rec = states.astype("<u4").tobytes() + tables + body
+    return rec + b"\0" * (_align(len(rec)) - len(rec)), n_words, max_seg
+
+
+def _lane_record_decode(rec: np.ndarray, steps: int, tab):
+    """Inverse of _lane_record: returns (symbols uint8 [steps x 32], end states[32])."""
+    S = steps // SEG_STEPS
+    states = np.frombuffer(rec[:4 * LANES].tobytes(), dtype="<u4").astype(np.uint64)
+    pos = 4 * LANES + 20 * S
+    lanes = [[] for _ in range(LANES)]
+    for sg in range(S):
+        t = struct.unpack("<HH16B", rec[4 * LANES + 20 * sg:4 * LANES + 20 * sg + 20].tobytes())
+        base, total, deltas = t[0], t[1], t[2:]
+        if sum(base + d for d in deltas) != total:
+            raise ValueError("corrupt lane-stream segment table")
+        for p in range(LANES // 2):
+            n = base + deltas[p]
+            region = np.frombuffer(rec[pos:pos + 2 * n].tobytes(), dtype="<u2")
+            lanes[2 * p].append((region, +1))
+            lanes[2 * p + 1].append((region, -1))
+            pos += 2 * n
+    sym = np.zeros((steps, LANES), dtype=np.uint8)
+    end = np.zeros(LANES, dtype=np.uint64)
+    # the split of a region between its two lanes is not stored: lane 2p decodes ascending, lane 2p+1 descending,
+    # each taking exactly the words its own renormalisations ask for
+    for lane in range(LANES):
+        x = int(states[lane])
+        out = []
+        for sg in range(S):
+            region, d = lanes[lane][sg]
+            words = region if d > 0 else region[::-1]
+            o, x, _ = codec.decode_scalar(x, words, SEG_STEPS, tab, WORD_BITS, STATE_LO_LOG2)
+            out.append(o)
+        sym[:, lane] = np.concatenate(out)
+        end[lane] = x
+    return sym, end
+
+
 def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
            scales: np.ndarray | None = None, zeros: np.ndarray | None = None,
            group_size: int = 0, w_scale: float = 1.0, tile_n: int = TILE_N):
@@ -188,6 +268,9 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     assert n_out % STRIPE_N == 0 and k_in % tile_k == 0 and tile_n in (32, 128)
     if flags & FLAG_STATE_PAYLOAD:
         assert fmt == FMT_BF16, "state payload carries raw-plane bytes: bf16 only"
+    if flags & FLAG_LANE_STREAMS:
+        assert tile_n == 32, "lane streams: 32-row tiles only"
+    max_seg_bytes = 0
     wps = WEIGHTS_PER_SYMBOL[fmt]
     sym_cols = tile_k // wps
     KT = k_in // tile_k
@@ -218,6 +301,15 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
                     plane, payload = _raw_tile_pack(rblk[rows, cols].reshape(steps, LANES), flags)
                     raws.append(plane)
                     x_init = x_init + payload
+                if flags & FLAG_LANE_STREAMS:
+                    rec, n_words, seg_bytes = _lane_record(sym.reshape(steps, LANES), tab, x_init)
+                    max_seg_bytes = max(max_seg_bytes, seg_bytes)
+                    records.append(rec)
+                    offsets.append(offsets[-1] + len(rec) // 16)
+                    state_bits += 32 * LANES
+                    payload_bits += 16 * n_words
+                    pad_bits += 8 * (len(rec) - 4 * LANES - 2 * n_words)   # segment tables + padding
+                    continue
                 states, words = codec.tile_encode(sym, LANES, tab, WORD_BITS, STATE_LO_LOG2, x_init)
                 rec = states.astype("<u4").tobytes() + words.astype("<u2").tobytes()
                 pad = _align(len(rec)) - len(rec)
@@ -247,7 +339,7 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     total = max(total, _align(off_records + len(rec_bytes) + TAIL_BYTES))   # tail rule
     hdr = Header(fmt, n_out, k_in, tile_n, tile_k, LANES, PROB_BITS, WORD_BITS, STATE_LO_LOG2, group_size, flags,
                  n_tiles, float(w_scale), off_freq, off_offsets, off_records, off_raw if raw_bytes else 0,
-                 off_scales if side else 0, 0, total)
+                 off_scales if side else 0, 0, total, max_seg_bytes)
     buf = np.zeros(total, dtype=np.uint8)
     buf[:HEADER_BYTES] = np.frombuffer(hdr.pack(), dtype=np.uint8)
     buf[off_freq:off_freq + 512] = np.frombuffer(f.astype("<u2").tobytes(), dtype=np.uint8)
@@ -299,9 +391,14 @@ def decode(buf: np.ndarray):
             r0 = stripe * STRIPE_N + q * tile_n
             a = h.off_records + 16 * int(offsets[t])
             e = h.off_records + 16 * int(offsets[t + 1])
-            states = np.frombuffer(buf[a:a + 4 * LANES].tobytes(), dtype="<u4").astype(np.uint64)
-            words = np.frombuffer(buf[a + 4 * LANES:e].tobytes(), dtype="<u2")
-            sym, end, used = codec.tile_decode(states, words, n_sym, LANES, tab, h.word_bits, h.state_lo_log2)
+            if h.flags & FLAG_LANE_STREAMS:
+                sym, end = _lane_record_decode(buf[a:e], steps, tab)
+                sym = sym.reshape(-1)
+                used = (e - a - 4 * LANES) // 2
+            else:
+                states = np.frombuffer(buf[a:a + 4 * LANES].tobytes(), dtype="<u4").astype(np.uint64)
+                words = np.frombuffer(buf[a + 4 * LANES:e].tobytes(), dtype="<u2")
+                sym, end, used = codec.tile_decode(states, words, n_sym, LANES, tab, h.word_bits, h.state_lo_log2)
             payload = end - np.uint64(L)
             if h.flags & FLAG_STATE_PAYLOAD:
                 if np.any(end < L) or np.any(payload > 0xFFFF):

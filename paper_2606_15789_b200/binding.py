@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libanslin.so")
 FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ = 0, 1, 2, 3
 DT_F32, DT_F16, DT_BF16, DT_I8, DT_FP8_E4M3 = 0, 1, 2, 3, 4
 FLAG_STATE_PAYLOAD = 1
+FLAG_LANE_STREAMS = 2
 X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_INT4_AWQ: DT_F16}
 
 EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_close", "anslin_describe",

@@ -24,13 +24,15 @@ constexpr uint32_t kL = 1u << kStateLoLog2;
 constexpr uint32_t kM = 1u << kProbBits;
 constexpr int kHeaderBytes = 128;
 constexpr int kTailBytes = 4096; // readable bytes guaranteed after the records section (ring read-ahead)
+constexpr int kSegSteps = 256;   // lane-stream layout: decode steps per record segment
+constexpr int kSegTableBytes = 20; // per segment: u16 base, u16 total words, 16 x u8 (region words - base)
 constexpr int kUnitBytes = 4096; // one operand unit = 128 rows x 32 B (one tcgen05.mma K step)
 
 struct Header {  // 128 bytes, little endian
   uint32_t magic, version, format, n_out, k_in, tile_n, tile_k, streams, prob_bits, word_bits,
       state_lo_log2, group_size, flags, n_tiles;
   float w_scale;
-  uint32_t reserved0;
+  uint32_t max_seg_bytes;  // lane-stream layout: shared-memory bytes the largest segment needs when staged (else 0)
   uint64_t off_freq, off_offsets, off_records, off_raw, off_scales, off_zeros, total_bytes, reserved1;
 };
 static_assert(sizeof(Header) == kHeaderBytes, "header must be 128 bytes");

@@ -173,22 +173,97 @@ __device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint3
   return e;
 }
 
+// ---- lane-stream layout (ANSLIN_FLAG_LANE_STREAMS): every lane reads its own word stream ----------------
+// The record is cut into segments of kSegSteps decode steps; a segment's words are staged whole in shared
+// memory, lanes 2p and 2p+1 sharing region p (lane 2p walks up from its start, lane 2p+1 down from its end).
+// No ballot, no prefix count, no ring upkeep: a step renormalises with a predicated load at the lane's cursor.
+struct LaneStream {
+  uint32_t x;          // this lane's rANS state
+  uint32_t ptr;        // shared address of this lane's next word
+  uint32_t w;          // last word loaded (kept live so that the predicated load never reads an undefined register)
+  uint32_t goff;       // byte offset, from the record start, of the next segment's words
+  const uint8_t *rec;  // record start in HBM
+};
+__device__ __forceinline__ void lane_open(LaneStream &s, const uint8_t *rec, int segments, int lane) {
+  s.x = reinterpret_cast<const uint32_t *>(rec)[lane];
+  s.rec = rec;
+  s.goff = 4 * kLanes + uint32_t(kSegTableBytes) * uint32_t(segments);
+  s.w = 0;
+  s.ptr = 0;
+}
+// Stage segment `seg` of the record into buf (bufbytes of shared memory) and point every lane at its stream.
+// All lanes have finished reading the previous segment (program order + the __syncwarp in stream_drain).
+__device__ __forceinline__ void lane_open_segment(LaneStream &s, uint32_t buf, uint32_t bufbytes, int seg, int lane) {
+  stream_drain();
+  const uint8_t *te = s.rec + 4 * kLanes + kSegTableBytes * seg;
+  const uint32_t hdr = *reinterpret_cast<const uint32_t *>(te);   // u16 base | u16 total words
+  const uint32_t base = hdr & 0xFFFFu, total = hdr >> 16;
+  const uint32_t size = lane < kLanes / 2 ? base + uint32_t(te[4 + lane]) : 0u;   // words of region `lane`
+  uint32_t end = size;
+#pragma unroll
+  for (int d = 1; d < kLanes / 2; d <<= 1) {
+    const uint32_t o = __shfl_up_sync(0xffffffffu, end, d);
+    if (lane >= d) end += o;
+  }
+  const uint32_t start = end - size;
+  const uint32_t start_p = __shfl_sync(0xffffffffu, start, lane >> 1), end_p = __shfl_sync(0xffffffffu, end, lane >> 1);
+  const uint32_t skew = s.goff & 15u;
+  const uint8_t *src = s.rec + (s.goff - skew);
+  const uint32_t nbytes = min((skew + 2u * total + 15u) & ~15u, bufbytes);   // a damaged table cannot overrun the buffer
+  for (uint32_t o = 16u * uint32_t(lane); o < nbytes; o += kFillBytes)
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(buf + o), "l"(src + o) : "memory");
+  cp_async_commit();
+  s.ptr = buf + skew + 2u * ((lane & 1) ? end_p - 1u : start_p);
+  s.goff += 2u * total;
+  stream_drain();
+}
+// One decode step of Alg V.2 for all 32 lanes of one lane-stream tile; dir = +2 (even lanes) / -2 (odd lanes).
+__device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uint32_t dir) {
+  uint32_t ea, e;
+  asm("mad.lo.u32 %0, %1, 4, %2;" : "=r"(ea) : "r"(s.x & (kM - 1)), "r"(tab_s));
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea));
+  uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.lt.u32 p, %0, 65536;\n\t"
+      "@p ld.shared.u16 %2, [%1];\n\t"
+      "@p mad.lo.u32 %0, %0, 65536, %2;\n\t"
+      "@p add.u32 %1, %1, %3;\n\t}"
+      : "+r"(xn), "+r"(s.ptr), "+r"(s.w)
+      : "r"(dir)
+      : "memory");
+  s.x = xn;
+  return e;
+}
+
+// The two word layouts as policies of decode_unit.
+struct InterleavedWords {
+  using S = Stream;
+  template <int J> static __device__ __forceinline__ void upkeep8(S (&s)[J], uint32_t ring0, int lane) { stream_upkeep8<J>(s, ring0, lane); }
+  static __device__ __forceinline__ uint32_t step(S &s, uint32_t tab, uint32_t lt) { return decode_step(s, tab, lt); }
+};
+struct LaneWords {
+  using S = LaneStream;
+  template <int J> static __device__ __forceinline__ void upkeep8(S (&)[J], uint32_t, int) {}
+  static __device__ __forceinline__ uint32_t step(S &s, uint32_t tab, uint32_t dir) { return lane_step(s, tab, dir); }
+};
+
 // Insert the symbol byte of table entry e at byte position `pos` of acc.
 template <int pos>
 __device__ __forceinline__ uint32_t put_sym(uint32_t acc, uint32_t e) {
   return __byte_perm(acc, e, (0x3210 & ~(0xF << (4 * pos))) | (4 << (4 * pos)));
 }
 // Four decode steps of each of the J streams, interleaved -> four symbol bytes per stream.
-template <int J>
-__device__ __forceinline__ void decode4(Stream (&s)[J], uint32_t (&q)[J], uint32_t tab, uint32_t lt) {
+template <class POL, int J>
+__device__ __forceinline__ void decode4(typename POL::S (&s)[J], uint32_t (&q)[J], uint32_t tab, uint32_t aux) {
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<0>(0u, decode_step(s[j], tab, lt));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<0>(0u, POL::step(s[j], tab, aux));
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<1>(q[j], decode_step(s[j], tab, lt));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<1>(q[j], POL::step(s[j], tab, aux));
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<2>(q[j], decode_step(s[j], tab, lt));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<2>(q[j], POL::step(s[j], tab, aux));
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<3>(q[j], decode_step(s[j], tab, lt));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<3>(q[j], POL::step(s[j], tab, aux));
 }
 
 // bf16: merge 4 exponent bytes (E) with 4 raw bytes (R = mantissa<<1 | sign) into 4 bf16 values:
@@ -252,8 +327,9 @@ struct RawReader {
 //     void packed(int j, int g, int lane, uint32_t b) for int4 when Emit::kOperand == false (4 packed bytes).
 //   ring0: shared address of stream 0's ring (stream j's follows at j * kStreamSmem).
 //   u: unit index inside the tile, V: raw vectors per tile (bf16).  sz[j]: int4: &(scale, zero)[group][first row of tile j].
-template <uint32_t FMT, int RB, int J, bool kPayload, class Emit>
-__device__ __forceinline__ void decode_unit(Stream (&s)[J], uint32_t ring0, uint32_t tab, int lane, uint32_t lt, int u, int V,
+//   POL: InterleavedWords (aux = lanemask_lt) or LaneWords (aux = this lane's cursor direction, +2 / -2).
+template <uint32_t FMT, int RB, int J, bool kPayload, class POL, class Emit>
+__device__ __forceinline__ void decode_unit(typename POL::S (&s)[J], uint32_t ring0, uint32_t tab, int lane, uint32_t lt, int u, int V,
                                             RawReader<kPayload> (&raw)[J], const uint32_t *const (&sz)[J], Emit &emit) {
   constexpr int G = 2 * RB;
   if constexpr (FMT == ANSLIN_FMT_BF16) {
@@ -265,10 +341,10 @@ __device__ __forceinline__ void decode_unit(Stream (&s)[J], uint32_t ring0, uint
       for (int j = 0; j < J; ++j) rv[j] = raw[j].take(v, V, lane);
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        stream_upkeep8<J>(s, ring0, lane);
+        POL::template upkeep8<J>(s, ring0, lane);
         uint32_t E0[J], E1[J];
-        decode4<J>(s, E0, tab, lt);
-        decode4<J>(s, E1, tab, lt);
+        decode4<POL, J>(s, E0, tab, lt);
+        decode4<POL, J>(s, E1, tab, lt);
 #pragma unroll
         for (int j = 0; j < J; ++j) {
           if (kPayload && h == 1 && v == V - 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
@@ -283,9 +359,9 @@ __device__ __forceinline__ void decode_unit(Stream (&s)[J], uint32_t ring0, uint
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll 1
     for (int g = 0; g < G; ++g) {
-      if ((g & 1) == 0) stream_upkeep8<J>(s, ring0, lane);
+      if ((g & 1) == 0) POL::template upkeep8<J>(s, ring0, lane);
       uint32_t B[J];
-      decode4<J>(s, B, tab, lt);
+      decode4<POL, J>(s, B, tab, lt);
 #pragma unroll
       for (int j = 0; j < J; ++j) {
         if constexpr (Emit::kOperand) {
@@ -304,12 +380,12 @@ __device__ __forceinline__ void decode_unit(Stream (&s)[J], uint32_t ring0, uint
 #pragma unroll 1
     for (int g = 0; g < G; ++g) {
       uint32_t q0[J], q1[J], q2[J], q3[J];
-      stream_upkeep8<J>(s, ring0, lane);
-      decode4<J>(s, q0, tab, lt);
-      decode4<J>(s, q1, tab, lt);
-      stream_upkeep8<J>(s, ring0, lane);
-      decode4<J>(s, q2, tab, lt);
-      decode4<J>(s, q3, tab, lt);
+      POL::template upkeep8<J>(s, ring0, lane);
+      decode4<POL, J>(s, q0, tab, lt);
+      decode4<POL, J>(s, q1, tab, lt);
+      POL::template upkeep8<J>(s, ring0, lane);
+      decode4<POL, J>(s, q2, tab, lt);
+      decode4<POL, J>(s, q3, tab, lt);
 #pragma unroll
       for (int j = 0; j < J; ++j) emit.chunk(j, g, lane, make_uint4(q0[j], q1[j], q2[j], q3[j]));
     }

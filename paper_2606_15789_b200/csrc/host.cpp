@@ -37,7 +37,7 @@ bool make_geometry(const anslin_desc *d, Geometry *g) {
   g->wps = weights_per_symbol(g->fmt);
   if (g->n_out == 0 || g->k_in == 0 || g->n_out % kTileN || g->k_in % g->tile_k) return false;
   if (g->tile_k % unit_k_of(g->fmt) || g->tile_k % 64 || g->tile_k > 1024) return false;
-  if ((g->flags & ~ANSLIN_FLAG_STATE_PAYLOAD) != 0) return false;
+  if ((g->flags & ~(ANSLIN_FLAG_STATE_PAYLOAD | ANSLIN_FLAG_LANE_STREAMS)) != 0) return false;
   if ((g->flags & ANSLIN_FLAG_STATE_PAYLOAD) && g->fmt != ANSLIN_FMT_BF16) return false;
   if (g->fmt == ANSLIN_FMT_INT4_AWQ && (g->group == 0 || g->group % 16 || g->k_in % g->group)) return false;
   g->sym_cols = int(g->tile_k) / g->wps;
@@ -48,6 +48,7 @@ bool make_geometry(const anslin_desc *d, Geometry *g) {
   g->KT = int(g->k_in / g->tile_k);
   g->stripes = int(g->n_out / kTileN);
   g->n_tiles = size_t(g->KT) * g->stripes * g->Q;
+  if ((g->flags & ANSLIN_FLAG_LANE_STREAMS) && (g->tile_n != 32 || g->steps % kSegSteps)) return false;
   g->row_syms = g->k_in / g->wps;
   return true;
 }
@@ -110,8 +111,9 @@ bool normalise(const uint64_t *cnt, uint32_t *f) {
 }
 
 // One tile -> record bytes (32 states + words in decoder read order + pad) and raw plane bytes.
-void encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *f, const uint32_t *c,
-                 std::vector<uint8_t> &rec, uint8_t *raw_out, uint64_t *n_words_out) {
+// Returns false if the lane-stream layout cannot represent the tile.  *seg_bytes_out: staged bytes of its largest segment.
+bool encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *f, const uint32_t *c,
+                 std::vector<uint8_t> &rec, uint8_t *raw_out, uint64_t *n_words_out, uint32_t *seg_bytes_out) {
   const int steps = g.steps, spc = g.spc, G = 2 * g.rb;
   const size_t grp = tile / g.Q, q = tile % g.Q, stripe = grp / g.KT, kt = grp % g.KT;
   const size_t row0 = stripe * kTileN + q * g.tile_n, col0 = kt * g.sym_cols;
@@ -136,7 +138,10 @@ void encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
   }
   // Words are produced back to front so that the buffer ends up in decoder read order
   // (step ascending, renormalising lanes ascending) without a reversal pass.
-  std::vector<uint16_t> words(sym.size() + 8);
+  const bool lane_streams = g.flags & ANSLIN_FLAG_LANE_STREAMS;
+  const int S = lane_streams ? steps / kSegSteps : 0;
+  std::vector<uint16_t> words(lane_streams ? 0 : sym.size() + 8);
+  std::vector<std::vector<uint16_t>> lw(size_t(S) * kLanes);   // lane streams: words of (segment, lane), filled back to front
   size_t wp = words.size();
   for (int t = steps; t-- > 0;)
     for (int lane = kLanes; lane-- > 0;) {
@@ -144,16 +149,50 @@ void encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
       const uint32_t fs = f[s];
       uint32_t xv = x[lane];
       if (uint64_t(xv) >= (uint64_t(fs) << (kStateLoLog2 - kProbBits + kWordBits))) {
-        words[--wp] = uint16_t(xv);
+        // the decoder reads this word right after decoding step t
+        if (lane_streams) lw[size_t(t / kSegSteps) * kLanes + lane].push_back(uint16_t(xv));
+        else words[--wp] = uint16_t(xv);
         xv >>= kWordBits;
       }
       x[lane] = ((xv / fs) << kProbBits) + (xv % fs) + c[s];
     }
-  const size_t nw = words.size() - wp;
-  rec.assign(align16(4 * kLanes + 2 * nw), 0);
-  std::memcpy(rec.data(), x, 4 * kLanes);
-  std::memcpy(rec.data() + 4 * kLanes, words.data() + wp, 2 * nw);
-  *n_words_out = nw;
+  *seg_bytes_out = 0;
+  if (lane_streams) {
+    // record = states | per segment {u16 base, u16 total, 16 x u8 delta} | per segment 16 regions: lane 2p ascending,
+    // lane 2p+1 descending from the region end (lw holds every lane's words in REVERSE read order already)
+    size_t nw = 0;
+    for (auto &v : lw) nw += v.size();
+    rec.assign(align16(4 * kLanes + size_t(kSegTableBytes) * S + 2 * nw), 0);
+    std::memcpy(rec.data(), x, 4 * kLanes);
+    uint8_t *tabp = rec.data() + 4 * kLanes;
+    uint16_t *wout = reinterpret_cast<uint16_t *>(tabp + size_t(kSegTableBytes) * S);
+    for (int sg = 0; sg < S; ++sg) {
+      size_t sizes[kLanes / 2], base = ~size_t(0), total = 0;
+      for (int p = 0; p < kLanes / 2; ++p) {
+        sizes[p] = lw[size_t(sg) * kLanes + 2 * p].size() + lw[size_t(sg) * kLanes + 2 * p + 1].size();
+        base = std::min(base, sizes[p]);
+        total += sizes[p];
+      }
+      if (total > 0xFFFF) return false;
+      uint16_t hdr[2] = {uint16_t(base), uint16_t(total)};
+      std::memcpy(tabp + size_t(kSegTableBytes) * sg, hdr, 4);
+      for (int p = 0; p < kLanes / 2; ++p) {
+        if (sizes[p] - base > 255) return false;
+        tabp[size_t(kSegTableBytes) * sg + 4 + p] = uint8_t(sizes[p] - base);
+        const auto &ev = lw[size_t(sg) * kLanes + 2 * p], &od = lw[size_t(sg) * kLanes + 2 * p + 1];
+        for (size_t i = ev.size(); i-- > 0;) *wout++ = ev[i];       // read order ascending
+        for (size_t i = 0; i < od.size(); ++i) *wout++ = od[i];     // reverse read order: lane 2p+1 walks down from the end
+      }
+      *seg_bytes_out = std::max<uint32_t>(*seg_bytes_out, uint32_t(align16(15 + 2 * total) + 16));
+    }
+    *n_words_out = nw;
+  } else {
+    const size_t nw = words.size() - wp;
+    rec.assign(align16(4 * kLanes + 2 * nw), 0);
+    std::memcpy(rec.data(), x, 4 * kLanes);
+    std::memcpy(rec.data() + 4 * kLanes, words.data() + wp, 2 * nw);
+    *n_words_out = nw;
+  }
   if (raw_out) {
     const int V = steps / 16;
     for (int v = 0; v < V; ++v) {
@@ -166,7 +205,11 @@ void encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
         }
     }
   }
+  return true;
 }
+
+int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const void *scales_host, const void *zeros_host,
+                void *container_out, size_t capacity, size_t *bytes_out, anslin_stats *st);
 
 }  // namespace
 
@@ -177,7 +220,7 @@ size_t anslin_encode_bound(const anslin_desc *desc) {
   if (!make_geometry(desc, &g)) return 0;
   const size_t tile_syms = size_t(g.steps) * kLanes;
   // every symbol costs at most 12 bits + one flush word per lane; round generously
-  const size_t rec = align16(4 * kLanes + 2 * (tile_syms * 3 / 4 + 2 * kLanes + 8));
+  const size_t rec = align16(4 * kLanes + 2 * (tile_syms * 3 / 4 + 2 * kLanes + 8)) + align16(size_t(kSegTableBytes) * (g.steps / kSegSteps + 1));
   size_t total = kHeaderBytes + 512 + align16(4 * (g.n_tiles + 1)) + g.n_tiles * rec + 64;
   if (g.fmt == ANSLIN_FMT_BF16) total += g.n_tiles * raw_tile_bytes(g.tile_n, g.tile_k, 0) + 16;
   return total + align16(side_bytes(g)) + 16 + kTailBytes;
@@ -189,6 +232,14 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   if (desc->format > ANSLIN_FMT_INT4_AWQ) return ANSLIN_ERR_UNSUPPORTED;
   Geometry g;
   if (!make_geometry(desc, &g)) return ANSLIN_ERR_UNSUPPORTED;
+  return encode_with(g, desc, w_host, scales_host, zeros_host, container_out, capacity, bytes_out, st);
+}
+
+}  // extern "C"
+
+namespace {
+int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const void *scales_host, const void *zeros_host,
+                void *container_out, size_t capacity, size_t *bytes_out, anslin_stats *st) {
   if (g.fmt == ANSLIN_FMT_INT8 && !scales_host) return ANSLIN_ERR_INVALID_ARG;
   if (g.fmt == ANSLIN_FMT_INT4_AWQ && (!scales_host || !zeros_host)) return ANSLIN_ERR_INVALID_ARG;
 
@@ -221,6 +272,8 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   // Encode tiles in parallel, then lay the records out in tile order.
   std::vector<std::vector<uint8_t>> recs(g.n_tiles);
   std::vector<uint64_t> nwords(g.n_tiles, 0);
+  std::vector<uint32_t> segbytes(g.n_tiles, 0);
+  std::atomic<bool> lane_fail(false);
   const size_t rtb = g.fmt == ANSLIN_FMT_BF16 ? raw_tile_bytes(g.tile_n, g.tile_k, g.flags) : 0;
   Header h;
   std::memset(&h, 0, sizeof(h));
@@ -240,10 +293,15 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
         for (;;) {
           size_t t = next.fetch_add(1);
           if (t >= g.n_tiles) break;
-          encode_tile(g, w_host, t, f, c, recs[t], rtb ? raw_all.data() + t * rtb : nullptr, &nwords[t]);
+          if (!encode_tile(g, w_host, t, f, c, recs[t], rtb ? raw_all.data() + t * rtb : nullptr, &nwords[t], &segbytes[t]))
+            lane_fail = true;
         }
       });
     for (auto &t : th) t.join();
+  }
+  if (lane_fail) {   // a tile does not fit the lane-stream tables: encode the matrix with interleaved words instead
+    g.flags &= ~ANSLIN_FLAG_LANE_STREAMS;
+    return encode_with(g, desc, w_host, scales_host, zeros_host, container_out, capacity, bytes_out, st);
   }
   size_t rec_total = 0;
   for (auto &r : recs) rec_total += r.size();
@@ -263,6 +321,7 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   h.tile_n = g.tile_n; h.tile_k = g.tile_k; h.streams = kLanes; h.prob_bits = kProbBits; h.word_bits = kWordBits;
   h.state_lo_log2 = kStateLoLog2; h.group_size = g.group; h.flags = g.flags; h.n_tiles = uint32_t(g.n_tiles);
   h.w_scale = g.fmt == ANSLIN_FMT_FP8_E4M3 ? desc->w_scale : 1.0f;
+  for (uint32_t b : segbytes) h.max_seg_bytes = std::max(h.max_seg_bytes, b);
 
   uint8_t *out = static_cast<uint8_t *>(container_out);
   std::memset(out, 0, h.total_bytes);
@@ -277,7 +336,7 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
     std::memcpy(out + h.off_records + pos, recs[t].data(), recs[t].size());
     pos += recs[t].size();
     payload_bits += 16 * nwords[t];
-    pad_bits += 8 * (recs[t].size() - 4 * kLanes - 2 * nwords[t]);
+    pad_bits += 8 * (recs[t].size() - 4 * kLanes - 2 * nwords[t]);   // record padding (+ lane-stream segment tables)
   }
   offs[g.n_tiles] = uint32_t(pos / 16);
   if (rtb) std::memcpy(out + h.off_raw, raw_all.data(), raw_all.size());
@@ -323,6 +382,9 @@ int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *
   }
   return ANSLIN_OK;
 }
+}  // namespace
+
+extern "C" {
 
 int anslin_open(const void *container_host, size_t bytes, const void *container_dev, anslin_weight **out) {
   if (!container_host || !out || bytes < size_t(kHeaderBytes)) return ANSLIN_ERR_INVALID_ARG;
@@ -357,10 +419,12 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   for (size_t t = 0; t < g.n_tiles; ++t) {
     // a record holds at least the 32 lane states and never more than the worst-case tile
     if (offs[t + 1] < offs[t] + 8 || offs[t + 1] > rec_units) return ANSLIN_ERR_CORRUPT;
-    if (uint64_t(offs[t + 1] - offs[t]) * 16 > 128 + uint64_t(g.steps) * kLanes * 2 + 16) return ANSLIN_ERR_CORRUPT;
+    if (uint64_t(offs[t + 1] - offs[t]) * 16 > 128 + uint64_t(g.steps) * kLanes * 2 + 16 + uint64_t(kSegTableBytes) * (g.steps / kSegSteps + 1))
+      return ANSLIN_ERR_CORRUPT;
   }
   if (g.fmt == ANSLIN_FMT_BF16 && !in(h.off_raw, raw_tile_bytes(g.tile_n, g.tile_k, g.flags) * g.n_tiles)) return ANSLIN_ERR_CORRUPT;
   if (side_bytes(g) && !in(h.off_scales, side_bytes(g))) return ANSLIN_ERR_CORRUPT;
+  if ((g.flags & ANSLIN_FLAG_LANE_STREAMS) && (h.max_seg_bytes < 32 || h.max_seg_bytes > 2 * 0xFFFF + 64)) return ANSLIN_ERR_CORRUPT;
   anslin_weight *w = new (std::nothrow) anslin_weight;
   if (!w) return ANSLIN_ERR_INVALID_ARG;
   w->h = h;

@@ -19,6 +19,7 @@
 #include <stdlib.h>
 #include <string.h>
 #include <algorithm>
+#include <type_traits>
 
 #include "anslin_internal.h"
 #include "decode_core.cuh"
@@ -152,7 +153,7 @@ template <> struct FmtTraits<ANSLIN_FMT_INT8> { static constexpr int kind = 2; s
 struct ContainerView {
   const uint8_t *base;
   uint64_t off_freq, off_offsets, off_records, off_raw, off_scales, total;
-  uint32_t n_out, k_in, tile_n, tile_k, KT, n_tiles, units, group, flags;
+  uint32_t n_out, k_in, tile_n, tile_k, KT, n_tiles, units, group, flags, max_seg_bytes;
   float w_scale;
 };
 
@@ -164,6 +165,7 @@ ContainerView view_of(const anslin_weight *w) {
   v.off_scales = h.off_scales; v.total = h.total_bytes;
   v.n_out = h.n_out; v.k_in = h.k_in; v.tile_n = h.tile_n; v.tile_k = h.tile_k; v.KT = h.k_in / h.tile_k; v.n_tiles = h.n_tiles;
   v.units = h.tile_k / unit_k_of(h.format); v.group = h.group_size; v.flags = h.flags; v.w_scale = h.w_scale;
+  v.max_seg_bytes = h.max_seg_bytes;
   return v;
 }
 
@@ -211,8 +213,12 @@ struct GlobalEmit {
 
 constexpr int kDecWarps = 8;
 
-template <uint32_t FMT, int RB, int J, bool PAYLOAD>
-__global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView cv, uint8_t *out) {
+// steps of one lane per operand unit of a 32-row tile (lane = row)
+__host__ __device__ constexpr int unit_steps32(uint32_t fmt) { return 2 * spc_of(fmt); }
+
+template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS>
+__global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView cv, uint8_t *out, uint32_t stream_bytes) {
+  using POL = typename std::conditional<LS, LaneWords, InterleavedWords>::type;
   constexpr int Q = TileTraits<RB, J>::Q;
   extern __shared__ __align__(16) uint8_t dsm[];
   uint32_t *tab = reinterpret_cast<uint32_t *>(dsm);
@@ -220,13 +226,15 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
   uint8_t *rings = dsm + 4 * kM + 1056;
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const uint32_t lt = lanemask_lt(), ring_s = smem_u32(rings) + uint32_t(warp) * J * kStreamSmem;
+  const uint32_t ring_s = smem_u32(rings) + uint32_t(warp) * J * stream_bytes;
+  const uint32_t aux = LS ? ((lane & 1) ? uint32_t(-2) : 2u) : lanemask_lt();
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
   const size_t row_bytes = row_bytes_of(FMT, cv.k_in), tile_row_bytes = row_bytes_of(FMT, cv.tile_k);
   const size_t rtb = raw_tile_bytes(32 * RB, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
   const int V = int(cv.units) * RB;
+  constexpr uint32_t kUnitsPerSeg = LS ? kSegSteps / unit_steps32(FMT) : 1;
   for (uint32_t job = blockIdx.x * kDecWarps + warp; job < cv.n_tiles / J; job += gridDim.x * kDecWarps) {
-    Stream s[J];
+    typename POL::S s[J];
     RawReader<PAYLOAD> raw[J];
     const uint32_t *sz[J];
     GlobalEmit<FMT, RB, J> emit;
@@ -235,14 +243,22 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
 #pragma unroll
     for (int j = 0; j < J; ++j) {
       const uint32_t t = job * J + j, grp = t / Q, q = t % Q, stripe = grp / cv.KT, kt = grp % cv.KT;
-      stream_open(s[j], cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s + j * kStreamSmem, lane);
+      const uint8_t *rec = cv.base + cv.off_records + size_t(offs[t]) * 16;
+      if constexpr (LS) lane_open(s[j], rec, int(cv.units / kUnitsPerSeg), lane);
+      else stream_open(s[j], rec, ring_s + j * stream_bytes, lane);
       emit.tile_out[j] = out + (size_t(stripe) * kTileN + size_t(q) * 32 * RB) * row_bytes + size_t(kt) * tile_row_bytes;
       if (FMT == ANSLIN_FMT_BF16) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
       sz[j] = nullptr;
     }
     for (uint32_t u = 0; u < cv.units; ++u) {
       emit.u = int(u);
-      decode_unit<FMT, RB, J, PAYLOAD>(s, ring_s, smem_u32(tab), lane, lt, int(u), V, raw, sz, emit);
+      if constexpr (LS) {
+        if (u % kUnitsPerSeg == 0) {
+#pragma unroll
+          for (int j = 0; j < J; ++j) lane_open_segment(s[j], ring_s + j * stream_bytes, stream_bytes, int(u / kUnitsPerSeg), lane);
+        }
+      }
+      decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, smem_u32(tab), lane, aux, int(u), V, raw, sz, emit);
     }
 #ifdef ANSLIN_PROBE_NOSTORE
     if (emit.chk == 0x12345678u) out[job] = 1;
@@ -420,6 +436,7 @@ struct FusedParams {
   Problem prob[kMaxProblems];
   uint32_t nprob;
   uint32_t U, D, B;        // operand slots (= teams * B), decoder warps, slots per team (>= 2)
+  uint32_t stream_bytes;   // shared memory per stream: word ring + mirror, or the largest staged lane-stream segment
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
 };
@@ -443,10 +460,11 @@ struct SmemEmit {
   __device__ __forceinline__ void packed(int, int, int, uint32_t) const {}
 };
 
-template <uint32_t FMT, int RB, int J, bool PAYLOAD>
+template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS>
 __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ TensorMaps tms,
                                                                       const __grid_constant__ FusedParams P) {
   using TR = FmtTraits<FMT>;
+  using POL = typename std::conditional<LS, LaneWords, InterleavedWords>::type;
   constexpr int NW = TileTraits<RB, J>::NW, Q = TileTraits<RB, J>::Q;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 2047u) & ~2047u;
@@ -461,7 +479,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   // carve-up
   const uint32_t slots_s = smem0;
   const uint32_t ring_off = P.U * P.slot_bytes;
-  const uint32_t tab_off = ring_off + P.D * J * kStreamSmem;
+  const uint32_t tab_off = ring_off + P.D * J * P.stream_bytes;
   uint32_t *tab = reinterpret_cast<uint32_t *>(smem + tab_off);
   uint32_t *cum = reinterpret_cast<uint32_t *>(smem + tab_off + 16384);
   const uint32_t bar_off = tab_off + 16384 + 1056;
@@ -495,7 +513,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     const uint32_t d = uint32_t(warp);
     {
       const uint32_t PT = P.D / NW, team = d / NW, hw = d % NW;   // teams of NW warps fill one 128-row unit together
-      const uint32_t lt = lanemask_lt(), ring_s = smem0 + ring_off + d * J * kStreamSmem, tab_s = smem0 + tab_off;
+      const uint32_t ring_s = smem0 + ring_off + d * J * P.stream_bytes, tab_s = smem0 + tab_off;
+      const uint32_t aux = LS ? ((lane & 1) ? uint32_t(-2) : 2u) : lanemask_lt();
+      constexpr uint32_t kUnitsPerSeg = LS ? kSegSteps / unit_steps32(FMT) : 1;
       const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
       const size_t rtb = raw_tile_bytes(32 * RB, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
       const uint32_t xbytes = mpad * 32u;
@@ -507,7 +527,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 #pragma unroll 1
       for (uint32_t i = team; i < t_end - t_begin; i += PT) {
         const uint32_t gt = t_begin + i, stripe = gt / KT, kt = gt % KT;
-        Stream s[J];
+        typename POL::S s[J];
         RawReader<PAYLOAD> raw[J];
         const uint32_t *sz[J];
         SmemEmit<RB, J> emit;
@@ -515,7 +535,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 #pragma unroll
         for (int j = 0; j < J; ++j) {
           const uint32_t q = hw * J + j, t = gt * Q + q;
-          stream_open(s[j], cv.base + cv.off_records + size_t(offs[t]) * 16, ring_s + j * kStreamSmem, lane);
+          const uint8_t *rec = cv.base + cv.off_records + size_t(offs[t]) * 16;
+          if constexpr (LS) lane_open(s[j], rec, int(units / kUnitsPerSeg), lane);
+          else stream_open(s[j], rec, ring_s + j * P.stream_bytes, lane);
           if (FMT == ANSLIN_FMT_BF16) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
           emit.row0[j] = q * 32u * RB;
           sz[j] = nullptr;
@@ -548,7 +570,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
               sz[j] = reinterpret_cast<const uint32_t *>(cv.base + cv.off_scales) + size_t(uint32_t(k_elem) / cv.group) * cv.n_out +
                       size_t(stripe) * kTileN + emit.row0[j];
           }
-          decode_unit<FMT, RB, J, PAYLOAD>(s, ring_s, tab_s, lane, lt, int(u), V, raw, sz, emit);
+          if constexpr (LS) {
+            if (u % kUnitsPerSeg == 0) {
+#pragma unroll
+              for (int j = 0; j < J; ++j) lane_open_segment(s[j], ring_s + j * P.stream_bytes, P.stream_bytes, int(u / kUnitsPerSeg), lane);
+            }
+          }
+          decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, tab_s, lane, aux, int(u), V, raw, sz, emit);
 #ifndef ANSLIN_DBG_NOFENCE
           fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
 #endif
@@ -799,9 +827,9 @@ bool x_dtype_ok(uint32_t fmt, uint32_t dt) {
 
 int sm_budget() { return std::max(1, num_sms()); }
 
-template <uint32_t FMT, int RB, bool PAYLOAD>
+template <uint32_t FMT, int RB, bool PAYLOAD, bool LS>
 int launch_fused(const TensorMaps &tms, const FusedParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
-  auto kern = fused_gemm_kernel<FMT, RB, (RB == 1 ? kJ32 : 1), PAYLOAD>;
+  auto kern = fused_gemm_kernel<FMT, RB, (RB == 1 ? kJ32 : 1), PAYLOAD, LS>;
   static thread_local size_t smem_set = 0;     // per instantiation: raise the dynamic shared memory limit once
   if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
@@ -833,7 +861,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     if (!w || !w->dev || !xs[i] || !ys[i]) return ANSLIN_ERR_INVALID_ARG;
     if (ms[i] < 1 || ms[i] > 256) return ANSLIN_ERR_UNSUPPORTED;
     const Header &h = w->h;
-    if (h.format != h0.format || h.tile_n != h0.tile_n || ((h.flags ^ h0.flags) & ANSLIN_FLAG_STATE_PAYLOAD)) return ANSLIN_ERR_INVALID_ARG;
+    if (h.format != h0.format || h.tile_n != h0.tile_n || h.flags != h0.flags) return ANSLIN_ERR_INVALID_ARG;
     if ((reinterpret_cast<uintptr_t>(xs[i]) | reinterpret_cast<uintptr_t>(ys[i])) & 15) return ANSLIN_ERR_INVALID_ARG;
     if (scaled && !x_scales[i]) return ANSLIN_ERR_INVALID_ARG;
     if (ldx[i] < int64_t(h.k_in) || (ldx[i] * xb) % 16 || ldy[i] < int64_t(h.n_out)) return ANSLIN_ERR_INVALID_ARG;
@@ -850,13 +878,21 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   const int RB = int(h0.tile_n) / 32, J = RB == 1 ? kJ32 : 1, NW = 4 / (RB * J);
   // shared memory: U operand slots, D*J stream rings, slot table, barriers
   const size_t fixed = 2048 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 96;
+  const bool ls = h0.flags & ANSLIN_FLAG_LANE_STREAMS;
+  if (ls && RB != 1) return ANSLIN_ERR_CORRUPT;
+  uint32_t stream_bytes = kStreamSmem;
+  if (ls) {
+    stream_bytes = 32;
+    for (int i = 0; i < n; ++i) stream_bytes = std::max<uint32_t>(stream_bytes, uint32_t(align16(ws[i]->h.max_seg_bytes)));
+  }
+  p.stream_bytes = stream_bytes;
   uint32_t D = kMaxDecWarps, U = 0;
   if (const char *denv = getenv("ANSLIN_DECODER_WARPS"))
     if (atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
   D -= D % NW;
   uint32_t Bslots = 0;
   for (; D >= uint32_t(NW); D -= NW) {   // most decoder warps that still leave every team two private operand slots
-    const size_t rings = size_t(D) * J * kStreamSmem;
+    const size_t rings = size_t(D) * J * stream_bytes;
     if (kSmemMax < fixed + rings) continue;
     const uint32_t PT = D / NW;
     Bslots = uint32_t(std::min<size_t>((kSmemMax - fixed - rings) / p.slot_bytes, kMaxSlots) / PT);
@@ -868,7 +904,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   p.D = D;
   p.U = U;
   p.B = Bslots;
-  const size_t smem = fixed + size_t(D) * J * kStreamSmem + size_t(U) * p.slot_bytes;
+  const size_t smem = fixed + size_t(D) * J * stream_bytes + size_t(U) * p.slot_bytes;
   // CTAs: one per SM in total, shared out in proportion to the problems' sizes (each at least one, at most one per group)
   const uint32_t S = uint32_t(sm_budget());
   uint32_t ncta[kMaxProblems], used = 0;
@@ -920,7 +956,9 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   if (cudaMemsetAsync(wsb, 0, counters_bytes, st) != cudaSuccess) return ANSLIN_ERR_CUDA;
   const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
   const uint32_t grid = cta0;
-#define ANSLIN_LAUNCH(F, PAY) (RB == 1 ? launch_fused<F, 1, PAY>(tms, p, grid, smem, st) : launch_fused<F, 4, PAY>(tms, p, grid, smem, st))
+#define ANSLIN_LAUNCH(F, PAY)                                                                                   \
+  (RB == 1 ? (ls ? launch_fused<F, 1, PAY, true>(tms, p, grid, smem, st) : launch_fused<F, 1, PAY, false>(tms, p, grid, smem, st)) \
+           : launch_fused<F, 4, PAY, false>(tms, p, grid, smem, st))
   switch (h0.format) {
     case ANSLIN_FMT_BF16: return pay ? ANSLIN_LAUNCH(ANSLIN_FMT_BF16, true) : ANSLIN_LAUNCH(ANSLIN_FMT_BF16, false);
     case ANSLIN_FMT_FP8_E4M3: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);
@@ -943,27 +981,30 @@ size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_ma
   return counters + per_launch;
 }
 
-template <uint32_t FMT, int RB, bool PAYLOAD>
+template <uint32_t FMT, int RB, bool PAYLOAD, bool LS>
 int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   uint32_t per_sm = 4;
   if (const char *e = getenv("ANSLIN_DECODE_CTAS_PER_SM")) per_sm = uint32_t(std::max(1, atoi(e)));  // debug knob
   constexpr int J = RB == 1 ? kJ32 : 1;
   const uint32_t jobs = cv.n_tiles / J;
   const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
-  auto kern = decode_kernel<FMT, RB, J, PAYLOAD>;
-  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * kStreamSmem;
-  static thread_local bool attr_set = false;   // per instantiation
-  if (!attr_set) {
+  auto kern = decode_kernel<FMT, RB, J, PAYLOAD, LS>;
+  const uint32_t stream_bytes = LS ? uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32))) : kStreamSmem;
+  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * stream_bytes;
+  if (smem > kSmemMax) return ANSLIN_ERR_UNSUPPORTED;
+  static thread_local size_t smem_set = 0;   // per instantiation
+  if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
-    attr_set = true;
+    smem_set = smem;
   }
-  kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out));
+  kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out), stream_bytes);
   ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 template <uint32_t FMT, bool PAYLOAD>
 int launch_decode(const ContainerView &cv, void *out, cudaStream_t st) {
-  return cv.tile_n == 32 ? launch_decode_t<FMT, 1, PAYLOAD>(cv, out, st) : launch_decode_t<FMT, 4, PAYLOAD>(cv, out, st);
+  if (cv.flags & ANSLIN_FLAG_LANE_STREAMS) return cv.tile_n == 32 ? launch_decode_t<FMT, 1, PAYLOAD, true>(cv, out, st) : int(ANSLIN_ERR_CORRUPT);
+  return cv.tile_n == 32 ? launch_decode_t<FMT, 1, PAYLOAD, false>(cv, out, st) : launch_decode_t<FMT, 4, PAYLOAD, false>(cv, out, st);
 }
 
 template <uint32_t FMT>

@@ -54,6 +54,15 @@ def _decode_cases():
     yield "fp8-32x384", B.FMT_FP8_E4M3, f8, 768, dict(tile_k=384, w_scale=sc, tile_n=32)
     yield "int4-32x256", B.FMT_INT4_AWQ, p4, 768, dict(tile_k=256, scales=s4, zeros=z4, group_size=128, tile_n=32)
     yield "bf16-constant-32", B.FMT_BF16, np.full((128, 64), 0xBF80, dtype=np.uint16), 64, dict(tile_k=64, tile_n=32)
+    # lane-stream layout (every lane its own word stream, segments of 256 steps)
+    wl = inputs.f32_to_bf16_bits(inputs.weights_f32(384, 1024, seed=45, jitter=True))
+    yield "bf16-32x256-lanes-payload", B.FMT_BF16, wl, 1024, dict(tile_k=256, flags=3, tile_n=32)
+    yield "bf16-32x512-lanes", B.FMT_BF16, wl, 1024, dict(tile_k=512, flags=2, tile_n=32)
+    yield "int8-32x256-lanes", B.FMT_INT8, q8, 768, dict(tile_k=256, scales=s8, tile_n=32, flags=2)
+    yield "fp8-32x768-lanes", B.FMT_FP8_E4M3, f8, 768, dict(tile_k=768, w_scale=sc, tile_n=32, flags=2)
+    p4l, s4l, z4l = inputs.quant_awq4_weights(inputs.weights_f32(256, 1024, seed=46, outliers=False), 128)
+    yield "int4-32x512-lanes", B.FMT_INT4_AWQ, p4l, 1024, dict(tile_k=512, scales=s4l, zeros=z4l, group_size=128, tile_n=32, flags=2)
+    yield "bf16-constant-lanes", B.FMT_BF16, np.full((128, 256), 0xBF80, dtype=np.uint16), 256, dict(tile_k=256, tile_n=32, flags=2)
 
 
 @pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_decode_cases()), ids=[c[0] for c in _decode_cases()])
@@ -80,18 +89,20 @@ def test_decode_config1_full():
 
 
 # ------------------------------------------------------------------ fused GEMM (a4-a10)
-TILES = [(128, 64), (32, 256)]      # (tile_n, bf16 tile_k): BASELINE config 1's 128 x 64 and the 32-row shape bench.py uses
+# (tile_n, bf16 tile_k, layout flag): BASELINE config 1's 128 x 64, 32-row tiles, and 32-row tiles with lane streams (bench.py)
+TILES = [(128, 64, 0), (32, 256, 0), (32, 256, 2)]
+TILE_IDS = ["128x64", "32x256", "32x256-lanes"]
 
 
 @pytest.mark.parametrize("m", [1, 8, 16, 47, 75])
 @pytest.mark.parametrize("flags", [0, 1])
-@pytest.mark.parametrize("tile", TILES, ids=["128x64", "32x256"])
+@pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 def test_gemm_bf16(m, flags, tile):
     rt = _rt()
     n, k = 640, 1024      # 5 stripes x 16 (4) k-tiles: spans several CTAs and split-K segments
     w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=51, jitter=True))
     x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=52))
-    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=flags, tile_n=tile[0])
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=flags | tile[2], tile_n=tile[0])
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
     y_ref, a_ref = og.gemm_bf16(x, w)
@@ -99,12 +110,12 @@ def test_gemm_bf16(m, flags, tile):
     dw.close()
 
 
-@pytest.mark.parametrize("tile", TILES, ids=["128x64", "32x256"])
+@pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 def test_gemm_config1_and_unit_vector(tile):
     """BASELINE config 1 (W 1024x1024 bf16, X 8x1024) and the e_k special case: Y = column k of W exactly."""
     rt = _rt()
     w, x = inputs.config1()
-    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=tile[1], flags=1, tile_n=tile[0])
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 1024, 1024, tile_k=tile[1], flags=1 | tile[2], tile_n=tile[0])
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
     check_gemm(y, *og.gemm_bf16(x, w))
@@ -116,15 +127,20 @@ def test_gemm_config1_and_unit_vector(tile):
     dw.close()
 
 
-@pytest.mark.parametrize("tile_n", [128, 32])
+LAYOUTS = [(128, 0), (32, 0), (32, 2)]      # (tile_n, layout flag)
+LAYOUT_IDS = ["128", "32", "32-lanes"]
+
+
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
 @pytest.mark.parametrize("m", [1, 32, 75])
-def test_gemm_int8(m, tile_n):
+def test_gemm_int8(m, lay):
+    tile_n, lflag = lay
     rt = _rt()
     import torch
     n, k = 384, 1536
     q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=61, jitter=True))
     xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=62))
-    buf, _ = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=256, scales=s, tile_n=tile_n)
+    buf, _ = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=256, scales=s, tile_n=tile_n, flags=lflag)
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
     y_ref, a_ref, acc = og.gemm_int8(xq, xs, q, s)
@@ -136,38 +152,41 @@ def test_gemm_int8(m, tile_n):
     dw.close()
 
 
-@pytest.mark.parametrize("tile_n", [128, 32])
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
 @pytest.mark.parametrize("m", [1, 20, 64])
-def test_gemm_fp8(m, tile_n):
+def test_gemm_fp8(m, lay):
+    tile_n, lflag = lay
     rt = _rt()
     import torch
     n, k = 256, 1536
     f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=71, std=0.015, outliers=False))
     x8, xs = inputs.quant_fp8_acts(inputs.acts_f32(m, k, seed=72))
-    buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc, tile_n=tile_n)
+    buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc, tile_n=tile_n, flags=lflag)
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
     check_gemm(y, *og.gemm_fp8(x8, xs, f8, sc))
     dw.close()
 
 
-@pytest.mark.parametrize("tile_n", [128, 32])
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
 @pytest.mark.parametrize("m", [1, 16, 64])
-def test_gemm_int4(m, tile_n):
+def test_gemm_int4(m, lay):
+    tile_n, lflag = lay
     rt = _rt()
     n, k = 256, 1024
     p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=81, outliers=False), 128)
     x = inputs.acts_f32(m, k, seed=82).astype(np.float16)
     buf, _ = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=256 if tile_n == 128 else 512, scales=s4, zeros=z4,
-                                  group_size=128, tile_n=tile_n)
+                                  group_size=128, tile_n=tile_n, flags=lflag)
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
     check_gemm(y, *og.gemm_int4(x, p4, s4, z4, 128))
     dw.close()
 
 
-@pytest.mark.parametrize("tile_n", [128, 32])
-def test_gemm_grouped_fp8(tile_n):
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
+def test_gemm_grouped_fp8(lay):
+    tile_n, lflag = lay
     """BASELINE config 5 in miniature: 8 experts, top-2 routing, rows sorted by expert."""
     rt = _rt()
     import torch
@@ -178,7 +197,7 @@ def test_gemm_grouped_fp8(tile_n):
     experts, refs = [], []
     for e in range(E):
         f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=100 + e, std=0.015, outliers=False))
-        buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc, tile_n=tile_n)
+        buf, _ = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=256, w_scale=sc, tile_n=tile_n, flags=lflag)
         experts.append(rt.DeviceWeight(buf))
         refs.append((f8, sc))
     y = rt.gemm_grouped(experts, rows, rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
@@ -201,7 +220,7 @@ def test_gemm_multi_qkv_shapes():
     ws, dws = [], []
     for i, n in enumerate((640, 128, 256)):
         w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=96 + i, jitter=True))
-        buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=1, tile_n=32)
+        buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
         ws.append(w); dws.append(rt.DeviceWeight(buf))
     mg = rt.MultiGemm(dws, [xd, xd, xd])
     ys = [y.cpu().numpy() for y in mg()]
@@ -244,7 +263,7 @@ def test_dense_gemm_int8_fp8():
 
 
 # ------------------------------------------------------------------ full-size launch configuration
-@pytest.mark.parametrize("tile", TILES, ids=["128x64", "32x256"])
+@pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 @pytest.mark.parametrize("name,n,k,m", [("gate", 13824, 5120, 75), ("down", 5120, 13824, 16), ("k", 1024, 5120, 1)])
 def test_gemm_bf16_full_size_projection(name, n, k, m, tile):
     """BASELINE config 2 shapes in the launch configuration bench.py times (148 persistent CTAs,
@@ -253,7 +272,7 @@ def test_gemm_bf16_full_size_projection(name, n, k, m, tile):
     rt = _rt()
     w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=7, jitter=True))
     x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=8))
-    buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=1, tile_n=tile[0])
+    buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=1 | tile[2], tile_n=tile[0])
     assert st["bits_per_weight"] - st["entropy_bits_per_symbol"] - st["raw_entropy_bits_per_symbol"] <= 0.1
     dw = rt.DeviceWeight(buf)
     assert np.array_equal(dw.decode().cpu().numpy().view(np.uint16), w)

@@ -38,6 +38,8 @@ def _cases():
     yield "bf16-tile128", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=128, flags=1)
     yield "bf16-32x256", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=256, flags=1, tile_n=32)
     yield "bf16-32x64", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=64, tile_n=32)
+    yield "bf16-32x256-lanes", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=256, flags=3, tile_n=32)
+    yield "bf16-32x512-lanes", oc.FMT_BF16, inputs.f32_to_bf16_bits(wf), 512, dict(tile_k=512, flags=2, tile_n=32)
     q8, s8 = inputs.quant_sq8_weights(wf)
     yield "int8", oc.FMT_INT8, q8, 512, dict(tile_k=256, scales=s8)
     f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(128, 512, seed=32, std=0.015, outliers=False))
@@ -47,6 +49,9 @@ def _cases():
     yield "int8-32x256", oc.FMT_INT8, q8, 512, dict(tile_k=256, scales=s8, tile_n=32)
     yield "fp8-32x512", oc.FMT_FP8_E4M3, f8, 512, dict(tile_k=512, w_scale=sc, tile_n=32)
     yield "int4-32x512", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=512, scales=s4, zeros=z4, group_size=128, tile_n=32)
+    yield "int8-32x512-lanes", oc.FMT_INT8, q8, 512, dict(tile_k=512, scales=s8, tile_n=32, flags=2)
+    yield "fp8-32x256-lanes", oc.FMT_FP8_E4M3, f8, 512, dict(tile_k=256, w_scale=sc, tile_n=32, flags=2)
+    yield "int4-32x512-lanes", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=512, scales=s4, zeros=z4, group_size=128, tile_n=32, flags=2)
 
 
 @pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_cases()), ids=[c[0] for c in _cases()])
