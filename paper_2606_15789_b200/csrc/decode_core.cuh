@@ -150,8 +150,9 @@ __device__ __forceinline__ void stream_upkeep8(Stream (&s)[J], uint32_t ring0, i
 // One decode step of Alg V.2 for all 32 lanes of one stream; returns the table entry (symbol in bits 7:0).
 __device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint32_t lt) {
   uint32_t ea, e;
-  asm("mad.lo.u32 %0, %1, 4, %2;" : "=r"(ea) : "r"(s.x & (kM - 1)), "r"(tab_s));
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea));
+  asm("mul.lo.u32 %0, %1, 4;" : "=r"(ea) : "r"(s.x));          // shift on the FMA pipe (IMAD.SHL), mask on the ALU,
+  asm("and.b32 %0, %0, 0x3FFC;" : "+r"(ea));                   // table base folded into the load's address operand
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea + tab_s));
   uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
   // renormalisation: the lanes with x < 2^16 read consecutive words, x = (x << 16) | word
   asm volatile(
@@ -220,8 +221,9 @@ __device__ __forceinline__ void lane_open_segment(LaneStream &s, uint32_t buf, u
 // One decode step of Alg V.2 for all 32 lanes of one lane-stream tile; dir = +2 (even lanes) / -2 (odd lanes).
 __device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uint32_t dir) {
   uint32_t ea, e;
-  asm("mad.lo.u32 %0, %1, 4, %2;" : "=r"(ea) : "r"(s.x & (kM - 1)), "r"(tab_s));
-  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea));
+  asm("mul.lo.u32 %0, %1, 4;" : "=r"(ea) : "r"(s.x));          // shift on the FMA pipe (IMAD.SHL), mask on the ALU,
+  asm("and.b32 %0, %0, 0x3FFC;" : "+r"(ea));                   // table base folded into the load's address operand
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea + tab_s));
   uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
@@ -266,14 +268,31 @@ __device__ __forceinline__ void decode4(typename POL::S (&s)[J], uint32_t (&q)[J
   for (int j = 0; j < J; ++j) q[j] = put_sym<3>(q[j], POL::step(s[j], tab, aux));
 }
 
-// bf16: merge 4 exponent bytes (E) with 4 raw bytes (R = mantissa<<1 | sign) into 4 bf16 values:
-// each 16-bit (E<<8 | R) rotated right by one bit.
-__device__ __forceinline__ uint2 bf16_merge4(uint32_t E, uint32_t R) {
-  const uint32_t p0 = __byte_perm(R, E, 0x5140), p1 = __byte_perm(R, E, 0x7362);
-  uint2 o;
-  o.x = ((p0 >> 1) & 0x7FFF7FFFu) | ((p0 << 15) & 0x80008000u);
-  o.y = ((p1 >> 1) & 0x7FFF7FFFu) | ((p1 << 15) & 0x80008000u);
+// bf16: two decode steps + two raw bytes (R = mantissa<<1 | sign, bytes 2k', 2k'+1 of Rw) -> two bf16 values.
+// p = [R_a, E_a, R_b, E_b] (two PRMTs straight from the table entries), then each 16-bit (E<<8 | R) is rotated
+// right by one bit: shift, shift, one bit-select.
+template <int KP>
+__device__ __forceinline__ uint32_t bf16_pair(uint32_t Rw, uint32_t e_a, uint32_t e_b) {
+  const uint32_t t = __byte_perm(Rw, e_a, KP == 0 ? 0x0140 : 0x0342);   // [R_a, E_a, R_b, -]
+  const uint32_t p = __byte_perm(t, e_b, 0x4210);                        // [R_a, E_a, R_b, E_b]
+  uint32_t o;
+  asm("lop3.b32 %0, %1, %2, 0x7FFF7FFF, 0xE4;" : "=r"(o) : "r"(p >> 1), "r"(p << 15));   // (a & c) | (b & ~c)
   return o;
+}
+// Eight decode steps of each of the J streams, interleaved, merged with 8 raw bytes (R0, R1) -> one 16-byte chunk each.
+template <class POL, int J>
+__device__ __forceinline__ void decode8_bf16(typename POL::S (&s)[J], uint32_t tab, uint32_t aux, const uint32_t (&R0)[J],
+                                             const uint32_t (&R1)[J], uint4 (&out)[J]) {
+  uint32_t ea[J], eb[J];
+#define ANSLIN_PAIR(KP, RW, DST)                                              \
+  _Pragma("unroll") for (int j = 0; j < J; ++j) ea[j] = POL::step(s[j], tab, aux); \
+  _Pragma("unroll") for (int j = 0; j < J; ++j) eb[j] = POL::step(s[j], tab, aux); \
+  _Pragma("unroll") for (int j = 0; j < J; ++j) out[j].DST = bf16_pair<KP>(RW[j], ea[j], eb[j]);
+  ANSLIN_PAIR(0, R0, x)
+  ANSLIN_PAIR(1, R0, y)
+  ANSLIN_PAIR(0, R1, z)
+  ANSLIN_PAIR(1, R1, w)
+#undef ANSLIN_PAIR
 }
 
 // int4 (AWQ-style): one packed byte (low nibble = even k) -> two fp16 weights (q - z) * s.
@@ -342,18 +361,24 @@ __device__ __forceinline__ void decode_unit(typename POL::S (&s)[J], uint32_t ri
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
         POL::template upkeep8<J>(s, ring0, lane);
-        uint32_t E0[J], E1[J];
-        decode4<POL, J>(s, E0, tab, lt);
-        decode4<POL, J>(s, E1, tab, lt);
+        uint32_t R0[J], R1[J];
+        uint4 o[J];
 #pragma unroll
-        for (int j = 0; j < J; ++j) {
-          if (kPayload && h == 1 && v == V - 1) {  // last 8 steps of the tile: bytes 14,15 ride in the state
-            const uint32_t p = s[j].x - kL;
-            rv[j].w = (rv[j].w & 0xFFFFu) | (p << 16);
+        for (int j = 0; j < J; ++j) { R0[j] = h ? rv[j].z : rv[j].x; R1[j] = h ? rv[j].w : rv[j].y; }
+        if (kPayload && h == 1 && v == V - 1) {
+          // last 8 steps of the tile: raw bytes 14,15 ride in the END state, known only after the last step, so
+          // the last pair is decoded without raw bytes and they are merged in afterwards
+          decode8_bf16<POL, J>(s, tab, lt, R0, R1, o);
+#pragma unroll
+          for (int j = 0; j < J; ++j) {
+            const uint32_t pl = s[j].x - kL;   // byte 14 | byte 15 << 8, each = mantissa<<1 | sign
+            o[j].w |= ((pl >> 1) & 0x7Fu) | ((pl & 1u) << 15) | (((pl >> 9) & 0x7Fu) << 16) | (((pl >> 8) & 1u) << 31);
           }
-          const uint2 a = bf16_merge4(E0[j], h ? rv[j].z : rv[j].x), b = bf16_merge4(E1[j], h ? rv[j].w : rv[j].y);
-          emit.chunk(j, g2 * 2 + h, lane, make_uint4(a.x, a.y, b.x, b.y));
+        } else {
+          decode8_bf16<POL, J>(s, tab, lt, R0, R1, o);
         }
+#pragma unroll
+        for (int j = 0; j < J; ++j) emit.chunk(j, g2 * 2 + h, lane, o[j]);
       }
     }
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
