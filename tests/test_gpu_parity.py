@@ -283,3 +283,79 @@ def test_gemm_bf16_full_size_projection(name, n, k, m, tile):
     y2 = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
     assert np.array_equal(y, y2), "split-K fix-up must be deterministic"
     dw.close()
+
+
+# ------------------------------------------------------------------ BASELINE configs 3-5 at full size
+def _sample_cols(n, seed, count=512):
+    return np.sort(np.random.default_rng(seed).choice(n, size=min(n, count), replace=False))
+
+
+@pytest.mark.parametrize("lay", [(128, 256, 0), (32, 1024, 2)], ids=["128x256", "32x1024-lanes"])
+def test_config3_int8_full_size(lay):
+    """BASELINE config 3: Qwen-14B gate projection 13824 x 5120 in SQ8-style int8, M = 75: decode bit-exact on the
+    whole tensor, fused GEMM on all rows x sampled channels, integer sums exact, bits/weight within 0.1 of H."""
+    rt = _rt()
+    import torch
+    n, k, m = 13824, 5120, 75
+    q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=5, jitter=True))
+    xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=6))
+    buf, st = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=lay[1], scales=s, tile_n=lay[0], flags=lay[2])
+    assert 0.0 <= st["bits_per_weight"] - st["entropy_bits_per_symbol"] <= 0.1
+    dw = rt.DeviceWeight(buf)
+    assert np.array_equal(dw.decode().cpu().numpy().view(np.int8), q)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
+    cols = _sample_cols(n, 9)
+    y_ref, a_ref, acc = og.gemm_int8(xq, xs, q[cols], s[cols])
+    check_gemm(y[:, cols], y_ref, a_ref)
+    back = np.rint(y[:, cols].astype(np.float64) / (xs.astype(np.float64)[:, None] * s[cols].astype(np.float64)[None, :]))
+    small = np.abs(acc) < (1 << 22)
+    assert np.array_equal(back[small], acc[small].astype(np.float64))
+    dw.close()
+
+
+@pytest.mark.parametrize("lay", [(128, 256, 0), (32, 1024, 2)], ids=["128x256", "32x1024-lanes"])
+def test_config4_int4_full_size(lay):
+    """BASELINE config 4: Llama-70B gate projection 28672 x 8192, AWQ-style int4 (group 128), fp16 X, M = 64."""
+    rt = _rt()
+    n, k, m = 28672, 8192, 64
+    p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=11, outliers=False), 128)
+    x = inputs.acts_f32(m, k, seed=12).astype(np.float16)
+    buf, st = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=lay[1], scales=s4, zeros=z4, group_size=128, tile_n=lay[0],
+                                  flags=lay[2])
+    assert 0.0 <= st["bits_per_weight"] - st["entropy_bits_per_symbol"] / 2 <= 0.1
+    dw = rt.DeviceWeight(buf)
+    assert np.array_equal(dw.decode().cpu().numpy(), p4)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
+    cols = _sample_cols(n, 13)
+    check_gemm(y[:, cols], *og.gemm_int4(x, p4[cols], s4[cols], z4[cols], 128))
+    dw.close()
+
+
+@pytest.mark.parametrize("lay", [(128, 256, 0), (32, 1024, 2)], ids=["128x256", "32x1024-lanes"])
+def test_config5_fp8_moe_full_size(lay):
+    """BASELINE config 5: 8 Mixtral-8x22B-shaped experts (gate 16384 x 6144, e4m3), 95 tokens routed top-2:
+    one grouped persistent launch over the active experts; every expert's rows checked on sampled channels."""
+    rt = _rt()
+    import torch
+    n, k, E, tokens = 16384, 6144, 8, 95
+    rows, tok = inputs.route_top2(tokens, E, seed=21)
+    x8_tok, xs_tok = inputs.quant_fp8_acts(inputs.acts_f32(tokens, k, seed=22))
+    x8, xs = x8_tok[tok], xs_tok[tok]
+    experts, refs = [], []
+    for e in range(E):
+        f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=30 + e, std=0.015, outliers=False))
+        buf, st = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=lay[1], w_scale=sc, tile_n=lay[0], flags=lay[2])
+        assert 0.0 <= st["bits_per_weight"] - st["entropy_bits_per_symbol"] <= 0.1
+        experts.append(rt.DeviceWeight(buf))
+        refs.append((f8, sc))
+    assert np.array_equal(experts[3].decode().cpu().numpy(), refs[3][0])
+    y = rt.gemm_grouped(experts, rows, rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
+    r0 = 0
+    for e in range(E):
+        r1 = r0 + int(rows[e])
+        if r1 > r0:
+            cols = _sample_cols(n, 40 + e, 256)
+            check_gemm(y[r0:r1][:, cols], *og.gemm_fp8(x8[r0:r1], xs[r0:r1], refs[e][0][cols], refs[e][1]))
+        r0 = r1
+    for d in experts:
+        d.close()
