@@ -607,6 +607,29 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       }
     };
     const uint32_t stripe0 = t_begin / KT;
+    // per-unit work of this warp is the serial bottleneck of the CTA once the decoders are fast (one unit per
+    // ~0.3 us): descriptors are advanced by adds, segment bookkeeping is hoisted out of the unit loop
+    const uint64_t adesc0 = make_smem_desc(slots_s, 16, 256, kLayoutSW32);
+    const uint32_t desc_hi = uint32_t(adesc0 >> 32), adesc0_lo = uint32_t(adesc0), slot_units = P.slot_bytes >> 4;
+    auto consume = [&](uint32_t slot, uint32_t par, uint32_t d_tmem, uint32_t accumulate, bool last, uint32_t tfull_bar) {
+      if (rel < n_commit) release(n_commit, false);
+      mbar_wait(full_s + 8 * slot, par);
+      tc_fence_after();
+      if (lane == 0) {
+        const uint32_t alo = adesc0_lo + slot * slot_units;   // start address field: (slots_s + slot * slot_bytes) >> 4
+        const uint64_t ad = (uint64_t(desc_hi) << 32) | alo, bd = (uint64_t(desc_hi) << 32) | (alo + (kUnitBytes >> 4));
+#ifndef ANSLIN_DBG_NOMMA
+        umma<TR::kind>(d_tmem, ad, bd, idesc, accumulate);
+        umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
+        if (last) umma_commit(tfull_bar);
+#else
+        (void)ad; (void)bd; (void)idesc;
+        mbar_arrive(empty_s + 8 * slot);
+        if (last) mbar_arrive(tfull_bar);
+#endif
+      }
+      __syncwarp();
+    };
 #ifdef ANSLIN_DBG_DECONLY
     if (false)
 #endif
@@ -623,32 +646,25 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           mbar_wait(tempty_s + 8 * (sg & 1u), ((sg >> 1) & 1u) ^ 1u);
           tc_fence_after();
         }
+        const uint32_t first1 = s1 == 0 ? 0u : (stripe0 + s1) * KT - t_begin, last1 = min(N, (stripe0 + s1 + 1) * KT - t_begin) - 1;
+        const uint32_t last2 = min(N, (stripe0 + s1 + 2) * KT - t_begin) - 1;   // segment s1 + 1 starts at e1 when it is in the window
+        const uint32_t d1 = tmem_base + (s1 & 1u) * mpad, d2 = tmem_base + ((s1 + 1) & 1u) * mpad;
+        const uint32_t tf1 = tfull_s + 8 * (s1 & 1u), tf2 = tfull_s + 8 * ((s1 + 1) & 1u);
+        uint32_t n_unit = rho * units, bsel = n_unit % P.B, par = (n_unit / P.B) & 1u;
         for (uint32_t u = 0; u < units; ++u) {
-          const uint32_t n_unit = rho * units + u, bsel = n_unit % P.B, par = (n_unit / P.B) & 1u;
-          for (uint32_t i = i0; i < e2; ++i) {
-            const uint32_t sg = i < e1 ? s1 : s1 + 1, ab = sg & 1u;
-            const uint32_t seg_first = sg == 0 ? 0u : (stripe0 + sg) * KT - t_begin, seg_last = min(N, (stripe0 + sg + 1) * KT - t_begin) - 1;
-            const uint32_t slot = (i - ga) * P.B + bsel;
-            release(n_commit, false);
-            mbar_wait(full_s + 8 * slot, par);
-            tc_fence_after();
-            const bool last = (u + 1 == units && i == seg_last);
-            if (lane == 0) {
-              const uint32_t a = slots_s + slot * P.slot_bytes, b = a + kUnitBytes;
-#ifndef ANSLIN_DBG_NOMMA
-              umma<TR::kind>(tmem_base + ab * mpad, make_smem_desc(a, 16, 256, kLayoutSW32), make_smem_desc(b, 16, 256, kLayoutSW32),
-                             idesc, (u == 0 && i == seg_first) ? 0u : 1u);
-              umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
-              if (last) umma_commit(tfull_s + 8 * ab);
-#else
-              (void)a; (void)b; (void)idesc;
-              mbar_arrive(empty_s + 8 * slot);
-              if (last) mbar_arrive(tfull_s + 8 * ab);
-#endif
-            }
+          const bool lastu = u + 1 == units;
+          uint32_t slot = (i0 - ga) * P.B + bsel;
+          for (uint32_t i = i0; i < e1; ++i, slot += P.B) {
+            const bool last = lastu && i == last1;
+            consume(slot, par, d1, (u == 0 && i == first1) ? 0u : 1u, last, tf1);
             if (last) ++n_commit;
-            __syncwarp();
           }
+          for (uint32_t i = e1; i < e2; ++i, slot += P.B) {
+            const bool last = lastu && i == last2;
+            consume(slot, par, d2, (u == 0 && i == e1) ? 0u : 1u, last, tf2);
+            if (last) ++n_commit;
+          }
+          if (++bsel == P.B) { bsel = 0; par ^= 1u; }
         }
         i0 = e2;
       }
