@@ -193,16 +193,47 @@ __host__ __device__ constexpr size_t row_bytes_of(uint32_t fmt, size_t k) {
 template <uint32_t FMT, int RB, int J>
 struct GlobalEmit {
   static constexpr bool kOperand = false;
+  // 32-row tiles (lane = row): a lane's 16-byte chunks of two consecutive units (64 B of its row) are staged in
+  // shared memory and written out as 64-byte row segments, 8 rows per store instruction, instead of one 16-byte
+  // store per lane into 32 different rows (which bound the kernel at a third of the decoder's rate).
+  static constexpr bool kStaged = RB == 1 && FMT != ANSLIN_FMT_INT4_AWQ;
+  static constexpr uint32_t kStageBytes = kStaged ? 2048 : 0;   // per stream
   uint8_t *tile_out[J];  // &W[first row of tile j][k0] in bytes
   size_t row_bytes;      // bytes per W row
+  uint32_t stage;        // shared address of this warp's J staging areas
   int u;
 #ifdef ANSLIN_PROBE_NOSTORE   // developer probe: decode throughput without the HBM stores
   uint32_t chk = 0;
   __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) { chk ^= v.x ^ v.y ^ v.z ^ v.w; }
+  __device__ __forceinline__ void unit_done(int) {}
 #else
   __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {  // bf16 / fp8 / int8: 16 B of row-major W
-    uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 32 + (g / RB) * 16;
-    *reinterpret_cast<uint4 *>(p) = v;
+    if constexpr (kStaged) {
+      const uint32_t c = uint32_t((u & 1) * 2 + g);
+      sts128(stage + uint32_t(j) * kStageBytes + uint32_t(lane) * 64u + ((c ^ ((uint32_t(lane) >> 1) & 3u)) << 4), v);
+    } else {
+      uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 32 + (g / RB) * 16;
+      *reinterpret_cast<uint4 *>(p) = v;
+    }
+  }
+  // after every unit; with staging, units 2n and 2n+1 are flushed together
+  __device__ __forceinline__ void unit_done(int lane) const {
+    if constexpr (kStaged) {
+      if ((u & 1) == 0) return;
+      __syncwarp();
+#pragma unroll
+      for (int j = 0; j < J; ++j)
+#pragma unroll
+        for (int it = 0; it < 4; ++it) {
+          const uint32_t r = uint32_t(it * 8 + (lane >> 2)), c = uint32_t(lane & 3);
+          uint4 v;
+          asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];"
+                       : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+                       : "r"(stage + uint32_t(j) * kStageBytes + r * 64u + ((c ^ ((r >> 1) & 3u)) << 4)));
+          *reinterpret_cast<uint4 *>(tile_out[j] + size_t(r) * row_bytes + size_t(u - 1) * 32 + c * 16) = v;
+        }
+      __syncwarp();
+    }
   }
 #endif
   __device__ __forceinline__ void packed(int j, int g, int lane, uint32_t b) const {  // int4: 4 packed bytes = 8 weights
@@ -227,6 +258,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
   build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cv.base + cv.off_freq));
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t ring_s = smem_u32(rings) + uint32_t(warp) * J * stream_bytes;
+  const uint32_t stage_s = smem_u32(rings) + uint32_t(kDecWarps) * J * stream_bytes + uint32_t(warp) * J * GlobalEmit<FMT, RB, J>::kStageBytes;
   const uint32_t aux = LS ? ((lane & 1) ? uint32_t(-2) : 2u) : lanemask_lt();
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
   const size_t row_bytes = row_bytes_of(FMT, cv.k_in), tile_row_bytes = row_bytes_of(FMT, cv.tile_k);
@@ -239,6 +271,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
     const uint32_t *sz[J];
     GlobalEmit<FMT, RB, J> emit;
     emit.row_bytes = row_bytes;
+    emit.stage = stage_s;
     stream_drain();
 #pragma unroll
     for (int j = 0; j < J; ++j) {
@@ -259,6 +292,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
         }
       }
       decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, smem_u32(tab), lane, aux, int(u), V, raw, sz, emit);
+      emit.unit_done(lane);
     }
 #ifdef ANSLIN_PROBE_NOSTORE
     if (emit.chk == 0x12345678u) out[job] = 1;
@@ -1006,7 +1040,7 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
   auto kern = decode_kernel<FMT, RB, J, PAYLOAD, LS>;
   const uint32_t stream_bytes = LS ? uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32))) : kStreamSmem;
-  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * stream_bytes;
+  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * (stream_bytes + GlobalEmit<FMT, RB, J>::kStageBytes);
   if (smem > kSmemMax) return ANSLIN_ERR_UNSUPPORTED;
   static thread_local size_t smem_set = 0;   // per instantiation
   if (smem > smem_set) {
