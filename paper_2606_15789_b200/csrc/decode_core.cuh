@@ -238,16 +238,58 @@ __device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uin
   return e;
 }
 
+// Two lane-stream tiles, one step each, written so that the in-order issue overlaps the two dependent chains: both
+// table loads first, then both state updates, then both predicated word loads, then both merges.
+__device__ __forceinline__ void lane_step2(LaneStream &s0, LaneStream &s1, uint32_t tab_s, uint32_t dir, uint32_t &e0, uint32_t &e1) {
+  uint32_t a0, a1;
+  asm("mul.lo.u32 %0, %1, 4;" : "=r"(a0) : "r"(s0.x));
+  asm("mul.lo.u32 %0, %1, 4;" : "=r"(a1) : "r"(s1.x));
+  asm("and.b32 %0, %0, 0x3FFC;" : "+r"(a0));
+  asm("and.b32 %0, %0, 0x3FFC;" : "+r"(a1));
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e0) : "r"(a0 + tab_s));
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e1) : "r"(a1 + tab_s));
+  uint32_t x0 = ((e0 >> 8) & 0xFFFu) * (s0.x >> kProbBits) + (e0 >> 20);
+  uint32_t x1 = ((e1 >> 8) & 0xFFFu) * (s1.x >> kProbBits) + (e1 >> 20);
+  asm volatile(
+      "{\n\t.reg .pred p, q;\n\t"
+      "setp.lt.u32 p, %0, 65536;\n\t"
+      "setp.lt.u32 q, %3, 65536;\n\t"
+      "@p ld.shared.u16 %2, [%1];\n\t"
+      "@q ld.shared.u16 %5, [%4];\n\t"
+      "@p mad.lo.u32 %0, %0, 65536, %2;\n\t"
+      "@q mad.lo.u32 %3, %3, 65536, %5;\n\t"
+      "@p add.u32 %1, %1, %6;\n\t"
+      "@q add.u32 %4, %4, %6;\n\t}"
+      : "+r"(x0), "+r"(s0.ptr), "+r"(s0.w), "+r"(x1), "+r"(s1.ptr), "+r"(s1.w)
+      : "r"(dir)
+      : "memory");
+  s0.x = x0;
+  s1.x = x1;
+}
+
 // The two word layouts as policies of decode_unit.
 struct InterleavedWords {
   using S = Stream;
   template <int J> static __device__ __forceinline__ void upkeep8(S (&s)[J], uint32_t ring0, int lane) { stream_upkeep8<J>(s, ring0, lane); }
   static __device__ __forceinline__ uint32_t step(S &s, uint32_t tab, uint32_t lt) { return decode_step(s, tab, lt); }
+  template <int J> static __device__ __forceinline__ void steps(S (&s)[J], uint32_t tab, uint32_t lt, uint32_t (&e)[J]) {
+#pragma unroll
+    for (int j = 0; j < J; ++j) e[j] = decode_step(s[j], tab, lt);
+  }
 };
 struct LaneWords {
   using S = LaneStream;
   template <int J> static __device__ __forceinline__ void upkeep8(S (&)[J], uint32_t, int) {}
   static __device__ __forceinline__ uint32_t step(S &s, uint32_t tab, uint32_t dir) { return lane_step(s, tab, dir); }
+  // one step of each of the J streams
+  template <int J> static __device__ __forceinline__ void steps(S (&s)[J], uint32_t tab, uint32_t dir, uint32_t (&e)[J]) {
+    if constexpr (J == 2) {
+      lane_step2(s[0], s[1], tab, dir, e[0], e[1]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < J; ++j) e[j] = lane_step(s[j], tab, dir);
+    }
+  }
 };
 
 // Insert the symbol byte of table entry e at byte position `pos` of acc.
@@ -258,14 +300,19 @@ __device__ __forceinline__ uint32_t put_sym(uint32_t acc, uint32_t e) {
 // Four decode steps of each of the J streams, interleaved -> four symbol bytes per stream.
 template <class POL, int J>
 __device__ __forceinline__ void decode4(typename POL::S (&s)[J], uint32_t (&q)[J], uint32_t tab, uint32_t aux) {
+  uint32_t e[J];
+  POL::template steps<J>(s, tab, aux, e);
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<0>(0u, POL::step(s[j], tab, aux));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<0>(0u, e[j]);
+  POL::template steps<J>(s, tab, aux, e);
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<1>(q[j], POL::step(s[j], tab, aux));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<1>(q[j], e[j]);
+  POL::template steps<J>(s, tab, aux, e);
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<2>(q[j], POL::step(s[j], tab, aux));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<2>(q[j], e[j]);
+  POL::template steps<J>(s, tab, aux, e);
 #pragma unroll
-  for (int j = 0; j < J; ++j) q[j] = put_sym<3>(q[j], POL::step(s[j], tab, aux));
+  for (int j = 0; j < J; ++j) q[j] = put_sym<3>(q[j], e[j]);
 }
 
 // bf16: two decode steps + two raw bytes (R = mantissa<<1 | sign, bytes 2k', 2k'+1 of Rw) -> two bf16 values.
@@ -285,8 +332,8 @@ __device__ __forceinline__ void decode8_bf16(typename POL::S (&s)[J], uint32_t t
                                              const uint32_t (&R1)[J], uint4 (&out)[J]) {
   uint32_t ea[J], eb[J];
 #define ANSLIN_PAIR(KP, RW, DST)                                              \
-  _Pragma("unroll") for (int j = 0; j < J; ++j) ea[j] = POL::step(s[j], tab, aux); \
-  _Pragma("unroll") for (int j = 0; j < J; ++j) eb[j] = POL::step(s[j], tab, aux); \
+  POL::template steps<J>(s, tab, aux, ea);                                    \
+  POL::template steps<J>(s, tab, aux, eb);                                    \
   _Pragma("unroll") for (int j = 0; j < J; ++j) out[j].DST = bf16_pair<KP>(RW[j], ea[j], eb[j]);
   ANSLIN_PAIR(0, R0, x)
   ANSLIN_PAIR(1, R0, y)

@@ -381,7 +381,9 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
         const uint32_t mm = c0 + j;
         if (mm < p.m) {
           if (whole) p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(v[j], kScaled ? p.x_scale[mm] : 1.0f, ws);
+#ifndef ANSLIN_DBG_NOPART
           else part[size_t(mm) * kTileN + row] = v[j];
+#endif
         }
       }
     }
@@ -392,7 +394,9 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     if (false)
 #endif
     if (!whole) {
+#ifndef ANSLIN_DBG_NOTF
       __threadfence();
+#endif
       named_bar_sync(1, kEpiWarps * 32);
       if (warp == 0 && lane == 0) {
         const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
@@ -412,39 +416,63 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
 template <uint32_t FMT>
 __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *fin, uint32_t KT, uint32_t G, uint32_t T) {
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
+  constexpr int kItems = 2;   // items per thread and pass: their loads are all issued before the first add
   for (int seg = 0; seg < 2; ++seg) {
+#ifdef ANSLIN_DBG_NOFIX
+    continue;
+#endif
     if (!fin[seg].valid) continue;
     const uint32_t stripe = fin[seg].stripe, c_first = fin[seg].c_first, c_last = fin[seg].c_last;
-    for (uint32_t it = threadIdx.x; it < p.m * 32u; it += blockDim.x) {
-      const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u, n4 = stripe * kTileN + r4;
-      uint32_t acc[4];
+    // contributor cc's partial slot: its first segment (slot 0) unless the stripe is its second one, which can only
+    // be the case for the first contributor (every later one starts inside the stripe)
+    const uint32_t first_slot = cta_first_tile(c_first, G, T) < stripe * KT ? 1u : 0u;
+    const size_t slot_words = size_t(p.mpad) * kTileN;
+    const uint32_t n_items = p.m * 32u;
+    for (uint32_t it0 = threadIdx.x; it0 < n_items; it0 += blockDim.x * kItems) {
+      uint32_t acc[kItems][4];
 #pragma unroll
-      for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-      for (uint32_t cb = c_first; cb <= c_last; cb += 8) {
-        uint4 v[8];
+      for (int q = 0; q < kItems; ++q)
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const uint32_t cc = cb + j;
-          v[j] = make_uint4(0, 0, 0, 0);
-          if (cc <= c_last) {
-            const uint32_t ps = cc * 2u + (cta_first_tile(cc, G, T) / KT == stripe ? 0u : 1u);
-            v[j] = ldcg128(p.partials + (size_t(ps) * p.mpad + mm) * kTileN + r4);
+        for (int j = 0; j < 4; ++j) acc[q][j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
+      for (uint32_t cb = c_first; cb <= c_last; cb += 4) {
+        uint4 v[kItems][4];
+#pragma unroll
+        for (int q = 0; q < kItems; ++q) {
+          const uint32_t it = it0 + q * blockDim.x, mm = it >> 5, r4 = (it & 31u) * 4u;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            const uint32_t cc = cb + j;
+            v[q][j] = make_uint4(0, 0, 0, 0);
+            if (cc <= c_last && it < n_items) {
+              const uint32_t ps = cc * 2u + (cc == c_first ? first_slot : 0u);
+              v[q][j] = ldcg128(p.partials + size_t(ps) * slot_words + size_t(mm) * kTileN + r4);
+            }
           }
         }
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {  // fixed CTA order -> bit-reproducible sums
-          acc[0] = acc_add<FMT>(acc[0], v[j].x); acc[1] = acc_add<FMT>(acc[1], v[j].y);
-          acc[2] = acc_add<FMT>(acc[2], v[j].z); acc[3] = acc_add<FMT>(acc[3], v[j].w);
-        }
-      }
-      const float xs = kScaled ? p.x_scale[mm] : 1.0f;
-      float *yo = p.y + size_t(mm) * p.ldy + n4;
+        for (int q = 0; q < kItems; ++q)
 #pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        float ws = 1.0f;
-        if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
-        if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
-        yo[j] = finalize<FMT>(acc[j], xs, ws);
+          for (int j = 0; j < 4; ++j) {  // fixed CTA order -> bit-reproducible sums
+            acc[q][0] = acc_add<FMT>(acc[q][0], v[q][j].x); acc[q][1] = acc_add<FMT>(acc[q][1], v[q][j].y);
+            acc[q][2] = acc_add<FMT>(acc[q][2], v[q][j].z); acc[q][3] = acc_add<FMT>(acc[q][3], v[q][j].w);
+          }
+      }
+#pragma unroll
+      for (int q = 0; q < kItems; ++q) {
+        const uint32_t it = it0 + q * blockDim.x, mm = it >> 5, n4 = stripe * kTileN + (it & 31u) * 4u;
+        if (it >= n_items) continue;
+        const float xs = kScaled ? p.x_scale[mm] : 1.0f;
+        float o[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          float ws = 1.0f;
+          if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
+          if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
+          o[j] = finalize<FMT>(acc[q][j], xs, ws);
+        }
+        float *yo = p.y + size_t(mm) * p.ldy + n4;
+        if ((reinterpret_cast<uintptr_t>(yo) & 15) == 0) *reinterpret_cast<float4 *>(yo) = make_float4(o[0], o[1], o[2], o[3]);
+        else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
       }
     }
     if (threadIdx.x == 0) p.counters[stripe] = 0;   // every contributor has arrived: ready for the next launch
