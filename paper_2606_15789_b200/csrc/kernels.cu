@@ -20,6 +20,8 @@
 #include <string.h>
 #include <algorithm>
 #include <type_traits>
+#include <atomic>
+#include <chrono>
 
 #include "anslin_internal.h"
 #include "decode_core.cuh"
@@ -336,7 +338,9 @@ struct EpiParams {
   float w_scale;            // fp8
   float *y;
   int64_t ldy;
-  uint32_t *partials, *counters;   // [2*G][mpad][128] raw accumulator bits; [stripes]
+  uint32_t *partials;              // [2*G][mpad][128] raw accumulator bits
+  unsigned long long *counters;    // [stripes]: launch epoch << 32 | split-K contributors that have arrived
+  uint32_t epoch;                  // unique per launch: stale counter contents (any bytes) read as "nobody arrived"
   uint32_t m, mpad;
 };
 // A stripe whose last split-K contributor is this CTA (shared memory; at most the first and the last segment).
@@ -400,7 +404,16 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
       named_bar_sync(1, kEpiWarps * 32);
       if (warp == 0 && lane == 0) {
         const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
-        const bool last = atomicAdd(&p.counters[stripe], 1u) == c_last - c_first;
+        // arrive: count within this launch's epoch; no memset before and no reset after the launch is needed
+        unsigned long long *ctr = &p.counters[stripe];
+        unsigned long long seen = *reinterpret_cast<volatile unsigned long long *>(ctr), assumed;
+        do {
+          assumed = seen;
+          const unsigned long long next = uint32_t(assumed >> 32) == p.epoch ? assumed + 1ull : ((unsigned long long)(p.epoch) << 32) | 1ull;
+          seen = atomicCAS(ctr, assumed, next);
+        } while (seen != assumed);
+        const uint32_t before = uint32_t(assumed >> 32) == p.epoch ? uint32_t(assumed) : 0u;
+        const bool last = before == c_last - c_first;
         __threadfence();
         fin[seg].stripe = stripe; fin[seg].c_first = c_first; fin[seg].c_last = c_last; fin[seg].valid = last ? 1u : 0u;
       }
@@ -475,7 +488,6 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
         else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
       }
     }
-    if (threadIdx.x == 0) p.counters[stripe] = 0;   // every contributor has arrived: ready for the next launch
   }
 }
 
@@ -491,13 +503,14 @@ struct Problem {
   float *y;
   int64_t ldy;
   uint32_t *partials;      // [2*ncta][mpad][128] raw accumulator bits
-  uint32_t *counters;      // [stripes]
+  unsigned long long *counters;   // [stripes]
   uint32_t m, mpad, cta0, ncta;
 };
 struct FusedParams {
   Problem prob[kMaxProblems];
   uint32_t nprob;
   uint32_t U, D, B;        // operand slots (= teams * B), decoder warps, slots per team (>= 2)
+  uint32_t epoch;          // launch id for the split-K counters
   uint32_t stream_bytes;   // shared memory per stream: word ring + mirror, or the largest staged lane-stream segment
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
@@ -564,7 +577,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 
   const uint32_t t_begin = cta_first_tile(c, G, T), t_end = cta_first_tile(c + 1, G, T);
   const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, pr.y, pr.ldy,
-                     pr.partials, pr.counters, pr.m, mpad};
+                     pr.partials, pr.counters, P.epoch, pr.m, mpad};
 
   // Warp roles: decoders 0..D-1, epilogue D..D+3 (TMEM lane quadrant = warp % 4), MMA issuer D+4.  The
   // scheduler favours high warp ids, so the MMA issuer reacts first: a finished unit is consumed and its
@@ -753,7 +766,9 @@ struct DenseParams {
   const float *x_scale;
   float *y;
   int64_t ldy;
-  uint32_t *partials, *counters;
+  uint32_t *partials;
+  unsigned long long *counters;
+  uint32_t epoch;
   uint32_t n_out, k_in, m, mpad, S /*stages*/, stage_bytes, tmem_cols, KB /*k blocks of 128 B*/;
 };
 constexpr int kDenseThreads = 32 * 6;  // warps 0-3 epilogue, 4 MMA, 5 TMA producer
@@ -785,7 +800,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
   const uint32_t t_begin = cta_first_tile(blockIdx.x, G, T), t_end = cta_first_tile(blockIdx.x + 1, G, T);
-  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.m, p.mpad};
+  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.epoch, p.m, p.mpad};
 
   if (warp == 5) {
     if (lane == 0) {
@@ -889,11 +904,18 @@ uint32_t grid_of(uint32_t n_tiles, uint32_t min_tiles) {
   return uint32_t(std::min<uint64_t>(by_work, uint64_t(std::max(1, num_sms()))));
 }
 
+// Launch ids for the split-K counters: unique within the process and unlikely to equal whatever bytes an earlier
+// owner of the workspace left behind (seeded from the clock), so the workspace never has to be cleared.
+uint32_t next_epoch() {
+  static std::atomic<uint32_t> e{uint32_t(std::chrono::steady_clock::now().time_since_epoch().count()) | 1u};
+  return e.fetch_add(1, std::memory_order_relaxed);
+}
+
 struct Workspace { size_t counters_off, partials_off, total; };
 Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
   Workspace w;
   w.counters_off = 0;
-  w.partials_off = align16(size_t(stripes) * 4 + 256);
+  w.partials_off = align16(size_t(stripes) * 8 + 256);
   w.total = w.partials_off + size_t(grid) * 2 * mpad * kTileN * 4;
   return w;
 }
@@ -1007,7 +1029,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   size_t off = 0;
   uint8_t *wsb = static_cast<uint8_t *>(workspace_dev);
   size_t counters_bytes = 0;
-  for (int i = 0; i < n; ++i) counters_bytes += align16(size_t(ws[i]->h.n_out / kTileN) * 4 + 256);
+  for (int i = 0; i < n; ++i) counters_bytes += align16(size_t(ws[i]->h.n_out / kTileN) * 8 + 256);
   size_t part_off = counters_bytes;
   uint32_t cta0 = 0;
   for (int i = 0; i < n; ++i) {
@@ -1022,8 +1044,8 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     q.cta0 = cta0;
     q.ncta = ncta[i];
     cta0 += ncta[i];
-    q.counters = reinterpret_cast<uint32_t *>(wsb + off);
-    off += align16(size_t(h.n_out / kTileN) * 4 + 256);
+    q.counters = reinterpret_cast<unsigned long long *>(wsb + off);
+    off += align16(size_t(h.n_out / kTileN) * 8 + 256);
     q.partials = reinterpret_cast<uint32_t *>(wsb + part_off);
     part_off += size_t(ncta[i]) * 2 * q.mpad * kTileN * 4;
     const uint32_t uk = unit_k_of(h.format);
@@ -1031,7 +1053,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
       return ANSLIN_ERR_CUDA;
   }
   if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
-  if (cudaMemsetAsync(wsb, 0, counters_bytes, st) != cudaSuccess) return ANSLIN_ERR_CUDA;
+  p.epoch = next_epoch();
   const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
   const uint32_t grid = cta0;
 #define ANSLIN_LAUNCH(F, PAY)                                                                                   \
@@ -1052,7 +1074,7 @@ size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_ma
   size_t counters = 0;
   for (int i = 0; i < n; ++i) {
     if (!ws[i]) return 0;
-    counters += align16(size_t(ws[i]->h.n_out / kTileN) * 4 + 256);
+    counters += align16(size_t(ws[i]->h.n_out / kTileN) * 8 + 256);
   }
   // all problems of a launch share one CTA per SM, so their partials never exceed one problem's worst case
   const size_t per_launch = size_t(std::max(sm_budget(), 148)) * 2 * mpad_of(m_max) * kTileN * 4;
@@ -1227,9 +1249,9 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   const uint32_t stripes = n_out / kTileN, T = stripes * p.KB, grid = grid_of(T, 8);
   const Workspace ws = workspace_layout(stripes, grid, p.mpad);
   if (workspace_bytes < ws.total) return ANSLIN_ERR_BUFFER_TOO_SMALL;
-  p.counters = reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(workspace_dev) + ws.counters_off);
+  p.counters = reinterpret_cast<unsigned long long *>(static_cast<uint8_t *>(workspace_dev) + ws.counters_off);
+  p.epoch = next_epoch();
   p.partials = reinterpret_cast<uint32_t *>(static_cast<uint8_t *>(workspace_dev) + ws.partials_off);
-  if (cudaMemsetAsync(p.counters, 0, size_t(stripes) * 4, st) != cudaSuccess) return ANSLIN_ERR_CUDA;
   CUtensorMap tmw, tmx;
   if (!make_map_2d(&tmw, w_dev, xb, k_in, n_out, k_in, ke, kTileN, CU_TENSOR_MAP_SWIZZLE_128B)) return ANSLIN_ERR_CUDA;
   if (!make_map_2d(&tmx, x_dev, xb, k_in, uint64_t(m), uint64_t(ldx), ke, p.mpad, CU_TENSOR_MAP_SWIZZLE_128B)) return ANSLIN_ERR_CUDA;
