@@ -66,6 +66,11 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (++tries > (1u << 22)) __trap();
   }
 }
+// Programmatic dependent launch: the next kernel of the stream may start (prologue, table build, tile fetch: weights
+// only) while this one drains; everything that depends on the previous kernel (X, scales, Y, workspace) is touched
+// only after grid_dep_wait().
+__device__ __forceinline__ void grid_dep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void grid_dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void fence_mbar_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -544,6 +549,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 2047u) & ~2047u;
   uint8_t *smem = smem_raw + (smem0 - smem_u32(smem_raw));
+  grid_dep_launch_dependents();
   // which problem does this CTA belong to?
   uint32_t pi = 0;
   while (pi + 1 < P.nprob && blockIdx.x >= P.prob[pi + 1].cta0) ++pi;
@@ -598,6 +604,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       // Groups of this CTA are dealt to the teams round-robin over the CTA's WHOLE range (group i ->
       // team i mod PT, round i div PT).  The MMA warp consumes units segment by segment (one
       // accumulator per stripe segment); inside a segment the order is (round, unit, group).
+      bool dep_waited = false;       // griddepcontrol.wait done (before the first load of X)
       uint32_t bsel = 0, bpar = 1;   // this team's next private slot (unit count mod B) and the parity its empty barrier must have passed
 #pragma unroll 1
       for (uint32_t i = team; i < t_end - t_begin; i += PT) {
@@ -628,6 +635,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 #endif
           if (++bsel == P.B) { bsel = 0; bpar ^= 1u; }
           const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
+          if (!dep_waited) { grid_dep_wait(); dep_waited = true; }
 #ifndef ANSLIN_DBG_DECONLY
           if (hw == 0 && lane == 0) {
 #ifndef ANSLIN_DBG_NOTMA
@@ -747,6 +755,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     release(n_commit, true);
   } else if (warp < mma_warp) {
     // ===================== epilogue warps =====================
+    grid_dep_wait();   // Y, the scales and the workspace belong to the stream's earlier kernels until they are done
 #ifndef ANSLIN_DBG_DECONLY
     epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp & 3, lane);
 #endif
@@ -754,6 +763,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   tc_fence_before();
   __syncthreads();
   if (warp == mma_warp) tmem_dealloc(tmem_base, P.tmem_cols);
+  grid_dep_wait();   // warps that had no work of their own join the fix-up: same rule
   splitk_fixup<FMT>(ep, fin, KT, G, T);
 }
 
@@ -935,7 +945,17 @@ int launch_fused(const TensorMaps &tms, const FusedParams &p, uint32_t grid, siz
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
     smem_set = kSmemMax;
   }
-  kern<<<grid, 32 * (kFirstDecWarp + p.D), smem, st>>>(tms, p);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * (kFirstDecWarp + p.D));
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // lets the kernel's prologue overlap its predecessor's tail
+  attr[0].val.programmaticStreamSerializationAllowed = getenv("ANSLIN_NO_PDL") ? 0 : 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, kern, tms, p) != cudaSuccess) return ANSLIN_ERR_CUDA;
   ++g_launches;
   if (getenv("ANSLIN_DEBUG")) {  // debugging aid only: synchronous error report
     cudaError_t e = cudaStreamSynchronize(st);
