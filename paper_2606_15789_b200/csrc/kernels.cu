@@ -209,11 +209,6 @@ struct GlobalEmit {
   size_t row_bytes;      // bytes per W row
   uint32_t stage;        // shared address of this warp's J staging areas
   int u;
-#ifdef ANSLIN_PROBE_NOSTORE   // developer probe: decode throughput without the HBM stores
-  uint32_t chk = 0;
-  __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) { chk ^= v.x ^ v.y ^ v.z ^ v.w; }
-  __device__ __forceinline__ void unit_done(int) {}
-#else
   __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {  // bf16 / fp8 / int8: 16 B of row-major W
     if constexpr (kStaged) {
       const uint32_t c = uint32_t((u & 1) * 2 + g);
@@ -242,7 +237,6 @@ struct GlobalEmit {
       __syncwarp();
     }
   }
-#endif
   __device__ __forceinline__ void packed(int j, int g, int lane, uint32_t b) const {  // int4: 4 packed bytes = 8 weights
     uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 8 + (g / RB) * 4;
     *reinterpret_cast<uint32_t *>(p) = b;
@@ -301,9 +295,6 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
       decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, smem_u32(tab), lane, aux, int(u), V, raw, sz, emit);
       emit.unit_done(lane);
     }
-#ifdef ANSLIN_PROBE_NOSTORE
-    if (emit.chk == 0x12345678u) out[job] = 1;
-#endif
   }
   cp_async_wait_all();
 }
@@ -379,9 +370,6 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     tc_fence_after();
     const uint32_t seg = (t == t_begin ? 0u : 1u);
     uint32_t *part = p.partials + size_t(c * 2u + seg) * p.mpad * kTileN;
-#ifdef ANSLIN_DBG_NOEPI
-    if (false)
-#endif
     for (uint32_t c0 = 0; c0 < p.mpad; c0 += 16) {
       uint32_t v[16];
       tmem_ld16(tmem_base + ((uint32_t(warp) * 32u) << 16) + ab * p.mpad + c0, v);
@@ -390,22 +378,15 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
         const uint32_t mm = c0 + j;
         if (mm < p.m) {
           if (whole) p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(v[j], kScaled ? p.x_scale[mm] : 1.0f, ws);
-#ifndef ANSLIN_DBG_NOPART
           else part[size_t(mm) * kTileN + row] = v[j];
-#endif
         }
       }
     }
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive(tempty_s + 8 * ab);
-#ifdef ANSLIN_DBG_NOEPI
-    if (false)
-#endif
     if (!whole) {
-#ifndef ANSLIN_DBG_NOTF
       __threadfence();
-#endif
       named_bar_sync(1, kEpiWarps * 32);
       if (warp == 0 && lane == 0) {
         const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
@@ -436,9 +417,6 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
   constexpr int kItems = 2;   // items per thread and pass: their loads are all issued before the first add
   for (int seg = 0; seg < 2; ++seg) {
-#ifdef ANSLIN_DBG_NOFIX
-    continue;
-#endif
     if (!fin[seg].valid) continue;
     const uint32_t stripe = fin[seg].stripe, c_first = fin[seg].c_first, c_last = fin[seg].c_last;
     // contributor cc's partial slot: its first segment (slot 0) unless the stripe is its second one, which can only
@@ -531,11 +509,7 @@ struct SmemEmit {
   uint32_t row0[J];      // first stripe row of stream j's tile
   __device__ __forceinline__ void chunk(int j, int g, int lane, uint4 v) const {
     const uint32_t row = row0[j] + uint32_t((g % RB) * 32 + lane), c = uint32_t(g / RB);
-#ifndef ANSLIN_DBG_NOSTS
     sts128(slot_a + row * 32u + ((c ^ ((uint32_t(lane) >> 2) & 1u)) << 4), v);  // Swizzle<1,4,3>
-#else
-    if (v.x == 0x12345678u && v.y == 77u) sts128(slot_a, v);
-#endif
   }
   __device__ __forceinline__ void packed(int, int, int, uint32_t) const {}
 };
@@ -630,22 +604,9 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           // only thing a producer ever waits for is the MMA that read ITS OWN slot B units ago.
           const uint32_t slot = team * P.B + bsel;
           const uint32_t slot_a = slots_s + slot * P.slot_bytes;
-#ifndef ANSLIN_DBG_DECONLY
           mbar_wait(empty_s + 8 * slot, bpar);
-#endif
           if (++bsel == P.B) { bsel = 0; bpar ^= 1u; }
           const int k_elem = int(kt * cv.tile_k + u * unit_k_of(FMT));
-          if (!dep_waited) { grid_dep_wait(); dep_waited = true; }
-#ifndef ANSLIN_DBG_DECONLY
-          if (hw == 0 && lane == 0) {
-#ifndef ANSLIN_DBG_NOTMA
-            mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
-            tma_load_2d(slot_a + kUnitBytes, &tms.m[pi], k_elem, 0, full_s + 8 * slot);
-#else
-            mbar_arrive(full_s + 8 * slot);
-#endif
-          }
-#endif
           emit.slot_a = slot_a;
           if (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll
@@ -659,14 +620,15 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
               for (int j = 0; j < J; ++j) lane_open_segment(s[j], ring_s + j * P.stream_bytes, P.stream_bytes, int(u / kUnitsPerSeg), lane);
             }
           }
+          if (!dep_waited) { grid_dep_wait(); dep_waited = true; }
+          if (hw == 0 && lane == 0) {
+            mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
+            tma_load_2d(slot_a + kUnitBytes, &tms.m[pi], k_elem, 0, full_s + 8 * slot);
+          }
           decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, tab_s, lane, aux, int(u), V, raw, sz, emit);
-#ifndef ANSLIN_DBG_NOFENCE
           fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
-#endif
           __syncwarp();
-#ifndef ANSLIN_DBG_DECONLY
           if (lane == 0) mbar_arrive(full_s + 8 * slot);
-#endif
         }
       }
       cp_async_wait_all();
@@ -701,21 +663,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       if (lane == 0) {
         const uint32_t alo = adesc0_lo + slot * slot_units;   // start address field: (slots_s + slot * slot_bytes) >> 4
         const uint64_t ad = (uint64_t(desc_hi) << 32) | alo, bd = (uint64_t(desc_hi) << 32) | (alo + (kUnitBytes >> 4));
-#ifndef ANSLIN_DBG_NOMMA
         umma<TR::kind>(d_tmem, ad, bd, idesc, accumulate);
         umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
         if (last) umma_commit(tfull_bar);
-#else
-        (void)ad; (void)bd; (void)idesc;
-        mbar_arrive(empty_s + 8 * slot);
-        if (last) mbar_arrive(tfull_bar);
-#endif
       }
       __syncwarp();
     };
-#ifdef ANSLIN_DBG_DECONLY
-    if (false)
-#endif
     for (uint32_t rho = 0; rho * PT < N; ++rho) {
       const uint32_t ga = rho * PT, gb = min(N, ga + PT);
       for (uint32_t i0 = ga; i0 < gb;) {
@@ -756,9 +709,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   } else if (warp < mma_warp) {
     // ===================== epilogue warps =====================
     grid_dep_wait();   // Y, the scales and the workspace belong to the stream's earlier kernels until they are done
-#ifndef ANSLIN_DBG_DECONLY
     epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp & 3, lane);
-#endif
   }
   tc_fence_before();
   __syncthreads();
