@@ -192,30 +192,51 @@ __device__ __forceinline__ void lane_open(LaneStream &s, const uint8_t *rec, int
   s.w = 0;
   s.ptr = 0;
 }
-// Stage segment `seg` of the record into buf (bufbytes of shared memory) and point every lane at its stream.
-// All lanes have finished reading the previous segment (program order + the __syncwarp in stream_drain).
-__device__ __forceinline__ void lane_open_segment(LaneStream &s, uint32_t buf, uint32_t bufbytes, int seg, int lane) {
+// Stage segment `seg` of J records into their buffers (stream j's at buf0 + j * bufbytes) and point every lane at
+// its stream.  All lanes have finished reading the previous segments (program order + the __syncwarp in
+// stream_drain).  The segment tables and the words are fetched together: when the buffer is no larger than the
+// container's tail rule allows to over-read, the whole buffer is copied from the segment start without waiting
+// for the table to say how many words there are.
+template <int J>
+__device__ __forceinline__ void lane_open_segments(LaneStream (&s)[J], uint32_t buf0, uint32_t bufbytes, int seg, int lane) {
   stream_drain();
-  const uint8_t *te = s.rec + 4 * kLanes + kSegTableBytes * seg;
-  const uint32_t hdr = *reinterpret_cast<const uint32_t *>(te);   // u16 base | u16 total words
-  const uint32_t base = hdr & 0xFFFFu, total = hdr >> 16;
-  const uint32_t size = lane < kLanes / 2 ? base + uint32_t(te[4 + lane]) : 0u;   // words of region `lane`
-  uint32_t end = size;
+  const bool spec = bufbytes <= uint32_t(kTailBytes);
+  uint32_t hdr[J], delta[J];
 #pragma unroll
-  for (int d = 1; d < kLanes / 2; d <<= 1) {
-    const uint32_t o = __shfl_up_sync(0xffffffffu, end, d);
-    if (lane >= d) end += o;
+  for (int j = 0; j < J; ++j) {
+    const uint8_t *te = s[j].rec + 4 * kLanes + kSegTableBytes * seg;
+    hdr[j] = *reinterpret_cast<const uint32_t *>(te);   // u16 base | u16 total words
+    delta[j] = lane < kLanes / 2 ? uint32_t(te[4 + lane]) : 0u;
+    if (spec) {
+      const uint32_t skew = s[j].goff & 15u;
+      const uint8_t *src = s[j].rec + (s[j].goff - skew);
+      for (uint32_t o = 16u * uint32_t(lane); o < bufbytes; o += kFillBytes)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(buf0 + uint32_t(j) * bufbytes + o), "l"(src + o) : "memory");
+    }
   }
-  const uint32_t start = end - size;
-  const uint32_t start_p = __shfl_sync(0xffffffffu, start, lane >> 1), end_p = __shfl_sync(0xffffffffu, end, lane >> 1);
-  const uint32_t skew = s.goff & 15u;
-  const uint8_t *src = s.rec + (s.goff - skew);
-  const uint32_t nbytes = min((skew + 2u * total + 15u) & ~15u, bufbytes);   // a damaged table cannot overrun the buffer
-  for (uint32_t o = 16u * uint32_t(lane); o < nbytes; o += kFillBytes)
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(buf + o), "l"(src + o) : "memory");
+#pragma unroll
+  for (int j = 0; j < J; ++j) {
+    const uint32_t base = hdr[j] & 0xFFFFu, total = hdr[j] >> 16, buf = buf0 + uint32_t(j) * bufbytes;
+    const uint32_t size = lane < kLanes / 2 ? base + delta[j] : 0u;   // words of region `lane`
+    uint32_t end = size;
+#pragma unroll
+    for (int d = 1; d < kLanes / 2; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(0xffffffffu, end, d);
+      if (lane >= d) end += o;
+    }
+    const uint32_t start = end - size;
+    const uint32_t start_p = __shfl_sync(0xffffffffu, start, lane >> 1), end_p = __shfl_sync(0xffffffffu, end, lane >> 1);
+    const uint32_t skew = s[j].goff & 15u;
+    if (!spec) {
+      const uint8_t *src = s[j].rec + (s[j].goff - skew);
+      const uint32_t nbytes = min((skew + 2u * total + 15u) & ~15u, bufbytes);   // a damaged table cannot overrun the buffer
+      for (uint32_t o = 16u * uint32_t(lane); o < nbytes; o += kFillBytes)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(buf + o), "l"(src + o) : "memory");
+    }
+    s[j].ptr = buf + skew + 2u * ((lane & 1) ? end_p - 1u : start_p);
+    s[j].goff += 2u * total;
+  }
   cp_async_commit();
-  s.ptr = buf + skew + 2u * ((lane & 1) ? end_p - 1u : start_p);
-  s.goff += 2u * total;
   stream_drain();
 }
 // One decode step of Alg V.2 for all 32 lanes of one lane-stream tile; dir = +2 (even lanes) / -2 (odd lanes).

@@ -288,8 +288,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
       emit.u = int(u);
       if constexpr (LS) {
         if (u % kUnitsPerSeg == 0) {
-#pragma unroll
-          for (int j = 0; j < J; ++j) lane_open_segment(s[j], ring_s + j * stream_bytes, stream_bytes, int(u / kUnitsPerSeg), lane);
+          lane_open_segments<J>(s, ring_s, stream_bytes, int(u / kUnitsPerSeg), lane);
         }
       }
       decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, smem_u32(tab), lane, aux, int(u), V, raw, sz, emit);
@@ -616,8 +615,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           }
           if constexpr (LS) {
             if (u % kUnitsPerSeg == 0) {
-#pragma unroll
-              for (int j = 0; j < J; ++j) lane_open_segment(s[j], ring_s + j * P.stream_bytes, P.stream_bytes, int(u / kUnitsPerSeg), lane);
+              lane_open_segments<J>(s, ring_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);
             }
           }
           if (!dep_waited) { grid_dep_wait(); dep_waited = true; }
