@@ -597,8 +597,21 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           emit.row0[j] = q * 32u * RB;
           sz[j] = nullptr;
         }
+        // the record offsets of this warp's NEXT tiles: loaded now, used after the first unit to pull the records
+        // (and the first raw vectors) into L2, so that the next tile switch waits for L2 rather than HBM
+        const bool has_next = i + PT < t_end - t_begin;
+        uint32_t next_off[J];
+#pragma unroll
+        for (int j = 0; j < J; ++j) next_off[j] = has_next ? offs[(gt + PT) * Q + hw * J + j] : 0u;
 #pragma unroll 1
         for (uint32_t u = 0; u < units; ++u) {
+          if (u == 1 && has_next) {
+#pragma unroll
+            for (int j = 0; j < J; ++j) {
+              if (lane < 24) prefetch_l2(cv.base + cv.off_records + size_t(next_off[j]) * 16 + lane * 128);
+              else if (FMT == ANSLIN_FMT_BF16) prefetch_l2(cv.base + cv.off_raw + size_t((gt + PT) * Q + hw * J + j) * rtb + (lane - 24) * 128);
+            }
+          }
           // team-private slots: unit n of this team lives in slot team*B + n % B (B = P.B buffers per team), so the
           // only thing a producer ever waits for is the MMA that read ITS OWN slot B units ago.
           const uint32_t slot = team * P.B + bsel;
