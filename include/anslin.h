@@ -48,13 +48,15 @@ typedef enum {
   ANSLIN_FMT_BF16 = 0,     /* w_host: uint16 bit patterns; coded symbol = exponent byte, sign+mantissa raw */
   ANSLIN_FMT_FP8_E4M3 = 1, /* w_host: e4m3fn bytes; coded symbol = the byte; per-tensor scale in desc.w_scale */
   ANSLIN_FMT_INT8 = 2,     /* w_host: int8; coded symbol = the byte; scales_host = fp16[n_out] (SQ8-style) */
-  ANSLIN_FMT_INT4_AWQ = 3  /* w_host: uint8[n_out][k_in/2], low nibble = even k; coded symbol = packed byte;
+  ANSLIN_FMT_INT4_AWQ = 3, /* w_host: uint8[n_out][k_in/2], low nibble = even k; coded symbol = packed byte;
                               scales_host/zeros_host = fp16[n_out][k_in/group_size]; w = (q - z) * s */
+  ANSLIN_FMT_FP8_E5M2 = 4  /* w_host: OCP e5m2 bytes (P:l.80 "FP8-E5M2"); otherwise as FP8_E4M3 */
 } anslin_format;
 
 /* Element type of X. */
 typedef enum {
-  ANSLIN_DT_F32 = 0, ANSLIN_DT_F16 = 1, ANSLIN_DT_BF16 = 2, ANSLIN_DT_I8 = 3, ANSLIN_DT_FP8_E4M3 = 4
+  ANSLIN_DT_F32 = 0, ANSLIN_DT_F16 = 1, ANSLIN_DT_BF16 = 2, ANSLIN_DT_I8 = 3, ANSLIN_DT_FP8_E4M3 = 4,
+  ANSLIN_DT_FP8_E5M2 = 5
 } anslin_dtype;
 
 /* Container flag bits. */
@@ -142,7 +144,8 @@ size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, in
 
 /*
  * Fused decode + GEMM, Y = X . W^T (Alg V.1): only compressed bytes of W cross HBM.
- *   x_dev: [m x k_in], dtype per format: bf16 -> BF16, int4 -> F16, int8 -> I8, fp8 -> FP8_E4M3.
+ *   x_dev: [m x k_in], dtype per format: bf16 -> BF16, int4 -> F16, int8 -> I8, fp8 (either kind) -> FP8_E4M3
+ *   or FP8_E5M2 (the tensor core multiplies the two fp8 kinds in any combination).
  *   x_scale_dev: int8/fp8: f32[m] per-token scales; else NULL.
  *   y_dev: f32 [m x n_out]; int8: acc * x_scale[m] * w_scale[n]; fp8: acc * x_scale[m] * desc.w_scale.
  *   1 <= m <= 256.

@@ -21,7 +21,7 @@ from . import codec
 
 MAGIC = 0x4C534E41  # "ANSL"
 VERSION = 1
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ = 0, 1, 2, 3
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2 = 0, 1, 2, 3, 4
 FLAG_STATE_PAYLOAD = 1
 FLAG_LANE_STREAMS = 2   # each lane's words stored as its own stream (tile_n = 32 only), see _lane_record
 SEG_STEPS = 256         # lane-stream records are cut into segments of this many decode steps
@@ -35,9 +35,9 @@ HEADER_BYTES = 128
 TAIL_BYTES = 4096      # readable bytes that must follow the records section
 
 # symbols per 16-byte operand chunk, and default tile_k (in weights) per format
-SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4}
-DEFAULT_TILE_K = {FMT_BF16: 64, FMT_FP8_E4M3: 256, FMT_INT8: 256, FMT_INT4_AWQ: 256}
-WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2}
+SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4, FMT_FP8_E5M2: 16}
+DEFAULT_TILE_K = {FMT_BF16: 64, FMT_FP8_E4M3: 256, FMT_INT8: 256, FMT_INT4_AWQ: 256, FMT_FP8_E5M2: 256}
+WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2, FMT_FP8_E5M2: 1}
 
 
 def _align(x: int, a: int = 16) -> int:

@@ -27,6 +27,18 @@ def e4m3_to_f64(code: np.ndarray) -> np.ndarray:
     return np.where(s == 1, -val, val)
 
 
+def e5m2_to_f64(code: np.ndarray) -> np.ndarray:
+    """OCP FP8 E5M2 (P:l.80): IEEE-like, bias 15: (-1)^s * 2^(e-15) * (1 + m/4), subnormals 2^-14 * m/4,
+    e = 31: infinity (m = 0) or NaN.  It is the upper byte of an IEEE binary16."""
+    c = code.view(np.uint8).astype(np.int64)
+    s = (c >> 7) & 1
+    e = (c >> 2) & 0x1F
+    m = c & 3
+    val = np.where(e == 0, np.ldexp(m / 4.0, -14), np.ldexp(1.0 + m / 4.0, e - 15))
+    val = np.where(e == 31, np.where(m == 0, np.inf, np.nan), val)
+    return np.where(s == 1, -val, val)
+
+
 def int4_unpack(packed: np.ndarray) -> np.ndarray:
     """uint8 [n x k/2], low nibble = even k  ->  uint8 [n x k] codes 0..15."""
     p = packed.view(np.uint8)
@@ -62,9 +74,9 @@ def gemm_int8(xq: np.ndarray, x_scale: np.ndarray, wq: np.ndarray, w_scale: np.n
     return acc.astype(np.float64) * sc, a, acc
 
 
-def gemm_fp8(xq: np.ndarray, x_scale: np.ndarray, wq: np.ndarray, w_scale: float):
-    """fp8-e4m3 (reading A15): Y = (sum_k x8*w8) * s_x[m] * s_w."""
-    y, a = gemm_f64(e4m3_to_f64(xq), e4m3_to_f64(wq))
+def gemm_fp8(xq: np.ndarray, x_scale: np.ndarray, wq: np.ndarray, w_scale: float, x_e5m2: bool = False, w_e5m2: bool = False):
+    """fp8 (reading A15): Y = (sum_k x8*w8) * s_x[m] * s_w; each operand e4m3 unless flagged e5m2."""
+    y, a = gemm_f64((e5m2_to_f64 if x_e5m2 else e4m3_to_f64)(xq), (e5m2_to_f64 if w_e5m2 else e4m3_to_f64)(wq))
     sc = x_scale.astype(np.float64)[:, None] * float(w_scale)
     return y * sc, a * sc
 

@@ -38,6 +38,8 @@ struct Header {  // 128 bytes, little endian
 static_assert(sizeof(Header) == kHeaderBytes, "header must be 128 bytes");
 
 // symbols per 16-byte operand chunk
+constexpr uint32_t kFormatMax = ANSLIN_FMT_FP8_E5M2;
+ANSLIN_HD constexpr bool is_fp8(uint32_t fmt) { return fmt == ANSLIN_FMT_FP8_E4M3 || fmt == ANSLIN_FMT_FP8_E5M2; }
 ANSLIN_HD constexpr int spc_of(uint32_t fmt) {
   return fmt == ANSLIN_FMT_BF16 ? 8 : fmt == ANSLIN_FMT_INT4_AWQ ? 4 : 16;
 }

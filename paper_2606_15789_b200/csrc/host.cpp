@@ -24,7 +24,7 @@ struct Geometry {
 };
 
 bool make_geometry(const anslin_desc *d, Geometry *g) {
-  if (!d || d->format > ANSLIN_FMT_INT4_AWQ) return false;
+  if (!d || d->format > kFormatMax) return false;
   g->fmt = d->format;
   g->n_out = d->n_out;
   g->k_in = d->k_in;
@@ -229,7 +229,7 @@ size_t anslin_encode_bound(const anslin_desc *desc) {
 int anslin_encode_host(const anslin_desc *desc, const void *w_host, const void *scales_host, const void *zeros_host,
                        void *container_out, size_t capacity, size_t *bytes_out, anslin_stats *st) {
   if (!desc || !w_host || !container_out || !bytes_out) return ANSLIN_ERR_INVALID_ARG;
-  if (desc->format > ANSLIN_FMT_INT4_AWQ) return ANSLIN_ERR_UNSUPPORTED;
+  if (desc->format > kFormatMax) return ANSLIN_ERR_UNSUPPORTED;
   Geometry g;
   if (!make_geometry(desc, &g)) return ANSLIN_ERR_UNSUPPORTED;
   return encode_with(g, desc, w_host, scales_host, zeros_host, container_out, capacity, bytes_out, st);
@@ -320,7 +320,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
   h.magic = kMagic; h.version = kVersion; h.format = g.fmt; h.n_out = g.n_out; h.k_in = g.k_in;
   h.tile_n = g.tile_n; h.tile_k = g.tile_k; h.streams = kLanes; h.prob_bits = kProbBits; h.word_bits = kWordBits;
   h.state_lo_log2 = kStateLoLog2; h.group_size = g.group; h.flags = g.flags; h.n_tiles = uint32_t(g.n_tiles);
-  h.w_scale = g.fmt == ANSLIN_FMT_FP8_E4M3 ? desc->w_scale : 1.0f;
+  h.w_scale = is_fp8(g.fmt) ? desc->w_scale : 1.0f;
   for (uint32_t b : segbytes) h.max_seg_bytes = std::max(h.max_seg_bytes, b);
 
   uint8_t *out = static_cast<uint8_t *>(container_out);
@@ -394,7 +394,7 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   if (h.magic != kMagic || h.version != kVersion) return ANSLIN_ERR_CORRUPT;
   anslin_desc d{h.format, h.n_out, h.k_in, h.tile_k, h.group_size, h.flags, h.w_scale, h.tile_n};
   Geometry g;
-  if (h.format > ANSLIN_FMT_INT4_AWQ || !make_geometry(&d, &g)) return ANSLIN_ERR_CORRUPT;
+  if (h.format > kFormatMax || !make_geometry(&d, &g)) return ANSLIN_ERR_CORRUPT;
   if (h.tile_n != g.tile_n || h.streams != kLanes || h.prob_bits != kProbBits || h.word_bits != kWordBits ||
       h.state_lo_log2 != kStateLoLog2 || h.n_tiles != g.n_tiles)
     return ANSLIN_ERR_CORRUPT;

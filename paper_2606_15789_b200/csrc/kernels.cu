@@ -496,6 +496,7 @@ struct FusedParams {
   uint32_t stream_bytes;   // shared memory per stream: word ring + mirror, or the largest staged lane-stream segment
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
+  uint32_t afmt, bfmt;     // tcgen05 a/b format codes (fp8: 0 = e4m3, 1 = e5m2, chosen at run time)
 };
 struct TensorMaps { CUtensorMap m[kMaxProblems]; };
 
@@ -646,7 +647,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     }
   } else if (warp == mma_warp) {
     // ===================== MMA issuer: one thread drives the tensor core =====================
-    const uint32_t idesc = make_idesc(TR::c, TR::ab, TR::ab, 128, mpad);
+    const uint32_t idesc = make_idesc(TR::c, P.afmt, P.bfmt, 128, mpad);
     const uint32_t PT = P.D / NW, N = t_end - t_begin;
     // Consumption order: rounds of PT groups; inside a round, units ascending and groups ascending, with
     // up to TWO stripe segments of the round interleaved (they own different TMEM accumulators), so the
@@ -742,6 +743,7 @@ struct DenseParams {
   unsigned long long *counters;
   uint32_t epoch;
   uint32_t n_out, k_in, m, mpad, S /*stages*/, stage_bytes, tmem_cols, KB /*k blocks of 128 B*/;
+  uint32_t afmt, bfmt;
 };
 constexpr int kDenseThreads = 32 * 6;  // warps 0-3 epilogue, 4 MMA, 5 TMA producer
 
@@ -787,7 +789,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
       }
     }
   } else if (warp == kMmaWarp) {
-    const uint32_t idesc = make_idesc(TR::c, TR::ab, TR::ab, 128, p.mpad);
+    const uint32_t idesc = make_idesc(TR::c, p.afmt, p.bfmt, 128, p.mpad);
     uint32_t seq = 0, si = 0;
     for (uint32_t t = t_begin; t < t_end; ++si) {
       const uint32_t ka = t % KT, nt = min(KT - ka, t_end - t), ab = si & 1u;
@@ -894,8 +896,11 @@ Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
 
 bool x_dtype_ok(uint32_t fmt, uint32_t dt) {
   return (fmt == ANSLIN_FMT_BF16 && dt == ANSLIN_DT_BF16) || (fmt == ANSLIN_FMT_INT4_AWQ && dt == ANSLIN_DT_F16) ||
-         (fmt == ANSLIN_FMT_INT8 && dt == ANSLIN_DT_I8) || (fmt == ANSLIN_FMT_FP8_E4M3 && dt == ANSLIN_DT_FP8_E4M3);
+         (fmt == ANSLIN_FMT_INT8 && dt == ANSLIN_DT_I8) || (is_fp8(fmt) && (dt == ANSLIN_DT_FP8_E4M3 || dt == ANSLIN_DT_FP8_E5M2));
 }
+// tcgen05 instruction-descriptor format code of the weight operand (a) / of X (b)
+uint32_t afmt_of(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT8 || fmt == ANSLIN_FMT_FP8_E5M2 ? 1u : 0u; }
+uint32_t bfmt_of(uint32_t fmt, uint32_t dt) { return is_fp8(fmt) ? (dt == ANSLIN_DT_FP8_E5M2 ? 1u : 0u) : afmt_of(fmt); }
 
 int sm_budget() { return std::max(1, num_sms()); }
 
@@ -933,7 +938,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   if (n < 1 || n > kMaxProblems || !workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) & 15)) return ANSLIN_ERR_INVALID_ARG;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
   const Header &h0 = ws[0]->h;
-  const bool scaled = h0.format == ANSLIN_FMT_INT8 || h0.format == ANSLIN_FMT_FP8_E4M3;
+  const bool scaled = h0.format == ANSLIN_FMT_INT8 || is_fp8(h0.format);
   const int xb = (h0.format == ANSLIN_FMT_BF16 || h0.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
   if (!x_dtype_ok(h0.format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
   uint32_t mpad_max = 16;
@@ -1036,6 +1041,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   }
   if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   p.epoch = next_epoch();
+  p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
   const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
   const uint32_t grid = cta0;
 #define ANSLIN_LAUNCH(F, PAY)                                                                                   \
@@ -1043,7 +1049,8 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
            : launch_fused<F, 4, PAY, false>(tms, p, grid, smem, st))
   switch (h0.format) {
     case ANSLIN_FMT_BF16: return pay ? ANSLIN_LAUNCH(ANSLIN_FMT_BF16, true) : ANSLIN_LAUNCH(ANSLIN_FMT_BF16, false);
-    case ANSLIN_FMT_FP8_E4M3: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);
+    case ANSLIN_FMT_FP8_E4M3:
+    case ANSLIN_FMT_FP8_E5M2: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);   // same bytes, another descriptor code
     case ANSLIN_FMT_INT8: return ANSLIN_LAUNCH(ANSLIN_FMT_INT8, false);
     case ANSLIN_FMT_INT4_AWQ: return ANSLIN_LAUNCH(ANSLIN_FMT_INT4_AWQ, false);
   }
@@ -1118,7 +1125,8 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
     case ANSLIN_FMT_BF16:
       return (h.flags & ANSLIN_FLAG_STATE_PAYLOAD) ? launch_decode<ANSLIN_FMT_BF16, true>(cv, w_out_dev, st)
                                                     : launch_decode<ANSLIN_FMT_BF16, false>(cv, w_out_dev, st);
-    case ANSLIN_FMT_FP8_E4M3: return launch_decode<ANSLIN_FMT_FP8_E4M3, false>(cv, w_out_dev, st);
+    case ANSLIN_FMT_FP8_E4M3:
+    case ANSLIN_FMT_FP8_E5M2: return launch_decode<ANSLIN_FMT_FP8_E4M3, false>(cv, w_out_dev, st);
     case ANSLIN_FMT_INT8: return launch_decode<ANSLIN_FMT_INT8, false>(cv, w_out_dev, st);
     case ANSLIN_FMT_INT4_AWQ: return launch_decode<ANSLIN_FMT_INT4_AWQ, false>(cv, w_out_dev, st);
   }
@@ -1204,7 +1212,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
                       int64_t ldy, void *workspace_dev, size_t workspace_bytes, void *stream) {
   g_launches = 0;
   if (!w_dev || !x_dev || !y_dev || !workspace_dev) return ANSLIN_ERR_INVALID_ARG;
-  if (format > ANSLIN_FMT_INT4_AWQ || m < 1 || m > 256) return ANSLIN_ERR_UNSUPPORTED;
+  if (format > kFormatMax || m < 1 || m > 256) return ANSLIN_ERR_UNSUPPORTED;
   // the int4 slot takes fp16 weights (what AWQ dequantises to): same MMA kind as the fused int4 path
   const uint32_t xd_need = format == ANSLIN_FMT_INT4_AWQ ? ANSLIN_DT_F16 : 0;
   if (format == ANSLIN_FMT_INT4_AWQ ? x_dtype != xd_need : !x_dtype_ok(format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
@@ -1214,7 +1222,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   if ((reinterpret_cast<uintptr_t>(w_dev) | reinterpret_cast<uintptr_t>(x_dev) | reinterpret_cast<uintptr_t>(y_dev) |
        reinterpret_cast<uintptr_t>(workspace_dev)) & 15)
     return ANSLIN_ERR_INVALID_ARG;
-  const bool scaled = format == ANSLIN_FMT_INT8 || format == ANSLIN_FMT_FP8_E4M3;
+  const bool scaled = format == ANSLIN_FMT_INT8 || is_fp8(format);
   if (scaled && !x_scale_dev) return ANSLIN_ERR_INVALID_ARG;
   if (format == ANSLIN_FMT_INT8 && !w_scale_dev) return ANSLIN_ERR_INVALID_ARG;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
@@ -1223,6 +1231,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   p.w_scale_h = w_scale_dev; p.w_scale = w_scale; p.x_scale = static_cast<const float *>(x_scale_dev);
   p.y = static_cast<float *>(y_dev); p.ldy = ldy; p.n_out = n_out; p.k_in = k_in; p.m = uint32_t(m); p.mpad = mpad_of(m);
   p.KB = k_in / ke;
+  p.afmt = afmt_of(format); p.bfmt = bfmt_of(format, x_dtype);
   p.stage_bytes = 16384 + p.mpad * 128u;
   p.tmem_cols = tmem_cols_of(p.mpad);
   const size_t fixed = 1024 + 16 * kMaxSlots + 96;
@@ -1240,7 +1249,8 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   switch (format) {
     case ANSLIN_FMT_BF16: return launch_dense<ANSLIN_FMT_BF16>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_INT4_AWQ: return launch_dense<ANSLIN_FMT_INT4_AWQ>(tmw, tmx, p, grid, smem, st);
-    case ANSLIN_FMT_FP8_E4M3: return launch_dense<ANSLIN_FMT_FP8_E4M3>(tmw, tmx, p, grid, smem, st);
+    case ANSLIN_FMT_FP8_E4M3:
+    case ANSLIN_FMT_FP8_E5M2: return launch_dense<ANSLIN_FMT_FP8_E4M3>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_INT8: return launch_dense<ANSLIN_FMT_INT8>(tmw, tmx, p, grid, smem, st);
   }
   return ANSLIN_ERR_UNSUPPORTED;

@@ -9,7 +9,7 @@ from __future__ import annotations
 
 import numpy as np
 
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ = 0, 1, 2, 3
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2 = 0, 1, 2, 3, 4
 
 # BASELINE.json configs 2/3 (Qwen-14B-shaped dense decoder layer), [n_out, k_in] = Linear.weight
 QWEN14B_LAYER = [("q", 5120, 5120), ("k", 1024, 5120), ("v", 1024, 5120), ("o", 5120, 5120),
@@ -100,6 +100,26 @@ def quant_fp8_acts(x: np.ndarray):
     s = (np.abs(x).max(axis=1) / 448.0).astype(np.float32)
     s = np.maximum(s, np.float32(1e-12))
     return f32_to_e4m3_bytes(x / s[:, None]), s
+
+
+def f32_to_e5m2_bytes(x: np.ndarray) -> np.ndarray:
+    """float32 -> OCP e5m2 byte codes via torch's CPU cast (values pre-scaled to |x| <= 57344)."""
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).to(torch.float8_e5m2)
+    return t.view(torch.uint8).numpy().copy()
+
+
+def quant_fp8_e5m2_weights(w: np.ndarray):
+    """Per-tensor e5m2: s = amax/57344 (the largest finite e5m2), same recipe as A15."""
+    s = float(np.abs(w).max() / 57344.0)
+    return f32_to_e5m2_bytes(w / np.float32(s)), s
+
+
+def quant_fp8_e5m2_acts(x: np.ndarray):
+    """Per-token e5m2: s[m] = amax_m/57344 (fp32)."""
+    s = (np.abs(x).max(axis=1) / 57344.0).astype(np.float32)
+    s = np.maximum(s, np.float32(1e-12))
+    return f32_to_e5m2_bytes(x / s[:, None]), s
 
 
 def route_top2(m_tokens: int, n_experts: int, seed: int):

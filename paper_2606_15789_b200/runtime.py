@@ -10,7 +10,7 @@ import torch
 from . import binding as B
 
 _TORCH_X = {B.FMT_BF16: torch.bfloat16, B.FMT_INT4_AWQ: torch.float16, B.FMT_INT8: torch.int8,
-            B.FMT_FP8_E4M3: torch.uint8}
+            B.FMT_FP8_E4M3: torch.uint8, B.FMT_FP8_E5M2: torch.uint8}
 
 
 def _stream() -> int:
@@ -58,13 +58,14 @@ class DeviceWeight:
             self._ws = torch.empty(need, dtype=torch.uint8, device=self.container_dev.device)
         return self._ws
 
-    def gemm(self, x: torch.Tensor, x_scale: torch.Tensor | None = None, y: torch.Tensor | None = None) -> torch.Tensor:
-        """anslin_gemm: Y[m x n_out] f32 = X . W^T with W decoded on the fly."""
+    def gemm(self, x: torch.Tensor, x_scale: torch.Tensor | None = None, y: torch.Tensor | None = None,
+             x_dtype: int | None = None) -> torch.Tensor:
+        """anslin_gemm: Y[m x n_out] f32 = X . W^T with W decoded on the fly (x_dtype: B.DT_*, default the format's own)."""
         m = x.shape[0]
         if y is None:
             y = torch.empty((m, self.n_out), dtype=torch.float32, device=x.device)
         ws = self.workspace(m)
-        B.anslin_gemm(self.weight, x.data_ptr(), B.X_DTYPE[self.fmt], x.stride(0), m,
+        B.anslin_gemm(self.weight, x.data_ptr(), B.X_DTYPE[self.fmt] if x_dtype is None else x_dtype, x.stride(0), m,
                       None if x_scale is None else x_scale.data_ptr(), y.data_ptr(), y.stride(0), ws.data_ptr(), ws.numel(), _stream())
         return y
 

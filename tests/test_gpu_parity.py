@@ -62,6 +62,9 @@ def _decode_cases():
     yield "fp8-32x768-lanes", B.FMT_FP8_E4M3, f8, 768, dict(tile_k=768, w_scale=sc, tile_n=32, flags=2)
     p4l, s4l, z4l = inputs.quant_awq4_weights(inputs.weights_f32(256, 1024, seed=46, outliers=False), 128)
     yield "int4-32x512-lanes", B.FMT_INT4_AWQ, p4l, 1024, dict(tile_k=512, scales=s4l, zeros=z4l, group_size=128, tile_n=32, flags=2)
+    f5, sc5 = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(256, 768, seed=47, std=0.015, outliers=False))
+    yield "e5m2", B.FMT_FP8_E5M2, f5, 768, dict(tile_k=256, w_scale=sc5)
+    yield "e5m2-32x768-lanes", B.FMT_FP8_E5M2, f5, 768, dict(tile_k=768, w_scale=sc5, tile_n=32, flags=2)
     yield "bf16-constant-lanes", B.FMT_BF16, np.full((128, 256), 0xBF80, dtype=np.uint16), 256, dict(tile_k=256, tile_n=32, flags=2)
 
 
@@ -181,6 +184,26 @@ def test_gemm_int4(m, lay):
     dw = rt.DeviceWeight(buf)
     y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
     check_gemm(y, *og.gemm_int4(x, p4, s4, z4, 128))
+    dw.close()
+
+
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
+@pytest.mark.parametrize("m", [1, 37])
+@pytest.mark.parametrize("x_kind", ["e5m2", "e4m3"])
+def test_gemm_fp8_e5m2(m, lay, x_kind):
+    """NEXT-2 format fp8-E5M2 (P:l.80): same byte coder, tensor-core descriptor code e5m2 for W; X in either fp8 kind."""
+    tile_n, lflag = lay
+    rt = _rt()
+    import torch
+    n, k = 256, 1536
+    f5, sc = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(n, k, seed=73, std=0.015, outliers=False))
+    xf = inputs.acts_f32(m, k, seed=74)
+    x8, xs = inputs.quant_fp8_e5m2_acts(xf) if x_kind == "e5m2" else inputs.quant_fp8_acts(xf)
+    buf, _ = B.anslin_encode_host(B.FMT_FP8_E5M2, f5, n, k, tile_k=256, w_scale=sc, tile_n=tile_n, flags=lflag)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_FP8_E5M2, x8), torch.from_numpy(xs).cuda(),
+                x_dtype=B.DT_FP8_E5M2 if x_kind == "e5m2" else B.DT_FP8_E4M3).cpu().numpy()
+    check_gemm(y, *og.gemm_fp8(x8, xs, f5, sc, x_e5m2=x_kind == "e5m2", w_e5m2=True))
     dw.close()
 
 

@@ -52,6 +52,9 @@ def _cases():
     yield "int8-32x512-lanes", oc.FMT_INT8, q8, 512, dict(tile_k=512, scales=s8, tile_n=32, flags=2)
     yield "fp8-32x256-lanes", oc.FMT_FP8_E4M3, f8, 512, dict(tile_k=256, w_scale=sc, tile_n=32, flags=2)
     yield "int4-32x512-lanes", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=512, scales=s4, zeros=z4, group_size=128, tile_n=32, flags=2)
+    f5, sc5 = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(128, 512, seed=34, std=0.015, outliers=False))
+    yield "e5m2", oc.FMT_FP8_E5M2, f5, 512, dict(tile_k=256, w_scale=sc5)
+    yield "e5m2-32x512-lanes", oc.FMT_FP8_E5M2, f5, 512, dict(tile_k=512, w_scale=sc5, tile_n=32, flags=2)
 
 
 @pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_cases()), ids=[c[0] for c in _cases()])

@@ -153,6 +153,33 @@ def test_e4m3_decode_against_torch_cast():
     assert got[0x7E] == 448.0 and got[0x01] == 2.0 ** -9
 
 
+def test_e5m2_decode_against_binary16_and_torch():
+    """e5m2 is the upper byte of an IEEE binary16 (pin 1: numpy's float16) and torch's float8_e5m2 (pin 2)."""
+    import torch
+    codes = np.arange(256, dtype=np.uint8)
+    got = og.e5m2_to_f64(codes)
+    ref16 = (codes.astype(np.uint16) << 8).view(np.float16).astype(np.float64)
+    ref_t = torch.from_numpy(codes).view(torch.float8_e5m2).to(torch.float64).numpy()
+    for ref in (ref16, ref_t):
+        assert np.array_equal(np.isnan(ref), np.isnan(got))
+        ok = ~np.isnan(ref)
+        assert np.array_equal(ref[ok], got[ok])
+    assert got[0x7B] == 57344.0 and got[0x01] == 2.0 ** -16 and got[0x3C] == 1.0 and got[0xFC] == -np.inf
+
+
+def test_roundtrip_and_gemm_fp8_e5m2():
+    f8, sc = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(128, 512, seed=14, std=0.015, outliers=False))
+    _, st, h, _ = _roundtrip(oc.FMT_FP8_E5M2, f8, 512, tile_k=256, w_scale=sc)
+    assert h.fmt == oc.FMT_FP8_E5M2 and st["bits_per_weight"] < 8.0
+    x8 = np.array([[0x3C, 0x40, 0xBC, 0x00]], np.uint8)       # 1, 2, -1, 0 in e5m2
+    w8 = np.array([[0x38, 0x38, 0x38, 0x7B]], np.uint8)       # 0.5, 0.5, 0.5, 57344
+    y, a = og.gemm_fp8(x8, np.array([2.0], np.float32), w8, 0.5, x_e5m2=True, w_e5m2=True)
+    assert y[0, 0] == (0.5 + 1.0 - 0.5) * 2.0 * 0.5 and a[0, 0] == 2.0 * 2.0 * 0.5
+    # mixed kinds: the same bytes read as e4m3 give 1.5 / 2 / -1.5 (0x3C = 1.5 in e4m3, 0x40 = 2)
+    y, _ = og.gemm_fp8(x8, np.array([1.0], np.float32), w8, 1.0, x_e5m2=False, w_e5m2=True)
+    assert y[0, 0] == (1.5 + 2.0 - 1.5) * 0.5
+
+
 def test_bf16_conversion_against_torch():
     import torch
     x = np.random.default_rng(1).standard_normal(4096).astype(np.float32) * 3
