@@ -16,7 +16,7 @@
  *   - kernels are enqueued on the caller's stream and run asynchronously; asynchronous faults
  *     surface at the caller's next synchronisation.  No hidden synchronisation.
  *   - device pointers must be 16-byte aligned (else ANSLIN_ERR_INVALID_ARG).
- *   - shapes: n_out % 128 == 0 and k_in % tile_k == 0 (else ANSLIN_ERR_UNSUPPORTED); 1 <= m <= 256.
+ *   - shapes: n_out % 128 == 0 and k_in % tile_k == 0 (else ANSLIN_ERR_UNSUPPORTED); m >= 1 (anslin_gemm_multi: <= 256 per problem).
  *   - orientation: W is [n_out x k_in] row-major (torch Linear.weight), X is [m x k_in] row-major
  *     with leading dimension ldx (elements), Y is [m x n_out] row-major float32 with ldy.
  *   - there is no CPU fallback: the device entry points fail with ANSLIN_ERR_CUDA when no sm_100
@@ -148,7 +148,8 @@ size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, in
  *   or FP8_E5M2 (the tensor core multiplies the two fp8 kinds in any combination).
  *   x_scale_dev: int8/fp8: f32[m] per-token scales; else NULL.
  *   y_dev: f32 [m x n_out]; int8: acc * x_scale[m] * w_scale[n]; fp8: acc * x_scale[m] * desc.w_scale.
- *   1 <= m <= 256.
+ *   m >= 1.  m <= 256 is the regime the kernel is built for (P:l.295-306).  A larger m is processed in blocks of 256 rows,
+ *   every block a problem of its own in one persistent launch (8 blocks per launch): each block decodes W again.
  */
 int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m,
                 const void *x_scale_dev, void *y_dev, int64_t ldy, void *workspace_dev,

@@ -1133,7 +1133,18 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
   return ANSLIN_ERR_UNSUPPORTED;
 }
 
-size_t anslin_gemm_workspace_bytes(const anslin_weight *w, int32_t m) { return multi_workspace_bytes(&w, 1, m); }
+// m > 256 (S: §8(f) NEXT-1, the paper's prefill workloads P:l.392): X is cut into blocks of kMaxM rows, each block a
+// problem of its own inside one persistent launch (kMaxProblems blocks per launch).  Every block decodes W again:
+// correct at any m, but the decoded tile is not shared between blocks.
+constexpr int32_t kMaxM = 256;
+
+size_t anslin_gemm_workspace_bytes(const anslin_weight *w, int32_t m) {
+  if (m <= kMaxM) return multi_workspace_bytes(&w, 1, m);
+  const anslin_weight *ws[kMaxProblems];
+  const int n = int(std::min<int64_t>(kMaxProblems, (int64_t(m) + kMaxM - 1) / kMaxM));
+  for (int i = 0; i < n; ++i) ws[i] = w;
+  return multi_workspace_bytes(ws, n, kMaxM);
+}
 
 size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, int32_t n, int32_t m_max) {
   return multi_workspace_bytes(weights, n, m_max);
@@ -1143,8 +1154,29 @@ int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int
                 void *y_dev, int64_t ldy, void *workspace_dev, size_t workspace_bytes, void *stream) {
   g_launches = 0;
   if (!w) return ANSLIN_ERR_INVALID_ARG;
-  return gemm_launch(1, &w, &x_dev, x_dtype, &ldx, &m, &x_scale_dev, &y_dev, &ldy, workspace_dev, workspace_bytes,
-                     static_cast<cudaStream_t>(stream));
+  if (m <= kMaxM)
+    return gemm_launch(1, &w, &x_dev, x_dtype, &ldx, &m, &x_scale_dev, &y_dev, &ldy, workspace_dev, workspace_bytes,
+                       static_cast<cudaStream_t>(stream));
+  if (!x_dev || !y_dev) return ANSLIN_ERR_INVALID_ARG;
+  const int xb = (w->h.format == ANSLIN_FMT_BF16 || w->h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
+  for (int32_t r0 = 0; r0 < m;) {
+    const anslin_weight *ws[kMaxProblems];
+    const void *xs[kMaxProblems], *xsc[kMaxProblems];
+    void *ys[kMaxProblems];
+    int64_t ldxs[kMaxProblems], ldys[kMaxProblems];
+    int32_t ms[kMaxProblems];
+    int cnt = 0;
+    for (; cnt < kMaxProblems && r0 < m; ++cnt, r0 += kMaxM) {
+      ws[cnt] = w;
+      xs[cnt] = static_cast<const uint8_t *>(x_dev) + size_t(r0) * ldx * xb;
+      xsc[cnt] = x_scale_dev ? static_cast<const float *>(x_scale_dev) + r0 : nullptr;
+      ys[cnt] = static_cast<float *>(y_dev) + size_t(r0) * ldy;
+      ldxs[cnt] = ldx; ldys[cnt] = ldy; ms[cnt] = std::min(kMaxM, m - r0);
+    }
+    const int rc = gemm_launch(cnt, ws, xs, x_dtype, ldxs, ms, xsc, ys, ldys, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
+    if (rc != ANSLIN_OK) return rc;
+  }
+  return ANSLIN_OK;
 }
 
 int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
@@ -1175,30 +1207,34 @@ int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts, 
   int32_t ms[kMaxProblems];
   int cnt = 0;
   int64_t row = 0;
-  for (int e = 0; e <= n_experts; ++e) {
-    if (e == n_experts || cnt == kMaxProblems) {
-      if (cnt > 0) {
-        int rc = gemm_launch(cnt, w, xs, x_dtype, ldxs, ms, xsc, ys, ldys, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
-        if (rc != ANSLIN_OK) return rc;
-      }
-      cnt = 0;
-      if (e == n_experts) break;
-    }
+  auto flush = [&]() -> int {
+    if (cnt == 0) return ANSLIN_OK;
+    const int rc = gemm_launch(cnt, w, xs, x_dtype, ldxs, ms, xsc, ys, ldys, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
+    cnt = 0;
+    return rc;
+  };
+  for (int e = 0; e < n_experts; ++e) {
     const int32_t rows = rows_per_expert_host[e];
     if (rows < 0 || !experts[e]) return ANSLIN_ERR_INVALID_ARG;
     if (rows == 0) continue;
     const Header &h = experts[e]->h;
     if (h.format != experts[0]->h.format || h.n_out != experts[0]->h.n_out || h.k_in != experts[0]->h.k_in) return ANSLIN_ERR_INVALID_ARG;
     const int xb = (h.format == ANSLIN_FMT_BF16 || h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
-    w[cnt] = experts[e];
-    xs[cnt] = static_cast<const uint8_t *>(x_dev) + size_t(row) * ldx * xb;   // row offsets keep 16-byte alignment only if the pitch does
-    xsc[cnt] = x_scale_dev ? static_cast<const float *>(x_scale_dev) + row : nullptr;
-    ys[cnt] = static_cast<float *>(y_dev) + size_t(row) * ldy;
-    ldxs[cnt] = ldx; ldys[cnt] = ldy; ms[cnt] = rows;
-    ++cnt;
+    for (int32_t r0 = 0; r0 < rows; r0 += kMaxM) {   // an expert with more than kMaxM rows is several problems (see anslin_gemm)
+      if (cnt == kMaxProblems) {
+        const int rc = flush();
+        if (rc != ANSLIN_OK) return rc;
+      }
+      w[cnt] = experts[e];
+      xs[cnt] = static_cast<const uint8_t *>(x_dev) + size_t(row + r0) * ldx * xb;   // row offsets keep 16-byte alignment only if the pitch does
+      xsc[cnt] = x_scale_dev ? static_cast<const float *>(x_scale_dev) + row + r0 : nullptr;
+      ys[cnt] = static_cast<float *>(y_dev) + size_t(row + r0) * ldy;
+      ldxs[cnt] = ldx; ldys[cnt] = ldy; ms[cnt] = std::min(kMaxM, rows - r0);
+      ++cnt;
+    }
     row += rows;
   }
-  return ANSLIN_OK;
+  return flush();
 }
 
 size_t anslin_dense_workspace_bytes(uint32_t n_out, uint32_t k_in, int32_t m) {

@@ -97,7 +97,9 @@ def gemm_grouped(experts, rows_per_expert, x: torch.Tensor, x_scale: torch.Tenso
     m = x.shape[0]
     if y is None:
         y = torch.empty((m, experts[0].n_out), dtype=torch.float32, device=x.device)
-    need = B.anslin_gemm_multi_workspace_bytes([e.weight for e in experts], int(max(max(rows_per_expert), 1)))
+    blocks = sum((int(r) + 255) // 256 for r in rows_per_expert)     # experts with > 256 rows run as several problems
+    per_launch = [experts[0].weight] * max(1, min(8, blocks)) if blocks > len(experts) else [e.weight for e in experts]
+    need = B.anslin_gemm_multi_workspace_bytes(per_launch, int(min(256, max(max(rows_per_expert), 1))))
     ws = experts[0]._ws
     if ws is None or ws.numel() < need:
         ws = experts[0]._ws = torch.empty(need, dtype=torch.uint8, device=x.device)

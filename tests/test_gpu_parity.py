@@ -113,6 +113,45 @@ def test_gemm_bf16(m, flags, tile):
     dw.close()
 
 
+@pytest.mark.parametrize("m", [257, 600, 2304])
+def test_gemm_bf16_large_m(m):
+    """S: §8(f) NEXT-1 (prefill-sized batches, P:l.392): m > 256 runs as blocks of 256 rows, 8 blocks per launch
+    (2304 rows = two launches, the second with a single block); a ragged last block."""
+    rt = _rt()
+    n, k = 384, 1024
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=53, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=54))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    check_gemm(y, *og.gemm_bf16(x, w))
+    assert B.lib().anslin_last_launch_count() == (m + 2047) // 2048
+    dw.close()
+
+
+def test_gemm_int8_large_m_and_grouped_large_expert():
+    rt = _rt()
+    import torch
+    n, k, m = 256, 1024, 300
+    q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=63, jitter=True))
+    xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=64))
+    buf, _ = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=256, scales=s)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
+    y_ref, a_ref, _ = og.gemm_int8(xq, xs, q, s)       # per-token scales follow their rows into every block
+    check_gemm(y, y_ref, a_ref)
+    # grouped: expert 0 owns 280 rows (two problems), expert 1 none, expert 2 the remaining 20
+    q2, s2 = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=65, jitter=True))
+    buf2, _ = B.anslin_encode_host(B.FMT_INT8, q2, n, k, tile_k=256, scales=s2)
+    dw2, dw3 = rt.DeviceWeight(buf2), rt.DeviceWeight(buf)
+    yg = rt.gemm_grouped([dw, dw3, dw2], [280, 0, 20], rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
+    check_gemm(yg[:280], y_ref[:280], a_ref[:280])
+    y_ref2, a_ref2, _ = og.gemm_int8(xq[280:], xs[280:], q2, s2)
+    check_gemm(yg[280:], y_ref2, a_ref2)
+    for d in (dw, dw2, dw3):
+        d.close()
+
+
 @pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 def test_gemm_config1_and_unit_vector(tile):
     """BASELINE config 1 (W 1024x1024 bf16, X 8x1024) and the e_k special case: Y = column k of W exactly."""
