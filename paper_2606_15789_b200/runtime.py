@@ -121,3 +121,45 @@ def dense_gemm(fmt: int, w: torch.Tensor, x: torch.Tensor, w_scale_vec: torch.Te
                         x.data_ptr(), B.X_DTYPE[fmt], x.stride(0), m, None if x_scale is None else x_scale.data_ptr(),
                         y.data_ptr(), y.stride(0), ws.data_ptr(), ws.numel(), _stream())
     return y
+
+
+# Tile geometries the library supports (tile_n, tile_k, layout flags), tried by autotune_tile.
+TILE_CANDIDATES = ((128, 64, 0), (128, 128, 0), (128, 256, 0), (32, 128, 0), (32, 256, 0), (32, 256, B.FLAG_LANE_STREAMS),
+                   (32, 512, B.FLAG_LANE_STREAMS), (32, 1024, B.FLAG_LANE_STREAMS))
+
+
+def autotune_tile(fmt: int, w: np.ndarray, n_out: int, k_in: int, m: int, x: torch.Tensor, x_scale: torch.Tensor | None = None,
+                  candidates=TILE_CANDIDATES, iters: int = 20, max_gap_bits: float | None = None, **encode_kw):
+    """Per-matrix choice of the tile geometry (P:l.167 "profiled to determine the optimal tensor-core tiling
+    geometry"; S: §8(f) NEXT-2): encode W with every candidate (tile_n, tile_k, layout flags) that fits the
+    shape, time anslin_gemm at batch size m with CUDA events, and return
+    (best, rows) -- best = dict(tile_n, tile_k, flags, us, bits_per_weight, container) of the fastest candidate
+    whose bits/weight is within max_gap_bits of the smallest one seen (None = no size constraint), rows = one
+    dict per candidate tried.  Measurement only: all arithmetic runs in the library."""
+    base_flags = int(encode_kw.pop("flags", 0))
+    rows = []
+    for tile_n, tile_k, lflags in candidates:
+        if k_in % tile_k or n_out % 128:
+            continue
+        try:
+            buf, st = B.anslin_encode_host(fmt, w, n_out, k_in, tile_k=tile_k, tile_n=tile_n, flags=base_flags | lflags, **encode_kw)
+        except B.AnslinError:
+            continue          # geometry not supported for this format
+        dw = DeviceWeight(buf)
+        y = torch.empty((m, n_out), dtype=torch.float32, device=x.device)
+        for _ in range(3):
+            dw.gemm(x, x_scale, y)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(iters):
+            dw.gemm(x, x_scale, y)
+        e1.record()
+        e1.synchronize()
+        rows.append(dict(tile_n=tile_n, tile_k=tile_k, flags=int(dw.weight.desc.flags), us=e0.elapsed_time(e1) * 1e3 / iters,
+                         bits_per_weight=st["bits_per_weight"], container=buf))
+        dw.close()
+    if not rows:
+        raise B.AnslinError("autotune_tile: no candidate geometry fits this shape")
+    smallest = min(r["bits_per_weight"] for r in rows)
+    ok = [r for r in rows if max_gap_bits is None or r["bits_per_weight"] <= smallest + max_gap_bits]
+    return min(ok, key=lambda r: r["us"]), rows

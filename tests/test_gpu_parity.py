@@ -324,6 +324,26 @@ def test_dense_gemm_int8_fp8():
     check_gemm(y, *og.gemm_fp8(x8, xs8, f8, sc))
 
 
+def test_autotune_tile_picks_a_supported_geometry():
+    """S: §8(f) NEXT-2 per-matrix tile-shape choice (P:l.167): every candidate must give the same Y within the
+    GEMM tolerance; the winner is one of the rows, the size constraint is honoured."""
+    rt = _rt()
+    n, k, m = 512, 2048, 16
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=55, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=56))
+    xd = rt.x_to_device(B.FMT_BF16, x)
+    best, rows = rt.autotune_tile(B.FMT_BF16, w, n, k, m, xd, flags=B.FLAG_STATE_PAYLOAD, iters=5, max_gap_bits=0.05)
+    assert len(rows) == len(rt.TILE_CANDIDATES) and best in rows
+    assert best["bits_per_weight"] <= min(r["bits_per_weight"] for r in rows) + 0.05
+    assert best["us"] == min(r["us"] for r in rows if r["bits_per_weight"] <= min(q["bits_per_weight"] for q in rows) + 0.05)
+    y_ref, a_ref = og.gemm_bf16(x, w)
+    for r in rows:
+        dw = rt.DeviceWeight(r["container"])
+        assert (dw.weight.desc.tile_n, dw.weight.desc.tile_k) == (r["tile_n"], r["tile_k"])
+        check_gemm(dw.gemm(xd).cpu().numpy(), y_ref, a_ref)
+        dw.close()
+
+
 # ------------------------------------------------------------------ full-size launch configuration
 @pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 @pytest.mark.parametrize("name,n,k,m", [("gate", 13824, 5120, 75), ("down", 5120, 13824, 16), ("k", 1024, 5120, 1)])
