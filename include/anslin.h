@@ -49,8 +49,12 @@ typedef enum {
   ANSLIN_FMT_FP8_E4M3 = 1, /* w_host: e4m3fn bytes; coded symbol = the byte; per-tensor scale in desc.w_scale */
   ANSLIN_FMT_INT8 = 2,     /* w_host: int8; coded symbol = the byte; scales_host = fp16[n_out] (SQ8-style) */
   ANSLIN_FMT_INT4_AWQ = 3, /* w_host: uint8[n_out][k_in/2], low nibble = even k; coded symbol = packed byte;
-                              scales_host/zeros_host = fp16[n_out][k_in/group_size]; w = (q - z) * s */
-  ANSLIN_FMT_FP8_E5M2 = 4  /* w_host: OCP e5m2 bytes (P:l.80 "FP8-E5M2"); otherwise as FP8_E4M3 */
+                              scales_host/zeros_host = fp16[n_out][k_in/group_size]; w = (q - z) * s.
+                              Plain per-channel int4 is this format with group_size = k_in (symmetric: z = 8) */
+  ANSLIN_FMT_FP8_E5M2 = 4, /* w_host: OCP e5m2 bytes (P:l.80 "FP8-E5M2"); otherwise as FP8_E4M3 */
+  ANSLIN_FMT_FP4_E2M1 = 5  /* w_host: uint8[n_out][k_in/2], low nibble = even k, OCP e2m1 codes s.ee.m (P:l.80 "FP4-E2M1");
+                              coded symbol = packed byte; per-tensor scale in desc.w_scale.  Every code is expanded
+                              exactly to e4m3 for the tensor core; X is fp8 (either kind) with per-token scales */
 } anslin_format;
 
 /* Element type of X. */

@@ -21,7 +21,7 @@ from . import codec
 
 MAGIC = 0x4C534E41  # "ANSL"
 VERSION = 1
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2 = 0, 1, 2, 3, 4
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1 = 0, 1, 2, 3, 4, 5
 FLAG_STATE_PAYLOAD = 1
 FLAG_LANE_STREAMS = 2   # each lane's words stored as its own stream (tile_n = 32 only), see _lane_record
 SEG_STEPS = 256         # lane-stream records are cut into segments of this many decode steps
@@ -35,9 +35,9 @@ HEADER_BYTES = 128
 TAIL_BYTES = 4096      # readable bytes that must follow the records section
 
 # symbols per 16-byte operand chunk, and default tile_k (in weights) per format
-SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4, FMT_FP8_E5M2: 16}
-DEFAULT_TILE_K = {FMT_BF16: 64, FMT_FP8_E4M3: 256, FMT_INT8: 256, FMT_INT4_AWQ: 256, FMT_FP8_E5M2: 256}
-WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2, FMT_FP8_E5M2: 1}
+SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4, FMT_FP8_E5M2: 16, FMT_FP4_E2M1: 8}
+DEFAULT_TILE_K = {FMT_BF16: 64, FMT_FP8_E4M3: 256, FMT_INT8: 256, FMT_INT4_AWQ: 256, FMT_FP8_E5M2: 256, FMT_FP4_E2M1: 256}
+WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2, FMT_FP8_E5M2: 1, FMT_FP4_E2M1: 2}
 
 
 def _align(x: int, a: int = 16) -> int:
@@ -53,7 +53,7 @@ def symbolise(fmt: int, w: np.ndarray):
     bf16 (w: uint16 bit patterns [n_out x k_in]): coded symbol = exponent bits 14..7;
         raw byte = (mantissa bits 6..0) << 1 | sign bit 15  (bf16 rotated left by one, low byte).
     fp8 / int8 (w: uint8 / int8 [n_out x k_in]): the byte itself.
-    int4 (w: uint8 [n_out x k_in/2], low nibble = even k): the packed byte (two K-adjacent codes).
+    int4 / fp4 (w: uint8 [n_out x k_in/2], low nibble = even k): the packed byte (two K-adjacent codes).
     """
     if fmt == FMT_BF16:
         w = np.ascontiguousarray(w).view(np.uint16)
@@ -76,7 +76,8 @@ def tile_order(fmt: int, tile_k: int, tile_n: int = TILE_N):
     symbol at (row rows[i], symbol column cols[i]) of the tile's [tile_n x sym_cols] symbol matrix.
 
     i = t*32 + lane.  The tile is cut along K into units of 32 operand bytes per row
-    (16 bf16/fp16 weights, 32 fp8/int8 weights); unit u is decoded completely before unit u+1.
+    (16 bf16/fp16 weights, 32 fp8/int8 weights; fp4 is expanded to one e4m3 byte per weight: 32 weights);
+    unit u is decoded completely before unit u+1.
     Inside a unit there are G = 2*tile_n/32 chunk rounds g; in round g lane l owns the 16-byte
     operand chunk (row (g mod tile_n/32)*32 + l, half g div (tile_n/32)) and produces its spc
     symbols in steps t = (u*G + g)*spc + e, e = 0..spc-1.  (tile_n = 32: lane l simply walks row l.)

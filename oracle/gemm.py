@@ -39,6 +39,17 @@ def e5m2_to_f64(code: np.ndarray) -> np.ndarray:
     return np.where(s == 1, -val, val)
 
 
+def e2m1_to_f64(code: np.ndarray) -> np.ndarray:
+    """OCP FP4 E2M1 (P:l.80), 4-bit codes s.ee.m, bias 1: (-1)^s * 2^(e-1) * (1 + m/2), subnormal (e = 0) m/2;
+    no infinities or NaNs: magnitudes 0, 0.5, 1, 1.5, 2, 3, 4, 6."""
+    c = code.astype(np.int64)
+    s = (c >> 3) & 1
+    e = (c >> 1) & 3
+    m = c & 1
+    val = np.where(e == 0, m / 2.0, np.ldexp(1.0 + m / 2.0, e - 1))
+    return np.where(s == 1, -val, val)
+
+
 def int4_unpack(packed: np.ndarray) -> np.ndarray:
     """uint8 [n x k/2], low nibble = even k  ->  uint8 [n x k] codes 0..15."""
     p = packed.view(np.uint8)
@@ -77,6 +88,14 @@ def gemm_int8(xq: np.ndarray, x_scale: np.ndarray, wq: np.ndarray, w_scale: np.n
 def gemm_fp8(xq: np.ndarray, x_scale: np.ndarray, wq: np.ndarray, w_scale: float, x_e5m2: bool = False, w_e5m2: bool = False):
     """fp8 (reading A15): Y = (sum_k x8*w8) * s_x[m] * s_w; each operand e4m3 unless flagged e5m2."""
     y, a = gemm_f64((e5m2_to_f64 if x_e5m2 else e4m3_to_f64)(xq), (e5m2_to_f64 if w_e5m2 else e4m3_to_f64)(wq))
+    sc = x_scale.astype(np.float64)[:, None] * float(w_scale)
+    return y * sc, a * sc
+
+
+def gemm_fp4(xq: np.ndarray, x_scale: np.ndarray, packed: np.ndarray, w_scale: float, x_e5m2: bool = False):
+    """fp4-e2m1 weights (two codes per byte, low nibble = even k), fp8 activations with per-token scales:
+    Y = (sum_k x8 * w4) * s_x[m] * s_w, the fp8 recipe of A15 with the 4-bit value set."""
+    y, a = gemm_f64((e5m2_to_f64 if x_e5m2 else e4m3_to_f64)(xq), e2m1_to_f64(int4_unpack(packed)))
     sc = x_scale.astype(np.float64)[:, None] * float(w_scale)
     return y * sc, a * sc
 

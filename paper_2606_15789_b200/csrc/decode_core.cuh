@@ -372,6 +372,19 @@ __device__ __forceinline__ uint32_t awq_dequant2(uint32_t byte, __half2 zoff, __
   return *reinterpret_cast<const uint32_t *>(&h);
 }
 
+// fp4-e2m1 (s.ee.m: 0, 0.5, 1, 1.5, 2, 3, 4, 6) -> the e4m3 byte of the same value, four codes at a time: the four
+// nibbles of sel[15:0] pick their magnitude byte from an 8-entry table held in two registers (PRMT), the sign
+// nibble-bit picks 0x00 / 0x80.  `mag` = codes & 0x7777..., `sgn` = (codes >> 3) & 0x1111... (upper 16 bits ignored).
+__device__ __forceinline__ uint32_t e2m1x4_to_e4m3(uint32_t mag, uint32_t sgn) {
+  return __byte_perm(0x3C383000u, 0x4C484440u, mag) | __byte_perm(0x00008000u, 0u, sgn);
+}
+// four packed bytes (8 codes, low nibble first) -> two words of e4m3 operand bytes
+__device__ __forceinline__ void e2m1x8_to_e4m3(uint32_t b, uint32_t &lo, uint32_t &hi) {
+  const uint32_t mag = b & 0x77777777u, sgn = (b >> 3) & 0x11111111u;
+  lo = e2m1x4_to_e4m3(mag, sgn);
+  hi = e2m1x4_to_e4m3(mag >> 16, sgn >> 16);
+}
+
 // Raw-plane (bf16 sign+mantissa) reader of one tile: 16 steps of one lane = one 16-byte vector,
 // fetched one vector ahead into registers, with an L2 prefetch four vectors ahead.
 template <bool kPayload>
@@ -466,6 +479,25 @@ __device__ __forceinline__ void decode_unit(typename POL::S (&s)[J], uint32_t ri
                                             awq_dequant2((B[j] >> 16) & 0xFF, zoff, sc), awq_dequant2(B[j] >> 24, zoff, sc)));
         } else {
           emit.packed(j, g, lane, B[j]);
+        }
+      }
+    }
+  } else if constexpr (FMT == ANSLIN_FMT_FP4_E2M1) {
+#pragma unroll 1
+    for (int g = 0; g < G; ++g) {   // 8 packed bytes = 16 codes = one 16-byte chunk of e4m3 operand bytes
+      POL::template upkeep8<J>(s, ring0, lane);
+      uint32_t B0[J], B1[J];
+      decode4<POL, J>(s, B0, tab, lt);
+      decode4<POL, J>(s, B1, tab, lt);
+#pragma unroll
+      for (int j = 0; j < J; ++j) {
+        if constexpr (Emit::kOperand) {
+          uint4 v;
+          e2m1x8_to_e4m3(B0[j], v.x, v.y);
+          e2m1x8_to_e4m3(B1[j], v.z, v.w);
+          emit.chunk(j, g, lane, v);
+        } else {
+          emit.packed8(j, g, lane, B0[j], B1[j]);
         }
       }
     }

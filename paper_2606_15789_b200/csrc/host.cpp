@@ -320,7 +320,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
   h.magic = kMagic; h.version = kVersion; h.format = g.fmt; h.n_out = g.n_out; h.k_in = g.k_in;
   h.tile_n = g.tile_n; h.tile_k = g.tile_k; h.streams = kLanes; h.prob_bits = kProbBits; h.word_bits = kWordBits;
   h.state_lo_log2 = kStateLoLog2; h.group_size = g.group; h.flags = g.flags; h.n_tiles = uint32_t(g.n_tiles);
-  h.w_scale = is_fp8(g.fmt) ? desc->w_scale : 1.0f;
+  h.w_scale = is_fp8_path(g.fmt) ? desc->w_scale : 1.0f;
   for (uint32_t b : segbytes) h.max_seg_bytes = std::max(h.max_seg_bytes, b);
 
   uint8_t *out = static_cast<uint8_t *>(container_out);

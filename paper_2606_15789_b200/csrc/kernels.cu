@@ -152,6 +152,7 @@ template <uint32_t FMT> struct FmtTraits;
 template <> struct FmtTraits<ANSLIN_FMT_BF16> { static constexpr int kind = 0; static constexpr uint32_t c = 1, ab = 1; static constexpr int xbytes = 2; };
 template <> struct FmtTraits<ANSLIN_FMT_INT4_AWQ> { static constexpr int kind = 0; static constexpr uint32_t c = 1, ab = 0; static constexpr int xbytes = 2; };
 template <> struct FmtTraits<ANSLIN_FMT_FP8_E4M3> { static constexpr int kind = 1; static constexpr uint32_t c = 1, ab = 0; static constexpr int xbytes = 1; };
+template <> struct FmtTraits<ANSLIN_FMT_FP4_E2M1> { static constexpr int kind = 1; static constexpr uint32_t c = 1, ab = 0; static constexpr int xbytes = 1; };
 template <> struct FmtTraits<ANSLIN_FMT_INT8> { static constexpr int kind = 2; static constexpr uint32_t c = 2, ab = 1; static constexpr int xbytes = 1; };
 
 // ------------------------------------------------------------------------------------------------
@@ -191,7 +192,7 @@ template <int RB, int J> struct TileTraits {
 constexpr int kJ32 = ANSLIN_J32;   // tiles a warp interleaves when tiles have 32 rows
 
 __host__ __device__ constexpr size_t row_bytes_of(uint32_t fmt, size_t k) {
-  return fmt == ANSLIN_FMT_BF16 ? k * 2 : fmt == ANSLIN_FMT_INT4_AWQ ? k / 2 : k;
+  return fmt == ANSLIN_FMT_BF16 ? k * 2 : is_packed4(fmt) ? k / 2 : k;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -203,7 +204,7 @@ struct GlobalEmit {
   // 32-row tiles (lane = row): a lane's 16-byte chunks of two consecutive units (64 B of its row) are staged in
   // shared memory and written out as 64-byte row segments, 8 rows per store instruction, instead of one 16-byte
   // store per lane into 32 different rows (which bound the kernel at a third of the decoder's rate).
-  static constexpr bool kStaged = RB == 1 && FMT != ANSLIN_FMT_INT4_AWQ;
+  static constexpr bool kStaged = RB == 1 && !is_packed4(FMT);
   static constexpr uint32_t kStageBytes = kStaged ? 2048 : 0;   // per stream
   uint8_t *tile_out[J];  // &W[first row of tile j][k0] in bytes
   size_t row_bytes;      // bytes per W row
@@ -240,6 +241,10 @@ struct GlobalEmit {
   __device__ __forceinline__ void packed(int j, int g, int lane, uint32_t b) const {  // int4: 4 packed bytes = 8 weights
     uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 8 + (g / RB) * 4;
     *reinterpret_cast<uint32_t *>(p) = b;
+  }
+  __device__ __forceinline__ void packed8(int j, int g, int lane, uint32_t b0, uint32_t b1) const {  // fp4: 8 packed bytes = 16 weights
+    uint8_t *p = tile_out[j] + size_t((g % RB) * 32 + lane) * row_bytes + size_t(u) * 16 + (g / RB) * 8;
+    *reinterpret_cast<uint2 *>(p) = make_uint2(b0, b1);
   }
 };
 
@@ -318,7 +323,7 @@ __host__ __device__ __forceinline__ uint32_t cta_of_tile(uint32_t t, uint32_t G,
 template <uint32_t FMT>
 __device__ __forceinline__ float finalize(uint32_t bits, float xs, float ws) {
   if constexpr (FMT == ANSLIN_FMT_INT8) return float(int32_t(bits)) * xs * ws;
-  else if constexpr (FMT == ANSLIN_FMT_FP8_E4M3) return __uint_as_float(bits) * xs * ws;
+  else if constexpr (is_fp8_path(FMT)) return __uint_as_float(bits) * xs * ws;
   else return __uint_as_float(bits);
 }
 template <uint32_t FMT>
@@ -353,7 +358,7 @@ template <uint32_t FMT>
 __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_base, uint32_t tfull_s, uint32_t tempty_s,
                                              FinSeg *fin, uint32_t t_begin, uint32_t t_end, uint32_t KT, uint32_t c, uint32_t G,
                                              uint32_t T, int warp, int lane) {
-  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
+  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   const uint32_t row = uint32_t(warp * 32 + lane);
   uint32_t si = 0;
   for (uint32_t t = t_begin; t < t_end; ++si) {
@@ -362,7 +367,7 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     const uint32_t n = stripe * kTileN + row;
     float ws = 1.0f;
     if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n]);
-    if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
+    if (is_fp8_path(FMT)) ws = p.w_scale;
     // The MMA warp watches the accumulator's mbarrier and releases us through a named barrier: the four
     // epilogue warps sleep in hardware meanwhile instead of polling next to the decoder warps.
     named_bar_sync(kBarEpiGo, (kEpiWarps + 1) * 32);
@@ -413,7 +418,7 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
 // 16-byte loads, up to 8 contributors in flight per thread.
 template <uint32_t FMT>
 __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *fin, uint32_t KT, uint32_t G, uint32_t T) {
-  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || FMT == ANSLIN_FMT_FP8_E4M3;
+  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   constexpr int kItems = 2;   // items per thread and pass: their loads are all issued before the first add
   for (int seg = 0; seg < 2; ++seg) {
     if (!fin[seg].valid) continue;
@@ -462,7 +467,7 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
         for (int j = 0; j < 4; ++j) {
           float ws = 1.0f;
           if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
-          if (FMT == ANSLIN_FMT_FP8_E4M3) ws = p.w_scale;
+          if (is_fp8_path(FMT)) ws = p.w_scale;
           o[j] = finalize<FMT>(acc[q][j], xs, ws);
         }
         float *yo = p.y + size_t(mm) * p.ldy + n4;
@@ -512,6 +517,7 @@ struct SmemEmit {
     sts128(slot_a + row * 32u + ((c ^ ((uint32_t(lane) >> 2) & 1u)) << 4), v);  // Swizzle<1,4,3>
   }
   __device__ __forceinline__ void packed(int, int, int, uint32_t) const {}
+  __device__ __forceinline__ void packed8(int, int, int, uint32_t, uint32_t) const {}
 };
 
 template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS>
@@ -896,11 +902,11 @@ Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
 
 bool x_dtype_ok(uint32_t fmt, uint32_t dt) {
   return (fmt == ANSLIN_FMT_BF16 && dt == ANSLIN_DT_BF16) || (fmt == ANSLIN_FMT_INT4_AWQ && dt == ANSLIN_DT_F16) ||
-         (fmt == ANSLIN_FMT_INT8 && dt == ANSLIN_DT_I8) || (is_fp8(fmt) && (dt == ANSLIN_DT_FP8_E4M3 || dt == ANSLIN_DT_FP8_E5M2));
+         (fmt == ANSLIN_FMT_INT8 && dt == ANSLIN_DT_I8) || (is_fp8_path(fmt) && (dt == ANSLIN_DT_FP8_E4M3 || dt == ANSLIN_DT_FP8_E5M2));
 }
 // tcgen05 instruction-descriptor format code of the weight operand (a) / of X (b)
 uint32_t afmt_of(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT8 || fmt == ANSLIN_FMT_FP8_E5M2 ? 1u : 0u; }
-uint32_t bfmt_of(uint32_t fmt, uint32_t dt) { return is_fp8(fmt) ? (dt == ANSLIN_DT_FP8_E5M2 ? 1u : 0u) : afmt_of(fmt); }
+uint32_t bfmt_of(uint32_t fmt, uint32_t dt) { return is_fp8_path(fmt) ? (dt == ANSLIN_DT_FP8_E5M2 ? 1u : 0u) : afmt_of(fmt); }
 
 int sm_budget() { return std::max(1, num_sms()); }
 
@@ -938,7 +944,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   if (n < 1 || n > kMaxProblems || !workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) & 15)) return ANSLIN_ERR_INVALID_ARG;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
   const Header &h0 = ws[0]->h;
-  const bool scaled = h0.format == ANSLIN_FMT_INT8 || is_fp8(h0.format);
+  const bool scaled = h0.format == ANSLIN_FMT_INT8 || is_fp8_path(h0.format);
   const int xb = (h0.format == ANSLIN_FMT_BF16 || h0.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
   if (!x_dtype_ok(h0.format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
   uint32_t mpad_max = 16;
@@ -1053,6 +1059,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     case ANSLIN_FMT_FP8_E5M2: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);   // same bytes, another descriptor code
     case ANSLIN_FMT_INT8: return ANSLIN_LAUNCH(ANSLIN_FMT_INT8, false);
     case ANSLIN_FMT_INT4_AWQ: return ANSLIN_LAUNCH(ANSLIN_FMT_INT4_AWQ, false);
+    case ANSLIN_FMT_FP4_E2M1: return ANSLIN_LAUNCH(ANSLIN_FMT_FP4_E2M1, false);
   }
 #undef ANSLIN_LAUNCH
   return ANSLIN_ERR_UNSUPPORTED;
@@ -1129,6 +1136,7 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
     case ANSLIN_FMT_FP8_E5M2: return launch_decode<ANSLIN_FMT_FP8_E4M3, false>(cv, w_out_dev, st);
     case ANSLIN_FMT_INT8: return launch_decode<ANSLIN_FMT_INT8, false>(cv, w_out_dev, st);
     case ANSLIN_FMT_INT4_AWQ: return launch_decode<ANSLIN_FMT_INT4_AWQ, false>(cv, w_out_dev, st);
+    case ANSLIN_FMT_FP4_E2M1: return launch_decode<ANSLIN_FMT_FP4_E2M1, false>(cv, w_out_dev, st);
   }
   return ANSLIN_ERR_UNSUPPORTED;
 }
@@ -1258,7 +1266,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   if ((reinterpret_cast<uintptr_t>(w_dev) | reinterpret_cast<uintptr_t>(x_dev) | reinterpret_cast<uintptr_t>(y_dev) |
        reinterpret_cast<uintptr_t>(workspace_dev)) & 15)
     return ANSLIN_ERR_INVALID_ARG;
-  const bool scaled = format == ANSLIN_FMT_INT8 || is_fp8(format);
+  const bool scaled = format == ANSLIN_FMT_INT8 || is_fp8_path(format);
   if (scaled && !x_scale_dev) return ANSLIN_ERR_INVALID_ARG;
   if (format == ANSLIN_FMT_INT8 && !w_scale_dev) return ANSLIN_ERR_INVALID_ARG;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
@@ -1286,7 +1294,9 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
     case ANSLIN_FMT_BF16: return launch_dense<ANSLIN_FMT_BF16>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_INT4_AWQ: return launch_dense<ANSLIN_FMT_INT4_AWQ>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_FP8_E4M3:
-    case ANSLIN_FMT_FP8_E5M2: return launch_dense<ANSLIN_FMT_FP8_E4M3>(tmw, tmx, p, grid, smem, st);
+    case ANSLIN_FMT_FP8_E5M2:
+    case ANSLIN_FMT_FP4_E2M1:   // the fp4 slot takes the e4m3 bytes fp4 expands to: same MMA kind as the fused fp4 path
+      return launch_dense<ANSLIN_FMT_FP8_E4M3>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_INT8: return launch_dense<ANSLIN_FMT_INT8>(tmw, tmx, p, grid, smem, st);
   }
   return ANSLIN_ERR_UNSUPPORTED;

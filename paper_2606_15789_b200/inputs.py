@@ -9,7 +9,7 @@ from __future__ import annotations
 
 import numpy as np
 
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2 = 0, 1, 2, 3, 4
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1 = 0, 1, 2, 3, 4, 5
 
 # BASELINE.json configs 2/3 (Qwen-14B-shaped dense decoder layer), [n_out, k_in] = Linear.weight
 QWEN14B_LAYER = [("q", 5120, 5120), ("k", 1024, 5120), ("v", 1024, 5120), ("o", 5120, 5120),
@@ -81,6 +81,17 @@ def quant_awq4_weights(w: np.ndarray, group: int = 128):
     return packed, s, z.astype(np.float16)
 
 
+def quant_int4_sym_weights(w: np.ndarray):
+    """Plain symmetric per-channel int4 (S: §8(f) NEXT-2 "plain int4"): s[n] = amax_n/7, q = clip(rint(w/s), -8, 7),
+    stored offset-binary (q + 8) so that it IS the AWQ container with one group per row and zero point 8.
+    Returns (packed uint8 [n x k/2], scales fp16 [n x 1], zeros fp16 [n x 1] = 8)."""
+    n, k = w.shape
+    s = np.maximum((np.abs(w).max(axis=1) / 7.0).astype(np.float16), np.float16(6e-8))
+    q = (np.clip(np.rint(w / s.astype(np.float32)[:, None]), -8, 7) + 8).astype(np.uint8)
+    packed = (q[:, 0::2] | (q[:, 1::2] << 4)).astype(np.uint8)
+    return packed, s.reshape(n, 1), np.full((n, 1), 8, dtype=np.float16)
+
+
 def f32_to_e4m3_bytes(x: np.ndarray) -> np.ndarray:
     """float32 -> OCP e4m3fn byte codes via torch's CPU cast (round to nearest even, saturating inputs
     are the caller's job: values are pre-scaled to |x| <= 448)."""
@@ -120,6 +131,20 @@ def quant_fp8_e5m2_acts(x: np.ndarray):
     s = (np.abs(x).max(axis=1) / 57344.0).astype(np.float32)
     s = np.maximum(s, np.float32(1e-12))
     return f32_to_e5m2_bytes(x / s[:, None]), s
+
+
+def quant_fp4_weights(w: np.ndarray):
+    """Per-tensor fp4-e2m1: s = amax/6, every w/s rounded to the nearest of the 8 magnitudes
+    0, 0.5, 1, 1.5, 2, 3, 4, 6 (ties to the even code), sign in bit 3.  Returns (packed uint8 [n x k/2], s)."""
+    s = float(np.abs(w).max() / 6.0)
+    grid = np.array([0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0], dtype=np.float32)
+    a = np.abs(w / np.float32(s)).astype(np.float32)
+    hi = np.clip(np.searchsorted(grid, a, side="left"), 1, 7)
+    lo = hi - 1
+    d_lo, d_hi = a - grid[lo], grid[hi] - a
+    code = np.where(d_lo < d_hi, lo, np.where(d_hi < d_lo, hi, np.where(lo % 2 == 0, lo, hi))).astype(np.uint8)
+    code |= (np.signbit(w).astype(np.uint8) << 3)
+    return (code[:, 0::2] | (code[:, 1::2] << 4)).astype(np.uint8), s
 
 
 def route_top2(m_tokens: int, n_experts: int, seed: int):

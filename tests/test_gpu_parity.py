@@ -65,6 +65,10 @@ def _decode_cases():
     f5, sc5 = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(256, 768, seed=47, std=0.015, outliers=False))
     yield "e5m2", B.FMT_FP8_E5M2, f5, 768, dict(tile_k=256, w_scale=sc5)
     yield "e5m2-32x768-lanes", B.FMT_FP8_E5M2, f5, 768, dict(tile_k=768, w_scale=sc5, tile_n=32, flags=2)
+    f4, sc4 = inputs.quant_fp4_weights(inputs.weights_f32(256, 1024, seed=48, outliers=False))
+    yield "fp4", B.FMT_FP4_E2M1, f4, 1024, dict(tile_k=256, w_scale=sc4)
+    yield "fp4-32x256", B.FMT_FP4_E2M1, f4, 1024, dict(tile_k=256, w_scale=sc4, tile_n=32)
+    yield "fp4-32x1024-lanes", B.FMT_FP4_E2M1, f4, 1024, dict(tile_k=1024, w_scale=sc4, tile_n=32, flags=2)
     yield "bf16-constant-lanes", B.FMT_BF16, np.full((128, 256), 0xBF80, dtype=np.uint16), 256, dict(tile_k=256, tile_n=32, flags=2)
 
 
@@ -227,6 +231,28 @@ def test_gemm_int4(m, lay):
 
 
 @pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
+def test_gemm_int4_plain_per_channel(lay):
+    """S: §8(f) NEXT-2 "plain int4": symmetric per-channel int4 is the AWQ container with group_size = k_in and zero
+    point 8; decode bit-exact, GEMM against (q - 8) * s[n] in float64."""
+    tile_n, lflag = lay
+    rt = _rt()
+    n, k, m = 256, 1024, 24
+    p4, s4, z4 = inputs.quant_int4_sym_weights(inputs.weights_f32(n, k, seed=83, outliers=False))
+    x = inputs.acts_f32(m, k, seed=84).astype(np.float16)
+    buf, st = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=256 if tile_n == 128 else 512, scales=s4, zeros=z4,
+                                   group_size=k, tile_n=tile_n, flags=lflag)
+    dw = rt.DeviceWeight(buf)
+    assert np.array_equal(dw.decode().cpu().numpy(), p4)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
+    y_ref, a_ref = og.gemm_int4(x, p4, s4, z4, k)
+    check_gemm(y, y_ref, a_ref)
+    q = og.int4_unpack(p4).astype(np.float64) - 8.0
+    assert np.allclose(y_ref, (x.astype(np.float64) @ q.T) * s4.astype(np.float64).T, rtol=1e-12, atol=1e-12)
+    assert st["bits_per_weight"] < 4.0
+    dw.close()
+
+
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
 @pytest.mark.parametrize("m", [1, 37])
 @pytest.mark.parametrize("x_kind", ["e5m2", "e4m3"])
 def test_gemm_fp8_e5m2(m, lay, x_kind):
@@ -243,6 +269,29 @@ def test_gemm_fp8_e5m2(m, lay, x_kind):
     y = dw.gemm(rt.x_to_device(B.FMT_FP8_E5M2, x8), torch.from_numpy(xs).cuda(),
                 x_dtype=B.DT_FP8_E5M2 if x_kind == "e5m2" else B.DT_FP8_E4M3).cpu().numpy()
     check_gemm(y, *og.gemm_fp8(x8, xs, f5, sc, x_e5m2=x_kind == "e5m2", w_e5m2=True))
+    dw.close()
+
+
+@pytest.mark.parametrize("lay", LAYOUTS, ids=LAYOUT_IDS)
+@pytest.mark.parametrize("m", [1, 37, 64])
+def test_gemm_fp4(m, lay):
+    """NEXT-2 format fp4-E2M1 (P:l.80): packed codes are the coded symbols; the decoder expands every code to the
+    e4m3 byte of the same value, so the products are exact and only the fp32 accumulation rounds."""
+    tile_n, lflag = lay
+    rt = _rt()
+    import torch
+    n, k = 256, 2048
+    p4, sc = inputs.quant_fp4_weights(inputs.weights_f32(n, k, seed=75, outliers=False))
+    x8, xs = inputs.quant_fp8_acts(inputs.acts_f32(m, k, seed=76))
+    buf, st = B.anslin_encode_host(B.FMT_FP4_E2M1, p4, n, k, tile_k=512, w_scale=sc, tile_n=tile_n, flags=lflag)
+    assert st["bits_per_weight"] < 4.0
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_FP4_E2M1, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
+    check_gemm(y, *og.gemm_fp4(x8, xs, p4, sc))
+    if m == 37:   # X in e5m2
+        x5, xs5 = inputs.quant_fp8_e5m2_acts(inputs.acts_f32(m, k, seed=76))
+        y = dw.gemm(rt.x_to_device(B.FMT_FP4_E2M1, x5), torch.from_numpy(xs5).cuda(), x_dtype=B.DT_FP8_E5M2).cpu().numpy()
+        check_gemm(y, *og.gemm_fp4(x5, xs5, p4, sc, x_e5m2=True))
     dw.close()
 
 

@@ -54,6 +54,9 @@ def _cases():
     yield "int4-32x512-lanes", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=512, scales=s4, zeros=z4, group_size=128, tile_n=32, flags=2)
     f5, sc5 = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(128, 512, seed=34, std=0.015, outliers=False))
     yield "e5m2", oc.FMT_FP8_E5M2, f5, 512, dict(tile_k=256, w_scale=sc5)
+    f4, sc4 = inputs.quant_fp4_weights(inputs.weights_f32(128, 512, seed=35, outliers=False))
+    yield "fp4", oc.FMT_FP4_E2M1, f4, 512, dict(tile_k=256, w_scale=sc4)
+    yield "fp4-32x512-lanes", oc.FMT_FP4_E2M1, f4, 512, dict(tile_k=512, w_scale=sc4, tile_n=32, flags=2)
     yield "e5m2-32x512-lanes", oc.FMT_FP8_E5M2, f5, 512, dict(tile_k=512, w_scale=sc5, tile_n=32, flags=2)
 
 
@@ -80,7 +83,7 @@ def test_cross_decode_and_stats(name, fmt, w, k_in, kw):
     assert abs(st["bits_per_weight"] - ost["bits_per_weight"]) < 0.01
     assert st["entropy_bits_per_symbol"] == pytest.approx(ost["entropy_bits_per_symbol"], abs=1e-9)
     assert st["xent_bits_per_symbol"] >= st["entropy_bits_per_symbol"]
-    wps = 2 if fmt == oc.FMT_INT4_AWQ else 1
+    wps = oc.WEIGHTS_PER_SYMBOL[fmt]
     assert st["bits_per_weight"] >= (st["entropy_bits_per_symbol"] + st["raw_entropy_bits_per_symbol"]) / wps
     total_bits = (st["payload_bits"] + st["state_bits"] + st["pad_bits"] + st["raw_bits"] + st["side_bits"])
     assert total_bits <= 8 * buf.size <= total_bits + st["offset_table_bits"] + st["freq_table_bits"] + 8 * (128 + 5 * 16 + 4096)

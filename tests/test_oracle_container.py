@@ -180,6 +180,26 @@ def test_roundtrip_and_gemm_fp8_e5m2():
     assert y[0, 0] == (1.5 + 2.0 - 1.5) * 0.5
 
 
+def test_e2m1_values_and_fp4_roundtrip():
+    """fp4-e2m1 (P:l.80): the 16 code values of the OCP table; each is exactly an e4m3 number (what the kernel
+    feeds the tensor core), checked through torch's e4m3 cast; container round trip; quantiser sanity."""
+    import torch
+    got = og.e2m1_to_f64(np.arange(16))
+    table = [0.0, 0.5, 1.0, 1.5, 2.0, 3.0, 4.0, 6.0]
+    assert got.tolist() == table + [-v for v in table] and np.signbit(got[8])
+    back = torch.from_numpy(got.astype(np.float32)).to(torch.float8_e4m3fn).to(torch.float64).numpy()
+    assert np.array_equal(back, got)
+    wf = inputs.weights_f32(128, 512, seed=15, outliers=False)
+    p4, sc = inputs.quant_fp4_weights(wf)
+    _, st, h, _ = _roundtrip(oc.FMT_FP4_E2M1, p4, 512, tile_k=256, w_scale=sc)
+    assert h.w_scale == pytest.approx(sc, rel=1e-6) and st["payload_bits"] / st["n_weights"] < 4.0
+    wd = og.e2m1_to_f64(og.int4_unpack(p4)) * sc
+    assert np.all(np.abs(wd - wf) <= 1.0 * sc + 1e-9)           # largest grid gap is 2 (4 -> 6): half of it
+    x8 = np.array([[0x38, 0x40]], np.uint8)                      # 1.0, 2.0 in e4m3
+    y, a = og.gemm_fp4(x8, np.array([2.0], np.float32), np.array([[0x7A]], np.uint8), 0.5)   # codes 0xA = -1.0, 0x7 = 6.0
+    assert y[0, 0] == (1.0 * -1.0 + 2.0 * 6.0) * 2.0 * 0.5 and a[0, 0] == 13.0
+
+
 def test_bf16_conversion_against_torch():
     import torch
     x = np.random.default_rng(1).standard_normal(4096).astype(np.float32) * 3
