@@ -196,6 +196,20 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
                       const void *x_scale_dev, void *y_dev, int64_t ldy, void *workspace_dev,
                       size_t workspace_bytes, void *stream);
 
+/*
+ * Entropy study (P:l.64-78, Fig. 2; S: NEXT-4): empirical 256-bin histograms of the 8-bit symbols of a row-major
+ * weight tensor resident in HBM, with the coder's own symbolisation (a1).
+ *   w_dev: 16-byte aligned; n_elems = stored elements (bf16: 16-bit values; every other format: bytes).
+ *   counts_dev: uint64[2][256], overwritten.  Plane 0 = coded symbols (bf16: exponent byte; fp8/int8: the byte;
+ *   int4/fp4: the packed byte of two codes).  Plane 1 = bf16: the raw byte (mantissa<<1 | sign); int4/fp4: the 4-bit
+ *   codes in bins 0..15; else zeros.  One pass over W, enqueued on `stream`; no synchronisation.
+ */
+int anslin_histogram(uint32_t format, const void *w_dev, uint64_t n_elems, void *counts_dev, void *stream);
+/* H = -sum p log2 p of a histogram of `bins` host counts (P:l.70), bits per symbol; 0 for an empty histogram. */
+double anslin_entropy_bits(const uint64_t *counts_host, int32_t bins);
+/* Symbol-weighted model entropy (P:l.74): sum_l n[l] * h[l] / sum_l n[l]; 0 if all n are 0. */
+double anslin_entropy_weighted(const double *h, const uint64_t *n, int32_t layers);
+
 /* Number of kernels the last device call on this thread enqueued (for bench.py's gpu_launches). */
 int anslin_last_launch_count(void);
 

@@ -23,7 +23,8 @@ X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_IN
 EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_close", "anslin_describe",
            "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm_multi_workspace_bytes", "anslin_gemm",
            "anslin_gemm_multi", "anslin_gemm_grouped",
-           "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_last_launch_count", "anslin_status_string"]
+           "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_histogram", "anslin_entropy_bits",
+           "anslin_entropy_weighted", "anslin_last_launch_count", "anslin_status_string"]
 
 
 class AnslinError(RuntimeError):
@@ -71,6 +72,10 @@ def lib() -> ctypes.CDLL:
         L.anslin_gemm_grouped.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(i32), vp, u32, i64, vp, vp, i64, vp, sz, vp]
         L.anslin_dense_workspace_bytes.argtypes = [u32, u32, i32]; L.anslin_dense_workspace_bytes.restype = sz
         L.anslin_dense_gemm.argtypes = [u32, vp, u32, u32, vp, ctypes.c_float, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
+        L.anslin_histogram.argtypes = [u32, vp, ctypes.c_uint64, vp, vp]
+        L.anslin_entropy_bits.argtypes = [ctypes.POINTER(ctypes.c_uint64), i32]; L.anslin_entropy_bits.restype = ctypes.c_double
+        L.anslin_entropy_weighted.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_uint64), i32]
+        L.anslin_entropy_weighted.restype = ctypes.c_double
         L.anslin_last_launch_count.restype = ctypes.c_int
         L.anslin_status_string.argtypes = [ctypes.c_int]; L.anslin_status_string.restype = ctypes.c_char_p
         _lib = L
@@ -198,6 +203,23 @@ def anslin_dense_gemm(fmt: int, w_ptr: int, n_out: int, k_in: int, w_scale_ptr: 
                                    ctypes.c_void_p(x_ptr), x_dtype, ldx, m, ctypes.c_void_p(x_scale_ptr or 0),
                                    ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.c_void_p(stream)),
            "anslin_dense_gemm")
+
+
+def anslin_histogram(fmt: int, w_ptr: int, n_elems: int, counts_ptr: int, stream: int = 0):
+    _check(lib().anslin_histogram(fmt, ctypes.c_void_p(w_ptr), n_elems, ctypes.c_void_p(counts_ptr), ctypes.c_void_p(stream)),
+           "anslin_histogram")
+
+
+def anslin_entropy_bits(counts) -> float:
+    c = np.ascontiguousarray(counts, dtype=np.uint64)
+    return float(lib().anslin_entropy_bits(c.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)), c.size))
+
+
+def anslin_entropy_weighted(hs, ns) -> float:
+    h = np.ascontiguousarray(hs, dtype=np.float64)
+    n = np.ascontiguousarray(ns, dtype=np.uint64)
+    return float(lib().anslin_entropy_weighted(h.ctypes.data_as(ctypes.POINTER(ctypes.c_double)),
+                                               n.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)), h.size))
 
 
 def anslin_last_launch_count() -> int:

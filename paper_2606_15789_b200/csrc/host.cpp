@@ -444,6 +444,27 @@ int anslin_describe(const anslin_weight *w, anslin_desc *out) {
   return ANSLIN_OK;
 }
 
+double anslin_entropy_bits(const uint64_t *counts_host, int32_t bins) {
+  if (!counts_host || bins < 1) return 0.0;
+  long double n = 0;
+  for (int32_t i = 0; i < bins; ++i) n += counts_host[i];
+  if (n == 0) return 0.0;
+  long double h = 0;
+  for (int32_t i = 0; i < bins; ++i)
+    if (counts_host[i]) {
+      const long double p = counts_host[i] / n;
+      h -= p * log2l(p);
+    }
+  return double(h);
+}
+
+double anslin_entropy_weighted(const double *h, const uint64_t *n, int32_t layers) {
+  if (!h || !n || layers < 1) return 0.0;
+  long double num = 0, den = 0;
+  for (int32_t i = 0; i < layers; ++i) { num += (long double)(n[i]) * h[i]; den += n[i]; }
+  return den == 0 ? 0.0 : double(num / den);
+}
+
 const char *anslin_status_string(int s) {
   switch (s) {
     case ANSLIN_OK: return "ok";

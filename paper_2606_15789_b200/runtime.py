@@ -163,3 +163,27 @@ def autotune_tile(fmt: int, w: np.ndarray, n_out: int, k_in: int, m: int, x: tor
     smallest = min(r["bits_per_weight"] for r in rows)
     ok = [r for r in rows if max_gap_bits is None or r["bits_per_weight"] <= smallest + max_gap_bits]
     return min(ok, key=lambda r: r["us"]), rows
+
+
+def entropy_study(fmt: int, tensors):
+    """P:l.64-78 entropy study over device-resident weight tensors of one numeric format (S: NEXT-4): per tensor the
+    256-bin histograms (anslin_histogram) and their entropies, and the symbol-weighted model entropy (P:l.74).
+    tensors: cuda tensors of the stored elements (bf16 as int16/bfloat16, others as bytes).  Returns
+    dict(layers=[dict(n_weights, counts[2][256], h_coded, h_side, bits_per_weight)], model_bits_per_weight);
+    bits_per_weight = H(exponent) + H(sign|mantissa) for bf16, H(byte) for fp8/int8, H(packed byte)/2 for int4/fp4
+    (h_side for those: the entropy of the single 4-bit code, the symbol Fig. 2 counts)."""
+    packed4 = fmt in (B.FMT_INT4_AWQ, B.FMT_FP4_E2M1)
+    layers, counts_dev = [], []
+    for t in tensors:
+        t = t.contiguous()
+        c = torch.empty((2, 256), dtype=torch.int64, device=t.device)
+        B.anslin_histogram(fmt, t.data_ptr(), t.numel(), c.data_ptr(), _stream())
+        counts_dev.append((t.numel(), c))
+    for n, c in counts_dev:
+        counts = c.cpu().numpy().astype(np.uint64)
+        h0 = B.anslin_entropy_bits(counts[0])
+        h1 = B.anslin_entropy_bits(counts[1][:16] if packed4 else counts[1])
+        bpw = h0 + h1 if fmt == B.FMT_BF16 else (h0 / 2 if packed4 else h0)
+        layers.append(dict(n_weights=n * (2 if packed4 else 1), counts=counts, h_coded=h0, h_side=h1, bits_per_weight=bpw))
+    model = B.anslin_entropy_weighted([l["bits_per_weight"] for l in layers], [l["n_weights"] for l in layers])
+    return dict(layers=layers, model_bits_per_weight=model)

@@ -393,6 +393,35 @@ def test_autotune_tile_picks_a_supported_geometry():
         dw.close()
 
 
+def test_histogram_and_entropy_study():
+    """S: §8(f) NEXT-4 (P:l.64-78): device histograms are bit-exact against a bincount of the oracle's symbol planes,
+    including a length that is not a multiple of the 16-byte vectors; model entropy = symbol-weighted mean."""
+    rt = _rt()
+    import torch
+    wb = inputs.f32_to_bf16_bits(inputs.weights_f32(1031, 517, seed=111, jitter=True))        # odd element count
+    coded, raw = oc.symbolise(oc.FMT_BF16, wb)
+    f8, _ = inputs.quant_fp8_weights(inputs.weights_f32(640, 1027, seed=112, std=0.015, outliers=False))
+    p4, _, _ = inputs.quant_awq4_weights(inputs.weights_f32(512, 2048, seed=113, outliers=False), 128)
+    tb = torch.from_numpy(wb.view(np.int16)).cuda()
+    st = rt.entropy_study(B.FMT_BF16, [tb, tb[:128].contiguous()])
+    l0 = st["layers"][0]
+    assert np.array_equal(l0["counts"][0], np.bincount(coded.ravel(), minlength=256).astype(np.uint64))
+    assert np.array_equal(l0["counts"][1], np.bincount(raw.ravel(), minlength=256).astype(np.uint64))
+    assert l0["n_weights"] == wb.size and int(l0["counts"][0].sum()) == wb.size
+    _, ost = oc.encode(oc.FMT_BF16, np.ascontiguousarray(wb[:1024, :512]), 512, tile_k=64)
+    sub = rt.entropy_study(B.FMT_BF16, [torch.from_numpy(np.ascontiguousarray(wb[:1024, :512]).view(np.int16)).cuda()])
+    assert sub["layers"][0]["bits_per_weight"] == pytest.approx(ost["h_sym_bits_per_weight"], abs=1e-9)
+    n0, n1 = st["layers"][0]["n_weights"], st["layers"][1]["n_weights"]
+    ref = (n0 * st["layers"][0]["bits_per_weight"] + n1 * st["layers"][1]["bits_per_weight"]) / (n0 + n1)
+    assert st["model_bits_per_weight"] == pytest.approx(ref, abs=1e-12)
+    s8 = rt.entropy_study(B.FMT_FP8_E4M3, [torch.from_numpy(f8).cuda()])["layers"][0]
+    assert np.array_equal(s8["counts"][0], np.bincount(f8.ravel(), minlength=256).astype(np.uint64)) and not s8["counts"][1].any()
+    s4 = rt.entropy_study(B.FMT_INT4_AWQ, [torch.from_numpy(p4).cuda()])["layers"][0]
+    assert np.array_equal(s4["counts"][0], np.bincount(p4.ravel(), minlength=256).astype(np.uint64))
+    assert np.array_equal(s4["counts"][1][:16], np.bincount(og.int4_unpack(p4).ravel(), minlength=16).astype(np.uint64))
+    assert s4["n_weights"] == 2 * p4.size and s4["bits_per_weight"] <= s4["h_side"] + 1e-12     # H(pair)/2 <= H(code)
+
+
 # ------------------------------------------------------------------ full-size launch configuration
 @pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 @pytest.mark.parametrize("name,n,k,m", [("gate", 13824, 5120, 75), ("down", 5120, 13824, 16), ("k", 1024, 5120, 1)])

@@ -89,6 +89,23 @@ def test_cross_decode_and_stats(name, fmt, w, k_in, kw):
     assert total_bits <= 8 * buf.size <= total_bits + st["offset_table_bits"] + st["freq_table_bits"] + 8 * (128 + 5 * 16 + 4096)
 
 
+def test_entropy_functions_closed_forms_and_oracle():
+    """anslin_entropy_bits / anslin_entropy_weighted (P:l.70, l.74): closed forms, and the oracle's own entropy of the
+    same histogram (computed by the oracle's C routine behind container stats)."""
+    assert B.anslin_entropy_bits(np.full(256, 7)) == pytest.approx(8.0, abs=1e-12)
+    assert B.anslin_entropy_bits([5, 5]) == pytest.approx(1.0, abs=1e-12)
+    assert B.anslin_entropy_bits([3, 1]) == pytest.approx(2.0 - 0.75 * np.log2(3.0), abs=1e-12)
+    assert B.anslin_entropy_bits([0, 9, 0]) == 0.0 and B.anslin_entropy_bits(np.zeros(256)) == 0.0
+    assert B.anslin_entropy_weighted([2.0, 4.0], [1, 3]) == pytest.approx(3.5, abs=1e-12)
+    assert B.anslin_entropy_weighted([2.0], [0]) == 0.0
+    w, _ = inputs.config1()
+    _, ost = oc.encode(oc.FMT_BF16, w, 1024, tile_k=64)
+    coded, raw = oc.symbolise(oc.FMT_BF16, w)
+    assert B.anslin_entropy_bits(np.bincount(coded.ravel(), minlength=256)) == pytest.approx(ost["entropy_bits_per_symbol"], abs=1e-9)
+    h = B.anslin_entropy_bits(np.bincount(coded.ravel(), minlength=256)) + B.anslin_entropy_bits(np.bincount(raw.ravel(), minlength=256))
+    assert h == pytest.approx(ost["h_sym_bits_per_weight"], abs=1e-9)
+
+
 def test_config1_gap_through_the_abi():
     """BASELINE target: bits/weight within 0.1 of the empirical entropy on config 1."""
     w, _ = inputs.config1()
