@@ -117,6 +117,28 @@ def test_gemm_bf16(m, flags, tile):
     dw.close()
 
 
+@pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
+@pytest.mark.parametrize("m", [250, 256])
+def test_gemm_bf16_max_batch_and_strided_buffers(m, tile):
+    """Edge cases of the boundary: the largest single-block batch (m = 256, and 250 padded to 256 tensor-core
+    columns), X and Y given as row-strided views (ldx > k_in, ldy > n_out): rows outside the views stay untouched."""
+    rt = _rt()
+    import torch
+    n, k = 384, 1024
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=57, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=58))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile[1], flags=1 | tile[2], tile_n=tile[0])
+    dw = rt.DeviceWeight(buf)
+    xbig = torch.zeros((m, k + 64), dtype=torch.bfloat16, device="cuda")
+    xbig[:, :k] = rt.x_to_device(B.FMT_BF16, x)
+    ybig = torch.full((m, n + 32), -7.0, dtype=torch.float32, device="cuda")
+    dw.gemm(xbig[:, :k], y=ybig[:, :n])
+    y = ybig.cpu().numpy()
+    check_gemm(y[:, :n], *og.gemm_bf16(x, w))
+    assert np.all(y[:, n:] == -7.0)
+    dw.close()
+
+
 @pytest.mark.parametrize("m", [257, 600, 2304])
 def test_gemm_bf16_large_m(m):
     """S: §8(f) NEXT-1 (prefill-sized batches, P:l.392): m > 256 runs as blocks of 256 rows, 8 blocks per launch
