@@ -1079,20 +1079,26 @@ size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_ma
 
 template <uint32_t FMT, int RB, bool PAYLOAD, bool LS>
 int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
-  uint32_t per_sm = 4;
-  if (const char *e = getenv("ANSLIN_DECODE_CTAS_PER_SM")) per_sm = uint32_t(std::max(1, atoi(e)));  // debug knob
   constexpr int J = RB == 1 ? kJ32 : 1;
   const uint32_t jobs = cv.n_tiles / J;
-  const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
   auto kern = decode_kernel<FMT, RB, J, PAYLOAD, LS>;
   const uint32_t stream_bytes = LS ? uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32))) : kStreamSmem;
   const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * (stream_bytes + GlobalEmit<FMT, RB, J>::kStageBytes);
   if (smem > kSmemMax) return ANSLIN_ERR_UNSUPPORTED;
-  static thread_local size_t smem_set = 0;   // per instantiation
+  static thread_local size_t smem_set = 0, smem_occ = 0;   // per instantiation
+  static thread_local int occ = 0;
   if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
     smem_set = smem;
   }
+  if (smem != smem_occ) {
+    // one resident wave: the grid is exactly what fits on the SMs at this shared-memory size, warps loop over jobs
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kDecWarps * 32, smem) != cudaSuccess || occ < 1) return ANSLIN_ERR_CUDA;
+    smem_occ = smem;
+  }
+  uint32_t per_sm = uint32_t(occ);
+  if (const char *e = getenv("ANSLIN_DECODE_CTAS_PER_SM")) per_sm = uint32_t(std::max(1, atoi(e)));  // debug knob
+  const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
   kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out), stream_bytes);
   ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
