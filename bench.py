@@ -249,13 +249,25 @@ def main():
         traffic = json.load(open(tp)).get("fused_gemm_bytes_per_launch_mean")
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned X in, Y out) inside the timed region
+    # Device->host reads of Y run on a copy stream of their own, behind an event per launch group, so that they
+    # overlap the next group's kernel; a group's next launch waits for the previous read of its Y buffers.
+    copy_stream = torch.cuda.Stream()
+    y_ready = [torch.cuda.Event() for _ in groups]
+    y_read = [torch.cuda.Event() for _ in groups]
+
     def step_e2e():
-        for g, call in zip(groups, calls):
+        main = torch.cuda.current_stream()
+        for gi, (g, call) in enumerate(zip(groups, calls)):
             for o in sorted({x_owner[i] for i in g}):
                 xs_dev[o].view(torch.int16).copy_(xs_host[o], non_blocking=True)
+            main.wait_event(y_read[gi])
             call()
-            for i in g:
-                ys_host[i].copy_(ys[i], non_blocking=True)
+            y_ready[gi].record(main)
+            copy_stream.wait_event(y_ready[gi])
+            with torch.cuda.stream(copy_stream):
+                for i in g:
+                    ys_host[i].copy_(ys[i], non_blocking=True)
+                y_read[gi].record(copy_stream)
     for _ in range(3):
         step_e2e()
     barrier()
