@@ -133,6 +133,12 @@ def run_reference(args):
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+# ALU-pipe warp instructions per decoded bf16 symbol in fused_gemm_kernel's hot loop (cuobjdump -sass):
+# table slot 1 (LOP3), entry fields 3 (SHF, LOP3, SHF), state shift 1 (SHF), renormalisation test 1 (ISETP),
+# symbol + raw byte -> bf16 4 per weight pair... = 3 (PRMT 1.5, SHF 1, LOP3 0.5), per-unit bookkeeping ~1.
+ALU_INSTR_PER_SYMBOL = 10.0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -291,6 +297,13 @@ def main():
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                         "traffic": traffic, "peak_kind": "of " + peak_kind,
                         "kernel": "fused_gemm_kernel<bf16,payload> (%d launches/step; bytes = containers + X + Y)" % len(calls)},
+           # the bound that actually binds (SURVEY §8(d) bound 3): the decoder's integer work on the ALU pipe.
+           # peak = SMs x 4 schedulers x 16 lanes/clk (one ALU-pipe warp instruction per 2 clk) x SM clock under load
+           #        / ALU-pipe instructions per decoded symbol in the hot loop's SASS
+           "decoder_bound": (lambda peak: {"bound": "alu", "achieved": n_weights / (ms_step * 1e-3) / 1e9, "peak": peak,
+                                           "unit": "Gsymbol/s", "frac": n_weights / (ms_step * 1e-3) / 1e9 / peak,
+                                           "alu_instr_per_symbol": ALU_INSTR_PER_SYMBOL, "sm_mhz": clocks.get("sm_mhz")})(
+               148 * 4 * 16 * float(clocks.get("sm_mhz") or 1965.0) * 1e6 / ALU_INSTR_PER_SYMBOL / 1e9),
            "compressed_gbs": world * comp_bytes / (ms_step * 1e-3) / 1e9,
            "decoded_weights_gbs": world * n_weights * 2 / (ms_step * 1e-3) / 1e9,
            "bits_per_weight": 8.0 * comp_bytes / n_weights,
