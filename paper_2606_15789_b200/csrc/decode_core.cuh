@@ -181,7 +181,8 @@ __device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint3
 struct LaneStream {
   uint32_t x;          // this lane's rANS state
   uint32_t ptr;        // shared address of this lane's next word
-  uint32_t w;          // last word loaded (kept live so that the predicated load never reads an undefined register)
+  uint32_t w;          // that word, loaded ahead: a renormalisation takes it from the register, then fetches the next
+                       // one, so the shared-memory latency of the word is off the state's dependency chain
   uint32_t goff;       // byte offset, from the record start, of the next segment's words
   const uint8_t *rec;  // record start in HBM
 };
@@ -238,6 +239,9 @@ __device__ __forceinline__ void lane_open_segments(LaneStream (&s)[J], uint32_t 
   }
   cp_async_commit();
   stream_drain();
+  // look-ahead word (a lane without words in this segment reads a neighbour's or stale bytes: never used)
+#pragma unroll
+  for (int j = 0; j < J; ++j) asm volatile("ld.shared.u16 %0, [%1];" : "=r"(s[j].w) : "r"(s[j].ptr) : "memory");
 }
 // One decode step of Alg V.2 for all 32 lanes of one lane-stream tile; dir = +2 (even lanes) / -2 (odd lanes).
 __device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uint32_t dir) {
@@ -249,9 +253,9 @@ __device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uin
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "setp.lt.u32 p, %0, 65536;\n\t"
-      "@p ld.shared.u16 %2, [%1];\n\t"
       "@p mad.lo.u32 %0, %0, 65536, %2;\n\t"
-      "@p add.u32 %1, %1, %3;\n\t}"
+      "@p add.u32 %1, %1, %3;\n\t"
+      "@p ld.shared.u16 %2, [%1];\n\t}"
       : "+r"(xn), "+r"(s.ptr), "+r"(s.w)
       : "r"(dir)
       : "memory");
@@ -260,7 +264,8 @@ __device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uin
 }
 
 // Two lane-stream tiles, one step each, written so that the in-order issue overlaps the two dependent chains: both
-// table loads first, then both state updates, then both predicated word loads, then both merges.
+// table loads first, then both state updates, then both merges with the look-ahead words, then the predicated
+// loads of the next look-ahead words.
 __device__ __forceinline__ void lane_step2(LaneStream &s0, LaneStream &s1, uint32_t tab_s, uint32_t dir, uint32_t &e0, uint32_t &e1) {
   uint32_t a0, a1;
   asm("mul.lo.u32 %0, %1, 4;" : "=r"(a0) : "r"(s0.x));
@@ -275,12 +280,12 @@ __device__ __forceinline__ void lane_step2(LaneStream &s0, LaneStream &s1, uint3
       "{\n\t.reg .pred p, q;\n\t"
       "setp.lt.u32 p, %0, 65536;\n\t"
       "setp.lt.u32 q, %3, 65536;\n\t"
-      "@p ld.shared.u16 %2, [%1];\n\t"
-      "@q ld.shared.u16 %5, [%4];\n\t"
       "@p mad.lo.u32 %0, %0, 65536, %2;\n\t"
       "@q mad.lo.u32 %3, %3, 65536, %5;\n\t"
       "@p add.u32 %1, %1, %6;\n\t"
-      "@q add.u32 %4, %4, %6;\n\t}"
+      "@q add.u32 %4, %4, %6;\n\t"
+      "@p ld.shared.u16 %2, [%1];\n\t"
+      "@q ld.shared.u16 %5, [%4];\n\t}"
       : "+r"(x0), "+r"(s0.ptr), "+r"(s0.w), "+r"(x1), "+r"(s1.ptr), "+r"(s1.w)
       : "r"(dir)
       : "memory");

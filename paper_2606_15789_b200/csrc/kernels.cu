@@ -1083,7 +1083,8 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   const uint32_t jobs = cv.n_tiles / J;
   auto kern = decode_kernel<FMT, RB, J, PAYLOAD, LS>;
   const uint32_t stream_bytes = LS ? uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32))) : kStreamSmem;
-  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * (stream_bytes + GlobalEmit<FMT, RB, J>::kStageBytes);
+  // + 16: a lane-stream's look-ahead word load may touch the two bytes after the last stream buffer
+  const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * (stream_bytes + GlobalEmit<FMT, RB, J>::kStageBytes) + 16;
   if (smem > kSmemMax) return ANSLIN_ERR_UNSUPPORTED;
   static thread_local size_t smem_set = 0, smem_occ = 0;   // per instantiation
   static thread_local int occ = 0;
