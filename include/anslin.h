@@ -210,6 +210,26 @@ double anslin_entropy_bits(const uint64_t *counts_host, int32_t bins);
 /* Symbol-weighted model entropy (P:l.74): sum_l n[l] * h[l] / sum_l n[l]; 0 if all n are 0. */
 double anslin_entropy_weighted(const double *h, const uint64_t *n, int32_t layers);
 
+/*
+ * GPU-side encoder (S: NEXT-6; the paper names it as future work, P:l.486): compress a row-major W that is resident
+ * in HBM into a container in HBM.  Same symbolisation, table normalisation, container layout and decoders as
+ * anslin_encode_host; restricted to the lane-stream layout (desc.tile_n = 32, ANSLIN_FLAG_LANE_STREAMS set, tile_k a
+ * multiple of 256 decode steps: 256 weights for bf16 / fp8 / int8, 512 for int4 / fp4).  An offline-stage call like
+ * anslin_encode_host: it SYNCHRONISES `stream` (the 256-bin histogram and the per-tile record sizes visit the host
+ * for the table normalisation and the offset prefix sum; W itself never leaves the device).
+ *   w_dev: row-major W as anslin_encode_host takes it, 16-byte aligned.  scales_host / zeros_host: as anslin_encode_host.
+ *   container_dev: >= anslin_encode_bound(desc) bytes.  head_host: >= anslin_encode_device_head_bytes(desc) bytes; receives
+ *   the header, frequency table and record offsets — what anslin_open needs as `container_host`.
+ *   workspace_dev: >= anslin_encode_device_workspace_bytes(desc) bytes.  *bytes_out = container size.
+ * ANSLIN_ERR_UNSUPPORTED if the geometry is not the one above or a tile does not fit the lane-stream segment tables
+ * (anslin_encode_host falls back to interleaved words in that case; this call does not).
+ */
+size_t anslin_encode_device_workspace_bytes(const anslin_desc *desc);
+size_t anslin_encode_device_head_bytes(const anslin_desc *desc);
+int anslin_encode_device(const anslin_desc *desc, const void *w_dev, const void *scales_host, const void *zeros_host,
+                         void *container_dev, size_t capacity, void *head_host, size_t head_capacity,
+                         void *workspace_dev, size_t workspace_bytes, size_t *bytes_out, void *stream);
+
 /* Number of kernels the last device call on this thread enqueued (for bench.py's gpu_launches). */
 int anslin_last_launch_count(void);
 

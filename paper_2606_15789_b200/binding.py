@@ -24,7 +24,8 @@ EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_c
            "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm_multi_workspace_bytes", "anslin_gemm",
            "anslin_gemm_multi", "anslin_gemm_grouped",
            "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_histogram", "anslin_entropy_bits",
-           "anslin_entropy_weighted", "anslin_last_launch_count", "anslin_status_string"]
+           "anslin_entropy_weighted", "anslin_encode_device_workspace_bytes", "anslin_encode_device_head_bytes",
+           "anslin_encode_device", "anslin_last_launch_count", "anslin_status_string"]
 
 
 class AnslinError(RuntimeError):
@@ -76,6 +77,9 @@ def lib() -> ctypes.CDLL:
         L.anslin_entropy_bits.argtypes = [ctypes.POINTER(ctypes.c_uint64), i32]; L.anslin_entropy_bits.restype = ctypes.c_double
         L.anslin_entropy_weighted.argtypes = [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_uint64), i32]
         L.anslin_entropy_weighted.restype = ctypes.c_double
+        L.anslin_encode_device_workspace_bytes.argtypes = [ctypes.POINTER(Desc)]; L.anslin_encode_device_workspace_bytes.restype = sz
+        L.anslin_encode_device_head_bytes.argtypes = [ctypes.POINTER(Desc)]; L.anslin_encode_device_head_bytes.restype = sz
+        L.anslin_encode_device.argtypes = [ctypes.POINTER(Desc), vp, vp, vp, vp, sz, vp, sz, vp, sz, ctypes.POINTER(sz), vp]
         L.anslin_last_launch_count.restype = ctypes.c_int
         L.anslin_status_string.argtypes = [ctypes.c_int]; L.anslin_status_string.restype = ctypes.c_char_p
         _lib = L
@@ -108,6 +112,36 @@ def anslin_encode_host(fmt: int, w: np.ndarray, n_out: int, k_in: int, tile_k: i
     _check(lib().anslin_encode_host(ctypes.byref(d), _hp(w), _hp(scales), _hp(zeros), _hp(out), cap, ctypes.byref(n),
                                     ctypes.byref(st)), "anslin_encode_host")
     return out[:n.value].copy(), st.as_dict()
+
+
+def anslin_encode_device(fmt: int, w_ptr: int, n_out: int, k_in: int, container_ptr: int, capacity: int, ws_ptr: int, ws_bytes: int,
+                         tile_k: int = 256, flags: int = FLAG_LANE_STREAMS, scales: np.ndarray | None = None,
+                         zeros: np.ndarray | None = None, group_size: int = 0, w_scale: float = 1.0, stream: int = 0):
+    """GPU-side encoder: W at w_ptr (device) -> container at container_ptr (device).  Returns (head bytes as np.uint8
+    array = what Weight() needs as container_host, container size in bytes)."""
+    d = Desc(fmt, n_out, k_in, tile_k, group_size, flags, w_scale, 32)
+    hb = int(lib().anslin_encode_device_head_bytes(ctypes.byref(d)))
+    if hb == 0:
+        raise AnslinError("anslin_encode_device: unsupported geometry (lane streams, 32-row tiles, 256-step segments)")
+    scales = None if scales is None else np.ascontiguousarray(scales, dtype=np.float16)
+    zeros = None if zeros is None else np.ascontiguousarray(zeros, dtype=np.float16)
+    head = np.zeros(hb, dtype=np.uint8)
+    n = ctypes.c_size_t(0)
+    _check(lib().anslin_encode_device(ctypes.byref(d), ctypes.c_void_p(w_ptr), _hp(scales), _hp(zeros), ctypes.c_void_p(container_ptr),
+                                      capacity, _hp(head), hb, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.byref(n), ctypes.c_void_p(stream)),
+           "anslin_encode_device")
+    return head, int(n.value)
+
+
+def anslin_encode_bound(fmt: int, n_out: int, k_in: int, tile_k: int = 0, flags: int = 0, group_size: int = 0, tile_n: int = 0) -> int:
+    d = Desc(fmt, n_out, k_in, tile_k, group_size, flags, 1.0, tile_n)
+    return int(lib().anslin_encode_bound(ctypes.byref(d)))
+
+
+def anslin_encode_device_workspace_bytes(fmt: int, n_out: int, k_in: int, tile_k: int = 256, flags: int = FLAG_LANE_STREAMS,
+                                         group_size: int = 0) -> int:
+    d = Desc(fmt, n_out, k_in, tile_k, group_size, flags, 1.0, 32)
+    return int(lib().anslin_encode_device_workspace_bytes(ctypes.byref(d)))
 
 
 class Weight:

@@ -213,6 +213,11 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
 
 }  // namespace
 
+namespace anslin {
+// the encoder's table normalisation, shared with the device-side encoder (encode_gpu.cu)
+bool normalise_freqs(const uint64_t *cnt, uint32_t *f) { return normalise(cnt, f); }
+}  // namespace anslin
+
 extern "C" {
 
 size_t anslin_encode_bound(const anslin_desc *desc) {

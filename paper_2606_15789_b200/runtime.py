@@ -70,6 +70,30 @@ class DeviceWeight:
         return y
 
 
+def encode_on_device(fmt: int, w: torch.Tensor, n_out: int, k_in: int, tile_k: int = 256, flags: int = B.FLAG_LANE_STREAMS,
+                     scales: np.ndarray | None = None, zeros: np.ndarray | None = None, group_size: int = 0,
+                     w_scale: float = 1.0) -> "DeviceWeight":
+    """anslin_encode_device: compress a cuda tensor W (stored elements, row-major) without moving it to the host.
+    Returns a DeviceWeight whose container lives in a device buffer trimmed to the container size."""
+    cap = B.anslin_encode_bound(fmt, n_out, k_in, tile_k, flags, group_size, 32)
+    need = B.anslin_encode_device_workspace_bytes(fmt, n_out, k_in, tile_k, flags, group_size)
+    if cap == 0 or need == 0:
+        raise B.AnslinError("encode_on_device: unsupported geometry")
+    w = w.contiguous()
+    out = torch.empty(cap, dtype=torch.uint8, device=w.device)
+    ws = torch.empty(need, dtype=torch.uint8, device=w.device)
+    head, n = B.anslin_encode_device(fmt, w.data_ptr(), n_out, k_in, out.data_ptr(), cap, ws.data_ptr(), need, tile_k=tile_k,
+                                     flags=flags, scales=scales, zeros=zeros, group_size=group_size, w_scale=w_scale, stream=_stream())
+    dw = DeviceWeight.__new__(DeviceWeight)
+    dw.container_host = head
+    dw.container_dev = out[:n]
+    dw.weight = B.Weight(head, out.data_ptr())
+    d = dw.weight.desc
+    dw.fmt, dw.n_out, dw.k_in = d.format, d.n_out, d.k_in
+    dw._ws = None
+    return dw
+
+
 class MultiGemm:
     """anslin_gemm_multi over weights that share format and tile geometry: ONE persistent launch for
     e.g. q/k/v (same X) or gate/up.  Buffers and the marshalled call are built once."""

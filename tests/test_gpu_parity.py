@@ -444,6 +444,54 @@ def test_histogram_and_entropy_study():
     assert s4["n_weights"] == 2 * p4.size and s4["bits_per_weight"] <= s4["h_side"] + 1e-12     # H(pair)/2 <= H(code)
 
 
+def _device_encode_cases():
+    wf = inputs.weights_f32(384, 1024, seed=121, jitter=True)
+    yield "bf16-payload", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 1024, dict(tile_k=256, flags=3)
+    yield "bf16-t512", B.FMT_BF16, inputs.f32_to_bf16_bits(wf), 1024, dict(tile_k=512, flags=2)
+    q8, s8 = inputs.quant_sq8_weights(wf)
+    yield "int8", B.FMT_INT8, q8, 1024, dict(tile_k=512, flags=2, scales=s8)
+    f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(256, 1024, seed=122, std=0.015, outliers=False))
+    yield "fp8-t1024", B.FMT_FP8_E4M3, f8, 1024, dict(tile_k=1024, flags=2, w_scale=sc)
+    p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(256, 1024, seed=123, outliers=False), 128)
+    yield "int4", B.FMT_INT4_AWQ, p4, 1024, dict(tile_k=512, flags=2, scales=s4, zeros=z4, group_size=128)
+    yield "bf16-constant", B.FMT_BF16, np.full((128, 256), 0xBF80, dtype=np.uint16), 256, dict(tile_k=256, flags=3)
+
+
+@pytest.mark.parametrize("name,fmt,w,k_in,kw", list(_device_encode_cases()), ids=[c[0] for c in _device_encode_cases()])
+def test_encode_on_device(name, fmt, w, k_in, kw):
+    """S: §8(f) NEXT-6 GPU-side encoder: the container it writes is decoded bit-exactly by the ORACLE and by
+    anslin_decode, has the host encoder's table and (same table, same rANS arithmetic) the host encoder's size."""
+    rt = _rt()
+    import torch
+    n_out = w.shape[0]
+    wd = torch.from_numpy(np.ascontiguousarray(w).view(np.uint8).reshape(n_out, -1)).cuda()
+    dw = rt.encode_on_device(fmt, wd, n_out, k_in, **kw)
+    buf = dw.container_dev.cpu().numpy()
+    h, w2, side = oc.decode(buf)
+    assert np.array_equal(w2.view(np.uint8), np.ascontiguousarray(w).view(np.uint8))
+    assert (h.tile_n, h.tile_k, h.flags) == (32, kw["tile_k"], kw["flags"])
+    if "scales" in kw:
+        assert np.array_equal(side["scales"], kw["scales"])
+    assert np.array_equal(dw.decode().cpu().numpy().view(np.uint8).reshape(n_out, -1), np.ascontiguousarray(w).view(np.uint8).reshape(n_out, -1))
+    hbuf, _ = B.anslin_encode_host(fmt, w, n_out, k_in, tile_n=32, **kw)
+    assert buf.size == hbuf.size and np.array_equal(buf[:h.off_records], hbuf[:h.off_records])
+    assert np.array_equal(buf, hbuf), "same table, same arithmetic, same layout: the two encoders agree byte for byte"
+    dw.close()
+
+
+def test_encode_on_device_then_gemm():
+    rt = _rt()
+    import torch
+    n, k, m = 640, 1024, 20
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=124, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=125))
+    dw = rt.encode_on_device(B.FMT_BF16, torch.from_numpy(w.view(np.int16)).cuda(), n, k, tile_k=256, flags=3)
+    check_gemm(dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy(), *og.gemm_bf16(x, w))
+    with pytest.raises(B.AnslinError):
+        rt.encode_on_device(B.FMT_BF16, torch.from_numpy(w.view(np.int16)).cuda(), n, k, tile_k=64, flags=2)   # 64 steps: no whole segment
+    dw.close()
+
+
 # ------------------------------------------------------------------ full-size launch configuration
 @pytest.mark.parametrize("tile", TILES, ids=TILE_IDS)
 @pytest.mark.parametrize("name,n,k,m", [("gate", 13824, 5120, 75), ("down", 5120, 13824, 16), ("k", 1024, 5120, 1)])
