@@ -150,6 +150,9 @@ def main():
     ap.add_argument("--tile", default="32x256", help="tile_n x tile_k of the compressed containers (128x64 = BASELINE config 1's shape)")
     ap.add_argument("--layout", default="lanes", choices=["lanes", "interleaved"], help="word layout of the containers: every lane "
                     "its own stream (32-row tiles only) or words interleaved in read order")
+    ap.add_argument("--symbols", default="paper", choices=["paper", "pair4"], help="paper = one coded symbol per weight (PAPER.md's "
+                    "symbolisation, the headline); pair4 = the variant that codes two K-adjacent bf16 exponents per symbol "
+                    "(SURVEY 8(f) NEXT-5, ANSLIN_FMT_BF16_PAIR4; lanes layout only)")
     ap.add_argument("--group", default="qkv,o,gateup,down", help="launch grouping of the 7 projections: 'each' = 7 launches, or "
                     "comma-separated groups out of qkv / q,k,v / gateup / gate,up / o / down (projections that share an input)")
     args = ap.parse_args()
@@ -173,7 +176,8 @@ def main():
     tile_n, tile_k = (int(v) for v in args.tile.split("x"))
     for (_, n, k, w) in layer:
         lflag = B.FLAG_LANE_STREAMS if (args.layout == "lanes" and tile_n == 32) else 0
-        buf, st = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=tile_k, flags=B.FLAG_STATE_PAYLOAD | lflag, tile_n=tile_n)
+        buf, st = B.anslin_encode_host(B.FMT_BF16_PAIR4 if args.symbols == "pair4" else B.FMT_BF16, w, n, k, tile_k=tile_k,
+                                       flags=B.FLAG_STATE_PAYLOAD | lflag, tile_n=tile_n)
         containers.append(buf); stats.append(st)
     dws = [rt.DeviceWeight(c) for c in containers]
     m = args.m
@@ -289,7 +293,7 @@ def main():
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
            "data": "synthetic",
-           "config": {"workload": WORKLOAD, "batch_m": m, "tile": args.tile, "word_layout": args.layout, "streams": 32, "prob_bits": 12,
+           "config": {"workload": WORKLOAD, "batch_m": m, "tile": args.tile, "word_layout": args.layout, "symbols": args.symbols, "streams": 32, "prob_bits": 12,
                       "launch_groups": group_names,
                       "l2_policy": "inputs larger than L2: %.0f MB of compressed weights stream per step" % (comp_bytes / 1e6),
                       "parallelism": "replicas, one batch per GPU" if world > 1 else "1 GPU"},

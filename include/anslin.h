@@ -52,9 +52,14 @@ typedef enum {
                               scales_host/zeros_host = fp16[n_out][k_in/group_size]; w = (q - z) * s.
                               Plain per-channel int4 is this format with group_size = k_in (symmetric: z = 8) */
   ANSLIN_FMT_FP8_E5M2 = 4, /* w_host: OCP e5m2 bytes (P:l.80 "FP8-E5M2"); otherwise as FP8_E4M3 */
-  ANSLIN_FMT_FP4_E2M1 = 5  /* w_host: uint8[n_out][k_in/2], low nibble = even k, OCP e2m1 codes s.ee.m (P:l.80 "FP4-E2M1");
+  ANSLIN_FMT_FP4_E2M1 = 5, /* w_host: uint8[n_out][k_in/2], low nibble = even k, OCP e2m1 codes s.ee.m (P:l.80 "FP4-E2M1");
                               coded symbol = packed byte; per-tensor scale in desc.w_scale.  Every code is expanded
                               exactly to e4m3 for the tensor core; X is fp8 (either kind) with per-token scales */
+  ANSLIN_FMT_BF16_PAIR4 = 6 /* VARIANT of BF16 (S: NEXT-5), not the paper's symbolisation: the 15 most frequent exponent
+                              bytes get 4-bit codes, code 15 = escape; coded symbol = the codes of two K-adjacent
+                              weights, so one rANS step decodes two weights.  An escaped exponent follows as a literal
+                              16-bit word in the lane's own stream.  Raw plane, payload flag, X and Y as BF16.
+                              Lane-stream layout on 32-row tiles only (segments of 128 steps) */
 } anslin_format;
 
 /* Element type of X. */

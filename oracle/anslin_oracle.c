@@ -272,3 +272,68 @@ size_t orc_tile_encode_by_simulation(const uint8_t *sym, size_t n, int R, const 
     free(q); free(qn); free(qr); free(x); free(lane_sym);
     return nw;
 }
+
+/*
+ * Lane stream with in-stream literals: a coded symbol holds two
+ * 4-bit codes (low nibble = first weight); code 15 is an escape whose true value follows in the lane's own word
+ * stream.  Steps come in chunks of four (eight weights = one 16-byte bf16 operand chunk): the decoder decodes and
+ * renormalises the four steps (0 or 1 word each), then reads one literal word per escaped nibble of the chunk, in
+ * weight order (step by step, low nibble first).  lit[] holds all literals consecutively in weight order.  n % 4 == 0.
+ * words_dec receives the stream in decoder read order; after_step[i] = words consumed once step i is complete
+ * (so a caller can cut the stream into segments of steps).  Returns the total number of words.
+ */
+size_t orc_encode_scalar_lit(const uint8_t *sym, size_t n, const uint32_t *f, const uint32_t *c,
+                             int b, int w, int Llog2, uint64_t x_init, const uint16_t *lit,
+                             uint64_t *state_out, uint16_t *words_dec, uint32_t *after_step)
+{
+    /* plain rANS first: emitted[i] = words the encoder put out BEFORE coding symbol i = what the decoder's
+     * renormalisation after step i reads */
+    uint16_t *emit = (uint16_t *)malloc((n * 2 + 8) * sizeof(uint16_t));
+    uint32_t *first = (uint32_t *)malloc((n + 1) * sizeof(uint32_t));   /* emission index range of step i: [first[i+1].. first[i]) in emission order */
+    size_t nw = 0;
+    uint64_t x = x_init;
+    for (size_t i = n; i-- > 0;) {
+        first[i + 1] = (uint32_t)nw;   /* emissions so far belong to later steps */
+        x = enc_step(x, f[sym[i]], c[sym[i]], b, w, Llog2, emit, &nw);
+    }
+    first[0] = (uint32_t)nw;
+    /* emissions of step i (made while coding symbol i) occupy emission indices [first[i+1], first[i]) */
+    size_t out = 0, li = 0;
+    for (size_t i = 0; i < n; ++i) {
+        for (uint32_t k = first[i]; k-- > first[i + 1];) words_dec[out++] = emit[k];   /* decoder reads them in reverse emission order */
+        if ((i & 3) == 3)
+            for (size_t j = i - 3; j <= i; ++j) {
+                if ((sym[j] & 15) == 15) words_dec[out++] = lit[li++];
+                if ((sym[j] >> 4) == 15) words_dec[out++] = lit[li++];
+            }
+        after_step[i] = (uint32_t)out;
+    }
+    free(emit); free(first);
+    *state_out = x;
+    return out;
+}
+
+/* Inverse of orc_encode_scalar_lit.  out_lit[2i], out_lit[2i+1]: the literal of step i's low / high nibble, or 0xFFFF
+ * when that nibble is not an escape.  Returns the number of words consumed. */
+size_t orc_decode_scalar_lit(uint64_t state, const uint16_t *words, size_t n,
+                             const uint32_t *f, const uint32_t *c, const uint8_t *sym_of_slot,
+                             int b, int w, int Llog2, uint8_t *out, uint16_t *out_lit, uint64_t *state_end)
+{
+    const uint64_t M = 1ull << b, L = 1ull << Llog2;
+    uint64_t x = state;
+    size_t r = 0;
+    for (size_t i = 0; i < n; ++i) {
+        uint64_t slot = x & (M - 1);
+        uint8_t s = sym_of_slot[slot];
+        out[i] = s;
+        x = (uint64_t)f[s] * (x >> b) + (slot - c[s]);
+        while (x < L) x = (x << w) | words[r++];
+        if ((i & 3) == 3)
+            for (size_t j = i - 3; j <= i; ++j) {
+                out_lit[2 * j] = (out[j] & 15) == 15 ? words[r++] : 0xFFFF;
+                out_lit[2 * j + 1] = (out[j] >> 4) == 15 ? words[r++] : 0xFFFF;
+            }
+    }
+    *state_end = x;
+    return r;
+}

@@ -43,6 +43,8 @@ def lib() -> ctypes.CDLL:
         L.orc_encode_scalar.argtypes = [u8p, sz, u32p, u32p, ci, ci, ci, u64, u64p, u16p]; L.orc_encode_scalar.restype = sz
         L.orc_decode_scalar.argtypes = [u64, u16p, sz, u32p, u32p, u8p, ci, ci, ci, u8p, u64p]; L.orc_decode_scalar.restype = sz
         L.orc_tile_encode.argtypes = [u8p, sz, ci, u32p, u32p, ci, ci, ci, u64p, u64p, u16p]; L.orc_tile_encode.restype = sz
+        L.orc_encode_scalar_lit.argtypes = [u8p, sz, u32p, u32p, ci, ci, ci, u64, u16p, u64p, u16p, u32p]; L.orc_encode_scalar_lit.restype = sz
+        L.orc_decode_scalar_lit.argtypes = [u64, u16p, sz, u32p, u32p, u8p, ci, ci, ci, u8p, u16p, u64p]; L.orc_decode_scalar_lit.restype = sz
         L.orc_tile_decode.argtypes = [u64p, u16p, sz, ci, u32p, u32p, u8p, ci, ci, ci, u8p, u64p]; L.orc_tile_decode.restype = sz
         L.orc_tile_encode_by_simulation.argtypes = [u8p, sz, ci, u32p, u32p, u8p, ci, ci, ci, u64p, u64p, u16p]
         L.orc_tile_encode_by_simulation.restype = sz
@@ -124,6 +126,32 @@ def decode_scalar(state: int, words, n: int, tab: Table, w: int, Llog2: int):
     used = lib().orc_decode_scalar(state, _p(words, ctypes.c_uint16), n, _p(tab.f, ctypes.c_uint32), _p(tab.c, ctypes.c_uint32),
                                    _p(tab.slots, ctypes.c_uint8), tab.b, w, Llog2, _p(out, ctypes.c_uint8), ctypes.byref(end))
     return out, int(end.value), int(used)
+
+
+def encode_scalar_lit(sym, tab: Table, w: int, Llog2: int, x_init: int, lit):
+    """Scalar stream whose symbols are pairs of 4-bit codes; code 15 = escape with an in-stream literal word
+    (see orc_encode_scalar_lit).  Returns (start state, words in read order, words consumed after each step)."""
+    sym = np.ascontiguousarray(sym, dtype=np.uint8)
+    lit = np.ascontiguousarray(np.concatenate([np.asarray(lit, dtype=np.uint16), np.zeros(1, np.uint16)]))
+    words = np.zeros(sym.size * 4 + 8, dtype=np.uint16)
+    after = np.zeros(sym.size, dtype=np.uint32)
+    st = ctypes.c_uint64(0)
+    n = lib().orc_encode_scalar_lit(_p(sym, ctypes.c_uint8), sym.size, _p(tab.f, ctypes.c_uint32), _p(tab.c, ctypes.c_uint32),
+                                    tab.b, w, Llog2, x_init, _p(lit, ctypes.c_uint16), ctypes.byref(st), _p(words, ctypes.c_uint16),
+                                    _p(after, ctypes.c_uint32))
+    return int(st.value), words[:n].copy(), after
+
+
+def decode_scalar_lit(state: int, words, n: int, tab: Table, w: int, Llog2: int):
+    """Returns (symbols, literal per nibble [2n] with 0xFFFF = none, end state, words consumed)."""
+    words = np.ascontiguousarray(np.concatenate([np.asarray(words, dtype=np.uint16), np.zeros(4, np.uint16)]))
+    out = np.zeros(n, dtype=np.uint8)
+    lit = np.zeros(2 * n, dtype=np.uint16)
+    end = ctypes.c_uint64(0)
+    used = lib().orc_decode_scalar_lit(state, _p(words, ctypes.c_uint16), n, _p(tab.f, ctypes.c_uint32), _p(tab.c, ctypes.c_uint32),
+                                       _p(tab.slots, ctypes.c_uint8), tab.b, w, Llog2, _p(out, ctypes.c_uint8), _p(lit, ctypes.c_uint16),
+                                       ctypes.byref(end))
+    return out, lit, int(end.value), int(used)
 
 
 def tile_encode(sym, R: int, tab: Table, w: int, Llog2: int, x_init, by_simulation: bool = False):

@@ -21,7 +21,7 @@ from . import codec
 
 MAGIC = 0x4C534E41  # "ANSL"
 VERSION = 1
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1 = 0, 1, 2, 3, 4, 5
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1, FMT_BF16_PAIR4 = 0, 1, 2, 3, 4, 5, 6
 FLAG_STATE_PAYLOAD = 1
 FLAG_LANE_STREAMS = 2   # each lane's words stored as its own stream (tile_n = 32 only), see _lane_record
 SEG_STEPS = 256         # lane-stream records are cut into segments of this many decode steps
@@ -35,9 +35,15 @@ HEADER_BYTES = 128
 TAIL_BYTES = 4096      # readable bytes that must follow the records section
 
 # symbols per 16-byte operand chunk, and default tile_k (in weights) per format
-SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4, FMT_FP8_E5M2: 16, FMT_FP4_E2M1: 8}
-DEFAULT_TILE_K = {FMT_BF16: 64, FMT_FP8_E4M3: 256, FMT_INT8: 256, FMT_INT4_AWQ: 256, FMT_FP8_E5M2: 256, FMT_FP4_E2M1: 256}
-WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2, FMT_FP8_E5M2: 1, FMT_FP4_E2M1: 2}
+SPC = {FMT_BF16: 8, FMT_FP8_E4M3: 16, FMT_INT8: 16, FMT_INT4_AWQ: 4, FMT_FP8_E5M2: 16, FMT_FP4_E2M1: 8, FMT_BF16_PAIR4: 4}
+DEFAULT_TILE_K = {FMT_BF16: 64, FMT_FP8_E4M3: 256, FMT_INT8: 256, FMT_INT4_AWQ: 256, FMT_FP8_E5M2: 256, FMT_FP4_E2M1: 256, FMT_BF16_PAIR4: 256}
+WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2, FMT_FP8_E5M2: 1, FMT_FP4_E2M1: 2, FMT_BF16_PAIR4: 2}
+
+
+def seg_steps(fmt: int) -> int:
+    """Decode steps per lane-stream segment: 8192 weights of a 32-row tile in every format that codes one symbol per
+    weight (256 steps); the bf16 pair variant decodes two weights per step (128 steps)."""
+    return SEG_STEPS // 2 if fmt == FMT_BF16_PAIR4 else SEG_STEPS
 
 
 def _align(x: int, a: int = 16) -> int:
@@ -61,6 +67,27 @@ def symbolise(fmt: int, w: np.ndarray):
         raw = (((w & 0x7F) << 1) | (w >> 15)).astype(np.uint8)
         return coded, raw
     return np.ascontiguousarray(w).view(np.uint8), None
+
+
+def pair_code_table(exps: np.ndarray) -> np.ndarray:
+    """bf16 pair variant (S: 8(f) NEXT-5): the 15 most frequent exponent bytes get the 4-bit codes 0..14 (descending
+    count, ties by smaller exponent); code 15 is the escape.  Returns uint8[16], entry 15 = 0."""
+    cnt = np.bincount(exps.ravel(), minlength=256)
+    order = sorted(range(256), key=lambda v: (-int(cnt[v]), v))[:15]
+    return np.array(order + [0], dtype=np.uint8)
+
+
+def symbolise_pair(w: np.ndarray, table: np.ndarray | None = None):
+    """bf16 -> (coded pairs uint8 [n x k/2] = code(even k) | code(odd k) << 4, raw plane uint8 [n x k] as for bf16,
+    exponent bytes uint8 [n x k], code table uint8[16])."""
+    w = np.ascontiguousarray(w).view(np.uint16)
+    exps = ((w >> 7) & 0xFF).astype(np.uint8)
+    raw = (((w & 0x7F) << 1) | (w >> 15)).astype(np.uint8)
+    table = pair_code_table(exps) if table is None else table
+    code_of = np.full(256, 15, dtype=np.uint8)
+    code_of[table[:15]] = np.arange(15, dtype=np.uint8)
+    codes = code_of[exps]
+    return (codes[:, 0::2] | (codes[:, 1::2] << 4)).astype(np.uint8), raw, exps, table
 
 
 def desymbolise(fmt: int, coded: np.ndarray, raw):
@@ -179,7 +206,7 @@ def _raw_tile_unpack(plane: np.ndarray, steps: int, flags: int, payload):
     return vec.transpose(0, 2, 1).reshape(steps, LANES)
 
 
-def _lane_record(sym_tile: np.ndarray, tab, x_init):
+def _lane_record(sym_tile: np.ndarray, tab, x_init, seg: int = SEG_STEPS, lits=None):
     """Lane-stream record of one tile (FLAG_LANE_STREAMS).  sym_tile: uint8 [steps x 32] in tile order.
 
     Every lane is an ordinary scalar rANS stream (P:l.192 "each warp lane maintains its own rANS state"); instead
@@ -192,17 +219,27 @@ def _lane_record(sym_tile: np.ndarray, tab, x_init):
              [segment 0 regions 0..15][segment 1 ...] zero-padded to 16 bytes.
     Returns (record bytes, number of payload words, staged bytes of the largest segment)."""
     steps = sym_tile.shape[0]
-    assert steps % SEG_STEPS == 0, "lane-stream tiles must have a multiple of %d steps" % SEG_STEPS
-    S = steps // SEG_STEPS
+    assert steps % seg == 0, "lane-stream tiles must have a multiple of %d steps" % seg
+    S = steps // seg
     states = np.zeros(LANES, dtype=np.uint64)
     seg_words = [[None] * LANES for _ in range(S)]
     for lane in range(LANES):
         col = np.ascontiguousarray(sym_tile[:, lane])
+        if lits is not None:   # pair variant: escape literals ride in the lane's stream (codec.encode_scalar_lit)
+            st, words, after = codec.encode_scalar_lit(col, tab, WORD_BITS, STATE_LO_LOG2, int(x_init[lane]), lits[lane])
+            states[lane] = st
+            used_prev = 0
+            for sg in range(S):
+                used = int(after[(sg + 1) * seg - 1])
+                seg_words[sg][lane] = words[used_prev:used]
+                used_prev = used
+            assert used_prev == words.size
+            continue
         st, words = codec.encode_scalar(col, tab, WORD_BITS, STATE_LO_LOG2, int(x_init[lane]))
         states[lane] = st
         used_prev = 0
-        for sg in range(S):   # words the decoder has consumed after (sg+1)*SEG_STEPS steps
-            _, _, used = codec.decode_scalar(st, words, (sg + 1) * SEG_STEPS, tab, WORD_BITS, STATE_LO_LOG2)
+        for sg in range(S):   # words the decoder has consumed after (sg+1)*seg steps
+            _, _, used = codec.decode_scalar(st, words, (sg + 1) * seg, tab, WORD_BITS, STATE_LO_LOG2)
             seg_words[sg][lane] = words[used_prev:used]
             used_prev = used
         assert used_prev == words.size
@@ -221,9 +258,10 @@ def _lane_record(sym_tile: np.ndarray, tab, x_init):
     return rec + b"\0" * (_align(len(rec)) - len(rec)), n_words, max_seg
 
 
-def _lane_record_decode(rec: np.ndarray, steps: int, tab):
-    """Inverse of _lane_record: returns (symbols uint8 [steps x 32], end states[32])."""
-    S = steps // SEG_STEPS
+def _lane_record_decode(rec: np.ndarray, steps: int, tab, seg: int = SEG_STEPS, pair: bool = False):
+    """Inverse of _lane_record: returns (symbols uint8 [steps x 32], end states[32]) and, for the pair variant,
+    the literal of every nibble (uint16 [2*steps x 32], 0xFFFF = not an escape)."""
+    S = steps // seg
     states = np.frombuffer(rec[:4 * LANES].tobytes(), dtype="<u4").astype(np.uint64)
     pos = 4 * LANES + 20 * S
     lanes = [[] for _ in range(LANES)]
@@ -240,19 +278,26 @@ def _lane_record_decode(rec: np.ndarray, steps: int, tab):
             pos += 2 * n
     sym = np.zeros((steps, LANES), dtype=np.uint8)
     end = np.zeros(LANES, dtype=np.uint64)
+    lit = np.full((2 * steps, LANES), 0xFFFF, dtype=np.uint16)
     # the split of a region between its two lanes is not stored: lane 2p decodes ascending, lane 2p+1 descending,
-    # each taking exactly the words its own renormalisations ask for
+    # each taking exactly the words its own renormalisations (and escapes) ask for
     for lane in range(LANES):
         x = int(states[lane])
-        out = []
+        out, lo = [], []
         for sg in range(S):
             region, d = lanes[lane][sg]
             words = region if d > 0 else region[::-1]
-            o, x, _ = codec.decode_scalar(x, words, SEG_STEPS, tab, WORD_BITS, STATE_LO_LOG2)
+            if pair:
+                o, l, x, _ = codec.decode_scalar_lit(x, words, seg, tab, WORD_BITS, STATE_LO_LOG2)
+                lo.append(l)
+            else:
+                o, x, _ = codec.decode_scalar(x, words, seg, tab, WORD_BITS, STATE_LO_LOG2)
             out.append(o)
         sym[:, lane] = np.concatenate(out)
+        if pair:
+            lit[:, lane] = np.concatenate(lo)
         end[lane] = x
-    return sym, end
+    return (sym, end, lit) if pair else (sym, end)
 
 
 def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
@@ -264,11 +309,16 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     scales/zeros: int8 -> fp16 [n_out]; int4 -> fp16 [n_out x k_in/group] each.
     """
     tile_k = tile_k or DEFAULT_TILE_K[fmt]
-    coded, raw = symbolise(fmt, w)
+    pair = fmt == FMT_BF16_PAIR4
+    if pair:
+        assert (flags & FLAG_LANE_STREAMS) and tile_n == 32, "bf16 pair variant: lane streams on 32-row tiles only"
+        coded, raw, exps, ctab = symbolise_pair(w)
+    else:
+        coded, raw = symbolise(fmt, w)
     n_out = coded.shape[0]
     assert n_out % STRIPE_N == 0 and k_in % tile_k == 0 and tile_n in (32, 128)
     if flags & FLAG_STATE_PAYLOAD:
-        assert fmt == FMT_BF16, "state payload carries raw-plane bytes: bf16 only"
+        assert fmt in (FMT_BF16, FMT_BF16_PAIR4), "state payload carries raw-plane bytes: bf16 only"
     if flags & FLAG_LANE_STREAMS:
         assert tile_n == 32, "lane streams: 32-row tiles only"
     max_seg_bytes = 0
@@ -297,13 +347,23 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
                 blk = coded[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols]
                 sym = blk[rows, cols]
                 x_init = np.full(LANES, L, dtype=np.uint64)
-                if raw is not None:
+                lits = None
+                if pair:   # one raw byte per WEIGHT (two per step): lane l = row l, vectors of 16 weights
+                    rblk = raw[r0:r0 + tile_n, kt * tile_k:(kt + 1) * tile_k]
+                    plane, payload = _raw_tile_pack(np.ascontiguousarray(rblk.T), flags)
+                    raws.append(plane)
+                    x_init = x_init + payload
+                    eblk = exps[r0:r0 + tile_n, kt * tile_k:(kt + 1) * tile_k]
+                    cw = np.zeros((tile_n, tile_k), dtype=np.uint8)
+                    cw[:, 0::2], cw[:, 1::2] = blk & 15, blk >> 4
+                    lits = [eblk[l][cw[l] == 15] for l in range(LANES)]       # in k order = step order, low nibble first
+                elif raw is not None:
                     rblk = raw[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols]
                     plane, payload = _raw_tile_pack(rblk[rows, cols].reshape(steps, LANES), flags)
                     raws.append(plane)
                     x_init = x_init + payload
                 if flags & FLAG_LANE_STREAMS:
-                    rec, n_words, seg_bytes = _lane_record(sym.reshape(steps, LANES), tab, x_init)
+                    rec, n_words, seg_bytes = _lane_record(sym.reshape(steps, LANES), tab, x_init, seg_steps(fmt), lits)
                     max_seg_bytes = max(max_seg_bytes, seg_bytes)
                     records.append(rec)
                     offsets.append(offsets[-1] + len(rec) // 16)
@@ -337,10 +397,14 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
     off_raw = _align(off_records + len(rec_bytes))
     off_scales = _align(off_raw + len(raw_bytes))
     total = _align(off_scales + len(side))
+    off_codes = 0
+    if pair:   # the 16-byte exponent code table sits where no other format has a section (header field off_zeros)
+        off_codes = off_scales
+        total = _align(off_codes + 16)
     total = max(total, _align(off_records + len(rec_bytes) + TAIL_BYTES))   # tail rule
     hdr = Header(fmt, n_out, k_in, tile_n, tile_k, LANES, PROB_BITS, WORD_BITS, STATE_LO_LOG2, group_size, flags,
                  n_tiles, float(w_scale), off_freq, off_offsets, off_records, off_raw if raw_bytes else 0,
-                 off_scales if side else 0, 0, total, max_seg_bytes)
+                 off_scales if side else 0, off_codes, total, max_seg_bytes)
     buf = np.zeros(total, dtype=np.uint8)
     buf[:HEADER_BYTES] = np.frombuffer(hdr.pack(), dtype=np.uint8)
     buf[off_freq:off_freq + 512] = np.frombuffer(f.astype("<u2").tobytes(), dtype=np.uint8)
@@ -350,6 +414,8 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
         buf[off_raw:off_raw + len(raw_bytes)] = np.frombuffer(raw_bytes, dtype=np.uint8)
     if side:
         buf[off_scales:off_scales + len(side)] = np.frombuffer(side, dtype=np.uint8)
+    if pair:
+        buf[off_codes:off_codes + 16] = ctab
 
     n_weights = n_out * k_in
     H_raw = codec.entropy(codec.histogram(raw)) if raw is not None else 0.0
@@ -358,7 +424,7 @@ def encode(fmt: int, w: np.ndarray, k_in: int, tile_k: int = 0, flags: int = 0,
                  side_bits=8 * len(side), entropy_bits_per_symbol=H, xent_bits_per_symbol=X,
                  raw_entropy_bits_per_symbol=H_raw,
                  # reading A2/A22: H_sym per weight = sum over planes; scales/zeros excluded from both sides
-                 h_sym_bits_per_weight=(H + H_raw) / wps,
+                 h_sym_bits_per_weight=H / wps + H_raw,
                  bits_per_weight=8.0 * (total - len(side)) / n_weights,
                  total_bytes=total)
     return buf, stats
@@ -384,7 +450,9 @@ def decode(buf: np.ndarray):
     steps = n_sym // LANES
     L = 1 << h.state_lo_log2
     coded = np.zeros((h.n_out, h.k_in // wps), dtype=np.uint8)
-    raw = np.zeros_like(coded) if fmt == FMT_BF16 else None
+    pair = fmt == FMT_BF16_PAIR4
+    raw = np.zeros_like(coded) if fmt == FMT_BF16 else (np.zeros((h.n_out, h.k_in), dtype=np.uint8) if pair else None)
+    lit_all = np.full((h.n_out, h.k_in), 0xFFFF, dtype=np.uint16) if pair else None
     rtb = raw_tile_bytes(tile_k, h.flags, tile_n)
     t = 0
     for stripe in range(h.n_out // STRIPE_N):
@@ -392,7 +460,12 @@ def decode(buf: np.ndarray):
             r0 = stripe * STRIPE_N + q * tile_n
             a = h.off_records + 16 * int(offsets[t])
             e = h.off_records + 16 * int(offsets[t + 1])
-            if h.flags & FLAG_LANE_STREAMS:
+            if pair:
+                sym, end, lit = _lane_record_decode(buf[a:e], steps, tab, seg_steps(fmt), True)
+                sym = sym.reshape(-1)
+                used = (e - a - 4 * LANES) // 2
+                lit_all[r0:r0 + tile_n, kt * tile_k:(kt + 1) * tile_k] = lit.T
+            elif h.flags & FLAG_LANE_STREAMS:
                 sym, end = _lane_record_decode(buf[a:e], steps, tab)
                 sym = sym.reshape(-1)
                 used = (e - a - 4 * LANES) // 2
@@ -411,14 +484,26 @@ def decode(buf: np.ndarray):
             blk = np.zeros((tile_n, sym_cols), dtype=np.uint8)
             blk[rows, cols] = sym
             coded[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols] = blk
-            if raw is not None:
+            if pair:
+                plane = buf[h.off_raw + t * rtb:h.off_raw + (t + 1) * rtb]
+                raw[r0:r0 + tile_n, kt * tile_k:(kt + 1) * tile_k] = _raw_tile_unpack(plane, tile_k, h.flags, payload).T
+            elif raw is not None:
                 plane = buf[h.off_raw + t * rtb:h.off_raw + (t + 1) * rtb]
                 rl = _raw_tile_unpack(plane, steps, h.flags, payload)
                 rblk = np.zeros((tile_n, sym_cols), dtype=np.uint8)
                 rblk[rows, cols] = rl.reshape(-1)
                 raw[r0:r0 + tile_n, kt * sym_cols:(kt + 1) * sym_cols] = rblk
             t += 1
-    w = desymbolise(fmt, coded, raw)
+    if pair:
+        ctab = buf[h.off_zeros:h.off_zeros + 16]
+        cw = np.zeros((h.n_out, h.k_in), dtype=np.uint8)
+        cw[:, 0::2], cw[:, 1::2] = coded & 15, coded >> 4
+        if np.any((cw == 15) != (lit_all != 0xFFFF)) or np.any(lit_all[cw == 15] > 0xFF):
+            raise ValueError("corrupt container: escape literals do not match the escape codes")
+        exps = np.where(cw == 15, lit_all.astype(np.uint8), ctab[np.minimum(cw, 14)])
+        w = desymbolise(FMT_BF16, exps, raw)
+    else:
+        w = desymbolise(fmt, coded, raw)
     side = {}
     if fmt == FMT_INT8:
         side["scales"] = np.frombuffer(buf[h.off_scales:h.off_scales + 2 * h.n_out].tobytes(), dtype=np.float16)

@@ -14,11 +14,11 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libanslin.so")
 
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1 = 0, 1, 2, 3, 4, 5
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1, FMT_BF16_PAIR4 = 0, 1, 2, 3, 4, 5, 6
 DT_F32, DT_F16, DT_BF16, DT_I8, DT_FP8_E4M3, DT_FP8_E5M2 = 0, 1, 2, 3, 4, 5
 FLAG_STATE_PAYLOAD = 1
 FLAG_LANE_STREAMS = 2
-X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_INT4_AWQ: DT_F16, FMT_FP8_E5M2: DT_FP8_E5M2, FMT_FP4_E2M1: DT_FP8_E4M3}
+X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_INT4_AWQ: DT_F16, FMT_FP8_E5M2: DT_FP8_E5M2, FMT_FP4_E2M1: DT_FP8_E4M3, FMT_BF16_PAIR4: DT_BF16}
 
 EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_close", "anslin_describe",
            "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm_multi_workspace_bytes", "anslin_gemm",

@@ -38,19 +38,23 @@ struct Header {  // 128 bytes, little endian
 static_assert(sizeof(Header) == kHeaderBytes, "header must be 128 bytes");
 
 // symbols per 16-byte operand chunk
-constexpr uint32_t kFormatMax = ANSLIN_FMT_FP4_E2M1;
+constexpr uint32_t kFormatMax = ANSLIN_FMT_BF16_PAIR4;
+// stored as 16-bit bf16 values; the sign + mantissa byte of every weight lives in the raw plane
+ANSLIN_HD constexpr bool is_bf16_like(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_BF16_PAIR4; }
+// decode steps per lane-stream segment: 8192 weights of a 32-row tile (the pair variant decodes two weights per step)
+ANSLIN_HD constexpr int seg_steps_of(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16_PAIR4 ? 128 : 256; }
 ANSLIN_HD constexpr bool is_fp8(uint32_t fmt) { return fmt == ANSLIN_FMT_FP8_E4M3 || fmt == ANSLIN_FMT_FP8_E5M2; }
 // formats whose MMA runs in kind::f8f6f4 with a per-tensor weight scale and fp8 activations (fp4 is expanded to e4m3)
 ANSLIN_HD constexpr bool is_fp8_path(uint32_t fmt) { return is_fp8(fmt) || fmt == ANSLIN_FMT_FP4_E2M1; }
 // two 4-bit codes per coded byte
 ANSLIN_HD constexpr bool is_packed4(uint32_t fmt) { return fmt == ANSLIN_FMT_INT4_AWQ || fmt == ANSLIN_FMT_FP4_E2M1; }
 ANSLIN_HD constexpr int spc_of(uint32_t fmt) {
-  return (fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_FP4_E2M1) ? 8 : fmt == ANSLIN_FMT_INT4_AWQ ? 4 : 16;
+  return (fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_FP4_E2M1) ? 8 : (fmt == ANSLIN_FMT_INT4_AWQ || fmt == ANSLIN_FMT_BF16_PAIR4) ? 4 : 16;
 }
-ANSLIN_HD constexpr int weights_per_symbol(uint32_t fmt) { return is_packed4(fmt) ? 2 : 1; }
+ANSLIN_HD constexpr int weights_per_symbol(uint32_t fmt) { return (is_packed4(fmt) || fmt == ANSLIN_FMT_BF16_PAIR4) ? 2 : 1; }
 // weights along K covered by one operand unit (32 bytes of bf16/fp16 = 16, of fp8/int8 = 32)
 ANSLIN_HD constexpr int unit_k_of(uint32_t fmt) {
-  return (fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT4_AWQ) ? 16 : 32;
+  return (is_bf16_like(fmt) || fmt == ANSLIN_FMT_INT4_AWQ) ? 16 : 32;
 }
 constexpr uint32_t default_tile_k(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 ? 64 : 256; }
 // bytes per stored weight element of row-major W (int4: half a byte -> handled by callers)

@@ -18,6 +18,7 @@
 #pragma once
 #include <cuda_fp16.h>
 #include <stdint.h>
+#include <type_traits>
 #include "anslin_internal.h"
 
 namespace anslin {
@@ -390,6 +391,42 @@ __device__ __forceinline__ void e2m1x8_to_e4m3(uint32_t b, uint32_t &lo, uint32_
   hi = e2m1x4_to_e4m3(mag >> 16, sgn >> 16);
 }
 
+// ---- bf16 pair variant (ANSLIN_FMT_BF16_PAIR4): a coded byte holds the 4-bit exponent codes of two K-adjacent weights ----
+struct PairLut { uint32_t t0, t1, t2, t3; };   // code -> exponent byte for codes 0..15 (the container's 16-byte code table)
+// q = 4 coded bytes = the codes of 8 weights (nibble n = weight n) -> their exponent bytes, weights 0..3 in lo, 4..7 in hi.
+// Two 8-entry PRMT look-ups per four codes, chosen per byte by the code's top bit (PRMT in sign-replication mode).
+__device__ __forceinline__ void pair_exps(uint32_t q, const PairLut &L, uint32_t &lo, uint32_t &hi) {
+  const uint32_t m = q & 0x77777777u, q4 = q << 4;
+  const uint32_t a0 = __byte_perm(L.t0, L.t1, m), b0 = __byte_perm(L.t2, L.t3, m);
+  const uint32_t a1 = __byte_perm(L.t0, L.t1, m >> 16), b1 = __byte_perm(L.t2, L.t3, m >> 16);
+  uint32_t k0, k1;   // 0xFF where the code is >= 8: PRMT with selector bit 3 set replicates the selected byte's top bit
+  asm("prmt.b32 %0, %1, %2, 0xD9C8;" : "=r"(k0) : "r"(q4), "r"(q));
+  asm("prmt.b32 %0, %1, %2, 0xFBEA;" : "=r"(k1) : "r"(q4), "r"(q));
+  asm("lop3.b32 %0, %1, %2, %3, 0xD8;" : "=r"(lo) : "r"(a0), "r"(b0), "r"(k0));     // k ? b : a
+  asm("lop3.b32 %0, %1, %2, %3, 0xD8;" : "=r"(hi) : "r"(a1), "r"(b1), "r"(k1));
+}
+// four exponent bytes E and four raw bytes R (mantissa << 1 | sign) -> bf16 weights 0,1 in x and 2,3 in y
+__device__ __forceinline__ void bf16x4(uint32_t R, uint32_t E, uint32_t &x, uint32_t &y) {
+  const uint32_t p0 = __byte_perm(R, E, 0x5140), p1 = __byte_perm(R, E, 0x7362);     // [R0,E0,R1,E1], [R2,E2,R3,E3]
+  asm("lop3.b32 %0, %1, %2, 0x7FFF7FFF, 0xE4;" : "=r"(x) : "r"(p0 >> 1), "r"(p0 << 15));
+  asm("lop3.b32 %0, %1, %2, 0x7FFF7FFF, 0xE4;" : "=r"(y) : "r"(p1 >> 1), "r"(p1 << 15));
+}
+// Escape literals of one 4-step chunk: every escaped weight (code 15) takes the next word of the lane's own stream as its
+// exponent byte, in weight order (the look-ahead word of the lane stream serves them like a renormalisation).
+__device__ __forceinline__ void pair_literals(LaneStream &s, uint32_t esc /* bit 4n set: weight n escaped */, uint32_t dir,
+                                              uint32_t &lo, uint32_t &hi) {
+  while (esc) {
+    const int n = (__ffs(int(esc)) - 1) >> 2;
+    esc &= esc - 1;
+    const uint32_t lit = s.w & 0xFFu;
+    s.ptr += dir;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=r"(s.w) : "r"(s.ptr) : "memory");
+    const uint32_t sh = 8u * uint32_t(n & 3), keep = ~(0xFFu << sh);
+    if (n < 4) lo = (lo & keep) | (lit << sh);
+    else hi = (hi & keep) | (lit << sh);
+  }
+}
+
 // Raw-plane (bf16 sign+mantissa) reader of one tile: 16 steps of one lane = one 16-byte vector,
 // fetched one vector ahead into registers, with an L2 prefetch four vectors ahead.
 template <bool kPayload>
@@ -435,9 +472,48 @@ struct RawReader {
 //   POL: InterleavedWords (aux = lanemask_lt) or LaneWords (aux = this lane's cursor direction, +2 / -2).
 template <uint32_t FMT, int RB, int J, bool kPayload, class POL, class Emit>
 __device__ __forceinline__ void decode_unit(typename POL::S (&s)[J], uint32_t ring0, uint32_t tab, int lane, uint32_t lt, int u, int V,
-                                            RawReader<kPayload> (&raw)[J], const uint32_t *const (&sz)[J], Emit &emit) {
+                                            RawReader<kPayload> (&raw)[J], const uint32_t *const (&sz)[J], Emit &emit,
+                                            const PairLut &pl = PairLut{0, 0, 0, 0}) {
   constexpr int G = 2 * RB;
-  if constexpr (FMT == ANSLIN_FMT_BF16) {
+  if constexpr (FMT == ANSLIN_FMT_BF16_PAIR4) {
+    // one unit = 16 weights per row = 8 steps; a 4-step chunk = 8 weights = one 16-byte operand chunk; the chunk's escape
+    // literals follow its last renormalisation.  32-row tiles and lane streams only (nothing else is ever launched).
+    if constexpr (std::is_same<POL, LaneWords>::value && RB == 1) {
+      uint4 rv[J];
+#pragma unroll
+      for (int j = 0; j < J; ++j) rv[j] = raw[j].take(u, V, lane);
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        uint32_t q[J], esc[J], any = 0;
+        decode4<POL, J>(s, q, tab, lt);
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          uint32_t t = q[j] & (q[j] >> 1);
+          t &= t >> 2;
+          esc[j] = t & 0x11111111u;   // nibble == 15
+          any |= esc[j];
+        }
+        uint32_t lo[J], hi[J];
+#pragma unroll
+        for (int j = 0; j < J; ++j) pair_exps(q[j], pl, lo[j], hi[j]);
+        if (__any_sync(0xffffffffu, any != 0)) {
+#pragma unroll
+          for (int j = 0; j < J; ++j) pair_literals(s[j], esc[j], lt, lo[j], hi[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+          uint4 o;
+          bf16x4(h ? rv[j].z : rv[j].x, lo[j], o.x, o.y);
+          bf16x4(h ? rv[j].w : rv[j].y, hi[j], o.z, o.w);
+          if (kPayload && h == 1 && u == V - 1) {   // raw bytes 14, 15 of the last vector ride in the END state
+            const uint32_t p2 = s[j].x - kL;
+            o.w |= ((p2 >> 1) & 0x7Fu) | ((p2 & 1u) << 15) | (((p2 >> 9) & 0x7Fu) << 16) | (((p2 >> 8) & 1u) << 31);
+          }
+          emit.chunk(j, h, lane, o);
+        }
+      }
+    }
+  } else if constexpr (FMT == ANSLIN_FMT_BF16) {
 #pragma unroll 1
     for (int g2 = 0; g2 < RB; ++g2) {  // two chunk rounds share one 16-byte raw vector
       const int v = u * RB + g2;

@@ -21,6 +21,8 @@ struct Geometry {
   uint32_t fmt, n_out, k_in, tile_n, tile_k, flags, group;
   int spc, wps, sym_cols /*symbols per tile row*/, units, steps, KT, stripes, Q /*tiles per (stripe, k-tile) group*/, rb /*tile_n / 32*/;
   size_t n_tiles, row_syms /*symbols per matrix row*/;
+  uint8_t code_of[256];   // bf16 pair variant: exponent byte -> 4-bit code (15 = escape)
+  uint8_t codes[16];      //                    code -> exponent byte (the container's code table)
 };
 
 bool make_geometry(const anslin_desc *d, Geometry *g) {
@@ -38,7 +40,8 @@ bool make_geometry(const anslin_desc *d, Geometry *g) {
   if (g->n_out == 0 || g->k_in == 0 || g->n_out % kTileN || g->k_in % g->tile_k) return false;
   if (g->tile_k % unit_k_of(g->fmt) || g->tile_k % 64 || g->tile_k > 1024) return false;
   if ((g->flags & ~(ANSLIN_FLAG_STATE_PAYLOAD | ANSLIN_FLAG_LANE_STREAMS)) != 0) return false;
-  if ((g->flags & ANSLIN_FLAG_STATE_PAYLOAD) && g->fmt != ANSLIN_FMT_BF16) return false;
+  if ((g->flags & ANSLIN_FLAG_STATE_PAYLOAD) && !is_bf16_like(g->fmt)) return false;
+  if (g->fmt == ANSLIN_FMT_BF16_PAIR4 && (!(g->flags & ANSLIN_FLAG_LANE_STREAMS) || g->tile_n != 32)) return false;
   if (g->fmt == ANSLIN_FMT_INT4_AWQ && (g->group == 0 || g->group % 16 || g->k_in % g->group)) return false;
   g->sym_cols = int(g->tile_k) / g->wps;
   g->units = g->sym_cols / (2 * g->spc);
@@ -48,7 +51,7 @@ bool make_geometry(const anslin_desc *d, Geometry *g) {
   g->KT = int(g->k_in / g->tile_k);
   g->stripes = int(g->n_out / kTileN);
   g->n_tiles = size_t(g->KT) * g->stripes * g->Q;
-  if ((g->flags & ANSLIN_FLAG_LANE_STREAMS) && (g->tile_n != 32 || g->steps % kSegSteps)) return false;
+  if ((g->flags & ANSLIN_FLAG_LANE_STREAMS) && (g->tile_n != 32 || g->steps % seg_steps_of(g->fmt))) return false;
   g->row_syms = g->k_in / g->wps;
   return true;
 }
@@ -62,6 +65,10 @@ size_t side_bytes(const Geometry &g) {
 // Coded symbol / raw byte of the weight element at (row, symbol column) of W.
 inline uint8_t coded_symbol(const Geometry &g, const void *w, size_t row, size_t col) {
   if (g.fmt == ANSLIN_FMT_BF16) return uint8_t(reinterpret_cast<const uint16_t *>(w)[row * g.k_in + col] >> 7);
+  if (g.fmt == ANSLIN_FMT_BF16_PAIR4) {   // col counts weight PAIRS
+    const uint16_t *p = reinterpret_cast<const uint16_t *>(w) + row * g.k_in + 2 * col;
+    return uint8_t(g.code_of[uint8_t(p[0] >> 7)] | (g.code_of[uint8_t(p[1] >> 7)] << 4));
+  }
   return reinterpret_cast<const uint8_t *>(w)[row * g.row_syms + col];
 }
 inline uint8_t raw_byte(const Geometry &g, const void *w, size_t row, size_t col) {
@@ -117,8 +124,15 @@ bool encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
   const int steps = g.steps, spc = g.spc, G = 2 * g.rb;
   const size_t grp = tile / g.Q, q = tile % g.Q, stripe = grp / g.KT, kt = grp % g.KT;
   const size_t row0 = stripe * kTileN + q * g.tile_n, col0 = kt * g.sym_cols;
+  const bool pair = g.fmt == ANSLIN_FMT_BF16_PAIR4;
   std::vector<uint8_t> sym(size_t(steps) * kLanes), raw;
   if (g.fmt == ANSLIN_FMT_BF16) raw.resize(sym.size());
+  if (pair) {   // one raw byte per WEIGHT: raw[k * 32 + lane], lane = row (32-row tiles)
+    raw.resize(size_t(g.tile_k) * kLanes);
+    for (size_t k = 0; k < g.tile_k; ++k)
+      for (int lane = 0; lane < kLanes; ++lane) raw[k * kLanes + lane] = raw_byte(g, w, row0 + lane, size_t(kt) * g.tile_k + k);
+  }
+  const size_t raw_steps = pair ? g.tile_k : size_t(steps);   // entries per lane in raw[]
   for (int u = 0; u < g.units; ++u)
     for (int gq = 0; gq < G; ++gq)
       for (int lane = 0; lane < kLanes; ++lane) {
@@ -126,7 +140,7 @@ bool encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
         for (int e = 0; e < spc; ++e) {
           size_t t = size_t(u * G + gq) * spc + e;
           sym[t * kLanes + lane] = coded_symbol(g, w, row, col + e);
-          if (!raw.empty()) raw[t * kLanes + lane] = raw_byte(g, w, row, col + e);
+          if (!raw.empty() && !pair) raw[t * kLanes + lane] = raw_byte(g, w, row, col + e);
         }
       }
   uint32_t x[kLanes];
@@ -134,12 +148,13 @@ bool encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
   for (int lane = 0; lane < kLanes; ++lane) {
     x[lane] = kL;
     if (payload)
-      x[lane] += uint32_t(raw[size_t(steps - 2) * kLanes + lane]) | (uint32_t(raw[size_t(steps - 1) * kLanes + lane]) << 8);
+      x[lane] += uint32_t(raw[(raw_steps - 2) * kLanes + lane]) | (uint32_t(raw[(raw_steps - 1) * kLanes + lane]) << 8);
   }
   // Words are produced back to front so that the buffer ends up in decoder read order
   // (step ascending, renormalising lanes ascending) without a reversal pass.
   const bool lane_streams = g.flags & ANSLIN_FLAG_LANE_STREAMS;
-  const int S = lane_streams ? steps / kSegSteps : 0;
+  const int seg = seg_steps_of(g.fmt);
+  const int S = lane_streams ? steps / seg : 0;
   std::vector<uint16_t> words(lane_streams ? 0 : sym.size() + 8);
   std::vector<std::vector<uint16_t>> lw(size_t(S) * kLanes);   // lane streams: words of (segment, lane), filled back to front
   size_t wp = words.size();
@@ -148,9 +163,19 @@ bool encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
       const uint8_t s = sym[size_t(t) * kLanes + lane];
       const uint32_t fs = f[s];
       uint32_t xv = x[lane];
+      if (pair && (t & 3) == 3) {
+        // escape literals of the 4-step chunk: read after the chunk's last renormalisation in weight order, so (this
+        // buffer is filled back to front) pushed first, last weight first
+        const uint16_t *pw = reinterpret_cast<const uint16_t *>(w) + (row0 + lane) * size_t(g.k_in) + size_t(kt) * g.tile_k;
+        for (int tt = t; tt > t - 4; --tt) {
+          const uint8_t sc = sym[size_t(tt) * kLanes + lane];
+          if ((sc >> 4) == 15) lw[size_t(t / seg) * kLanes + lane].push_back(uint16_t(uint8_t(pw[2 * tt + 1] >> 7)));
+          if ((sc & 15) == 15) lw[size_t(t / seg) * kLanes + lane].push_back(uint16_t(uint8_t(pw[2 * tt] >> 7)));
+        }
+      }
       if (uint64_t(xv) >= (uint64_t(fs) << (kStateLoLog2 - kProbBits + kWordBits))) {
         // the decoder reads this word right after decoding step t
-        if (lane_streams) lw[size_t(t / kSegSteps) * kLanes + lane].push_back(uint16_t(xv));
+        if (lane_streams) lw[size_t(t / seg) * kLanes + lane].push_back(uint16_t(xv));
         else words[--wp] = uint16_t(xv);
         xv >>= kWordBits;
       }
@@ -194,7 +219,7 @@ bool encode_tile(const Geometry &g, const void *w, size_t tile, const uint32_t *
     *n_words_out = nw;
   }
   if (raw_out) {
-    const int V = steps / 16;
+    const int V = int(raw_steps / 16);
     for (int v = 0; v < V; ++v) {
       const bool last = payload && v == V - 1;
       for (int lane = 0; lane < kLanes; ++lane)
@@ -225,9 +250,11 @@ size_t anslin_encode_bound(const anslin_desc *desc) {
   if (!make_geometry(desc, &g)) return 0;
   const size_t tile_syms = size_t(g.steps) * kLanes;
   // every symbol costs at most 12 bits + one flush word per lane; round generously
-  const size_t rec = align16(4 * kLanes + 2 * (tile_syms * 3 / 4 + 2 * kLanes + 8)) + align16(size_t(kSegTableBytes) * (g.steps / kSegSteps + 1));
+  // pair variant: a step may also carry two literal words
+  const size_t words_max = g.fmt == ANSLIN_FMT_BF16_PAIR4 ? tile_syms * 3 : tile_syms * 3 / 4;
+  const size_t rec = align16(4 * kLanes + 2 * (words_max + 2 * kLanes + 8)) + align16(size_t(kSegTableBytes) * (g.steps / seg_steps_of(g.fmt) + 1));
   size_t total = kHeaderBytes + 512 + align16(4 * (g.n_tiles + 1)) + g.n_tiles * rec + 64;
-  if (g.fmt == ANSLIN_FMT_BF16) total += g.n_tiles * raw_tile_bytes(g.tile_n, g.tile_k, 0) + 16;
+  if (is_bf16_like(g.fmt)) total += g.n_tiles * raw_tile_bytes(g.tile_n, g.tile_k, 0) + 16 + 32;
   return total + align16(side_bytes(g)) + 16 + kTailBytes;
 }
 
@@ -251,6 +278,19 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
   unsigned nthr = std::max(1u, std::min(32u, std::thread::hardware_concurrency()));
   if (g.n_tiles < 64) nthr = 1;
 
+  if (g.fmt == ANSLIN_FMT_BF16_PAIR4) {
+    // code table: the 15 most frequent exponent bytes, descending count, ties by smaller exponent; code 15 = escape
+    std::vector<uint64_t> ce(256, 0);
+    const uint16_t *p = static_cast<const uint16_t *>(w_host);
+    for (size_t i = 0, n = size_t(g.n_out) * g.k_in; i < n; ++i) ++ce[uint8_t(p[i] >> 7)];
+    int order[256];
+    for (int s = 0; s < 256; ++s) order[s] = s;
+    std::stable_sort(order, order + 256, [&](int a, int b) { return ce[a] > ce[b]; });
+    std::memset(g.code_of, 15, sizeof(g.code_of));
+    std::memset(g.codes, 0, sizeof(g.codes));
+    for (int i = 0; i < 15; ++i) { g.codes[i] = uint8_t(order[i]); g.code_of[order[i]] = uint8_t(i); }
+  }
+
   // P:l.167: statistics aggregated over the whole matrix -> one shared codebook.
   std::vector<std::vector<uint64_t>> hist(nthr, std::vector<uint64_t>(512, 0));
   {
@@ -263,6 +303,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
           for (size_t c = 0; c < g.row_syms; ++c) {
             ++hc[coded_symbol(g, w_host, r, c)];
             if (g.fmt == ANSLIN_FMT_BF16) ++hr[raw_byte(g, w_host, r, c)];
+            if (g.fmt == ANSLIN_FMT_BF16_PAIR4) { ++hr[raw_byte(g, w_host, r, 2 * c)]; ++hr[raw_byte(g, w_host, r, 2 * c + 1)]; }
           }
       });
     for (auto &t : th) t.join();
@@ -279,7 +320,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
   std::vector<uint64_t> nwords(g.n_tiles, 0);
   std::vector<uint32_t> segbytes(g.n_tiles, 0);
   std::atomic<bool> lane_fail(false);
-  const size_t rtb = g.fmt == ANSLIN_FMT_BF16 ? raw_tile_bytes(g.tile_n, g.tile_k, g.flags) : 0;
+  const size_t rtb = is_bf16_like(g.fmt) ? raw_tile_bytes(g.tile_n, g.tile_k, g.flags) : 0;
   Header h;
   std::memset(&h, 0, sizeof(h));
   h.off_freq = kHeaderBytes;
@@ -305,6 +346,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
     for (auto &t : th) t.join();
   }
   if (lane_fail) {   // a tile does not fit the lane-stream tables: encode the matrix with interleaved words instead
+    if (g.fmt == ANSLIN_FMT_BF16_PAIR4) return ANSLIN_ERR_UNSUPPORTED;   // the pair variant has no interleaved layout
     g.flags &= ~ANSLIN_FLAG_LANE_STREAMS;
     return encode_with(g, desc, w_host, scales_host, zeros_host, container_out, capacity, bytes_out, st);
   }
@@ -315,6 +357,10 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
   const size_t after_raw = rtb ? h.off_raw + raw_all.size() : h.off_records + rec_total;
   h.off_scales = sb ? align16(after_raw) : 0;
   h.total_bytes = align16(sb ? h.off_scales + sb : after_raw);
+  if (g.fmt == ANSLIN_FMT_BF16_PAIR4) {   // 16-byte exponent code table, in the section slot no other format uses
+    h.off_zeros = align16(after_raw);
+    h.total_bytes = h.off_zeros + 16;
+  }
   // tail rule: the decoder's compressed-word ring reads ahead of the record it decodes, so at least
   // kTailBytes readable bytes follow the records section (zero padding if the sections after it are short)
   h.total_bytes = std::max<uint64_t>(h.total_bytes, align16(h.off_records + rec_total + kTailBytes));
@@ -345,6 +391,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
   }
   offs[g.n_tiles] = uint32_t(pos / 16);
   if (rtb) std::memcpy(out + h.off_raw, raw_all.data(), raw_all.size());
+  if (g.fmt == ANSLIN_FMT_BF16_PAIR4) std::memcpy(out + h.off_zeros, g.codes, 16);
   if (g.fmt == ANSLIN_FMT_INT8) {
     std::memcpy(out + h.off_scales, scales_host, sb);
   } else if (g.fmt == ANSLIN_FMT_INT4_AWQ) {
@@ -377,7 +424,7 @@ int encode_with(Geometry g, const anslin_desc *desc, const void *w_host, const v
       return n > 0 ? e : 0.0;
     };
     st->entropy_bits_per_symbol = H(cnt);
-    st->raw_entropy_bits_per_symbol = g.fmt == ANSLIN_FMT_BF16 ? H(cnt_raw) : 0.0;
+    st->raw_entropy_bits_per_symbol = is_bf16_like(g.fmt) ? H(cnt_raw) : 0.0;
     double n = 0, x = 0;
     for (int s = 0; s < 256; ++s) n += double(cnt[s]);
     for (int s = 0; s < 256; ++s)
@@ -416,7 +463,7 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   }
   if (sum != kM) return ANSLIN_ERR_CORRUPT;
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(p + h.off_offsets);
-  uint64_t rec_end = g.fmt == ANSLIN_FMT_BF16 ? h.off_raw : (h.off_scales ? h.off_scales : T);
+  uint64_t rec_end = is_bf16_like(g.fmt) ? h.off_raw : (h.off_scales ? h.off_scales : T);
   if (rec_end < h.off_records || rec_end > T) return ANSLIN_ERR_CORRUPT;
   const uint64_t rec_units = (rec_end - h.off_records) / 16;
   if (offs[0] != 0) return ANSLIN_ERR_CORRUPT;
@@ -424,10 +471,11 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   for (size_t t = 0; t < g.n_tiles; ++t) {
     // a record holds at least the 32 lane states and never more than the worst-case tile
     if (offs[t + 1] < offs[t] + 8 || offs[t + 1] > rec_units) return ANSLIN_ERR_CORRUPT;
-    if (uint64_t(offs[t + 1] - offs[t]) * 16 > 128 + uint64_t(g.steps) * kLanes * 2 + 16 + uint64_t(kSegTableBytes) * (g.steps / kSegSteps + 1))
+    if (uint64_t(offs[t + 1] - offs[t]) * 16 > 128 + uint64_t(g.steps) * kLanes * (g.fmt == ANSLIN_FMT_BF16_PAIR4 ? 6 : 2) + 16 + uint64_t(kSegTableBytes) * (g.steps / seg_steps_of(g.fmt) + 1))
       return ANSLIN_ERR_CORRUPT;
   }
-  if (g.fmt == ANSLIN_FMT_BF16 && !in(h.off_raw, raw_tile_bytes(g.tile_n, g.tile_k, g.flags) * g.n_tiles)) return ANSLIN_ERR_CORRUPT;
+  if (is_bf16_like(g.fmt) && !in(h.off_raw, raw_tile_bytes(g.tile_n, g.tile_k, g.flags) * g.n_tiles)) return ANSLIN_ERR_CORRUPT;
+  if (g.fmt == ANSLIN_FMT_BF16_PAIR4 && !in(h.off_zeros, 16)) return ANSLIN_ERR_CORRUPT;
   if (side_bytes(g) && !in(h.off_scales, side_bytes(g))) return ANSLIN_ERR_CORRUPT;
   if ((g.flags & ANSLIN_FLAG_LANE_STREAMS) && (h.max_seg_bytes < 32 || h.max_seg_bytes > 2 * 0xFFFF + 64)) return ANSLIN_ERR_CORRUPT;
   anslin_weight *w = new (std::nothrow) anslin_weight;

@@ -150,6 +150,7 @@ __host__ __device__ constexpr uint32_t make_idesc(uint32_t cfmt, uint32_t afmt, 
 }
 template <uint32_t FMT> struct FmtTraits;
 template <> struct FmtTraits<ANSLIN_FMT_BF16> { static constexpr int kind = 0; static constexpr uint32_t c = 1, ab = 1; static constexpr int xbytes = 2; };
+template <> struct FmtTraits<ANSLIN_FMT_BF16_PAIR4> : FmtTraits<ANSLIN_FMT_BF16> {};
 template <> struct FmtTraits<ANSLIN_FMT_INT4_AWQ> { static constexpr int kind = 0; static constexpr uint32_t c = 1, ab = 0; static constexpr int xbytes = 2; };
 template <> struct FmtTraits<ANSLIN_FMT_FP8_E4M3> { static constexpr int kind = 1; static constexpr uint32_t c = 1, ab = 0; static constexpr int xbytes = 1; };
 template <> struct FmtTraits<ANSLIN_FMT_FP4_E2M1> { static constexpr int kind = 1; static constexpr uint32_t c = 1, ab = 0; static constexpr int xbytes = 1; };
@@ -170,7 +171,7 @@ ContainerView view_of(const anslin_weight *w) {
   ContainerView v;
   v.base = w->dev;
   v.off_freq = h.off_freq; v.off_offsets = h.off_offsets; v.off_records = h.off_records; v.off_raw = h.off_raw;
-  v.off_scales = h.off_scales; v.total = h.total_bytes;
+  v.off_scales = h.format == ANSLIN_FMT_BF16_PAIR4 ? h.off_zeros /* the 16-byte exponent code table */ : h.off_scales; v.total = h.total_bytes;
   v.n_out = h.n_out; v.k_in = h.k_in; v.tile_n = h.tile_n; v.tile_k = h.tile_k; v.KT = h.k_in / h.tile_k; v.n_tiles = h.n_tiles;
   v.units = h.tile_k / unit_k_of(h.format); v.group = h.group_size; v.flags = h.flags; v.w_scale = h.w_scale;
   v.max_seg_bytes = h.max_seg_bytes;
@@ -192,7 +193,7 @@ template <int RB, int J> struct TileTraits {
 constexpr int kJ32 = ANSLIN_J32;   // tiles a warp interleaves when tiles have 32 rows
 
 __host__ __device__ constexpr size_t row_bytes_of(uint32_t fmt, size_t k) {
-  return fmt == ANSLIN_FMT_BF16 ? k * 2 : is_packed4(fmt) ? k / 2 : k;
+  return is_bf16_like(fmt) ? k * 2 : is_packed4(fmt) ? k / 2 : k;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -267,10 +268,15 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
   const uint32_t stage_s = smem_u32(rings) + uint32_t(kDecWarps) * J * stream_bytes + uint32_t(warp) * J * GlobalEmit<FMT, RB, J>::kStageBytes;
   const uint32_t aux = LS ? ((lane & 1) ? uint32_t(-2) : 2u) : lanemask_lt();
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
+  PairLut plut{0, 0, 0, 0};
+  if constexpr (FMT == ANSLIN_FMT_BF16_PAIR4) {
+    const uint4 c = *reinterpret_cast<const uint4 *>(cv.base + cv.off_scales);
+    plut = PairLut{c.x, c.y, c.z, c.w};
+  }
   const size_t row_bytes = row_bytes_of(FMT, cv.k_in), tile_row_bytes = row_bytes_of(FMT, cv.tile_k);
   const size_t rtb = raw_tile_bytes(32 * RB, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
   const int V = int(cv.units) * RB;
-  constexpr uint32_t kUnitsPerSeg = LS ? kSegSteps / unit_steps32(FMT) : 1;
+  constexpr uint32_t kUnitsPerSeg = LS ? seg_steps_of(FMT) / unit_steps32(FMT) : 1;
   for (uint32_t job = blockIdx.x * kDecWarps + warp; job < cv.n_tiles / J; job += gridDim.x * kDecWarps) {
     typename POL::S s[J];
     RawReader<PAYLOAD> raw[J];
@@ -286,7 +292,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
       if constexpr (LS) lane_open(s[j], rec, int(cv.units / kUnitsPerSeg), lane);
       else stream_open(s[j], rec, ring_s + j * stream_bytes, lane);
       emit.tile_out[j] = out + (size_t(stripe) * kTileN + size_t(q) * 32 * RB) * row_bytes + size_t(kt) * tile_row_bytes;
-      if (FMT == ANSLIN_FMT_BF16) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
+      if (is_bf16_like(FMT)) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
       sz[j] = nullptr;
     }
     for (uint32_t u = 0; u < cv.units; ++u) {
@@ -296,7 +302,7 @@ __global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView
           lane_open_segments<J>(s, ring_s, stream_bytes, int(u / kUnitsPerSeg), lane);
         }
       }
-      decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, smem_u32(tab), lane, aux, int(u), V, raw, sz, emit);
+      decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, smem_u32(tab), lane, aux, int(u), V, raw, sz, emit, plut);
       emit.unit_done(lane);
     }
   }
@@ -576,7 +582,12 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
       const uint32_t PT = P.D / NW, team = d / NW, hw = d % NW;   // teams of NW warps fill one 128-row unit together
       const uint32_t ring_s = smem0 + ring_off + d * J * P.stream_bytes, tab_s = smem0 + tab_off;
       const uint32_t aux = LS ? ((lane & 1) ? uint32_t(-2) : 2u) : lanemask_lt();
-      constexpr uint32_t kUnitsPerSeg = LS ? kSegSteps / unit_steps32(FMT) : 1;
+      PairLut plut{0, 0, 0, 0};
+      if constexpr (FMT == ANSLIN_FMT_BF16_PAIR4) {
+        const uint4 c = *reinterpret_cast<const uint4 *>(cv.base + cv.off_scales);
+        plut = PairLut{c.x, c.y, c.z, c.w};
+      }
+      constexpr uint32_t kUnitsPerSeg = LS ? seg_steps_of(FMT) / unit_steps32(FMT) : 1;
       const uint32_t *offs = reinterpret_cast<const uint32_t *>(cv.base + cv.off_offsets);
       const size_t rtb = raw_tile_bytes(32 * RB, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
       const uint32_t xbytes = mpad * 32u;
@@ -600,7 +611,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
           const uint8_t *rec = cv.base + cv.off_records + size_t(offs[t]) * 16;
           if constexpr (LS) lane_open(s[j], rec, int(units / kUnitsPerSeg), lane);
           else stream_open(s[j], rec, ring_s + j * P.stream_bytes, lane);
-          if (FMT == ANSLIN_FMT_BF16) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
+          if (is_bf16_like(FMT)) raw[j].open(cv.base + cv.off_raw + size_t(t) * rtb, V, lane);
           emit.row0[j] = q * 32u * RB;
           sz[j] = nullptr;
         }
@@ -616,7 +627,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 #pragma unroll
             for (int j = 0; j < J; ++j) {
               if (lane < 24) prefetch_l2(cv.base + cv.off_records + size_t(next_off[j]) * 16 + lane * 128);
-              else if (FMT == ANSLIN_FMT_BF16) prefetch_l2(cv.base + cv.off_raw + size_t((gt + PT) * Q + hw * J + j) * rtb + (lane - 24) * 128);
+              else if (is_bf16_like(FMT)) prefetch_l2(cv.base + cv.off_raw + size_t((gt + PT) * Q + hw * J + j) * rtb + (lane - 24) * 128);
             }
           }
           // team-private slots: unit n of this team lives in slot team*B + n % B (B = P.B buffers per team), so the
@@ -643,7 +654,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
             mbar_arrive_expect_tx(full_s + 8 * slot, xbytes);
             tma_load_2d(slot_a + kUnitBytes, &tms.m[pi], k_elem, 0, full_s + 8 * slot);
           }
-          decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, tab_s, lane, aux, int(u), V, raw, sz, emit);
+          decode_unit<FMT, RB, J, PAYLOAD, POL>(s, ring_s, tab_s, lane, aux, int(u), V, raw, sz, emit, plut);
           fence_proxy_async();  // generic-proxy stores -> visible to the tensor core's async proxy
           __syncwarp();
           if (lane == 0) mbar_arrive(full_s + 8 * slot);
@@ -901,11 +912,11 @@ Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
 }
 
 bool x_dtype_ok(uint32_t fmt, uint32_t dt) {
-  return (fmt == ANSLIN_FMT_BF16 && dt == ANSLIN_DT_BF16) || (fmt == ANSLIN_FMT_INT4_AWQ && dt == ANSLIN_DT_F16) ||
+  return (is_bf16_like(fmt) && dt == ANSLIN_DT_BF16) || (fmt == ANSLIN_FMT_INT4_AWQ && dt == ANSLIN_DT_F16) ||
          (fmt == ANSLIN_FMT_INT8 && dt == ANSLIN_DT_I8) || (is_fp8_path(fmt) && (dt == ANSLIN_DT_FP8_E4M3 || dt == ANSLIN_DT_FP8_E5M2));
 }
 // tcgen05 instruction-descriptor format code of the weight operand (a) / of X (b)
-uint32_t afmt_of(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT8 || fmt == ANSLIN_FMT_FP8_E5M2 ? 1u : 0u; }
+uint32_t afmt_of(uint32_t fmt) { return is_bf16_like(fmt) || fmt == ANSLIN_FMT_INT8 || fmt == ANSLIN_FMT_FP8_E5M2 ? 1u : 0u; }
 uint32_t bfmt_of(uint32_t fmt, uint32_t dt) { return is_fp8_path(fmt) ? (dt == ANSLIN_DT_FP8_E5M2 ? 1u : 0u) : afmt_of(fmt); }
 
 int sm_budget() { return std::max(1, num_sms()); }
@@ -945,7 +956,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
   const Header &h0 = ws[0]->h;
   const bool scaled = h0.format == ANSLIN_FMT_INT8 || is_fp8_path(h0.format);
-  const int xb = (h0.format == ANSLIN_FMT_BF16 || h0.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
+  const int xb = (is_bf16_like(h0.format) || h0.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
   if (!x_dtype_ok(h0.format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
   uint32_t mpad_max = 16;
   uint64_t work[kMaxProblems], work_sum = 0;
@@ -1055,6 +1066,10 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
            : launch_fused<F, 4, PAY, false>(tms, p, grid, smem, st))
   switch (h0.format) {
     case ANSLIN_FMT_BF16: return pay ? ANSLIN_LAUNCH(ANSLIN_FMT_BF16, true) : ANSLIN_LAUNCH(ANSLIN_FMT_BF16, false);
+    case ANSLIN_FMT_BF16_PAIR4:   // lane streams on 32-row tiles only (anslin_open checked)
+      if (RB != 1 || !ls) return ANSLIN_ERR_CORRUPT;
+      return pay ? launch_fused<ANSLIN_FMT_BF16_PAIR4, 1, true, true>(tms, p, grid, smem, st)
+                 : launch_fused<ANSLIN_FMT_BF16_PAIR4, 1, false, true>(tms, p, grid, smem, st);
     case ANSLIN_FMT_FP8_E4M3:
     case ANSLIN_FMT_FP8_E5M2: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);   // same bytes, another descriptor code
     case ANSLIN_FMT_INT8: return ANSLIN_LAUNCH(ANSLIN_FMT_INT8, false);
@@ -1139,6 +1154,10 @@ int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void
     case ANSLIN_FMT_BF16:
       return (h.flags & ANSLIN_FLAG_STATE_PAYLOAD) ? launch_decode<ANSLIN_FMT_BF16, true>(cv, w_out_dev, st)
                                                     : launch_decode<ANSLIN_FMT_BF16, false>(cv, w_out_dev, st);
+    case ANSLIN_FMT_BF16_PAIR4:
+      if (cv.tile_n != 32 || !(cv.flags & ANSLIN_FLAG_LANE_STREAMS)) return ANSLIN_ERR_CORRUPT;
+      return (h.flags & ANSLIN_FLAG_STATE_PAYLOAD) ? launch_decode_t<ANSLIN_FMT_BF16_PAIR4, 1, true, true>(cv, w_out_dev, st)
+                                                    : launch_decode_t<ANSLIN_FMT_BF16_PAIR4, 1, false, true>(cv, w_out_dev, st);
     case ANSLIN_FMT_FP8_E4M3:
     case ANSLIN_FMT_FP8_E5M2: return launch_decode<ANSLIN_FMT_FP8_E4M3, false>(cv, w_out_dev, st);
     case ANSLIN_FMT_INT8: return launch_decode<ANSLIN_FMT_INT8, false>(cv, w_out_dev, st);
@@ -1173,7 +1192,7 @@ int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int
     return gemm_launch(1, &w, &x_dev, x_dtype, &ldx, &m, &x_scale_dev, &y_dev, &ldy, workspace_dev, workspace_bytes,
                        static_cast<cudaStream_t>(stream));
   if (!x_dev || !y_dev) return ANSLIN_ERR_INVALID_ARG;
-  const int xb = (w->h.format == ANSLIN_FMT_BF16 || w->h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
+  const int xb = (is_bf16_like(w->h.format) || w->h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
   for (int32_t r0 = 0; r0 < m;) {
     const anslin_weight *ws[kMaxProblems];
     const void *xs[kMaxProblems], *xsc[kMaxProblems];
@@ -1234,7 +1253,7 @@ int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts, 
     if (rows == 0) continue;
     const Header &h = experts[e]->h;
     if (h.format != experts[0]->h.format || h.n_out != experts[0]->h.n_out || h.k_in != experts[0]->h.k_in) return ANSLIN_ERR_INVALID_ARG;
-    const int xb = (h.format == ANSLIN_FMT_BF16 || h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
+    const int xb = (is_bf16_like(h.format) || h.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
     for (int32_t r0 = 0; r0 < rows; r0 += kMaxM) {   // an expert with more than kMaxM rows is several problems (see anslin_gemm)
       if (cnt == kMaxProblems) {
         const int rc = flush();
@@ -1267,7 +1286,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   // the int4 slot takes fp16 weights (what AWQ dequantises to): same MMA kind as the fused int4 path
   const uint32_t xd_need = format == ANSLIN_FMT_INT4_AWQ ? ANSLIN_DT_F16 : 0;
   if (format == ANSLIN_FMT_INT4_AWQ ? x_dtype != xd_need : !x_dtype_ok(format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
-  const int xb = (format == ANSLIN_FMT_BF16 || format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
+  const int xb = (is_bf16_like(format) || format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
   const uint32_t ke = 128 / xb;
   if (n_out % kTileN || k_in % ke) return ANSLIN_ERR_UNSUPPORTED;
   if ((reinterpret_cast<uintptr_t>(w_dev) | reinterpret_cast<uintptr_t>(x_dev) | reinterpret_cast<uintptr_t>(y_dev) |
@@ -1298,7 +1317,8 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   if (!make_map_2d(&tmw, w_dev, xb, k_in, n_out, k_in, ke, kTileN, CU_TENSOR_MAP_SWIZZLE_128B)) return ANSLIN_ERR_CUDA;
   if (!make_map_2d(&tmx, x_dev, xb, k_in, uint64_t(m), uint64_t(ldx), ke, p.mpad, CU_TENSOR_MAP_SWIZZLE_128B)) return ANSLIN_ERR_CUDA;
   switch (format) {
-    case ANSLIN_FMT_BF16: return launch_dense<ANSLIN_FMT_BF16>(tmw, tmx, p, grid, smem, st);
+    case ANSLIN_FMT_BF16:
+    case ANSLIN_FMT_BF16_PAIR4: return launch_dense<ANSLIN_FMT_BF16>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_INT4_AWQ: return launch_dense<ANSLIN_FMT_INT4_AWQ>(tmw, tmx, p, grid, smem, st);
     case ANSLIN_FMT_FP8_E4M3:
     case ANSLIN_FMT_FP8_E5M2:

@@ -9,7 +9,7 @@ from __future__ import annotations
 
 import numpy as np
 
-FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1 = 0, 1, 2, 3, 4, 5
+FMT_BF16, FMT_FP8_E4M3, FMT_INT8, FMT_INT4_AWQ, FMT_FP8_E5M2, FMT_FP4_E2M1, FMT_BF16_PAIR4 = 0, 1, 2, 3, 4, 5, 6
 
 # BASELINE.json configs 2/3 (Qwen-14B-shaped dense decoder layer), [n_out, k_in] = Linear.weight
 QWEN14B_LAYER = [("q", 5120, 5120), ("k", 1024, 5120), ("v", 1024, 5120), ("o", 5120, 5120),

@@ -9,7 +9,7 @@ import torch
 
 from . import binding as B
 
-_TORCH_X = {B.FMT_BF16: torch.bfloat16, B.FMT_INT4_AWQ: torch.float16, B.FMT_INT8: torch.int8,
+_TORCH_X = {B.FMT_BF16: torch.bfloat16, B.FMT_BF16_PAIR4: torch.bfloat16, B.FMT_INT4_AWQ: torch.float16, B.FMT_INT8: torch.int8,
             B.FMT_FP8_E4M3: torch.uint8, B.FMT_FP8_E5M2: torch.uint8, B.FMT_FP4_E2M1: torch.uint8}
 
 
@@ -43,7 +43,7 @@ class DeviceWeight:
 
     def decode(self) -> torch.Tensor:
         """anslin_decode -> row-major W in its original dtype/packing (bf16 as int16 bit patterns)."""
-        if self.fmt == B.FMT_BF16:
+        if self.fmt in (B.FMT_BF16, B.FMT_BF16_PAIR4):
             out = torch.empty((self.n_out, self.k_in), dtype=torch.int16, device=self.container_dev.device)
         elif self.fmt in (B.FMT_INT4_AWQ, B.FMT_FP4_E2M1):
             out = torch.empty((self.n_out, self.k_in // 2), dtype=torch.uint8, device=self.container_dev.device)

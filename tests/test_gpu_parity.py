@@ -69,6 +69,11 @@ def _decode_cases():
     yield "fp4", B.FMT_FP4_E2M1, f4, 1024, dict(tile_k=256, w_scale=sc4)
     yield "fp4-32x256", B.FMT_FP4_E2M1, f4, 1024, dict(tile_k=256, w_scale=sc4, tile_n=32)
     yield "fp4-32x1024-lanes", B.FMT_FP4_E2M1, f4, 1024, dict(tile_k=1024, w_scale=sc4, tile_n=32, flags=2)
+    wpair = wl.copy()
+    wpair[3, 5], wpair[200, 300], wpair[200, 301], wpair[31, 1023], wpair[31, 1022], wpair[64, 255] = 0x0001, 0x7F7F, 0x0080, 0x0003, 0x7F00, 0xFF80
+    yield "pair4-32x256-payload", B.FMT_BF16_PAIR4, wpair, 1024, dict(tile_k=256, flags=3, tile_n=32)
+    yield "pair4-32x512", B.FMT_BF16_PAIR4, wpair, 1024, dict(tile_k=512, flags=2, tile_n=32)
+    yield "pair4-constant", B.FMT_BF16_PAIR4, np.full((128, 256), 0xBF80, dtype=np.uint16), 256, dict(tile_k=256, tile_n=32, flags=3)
     yield "bf16-constant-lanes", B.FMT_BF16, np.full((128, 256), 0xBF80, dtype=np.uint16), 256, dict(tile_k=256, tile_n=32, flags=2)
 
 
@@ -114,6 +119,24 @@ def test_gemm_bf16(m, flags, tile):
     y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
     y_ref, a_ref = og.gemm_bf16(x, w)
     check_gemm(y, y_ref, a_ref)
+    dw.close()
+
+
+@pytest.mark.parametrize("m", [1, 16, 75])
+@pytest.mark.parametrize("tk,flags", [(256, 3), (512, 2)])
+def test_gemm_bf16_pair_variant(m, tk, flags):
+    """S: 8(f) NEXT-5: two K-adjacent bf16 exponents per rANS step (4-bit codes, escapes as in-stream literals);
+    the GEMM sees exactly the original weights."""
+    rt = _rt()
+    n, k = 640, 1024
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=59, jitter=True)).copy()
+    w[0, 0], w[639, 1023], w[300, 511], w[300, 512] = 0x0001, 0x5F7F, 0x0080, 0x8003    # rare exponents -> escapes (finite in fp32 sums)
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=60))
+    buf, st = B.anslin_encode_host(B.FMT_BF16_PAIR4, w, n, k, tile_k=tk, flags=flags, tile_n=32)
+    dw = rt.DeviceWeight(buf)
+    assert np.array_equal(dw.decode().cpu().numpy().view(np.uint16), w)
+    y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    check_gemm(y, *og.gemm_bf16(x, w))
     dw.close()
 
 

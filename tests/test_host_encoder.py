@@ -54,6 +54,10 @@ def _cases():
     yield "int4-32x512-lanes", oc.FMT_INT4_AWQ, p4, 512, dict(tile_k=512, scales=s4, zeros=z4, group_size=128, tile_n=32, flags=2)
     f5, sc5 = inputs.quant_fp8_e5m2_weights(inputs.weights_f32(128, 512, seed=34, std=0.015, outliers=False))
     yield "e5m2", oc.FMT_FP8_E5M2, f5, 512, dict(tile_k=256, w_scale=sc5)
+    wp = inputs.f32_to_bf16_bits(wf).copy()
+    wp[3, 5], wp[200, 300], wp[200, 301], wp[31, 511], wp[31, 510] = 0x0001, 0x7F7F, 0x0080, 0x0003, 0x7F00   # rare exponents: escapes
+    yield "pair4-32x256-lanes-payload", oc.FMT_BF16_PAIR4, wp, 512, dict(tile_k=256, flags=3, tile_n=32)
+    yield "pair4-32x512-lanes", oc.FMT_BF16_PAIR4, wp, 512, dict(tile_k=512, flags=2, tile_n=32)
     f4, sc4 = inputs.quant_fp4_weights(inputs.weights_f32(128, 512, seed=35, outliers=False))
     yield "fp4", oc.FMT_FP4_E2M1, f4, 512, dict(tile_k=256, w_scale=sc4)
     yield "fp4-32x512-lanes", oc.FMT_FP4_E2M1, f4, 512, dict(tile_k=512, w_scale=sc4, tile_n=32, flags=2)

@@ -200,6 +200,37 @@ def test_e2m1_values_and_fp4_roundtrip():
     assert y[0, 0] == (1.0 * -1.0 + 2.0 * 6.0) * 2.0 * 0.5 and a[0, 0] == 13.0
 
 
+def test_pair_variant_stream_and_container():
+    """S: 8(f) NEXT-5 bf16 pair variant.  Pins: without escapes the literal-carrying stream IS the plain rANS stream;
+    with escapes it round-trips and every literal comes back at its nibble; the container is lossless, carries its
+    code table, and costs within 0.03 bit/weight of the one-symbol-per-weight bf16 container."""
+    rng = np.random.default_rng(5)
+    codes = rng.choice(16, size=512, p=np.r_[np.full(15, 0.98 / 15), 0.02])
+    sym = (codes[0::2] | (codes[1::2] << 4)).astype(np.uint8)
+    tab = codec.Table(codec.normalize(codec.histogram(sym), 12), 12)
+    lits = rng.integers(0, 256, size=int((codes == 15).sum()))
+    st, words, after = codec.encode_scalar_lit(sym, tab, 16, 16, 65536 + 77, lits)
+    o, l, end, used = codec.decode_scalar_lit(st, words, sym.size, tab, 16, 16)
+    assert np.array_equal(o, sym) and end == 65536 + 77 and used == words.size == after[-1]
+    assert np.array_equal(l[l != 0xFFFF], lits) and np.array_equal(np.flatnonzero(l != 0xFFFF), np.flatnonzero(codes == 15))
+    assert np.all(np.diff(after.astype(np.int64)) >= 0)
+    calm = (np.minimum(sym & 15, 14) | (np.minimum(sym >> 4, 14) << 4)).astype(np.uint8)
+    tab2 = codec.Table(codec.normalize(codec.histogram(calm), 12), 12)
+    s1, w1 = codec.encode_scalar(calm, tab2, 16, 16, 65536)
+    s2, w2, _ = codec.encode_scalar_lit(calm, tab2, 16, 16, 65536, [])
+    assert s1 == s2 and np.array_equal(w1, w2)
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(256, 512, seed=16, jitter=True)).copy()
+    w[5, 17], w[200, 300], w[200, 301] = 0x0001, 0x7F7F, 0x0080
+    coded, raw, exps, table = oc.symbolise_pair(w)
+    cnt = np.bincount(exps.ravel(), minlength=256)
+    assert len(set(table[:15].tolist())) == 15 and min(cnt[table[:15]]) >= max(np.delete(cnt, table[:15]))
+    buf, st = _roundtrip(oc.FMT_BF16_PAIR4, w, 512, tile_k=256, flags=3, tile_n=32)[:2]
+    _, st0 = oc.encode(oc.FMT_BF16, w, 512, tile_k=256, flags=3, tile_n=32)
+    assert 0.0 <= st["bits_per_weight"] - st0["bits_per_weight"] <= 0.03
+    h = oc.Header.unpack(buf)
+    assert np.array_equal(buf[h.off_zeros:h.off_zeros + 16], table)
+
+
 def test_bf16_conversion_against_torch():
     import torch
     x = np.random.default_rng(1).standard_normal(4096).astype(np.float32) * 3
