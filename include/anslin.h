@@ -74,7 +74,7 @@ typedef enum {
 
 #define ANSLIN_FLAG_LANE_STREAMS 2u  /* 32-row tiles only: every lane's 16-bit words are stored as a stream of its own
                                         (two lanes share a region, one ascending, one descending; 20 bytes of region
-                                        sizes per 256 decode steps) instead of interleaved in read order: the decoder
+                                        sizes per segment = 256 decode steps for bf16 / int8, 128 for the other formats) instead of interleaved in read order: the decoder
                                         needs no ballot / prefix count.  Costs ~0.02 bit/weight.  If a tile cannot be
                                         represented (region sizes spread over > 255 words) the encoder silently drops
                                         the flag; anslin_describe reports the flags actually used. */
@@ -219,7 +219,7 @@ double anslin_entropy_weighted(const double *h, const uint64_t *n, int32_t layer
  * GPU-side encoder (S: NEXT-6; the paper names it as future work, P:l.486): compress a row-major W that is resident
  * in HBM into a container in HBM.  Same symbolisation, table normalisation, container layout and decoders as
  * anslin_encode_host; restricted to the lane-stream layout (desc.tile_n = 32, ANSLIN_FLAG_LANE_STREAMS set, tile_k a
- * multiple of 256 decode steps: 256 weights for bf16 / fp8 / int8, 512 for int4 / fp4).  An offline-stage call like
+ * whole number of segments: a multiple of 256 weights for bf16 / int8 / int4 / fp4, of 128 for fp8).  An offline-stage call like
  * anslin_encode_host: it SYNCHRONISES `stream` (the 256-bin histogram and the per-tile record sizes visit the host
  * for the table normalisation and the offset prefix sum; W itself never leaves the device).
  *   w_dev: row-major W as anslin_encode_host takes it, 16-byte aligned.  scales_host / zeros_host: as anslin_encode_host.

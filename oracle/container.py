@@ -41,9 +41,9 @@ WEIGHTS_PER_SYMBOL = {FMT_BF16: 1, FMT_FP8_E4M3: 1, FMT_INT8: 1, FMT_INT4_AWQ: 2
 
 
 def seg_steps(fmt: int) -> int:
-    """Decode steps per lane-stream segment: 8192 weights of a 32-row tile in every format that codes one symbol per
-    weight (256 steps); the bf16 pair variant decodes two weights per step (128 steps)."""
-    return SEG_STEPS // 2 if fmt == FMT_BF16_PAIR4 else SEG_STEPS
+    """Decode steps per lane-stream segment: 256 where a symbol carries few bits (bf16 exponents, SQ8), 128 where it
+    carries 6-7 bits (fp8, packed 4-bit pairs, bf16 exponent pairs): a segment is what the decoder stages at once."""
+    return SEG_STEPS if fmt in (FMT_BF16, FMT_INT8) else SEG_STEPS // 2
 
 
 def _align(x: int, a: int = 16) -> int:
@@ -466,7 +466,7 @@ def decode(buf: np.ndarray):
                 used = (e - a - 4 * LANES) // 2
                 lit_all[r0:r0 + tile_n, kt * tile_k:(kt + 1) * tile_k] = lit.T
             elif h.flags & FLAG_LANE_STREAMS:
-                sym, end = _lane_record_decode(buf[a:e], steps, tab)
+                sym, end = _lane_record_decode(buf[a:e], steps, tab, seg_steps(fmt))
                 sym = sym.reshape(-1)
                 used = (e - a - 4 * LANES) // 2
             else:

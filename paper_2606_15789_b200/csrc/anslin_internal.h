@@ -41,8 +41,10 @@ static_assert(sizeof(Header) == kHeaderBytes, "header must be 128 bytes");
 constexpr uint32_t kFormatMax = ANSLIN_FMT_BF16_PAIR4;
 // stored as 16-bit bf16 values; the sign + mantissa byte of every weight lives in the raw plane
 ANSLIN_HD constexpr bool is_bf16_like(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_BF16_PAIR4; }
-// decode steps per lane-stream segment: 8192 weights of a 32-row tile (the pair variant decodes two weights per step)
-ANSLIN_HD constexpr int seg_steps_of(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16_PAIR4 ? 128 : 256; }
+// Decode steps per lane-stream segment (a segment is staged whole in shared memory, and costs a 20-byte table): 256 for the
+// formats whose symbols carry few bits (bf16 exponents 2.6 bit, SQ8 4.5 bit), 128 where a symbol carries 6-7 bits (fp8, the
+// packed 4-bit pairs, the bf16 exponent pairs) so that a staged segment stays near 3 KB and 16 decoder warps fit.
+ANSLIN_HD constexpr int seg_steps_of(uint32_t fmt) { return (fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT8) ? 256 : 128; }
 ANSLIN_HD constexpr bool is_fp8(uint32_t fmt) { return fmt == ANSLIN_FMT_FP8_E4M3 || fmt == ANSLIN_FMT_FP8_E5M2; }
 // formats whose MMA runs in kind::f8f6f4 with a per-tensor weight scale and fp8 activations (fp4 is expanded to e4m3)
 ANSLIN_HD constexpr bool is_fp8_path(uint32_t fmt) { return is_fp8(fmt) || fmt == ANSLIN_FMT_FP4_E2M1; }

@@ -27,10 +27,10 @@ bool normalise_freqs(const uint64_t *cnt, uint32_t *f);   // host.cpp
 namespace {
 
 constexpr int kEncWarps = 4;
-constexpr int kMaxSeg = 4;   // tile_k <= 1024 weights -> at most 1024 steps = 4 segments
+constexpr int kMaxSeg = 8;   // tile_k <= 1024 weights -> at most 1024 steps = 8 segments of 128
 
 struct EncGeom {
-  uint32_t fmt, flags, n_tiles, KT, steps, nseg;
+  uint32_t fmt, flags, n_tiles, KT, steps, nseg, seg /*steps per segment*/;
   uint32_t es;            // bytes of one coded symbol's source element along a row: bf16 2, every other format 1
   uint64_t row_bytes;     // bytes of one row of W
   uint32_t raw_tile_bytes;
@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(kEncWarps * 32) enc_count_kernel(EncGeom g, co
     bool bad = false;
     for (int sg = int(g.nseg) - 1; sg >= 0; --sg) {
       uint32_t c = 0, word;
-      for (int t = sg * kSegSteps + kSegSteps - 1; t >= sg * kSegSteps; --t) c += enc_step(x, stab[coded_at(g, row, t)], word) ? 1u : 0u;
+      for (int t = (sg + 1) * int(g.seg) - 1; t >= sg * int(g.seg); --t) c += enc_step(x, stab[coded_at(g, row, t)], word) ? 1u : 0u;
       counts[(size_t(tile) * g.nseg + sg) * 32 + lane] = uint16_t(c);
       const uint32_t pair = c + __shfl_xor_sync(0xffffffffu, c, 1), total = warp_sum(c);
       bad |= warp_max(pair) - warp_min(pair) > 255u || total > 0xFFFFu;
@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(kEncWarps * 32) enc_write_kernel(EncGeom g, co
     for (int sg = kMaxSeg - 1; sg >= 0; --sg) {
       if (sg < int(g.nseg)) {
         uint32_t at = cur[sg], word;
-        for (int t = sg * kSegSteps + kSegSteps - 1; t >= sg * kSegSteps; --t) {
+        for (int t = (sg + 1) * int(g.seg) - 1; t >= sg * int(g.seg); --t) {
           if (enc_step(x, stab[coded_at(g, row, t)], word)) {
             *reinterpret_cast<uint16_t *>(rec + at) = uint16_t(word);
             at += uint32_t(dir);
@@ -204,8 +204,10 @@ bool enc_geometry(const anslin_desc *d, EncGeom *g, uint32_t *n_out, uint32_t *k
   const uint32_t wps = uint32_t(weights_per_symbol(d->format));
   g->fmt = d->format; g->flags = d->flags;
   g->steps = tile_k / wps;
-  if (g->steps % kSegSteps) return false;
-  g->nseg = g->steps / kSegSteps;
+  g->seg = uint32_t(seg_steps_of(d->format));
+  if (g->steps % g->seg) return false;
+  g->nseg = g->steps / g->seg;
+  if (g->nseg > uint32_t(kMaxSeg) || d->format == ANSLIN_FMT_BF16_PAIR4) return false;   // (the pair variant is host-encoded only)
   g->KT = d->k_in / tile_k;
   g->n_tiles = (d->n_out / kTileN) * g->KT * 4u;
   g->es = d->format == ANSLIN_FMT_BF16 ? 2u : 1u;
