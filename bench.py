@@ -139,6 +139,92 @@ def run_reference(args):
 ALU_INSTR_PER_SYMBOL = 10.0
 
 
+def run_other_config(args):
+    """--workload c3 | c4 | c5: the other BASELINE.json configs (parity-test cases; DESIGN.md §8 table), one launch of
+    the fused kernel per step on the config's largest matrix (c5: all 8 experts of the grouped gate GEMM).  Same JSON
+    keys as the headline line; a diagnostic, not the line the driver reads (the default workload stays config 2)."""
+    import torch
+    from paper_2606_15789_b200 import binding as B, build as libbuild, inputs, runtime as rt
+    libbuild.build()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: anslin has no CPU fallback")
+    torch.cuda.set_device(0)
+    tile_n, tile_k, lflag = 32, 1024, B.FLAG_LANE_STREAMS
+    if args.workload == "c3":
+        n, k, m = 13824, 5120, 75
+        q, s8 = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=5, jitter=True))
+        xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=6))
+        buf, st = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=tile_k, scales=s8, tile_n=tile_n, flags=lflag)
+        copies = [rt.DeviceWeight(buf) for _ in range(6)]          # 6 x 41 MB > L2
+        x, xsd = rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()
+        y = torch.empty((m, n), dtype=torch.float32, device="cuda")
+        calls = [(lambda d=d: d.gemm(x, xsd, y)) for d in copies]
+        name, dtype, nbytes, nw, flops = "config3: SQ8 int8 gate 13824x5120, M=75", "int8", buf.size, n * k, 2.0 * m * n * k
+        x_host, y_rows = torch.from_numpy(xq).pin_memory(), m
+    elif args.workload == "c4":
+        n, k, m = 28672, 8192, 64
+        p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=11, outliers=False), 128)
+        xh = inputs.acts_f32(m, k, seed=12).astype(np.float16)
+        buf, st = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=tile_k, scales=s4, zeros=z4, group_size=128, tile_n=tile_n, flags=lflag)
+        copies = [rt.DeviceWeight(buf) for _ in range(3)]          # 3 x 125 MB > L2
+        x, y = rt.x_to_device(B.FMT_INT4_AWQ, xh), torch.empty((m, n), dtype=torch.float32, device="cuda")
+        calls = [(lambda d=d: d.gemm(x, None, y)) for d in copies]
+        name, dtype, nbytes, nw, flops = "config4: AWQ int4 g128 gate 28672x8192, M=64", "f16", buf.size, n * k, 2.0 * m * n * k
+        x_host, y_rows = torch.from_numpy(xh).pin_memory(), m
+    else:
+        n, k, E, tokens = 16384, 6144, 8, 95
+        rows, tok = inputs.route_top2(tokens, E, seed=21)
+        x8t, xst = inputs.quant_fp8_acts(inputs.acts_f32(tokens, k, seed=22))
+        x8, xs = x8t[tok], xst[tok]
+        experts, nbytes = [], 0
+        for e in range(E):
+            f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=30 + e, std=0.015, outliers=False))
+            buf, st = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=tile_k, w_scale=sc, tile_n=tile_n, flags=lflag)
+            experts.append(rt.DeviceWeight(buf)); nbytes += buf.size      # 8 x 83 MB > L2
+        x, xsd = rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()
+        y = torch.empty((2 * tokens, n), dtype=torch.float32, device="cuda")
+        calls = [lambda: rt.gemm_grouped(experts, rows, x, xsd, y)]
+        name, dtype, nw, flops = "config5: Mixtral-shaped MoE, 8 experts fp8 gate 16384x6144, 95 tokens top-2", "fp8", E * n * k, 2.0 * 2 * tokens * n * k
+        x_host, y_rows = torch.from_numpy(x8).pin_memory(), 2 * tokens
+    y_host = torch.empty((y_rows, n), dtype=torch.float32).pin_memory()
+    sampler = ClockSampler(0); sampler.start(); sampler.wait_first()
+    for i in range(max(args.warmup, 3)):
+        calls[i % len(calls)]()
+    torch.cuda.synchronize()
+    lo = sampler.mark()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches = 0
+    e0.record()
+    for i in range(args.steps):
+        calls[i % len(calls)]()
+        launches += B.anslin_last_launch_count()
+    e1.record(); torch.cuda.synchronize()
+    time.sleep(0.03)
+    clocks = sampler.stop(lo, sampler.mark())
+    ms = e0.elapsed_time(e1) / args.steps
+    t0 = time.perf_counter()
+    for i in range(args.steps):                      # e2e: pinned X in, Y out every step
+        x.view(torch.uint8).copy_(x_host.view(torch.uint8), non_blocking=True)
+        calls[i % len(calls)]()
+        y_host.copy_(y, non_blocking=True)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / args.steps
+    hbm_peak, _, kind = peaks()
+    algo = nbytes + x.numel() * x.element_size() + y.numel() * 4
+    print(json.dumps({"metric": METRIC, "value": flops / (ms * 1e-3) / 1e12, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+                      "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": dtype, "data": "synthetic",
+                      "config": {"workload": name, "tile": "%dx%d" % (tile_n, tile_k), "word_layout": "lanes",
+                                 "l2_policy": "rotating copies / experts larger than L2"},
+                      "clocks": clocks, "gpu_launches": launches,
+                      "e2e": {"value": flops / e2e_s / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(x.numel() * x.element_size()),
+                              "d2h_bytes_per_step": int(y.numel() * 4)},
+                      "roofline": {"bound": "hbm", "achieved": algo / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                                   "frac": algo / (ms * 1e-3) / 1e9 / hbm_peak, "traffic": None, "peak_kind": "of " + kind},
+                      "gsym_per_s": nw / (2 if args.workload == "c4" else 1) / (ms * 1e-3) / 1e9,
+                      "bits_per_weight": st["bits_per_weight"]}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -153,11 +239,15 @@ def main():
     ap.add_argument("--symbols", default="paper", choices=["paper", "pair4"], help="paper = one coded symbol per weight (PAPER.md's "
                     "symbolisation, the headline); pair4 = the variant that codes two K-adjacent bf16 exponents per symbol "
                     "(SURVEY 8(f) NEXT-5, ANSLIN_FMT_BF16_PAIR4; lanes layout only)")
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3", "c4", "c5"], help="c2 = the headline (BASELINE config 2); c3 / c4 / c5 = "
+                    "diagnostic lines for the other configs (int8, int4, fp8 MoE)")
     ap.add_argument("--group", default="qkv,o,gateup,down", help="launch grouping of the 7 projections: 'each' = 7 launches, or "
                     "comma-separated groups out of qkv / q,k,v / gateup / gate,up / o / down (projections that share an input)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload != "c2":
+        return run_other_config(args)
 
     import torch
     from paper_2606_15789_b200 import binding as B, build as libbuild, inputs, runtime as rt
