@@ -543,6 +543,29 @@ def _sample_cols(n, seed, count=512):
     return np.sort(np.random.default_rng(seed).choice(n, size=min(n, count), replace=False))
 
 
+def test_pair_variant_and_device_encoder_full_size():
+    """The two widened paths at a BASELINE config 2 shape (o: 5120 x 5120, M = 47) in the launch configuration
+    bench.py times: the bf16 pair variant decodes bit-exactly and multiplies in tolerance, with its own size gap
+    stated; the GPU-side encoder reproduces the host encoder's container byte for byte."""
+    rt = _rt()
+    import torch
+    n, k, m = 5120, 5120, 47
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=17, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=18))
+    buf, st = B.anslin_encode_host(B.FMT_BF16_PAIR4, w, n, k, tile_k=256, flags=3, tile_n=32)
+    buf0, st0 = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
+    assert 0.0 < st["bits_per_weight"] - st0["bits_per_weight"] < 0.03
+    dw = rt.DeviceWeight(buf)
+    assert np.array_equal(dw.decode().cpu().numpy().view(np.uint16), w)
+    cols = np.sort(np.random.default_rng(19).choice(n, size=1024, replace=False))
+    y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    check_gemm(y[:, cols], *og.gemm_bf16(x, w[cols]))
+    dw.close()
+    de = rt.encode_on_device(B.FMT_BF16, torch.from_numpy(w.view(np.int16)).cuda(), n, k, tile_k=256, flags=3)
+    assert np.array_equal(de.container_dev.cpu().numpy(), buf0)
+    de.close()
+
+
 @pytest.mark.parametrize("lay", [(128, 256, 0), (32, 1024, 2)], ids=["128x256", "32x1024-lanes"])
 def test_config3_int8_full_size(lay):
     """BASELINE config 3: Qwen-14B gate projection 13824 x 5120 in SQ8-style int8, M = 75: decode bit-exact on the
