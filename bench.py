@@ -439,7 +439,20 @@ def main():
         t = a.elapsed_time(b) / 5
         out["dense_uncompressed"] = {"ms": round(t, 4), "tflops": round(flops_step / (t * 1e-3) / 1e12, 3),
                                      "hbm_gbs": round(n_weights * 2 / (t * 1e-3) / 1e9, 1)}
-        del wd
+        # context only (SURVEY 8(d) "torch.matmul may be printed as extra context"): the same seven GEMMs through cuBLAS
+        wt = [t.view(torch.bfloat16) for t in wd]
+        for _ in range(3):
+            for i in range(len(layer)):
+                torch.matmul(xs[i], wt[i].t())
+        torch.cuda.synchronize(); a.record()
+        for _ in range(5):
+            for i in range(len(layer)):
+                torch.matmul(xs[i], wt[i].t())
+        b.record(); torch.cuda.synchronize()
+        t = a.elapsed_time(b) / 5
+        out["dense_cublas_context"] = {"ms": round(t, 4), "tflops": round(flops_step / (t * 1e-3) / 1e12, 3),
+                                       "hbm_gbs": round(n_weights * 2 / (t * 1e-3) / 1e9, 1), "note": "torch.matmul, bf16 out; context, not the comparator"}
+        del wd, wt
         a.record()
         for _ in range(3):
             for dw in dws:
