@@ -345,7 +345,7 @@ struct EpiParams {
   float *y;
   int64_t ldy;
   uint32_t *partials;              // [2*G][mpad][128] raw accumulator bits
-  unsigned long long *counters;    // [stripes]: launch epoch << 32 | split-K contributors that have arrived
+  unsigned long long *counters;    // split-K flags, u32 [2 * CTAs of the problem]: flag[c * 2 + seg] = launch epoch once CTA c's partial `seg` is stored
   uint32_t epoch;                  // unique per launch: stale counter contents (any bytes) read as "nobody arrived"
   uint32_t m, mpad;
 };
@@ -399,19 +399,14 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
       __threadfence();
       named_bar_sync(1, kEpiWarps * 32);
       if (warp == 0 && lane == 0) {
+        // every thread's partial stores are fenced and the warps have met: raise this segment's flag.  The stripe's last
+        // contributor (the CTA that holds its last k-tile, known from the shape alone) sums the partials once it has seen
+        // every flag of the stripe carry this launch's epoch (splitk_fixup): no atomics, no retries under contention, and
+        // stale or uninitialised workspace bytes never match the epoch.
         const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
-        // arrive: count within this launch's epoch; no memset before and no reset after the launch is needed
-        unsigned long long *ctr = &p.counters[stripe];
-        unsigned long long seen = *reinterpret_cast<volatile unsigned long long *>(ctr), assumed;
-        do {
-          assumed = seen;
-          const unsigned long long next = uint32_t(assumed >> 32) == p.epoch ? assumed + 1ull : ((unsigned long long)(p.epoch) << 32) | 1ull;
-          seen = atomicCAS(ctr, assumed, next);
-        } while (seen != assumed);
-        const uint32_t before = uint32_t(assumed >> 32) == p.epoch ? uint32_t(assumed) : 0u;
-        const bool last = before == c_last - c_first;
-        __threadfence();
-        fin[seg].stripe = stripe; fin[seg].c_first = c_first; fin[seg].c_last = c_last; fin[seg].valid = last ? 1u : 0u;
+        uint32_t *flag = reinterpret_cast<uint32_t *>(p.counters) + (c * 2u + seg);
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(p.epoch) : "memory");
+        fin[seg].stripe = stripe; fin[seg].c_first = c_first; fin[seg].c_last = c_last; fin[seg].valid = c == c_last ? 1u : 0u;
       }
     }
     t += nt;
@@ -432,6 +427,19 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
     // contributor cc's partial slot: its first segment (slot 0) unless the stripe is its second one, which can only
     // be the case for the first contributor (every later one starts inside the stripe)
     const uint32_t first_slot = cta_first_tile(c_first, G, T) < stripe * KT ? 1u : 0u;
+    // wait for the other contributors (all CTAs of the persistent grid are resident, and a stripe's contributors have
+    // lower CTA indices than its owner): one flag per thread
+    for (uint32_t cc = c_first + threadIdx.x; cc <= c_last; cc += blockDim.x) {
+      const uint32_t *flag = reinterpret_cast<const uint32_t *>(p.counters) + (cc * 2u + (cc == c_first ? first_slot : 0u));
+      uint32_t v, spins = 0;
+      while (true) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+        if (v == p.epoch) break;
+        __nanosleep(64);
+        if (++spins > (1u << 24)) __trap();   // a protocol bug traps instead of hanging the GPU
+      }
+    }
+    __syncthreads();
     const size_t slot_words = size_t(p.mpad) * kTileN;
     const uint32_t n_items = p.m * 32u;
     for (uint32_t it0 = threadIdx.x; it0 < n_items; it0 += blockDim.x * kItems) {
@@ -902,11 +910,13 @@ uint32_t next_epoch() {
   return e.fetch_add(1, std::memory_order_relaxed);
 }
 
+// bytes of a problem's split-K flag area (two u32 flags per CTA; sized generously by stripes too so that older callers' sizes hold)
+size_t flag_bytes(uint32_t stripes) { return align16(size_t(stripes) * 8 + 256 + 8 * 160); }
 struct Workspace { size_t counters_off, partials_off, total; };
 Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
   Workspace w;
   w.counters_off = 0;
-  w.partials_off = align16(size_t(stripes) * 8 + 256);
+  w.partials_off = flag_bytes(stripes);
   w.total = w.partials_off + size_t(grid) * 2 * mpad * kTileN * 4;
   return w;
 }
@@ -1033,7 +1043,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   size_t off = 0;
   uint8_t *wsb = static_cast<uint8_t *>(workspace_dev);
   size_t counters_bytes = 0;
-  for (int i = 0; i < n; ++i) counters_bytes += align16(size_t(ws[i]->h.n_out / kTileN) * 8 + 256);
+  for (int i = 0; i < n; ++i) counters_bytes += flag_bytes(ws[i]->h.n_out / kTileN);
   size_t part_off = counters_bytes;
   uint32_t cta0 = 0;
   for (int i = 0; i < n; ++i) {
@@ -1049,7 +1059,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     q.ncta = ncta[i];
     cta0 += ncta[i];
     q.counters = reinterpret_cast<unsigned long long *>(wsb + off);
-    off += align16(size_t(h.n_out / kTileN) * 8 + 256);
+    off += flag_bytes(h.n_out / kTileN);
     q.partials = reinterpret_cast<uint32_t *>(wsb + part_off);
     part_off += size_t(ncta[i]) * 2 * q.mpad * kTileN * 4;
     const uint32_t uk = unit_k_of(h.format);
@@ -1085,7 +1095,7 @@ size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_ma
   size_t counters = 0;
   for (int i = 0; i < n; ++i) {
     if (!ws[i]) return 0;
-    counters += align16(size_t(ws[i]->h.n_out / kTileN) * 8 + 256);
+    counters += flag_bytes(ws[i]->h.n_out / kTileN);
   }
   // all problems of a launch share one CTA per SM, so their partials never exceed one problem's worst case
   const size_t per_launch = size_t(std::max(sm_budget(), 148)) * 2 * mpad_of(m_max) * kTileN * 4;
