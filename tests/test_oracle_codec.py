@@ -196,3 +196,51 @@ def test_compressed_size_tracks_entropy():
     ideal = float(np.sum(np.log2(4096.0 / f[msg])))
     written = 32 + 16 * len(words)
     assert ideal <= written <= ideal + 32 + 0.001 * ideal
+
+
+# ------------------------------------------------------------------------------------------------
+# Property tests (hypothesis): any histogram, any stream, any legal start state
+# ------------------------------------------------------------------------------------------------
+from hypothesis import given, settings, strategies as st_
+
+
+@settings(max_examples=60, deadline=None)
+@given(st_.lists(st_.integers(0, 255), min_size=1, max_size=600), st_.integers(0, 0xFFFF))
+def test_property_scalar_round_trip_and_size(sym_list, payload):
+    """For ANY symbol sequence: the scalar rANS stream decodes to the sequence, ends in its start state (any state in
+    [L, 2L) is a legal start, reading A4), and its size is within the coder's worst case of the table's cross entropy."""
+    sym = np.array(sym_list, dtype=np.uint8)
+    cnt = codec.histogram(sym)
+    f = codec.normalize(cnt, 12)
+    assert int(f.sum()) == 4096 and np.all(f[cnt > 0] >= 1) and np.all(f[cnt == 0] == 0) | (np.count_nonzero(cnt) == 1)
+    tab = codec.Table(f, 12)
+    x_init = (1 << 16) + payload
+    state, words = codec.encode_scalar(sym, tab, 16, 16, x_init)
+    out, end, used = codec.decode_scalar(state, words, sym.size, tab, 16, 16)
+    assert np.array_equal(out, sym) and end == x_init and used == words.size
+    assert (1 << 16) <= state < (1 << 32)
+    ideal = codec.cross_entropy(cnt, f, 12) * sym.size          # bits
+    assert 16 * words.size + 32 >= ideal - 1e-6                 # never below the table's own bound (state bits included)
+    assert 16 * words.size <= ideal + 32 + 16                   # at most the start state's bits and one word of slack above it
+
+
+@settings(max_examples=40, deadline=None)
+@given(st_.lists(st_.integers(0, 15), min_size=8, max_size=512).filter(lambda v: len(v) % 8 == 0), st_.data())
+def test_property_pair_stream_with_literals(code_list, data):
+    """bf16 pair variant's lane stream: for ANY sequence of 4-bit codes (15 = escape) and ANY literals the stream round
+    trips, every literal returns at its own nibble, and literal words sit after the renormalisation of their 4-step chunk."""
+    codes = np.array(code_list, dtype=np.uint8)
+    sym = (codes[0::2] | (codes[1::2] << 4)).astype(np.uint8)
+    n_esc = int((codes == 15).sum())
+    lits = np.array(data.draw(st_.lists(st_.integers(0, 255), min_size=n_esc, max_size=n_esc)), dtype=np.uint16)
+    tab = codec.Table(codec.normalize(codec.histogram(sym), 12), 12)
+    state, words, after = codec.encode_scalar_lit(sym, tab, 16, 16, 1 << 16, lits)
+    out, lit, end, used = codec.decode_scalar_lit(state, words, sym.size, tab, 16, 16)
+    assert np.array_equal(out, sym) and end == (1 << 16) and used == words.size == int(after[-1])
+    assert np.array_equal(lit[codes == 15], lits) and np.all(lit[codes != 15] == 0xFFFF)
+    plain_state, plain_words = codec.encode_scalar(sym, tab, 16, 16, 1 << 16)
+    assert plain_state == state and words.size == plain_words.size + n_esc       # literals are the only extra words
+    # the words consumed inside a chunk before its last step never include that chunk's literals
+    esc_per_chunk = (codes.reshape(-1, 8) == 15).sum(axis=1)
+    rn = np.diff(np.concatenate([[0], after.astype(np.int64)]))
+    assert np.all(rn.reshape(-1, 4)[:, :3] <= 1) and np.all(rn.reshape(-1, 4)[:, 3] <= 1 + esc_per_chunk)
