@@ -157,6 +157,7 @@ size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, in
  *   or FP8_E5M2 (the tensor core multiplies the two fp8 kinds in any combination).
  *   x_scale_dev: int8/fp8: f32[m] per-token scales; else NULL.
  *   y_dev: f32 [m x n_out]; int8: acc * x_scale[m] * w_scale[n]; fp8: acc * x_scale[m] * desc.w_scale.
+ *   The launch may be captured in a CUDA graph and replayed (workspace and buffers must stay where they were).
  *   m >= 1.  m <= 256 is the regime the kernel is built for (P:l.295-306).  A larger m is processed in blocks of 256 rows,
  *   every block a problem of its own in one persistent launch (8 blocks per launch): each block decodes W again.
  */

@@ -438,6 +438,8 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
         __nanosleep(64);
         if (++spins > (1u << 24)) __trap();   // a protocol bug traps instead of hanging the GPU
       }
+      // consumed: clear the flag, so that a replay of this very launch (CUDA graph: same epoch) starts from "not stored"
+      *const_cast<volatile uint32_t *>(flag) = 0u;
     }
     __syncthreads();
     const size_t slot_words = size_t(p.mpad) * kTileN;
@@ -907,7 +909,9 @@ uint32_t grid_of(uint32_t n_tiles, uint32_t min_tiles) {
 // owner of the workspace left behind (seeded from the clock), so the workspace never has to be cleared.
 uint32_t next_epoch() {
   static std::atomic<uint32_t> e{uint32_t(std::chrono::steady_clock::now().time_since_epoch().count()) | 1u};
-  return e.fetch_add(1, std::memory_order_relaxed);
+  uint32_t v = e.fetch_add(1, std::memory_order_relaxed);
+  if (v == 0) v = e.fetch_add(1, std::memory_order_relaxed);   // 0 means "flag cleared"
+  return v;
 }
 
 // bytes of a problem's split-K flag area (two u32 flags per CTA; sized generously by stripes too so that older callers' sizes hold)

@@ -162,6 +162,34 @@ def test_gemm_bf16_max_batch_and_strided_buffers(m, tile):
     dw.close()
 
 
+def test_gemm_replayed_from_a_cuda_graph():
+    """A captured launch is replayed with its kernel parameters frozen, the split-K epoch among them: the stripe owner
+    clears the flags it consumed, so every replay starts from "not stored" and sums this replay's partials."""
+    rt = _rt()
+    import torch
+    n, k, m = 640, 2048, 33           # 8 k-tiles per stripe over many CTAs: every stripe is split
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=131, jitter=True))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
+    dw = rt.DeviceWeight(buf)
+    xd = torch.zeros((m, k), dtype=torch.bfloat16, device="cuda")
+    y = torch.zeros((m, n), dtype=torch.float32, device="cuda")
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        dw.gemm(xd, None, y)              # warm-up outside the capture: workspace allocation, function attributes
+    torch.cuda.current_stream().wait_stream(side)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        dw.gemm(xd, None, y)
+    for trial in range(3):
+        x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=140 + trial))
+        xd.copy_(rt.x_to_device(B.FMT_BF16, x))
+        g.replay()
+        torch.cuda.synchronize()
+        check_gemm(y.cpu().numpy(), *og.gemm_bf16(x, w))
+    dw.close()
+
+
 @pytest.mark.parametrize("m", [257, 600, 2304])
 def test_gemm_bf16_large_m(m):
     """S: §8(f) NEXT-1 (prefill-sized batches, P:l.392): m > 256 runs as blocks of 256 rows, 8 blocks per launch
