@@ -695,19 +695,6 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
     // ~0.3 us): descriptors are advanced by adds, segment bookkeeping is hoisted out of the unit loop
     const uint64_t adesc0 = make_smem_desc(slots_s, 16, 256, kLayoutSW32);
     const uint32_t desc_hi = uint32_t(adesc0 >> 32), adesc0_lo = uint32_t(adesc0), slot_units = P.slot_bytes >> 4;
-    auto consume = [&](uint32_t slot, uint32_t par, uint32_t d_tmem, uint32_t accumulate, bool last, uint32_t tfull_bar) {
-      if (rel < n_commit) release(n_commit, false);
-      mbar_wait(full_s + 8 * slot, par);
-      tc_fence_after();
-      if (lane == 0) {
-        const uint32_t alo = adesc0_lo + slot * slot_units;   // start address field: (slots_s + slot * slot_bytes) >> 4
-        const uint64_t ad = (uint64_t(desc_hi) << 32) | alo, bd = (uint64_t(desc_hi) << 32) | (alo + (kUnitBytes >> 4));
-        umma<TR::kind>(d_tmem, ad, bd, idesc, accumulate);
-        umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
-        if (last) umma_commit(tfull_bar);
-      }
-      __syncwarp();
-    };
     for (uint32_t rho = 0; rho * PT < N; ++rho) {
       const uint32_t ga = rho * PT, gb = min(N, ga + PT);
       for (uint32_t i0 = ga; i0 < gb;) {
@@ -728,17 +715,28 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
         uint32_t n_unit = rho * units, bsel = n_unit % P.B, par = (n_unit / P.B) & 1u;
         for (uint32_t u = 0; u < units; ++u) {
           const bool lastu = u + 1 == units;
-          uint32_t slot = (i0 - ga) * P.B + bsel;
-          for (uint32_t i = i0; i < e1; ++i, slot += P.B) {
-            const bool last = lastu && i == last1;
-            consume(slot, par, d1, (u == 0 && i == first1) ? 0u : 1u, last, tf1);
-            if (last) ++n_commit;
+          // One unit ROW of the window at a time: lane l waits for the full barrier of group i0 + l (all of them in
+          // parallel, instead of one barrier round trip per unit), then one thread issues the row's MMAs back to back.
+          if (rel < n_commit) release(n_commit, false);
+          const uint32_t slot0 = (i0 - ga) * P.B + bsel, nrow = e2 - i0;
+          if (uint32_t(lane) < nrow) mbar_wait(full_s + 8 * (slot0 + uint32_t(lane) * P.B), par);
+          __syncwarp();
+          tc_fence_after();
+          if (lane == 0) {
+            uint32_t slot = slot0;
+            for (uint32_t i = i0; i < e2; ++i, slot += P.B) {
+              const bool run1 = i < e1;
+              const bool last = lastu && i == (run1 ? last1 : last2);
+              const uint32_t accumulate = (u == 0 && i == (run1 ? first1 : e1)) ? 0u : 1u;
+              const uint32_t alo = adesc0_lo + slot * slot_units;   // start address field: (slots_s + slot * slot_bytes) >> 4
+              const uint64_t ad = (uint64_t(desc_hi) << 32) | alo, bd = (uint64_t(desc_hi) << 32) | (alo + (kUnitBytes >> 4));
+              umma<TR::kind>(run1 ? d1 : d2, ad, bd, idesc, accumulate);
+              umma_commit(empty_s + 8 * slot);  // frees the slot when the MMA has read it
+              if (last) umma_commit(run1 ? tf1 : tf2);
+            }
           }
-          for (uint32_t i = e1; i < e2; ++i, slot += P.B) {
-            const bool last = lastu && i == last2;
-            consume(slot, par, d2, (u == 0 && i == e1) ? 0u : 1u, last, tf2);
-            if (last) ++n_commit;
-          }
+          __syncwarp();
+          if (lastu) n_commit += (last1 >= i0 && last1 < e1 ? 1u : 0u) + (last2 >= e1 && last2 < e2 ? 1u : 0u);
           if (++bsel == P.B) { bsel = 0; par ^= 1u; }
         }
         i0 = e2;
