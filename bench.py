@@ -355,9 +355,10 @@ def main():
     y_ready = [torch.cuda.Event() for _ in groups]
     y_read = [torch.cuda.Event() for _ in groups]
 
-    def step_e2e():
+    def step_e2e(calls_=None, ys_=None, ys_host_=None):
+        calls_, ys_, ys_host_ = calls_ or calls, ys_ or ys, ys_host_ or ys_host
         main = torch.cuda.current_stream()
-        for gi, (g, call) in enumerate(zip(groups, calls)):
+        for gi, (g, call) in enumerate(zip(groups, calls_)):
             for o in sorted({x_owner[i] for i in g}):
                 xs_dev[o].view(torch.int16).copy_(xs_host[o], non_blocking=True)
             main.wait_event(y_read[gi])
@@ -366,7 +367,7 @@ def main():
             copy_stream.wait_event(y_ready[gi])
             with torch.cuda.stream(copy_stream):
                 for i in g:
-                    ys_host[i].copy_(ys[i], non_blocking=True)
+                    ys_host_[i].copy_(ys_[i], non_blocking=True)
                 y_read[gi].record(copy_stream)
     for _ in range(3):
         step_e2e()
@@ -406,6 +407,20 @@ def main():
            "per_launch_us": {nm: round(1e3 * float(t), 2) for nm, t in zip(group_names, kern_ms_mean)}}
 
     if rank == 0 and not args.no_extras:
+        # the same end-to-end step with Y produced in bf16 (anslin_gemm_multi_ex): half the device-to-host bytes
+        ys_b = [torch.empty((m, n), dtype=torch.bfloat16, device="cuda") for (_, n, k, _) in layer]
+        ys_host_b = [torch.empty((m, n), dtype=torch.bfloat16).pin_memory() for (_, n, k, _) in layer]
+        calls_b = [rt.MultiGemm([dws[i] for i in g], [xs[i] for i in g], None, [ys_b[i] for i in g]) for g in groups]
+        for _ in range(3):
+            step_e2e(calls_b, ys_b, ys_host_b)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            step_e2e(calls_b, ys_b, ys_host_b)
+        barrier()
+        tb = time.perf_counter() - t0
+        out["e2e_y_bf16"] = {"value": flops_step * args.steps / tb / 1e12, "unit": UNIT,
+                             "h2d_bytes_per_step": e2e["h2d_bytes_per_step"], "d2h_bytes_per_step": int(sum(m * n * 2 for (_, n, k, _) in layer))}
         # per-M table (BASELINE config 2: M in {1,16,47,75}), dense comparator, decode-only; then the CPU oracle leg
         extra = {}
         for mm in (1, 16, 47, 75):

@@ -177,6 +177,12 @@ int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void
                       uint32_t x_dtype, const int64_t *ldx, const int32_t *m,
                       const void *const *x_scale_dev, void *const *y_dev, const int64_t *ldy,
                       void *workspace_dev, size_t workspace_bytes, void *stream);
+/* The same with the element type of every Y chosen: ANSLIN_DT_F32 (as anslin_gemm_multi) or ANSLIN_DT_BF16 (the fp32
+ * result rounded to nearest even; ldy in elements of that type; rows 8-byte aligned for vector stores, else scalar). */
+int anslin_gemm_multi_ex(const anslin_weight *const *weights, int32_t n, const void *const *x_dev,
+                         uint32_t x_dtype, const int64_t *ldx, const int32_t *m,
+                         const void *const *x_scale_dev, void *const *y_dev, uint32_t y_dtype,
+                         const int64_t *ldy, void *workspace_dev, size_t workspace_bytes, void *stream);
 
 /*
  * Grouped fused decode-GEMM over MoE experts (BASELINE config 5): rows of X already sorted by

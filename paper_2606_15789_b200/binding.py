@@ -22,7 +22,7 @@ X_DTYPE = {FMT_BF16: DT_BF16, FMT_FP8_E4M3: DT_FP8_E4M3, FMT_INT8: DT_I8, FMT_IN
 
 EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_close", "anslin_describe",
            "anslin_decode", "anslin_gemm_workspace_bytes", "anslin_gemm_multi_workspace_bytes", "anslin_gemm",
-           "anslin_gemm_multi", "anslin_gemm_grouped",
+           "anslin_gemm_multi", "anslin_gemm_multi_ex", "anslin_gemm_grouped",
            "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_histogram", "anslin_entropy_bits",
            "anslin_entropy_weighted", "anslin_encode_device_workspace_bytes", "anslin_encode_device_head_bytes",
            "anslin_encode_device", "anslin_last_launch_count", "anslin_status_string"]
@@ -70,6 +70,8 @@ def lib() -> ctypes.CDLL:
         L.anslin_gemm_multi_workspace_bytes.restype = sz
         L.anslin_gemm_multi.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(vp), u32, ctypes.POINTER(i64), ctypes.POINTER(i32),
                                         ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i64), vp, sz, vp]
+        L.anslin_gemm_multi_ex.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(vp), u32, ctypes.POINTER(i64), ctypes.POINTER(i32),
+                                           ctypes.POINTER(vp), ctypes.POINTER(vp), u32, ctypes.POINTER(i64), vp, sz, vp]
         L.anslin_gemm_grouped.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(i32), vp, u32, i64, vp, vp, i64, vp, sz, vp]
         L.anslin_dense_workspace_bytes.argtypes = [u32, u32, i32]; L.anslin_dense_workspace_bytes.restype = sz
         L.anslin_dense_gemm.argtypes = [u32, vp, u32, u32, vp, ctypes.c_float, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
@@ -195,8 +197,9 @@ def anslin_gemm_multi_workspace_bytes(weights, m_max: int) -> int:
 class MultiCall:
     """Marshalled argument arrays of one anslin_gemm_multi call (built once, reusable every step)."""
 
-    def __init__(self, weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes):
+    def __init__(self, weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes, y_dtype: int = DT_F32):
         n = self.n = len(weights)
+        self.y_dtype = y_dtype
         vp, i64, i32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32
         self.w = (vp * n)(*[w.handle for w in weights])
         self.x = (vp * n)(*[int(p) for p in x_ptrs])
@@ -208,12 +211,19 @@ class MultiCall:
         self.x_dtype, self.ws_ptr, self.ws_bytes = x_dtype, ctypes.c_void_p(ws_ptr), ws_bytes
 
     def __call__(self, stream: int = 0):
-        _check(lib().anslin_gemm_multi(self.w, self.n, self.x, self.x_dtype, self.ldx, self.m, self.xs, self.y, self.ldy,
-                                       self.ws_ptr, self.ws_bytes, ctypes.c_void_p(stream)), "anslin_gemm_multi")
+        _check(lib().anslin_gemm_multi_ex(self.w, self.n, self.x, self.x_dtype, self.ldx, self.m, self.xs, self.y, self.y_dtype, self.ldy,
+                                          self.ws_ptr, self.ws_bytes, ctypes.c_void_p(stream)), "anslin_gemm_multi_ex")
 
 
 def anslin_gemm_multi(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes, stream: int = 0):
-    MultiCall(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes)(stream)
+    n = len(weights)
+    c = MultiCall(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes)
+    _check(lib().anslin_gemm_multi(c.w, n, c.x, c.x_dtype, c.ldx, c.m, c.xs, c.y, c.ldy, c.ws_ptr, c.ws_bytes, ctypes.c_void_p(stream)),
+           "anslin_gemm_multi")
+
+
+def anslin_gemm_multi_ex(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, y_dtype, ldys, ws_ptr, ws_bytes, stream: int = 0):
+    MultiCall(weights, x_ptrs, x_dtype, ldxs, ms, x_scale_ptrs, y_ptrs, ldys, ws_ptr, ws_bytes, y_dtype)(stream)
 
 
 def anslin_gemm_grouped(experts, rows_per_expert, x_ptr: int, x_dtype: int, ldx: int, x_scale_ptr: int | None, y_ptr: int,

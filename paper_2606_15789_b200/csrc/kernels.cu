@@ -14,6 +14,7 @@
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>
+#include <cuda_bf16.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -348,6 +349,7 @@ struct EpiParams {
   unsigned long long *counters;    // split-K flags, u32 [2 * CTAs of the problem]: flag[c * 2 + seg] = launch epoch once CTA c's partial `seg` is stored
   uint32_t epoch;                  // unique per launch: stale counter contents (any bytes) read as "nobody arrived"
   uint32_t m, mpad;
+  uint32_t y_bf16;                 // Y holds bf16 (round to nearest even of the fp32 result) instead of f32
 };
 // A stripe whose last split-K contributor is this CTA (shared memory; at most the first and the last segment).
 struct FinSeg { uint32_t valid, stripe, c_first, c_last; };
@@ -387,7 +389,11 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
       for (int j = 0; j < 16; ++j) {
         const uint32_t mm = c0 + j;
         if (mm < p.m) {
-          if (whole) p.y[size_t(mm) * p.ldy + n] = finalize<FMT>(v[j], kScaled ? p.x_scale[mm] : 1.0f, ws);
+          if (whole) {
+            const float f = finalize<FMT>(v[j], kScaled ? p.x_scale[mm] : 1.0f, ws);
+            if (p.y_bf16) reinterpret_cast<__nv_bfloat16 *>(p.y)[size_t(mm) * p.ldy + n] = __float2bfloat16_rn(f);
+            else p.y[size_t(mm) * p.ldy + n] = f;
+          }
           else part[size_t(mm) * kTileN + row] = v[j];
         }
       }
@@ -486,6 +492,14 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
           if (is_fp8_path(FMT)) ws = p.w_scale;
           o[j] = finalize<FMT>(acc[q][j], xs, ws);
         }
+        if (p.y_bf16) {
+          __nv_bfloat16 *yb = reinterpret_cast<__nv_bfloat16 *>(p.y) + size_t(mm) * p.ldy + n4;
+          const __nv_bfloat162 lo = __floats2bfloat162_rn(o[0], o[1]), hi = __floats2bfloat162_rn(o[2], o[3]);
+          if ((reinterpret_cast<uintptr_t>(yb) & 7) == 0)
+            *reinterpret_cast<uint2 *>(yb) = make_uint2(*reinterpret_cast<const uint32_t *>(&lo), *reinterpret_cast<const uint32_t *>(&hi));
+          else { yb[0] = lo.x; yb[1] = lo.y; yb[2] = hi.x; yb[3] = hi.y; }
+          continue;
+        }
         float *yo = p.y + size_t(mm) * p.ldy + n4;
         if ((reinterpret_cast<uintptr_t>(yo) & 15) == 0) *reinterpret_cast<float4 *>(yo) = make_float4(o[0], o[1], o[2], o[3]);
         else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
@@ -518,6 +532,7 @@ struct FusedParams {
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
   uint32_t afmt, bfmt;     // tcgen05 a/b format codes (fp8: 0 = e4m3, 1 = e5m2, chosen at run time)
+  uint32_t y_bf16;         // the launch's Y buffers hold bf16
 };
 struct TensorMaps { CUtensorMap m[kMaxProblems]; };
 
@@ -579,7 +594,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 
   const uint32_t t_begin = cta_first_tile(c, G, T), t_end = cta_first_tile(c + 1, G, T);
   const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, pr.y, pr.ldy,
-                     pr.partials, pr.counters, P.epoch, pr.m, mpad};
+                     pr.partials, pr.counters, P.epoch, pr.m, mpad, P.y_bf16};
 
   // Warp roles: decoders 0..D-1, epilogue D..D+3 (TMEM lane quadrant = warp % 4), MMA issuer D+4.  The
   // scheduler favours high warp ids, so the MMA issuer reacts first: a finished unit is consumed and its
@@ -799,7 +814,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
   const uint32_t t_begin = cta_first_tile(blockIdx.x, G, T), t_end = cta_first_tile(blockIdx.x + 1, G, T);
-  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.epoch, p.m, p.mpad};
+  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.epoch, p.m, p.mpad, 0u};
 
   if (warp == 5) {
     if (lane == 0) {
@@ -963,8 +978,9 @@ int launch_fused(const TensorMaps &tms, const FusedParams &p, uint32_t grid, siz
 // One launch over n <= kMaxProblems independent GEMMs that share format and tile geometry.
 int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, uint32_t x_dtype, const int64_t *ldx, const int32_t *ms,
                 const void *const *x_scales, void *const *ys, const int64_t *ldy, void *workspace_dev, size_t workspace_bytes,
-                cudaStream_t st) {
+                cudaStream_t st, uint32_t y_dtype = ANSLIN_DT_F32) {
   if (n < 1 || n > kMaxProblems || !workspace_dev || (reinterpret_cast<uintptr_t>(workspace_dev) & 15)) return ANSLIN_ERR_INVALID_ARG;
+  if (y_dtype != ANSLIN_DT_F32 && y_dtype != ANSLIN_DT_BF16) return ANSLIN_ERR_UNSUPPORTED;
   if (num_sms() <= 0) return ANSLIN_ERR_CUDA;
   const Header &h0 = ws[0]->h;
   const bool scaled = h0.format == ANSLIN_FMT_INT8 || is_fp8_path(h0.format);
@@ -1071,6 +1087,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   p.epoch = next_epoch();
   p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
+  p.y_bf16 = y_dtype == ANSLIN_DT_BF16 ? 1u : 0u;
   const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
   const uint32_t grid = cta0;
 #define ANSLIN_LAUNCH(F, PAY)                                                                                   \
@@ -1225,19 +1242,25 @@ int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int
   return ANSLIN_OK;
 }
 
-int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
-                      const int32_t *m, const void *const *x_scale_dev, void *const *y_dev, const int64_t *ldy, void *workspace_dev,
-                      size_t workspace_bytes, void *stream) {
+int anslin_gemm_multi_ex(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
+                         const int32_t *m, const void *const *x_scale_dev, void *const *y_dev, uint32_t y_dtype, const int64_t *ldy,
+                         void *workspace_dev, size_t workspace_bytes, void *stream) {
   g_launches = 0;
   if (!weights || n < 1 || !x_dev || !ldx || !m || !y_dev || !ldy) return ANSLIN_ERR_INVALID_ARG;
   const void *no_scales[kMaxProblems] = {nullptr};
   for (int32_t i0 = 0; i0 < n; i0 += kMaxProblems) {   // more than kMaxProblems: consecutive launches on the same stream
     const int cnt = std::min<int32_t>(kMaxProblems, n - i0);
     int rc = gemm_launch(cnt, weights + i0, x_dev + i0, x_dtype, ldx + i0, m + i0, x_scale_dev ? x_scale_dev + i0 : no_scales, y_dev + i0,
-                         ldy + i0, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream));
+                         ldy + i0, workspace_dev, workspace_bytes, static_cast<cudaStream_t>(stream), y_dtype);
     if (rc != ANSLIN_OK) return rc;
   }
   return ANSLIN_OK;
+}
+
+int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
+                      const int32_t *m, const void *const *x_scale_dev, void *const *y_dev, const int64_t *ldy, void *workspace_dev,
+                      size_t workspace_bytes, void *stream) {
+  return anslin_gemm_multi_ex(weights, n, x_dev, x_dtype, ldx, m, x_scale_dev, y_dev, ANSLIN_DT_F32, ldy, workspace_dev, workspace_bytes, stream);
 }
 
 int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts, const int32_t *rows_per_expert_host,

@@ -98,19 +98,21 @@ class MultiGemm:
     """anslin_gemm_multi over weights that share format and tile geometry: ONE persistent launch for
     e.g. q/k/v (same X) or gate/up.  Buffers and the marshalled call are built once."""
 
-    def __init__(self, dws, xs, x_scales=None, ys=None):
+    def __init__(self, dws, xs, x_scales=None, ys=None, y_dtype: torch.dtype = torch.float32):
         self.dws, self.xs = list(dws), list(xs)
         dev = self.xs[0].device
         ms = [int(x.shape[0]) for x in self.xs]
-        self.ys = list(ys) if ys is not None else [torch.empty((m, d.n_out), dtype=torch.float32, device=dev)
+        self.ys = list(ys) if ys is not None else [torch.empty((m, d.n_out), dtype=y_dtype, device=dev)
                                                    for m, d in zip(ms, self.dws)]
+        ydt = {torch.float32: B.DT_F32, torch.bfloat16: B.DT_BF16}[self.ys[0].dtype]
+        assert all(y.dtype == self.ys[0].dtype for y in self.ys)
         self.x_scales = x_scales
         need = B.anslin_gemm_multi_workspace_bytes([d.weight for d in self.dws], max(ms))
         self.ws = torch.empty(need, dtype=torch.uint8, device=dev)
         self.call = B.MultiCall([d.weight for d in self.dws], [x.data_ptr() for x in self.xs], B.X_DTYPE[self.dws[0].fmt],
                                 [x.stride(0) for x in self.xs], ms,
                                 None if x_scales is None else [s.data_ptr() for s in x_scales],
-                                [y.data_ptr() for y in self.ys], [y.stride(0) for y in self.ys], self.ws.data_ptr(), self.ws.numel())
+                                [y.data_ptr() for y in self.ys], [y.stride(0) for y in self.ys], self.ws.data_ptr(), self.ws.numel(), ydt)
 
     def __call__(self):
         self.call(_stream())

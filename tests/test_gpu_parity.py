@@ -162,6 +162,35 @@ def test_gemm_bf16_max_batch_and_strided_buffers(m, tile):
     dw.close()
 
 
+def test_gemm_multi_bf16_output():
+    """anslin_gemm_multi_ex with bf16 Y: every element is the fp32 result rounded to nearest even, i.e. within one
+    bf16 ulp of the float64 oracle's value rounded the same way (whole stripes and split-K stripes, odd row pitch)."""
+    rt = _rt()
+    import torch
+    k, m = 2048, 37
+    shapes = [640, 128]
+    ws_, dws, refs = [], [], []
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=150))
+    xd = rt.x_to_device(B.FMT_BF16, x)
+    for i, n in enumerate(shapes):
+        w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=151 + i, jitter=True))
+        buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
+        dws.append(rt.DeviceWeight(buf)); refs.append(og.gemm_bf16(x, w))
+    ybig = [torch.full((m, n + 3), 7.0, dtype=torch.bfloat16, device="cuda") for n in shapes]      # odd pitch: scalar stores
+    mg = rt.MultiGemm(dws, [xd, xd], None, [yb[:, :n] for yb, n in zip(ybig, shapes)])
+    mg()
+    mg32 = rt.MultiGemm(dws, [xd, xd])
+    y32 = [t.cpu().numpy() for t in mg32()]
+    for yb, n, (y_ref, a_ref), yf in zip(ybig, shapes, refs, y32):
+        got = yb.float().cpu().numpy()
+        assert np.all(got[:, n:] == 7.0)
+        want = torch.from_numpy(yf).to(torch.bfloat16).float().numpy()          # RNE of the library's own fp32 result
+        assert np.array_equal(got[:, :n], want)
+        check_gemm(yf, y_ref, a_ref)
+    for d in dws:
+        d.close()
+
+
 def test_gemm_replayed_from_a_cuda_graph():
     """A captured launch is replayed with its kernel parameters frozen, the split-K epoch among them: the stripe owner
     clears the flags it consumed, so every replay starts from "not stored" and sums this replay's partials."""
