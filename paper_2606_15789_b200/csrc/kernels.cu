@@ -349,7 +349,6 @@ struct EpiParams {
   unsigned long long *counters;    // split-K flags, u32 [2 * CTAs of the problem]: flag[c * 2 + seg] = launch epoch once CTA c's partial `seg` is stored
   uint32_t epoch;                  // unique per launch: stale counter contents (any bytes) read as "nobody arrived"
   uint32_t m, mpad;
-  uint32_t y_bf16;                 // Y holds bf16 (round to nearest even of the fp32 result) instead of f32
 };
 // A stripe whose last split-K contributor is this CTA (shared memory; at most the first and the last segment).
 struct FinSeg { uint32_t valid, stripe, c_first, c_last; };
@@ -362,7 +361,9 @@ __device__ __forceinline__ uint4 ldcg128(const uint32_t *p) {
 
 // Epilogue (a10), warps 0..3: TMEM -> registers -> Y for whole stripes, or -> split-K partial.  The CTA
 // that contributes LAST to a stripe (global counter) records it in fin[]; splitk_fixup sums it up later.
-template <uint32_t FMT>
+// YB: Y holds bf16 (the fp32 result rounded to nearest even) instead of f32; a template parameter, so that the f32 kernels'
+// code is exactly what it was (a run-time branch here cost the whole kernel 3 % through register allocation).
+template <uint32_t FMT, bool YB = false>
 __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_base, uint32_t tfull_s, uint32_t tempty_s,
                                              FinSeg *fin, uint32_t t_begin, uint32_t t_end, uint32_t KT, uint32_t c, uint32_t G,
                                              uint32_t T, int warp, int lane) {
@@ -391,7 +392,7 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
         if (mm < p.m) {
           if (whole) {
             const float f = finalize<FMT>(v[j], kScaled ? p.x_scale[mm] : 1.0f, ws);
-            if (p.y_bf16) reinterpret_cast<__nv_bfloat16 *>(p.y)[size_t(mm) * p.ldy + n] = __float2bfloat16_rn(f);
+            if constexpr (YB) reinterpret_cast<__nv_bfloat16 *>(p.y)[size_t(mm) * p.ldy + n] = __float2bfloat16_rn(f);
             else p.y[size_t(mm) * p.ldy + n] = f;
           }
           else part[size_t(mm) * kTileN + row] = v[j];
@@ -423,7 +424,7 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
 // epilogue_run): for each stripe recorded in fin[], sum the partials of its contributors in CTA order
 // (bit-reproducible), apply the scales and store Y.  One item = one batch row x 4 output channels;
 // 16-byte loads, up to 8 contributors in flight per thread.
-template <uint32_t FMT>
+template <uint32_t FMT, bool YB = false>
 __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *fin, uint32_t KT, uint32_t G, uint32_t T) {
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   constexpr int kItems = 2;   // items per thread and pass: their loads are all issued before the first add
@@ -492,7 +493,7 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
           if (is_fp8_path(FMT)) ws = p.w_scale;
           o[j] = finalize<FMT>(acc[q][j], xs, ws);
         }
-        if (p.y_bf16) {
+        if constexpr (YB) {
           __nv_bfloat16 *yb = reinterpret_cast<__nv_bfloat16 *>(p.y) + size_t(mm) * p.ldy + n4;
           const __nv_bfloat162 lo = __floats2bfloat162_rn(o[0], o[1]), hi = __floats2bfloat162_rn(o[2], o[3]);
           if ((reinterpret_cast<uintptr_t>(yb) & 7) == 0)
@@ -532,7 +533,6 @@ struct FusedParams {
   uint32_t slot_bytes;     // 4096 + max mpad * 32
   uint32_t tmem_cols;
   uint32_t afmt, bfmt;     // tcgen05 a/b format codes (fp8: 0 = e4m3, 1 = e5m2, chosen at run time)
-  uint32_t y_bf16;         // the launch's Y buffers hold bf16
 };
 struct TensorMaps { CUtensorMap m[kMaxProblems]; };
 
@@ -551,7 +551,7 @@ struct SmemEmit {
   __device__ __forceinline__ void packed8(int, int, int, uint32_t, uint32_t) const {}
 };
 
-template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS>
+template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS, bool YB>
 __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ TensorMaps tms,
                                                                       const __grid_constant__ FusedParams P) {
   using TR = FmtTraits<FMT>;
@@ -594,7 +594,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
 
   const uint32_t t_begin = cta_first_tile(c, G, T), t_end = cta_first_tile(c + 1, G, T);
   const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cv.base + cv.off_scales), cv.w_scale, pr.y, pr.ldy,
-                     pr.partials, pr.counters, P.epoch, pr.m, mpad, P.y_bf16};
+                     pr.partials, pr.counters, P.epoch, pr.m, mpad};
 
   // Warp roles: decoders 0..D-1, epilogue D..D+3 (TMEM lane quadrant = warp % 4), MMA issuer D+4.  The
   // scheduler favours high warp ids, so the MMA issuer reacts first: a finished unit is consumed and its
@@ -761,13 +761,13 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   } else if (warp < mma_warp) {
     // ===================== epilogue warps =====================
     grid_dep_wait();   // Y, the scales and the workspace belong to the stream's earlier kernels until they are done
-    epilogue_run<FMT>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp & 3, lane);
+    epilogue_run<FMT, YB>(ep, tmem_base, tfull_s, tempty_s, fin, t_begin, t_end, KT, c, G, T, warp & 3, lane);
   }
   tc_fence_before();
   __syncthreads();
   if (warp == mma_warp) tmem_dealloc(tmem_base, P.tmem_cols);
   grid_dep_wait();   // warps that had no work of their own join the fix-up: same rule
-  splitk_fixup<FMT>(ep, fin, KT, G, T);
+  splitk_fixup<FMT, YB>(ep, fin, KT, G, T);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -814,7 +814,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
   const uint32_t t_begin = cta_first_tile(blockIdx.x, G, T), t_end = cta_first_tile(blockIdx.x + 1, G, T);
-  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.epoch, p.m, p.mpad, 0u};
+  const EpiParams ep{p.x_scale, reinterpret_cast<const __half *>(p.w_scale_h), p.w_scale, p.y, p.ldy, p.partials, p.counters, p.epoch, p.m, p.mpad};
 
   if (warp == 5) {
     if (lane == 0) {
@@ -948,9 +948,9 @@ uint32_t bfmt_of(uint32_t fmt, uint32_t dt) { return is_fp8_path(fmt) ? (dt == A
 
 int sm_budget() { return std::max(1, num_sms()); }
 
-template <uint32_t FMT, int RB, bool PAYLOAD, bool LS>
-int launch_fused(const TensorMaps &tms, const FusedParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
-  auto kern = fused_gemm_kernel<FMT, RB, (RB == 1 ? kJ32 : 1), PAYLOAD, LS>;
+template <uint32_t FMT, int RB, bool PAYLOAD, bool LS, bool YB>
+int launch_fused_y(const TensorMaps &tms, const FusedParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
+  auto kern = fused_gemm_kernel<FMT, RB, (RB == 1 ? kJ32 : 1), PAYLOAD, LS, YB>;
   static thread_local size_t smem_set = 0;     // per instantiation: raise the dynamic shared memory limit once
   if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
@@ -1087,18 +1087,18 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   p.epoch = next_epoch();
   p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
-  p.y_bf16 = y_dtype == ANSLIN_DT_BF16 ? 1u : 0u;
+  const bool ybf = y_dtype == ANSLIN_DT_BF16;
   const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
   const uint32_t grid = cta0;
+#define launch_fused(...) (ybf ? launch_fused_y<__VA_ARGS__, true>(tms, p, grid, smem, st) : launch_fused_y<__VA_ARGS__, false>(tms, p, grid, smem, st))
 #define ANSLIN_LAUNCH(F, PAY)                                                                                   \
-  (RB == 1 ? (ls ? launch_fused<F, 1, PAY, true>(tms, p, grid, smem, st) : launch_fused<F, 1, PAY, false>(tms, p, grid, smem, st)) \
-           : launch_fused<F, 4, PAY, false>(tms, p, grid, smem, st))
+  (RB == 1 ? (ls ? launch_fused(F, 1, PAY, true) : launch_fused(F, 1, PAY, false)) \
+           : launch_fused(F, 4, PAY, false))
   switch (h0.format) {
     case ANSLIN_FMT_BF16: return pay ? ANSLIN_LAUNCH(ANSLIN_FMT_BF16, true) : ANSLIN_LAUNCH(ANSLIN_FMT_BF16, false);
     case ANSLIN_FMT_BF16_PAIR4:   // lane streams on 32-row tiles only (anslin_open checked)
       if (RB != 1 || !ls) return ANSLIN_ERR_CORRUPT;
-      return pay ? launch_fused<ANSLIN_FMT_BF16_PAIR4, 1, true, true>(tms, p, grid, smem, st)
-                 : launch_fused<ANSLIN_FMT_BF16_PAIR4, 1, false, true>(tms, p, grid, smem, st);
+      return pay ? launch_fused(ANSLIN_FMT_BF16_PAIR4, 1, true, true) : launch_fused(ANSLIN_FMT_BF16_PAIR4, 1, false, true);
     case ANSLIN_FMT_FP8_E4M3:
     case ANSLIN_FMT_FP8_E5M2: return ANSLIN_LAUNCH(ANSLIN_FMT_FP8_E4M3, false);   // same bytes, another descriptor code
     case ANSLIN_FMT_INT8: return ANSLIN_LAUNCH(ANSLIN_FMT_INT8, false);
@@ -1106,6 +1106,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     case ANSLIN_FMT_FP4_E2M1: return ANSLIN_LAUNCH(ANSLIN_FMT_FP4_E2M1, false);
   }
 #undef ANSLIN_LAUNCH
+#undef launch_fused
   return ANSLIN_ERR_UNSUPPORTED;
 }
 
