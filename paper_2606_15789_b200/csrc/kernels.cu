@@ -258,7 +258,7 @@ constexpr int kDecWarps = 8;
 __host__ __device__ constexpr int unit_steps32(uint32_t fmt) { return 2 * spc_of(fmt); }
 
 template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS>
-__global__ void __launch_bounds__(kDecWarps * 32, 3) decode_kernel(ContainerView cv, uint8_t *out, uint32_t stream_bytes) {
+__global__ void __launch_bounds__(kDecWarps * 32, 2) decode_kernel(ContainerView cv, uint8_t *out, uint32_t stream_bytes) {
   using POL = typename std::conditional<LS, LaneWords, InterleavedWords>::type;
   constexpr int Q = TileTraits<RB, J>::Q;
   extern __shared__ __align__(16) uint8_t dsm[];
