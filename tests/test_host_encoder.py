@@ -174,3 +174,28 @@ def test_gemm_entry_points_fail_loudly_without_a_device():
     with pytest.raises(B.AnslinError):
         B.anslin_gemm(hw, 16, B.DT_BF16, 128, 1, None, 16, 128, 16, 1 << 20)
     hw.close()
+
+
+def test_widened_calls_validate_their_arguments_without_a_device():
+    """The calls added for SURVEY 8(f) reject bad arguments before touching CUDA (so these checks run on any host)."""
+    L = B.lib()
+    ok = B.Desc(B.FMT_BF16, 256, 1024, 256, 0, B.FLAG_LANE_STREAMS | B.FLAG_STATE_PAYLOAD, 1.0, 32)
+    assert L.anslin_encode_device_head_bytes(ctypes.byref(ok)) == 128 + 512 + 4 * (2 * 4 * 4 + 1) + 12    # header, table, offsets (aligned)
+    assert L.anslin_encode_device_workspace_bytes(ctypes.byref(ok)) > 0
+    for bad in (B.Desc(B.FMT_BF16, 256, 1024, 256, 0, B.FLAG_STATE_PAYLOAD, 1.0, 32),          # interleaved words: host encoder only
+                B.Desc(B.FMT_BF16, 256, 1024, 256, 0, B.FLAG_LANE_STREAMS, 1.0, 128),          # 128-row tiles
+                B.Desc(B.FMT_BF16, 256, 1024, 64, 0, B.FLAG_LANE_STREAMS, 1.0, 32),            # less than one segment per tile
+                B.Desc(B.FMT_BF16_PAIR4, 256, 1024, 256, 0, B.FLAG_LANE_STREAMS, 1.0, 32),     # pair variant: host encoder only
+                B.Desc(B.FMT_INT8, 256, 1024, 256, 0, B.FLAG_LANE_STREAMS | B.FLAG_STATE_PAYLOAD, 1.0, 32)):
+        assert L.anslin_encode_device_head_bytes(ctypes.byref(bad)) == 0
+        assert L.anslin_encode_device_workspace_bytes(ctypes.byref(bad)) == 0
+    n = ctypes.c_size_t(0)
+    assert L.anslin_encode_device(ctypes.byref(ok), None, None, None, None, 0, None, 0, None, 0, ctypes.byref(n), None) == 1   # INVALID_ARG
+    assert L.anslin_histogram(B.FMT_BF16, None, 16, None, None) == 1
+    buf = np.zeros(64, dtype=np.uint8)
+    assert L.anslin_histogram(B.FMT_BF16, ctypes.c_void_p(buf.ctypes.data + 1), 16, ctypes.c_void_p(buf.ctypes.data), None) == 1   # misaligned
+    assert L.anslin_histogram(99, ctypes.c_void_p(buf.ctypes.data), 16, ctypes.c_void_p(buf.ctypes.data), None) in (1, 2)
+    with pytest.raises(B.AnslinError):
+        B.anslin_encode_host(B.FMT_BF16_PAIR4, np.zeros((128, 256), np.uint16), 128, 256, tile_k=256, flags=0, tile_n=32)   # needs lane streams
+    with pytest.raises(B.AnslinError):
+        B.anslin_encode_host(B.FMT_BF16_PAIR4, np.zeros((128, 256), np.uint16), 128, 256, tile_k=256, flags=2, tile_n=128)
