@@ -1,0 +1,538 @@
+// Fused rANS-decode + tcgen05 GEMM, second design: the decoded weights reach the tensor core through TENSOR MEMORY.
+// Included by kernels.cu inside its anonymous namespace (after the PTX wrappers, FmtTraits, Problem, TensorMaps).
+//
+// Alg V.1 (P:l.196-252) for lane-stream containers with 32-row tiles, re-cut for sm_100a:
+//   * a TEAM = 4 decoder warps = one 128-row stripe; warp q of a team owns TMEM lane quadrant q, so lane l of warp q
+//     IS row 32q+l of the MMA's A operand: the 16 weights (32 operand bytes) a lane decodes per unit go from its
+//     registers into 8 TMEM columns with one tcgen05.st — no shared-memory operand slot, no swizzle, no proxy fence
+//     ("writes the decoded value directly into the shared-memory" P:l.254 becomes "into tensor memory");
+//   * every warp runs Alg V.2 (P:l.260-287) on TWO tiles at once (k-tiles kt, kt+1 of its stripe quadrant), their
+//     steps interleaved, so a team hands the tensor core two K slices per unit step;
+//   * there is no central MMA warp: the team meets on a named barrier and ITS OWN warp 0 issues the two
+//     tcgen05.mma (A from TMEM, X slice from shared memory, accumulator in TMEM) and the commit that frees the
+//     A columns and the X ring slot ("ready[2]" flags of P:l.210 -> one mbarrier per ring slot);
+//   * the X slices (pad16(m) rows x 32 bytes, SWIZZLE_32B) arrive by TMA one unit step ahead, in a 2-deep ring
+//     per team, issued by warp 1 of the team (which otherwise only waits for warp 0 at that point);
+//   * nothing in the decode loop waits for HBM: the bf16 sign/mantissa bytes of the NEXT unit travel by cp.async into a
+//     shared-memory double buffer (a register-destination global load shares scoreboards with the loop's LDS and
+//     stalled every unit for an HBM round trip);
+//   * the team reads its own accumulator back (tcgen05.ld: warp q -> lanes 32q..) at the end of a stripe segment;
+//   * split-K: a team is a "virtual CTA" of the stream-K split.  Every contributor of a stripe stores its partial,
+//     raises a flag, waits for the other contributors' flags and then reduces ITS OWN slice of the stripe's outputs,
+//     summing the contributors in team order (bit-reproducible; the reduction is spread over all contributors
+//     instead of falling on one of them).
+// TMEM budget: T teams x (pad16(m) accumulator columns + 16 operand columns) <= 512  ->  T = 5 up to m = 80.
+#pragma once
+
+constexpr int kTeamWarps = 4;
+constexpr int kMaxTeams = 5;
+constexpr int kTmemThreads = 32 * kTeamWarps * kMaxTeams;   // 640: lets ptxas use up to 96 registers
+constexpr uint32_t kACols = 8;                               // TMEM columns of one operand unit (32 bytes per row)
+constexpr uint32_t kNT = 32 * kTeamWarps;                    // threads of a team
+
+// shared-memory carve-up, from the 1024-byte aligned base: slot table | prefix scratch | barriers | X rings | raw | staging
+constexpr uint32_t kTmBarOff = 16384 + 1088;                 // 64 bytes of mbarriers per team
+constexpr uint32_t kTmPtrOff = kTmBarOff + 64 * kMaxTeams;
+constexpr uint32_t kTmXOff = 18432;
+constexpr uint32_t kRawBufBytes = 1024;                      // bf16: two 512-byte raw vectors per chain
+__host__ __device__ constexpr bool tmem_has_raw(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16; }
+__host__ __device__ constexpr size_t tmem_smem_bytes(uint32_t T, uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
+  return 1024 /*align slack*/ + kTmXOff + size_t(T) * 4 * mpad_max * 32 + (tmem_has_raw(fmt) ? size_t(T) * kTeamWarps * 2 * kRawBufBytes : 0) +
+         size_t(T) * kTeamWarps * 2 * stream_bytes + 16;
+}
+// split-K control words of a problem (inside its flag area): u32 flag[2 * teams] | u32 stripe_count[stripes]
+constexpr size_t kTmStripeCntOff = 8 * 160 * kMaxTeams + 256;
+
+struct TmemParams {
+  Problem prob[kMaxProblems];
+  uint32_t nprob;
+  uint32_t T;              // teams per CTA
+  uint32_t epoch;          // launch id for the split-K flags
+  uint32_t stream_bytes;   // shared memory per staged lane-stream segment
+  uint32_t xslice_bytes;   // max mpad * 32
+  uint32_t tmem_stride;    // TMEM columns per team: max mpad + 2 * kACols
+  uint32_t afmt, bfmt;
+};
+
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]),
+               "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+               : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+template <int KIND>  // A operand in tensor memory
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  if constexpr (KIND == 0)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+                 "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+                 : "memory");
+  else if constexpr (KIND == 1)
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::f8f6f4 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+                 "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+                 : "memory");
+  else
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\ttcgen05.mma.cta_group::1.kind::i8 [%0], [%1], %2, %3, p;\n\t}" ::"r"(d_tmem),
+                 "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+                 : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t a) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ uint32_t lds16(uint32_t a) {
+  uint32_t v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+  return v;
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+
+// One operand unit (32 operand bytes per row = 8 registers) of the warp's two tiles.  rv[j]: bf16: the unit's 16 raw
+// (sign | mantissa) bytes of this lane.  sz[j]: int4: this lane's (scale, zero) pair of the unit's quantisation group.
+template <uint32_t FMT, bool PAYLOAD>
+__device__ __forceinline__ void decode_unit_regs(LaneStream (&s)[2], uint32_t tab_s, uint32_t dir, bool last_unit, const uint4 (&rv)[2],
+                                                 const uint32_t (&sz)[2], uint32_t (&r)[2][8]) {
+  static_assert(FMT != ANSLIN_FMT_BF16_PAIR4, "the pair variant runs on the shared-memory operand path");
+  if constexpr (FMT == ANSLIN_FMT_BF16) {
+    uint32_t R0[2] = {rv[0].x, rv[1].x}, R1[2] = {rv[0].y, rv[1].y};
+    uint4 o[2];
+    decode8_bf16<LaneWords, 2>(s, tab_s, dir, R0, R1, o);
+#pragma unroll
+    for (int j = 0; j < 2; ++j) { r[j][0] = o[j].x; r[j][1] = o[j].y; r[j][2] = o[j].z; r[j][3] = o[j].w; }
+    R0[0] = rv[0].z; R0[1] = rv[1].z; R1[0] = rv[0].w; R1[1] = rv[1].w;
+    decode8_bf16<LaneWords, 2>(s, tab_s, dir, R0, R1, o);
+    if (PAYLOAD && last_unit) {
+      // raw bytes 14, 15 of the tile's last vector ride in the END state (A4): merge them in now
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const uint32_t pl = s[j].x - kL;   // byte 14 | byte 15 << 8, each = mantissa << 1 | sign
+        o[j].w |= ((pl >> 1) & 0x7Fu) | ((pl & 1u) << 15) | (((pl >> 9) & 0x7Fu) << 16) | (((pl >> 8) & 1u) << 31);
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < 2; ++j) { r[j][4] = o[j].x; r[j][5] = o[j].y; r[j][6] = o[j].z; r[j][7] = o[j].w; }
+  } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
+    uint32_t B0[2], B1[2];
+    decode4<LaneWords, 2>(s, B0, tab_s, dir);
+    decode4<LaneWords, 2>(s, B1, tab_s, dir);
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      const __half2 szh = *reinterpret_cast<const __half2 *>(&sz[j]);
+      const __half2 sc = __half2half2(__low2half(szh));
+      const __half2 zoff = __hadd2(__half2half2(__high2half(szh)), __float2half2_rn(1024.f));
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        r[j][b] = awq_dequant2((B0[j] >> (8 * b)) & 0xFFu, zoff, sc);
+        r[j][4 + b] = awq_dequant2((B1[j] >> (8 * b)) & 0xFFu, zoff, sc);
+      }
+    }
+  } else if constexpr (FMT == ANSLIN_FMT_FP4_E2M1) {
+#pragma unroll
+    for (int h = 0; h < 4; ++h) {
+      uint32_t Bq[2];
+      decode4<LaneWords, 2>(s, Bq, tab_s, dir);
+#pragma unroll
+      for (int j = 0; j < 2; ++j) e2m1x8_to_e4m3(Bq[j], r[j][2 * h], r[j][2 * h + 1]);
+    }
+  } else {   // fp8 / int8: the symbol byte is the operand byte
+#pragma unroll
+    for (int h = 0; h < 8; ++h) {
+      uint32_t q[2];
+      decode4<LaneWords, 2>(s, q, tab_s, dir);
+      r[0][h] = q[0];
+      r[1][h] = q[1];
+    }
+  }
+}
+
+#ifdef ANSLIN_TRACE
+__device__ unsigned long long g_trace[160 * kMaxTeams * 8];
+__device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+#define TRACE(slot) do { if (q == 0 && lane == 0) g_trace[(blockIdx.x * kMaxTeams + team) * 8 + (slot)] = gtimer(); } while (0)
+__device__ unsigned long long g_prof[160 * kMaxTeams * 4 * 8];
+#define PROF_DECL long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0};
+#define PROF(i) do { const long long pf_n = clock64(); pf_acc[i] += pf_n - pf_t; pf_t = pf_n; } while (0)
+#define PROF_DUMP do { if (lane == 0) for (int pf_i = 0; pf_i < 6; ++pf_i) g_prof[((blockIdx.x * kMaxTeams + team) * 4 + q) * 8 + pf_i] = (unsigned long long)pf_acc[pf_i]; } while (0)
+#else
+#define TRACE(slot) do {} while (0)
+#define PROF_DECL
+#define PROF(i) do {} while (0)
+#define PROF_DUMP do {} while (0)
+#endif
+
+// The contributors of a stripe, in the order their partials are summed: the distinct teams that own one of its pairs.
+struct StripeTeams {
+  uint32_t V, Ptot, PK, stripe, v_first, v_last, count;
+  bool dense;   // V <= Ptot: every team has work, the contributors are v_first..v_last
+  __device__ __forceinline__ StripeTeams(uint32_t V_, uint32_t Ptot_, uint32_t PK_, uint32_t stripe_)
+      : V(V_), Ptot(Ptot_), PK(PK_), stripe(stripe_) {
+    v_first = cta_of_tile(stripe * PK, V, Ptot);
+    v_last = cta_of_tile(stripe * PK + PK - 1, V, Ptot);
+    dense = V <= Ptot;
+    count = dense ? v_last - v_first + 1 : PK;   // more teams than pairs: one team per pair
+  }
+  __device__ __forceinline__ uint32_t team(uint32_t k) const { return dense ? v_first + k : cta_of_tile(stripe * PK + k, V, Ptot); }
+  __device__ __forceinline__ uint32_t index_of(uint32_t v, uint32_t first_pair_of_v) const {
+    return dense ? v - v_first : first_pair_of_v - stripe * PK;
+  }
+  // partial slot of contributor vv: its first segment (slot 0) unless the stripe is its second one, which can only be the
+  // case for the first contributor (every later one starts inside the stripe)
+  __device__ __forceinline__ uint32_t slot(uint32_t vv) const {
+    return vv * 2u + ((vv == v_first && cta_first_tile(vv, V, Ptot) < stripe * PK) ? 1u : 0u);
+  }
+};
+
+// Distributed deterministic split-K reduction of one stripe by one of its contributors (all 128 threads of the team).
+template <uint32_t FMT, bool YB>
+__device__ __forceinline__ void team_reduce(const EpiParams &p, const StripeTeams &st, uint32_t my_index, uint32_t tid, int bar) {
+  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
+  uint32_t *flags = reinterpret_cast<uint32_t *>(p.counters);
+  // wait for every contributor's partial (one flag per thread)
+  for (uint32_t k = tid; k < st.count; k += kNT) {
+    const uint32_t *flag = flags + st.slot(st.team(k));
+    uint32_t val, spins = 0;
+    while (true) {
+      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(val) : "l"(flag) : "memory");
+      if (val == p.epoch) break;
+      __nanosleep(200);
+      if (++spins > (1u << 24)) __trap();   // a protocol bug traps instead of hanging the GPU
+    }
+  }
+  named_bar_sync(bar, kNT);
+  const size_t slot_words = size_t(p.mpad) * kTileN;
+  const uint32_t n_items = p.m * 32u;   // one item = one batch row x 4 output channels
+  const uint32_t it_begin = uint32_t(uint64_t(my_index) * n_items / st.count), it_end = uint32_t(uint64_t(my_index + 1) * n_items / st.count);
+  for (uint32_t it = it_begin + tid; it < it_end; it += kNT) {
+    const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u;
+    uint32_t acc[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
+    for (uint32_t kb = 0; kb < st.count; kb += 8) {
+      uint4 val[8];
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        val[j] = make_uint4(0, 0, 0, 0);
+        if (kb + j < st.count) val[j] = ldcg128(p.partials + size_t(st.slot(st.team(kb + j))) * slot_words + size_t(mm) * kTileN + r4);
+      }
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {   // fixed team order -> bit-reproducible sums
+        if (kb + j < st.count) {
+          acc[0] = acc_add<FMT>(acc[0], val[j].x); acc[1] = acc_add<FMT>(acc[1], val[j].y);
+          acc[2] = acc_add<FMT>(acc[2], val[j].z); acc[3] = acc_add<FMT>(acc[3], val[j].w);
+        }
+      }
+    }
+    const uint32_t n4 = st.stripe * kTileN + r4;
+    const float xs = kScaled ? p.x_scale[mm] : 1.0f;
+    float o[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      float ws = 1.0f;
+      if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
+      if (is_fp8_path(FMT)) ws = p.w_scale;
+      o[j] = finalize<FMT>(acc[j], xs, ws);
+    }
+    if constexpr (YB) {
+      __nv_bfloat16 *yb = reinterpret_cast<__nv_bfloat16 *>(p.y) + size_t(mm) * p.ldy + n4;
+      const __nv_bfloat162 lo = __floats2bfloat162_rn(o[0], o[1]), hi = __floats2bfloat162_rn(o[2], o[3]);
+      if ((reinterpret_cast<uintptr_t>(yb) & 7) == 0)
+        *reinterpret_cast<uint2 *>(yb) = make_uint2(*reinterpret_cast<const uint32_t *>(&lo), *reinterpret_cast<const uint32_t *>(&hi));
+      else { yb[0] = lo.x; yb[1] = lo.y; yb[2] = hi.x; yb[3] = hi.y; }
+    } else {
+      float *yo = p.y + size_t(mm) * p.ldy + n4;
+      if ((reinterpret_cast<uintptr_t>(yo) & 15) == 0) *reinterpret_cast<float4 *>(yo) = make_float4(o[0], o[1], o[2], o[3]);
+      else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
+    }
+  }
+  // The last contributor to finish reading clears the stripe's flags and its counter, so that a replay of this very launch
+  // (CUDA graph: same epoch) starts from "nothing stored".  Counter word = epoch tag << 8 | readers done; any other tag
+  // (stale or never written bytes) reads as zero readers.
+  named_bar_sync(bar, kNT);
+  if (tid == 0) {
+    uint32_t *cnt = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(p.counters) + kTmStripeCntOff) + st.stripe;
+    const uint32_t tag = (p.epoch << 8);
+    uint32_t old = *reinterpret_cast<volatile uint32_t *>(cnt), done;
+    while (true) {
+      done = ((old & 0xFFFFFF00u) == tag ? (old & 0xFFu) : 0u) + 1u;
+      const uint32_t seen = atomicCAS(cnt, old, done == st.count ? 0u : (tag | done));
+      if (seen == old) break;
+      old = seen;
+    }
+    if (done == st.count) {
+      for (uint32_t k = 0; k < st.count; ++k) flags[st.slot(st.team(k))] = 0u;
+    }
+  }
+}
+
+template <uint32_t FMT, bool PAYLOAD, bool YB>
+__global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __grid_constant__ TensorMaps tms,
+                                                                      const __grid_constant__ TmemParams P) {
+  using TR = FmtTraits<FMT>;
+  constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
+  constexpr bool kRaw = tmem_has_raw(FMT);
+  constexpr uint32_t kUnitsPerSeg = seg_steps_of(FMT) / unit_steps32(FMT);
+  constexpr uint32_t kUnitK = unit_k_of(FMT);
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t *smem = smem_raw + (smem0 - smem_u32(smem_raw));
+  grid_dep_launch_dependents();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t T = P.T, team = uint32_t(warp) / kTeamWarps, q = uint32_t(warp) % kTeamWarps;
+#ifdef ANSLIN_TRACE
+  if ((threadIdx.x & 127) == 0) g_trace[(blockIdx.x * kMaxTeams + team) * 8 + 0] = gtimer();
+#endif
+  uint32_t pi = 0;
+  while (pi + 1 < P.nprob && blockIdx.x >= P.prob[pi + 1].cta0) ++pi;
+  const Problem &pr = P.prob[pi];
+  // the problem's geometry, copied out of the parameter block once
+  const uint8_t *const cbase = pr.cv.base;
+  const uint32_t c = blockIdx.x - pr.cta0, G = pr.ncta, KT = pr.cv.KT, units = pr.cv.units, mpad = pr.mpad, tile_k = pr.cv.tile_k;
+  const uint64_t off_records = pr.cv.off_records, off_raw = pr.cv.off_raw, off_scales = pr.cv.off_scales;
+  const uint32_t n_out = pr.cv.n_out, qgroup = pr.cv.group;
+  const CUtensorMap *const xmap = &tms.m[pi];
+  uint32_t *tab = reinterpret_cast<uint32_t *>(smem);
+  uint32_t *cum = reinterpret_cast<uint32_t *>(smem + 16384);
+  const uint32_t bars_s = smem0 + kTmBarOff;   // per team: done[2], xfull[2], accfull
+  volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + kTmPtrOff);
+  const uint32_t raw_off = kTmXOff + T * 4u * P.xslice_bytes;
+  const uint32_t stage_off = raw_off + (kRaw ? T * kTeamWarps * 2u * kRawBufBytes : 0u);
+
+  if (threadIdx.x == 0) {
+    for (uint32_t i = 0; i < T; ++i)
+      for (uint32_t b = 0; b < 5; ++b) mbar_init(bars_s + 64 * i + 8 * b, 1);
+    fence_mbar_init();
+  }
+  if (warp == 0) tmem_alloc(smem0 + kTmPtrOff, 512);
+  tc_fence_before();
+  build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cbase + pr.cv.off_freq));   // ends with __syncthreads()
+  tc_fence_after();
+  const uint32_t tmem_base = *tmemptr;
+
+  const uint32_t done_s = bars_s + 64 * team, xfull_s = done_s + 16, accfull_s = done_s + 32;
+  const uint32_t acc_t = tmem_base + team * P.tmem_stride, a_t = acc_t + mpad;   // accumulator, then two operand units
+  const uint32_t lane_t = (q * 32u) << 16;
+  const uint32_t xring_s = smem0 + kTmXOff + team * 4u * P.xslice_bytes;          // slot sl, slice j at (sl * 2 + j) * xslice_bytes
+  const uint32_t rawbuf_s = smem0 + raw_off + uint32_t(warp) * 2u * kRawBufBytes;  // chain j, vector parity b at j * 1024 + b * 512
+  const uint32_t stage_s = smem0 + stage_off + uint32_t(warp) * 2u * P.stream_bytes, tab_s = smem0;
+  const uint32_t dir = (lane & 1) ? uint32_t(-2) : 2u;
+  const int bar_id = 1 + int(team);
+
+  // stream-K split over TEAMS: team v of V owns pairs [first(v), first(v+1)) of the stripe-major sequence of
+  // (stripe, k-tile pair) items; v is team-major so that a small launch spreads over all SMs first
+  const uint32_t PK = (KT + 1) / 2, stripes = n_out / kTileN, Ptot = stripes * PK;
+  const uint32_t V = G * T, v = team * G + c;
+  const uint32_t p_begin = cta_first_tile(v, V, Ptot), p_end = cta_first_tile(v + 1, V, Ptot);
+  const uint32_t N = (p_end - p_begin) * units;   // unit steps of this team
+  const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cbase + off_scales), pr.cv.w_scale, pr.y, pr.ldy,
+                     pr.partials, pr.counters, P.epoch, pr.m, mpad};
+  const uint32_t idesc = make_idesc(TR::c, P.afmt, P.bfmt, 128, mpad);
+  const uint32_t xbytes = mpad * 32u;
+  const uint32_t *offs = reinterpret_cast<const uint32_t *>(cbase + pr.cv.off_offsets);
+  const size_t rtb = raw_tile_bytes(32, tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
+  const bool issuer = q == 0, loader = q == 1;
+  uint32_t fin_stripe[2] = {0, 0};
+  bool fin_valid[2] = {false, false};
+
+  // X loader state (warp 1, lane 0): the (pair-in-stripe, unit) of the NEXT unit step to fetch
+  uint32_t lx_kp = p_begin % PK, lx_u = 0, lx_n = 0;
+  auto load_next_x = [&]() {   // issues the two X slices of unit step lx_n, then advances
+    const uint32_t ktA = 2u * lx_kp, sl = lx_n & 1u, bar = xfull_s + 8 * sl;
+    const bool hasB = ktA + 1 < KT;
+    const int kA = int(ktA * tile_k + lx_u * kUnitK);
+    mbar_arrive_expect_tx(bar, hasB ? 2 * xbytes : xbytes);
+    tma_load_2d(xring_s + (sl * 2u) * P.xslice_bytes, xmap, kA, 0, bar);
+    if (hasB) tma_load_2d(xring_s + (sl * 2u + 1u) * P.xslice_bytes, xmap, kA + int(tile_k), 0, bar);
+    ++lx_n;
+    if (++lx_u == units) { lx_u = 0; if (++lx_kp == PK) lx_kp = 0; }
+  };
+  const uint64_t bdesc0 = make_smem_desc(xring_s, 16, 256, kLayoutSW32);
+  const uint32_t bdesc_step = P.xslice_bytes >> 4;
+
+  uint32_t n = 0, seg_i = 0;
+  bool dep_waited = false;
+  TRACE(1);
+  PROF_DECL
+#pragma unroll 1
+  for (uint32_t p = p_begin; p < p_end; ++seg_i) {
+    const uint32_t stripe = p / PK, kp0 = p % PK, np = min(PK - kp0, p_end - p);
+    const bool whole = kp0 == 0 && np == PK;
+#pragma unroll 1
+    for (uint32_t i = 0; i < np; ++i) {
+      const uint32_t ktA = 2u * (kp0 + i);
+      const bool hasB = ktA + 1 < KT;
+      LaneStream s[2];
+      uint32_t tile[2];
+      tile[0] = (stripe * KT + ktA) * 4u + q;
+      tile[1] = hasB ? tile[0] + 4u : tile[0];   // odd KT: the second chain re-decodes the first tile; its output is never multiplied
+      const uint8_t *rawp[2] = {nullptr, nullptr};   // this lane's 16 bytes of the NEXT raw vector to fetch
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const uint8_t *rec = cbase + off_records + size_t(offs[tile[j]]) * 16;
+        lane_open(s[j], rec, int(units / kUnitsPerSeg), lane);
+        if (kRaw) {
+          rawp[j] = cbase + off_raw + size_t(tile[j]) * rtb + 16 * lane;
+          cp_async16(rawbuf_s + uint32_t(j) * kRawBufBytes + 16u * uint32_t(lane), rawp[j]);   // vector 0 -> parity 0 (completes with the segment staging)
+          rawp[j] += 512;
+        }
+      }
+      // the records of this warp's next pair: pulled into L2 during the first unit
+      const bool has_next = p + i + 1 < p_end;
+      uint32_t next_tile = 0, next_off[2] = {0, 0};
+      if (has_next) {
+        const uint32_t pn = p + i + 1, sn = pn / PK, kn = 2u * (pn % PK);
+        next_tile = (sn * KT + kn) * 4u + q;
+        next_off[0] = offs[next_tile];
+        next_off[1] = offs[next_tile + (kn + 1 < KT ? 4u : 0u)];
+      }
+#pragma unroll 1
+      for (uint32_t u = 0; u < units; ++u, ++n) {
+        if (u == 1 && has_next) {
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            if (lane < 24) prefetch_l2(cbase + off_records + size_t(next_off[j]) * 16 + lane * 128);
+            else if (kRaw) prefetch_l2(cbase + off_raw + size_t(next_tile + 4u * uint32_t(j)) * rtb + (lane - 24) * 128);
+          }
+        }
+        if (u % kUnitsPerSeg == 0) lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);   // drains cp.async first and last
+        if (!dep_waited) {   // everything before this point read the container only
+          grid_dep_wait();
+          dep_waited = true;
+          if (loader && lane == 0) load_next_x();
+        }
+        const bool last_unit = u + 1 == units;
+        uint4 rv[2] = {make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0)};
+        uint32_t sz[2] = {0, 0};
+        if constexpr (kRaw) {
+          // this unit's raw vector was copied during the previous unit; fetch the next one into the other half
+          cp_async_wait_all();
+          const uint32_t rb = rawbuf_s + (u & 1u) * 512u;
+          if (PAYLOAD && last_unit) {
+            // last vector with the state-payload flag: 7 sub-rows of 32 x 2 bytes (bytes 14, 15 come from the end state)
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              uint32_t h[7];
+#pragma unroll
+              for (int k = 0; k < 7; ++k) h[k] = lds16(rb + uint32_t(j) * kRawBufBytes + uint32_t(k) * 64u + 2u * uint32_t(lane));
+              rv[j] = make_uint4(h[0] | (h[1] << 16), h[2] | (h[3] << 16), h[4] | (h[5] << 16), h[6]);
+            }
+          } else {
+#pragma unroll
+            for (int j = 0; j < 2; ++j) rv[j] = lds128(rb + uint32_t(j) * kRawBufBytes + 16u * uint32_t(lane));
+          }
+          if (!last_unit) {
+            const bool short_vec = PAYLOAD && u + 2 == units;   // the next vector is the payload-shortened one: 448 bytes
+            if (!short_vec || lane < 28) {
+#pragma unroll
+              for (int j = 0; j < 2; ++j) cp_async16(rawbuf_s + uint32_t(j) * kRawBufBytes + ((u + 1) & 1u) * 512u + 16u * uint32_t(lane), rawp[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < 2; ++j) rawp[j] += 512;
+            cp_async_commit();
+          }
+        }
+        if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
+#pragma unroll
+          for (int j = 0; j < 2; ++j) {
+            const uint32_t k_elem = (ktA + uint32_t(j)) * tile_k + u * kUnitK;
+            sz[j] = __ldg(reinterpret_cast<const uint32_t *>(cbase + off_scales) + size_t(k_elem / qgroup) * n_out + size_t(stripe) * kTileN +
+                          q * 32u + uint32_t(lane));
+          }
+        }
+        uint32_t r[2][8];
+        PROF(0);
+        decode_unit_regs<FMT, PAYLOAD>(s, tab_s, dir, last_unit, rv, sz, r);
+        PROF(1);
+        // ---- hand-over: registers -> tensor memory -> tcgen05.mma ----
+        if (n > 0) mbar_wait(done_s + 8 * ((n - 1) & 1u), ((n - 1) >> 1) & 1u);   // the MMAs of step n-1 have read the operand columns
+        PROF(2);
+        tmem_st8(a_t + lane_t, r[0]);
+        tmem_st8(a_t + kACols + lane_t, r[1]);
+        tmem_wait_st();
+        tc_fence_before();
+        PROF(3);
+        if (!issuer) {
+          named_bar_arrive(bar_id, kNT);
+          // ring slot (n+1)&1 was last read by the MMAs of step n-1: their completion was waited for above
+          if (loader && lane == 0 && lx_n < N) load_next_x();
+        } else {
+          named_bar_sync(bar_id, kNT);
+          tc_fence_after();
+          PROF(4);
+          mbar_wait(xfull_s + 8 * (n & 1u), (n >> 1) & 1u);
+          if (lane == 0) {
+            const uint32_t sl = n & 1u;
+            const uint64_t bdA = bdesc0 + uint64_t(sl * 2u * bdesc_step);
+            umma_ts<TR::kind>(acc_t, a_t, bdA, idesc, (i == 0 && u == 0) ? 0u : 1u);
+            if (hasB) umma_ts<TR::kind>(acc_t, a_t + kACols, bdA + bdesc_step, idesc, 1u);
+            umma_commit(done_s + 8 * sl);
+            if (i + 1 == np && last_unit) umma_commit(accfull_s);
+          }
+          __syncwarp();
+          PROF(5);
+        }
+      }
+    }
+    PROF_DUMP;
+    // ---- epilogue of this stripe segment: the team reads its own accumulator ----
+    TRACE(2);
+    mbar_wait(accfull_s, seg_i & 1u);
+    TRACE(3);
+    tc_fence_after();
+    {
+      const uint32_t row = q * 32u + uint32_t(lane), nrow = stripe * kTileN + row;
+      float ws = 1.0f;
+      if (FMT == ANSLIN_FMT_INT8) ws = __half2float(ep.w_scale_h[nrow]);
+      if (is_fp8_path(FMT)) ws = ep.w_scale;
+      const uint32_t seg = (p == p_begin ? 0u : 1u);
+      uint32_t *part = ep.partials + size_t(v * 2u + seg) * mpad * kTileN;
+      for (uint32_t c0 = 0; c0 < mpad; c0 += 16) {
+        uint32_t val[16];
+        tmem_ld16(acc_t + lane_t + c0, val);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const uint32_t mm = c0 + j;
+          if (mm < ep.m) {
+            if (whole) {
+              const float f = finalize<FMT>(val[j], kScaled ? ep.x_scale[mm] : 1.0f, ws);
+              if constexpr (YB) reinterpret_cast<__nv_bfloat16 *>(ep.y)[size_t(mm) * ep.ldy + nrow] = __float2bfloat16_rn(f);
+              else ep.y[size_t(mm) * ep.ldy + nrow] = f;
+            } else {
+              part[size_t(mm) * kTileN + row] = val[j];
+            }
+          }
+        }
+      }
+      tc_fence_before();   // the next segment's first MMA (after the next team barrier) overwrites the accumulator
+      if (!whole) {
+        __threadfence();
+        named_bar_sync(bar_id, kNT);
+        if (issuer && lane == 0) {
+          uint32_t *flag = reinterpret_cast<uint32_t *>(ep.counters) + (v * 2u + seg);
+          asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(ep.epoch) : "memory");
+        }
+        if (seg == 0) { fin_stripe[0] = stripe; fin_valid[0] = true; }
+        else { fin_stripe[1] = stripe; fin_valid[1] = true; }
+      }
+    }
+    p += np;
+  }
+  cp_async_wait_all();
+  TRACE(4);
+  // ---- split-K: reduce this team's slice of every stripe it holds a partial of ----
+  if (!dep_waited) grid_dep_wait();
+  const uint32_t tid = q * 32u + uint32_t(lane);
+#pragma unroll 1
+  for (int sg = 0; sg < 2; ++sg) {
+    if (!(sg == 0 ? fin_valid[0] : fin_valid[1])) continue;
+    const StripeTeams st(V, Ptot, PK, sg == 0 ? fin_stripe[0] : fin_stripe[1]);
+    team_reduce<FMT, YB>(ep, st, st.index_of(v, p_begin), tid, bar_id);
+  }
+  TRACE(5);
+  tc_fence_before();
+  __syncthreads();
+  TRACE(6);
+  if (warp == 0) tmem_dealloc(tmem_base, 512);
+}

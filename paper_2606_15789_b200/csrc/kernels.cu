@@ -553,6 +553,8 @@ struct SmemEmit {
   __device__ __forceinline__ void packed8(int, int, int, uint32_t, uint32_t) const {}
 };
 
+#include "fused_tmem.cuh"
+
 template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS, bool YB>
 __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ TensorMaps tms,
                                                                       const __grid_constant__ FusedParams P) {
@@ -930,7 +932,7 @@ uint32_t next_epoch() {
 }
 
 // bytes of a problem's split-K flag area (two u32 flags per CTA; sized generously by stripes too so that older callers' sizes hold)
-size_t flag_bytes(uint32_t stripes) { return align16(size_t(stripes) * 8 + 256 + 8 * 160); }
+size_t flag_bytes(uint32_t stripes) { return align16(size_t(stripes) * 8 + 256 + 8 * 160 * kMaxTeams); }
 struct Workspace { size_t counters_off, partials_off, total; };
 Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
   Workspace w;
@@ -965,19 +967,81 @@ int launch_fused_y(const TensorMaps &tms, const FusedParams &p, uint32_t grid, s
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // lets the kernel's prologue overlap its predecessor's tail
-  attr[0].val.programmaticStreamSerializationAllowed = getenv("ANSLIN_NO_PDL") ? 0 : 1;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if (cudaLaunchKernelEx(&cfg, kern, tms, p) != cudaSuccess) return ANSLIN_ERR_CUDA;
   ++g_launches;
-  if (getenv("ANSLIN_DEBUG")) {  // debugging aid only: synchronous error report
-    cudaError_t e = cudaStreamSynchronize(st);
-    fprintf(stderr, "[anslin] fused grid=%u smem=%zu D=%u U=%u nprob=%u: %s\n", grid, smem, p.D, p.U, p.nprob, cudaGetErrorString(e));
-  }
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 
+// Teams per CTA of the TMEM design (fused_tmem.cuh) for the largest padded batch of a launch and the staged segment size:
+// bounded by tensor memory (mpad accumulator + 16 operand columns per team) and by shared memory; 0 = does not fit.
+uint32_t tmem_teams(uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
+  uint32_t T = std::min<uint32_t>(kMaxTeams, 512u / (mpad_max + 2 * kACols));
+  while (T > 0 && tmem_smem_bytes(T, mpad_max, stream_bytes, fmt) > kSmemMax) --T;
+  return T;
+}
+bool tmem_eligible(const Header &h) {
+  return (h.flags & ANSLIN_FLAG_LANE_STREAMS) && h.tile_n == 32 && h.format != ANSLIN_FMT_BF16_PAIR4 && h.tile_k / unit_k_of(h.format) >= 2;
+}
+
+template <uint32_t FMT, bool PAYLOAD, bool YB>
+int launch_tmem_y(const TensorMaps &tms, const TmemParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
+  auto kern = fused_tmem_kernel<FMT, PAYLOAD, YB>;
+  static thread_local size_t smem_set = 0;
+  if (smem > smem_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
+    smem_set = kSmemMax;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(32 * kTeamWarps * p.T);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // the prologue overlaps the predecessor's tail
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, kern, tms, p) != cudaSuccess) return ANSLIN_ERR_CUDA;
+  ++g_launches;
+  return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
+}
+template <uint32_t FMT, bool PAYLOAD>
+int launch_tmem(bool ybf, const TensorMaps &tms, const TmemParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
+  return ybf ? launch_tmem_y<FMT, PAYLOAD, true>(tms, p, grid, smem, st) : launch_tmem_y<FMT, PAYLOAD, false>(tms, p, grid, smem, st);
+}
+
 // One launch over n <= kMaxProblems independent GEMMs that share format and tile geometry.
+// CTAs of a persistent launch, shared out between its problems in proportion to their sizes: each problem at least one CTA
+// and at most `cap[i]`, never more than S in total when n <= S.
+void share_ctas(int n, const uint64_t *work, const uint32_t *cap, uint32_t S, uint32_t *ncta) {
+  uint64_t work_sum = 0;
+  for (int i = 0; i < n; ++i) work_sum += work[i];
+  uint32_t used = 0;
+  for (int i = 0; i < n; ++i) {
+    ncta[i] = uint32_t(std::min<uint64_t>(cap[i], std::max<uint64_t>(1, uint64_t(S) * work[i] / work_sum)));
+    used += ncta[i];
+  }
+  while (used > S) {   // the one-CTA minimum of tiny problems: take CTAs back from the problem with the least work per CTA
+    int worst = -1;
+    for (int i = 0; i < n; ++i)
+      if (ncta[i] > 1 && (worst < 0 || work[i] * ncta[worst] < work[worst] * ncta[i])) worst = i;
+    if (worst < 0) break;
+    --ncta[worst]; --used;
+  }
+  for (bool grown = true; used < S && grown;) {  // hand out what rounding left over, largest work per CTA first
+    grown = false;
+    int best = -1;
+    for (int i = 0; i < n; ++i) {
+      if (ncta[i] >= cap[i]) continue;
+      if (best < 0 || work[i] * ncta[best] > work[best] * ncta[i]) best = i;
+    }
+    if (best >= 0) { ++ncta[best]; ++used; grown = true; }
+  }
+}
+
 int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, uint32_t x_dtype, const int64_t *ldx, const int32_t *ms,
                 const void *const *x_scales, void *const *ys, const int64_t *ldy, void *workspace_dev, size_t workspace_bytes,
                 cudaStream_t st, uint32_t y_dtype = ANSLIN_DT_F32) {
@@ -989,7 +1053,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   const int xb = (is_bf16_like(h0.format) || h0.format == ANSLIN_FMT_INT4_AWQ) ? 2 : 1;
   if (!x_dtype_ok(h0.format, x_dtype)) return ANSLIN_ERR_INVALID_ARG;
   uint32_t mpad_max = 16;
-  uint64_t work[kMaxProblems], work_sum = 0;
+  uint64_t work[kMaxProblems];
   for (int i = 0; i < n; ++i) {
     const anslin_weight *w = ws[i];
     if (!w || !w->dev || !xs[i] || !ys[i]) return ANSLIN_ERR_INVALID_ARG;
@@ -1001,28 +1065,93 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     if (ldx[i] < int64_t(h.k_in) || (ldx[i] * xb) % 16 || ldy[i] < int64_t(h.n_out)) return ANSLIN_ERR_INVALID_ARG;
     mpad_max = std::max(mpad_max, mpad_of(ms[i]));
     work[i] = uint64_t(h.n_out) * h.k_in;
-    work_sum += work[i];
   }
-  FusedParams p;
-  TensorMaps tms;
-  memset(&p, 0, sizeof(p));
-  p.nprob = uint32_t(n);
-  p.slot_bytes = kUnitBytes + mpad_max * 32u;
-  p.tmem_cols = tmem_cols_of(mpad_max);
   const int RB = int(h0.tile_n) / 32, J = RB == 1 ? kJ32 : 1, NW = 4 / (RB * J);
-  // shared memory: U operand slots, D*J stream rings, slot table, barriers
-  const size_t fixed = 2048 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 96;
   const bool ls = h0.flags & ANSLIN_FLAG_LANE_STREAMS;
   if (ls && RB != 1) return ANSLIN_ERR_CORRUPT;
   uint32_t stream_bytes = kStreamSmem;
+  bool tmem_ok = true;
   if (ls) {
     stream_bytes = 32;
-    for (int i = 0; i < n; ++i) stream_bytes = std::max<uint32_t>(stream_bytes, uint32_t(align16(ws[i]->h.max_seg_bytes)));
+    for (int i = 0; i < n; ++i) {
+      stream_bytes = std::max<uint32_t>(stream_bytes, uint32_t(align16(ws[i]->h.max_seg_bytes)));
+      tmem_ok = tmem_ok && tmem_eligible(ws[i]->h);
+    }
   }
+  // which design: decoded operand through tensor memory (fused_tmem.cuh) or through shared-memory operand slots
+  const uint32_t T = (ls && tmem_ok) ? tmem_teams(mpad_max, stream_bytes, h0.format) : 0u;
+  const bool use_tmem = T >= 2;
+  // CTAs: one per SM in total, shared out in proportion to the problems' sizes
+  const uint32_t S = uint32_t(sm_budget());
+  uint32_t ncta[kMaxProblems], cap[kMaxProblems];
+  for (int i = 0; i < n; ++i) cap[i] = (ws[i]->h.n_out / kTileN) * (ws[i]->h.k_in / ws[i]->h.tile_k);
+  share_ctas(n, work, cap, S, ncta);
+  // workspace: flags of all problems, then the split-K partials (two per CTA, or two per team)
+  const uint32_t teams = use_tmem ? T : 1u;
+  size_t off = 0;
+  uint8_t *wsb = static_cast<uint8_t *>(workspace_dev);
+  size_t counters_bytes = 0;
+  for (int i = 0; i < n; ++i) counters_bytes += flag_bytes(ws[i]->h.n_out / kTileN);
+  size_t part_off = counters_bytes;
+  uint32_t cta0 = 0;
+  Problem prob[kMaxProblems];
+  TensorMaps tms;
+  for (int i = 0; i < n; ++i) {
+    const Header &h = ws[i]->h;
+    Problem &q = prob[i];
+    q.cv = view_of(ws[i]);
+    q.x_scale = static_cast<const float *>(x_scales ? x_scales[i] : nullptr);
+    q.y = static_cast<float *>(ys[i]);
+    q.ldy = ldy[i];
+    q.m = uint32_t(ms[i]);
+    q.mpad = mpad_of(ms[i]);
+    q.cta0 = cta0;
+    q.ncta = ncta[i];
+    cta0 += ncta[i];
+    q.counters = reinterpret_cast<unsigned long long *>(wsb + off);
+    off += flag_bytes(h.n_out / kTileN);
+    q.partials = reinterpret_cast<uint32_t *>(wsb + part_off);
+    part_off += size_t(ncta[i]) * teams * 2 * q.mpad * kTileN * 4;
+    const uint32_t uk = unit_k_of(h.format);
+    if (!make_map_2d(&tms.m[i], xs[i], xb, h.k_in, uint64_t(ms[i]), uint64_t(ldx[i]), uk, q.mpad, CU_TENSOR_MAP_SWIZZLE_32B))
+      return ANSLIN_ERR_CUDA;
+  }
+  if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
+  const uint32_t grid = cta0;
+  const bool ybf = y_dtype == ANSLIN_DT_BF16;
+  const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
+  if (use_tmem) {
+    TmemParams p;
+    memset(&p, 0, sizeof(p));
+    memcpy(p.prob, prob, sizeof(Problem) * size_t(n));
+    p.nprob = uint32_t(n);
+    p.T = T;
+    p.epoch = next_epoch();
+    p.stream_bytes = stream_bytes;
+    p.xslice_bytes = mpad_max * 32u;
+    p.tmem_stride = mpad_max + 2 * kACols;
+    p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
+    const size_t smem = tmem_smem_bytes(T, mpad_max, stream_bytes, h0.format);
+    switch (h0.format) {
+      case ANSLIN_FMT_BF16: return pay ? launch_tmem<ANSLIN_FMT_BF16, true>(ybf, tms, p, grid, smem, st) : launch_tmem<ANSLIN_FMT_BF16, false>(ybf, tms, p, grid, smem, st);
+      case ANSLIN_FMT_FP8_E4M3:
+      case ANSLIN_FMT_FP8_E5M2: return launch_tmem<ANSLIN_FMT_FP8_E4M3, false>(ybf, tms, p, grid, smem, st);
+      case ANSLIN_FMT_INT8: return launch_tmem<ANSLIN_FMT_INT8, false>(ybf, tms, p, grid, smem, st);
+      case ANSLIN_FMT_INT4_AWQ: return launch_tmem<ANSLIN_FMT_INT4_AWQ, false>(ybf, tms, p, grid, smem, st);
+      case ANSLIN_FMT_FP4_E2M1: return launch_tmem<ANSLIN_FMT_FP4_E2M1, false>(ybf, tms, p, grid, smem, st);
+    }
+    return ANSLIN_ERR_UNSUPPORTED;
+  }
+  FusedParams p;
+  memset(&p, 0, sizeof(p));
+  memcpy(p.prob, prob, sizeof(Problem) * size_t(n));
+  p.nprob = uint32_t(n);
+  p.slot_bytes = kUnitBytes + mpad_max * 32u;
+  p.tmem_cols = tmem_cols_of(mpad_max);
+  // shared memory: U operand slots, D*J stream rings, slot table, barriers
+  const size_t fixed = 2048 /*align slack*/ + 16384 + 1056 + 16 * kMaxSlots + 96;
   p.stream_bytes = stream_bytes;
   uint32_t D = kMaxDecWarps, U = 0;
-  if (const char *denv = getenv("ANSLIN_DECODER_WARPS"))
-    if (atoi(denv) > 0) D = uint32_t(std::min(atoi(denv), kMaxDecWarps));
   D -= D % NW;
   uint32_t Bslots = 0;
   for (; D >= uint32_t(NW); D -= NW) {   // most decoder warps that still leave every team two private operand slots
@@ -1039,59 +1168,8 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   p.U = U;
   p.B = Bslots;
   const size_t smem = fixed + size_t(D) * J * stream_bytes + size_t(U) * p.slot_bytes;
-  // CTAs: one per SM in total, shared out in proportion to the problems' sizes (each at least one, at most one per group)
-  const uint32_t S = uint32_t(sm_budget());
-  uint32_t ncta[kMaxProblems], used = 0;
-  for (int i = 0; i < n; ++i) {
-    const Header &h = ws[i]->h;
-    const uint32_t groups = (h.n_out / kTileN) * (h.k_in / h.tile_k);
-    ncta[i] = uint32_t(std::min<uint64_t>(groups, std::max<uint64_t>(1, uint64_t(S) * work[i] / work_sum)));
-    used += ncta[i];
-  }
-  for (bool grown = true; used < S && grown;) {  // hand out what rounding left over, largest work per CTA first
-    grown = false;
-    int best = -1;
-    for (int i = 0; i < n; ++i) {
-      const Header &h = ws[i]->h;
-      const uint32_t groups = (h.n_out / kTileN) * (h.k_in / h.tile_k);
-      if (ncta[i] >= groups) continue;
-      if (best < 0 || work[i] * ncta[best] > work[best] * ncta[i]) best = i;
-    }
-    if (best >= 0) { ++ncta[best]; ++used; grown = true; }
-  }
-  // workspace: counters of all problems, then partials carved by the CTAs each problem got
-  size_t off = 0;
-  uint8_t *wsb = static_cast<uint8_t *>(workspace_dev);
-  size_t counters_bytes = 0;
-  for (int i = 0; i < n; ++i) counters_bytes += flag_bytes(ws[i]->h.n_out / kTileN);
-  size_t part_off = counters_bytes;
-  uint32_t cta0 = 0;
-  for (int i = 0; i < n; ++i) {
-    const Header &h = ws[i]->h;
-    Problem &q = p.prob[i];
-    q.cv = view_of(ws[i]);
-    q.x_scale = static_cast<const float *>(x_scales ? x_scales[i] : nullptr);
-    q.y = static_cast<float *>(ys[i]);
-    q.ldy = ldy[i];
-    q.m = uint32_t(ms[i]);
-    q.mpad = mpad_of(ms[i]);
-    q.cta0 = cta0;
-    q.ncta = ncta[i];
-    cta0 += ncta[i];
-    q.counters = reinterpret_cast<unsigned long long *>(wsb + off);
-    off += flag_bytes(h.n_out / kTileN);
-    q.partials = reinterpret_cast<uint32_t *>(wsb + part_off);
-    part_off += size_t(ncta[i]) * 2 * q.mpad * kTileN * 4;
-    const uint32_t uk = unit_k_of(h.format);
-    if (!make_map_2d(&tms.m[i], xs[i], xb, h.k_in, uint64_t(ms[i]), uint64_t(ldx[i]), uk, q.mpad, CU_TENSOR_MAP_SWIZZLE_32B))
-      return ANSLIN_ERR_CUDA;
-  }
-  if (workspace_bytes < part_off) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   p.epoch = next_epoch();
   p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
-  const bool ybf = y_dtype == ANSLIN_DT_BF16;
-  const bool pay = h0.flags & ANSLIN_FLAG_STATE_PAYLOAD;
-  const uint32_t grid = cta0;
 #define launch_fused(...) (ybf ? launch_fused_y<__VA_ARGS__, true>(tms, p, grid, smem, st) : launch_fused_y<__VA_ARGS__, false>(tms, p, grid, smem, st))
 #define ANSLIN_LAUNCH(F, PAY)                                                                                   \
   (RB == 1 ? (ls ? launch_fused(F, 1, PAY, true) : launch_fused(F, 1, PAY, false)) \
@@ -1115,12 +1193,24 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
 size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_max) {
   if (!ws || n < 1 || m_max < 1 || m_max > 256) return 0;
   size_t counters = 0;
+  uint32_t stream_bytes = 32;
+  bool tmem_ok = true;
   for (int i = 0; i < n; ++i) {
     if (!ws[i]) return 0;
     counters += flag_bytes(ws[i]->h.n_out / kTileN);
+    stream_bytes = std::max<uint32_t>(stream_bytes, uint32_t(align16(ws[i]->h.max_seg_bytes)));
+    tmem_ok = tmem_ok && tmem_eligible(ws[i]->h);
   }
-  // all problems of a launch share one CTA per SM, so their partials never exceed one problem's worst case
-  const size_t per_launch = size_t(std::max(sm_budget(), 148)) * 2 * mpad_of(m_max) * kTileN * 4;
+  // all problems of a launch share one CTA per SM, so their partials never exceed one problem's worst case: two partials
+  // per CTA, or per team of the tensor-memory design (a smaller batch may run with more teams: take the largest
+  // teams x mpad product up to m_max)
+  size_t rows = mpad_of(m_max);
+  if (tmem_ok)
+    for (uint32_t mp = 16; mp <= mpad_of(m_max); mp += 16) {
+      const uint32_t T = tmem_teams(mp, stream_bytes, ws[0]->h.format);
+      if (T >= 2) rows = std::max(rows, size_t(T) * mp);
+    }
+  const size_t per_launch = size_t(std::max(sm_budget(), 148)) * 2 * rows * kTileN * 4;
   return counters + per_launch;
 }
 
@@ -1145,7 +1235,6 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
     smem_occ = smem;
   }
   uint32_t per_sm = uint32_t(occ);
-  if (const char *e = getenv("ANSLIN_DECODE_CTAS_PER_SM")) per_sm = uint32_t(std::max(1, atoi(e)));  // debug knob
   const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
   kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out), stream_bytes);
   ++g_launches;
@@ -1169,6 +1258,15 @@ int launch_dense(const CUtensorMap &tmw, const CUtensorMap &tmx, DenseParams &p,
 }  // namespace
 
 extern "C" {
+
+#ifdef ANSLIN_TRACE
+int anslin_debug_trace(void *host_out, size_t bytes) {
+  return cudaMemcpyFromSymbol(host_out, g_trace, std::min(bytes, sizeof(g_trace))) == cudaSuccess ? 0 : 5;
+}
+int anslin_debug_prof(void *host_out, size_t bytes) {
+  return cudaMemcpyFromSymbol(host_out, g_prof, std::min(bytes, sizeof(g_prof))) == cudaSuccess ? 0 : 5;
+}
+#endif
 
 int anslin_last_launch_count(void) { return g_launches; }
 
