@@ -199,8 +199,11 @@ __device__ __forceinline__ void lane_open(LaneStream &s, const uint8_t *rec, int
 // stream_drain).  The segment tables and the words are fetched together: when the buffer is no larger than the
 // container's tail rule allows to over-read, the whole buffer is copied from the segment start without waiting
 // for the table to say how many words there are.
-template <int J>
-__device__ __forceinline__ void lane_open_segments(LaneStream (&s)[J], uint32_t buf0, uint32_t bufbytes, int seg, int lane) {
+struct NoExtraCopies { __device__ __forceinline__ void operator()() const {} };
+// extra(): further cp.async copies of the caller, issued into the same group as the segment's (one wait for both)
+template <int J, class Extra = NoExtraCopies>
+__device__ __forceinline__ void lane_open_segments(LaneStream (&s)[J], uint32_t buf0, uint32_t bufbytes, int seg, int lane,
+                                                   const Extra &extra = Extra()) {
   stream_drain();
   const bool spec = bufbytes <= uint32_t(kTailBytes);
   uint32_t hdr[J], delta[J];
@@ -238,6 +241,7 @@ __device__ __forceinline__ void lane_open_segments(LaneStream (&s)[J], uint32_t 
     s[j].ptr = buf + skew + 2u * ((lane & 1) ? end_p - 1u : start_p);
     s[j].goff += 2u * total;
   }
+  extra();
   cp_async_commit();
   stream_drain();
   // look-ahead word (a lane without words in this segment reads a neighbour's or stale bytes: never used)

@@ -162,36 +162,37 @@ __device__ unsigned long long g_prof[160 * kMaxTeams * 4 * 8];
 #define PROF_DUMP do {} while (0)
 #endif
 
-// The contributors of a stripe, in the order their partials are summed: the distinct teams that own one of its pairs.
-struct StripeTeams {
-  uint32_t V, Ptot, PK, stripe, v_first, v_last, count;
-  bool dense;   // V <= Ptot: every team has work, the contributors are v_first..v_last
-  __device__ __forceinline__ StripeTeams(uint32_t V_, uint32_t Ptot_, uint32_t PK_, uint32_t stripe_)
-      : V(V_), Ptot(Ptot_), PK(PK_), stripe(stripe_) {
-    v_first = cta_of_tile(stripe * PK, V, Ptot);
-    v_last = cta_of_tile(stripe * PK + PK - 1, V, Ptot);
-    dense = V <= Ptot;
-    count = dense ? v_last - v_first + 1 : PK;   // more teams than pairs: one team per pair
+// Two-level stream-K split of the stripe-major sequence of Ptot (stripe, k-tile pair) items: first evenly over the G CTAs of
+// the problem (so that every SM gets the same amount of work), then evenly over the T teams of a CTA.  Team v = c * T + t.
+struct TeamMap {
+  uint32_t G, T, Ptot;
+  __device__ __forceinline__ uint32_t first(uint32_t v) const {   // first pair of team v (v = G * T: Ptot)
+    const uint32_t c = v / T, t = v - c * T;
+    const uint32_t a = cta_first_tile(c, G, Ptot), nc = cta_first_tile(c + 1, G, Ptot) - a;
+    return a + uint32_t(uint64_t(t) * nc / T);
   }
-  __device__ __forceinline__ uint32_t team(uint32_t k) const { return dense ? v_first + k : cta_of_tile(stripe * PK + k, V, Ptot); }
-  __device__ __forceinline__ uint32_t index_of(uint32_t v, uint32_t first_pair_of_v) const {
-    return dense ? v - v_first : first_pair_of_v - stripe * PK;
-  }
-  // partial slot of contributor vv: its first segment (slot 0) unless the stripe is its second one, which can only be the
-  // case for the first contributor (every later one starts inside the stripe)
-  __device__ __forceinline__ uint32_t slot(uint32_t vv) const {
-    return vv * 2u + ((vv == v_first && cta_first_tile(vv, V, Ptot) < stripe * PK) ? 1u : 0u);
+  __device__ __forceinline__ uint32_t owner(uint32_t p) const {   // the team that owns pair p
+    const uint32_t c = cta_of_tile(p, G, Ptot);
+    const uint32_t a = cta_first_tile(c, G, Ptot), nc = cta_first_tile(c + 1, G, Ptot) - a;
+    return c * T + cta_of_tile(p - a, T, nc);
   }
 };
 
 // Distributed deterministic split-K reduction of one stripe by one of its contributors (all 128 threads of the team).
+// The contributors are the distinct owners of the stripe's PK pairs, in pair order; contributor vv's partial slot is its first
+// segment (slot 0) unless the stripe is its second one, which can only be the case for the stripe's first contributor.
 template <uint32_t FMT, bool YB>
-__device__ __forceinline__ void team_reduce(const EpiParams &p, const StripeTeams &st, uint32_t my_index, uint32_t tid, int bar) {
+__device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &tm, uint32_t PK, uint32_t stripe, uint32_t v, uint32_t tid,
+                                            int bar, uint32_t *list /* team-private shared scratch, PK + 1 words */) {
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   uint32_t *flags = reinterpret_cast<uint32_t *>(p.counters);
-  // wait for every contributor's partial (one flag per thread)
-  for (uint32_t k = tid; k < st.count; k += kNT) {
-    const uint32_t *flag = flags + st.slot(st.team(k));
+  const uint32_t p0 = stripe * PK;
+  // the partial slot of every pair's owner (one pair per thread), then wait for that partial's flag
+  for (uint32_t k = tid; k < PK; k += kNT) {
+    const uint32_t vv = tm.owner(p0 + k), v_first = tm.owner(p0);
+    const uint32_t slot = vv * 2u + ((vv == v_first && tm.first(v_first) < p0) ? 1u : 0u);
+    list[k] = slot;
+    const uint32_t *flag = flags + slot;
     uint32_t val, spins = 0;
     while (true) {
       asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(val) : "l"(flag) : "memory");
@@ -201,30 +202,44 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const StripeTeam
     }
   }
   named_bar_sync(bar, kNT);
+  // how many contributors, and which one am I (consecutive pairs of one owner share a slot)
+  uint32_t count = 0, my_index = 0;
+  for (uint32_t k = 0, prev = 0xFFFFFFFFu; k < PK; ++k) {
+    const uint32_t sl = list[k];
+    if (sl != prev) { if ((sl >> 1) == v) my_index = count; ++count; prev = sl; }
+  }
   const size_t slot_words = size_t(p.mpad) * kTileN;
   const uint32_t n_items = p.m * 32u;   // one item = one batch row x 4 output channels
-  const uint32_t it_begin = uint32_t(uint64_t(my_index) * n_items / st.count), it_end = uint32_t(uint64_t(my_index + 1) * n_items / st.count);
+  const uint32_t it_begin = uint32_t(uint64_t(my_index) * n_items / count), it_end = uint32_t(uint64_t(my_index + 1) * n_items / count);
   for (uint32_t it = it_begin + tid; it < it_end; it += kNT) {
     const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u;
+    const uint32_t *src = p.partials + size_t(mm) * kTileN + r4;
     uint32_t acc[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-    for (uint32_t kb = 0; kb < st.count; kb += 8) {
+    uint32_t prev = 0xFFFFFFFFu;
+    for (uint32_t kb = 0; kb < PK; kb += 8) {
       uint4 val[8];
+      bool use[8];
 #pragma unroll
       for (int j = 0; j < 8; ++j) {
-        val[j] = make_uint4(0, 0, 0, 0);
-        if (kb + j < st.count) val[j] = ldcg128(p.partials + size_t(st.slot(st.team(kb + j))) * slot_words + size_t(mm) * kTileN + r4);
+        use[j] = false;
+        if (kb + j < PK) {
+          const uint32_t sl = list[kb + j];
+          use[j] = sl != prev;
+          prev = sl;
+          if (use[j]) val[j] = ldcg128(src + size_t(sl) * slot_words);
+        }
       }
 #pragma unroll
       for (int j = 0; j < 8; ++j) {   // fixed team order -> bit-reproducible sums
-        if (kb + j < st.count) {
+        if (use[j]) {
           acc[0] = acc_add<FMT>(acc[0], val[j].x); acc[1] = acc_add<FMT>(acc[1], val[j].y);
           acc[2] = acc_add<FMT>(acc[2], val[j].z); acc[3] = acc_add<FMT>(acc[3], val[j].w);
         }
       }
     }
-    const uint32_t n4 = st.stripe * kTileN + r4;
+    const uint32_t n4 = stripe * kTileN + r4;
     const float xs = kScaled ? p.x_scale[mm] : 1.0f;
     float o[4];
 #pragma unroll
@@ -251,17 +266,17 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const StripeTeam
   // (stale or never written bytes) reads as zero readers.
   named_bar_sync(bar, kNT);
   if (tid == 0) {
-    uint32_t *cnt = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(p.counters) + kTmStripeCntOff) + st.stripe;
+    uint32_t *cnt = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(p.counters) + kTmStripeCntOff) + stripe;
     const uint32_t tag = (p.epoch << 8);
     uint32_t old = *reinterpret_cast<volatile uint32_t *>(cnt), done;
     while (true) {
       done = ((old & 0xFFFFFF00u) == tag ? (old & 0xFFu) : 0u) + 1u;
-      const uint32_t seen = atomicCAS(cnt, old, done == st.count ? 0u : (tag | done));
+      const uint32_t seen = atomicCAS(cnt, old, done == count ? 0u : (tag | done));
       if (seen == old) break;
       old = seen;
     }
-    if (done == st.count) {
-      for (uint32_t k = 0; k < st.count; ++k) flags[st.slot(st.team(k))] = 0u;
+    if (done == count) {
+      for (uint32_t k = 0; k < PK; ++k) flags[list[k]] = 0u;
     }
   }
 }
@@ -319,11 +334,12 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   const uint32_t dir = (lane & 1) ? uint32_t(-2) : 2u;
   const int bar_id = 1 + int(team);
 
-  // stream-K split over TEAMS: team v of V owns pairs [first(v), first(v+1)) of the stripe-major sequence of
-  // (stripe, k-tile pair) items; v is team-major so that a small launch spreads over all SMs first
+  // stream-K split over TEAMS (TeamMap): team v owns pairs [first(v), first(v+1)) of the stripe-major sequence of
+  // (stripe, k-tile pair) items
   const uint32_t PK = (KT + 1) / 2, stripes = n_out / kTileN, Ptot = stripes * PK;
-  const uint32_t V = G * T, v = team * G + c;
-  const uint32_t p_begin = cta_first_tile(v, V, Ptot), p_end = cta_first_tile(v + 1, V, Ptot);
+  const TeamMap tm{G, T, Ptot};
+  const uint32_t v = c * T + team;
+  const uint32_t p_begin = tm.first(v), p_end = tm.first(v + 1);
   const uint32_t N = (p_end - p_begin) * units;   // unit steps of this team
   const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cbase + off_scales), pr.cv.w_scale, pr.y, pr.ldy,
                      pr.partials, pr.counters, P.epoch, pr.m, mpad};
@@ -371,11 +387,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       for (int j = 0; j < 2; ++j) {
         const uint8_t *rec = cbase + off_records + size_t(offs[tile[j]]) * 16;
         lane_open(s[j], rec, int(units / kUnitsPerSeg), lane);
-        if (kRaw) {
-          rawp[j] = cbase + off_raw + size_t(tile[j]) * rtb + 16 * lane;
-          cp_async16(rawbuf_s + uint32_t(j) * kRawBufBytes + 16u * uint32_t(lane), rawp[j]);   // vector 0 -> parity 0 (completes with the segment staging)
-          rawp[j] += 512;
-        }
+        if (kRaw) rawp[j] = cbase + off_raw + size_t(tile[j]) * rtb + 16 * lane;
       }
       // the records of this warp's next pair: pulled into L2 during the first unit
       const bool has_next = p + i + 1 < p_end;
@@ -395,7 +407,17 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
             else if (kRaw) prefetch_l2(cbase + off_raw + size_t(next_tile + 4u * uint32_t(j)) * rtb + (lane - 24) * 128);
           }
         }
-        if (u % kUnitsPerSeg == 0) lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);   // drains cp.async first and last
+        if (u % kUnitsPerSeg == 0) {
+          // stage the segment (drains cp.async first and last); at the tile's start its first raw vector rides in the same group
+          if (kRaw && u == 0) {
+            lane_open_segments<2>(s, stage_s, P.stream_bytes, 0, lane, [&]() {
+#pragma unroll
+              for (int j = 0; j < 2; ++j) { cp_async16(rawbuf_s + uint32_t(j) * kRawBufBytes + 16u * uint32_t(lane), rawp[j]); rawp[j] += 512; }
+            });
+          } else {
+            lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);
+          }
+        }
         if (!dep_waited) {   // everything before this point read the container only
           grid_dep_wait();
           dep_waited = true;
@@ -527,8 +549,10 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
 #pragma unroll 1
   for (int sg = 0; sg < 2; ++sg) {
     if (!(sg == 0 ? fin_valid[0] : fin_valid[1])) continue;
-    const StripeTeams st(V, Ptot, PK, sg == 0 ? fin_stripe[0] : fin_stripe[1]);
-    team_reduce<FMT, YB>(ep, st, st.index_of(v, p_begin), tid, bar_id);
+    // scratch: the team's own staging area (no segment is staged any more)
+    team_reduce<FMT, YB>(ep, tm, PK, sg == 0 ? fin_stripe[0] : fin_stripe[1], v, tid, bar_id,
+                         reinterpret_cast<uint32_t *>(smem + stage_off + size_t(team) * kTeamWarps * 2u * P.stream_bytes));
+    named_bar_sync(bar_id, kNT);   // the list is reused by the next stripe
   }
   TRACE(5);
   tc_fence_before();
