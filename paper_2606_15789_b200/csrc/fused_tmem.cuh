@@ -25,9 +25,11 @@
 #pragma once
 
 constexpr int kTeamWarps = 4;
-constexpr int kMaxTeams = 5;
-constexpr int kTmemThreads = 32 * kTeamWarps * kMaxTeams;   // 640: lets ptxas use up to 96 registers
+constexpr int kMaxTeams = 4;
+constexpr int kTmemThreads = 32 * (kTeamWarps + 1) * kMaxTeams;   // 16 decoder warps + one issuer warp per team = 640: up to 96 registers
 constexpr uint32_t kACols = 8;                               // TMEM columns of one operand unit (32 bytes per row)
+constexpr uint32_t kASlotCols = 4 * kACols;                  // per team: two operand units (one per chain), double buffered
+constexpr uint32_t kXDepth = 3;                              // X ring slots per team (each: the two slices of one unit step)
 constexpr uint32_t kNT = 32 * kTeamWarps;                    // threads of a team
 
 // shared-memory carve-up, from the 1024-byte aligned base: slot table | prefix scratch | barriers | X rings | raw | staging
@@ -37,7 +39,7 @@ constexpr uint32_t kTmXOff = 18432;
 constexpr uint32_t kRawBufBytes = 1024;                      // bf16: two 512-byte raw vectors per chain
 __host__ __device__ constexpr bool tmem_has_raw(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16; }
 __host__ __device__ constexpr size_t tmem_smem_bytes(uint32_t T, uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
-  return 1024 /*align slack*/ + kTmXOff + size_t(T) * 4 * mpad_max * 32 + (tmem_has_raw(fmt) ? size_t(T) * kTeamWarps * 2 * kRawBufBytes : 0) +
+  return 1024 /*align slack*/ + kTmXOff + size_t(T) * kXDepth * 2 * mpad_max * 32 + (tmem_has_raw(fmt) ? size_t(T) * kTeamWarps * 2 * kRawBufBytes : 0) +
          size_t(T) * kTeamWarps * 2 * stream_bytes + 16;
 }
 // split-K control words of a problem (inside its flag area): u32 flag[2 * teams] | u32 stripe_count[stripes]
@@ -50,7 +52,7 @@ struct TmemParams {
   uint32_t epoch;          // launch id for the split-K flags
   uint32_t stream_bytes;   // shared memory per staged lane-stream segment
   uint32_t xslice_bytes;   // max mpad * 32
-  uint32_t tmem_stride;    // TMEM columns per team: max mpad + 2 * kACols
+  uint32_t tmem_stride;    // TMEM columns per team: max mpad + kASlotCols
   uint32_t afmt, bfmt;
 };
 
@@ -58,6 +60,11 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8])
   asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]),
                "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
                : "memory");
+}
+__device__ __forceinline__ bool elect_one_sync() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 template <int KIND>  // A operand in tensor memory
@@ -309,14 +316,29 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   const CUtensorMap *const xmap = &tms.m[pi];
   uint32_t *tab = reinterpret_cast<uint32_t *>(smem);
   uint32_t *cum = reinterpret_cast<uint32_t *>(smem + 16384);
-  const uint32_t bars_s = smem0 + kTmBarOff;   // per team: done[2], xfull[2], accfull
+  const uint32_t bars_s = smem0 + kTmBarOff;   // per team: done[2] +0, xfull[3] +16, accfull +40, full[2] +48
   volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + kTmPtrOff);
-  const uint32_t raw_off = kTmXOff + T * 4u * P.xslice_bytes;
+  const uint32_t raw_off = kTmXOff + T * kXDepth * 2u * P.xslice_bytes;
   const uint32_t stage_off = raw_off + (kRaw ? T * kTeamWarps * 2u * kRawBufBytes : 0u);
 
+  // stream-K split over TEAMS (TeamMap): team v owns pairs [first(v), first(v+1)) of the stripe-major sequence of
+  // (stripe, k-tile pair) items
+  const uint32_t PK = (KT + 1) / 2, stripes = n_out / kTileN, Ptot = stripes * PK;
+  const TeamMap tm{G, T, Ptot};
+  const bool decoder = uint32_t(warp) < kTeamWarps * T;
+  const uint32_t v = c * T + (decoder ? team : 0u);
+  const uint32_t p_begin = tm.first(v), p_end = decoder ? tm.first(v + 1) : p_begin;
+  const uint32_t *offs = reinterpret_cast<const uint32_t *>(cbase + pr.cv.off_offsets);
+  // record offsets of this warp's first pair of tiles: in flight while the slot table is built
+  uint32_t cur_off[2] = {0, 0};
+  if (p_begin < p_end) {
+    const uint32_t s0 = p_begin / PK, k0 = 2u * (p_begin % PK), t0 = (s0 * KT + k0) * 4u + q;
+    cur_off[0] = offs[t0];
+    cur_off[1] = offs[t0 + (k0 + 1 < KT ? 4u : 0u)];
+  }
   if (threadIdx.x == 0) {
     for (uint32_t i = 0; i < T; ++i)
-      for (uint32_t b = 0; b < 5; ++b) mbar_init(bars_s + 64 * i + 8 * b, 1);
+      for (uint32_t b = 0; b < 8; ++b) mbar_init(bars_s + 64 * i + 8 * b, b >= 6 ? kTeamWarps : 1);
     fence_mbar_init();
   }
   if (warp == 0) tmem_alloc(smem0 + kTmPtrOff, 512);
@@ -325,47 +347,77 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
 
-  const uint32_t done_s = bars_s + 64 * team, xfull_s = done_s + 16, accfull_s = done_s + 32;
+  const uint32_t done_s = bars_s + 64 * team, accfull_s = done_s + 40, full_s = done_s + 48;
   const uint32_t acc_t = tmem_base + team * P.tmem_stride, a_t = acc_t + mpad;   // accumulator, then two operand units
   const uint32_t lane_t = (q * 32u) << 16;
-  const uint32_t xring_s = smem0 + kTmXOff + team * 4u * P.xslice_bytes;          // slot sl, slice j at (sl * 2 + j) * xslice_bytes
   const uint32_t rawbuf_s = smem0 + raw_off + uint32_t(warp) * 2u * kRawBufBytes;  // chain j, vector parity b at j * 1024 + b * 512
   const uint32_t stage_s = smem0 + stage_off + uint32_t(warp) * 2u * P.stream_bytes, tab_s = smem0;
   const uint32_t dir = (lane & 1) ? uint32_t(-2) : 2u;
   const int bar_id = 1 + int(team);
 
-  // stream-K split over TEAMS (TeamMap): team v owns pairs [first(v), first(v+1)) of the stripe-major sequence of
-  // (stripe, k-tile pair) items
-  const uint32_t PK = (KT + 1) / 2, stripes = n_out / kTileN, Ptot = stripes * PK;
-  const TeamMap tm{G, T, Ptot};
-  const uint32_t v = c * T + team;
-  const uint32_t p_begin = tm.first(v), p_end = tm.first(v + 1);
-  const uint32_t N = (p_end - p_begin) * units;   // unit steps of this team
+
   const EpiParams ep{pr.x_scale, reinterpret_cast<const __half *>(cbase + off_scales), pr.cv.w_scale, pr.y, pr.ldy,
                      pr.partials, pr.counters, P.epoch, pr.m, mpad};
   const uint32_t idesc = make_idesc(TR::c, P.afmt, P.bfmt, 128, mpad);
   const uint32_t xbytes = mpad * 32u;
-  const uint32_t *offs = reinterpret_cast<const uint32_t *>(cbase + pr.cv.off_offsets);
   const size_t rtb = raw_tile_bytes(32, tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
-  const bool issuer = q == 0, loader = q == 1;
   uint32_t fin_stripe[2] = {0, 0};
   bool fin_valid[2] = {false, false};
 
-  // X loader state (warp 1, lane 0): the (pair-in-stripe, unit) of the NEXT unit step to fetch
-  uint32_t lx_kp = p_begin % PK, lx_u = 0, lx_n = 0;
-  auto load_next_x = [&]() {   // issues the two X slices of unit step lx_n, then advances
-    const uint32_t ktA = 2u * lx_kp, sl = lx_n & 1u, bar = xfull_s + 8 * sl;
-    const bool hasB = ktA + 1 < KT;
-    const int kA = int(ktA * tile_k + lx_u * kUnitK);
-    mbar_arrive_expect_tx(bar, hasB ? 2 * xbytes : xbytes);
-    tma_load_2d(xring_s + (sl * 2u) * P.xslice_bytes, xmap, kA, 0, bar);
-    if (hasB) tma_load_2d(xring_s + (sl * 2u + 1u) * P.xslice_bytes, xmap, kA + int(tile_k), 0, bar);
-    ++lx_n;
-    if (++lx_u == units) { lx_u = 0; if (++lx_kp == PK) lx_kp = 0; }
-  };
-  const uint64_t bdesc0 = make_smem_desc(xring_s, 16, 256, kLayoutSW32);
-  const uint32_t bdesc_step = P.xslice_bytes >> 4;
-
+  if (uint32_t(warp) >= kTeamWarps * T) {
+    // ===================== issuer warp of team `it`: drives the tensor core and the team's X ring =====================
+    // Every wait is a hardware-suspended mbarrier wait, so this warp costs the decoders next to nothing, and the MMAs and
+    // TMA requests of a unit step cost the decoder warps nothing at all.
+    const uint32_t it = uint32_t(warp) - kTeamWarps * T, vt = c * T + it;
+    const uint32_t pb = tm.first(vt), pe = tm.first(vt + 1), Nt = (pe - pb) * units;
+    const uint32_t bt = bars_s + 64 * it, acc = tmem_base + it * P.tmem_stride, at = acc + mpad;
+    const uint32_t xr = smem0 + kTmXOff + it * kXDepth * 2u * P.xslice_bytes;   // ring slot sx, slice j at (sx * 2 + j) * xslice_bytes
+    const uint64_t bdesc0 = make_smem_desc(xr, 16, 256, kLayoutSW32);
+    const uint32_t bdesc_step = P.xslice_bytes >> 4;
+    const bool leader = elect_one_sync();
+    uint32_t kpx = pb % PK, ux = 0, sxx = 0, nx = 0;   // X request cursor: pair in stripe, unit, ring slot, unit step
+    auto request_x = [&]() {   // the two X slices of unit step nx
+      if (leader) {
+        const uint32_t ktA = 2u * kpx, bar = bt + 16 + 8 * sxx;
+        const bool hasB = ktA + 1 < KT;
+        const int kA = int(ktA * tile_k + ux * kUnitK);
+        mbar_arrive_expect_tx(bar, hasB ? 2 * xbytes : xbytes);
+        tma_load_2d(xr + (sxx * 2u) * P.xslice_bytes, xmap, kA, 0, bar);
+        if (hasB) tma_load_2d(xr + (sxx * 2u + 1u) * P.xslice_bytes, xmap, kA + int(tile_k), 0, bar);
+      }
+      ++nx;
+      if (++sxx == kXDepth) sxx = 0;
+      if (++ux == units) { ux = 0; if (++kpx == PK) kpx = 0; }
+    };
+    grid_dep_wait();   // X belongs to the stream's earlier kernels until they are done
+    if (Nt > 0) request_x();
+    if (Nt > 1) request_x();
+    uint32_t pp = pb, kp = pb % PK, u = 0, sx = 0, xpar = 0;
+#pragma unroll 1
+    for (uint32_t n = 0; n < Nt; ++n) {
+      const uint32_t sa = n & 1u;
+      mbar_wait(bt + 48 + 8 * sa, (n >> 1) & 1u);   // all four decoder warps have stored this step's operand columns
+      mbar_wait(bt + 16 + 8 * sx, xpar);            // its X slices have landed
+      tc_fence_after();
+      const bool hasB = 2u * kp + 1 < KT, last_unit = u + 1 == units;
+      const bool seg_first = u == 0 && (pp == pb || kp == 0), seg_last = last_unit && (pp + 1 == pe || kp + 1 == PK);
+      if (leader) {
+        const uint64_t bdA = bdesc0 + uint64_t(sx * 2u * bdesc_step);
+        umma_ts<TR::kind>(acc, at + sa * 2u * kACols, bdA, idesc, seg_first ? 0u : 1u);
+        if (hasB) umma_ts<TR::kind>(acc, at + sa * 2u * kACols + kACols, bdA + bdesc_step, idesc, 1u);
+        umma_commit(bt + 8 * sa);
+        if (seg_last) umma_commit(bt + 40);
+      }
+      __syncwarp();
+      if (++sx == kXDepth) { sx = 0; xpar ^= 1u; }
+      if (last_unit) { u = 0; ++pp; if (++kp == PK) kp = 0; } else ++u;
+      // the X slices of step n + 2 go to the ring slot last read by the MMAs of step n - 1 (issued one step ago)
+      if (nx < Nt) {
+        if (n >= 1) mbar_wait(bt + 8 * ((n - 1) & 1u), ((n - 1) >> 1) & 1u);
+        request_x();
+      }
+    }
+  } else {
   uint32_t n = 0, seg_i = 0;
   bool dep_waited = false;
   TRACE(1);
@@ -385,7 +437,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       const uint8_t *rawp[2] = {nullptr, nullptr};   // this lane's 16 bytes of the NEXT raw vector to fetch
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const uint8_t *rec = cbase + off_records + size_t(offs[tile[j]]) * 16;
+        const uint8_t *rec = cbase + off_records + size_t(cur_off[j]) * 16;
         lane_open(s[j], rec, int(units / kUnitsPerSeg), lane);
         if (kRaw) rawp[j] = cbase + off_raw + size_t(tile[j]) * rtb + 16 * lane;
       }
@@ -405,6 +457,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
           for (int j = 0; j < 2; ++j) {
             if (lane < 24) prefetch_l2(cbase + off_records + size_t(next_off[j]) * 16 + lane * 128);
             else if (kRaw) prefetch_l2(cbase + off_raw + size_t(next_tile + 4u * uint32_t(j)) * rtb + (lane - 24) * 128);
+            cur_off[j] = next_off[j];   // the next pair opens without another look at the offset table
           }
         }
         if (u % kUnitsPerSeg == 0) {
@@ -418,10 +471,10 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
             lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);
           }
         }
+        if (u == 0) PROF(4);
         if (!dep_waited) {   // everything before this point read the container only
           grid_dep_wait();
           dep_waited = true;
-          if (loader && lane == 0) load_next_x();
         }
         const bool last_unit = u + 1 == units;
         uint4 rv[2] = {make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0)};
@@ -468,36 +521,19 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         decode_unit_regs<FMT, PAYLOAD>(s, tab_s, dir, last_unit, rv, sz, r);
         PROF(1);
         // ---- hand-over: registers -> tensor memory -> tcgen05.mma ----
-        if (n > 0) mbar_wait(done_s + 8 * ((n - 1) & 1u), ((n - 1) >> 1) & 1u);   // the MMAs of step n-1 have read the operand columns
+        const uint32_t sa = n & 1u;
+        if (n > 1) mbar_wait(done_s + 8 * sa, ((n - 2) >> 1) & 1u);   // the MMAs of step n-2 have read this half of the operand columns
         PROF(2);
-        tmem_st8(a_t + lane_t, r[0]);
-        tmem_st8(a_t + kACols + lane_t, r[1]);
+        tmem_st8(a_t + sa * 2u * kACols + lane_t, r[0]);
+        tmem_st8(a_t + sa * 2u * kACols + kACols + lane_t, r[1]);
         tmem_wait_st();
         tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(full_s + 8 * sa);   // the fourth arrival lets the team's issuer warp multiply this unit step
         PROF(3);
-        if (!issuer) {
-          named_bar_arrive(bar_id, kNT);
-          // ring slot (n+1)&1 was last read by the MMAs of step n-1: their completion was waited for above
-          if (loader && lane == 0 && lx_n < N) load_next_x();
-        } else {
-          named_bar_sync(bar_id, kNT);
-          tc_fence_after();
-          PROF(4);
-          mbar_wait(xfull_s + 8 * (n & 1u), (n >> 1) & 1u);
-          if (lane == 0) {
-            const uint32_t sl = n & 1u;
-            const uint64_t bdA = bdesc0 + uint64_t(sl * 2u * bdesc_step);
-            umma_ts<TR::kind>(acc_t, a_t, bdA, idesc, (i == 0 && u == 0) ? 0u : 1u);
-            if (hasB) umma_ts<TR::kind>(acc_t, a_t + kACols, bdA + bdesc_step, idesc, 1u);
-            umma_commit(done_s + 8 * sl);
-            if (i + 1 == np && last_unit) umma_commit(accfull_s);
-          }
-          __syncwarp();
-          PROF(5);
-        }
       }
     }
-    PROF_DUMP;
+    PROF(0);
     // ---- epilogue of this stripe segment: the team reads its own accumulator ----
     TRACE(2);
     mbar_wait(accfull_s, seg_i & 1u);
@@ -529,23 +565,28 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
       tc_fence_before();   // the next segment's first MMA (after the next team barrier) overwrites the accumulator
       if (!whole) {
-        __threadfence();
+        // the team's partial stores are ordered before the barrier; the one thread that raises the flag then fences at
+        // GPU scope (cumulative over what the barrier made visible to it), as a grid-wide barrier would
         named_bar_sync(bar_id, kNT);
-        if (issuer && lane == 0) {
+        if (q == 0 && lane == 0) {
           uint32_t *flag = reinterpret_cast<uint32_t *>(ep.counters) + (v * 2u + seg);
+          __threadfence();
           asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(ep.epoch) : "memory");
         }
         if (seg == 0) { fin_stripe[0] = stripe; fin_valid[0] = true; }
         else { fin_stripe[1] = stripe; fin_valid[1] = true; }
       }
     }
+    PROF(5);
     p += np;
   }
+  PROF_DUMP;
   cp_async_wait_all();
   TRACE(4);
   // ---- split-K: reduce this team's slice of every stripe it holds a partial of ----
   if (!dep_waited) grid_dep_wait();
   const uint32_t tid = q * 32u + uint32_t(lane);
+  if (fin_valid[0] || fin_valid[1]) named_bar_sync(bar_id, kNT);   // the scratch below is the staging area the team's warps decode from
 #pragma unroll 1
   for (int sg = 0; sg < 2; ++sg) {
     if (!(sg == 0 ? fin_valid[0] : fin_valid[1])) continue;
@@ -555,6 +596,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
     named_bar_sync(bar_id, kNT);   // the list is reused by the next stripe
   }
   TRACE(5);
+  }   // decoder warps
   tc_fence_before();
   __syncthreads();
   TRACE(6);

@@ -978,7 +978,7 @@ int launch_fused_y(const TensorMaps &tms, const FusedParams &p, uint32_t grid, s
 // Teams per CTA of the TMEM design (fused_tmem.cuh) for the largest padded batch of a launch and the staged segment size:
 // bounded by tensor memory (mpad accumulator + 16 operand columns per team) and by shared memory; 0 = does not fit.
 uint32_t tmem_teams(uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
-  uint32_t T = std::min<uint32_t>(kMaxTeams, 512u / (mpad_max + 2 * kACols));
+  uint32_t T = std::min<uint32_t>(kMaxTeams, 512u / (mpad_max + kASlotCols));
   while (T > 0 && tmem_smem_bytes(T, mpad_max, stream_bytes, fmt) > kSmemMax) --T;
   return T;
 }
@@ -996,7 +996,7 @@ int launch_tmem_y(const TensorMaps &tms, const TmemParams &p, uint32_t grid, siz
   }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grid);
-  cfg.blockDim = dim3(32 * kTeamWarps * p.T);
+  cfg.blockDim = dim3(32 * (kTeamWarps + 1) * p.T);   // T teams of four decoder warps + one issuer warp per team
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
@@ -1129,7 +1129,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     p.epoch = next_epoch();
     p.stream_bytes = stream_bytes;
     p.xslice_bytes = mpad_max * 32u;
-    p.tmem_stride = mpad_max + 2 * kACols;
+    p.tmem_stride = mpad_max + kASlotCols;
     p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
     const size_t smem = tmem_smem_bytes(T, mpad_max, stream_bytes, h0.format);
     switch (h0.format) {
