@@ -154,6 +154,7 @@ __device__ __forceinline__ void decode_unit_regs(LaneStream (&s)[2], uint32_t ta
   }
 }
 
+
 #ifdef ANSLIN_TRACE
 __device__ unsigned long long g_trace[160 * kMaxTeams * 8];
 __device__ __forceinline__ unsigned long long gtimer() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
@@ -162,8 +163,10 @@ __device__ unsigned long long g_prof[160 * kMaxTeams * 4 * 8];
 #define PROF_DECL long long pf_t = clock64(), pf_acc[6] = {0, 0, 0, 0, 0, 0};
 #define PROF(i) do { const long long pf_n = clock64(); pf_acc[i] += pf_n - pf_t; pf_t = pf_n; } while (0)
 #define PROF_DUMP do { if (lane == 0) for (int pf_i = 0; pf_i < 6; ++pf_i) g_prof[((blockIdx.x * kMaxTeams + team) * 4 + q) * 8 + pf_i] = (unsigned long long)pf_acc[pf_i]; } while (0)
+#define RTRACE(slot) do { if (tid == 0) g_trace[(blockIdx.x * kMaxTeams + (bar - 1)) * 8 + (slot)] = gtimer(); } while (0)
 #else
 #define TRACE(slot) do {} while (0)
+#define RTRACE(slot) do {} while (0)
 #define PROF_DECL
 #define PROF(i) do {} while (0)
 #define PROF_DUMP do {} while (0)
@@ -172,109 +175,124 @@ __device__ unsigned long long g_prof[160 * kMaxTeams * 4 * 8];
 // Two-level stream-K split of the stripe-major sequence of Ptot (stripe, k-tile pair) items: first evenly over the G CTAs of
 // the problem (so that every SM gets the same amount of work), then evenly over the T teams of a CTA.  Team v = c * T + t.
 struct TeamMap {
-  uint32_t G, T, Ptot;
+  uint32_t G, T, Ptot;   // the launcher guarantees (Ptot + 1) * (G + 1) < 2^32: 32-bit arithmetic throughout
+  static __device__ __forceinline__ uint32_t first_of(uint32_t c, uint32_t G, uint32_t n) { return c * n / G; }
+  static __device__ __forceinline__ uint32_t owner_of(uint32_t t, uint32_t G, uint32_t n) { return ((t + 1) * G + n - 1) / n - 1; }   // largest c with first_of(c) <= t
   __device__ __forceinline__ uint32_t first(uint32_t v) const {   // first pair of team v (v = G * T: Ptot)
     const uint32_t c = v / T, t = v - c * T;
-    const uint32_t a = cta_first_tile(c, G, Ptot), nc = cta_first_tile(c + 1, G, Ptot) - a;
-    return a + uint32_t(uint64_t(t) * nc / T);
+    const uint32_t a = first_of(c, G, Ptot), nc = first_of(c + 1, G, Ptot) - a;
+    return a + first_of(t, T, nc);
   }
   __device__ __forceinline__ uint32_t owner(uint32_t p) const {   // the team that owns pair p
-    const uint32_t c = cta_of_tile(p, G, Ptot);
-    const uint32_t a = cta_first_tile(c, G, Ptot), nc = cta_first_tile(c + 1, G, Ptot) - a;
-    return c * T + cta_of_tile(p - a, T, nc);
+    const uint32_t c = owner_of(p, G, Ptot);
+    const uint32_t a = first_of(c, G, Ptot), nc = first_of(c + 1, G, Ptot) - a;
+    return c * T + owner_of(p - a, T, nc);
   }
 };
 
-// Distributed deterministic split-K reduction of one stripe by one of its contributors (all 128 threads of the team).
-// The contributors are the distinct owners of the stripe's PK pairs, in pair order; contributor vv's partial slot is its first
-// segment (slot 0) unless the stripe is its second one, which can only be the case for the stripe's first contributor.
+// Distributed deterministic split-K reduction by one contributor team (all 128 threads) of the ns <= 2 stripes it holds a
+// partial of.  The contributors of a stripe are the distinct owners of its PK pairs, in pair order; contributor vv's partial
+// slot is its first segment (slot 0) unless the stripe is its second one, which can only be the case for the stripe's first
+// contributor.  Every contributor sums ITS slice of the stripe's outputs over all contributors, in that order.
+// scratch: team-private shared memory, 2 * (PK + 1) words.
 template <uint32_t FMT, bool YB>
-__device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &tm, uint32_t PK, uint32_t stripe, uint32_t v, uint32_t tid,
-                                            int bar, uint32_t *list /* team-private shared scratch, PK + 1 words */) {
+__device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &tm, uint32_t PK, int ns, const uint32_t (&stripes)[2], uint32_t v,
+                                            uint32_t tid, int bar, uint32_t *scratch) {
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   uint32_t *flags = reinterpret_cast<uint32_t *>(p.counters);
-  const uint32_t p0 = stripe * PK;
-  // the partial slot of every pair's owner (one pair per thread), then wait for that partial's flag
-  for (uint32_t k = tid; k < PK; k += kNT) {
-    const uint32_t vv = tm.owner(p0 + k), v_first = tm.owner(p0);
-    const uint32_t slot = vv * 2u + ((vv == v_first && tm.first(v_first) < p0) ? 1u : 0u);
-    list[k] = slot;
-    const uint32_t *flag = flags + slot;
-    uint32_t val, spins = 0;
-    while (true) {
-      asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(val) : "l"(flag) : "memory");
-      if (val == p.epoch) break;
-      __nanosleep(200);
-      if (++spins > (1u << 24)) __trap();   // a protocol bug traps instead of hanging the GPU
+  // 1. the partial slot of every pair's owner (one pair per thread), then wait for that partial's flag
+  for (int sg = 0; sg < ns; ++sg) {
+    uint32_t *list = scratch + sg * (PK + 1);
+    const uint32_t p0 = stripes[sg] * PK;
+    for (uint32_t k = tid; k < PK; k += kNT) {
+      const uint32_t vv = tm.owner(p0 + k), v_first = tm.owner(p0);
+      const uint32_t slot = vv * 2u + ((vv == v_first && tm.first(v_first) < p0) ? 1u : 0u);
+      list[k] = slot;
+      const uint32_t *flag = flags + slot;
+      uint32_t val, spins = 0;
+      while (true) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(val) : "l"(flag) : "memory");
+        if (val == p.epoch) break;
+        __nanosleep(100);
+        if (++spins > (1u << 24)) __trap();   // a protocol bug traps instead of hanging the GPU
+      }
     }
   }
+  RTRACE(5);
   named_bar_sync(bar, kNT);
-  // how many contributors, and which one am I (consecutive pairs of one owner share a slot)
-  uint32_t count = 0, my_index = 0;
-  for (uint32_t k = 0, prev = 0xFFFFFFFFu; k < PK; ++k) {
-    const uint32_t sl = list[k];
-    if (sl != prev) { if ((sl >> 1) == v) my_index = count; ++count; prev = sl; }
-  }
   const size_t slot_words = size_t(p.mpad) * kTileN;
   const uint32_t n_items = p.m * 32u;   // one item = one batch row x 4 output channels
-  const uint32_t it_begin = uint32_t(uint64_t(my_index) * n_items / count), it_end = uint32_t(uint64_t(my_index + 1) * n_items / count);
-  for (uint32_t it = it_begin + tid; it < it_end; it += kNT) {
-    const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u;
-    const uint32_t *src = p.partials + size_t(mm) * kTileN + r4;
-    uint32_t acc[4];
+  uint32_t counts[2] = {0, 0};
+  for (int sg = 0; sg < ns; ++sg) {
+    const uint32_t *list = scratch + sg * (PK + 1);
+    // 2. how many contributors, and which one am I (consecutive pairs of one owner share a slot)
+    uint32_t count = 0, my_index = 0;
+    for (uint32_t k = 0, prev = 0xFFFFFFFFu; k < PK; ++k) {
+      const uint32_t sl = list[k];
+      if (sl != prev) { if ((sl >> 1) == v) my_index = count; ++count; prev = sl; }
+    }
+    counts[sg] = count;
+    // 3. my slice of the stripe's items
+    const uint32_t it_begin = my_index * n_items / count, it_end = (my_index + 1) * n_items / count;
+    for (uint32_t it = it_begin + tid; it < it_end; it += kNT) {
+      const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u;
+      const uint32_t *src = p.partials + size_t(mm) * kTileN + r4;
+      uint32_t acc[4];
 #pragma unroll
-    for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-    uint32_t prev = 0xFFFFFFFFu;
-    for (uint32_t kb = 0; kb < PK; kb += 8) {
-      uint4 val[8];
-      bool use[8];
+      for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
+      uint32_t prev = 0xFFFFFFFFu;
+      for (uint32_t kb = 0; kb < PK; kb += 8) {
+        uint4 val[8];
+        bool use[8];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {
-        use[j] = false;
-        if (kb + j < PK) {
-          const uint32_t sl = list[kb + j];
-          use[j] = sl != prev;
-          prev = sl;
-          if (use[j]) val[j] = ldcg128(src + size_t(sl) * slot_words);
+        for (int j = 0; j < 8; ++j) {
+          use[j] = false;
+          if (kb + j < PK) {
+            const uint32_t sl = list[kb + j];
+            use[j] = sl != prev;
+            prev = sl;
+            if (use[j]) val[j] = ldcg128(src + size_t(sl) * slot_words);
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {   // fixed team order -> bit-reproducible sums
+          if (use[j]) {
+            acc[0] = acc_add<FMT>(acc[0], val[j].x); acc[1] = acc_add<FMT>(acc[1], val[j].y);
+            acc[2] = acc_add<FMT>(acc[2], val[j].z); acc[3] = acc_add<FMT>(acc[3], val[j].w);
+          }
         }
       }
+      const uint32_t n4 = stripes[sg] * kTileN + r4;
+      const float xs = kScaled ? p.x_scale[mm] : 1.0f;
+      float o[4];
 #pragma unroll
-      for (int j = 0; j < 8; ++j) {   // fixed team order -> bit-reproducible sums
-        if (use[j]) {
-          acc[0] = acc_add<FMT>(acc[0], val[j].x); acc[1] = acc_add<FMT>(acc[1], val[j].y);
-          acc[2] = acc_add<FMT>(acc[2], val[j].z); acc[3] = acc_add<FMT>(acc[3], val[j].w);
-        }
+      for (int j = 0; j < 4; ++j) {
+        float ws = 1.0f;
+        if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
+        if (is_fp8_path(FMT)) ws = p.w_scale;
+        o[j] = finalize<FMT>(acc[j], xs, ws);
       }
-    }
-    const uint32_t n4 = stripe * kTileN + r4;
-    const float xs = kScaled ? p.x_scale[mm] : 1.0f;
-    float o[4];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      float ws = 1.0f;
-      if (FMT == ANSLIN_FMT_INT8) ws = __half2float(p.w_scale_h[n4 + j]);
-      if (is_fp8_path(FMT)) ws = p.w_scale;
-      o[j] = finalize<FMT>(acc[j], xs, ws);
-    }
-    if constexpr (YB) {
-      __nv_bfloat16 *yb = reinterpret_cast<__nv_bfloat16 *>(p.y) + size_t(mm) * p.ldy + n4;
-      const __nv_bfloat162 lo = __floats2bfloat162_rn(o[0], o[1]), hi = __floats2bfloat162_rn(o[2], o[3]);
-      if ((reinterpret_cast<uintptr_t>(yb) & 7) == 0)
-        *reinterpret_cast<uint2 *>(yb) = make_uint2(*reinterpret_cast<const uint32_t *>(&lo), *reinterpret_cast<const uint32_t *>(&hi));
-      else { yb[0] = lo.x; yb[1] = lo.y; yb[2] = hi.x; yb[3] = hi.y; }
-    } else {
-      float *yo = p.y + size_t(mm) * p.ldy + n4;
-      if ((reinterpret_cast<uintptr_t>(yo) & 15) == 0) *reinterpret_cast<float4 *>(yo) = make_float4(o[0], o[1], o[2], o[3]);
-      else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
+      if constexpr (YB) {
+        __nv_bfloat16 *yb = reinterpret_cast<__nv_bfloat16 *>(p.y) + size_t(mm) * p.ldy + n4;
+        const __nv_bfloat162 lo = __floats2bfloat162_rn(o[0], o[1]), hi = __floats2bfloat162_rn(o[2], o[3]);
+        if ((reinterpret_cast<uintptr_t>(yb) & 7) == 0)
+          *reinterpret_cast<uint2 *>(yb) = make_uint2(*reinterpret_cast<const uint32_t *>(&lo), *reinterpret_cast<const uint32_t *>(&hi));
+        else { yb[0] = lo.x; yb[1] = lo.y; yb[2] = hi.x; yb[3] = hi.y; }
+      } else {
+        float *yo = p.y + size_t(mm) * p.ldy + n4;
+        if ((reinterpret_cast<uintptr_t>(yo) & 15) == 0) *reinterpret_cast<float4 *>(yo) = make_float4(o[0], o[1], o[2], o[3]);
+        else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
+      }
     }
   }
-  // The last contributor to finish reading clears the stripe's flags and its counter, so that a replay of this very launch
-  // (CUDA graph: same epoch) starts from "nothing stored".  Counter word = epoch tag << 8 | readers done; any other tag
-  // (stale or never written bytes) reads as zero readers.
+  RTRACE(6);
+  // 4. The last contributor to finish reading a stripe clears its flags and its counter, so that a replay of this very
+  // launch (CUDA graph: same epoch) starts from "nothing stored".  Counter word = epoch tag << 8 | readers done; any other
+  // tag (stale or never written bytes) reads as zero readers.
   named_bar_sync(bar, kNT);
-  if (tid == 0) {
-    uint32_t *cnt = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(p.counters) + kTmStripeCntOff) + stripe;
-    const uint32_t tag = (p.epoch << 8);
+  if (tid < uint32_t(ns)) {
+    uint32_t *cnt = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(p.counters) + kTmStripeCntOff) + stripes[tid];
+    const uint32_t tag = (p.epoch << 8), count = tid == 0 ? counts[0] : counts[1];
     uint32_t old = *reinterpret_cast<volatile uint32_t *>(cnt), done;
     while (true) {
       done = ((old & 0xFFFFFF00u) == tag ? (old & 0xFFu) : 0u) + 1u;
@@ -282,9 +300,13 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
       if (seen == old) break;
       old = seen;
     }
-    if (done == count) {
-      for (uint32_t k = 0; k < PK; ++k) flags[list[k]] = 0u;
-    }
+    scratch[tid * (PK + 1) + PK] = done == count ? 1u : 0u;
+  }
+  named_bar_sync(bar, kNT);
+  for (int sg = 0; sg < ns; ++sg) {
+    const uint32_t *list = scratch + sg * (PK + 1);
+    if (list[PK])
+      for (uint32_t k = tid; k < PK; k += kNT) flags[list[k]] = 0u;
   }
 }
 
@@ -549,18 +571,19 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       for (uint32_t c0 = 0; c0 < mpad; c0 += 16) {
         uint32_t val[16];
         tmem_ld16(acc_t + lane_t + c0, val);
+        if (whole) {
 #pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const uint32_t mm = c0 + j;
-          if (mm < ep.m) {
-            if (whole) {
+          for (int j = 0; j < 16; ++j) {
+            const uint32_t mm = c0 + j;
+            if (mm < ep.m) {
               const float f = finalize<FMT>(val[j], kScaled ? ep.x_scale[mm] : 1.0f, ws);
               if constexpr (YB) reinterpret_cast<__nv_bfloat16 *>(ep.y)[size_t(mm) * ep.ldy + nrow] = __float2bfloat16_rn(f);
               else ep.y[size_t(mm) * ep.ldy + nrow] = f;
-            } else {
-              part[size_t(mm) * kTileN + row] = val[j];
             }
           }
+        } else {   // the partial buffer has mpad rows: no guards
+#pragma unroll
+          for (int j = 0; j < 16; ++j) part[size_t(c0 + j) * kTileN + row] = val[j];
         }
       }
       tc_fence_before();   // the next segment's first MMA (after the next team barrier) overwrites the accumulator
@@ -586,19 +609,15 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   // ---- split-K: reduce this team's slice of every stripe it holds a partial of ----
   if (!dep_waited) grid_dep_wait();
   const uint32_t tid = q * 32u + uint32_t(lane);
-  if (fin_valid[0] || fin_valid[1]) named_bar_sync(bar_id, kNT);   // the scratch below is the staging area the team's warps decode from
-#pragma unroll 1
-  for (int sg = 0; sg < 2; ++sg) {
-    if (!(sg == 0 ? fin_valid[0] : fin_valid[1])) continue;
-    // scratch: the team's own staging area (no segment is staged any more)
-    team_reduce<FMT, YB>(ep, tm, PK, sg == 0 ? fin_stripe[0] : fin_stripe[1], v, tid, bar_id,
+  if (fin_valid[0] || fin_valid[1]) {
+    named_bar_sync(bar_id, kNT);   // the scratch below is the staging area the team's warps decoded from
+    uint32_t st[2] = {fin_valid[0] ? fin_stripe[0] : fin_stripe[1], fin_stripe[1]};
+    team_reduce<FMT, YB>(ep, tm, PK, (fin_valid[0] && fin_valid[1]) ? 2 : 1, st, v, tid, bar_id,
                          reinterpret_cast<uint32_t *>(smem + stage_off + size_t(team) * kTeamWarps * 2u * P.stream_bytes));
-    named_bar_sync(bar_id, kNT);   // the list is reused by the next stripe
   }
-  TRACE(5);
+  TRACE(7);
   }   // decoder warps
   tc_fence_before();
   __syncthreads();
-  TRACE(6);
   if (warp == 0) tmem_dealloc(tmem_base, 512);
 }
