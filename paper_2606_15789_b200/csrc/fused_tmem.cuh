@@ -66,6 +66,15 @@ __device__ __forceinline__ bool elect_one_sync() {
   asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
   return pred != 0;
 }
+// Wait of a warp that has time to spare (the issuer warps): probe, then sleep.  mbarrier.try_wait's own suspension is woken
+// by every barrier event of the CTA (one per ~75 clk here), and the re-probing took a sixth of the SM's issue slots.
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity, uint32_t ns) {
+  uint32_t tries = 0;
+  while (!mbar_test(bar, parity)) {
+    __nanosleep(ns);
+    if (++tries > (1u << 24)) __trap();
+  }
+}
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 template <int KIND>  // A operand in tensor memory
 __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -357,6 +366,12 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
     const uint32_t s0 = p_begin / PK, k0 = 2u * (p_begin % PK), t0 = (s0 * KT + k0) * 4u + q;
     cur_off[0] = offs[t0];
     cur_off[1] = offs[t0 + (k0 + 1 < KT ? 4u : 0u)];
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {   // ... and the records themselves (and their raw bytes) on their way into L2
+      if (lane < 24) prefetch_l2(cbase + off_records + size_t(cur_off[j]) * 16 + lane * 128);
+      else if (tmem_has_raw(FMT))
+        prefetch_l2(cbase + off_raw + size_t(t0 + (j && k0 + 1 < KT ? 4u : 0u)) * raw_tile_bytes(32, tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0) + (lane - 24) * 128);
+    }
   }
   if (threadIdx.x == 0) {
     for (uint32_t i = 0; i < T; ++i)
@@ -418,8 +433,8 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
 #pragma unroll 1
     for (uint32_t n = 0; n < Nt; ++n) {
       const uint32_t sa = n & 1u;
-      mbar_wait(bt + 48 + 8 * sa, (n >> 1) & 1u);   // all four decoder warps have stored this step's operand columns
-      mbar_wait(bt + 16 + 8 * sx, xpar);            // its X slices have landed
+      mbar_wait_relaxed(bt + 48 + 8 * sa, (n >> 1) & 1u, 250);   // all four decoder warps have stored this step's operand columns
+      mbar_wait_relaxed(bt + 16 + 8 * sx, xpar, 100);            // its X slices have landed
       tc_fence_after();
       const bool hasB = 2u * kp + 1 < KT, last_unit = u + 1 == units;
       const bool seg_first = u == 0 && (pp == pb || kp == 0), seg_last = last_unit && (pp + 1 == pe || kp + 1 == PK);
@@ -435,13 +450,16 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       if (last_unit) { u = 0; ++pp; if (++kp == PK) kp = 0; } else ++u;
       // the X slices of step n + 2 go to the ring slot last read by the MMAs of step n - 1 (issued one step ago)
       if (nx < Nt) {
-        if (n >= 1) mbar_wait(bt + 8 * ((n - 1) & 1u), ((n - 1) >> 1) & 1u);
+        if (n >= 1) mbar_wait_relaxed(bt + 8 * ((n - 1) & 1u), ((n - 1) >> 1) & 1u, 100);
         request_x();
       }
     }
   } else {
   uint32_t n = 0, seg_i = 0;
   bool dep_waited = false;
+#ifdef ANSLIN_STAGGER_NS
+  __nanosleep(team * ANSLIN_STAGGER_NS);   // teams out of phase: one team's hand-over overlaps the others' decoding
+#endif
   TRACE(1);
   PROF_DECL
 #pragma unroll 1
@@ -501,6 +519,9 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         const bool last_unit = u + 1 == units;
         uint4 rv[2] = {make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0)};
         uint32_t sz[2] = {0, 0};
+#ifdef ANSLIN_SKEL_NO_RAW   // timing experiment only (wrong results): how much does the raw-byte path cost
+        if (false)
+#endif
         if constexpr (kRaw) {
           // this unit's raw vector was copied during the previous unit; fetch the next one into the other half
           cp_async_wait_all();
@@ -538,17 +559,30 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
                           q * 32u + uint32_t(lane));
           }
         }
+        const uint32_t sa = n & 1u;
+        // have the MMAs of step n-2 read this half of the operand columns?  Asked now, needed after the unit is decoded
+        const bool slot_free = n < 2 || mbar_test(done_s + 8 * sa, ((n - 2) >> 1) & 1u);
         uint32_t r[2][8];
         PROF(0);
+#ifdef ANSLIN_SKEL_NO_DECODE   // timing experiment only (wrong results): everything but the rANS steps
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { r[0][k] = rv[0].x + k; r[1][k] = rv[1].y ^ k; }
+#else
         decode_unit_regs<FMT, PAYLOAD>(s, tab_s, dir, last_unit, rv, sz, r);
+#endif
         PROF(1);
         // ---- hand-over: registers -> tensor memory -> tcgen05.mma ----
-        const uint32_t sa = n & 1u;
-        if (n > 1) mbar_wait(done_s + 8 * sa, ((n - 2) >> 1) & 1u);   // the MMAs of step n-2 have read this half of the operand columns
+        if (!slot_free) mbar_wait(done_s + 8 * sa, ((n - 2) >> 1) & 1u);
         PROF(2);
+#ifdef ANSLIN_SKEL_NO_STTM   // timing experiment only (wrong results): how much do the tensor-memory stores cost
+        if (r[0][0] == 0x12345678u && r[1][7] == 0x9abcdef0u && r[0][3] == 1u && r[1][2] == 7u) {
+#endif
         tmem_st8(a_t + sa * 2u * kACols + lane_t, r[0]);
         tmem_st8(a_t + sa * 2u * kACols + kACols + lane_t, r[1]);
         tmem_wait_st();
+#ifdef ANSLIN_SKEL_NO_STTM
+        }
+#endif
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(full_s + 8 * sa);   // the fourth arrival lets the team's issuer warp multiply this unit step

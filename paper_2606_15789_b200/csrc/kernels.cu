@@ -1081,7 +1081,12 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   }
   // which design: decoded operand through tensor memory (fused_tmem.cuh) or through shared-memory operand slots
   const uint32_t T = (ls && tmem_ok) ? tmem_teams(mpad_max, stream_bytes, h0.format) : 0u;
-  const bool use_tmem = T >= 2;
+  // The tensor-memory design works on pairs of k-tiles of one stripe.  A launch with fewer pairs than 0.6 x teams (few, long
+  // tiles: e.g. 32 x 1024 int8 tiles of a 13824 x 5120 matrix) is bound by the sequential length of a tile pair; the
+  // shared-memory design splits such a launch by single k-tiles and finishes sooner.
+  uint64_t pairs = 0;
+  for (int i = 0; i < n; ++i) pairs += uint64_t(ws[i]->h.n_out / kTileN) * ((ws[i]->h.k_in / ws[i]->h.tile_k + 1) / 2);
+  const bool use_tmem = T >= 2 && pairs * 10 >= uint64_t(sm_budget()) * T * 6;
   // CTAs: one per SM in total, shared out in proportion to the problems' sizes
   const uint32_t S = uint32_t(sm_budget());
   uint32_t ncta[kMaxProblems], cap[kMaxProblems];
