@@ -563,6 +563,9 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         // have the MMAs of step n-2 read this half of the operand columns?  Asked now, needed after the unit is decoded
         const bool slot_free = n < 2 || mbar_test(done_s + 8 * sa, ((n - 2) >> 1) & 1u);
         uint32_t r[2][8];
+#ifdef ANSLIN_TRACE
+        if (blockIdx.x == 7 && lane == 0 && n < 48) g_prof[160 * kMaxTeams * 4 * 8 - 4 * 4 * 48 + ((team * 4 + q) * 48 + n)] = gtimer();
+#endif
         PROF(0);
 #ifdef ANSLIN_SKEL_NO_DECODE   // timing experiment only (wrong results): everything but the rANS steps
 #pragma unroll

@@ -692,3 +692,122 @@ def test_config5_fp8_moe_full_size(lay):
         r0 = r1
     for d in experts:
         d.close()
+
+
+# ------------------------------------------------------------------ the long-K `down` projections of configs 3-5
+@pytest.mark.parametrize("m", [1, 75])
+def test_config3_int8_down_long_k(m):
+    """BASELINE config 3 `down`: 5120 x 13824 int8 (K = 13824: 54 k-tiles, the long accumulation), M in {1, 75}: fused GEMM on all
+    rows x sampled channels inside both tolerances, integer sums exact."""
+    rt = _rt()
+    import torch
+    n, k = 5120, 13824
+    q, s = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=61, jitter=True))
+    xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=62))
+    buf, st = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=512, scales=s, tile_n=32, flags=2)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()).cpu().numpy()
+    cols = _sample_cols(n, 63)
+    y_ref, a_ref, acc = og.gemm_int8(xq, xs, q[cols], s[cols])
+    check_gemm(y[:, cols], y_ref, a_ref)
+    back = np.rint(y[:, cols].astype(np.float64) / (xs.astype(np.float64)[:, None] * s[cols].astype(np.float64)[None, :]))
+    small = np.abs(acc) < (1 << 22)
+    assert np.array_equal(back[small], acc[small].astype(np.float64))
+    dw.close()
+
+
+@pytest.mark.parametrize("m", [1, 64])
+def test_config4_int4_down_long_k(m):
+    """BASELINE config 4 `down`: 8192 x 28672 AWQ int4 (224 groups of 128 along K, fp16 dequantisation rounding accumulated over
+    28672 terms), fp16 X, M in {1, 64}."""
+    rt = _rt()
+    n, k = 8192, 28672
+    p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=64, outliers=False), 128)
+    x = inputs.acts_f32(m, k, seed=65).astype(np.float16)
+    buf, st = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=1024, scales=s4, zeros=z4, group_size=128, tile_n=32, flags=2)
+    assert 0.0 <= st["bits_per_weight"] - st["entropy_bits_per_symbol"] / 2 <= 0.1
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_INT4_AWQ, x)).cpu().numpy()
+    cols = _sample_cols(n, 66)
+    check_gemm(y[:, cols], *og.gemm_int4(x, p4[cols], s4[cols], z4[cols], 128))
+    dw.close()
+
+
+@pytest.mark.parametrize("tokens", [20, 95])
+def test_config5_fp8_moe_down_long_k(tokens):
+    """BASELINE config 5 `down`: 8 experts 6144 x 16384 e4m3 (K = 16384, the case SURVEY 7-8 flags for fp8 accumulation
+    precision), `tokens` tokens routed top-2, one grouped launch; every active expert's rows on sampled channels."""
+    rt = _rt()
+    import torch
+    n, k, E = 6144, 16384, 8
+    rows, tok = inputs.route_top2(tokens, E, seed=71)
+    x8_tok, xs_tok = inputs.quant_fp8_acts(inputs.acts_f32(tokens, k, seed=72))
+    x8, xs = x8_tok[tok], xs_tok[tok]
+    experts, refs = [], []
+    for e in range(E):
+        f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=80 + e, std=0.015, outliers=False))
+        buf, st = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=1024, w_scale=sc, tile_n=32, flags=2)
+        experts.append(rt.DeviceWeight(buf))
+        refs.append((f8, sc))
+    y = rt.gemm_grouped(experts, rows, rt.x_to_device(B.FMT_FP8_E4M3, x8), torch.from_numpy(xs).cuda()).cpu().numpy()
+    r0 = 0
+    for e in range(E):
+        r1 = r0 + int(rows[e])
+        if r1 > r0:
+            cols = _sample_cols(n, 90 + e, 256)
+            check_gemm(y[r0:r1][:, cols], *og.gemm_fp8(x8[r0:r1], xs[r0:r1], refs[e][0][cols], refs[e][1]))
+        r0 = r1
+    for d in experts:
+        d.close()
+
+
+@pytest.mark.parametrize("name", ["q", "o"])
+def test_config2_bf16_square_projection_m47(name):
+    """BASELINE config 2 q / o: 5120 x 5120 plain bf16 at M = 47 (the paper's uncompressed max batch, P:l.378)."""
+    rt = _rt()
+    n = k = 5120
+    m = 47
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=101 if name == "q" else 102, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=103))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
+    dw = rt.DeviceWeight(buf)
+    y = dw.gemm(rt.x_to_device(B.FMT_BF16, x)).cpu().numpy()
+    cols = _sample_cols(n, 104, 1024)
+    check_gemm(y[:, cols], *og.gemm_bf16(x, w[cols]))
+    dw.close()
+
+
+def test_bench_step_full_size():
+    """Exactly the step bench.py times: the Qwen-14B-shaped bf16 layer at M = 75, 32 x 256 tiles, lane streams + payload, four
+    persistent multi-problem launches (q+k+v, o, gate+up, down) whose problems share the SMs.  Every Y is checked against the
+    float64 oracle on 512 sampled channels per projection, and a second run must reproduce every Y bit for bit."""
+    rt = _rt()
+    import torch
+    m = 75
+    layer = [(nm, n, k, inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=1 + i, jitter=True)))
+             for i, (nm, n, k) in enumerate(inputs.QWEN14B_LAYER)]
+    names = [t[0] for t in layer]
+    dws = [rt.DeviceWeight(B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)[0]) for (_, n, k, w) in layer]
+    share = {"k": "q", "v": "q", "up": "gate"}
+    xs_np = {nm: inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=500 + i)) for i, (nm, n, k, _) in enumerate(layer) if nm not in share}
+    xs_dev = {nm: rt.x_to_device(B.FMT_BF16, x) for nm, x in xs_np.items()}
+    groups = [["q", "k", "v"], ["o"], ["gate", "up"], ["down"]]
+    calls = [rt.MultiGemm([dws[names.index(nm)] for nm in g], [xs_dev[share.get(nm, nm)] for nm in g]) for g in groups]
+    first = None
+    for rep in range(2):
+        ys = {}
+        for g, call in zip(groups, calls):
+            for nm, y in zip(g, call()):
+                ys[nm] = y
+        torch.cuda.synchronize()
+        got = {nm: y.cpu().numpy().copy() for nm, y in ys.items()}
+        if first is None:
+            first = got
+        else:
+            for nm in names:
+                assert np.array_equal(first[nm], got[nm]), "run-to-run difference in " + nm
+    for i, (nm, n, k, w) in enumerate(layer):
+        cols = _sample_cols(n, 600 + i, 512)
+        check_gemm(first[nm][:, cols], *og.gemm_bf16(xs_np[share.get(nm, nm)], w[cols]))
+    for d in dws:
+        d.close()
