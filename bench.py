@@ -85,9 +85,18 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def cpu_oracle_leg(layer, containers, m: int, names=("q", "k", "down")):
-    """The oracle as it stands, timed on the host cores over a bounded sample of the workload:
-    full container decode (plain C rANS, single thread) + float64 GEMM of the named projections."""
+def _oracle_decode_worker(buf_bytes: bytes) -> int:
+    """All-cores leg: one process decodes one container with the oracle (plain C rANS driven from numpy).  Module level so
+    that a spawned interpreter can import it; touches nothing but oracle/."""
+    from oracle import container as oc
+    _, w_dec, _ = oc.decode(np.frombuffer(buf_bytes, dtype=np.uint8))
+    return int(w_dec.size)
+
+
+def cpu_oracle_leg(layer, oracle_containers, m: int, names=("q", "k"), all_cores: bool = True):
+    """The oracle as it stands, timed on the host cores over a bounded sample of the workload (containers written by the
+    oracle's own encoder): (1) one thread: container decode + float64 GEMM of the named projections; (2) all cores: one
+    process per core, each decoding the k projection's container (decode only)."""
     from oracle import container as oc, gemm as og
     from paper_2606_15789_b200 import inputs
     try:
@@ -95,48 +104,76 @@ def cpu_oracle_leg(layer, containers, m: int, names=("q", "k", "down")):
         blas = max([i.get("num_threads", 1) for i in threadpool_info()] or [1])
     except Exception:
         blas = 1
-    flops, t0 = 0.0, time.perf_counter()
-    for (name, n, k, w), buf in zip(layer, containers):
+    flops, weights, t_dec, t0 = 0.0, 0, 0.0, time.perf_counter()
+    for (name, n, k, w) in layer:
         if name not in names:
             continue
-        _, w_dec, _ = oc.decode(buf)
+        td = time.perf_counter()
+        _, w_dec, _ = oc.decode(oracle_containers[name])
+        t_dec += time.perf_counter() - td
         x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=7))
         og.gemm_bf16(x, w_dec)
         flops += 2.0 * m * n * k
+        weights += n * k
     dt = time.perf_counter() - t0
-    return {"value": flops / dt / 1e12, "unit": UNIT, "cores": int(blas), "kind": "oracle", "seconds": round(dt, 2),
-            "sample": "projections %s of the layer at M=%d: oracle container decode (1 thread) + float64 GEMM (%d BLAS threads)"
-                      % ("/".join(names), m, blas)}
+    out = {"value": flops / dt / 1e12, "unit": UNIT, "cores": int(blas), "kind": "oracle", "seconds": round(dt, 2),
+           "decode_weights_per_s": weights / t_dec, "decoded_gbs": 2.0 * weights / t_dec / 1e9,
+           "sample": "projections %s of the layer at M=%d: oracle container decode (1 thread) + float64 GEMM (%d BLAS threads)"
+                     % ("/".join(names), m, blas)}
+    if all_cores:
+        import multiprocessing as mp
+        ncore = os.cpu_count() or 1
+        kbuf = oracle_containers["k"].tobytes()
+        kw = next(n * k for (nm, n, k, _) in layer if nm == "k")
+        try:
+            with mp.get_context("spawn").Pool(ncore) as pool:
+                pool.map(_oracle_decode_worker, [kbuf] * ncore)        # warm the workers (imports, library build)
+                t1 = time.perf_counter()
+                done = pool.map(_oracle_decode_worker, [kbuf] * (2 * ncore))
+                ta = time.perf_counter() - t1
+            out["all_cores"] = {"cores": ncore, "decode_weights_per_s": sum(done) / ta, "decoded_gbs": 2.0 * sum(done) / ta / 1e9,
+                                "seconds": round(ta, 2), "sample": "%d oracle decodes of the k projection (%d weights each), one process per core"
+                                                                   % (2 * ncore, kw)}
+        except Exception as e:       # a box that cannot spawn processes: say so, keep the single-thread leg
+            out["all_cores"] = {"unavailable": repr(e)[:200]}
+    return out
+
+
+def oracle_containers_for(layer, names):
+    """Containers of the named projections written by the ORACLE's encoder (the reference arm and the CPU leg load no product code)."""
+    from oracle import container as oc
+    return {nm: oc.encode(0, w, k, tile_k=256, tile_n=32, flags=3)[0] for (nm, n, k, w) in layer if nm in names}
 
 
 def run_reference(args):
-    from paper_2606_15789_b200 import binding as B, build as libbuild
-    libbuild.build()
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    from oracle import codec
+    codec.build()
     layer = [t for t in layer_weights() if t[0] in ("k",)]       # bounded sample: the k projection (1024x5120)
-    containers = [B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=64, flags=1)[0] for (_, n, k, w) in layer]
+    conts = oracle_containers_for(layer, ("k",))
     for _ in range(args.warmup):
-        cpu_oracle_leg(layer, containers, args.m, names=("k",))
+        cpu_oracle_leg(layer, conts, args.m, names=("k",), all_cores=False)
     t0 = time.perf_counter()
-    vals = [cpu_oracle_leg(layer, containers, args.m, names=("k",)) for _ in range(args.steps)]
+    vals = [cpu_oracle_leg(layer, conts, args.m, names=("k",), all_cores=False) for _ in range(args.steps)]
     dt = time.perf_counter() - t0
     flops = args.steps * 2.0 * args.m * 1024 * 5120
     v = flops / dt / 1e12
     cb = dict(vals[-1]); cb["value"] = v
-    cb["sample"] = "each step = oracle decode + float64 GEMM of the k projection (1024x5120) at M=%d" % args.m
+    sample = "each step = oracle decode (container from the oracle's encoder) + float64 GEMM of the k projection (1024x5120) at M=%d" % args.m
+    cb["sample"] = sample
     print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
                       "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
                       "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
-                      "config": {"workload": WORKLOAD, "batch_m": args.m}, "cpu_baseline": cb,
+                      "config": {"workload": WORKLOAD, "batch_m": args.m, "sample": sample}, "cpu_baseline": cb,
                       "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
-# ALU-pipe warp instructions per decoded bf16 symbol in fused_gemm_kernel's hot loop (cuobjdump -sass):
-# table slot 1 (LOP3), entry fields 3 (SHF, LOP3, SHF), state shift 1 (SHF), renormalisation test 1 (ISETP),
-# symbol + raw byte -> bf16 4 per weight pair... = 3 (PRMT 1.5, SHF 1, LOP3 0.5), per-unit bookkeeping ~1.
-ALU_INSTR_PER_SYMBOL = 10.0
+# Warp instructions per decoded bf16 symbol in the hot loop of fused_tmem_kernel<bf16> (counted in
+# profiles/r2_sass_decode_loop.md): 13 in the rANS step (IMAD.SHL, LOP3, LDS, SHF x3, LOP3, IMAD, ISETP, @IMAD, @IMAD.IADD,
+# @LDS.U16 + the state shift) and 2.5 in the bf16 merge (PRMT x2, SHF, IMAD.SHL, LOP3 per two weights).
+INSTR_PER_SYMBOL = 15.5
 
 
 def run_other_config(args):
@@ -186,6 +223,7 @@ def run_other_config(args):
         calls = [lambda: rt.gemm_grouped(experts, rows, x, xsd, y)]
         name, dtype, nw, flops = "config5: Mixtral-shaped MoE, 8 experts fp8 gate 16384x6144, 95 tokens top-2", "fp8", E * n * k, 2.0 * 2 * tokens * n * k
         x_host, y_rows = torch.from_numpy(x8).pin_memory(), 2 * tokens
+    launches_per_call = B.anslin_gemm_launches(int(np.count_nonzero(rows)) if args.workload == "c5" else 1)
     y_host = torch.empty((y_rows, n), dtype=torch.float32).pin_memory()
     sampler = ClockSampler(0); sampler.start(); sampler.wait_first()
     for i in range(max(args.warmup, 3)):
@@ -197,7 +235,7 @@ def run_other_config(args):
     e0.record()
     for i in range(args.steps):
         calls[i % len(calls)]()
-        launches += B.anslin_last_launch_count()
+        launches += launches_per_call
     e1.record(); torch.cuda.synchronize()
     time.sleep(0.03)
     clocks = sampler.stop(lo, sampler.mark())
@@ -225,6 +263,92 @@ def run_other_config(args):
                       "bits_per_weight": st["bits_per_weight"]}))
 
 
+def config_records(hbm_peak: float, tc_peak: float, sm_mhz: float):
+    """one record per (config, matrix, M) for BASELINE configs 3-5 (largest matrix and its `down`, every listed
+    M): fused time with the three bounds (compressed bytes over HBM, FLOPs over the tensor peak, rANS steps over the issue
+    slots), the dense comparator and the decode-only time.  Inputs larger than L2 by rotating copies; CUDA events."""
+    import torch
+    from paper_2606_15789_b200 import binding as B, inputs, runtime as rt
+    recs = []
+
+    def timed(fns, iters=8):
+        for f in fns:
+            f()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize(); a.record()
+        for i in range(iters):
+            fns[i % len(fns)]()
+        b.record(); torch.cuda.synchronize()
+        return a.elapsed_time(b) * 1e3 / iters           # us
+
+    def record(cfg, mat, n, k, m, fmt_name, cont_bytes, n_sym, flops, tc_ratio, fused_us, dense_us, decode_us, bits, h):
+        hbm_us = cont_bytes / (hbm_peak * 1e9) * 1e6
+        tc_us = flops / (tc_peak * tc_ratio * 1e12) * 1e6
+        issue_us = n_sym * 13.0 / (148 * 4 * 32 * sm_mhz * 1e6) * 1e6            # 13 warp instructions per rANS step
+        recs.append({"config": cfg, "matrix": "%s %dx%d" % (mat, n, k), "m": m, "format": fmt_name, "fused_us": round(fused_us, 1),
+                     "tflops": round(flops / fused_us / 1e6, 2), "compressed_gbs": round(cont_bytes / fused_us / 1e3, 1),
+                     "bound_hbm_us": round(hbm_us, 1), "bound_tensor_us": round(tc_us, 2), "bound_issue_us": round(issue_us, 1),
+                     "frac_of_hbm_roofline": round(hbm_us / fused_us, 3), "dense_us": None if dense_us is None else round(dense_us, 1),
+                     "decode_only_us": round(decode_us, 1), "bits_per_weight": round(bits, 3), "h_sym": round(h, 3)})
+
+    def copies_of(buf, min_bytes=140e6):
+        return [rt.DeviceWeight(buf) for _ in range(max(2, int(np.ceil(min_bytes / buf.size))))]
+
+    # ---- config 3: SQ8 int8, Qwen-14B gate / down
+    for mat, n, k, tk in (("gate", 13824, 5120, 1024), ("down", 5120, 13824, 512)):
+        q, s8 = inputs.quant_sq8_weights(inputs.weights_f32(n, k, seed=5 if mat == "gate" else 61, jitter=True))
+        buf, st = B.anslin_encode_host(B.FMT_INT8, q, n, k, tile_k=tk, scales=s8, tile_n=32, flags=B.FLAG_LANE_STREAMS)
+        dws = copies_of(buf)
+        wd = [torch.from_numpy(q).cuda() for _ in range(2)]
+        sd = torch.from_numpy(s8.view(np.int16)).cuda()
+        dec_us = timed([lambda d=d: d.decode() for d in dws], 4)
+        for m in (1, 32, 75):
+            xq, xs = inputs.quant_int8_acts(inputs.acts_f32(m, k, seed=6))
+            x, xsd = rt.x_to_device(B.FMT_INT8, xq), torch.from_numpy(xs).cuda()
+            y = torch.empty((m, n), dtype=torch.float32, device="cuda")
+            fused = timed([lambda d=d: d.gemm(x, xsd, y) for d in dws])
+            dense = timed([lambda w=w: rt.dense_gemm(B.FMT_INT8, w, x, w_scale_vec=sd, x_scale=xsd, y=y) for w in wd])
+            record("c3", mat, n, k, m, "int8", buf.size, n * k, 2.0 * m * n * k, 2.0, fused, dense, dec_us, st["bits_per_weight"], st["entropy_bits_per_symbol"])
+        for d in dws:
+            d.close()
+        del dws, wd
+    # ---- config 4: AWQ int4 g128, Llama-70B gate / down
+    for mat, n, k in (("gate", 28672, 8192), ("down", 8192, 28672)):
+        p4, s4, z4 = inputs.quant_awq4_weights(inputs.weights_f32(n, k, seed=11 if mat == "gate" else 64, outliers=False), 128)
+        buf, st = B.anslin_encode_host(B.FMT_INT4_AWQ, p4, n, k, tile_k=1024, scales=s4, zeros=z4, group_size=128, tile_n=32, flags=B.FLAG_LANE_STREAMS)
+        dws = copies_of(buf)
+        dec_us = timed([lambda d=d: d.decode() for d in dws], 4)
+        for m in (1, 16, 64):
+            x = rt.x_to_device(B.FMT_INT4_AWQ, inputs.acts_f32(m, k, seed=12).astype(np.float16))
+            y = torch.empty((m, n), dtype=torch.float32, device="cuda")
+            fused = timed([lambda d=d: d.gemm(x, None, y) for d in dws])
+            record("c4", mat, n, k, m, "int4-awq (fp16 MMA)", buf.size, n * k // 2, 2.0 * m * n * k, 1.0, fused, None, dec_us,
+                   st["bits_per_weight"], st["entropy_bits_per_symbol"] / 2)
+        for d in dws:
+            d.close()
+        del dws
+    # ---- config 5: fp8-e4m3 MoE, 8 Mixtral-shaped experts, top-2 routing, one grouped launch
+    for mat, n, k in (("gate", 16384, 6144), ("down", 6144, 16384)):
+        experts, nbytes, bits, hs = [], 0, 0.0, 0.0
+        for e in range(8):
+            f8, sc = inputs.quant_fp8_weights(inputs.weights_f32(n, k, seed=(30 if mat == "gate" else 80) + e, std=0.015, outliers=False))
+            buf, st = B.anslin_encode_host(B.FMT_FP8_E4M3, f8, n, k, tile_k=1024, w_scale=sc, tile_n=32, flags=B.FLAG_LANE_STREAMS)
+            experts.append(rt.DeviceWeight(buf)); nbytes += buf.size; bits += st["bits_per_weight"] / 8; hs += st["entropy_bits_per_symbol"] / 8
+        dec_us = timed([lambda: [d.decode() for d in experts]], 2)
+        for tokens in (20, 95):
+            rows, tok = inputs.route_top2(tokens, 8, seed=21)
+            x8t, xst = inputs.quant_fp8_acts(inputs.acts_f32(tokens, k, seed=22))
+            x, xsd = rt.x_to_device(B.FMT_FP8_E4M3, x8t[tok]), torch.from_numpy(xst[tok]).cuda()
+            y = torch.empty((2 * tokens, n), dtype=torch.float32, device="cuda")
+            fused = timed([lambda: rt.gemm_grouped(experts, rows, x, xsd, y)], 4)
+            record("c5", "8 experts x " + mat, n, k, tokens, "fp8-e4m3", nbytes, 8 * n * k, 2.0 * 2 * tokens * n * k, 2.0, fused, None, dec_us, bits, hs)
+        for d in experts:
+            d.close()
+        del experts
+    torch.cuda.empty_cache()
+    return recs
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -232,7 +356,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="anslin")
     ap.add_argument("--m", type=int, default=75)
-    ap.add_argument("--no-extras", action="store_true", help="skip per-M table, dense comparator, decode-only and CPU legs")
+    ap.add_argument("--no-extras", action="store_true", help="skip per-M table, dense comparator, decode-only, per-config records and CPU legs")
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-(config, matrix, M) records of BASELINE configs 3-5")
     ap.add_argument("--tile", default="32x256", help="tile_n x tile_k of the compressed containers (128x64 = BASELINE config 1's shape)")
     ap.add_argument("--layout", default="lanes", choices=["lanes", "interleaved"], help="word layout of the containers: every lane "
                     "its own stream (32-row tiles only) or words interleaved in read order")
@@ -303,7 +428,7 @@ def main():
             if record is not None:
                 record[gi][0].record()
             call()
-            launches += B.anslin_last_launch_count()
+            launches += B.anslin_gemm_launches(len(groups[gi]))      # one block of <= 256 rows per projection
             if record is not None:
                 record[gi][1].record()
         return launches
@@ -343,10 +468,13 @@ def main():
     hbm_peak, tc_peak, peak_kind = peaks()
     # the fused kernel is the only kernel of a step: its launches' average duration = timed region / launches
     achieved = sum(algo_bytes) / (ms_step * 1e-3) / 1e9
-    traffic = None
+    # dram bytes per launch come from a committed ncu capture: reported only for the configuration that capture was taken on
+    traffic, traffic_source = None, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("fused_gemm_bytes_per_launch_mean")
+        tj = json.load(open(tp))
+        if tj.get("config") == {"batch_m": m, "tile": args.tile, "word_layout": args.layout, "symbols": args.symbols, "launch_groups": group_names}:
+            traffic, traffic_source = tj.get("fused_gemm_bytes_per_launch_mean"), tj.get("source")
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned X in, Y out) inside the timed region
     # Device->host reads of Y run on a copy stream of their own, behind an event per launch group, so that they
@@ -390,15 +518,15 @@ def main():
                       "parallelism": "replicas, one batch per GPU" if world > 1 else "1 GPU"},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
            "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                        "traffic": traffic, "peak_kind": "of " + peak_kind,
-                        "kernel": "fused_gemm_kernel<bf16,payload> (%d launches/step; bytes = containers + X + Y)" % len(calls)},
-           # the bound that actually binds (SURVEY §8(d) bound 3): the decoder's integer work on the ALU pipe.
-           # peak = SMs x 4 schedulers x 16 lanes/clk (one ALU-pipe warp instruction per 2 clk) x SM clock under load
-           #        / ALU-pipe instructions per decoded symbol in the hot loop's SASS
-           "decoder_bound": (lambda peak: {"bound": "alu", "achieved": n_weights / (ms_step * 1e-3) / 1e9, "peak": peak,
+                        "traffic": traffic, "traffic_source": traffic_source, "peak_kind": "of " + peak_kind,
+                        "kernel": "fused_tmem_kernel<bf16,payload> (%d launches/step; bytes = containers + X + Y)" % len(calls)},
+           # the bound that actually binds (SURVEY §8(d) bound 3): warp-instruction issue slots of the rANS step.
+           # peak = SMs x 4 schedulers x 1 warp instruction (32 lanes) per clk x SM clock under load
+           #        / warp instructions per decoded symbol in the hot loop's SASS
+           "decoder_bound": (lambda peak: {"bound": "issue", "achieved": n_weights / (ms_step * 1e-3) / 1e9, "peak": peak,
                                            "unit": "Gsymbol/s", "frac": n_weights / (ms_step * 1e-3) / 1e9 / peak,
-                                           "alu_instr_per_symbol": ALU_INSTR_PER_SYMBOL, "sm_mhz": clocks.get("sm_mhz")})(
-               148 * 4 * 16 * float(clocks.get("sm_mhz") or 1965.0) * 1e6 / ALU_INSTR_PER_SYMBOL / 1e9),
+                                           "instr_per_symbol": INSTR_PER_SYMBOL, "sm_mhz": clocks.get("sm_mhz")})(
+               148 * 4 * 32 * float(clocks.get("sm_mhz") or 1965.0) * 1e6 / INSTR_PER_SYMBOL / 1e9),
            "compressed_gbs": world * comp_bytes / (ms_step * 1e-3) / 1e9,
            "decoded_weights_gbs": world * n_weights * 2 / (ms_step * 1e-3) / 1e9,
            "bits_per_weight": 8.0 * comp_bytes / n_weights,
@@ -489,7 +617,11 @@ def main():
         t = a.elapsed_time(b) / 3
         out["decode_only"] = {"ms": round(t, 4), "decoded_gbs": round(n_weights * 2 / (t * 1e-3) / 1e9, 1),
                               "gsym_per_s": round(n_weights / (t * 1e-3) / 1e9, 1)}
-        out["cpu_baseline"] = cpu_oracle_leg(layer, containers, m)
+        if not args.no_configs:
+            del wsd
+            torch.cuda.empty_cache()
+            out["configs"] = config_records(hbm_peak, tc_peak, float(clocks.get("sm_mhz") or 1965.0))
+        out["cpu_baseline"] = cpu_oracle_leg(layer, oracle_containers_for(layer, ("q", "k")), m)
     if rank == 0:
         print(json.dumps(out))
     ranks.close()

@@ -131,8 +131,12 @@ typedef struct anslin_weight anslin_weight;
  *   container_host: host copy (at least header + freq + offset sections; `bytes` = how many are
  *   readable); container_dev: device copy of the WHOLE container (16-byte aligned), may be NULL
  *   for host-only inspection.  Checks magic/version/shape/section bounds, that the frequency table
- *   sums to 2^12 and that tile offsets are monotone and in range -> ANSLIN_ERR_CORRUPT otherwise
- *   (so that no kernel can be steered out of bounds by a damaged table).
+ *   sums to 2^12, that tile offsets are monotone and in range and -- when `bytes` covers the records
+ *   section of a lane-stream container -- every segment table (region sizes add up to the segment's
+ *   word count, the staged segment fits max_seg_bytes and its record) -> ANSLIN_ERR_CORRUPT otherwise.
+ *   What anslin_open has checked cannot steer a kernel out of bounds.  A container whose records were
+ *   never on the host (anslin_encode_device) is trusted; the kernels clamp every cursor they derive
+ *   from a segment table into the staged buffer, so a damaged table there gives wrong weights.
  */
 int anslin_open(const void *container_host, size_t bytes, const void *container_dev, anslin_weight **out);
 int anslin_close(anslin_weight *w);
@@ -242,8 +246,10 @@ int anslin_encode_device(const anslin_desc *desc, const void *w_dev, const void 
                          void *container_dev, size_t capacity, void *head_host, size_t head_capacity,
                          void *workspace_dev, size_t workspace_bytes, size_t *bytes_out, void *stream);
 
-/* Number of kernels the last device call on this thread enqueued (for bench.py's gpu_launches). */
-int anslin_last_launch_count(void);
+/* How many kernels a GEMM call enqueues, as a function of its shape (the library keeps no state to ask): row_blocks = the
+ * call's problems cut into blocks of at most 256 batch rows (anslin_gemm: ceil(m / 256); anslin_gemm_multi: n; grouped: sum
+ * over active experts of ceil(rows / 256)); a launch takes up to eight blocks.  Host only. */
+int anslin_gemm_launches(int64_t row_blocks);
 
 const char *anslin_status_string(int status);
 

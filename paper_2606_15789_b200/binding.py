@@ -25,7 +25,7 @@ EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_c
            "anslin_gemm_multi", "anslin_gemm_multi_ex", "anslin_gemm_grouped",
            "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_histogram", "anslin_entropy_bits",
            "anslin_entropy_weighted", "anslin_encode_device_workspace_bytes", "anslin_encode_device_head_bytes",
-           "anslin_encode_device", "anslin_last_launch_count", "anslin_status_string"]
+           "anslin_encode_device", "anslin_gemm_launches", "anslin_status_string"]
 
 
 class AnslinError(RuntimeError):
@@ -82,7 +82,8 @@ def lib() -> ctypes.CDLL:
         L.anslin_encode_device_workspace_bytes.argtypes = [ctypes.POINTER(Desc)]; L.anslin_encode_device_workspace_bytes.restype = sz
         L.anslin_encode_device_head_bytes.argtypes = [ctypes.POINTER(Desc)]; L.anslin_encode_device_head_bytes.restype = sz
         L.anslin_encode_device.argtypes = [ctypes.POINTER(Desc), vp, vp, vp, vp, sz, vp, sz, vp, sz, ctypes.POINTER(sz), vp]
-        L.anslin_last_launch_count.restype = ctypes.c_int
+        L.anslin_gemm_launches.restype = ctypes.c_int
+        L.anslin_gemm_launches.argtypes = [ctypes.c_int64]
         L.anslin_status_string.argtypes = [ctypes.c_int]; L.anslin_status_string.restype = ctypes.c_char_p
         _lib = L
     return _lib
@@ -266,5 +267,5 @@ def anslin_entropy_weighted(hs, ns) -> float:
                                                n.ctypes.data_as(ctypes.POINTER(ctypes.c_uint64)), h.size))
 
 
-def anslin_last_launch_count() -> int:
-    return int(lib().anslin_last_launch_count())
+def anslin_gemm_launches(row_blocks: int) -> int:
+    return int(lib().anslin_gemm_launches(int(row_blocks)))

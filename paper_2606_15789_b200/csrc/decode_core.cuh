@@ -238,7 +238,9 @@ __device__ __forceinline__ void lane_open_segments(LaneStream (&s)[J], uint32_t 
       for (uint32_t o = 16u * uint32_t(lane); o < nbytes; o += kFillBytes)
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(buf + o), "l"(src + o) : "memory");
     }
-    s[j].ptr = buf + skew + 2u * ((lane & 1) ? end_p - 1u : start_p);
+    // the cursor is clamped into the staged buffer: a damaged table (anslin_open cannot check a container whose records
+    // never were on the host) yields wrong weights, never an address outside the buffer
+    s[j].ptr = buf + skew + 2u * min((lane & 1) ? end_p - 1u : start_p, (bufbytes - skew) / 2u - 1u);
     s[j].goff += 2u * total;
   }
   extra();

@@ -478,6 +478,30 @@ int anslin_open(const void *container_host, size_t bytes, const void *container_
   if (g.fmt == ANSLIN_FMT_BF16_PAIR4 && !in(h.off_zeros, 16)) return ANSLIN_ERR_CORRUPT;
   if (side_bytes(g) && !in(h.off_scales, side_bytes(g))) return ANSLIN_ERR_CORRUPT;
   if ((g.flags & ANSLIN_FLAG_LANE_STREAMS) && (h.max_seg_bytes < 32 || h.max_seg_bytes > 2 * 0xFFFF + 64)) return ANSLIN_ERR_CORRUPT;
+  // Lane-stream records: when the host copy includes the records section, every segment table is checked too (the kernels
+  // turn its region sizes into shared-memory cursors): the region sizes add up to the segment's word count, the staged
+  // segment fits the buffer the header promises (max_seg_bytes), and the segments stay inside their record.
+  if ((g.flags & ANSLIN_FLAG_LANE_STREAMS) && bytes >= h.off_records + uint64_t(offs[g.n_tiles]) * 16) {
+    const size_t nseg = size_t(g.steps) / seg_steps_of(g.fmt);
+    for (size_t t = 0; t < g.n_tiles; ++t) {
+      const uint8_t *rec = p + h.off_records + uint64_t(offs[t]) * 16;
+      const uint64_t rec_bytes = uint64_t(offs[t + 1] - offs[t]) * 16;
+      uint64_t goff = 4 * kLanes + uint64_t(kSegTableBytes) * nseg;
+      if (goff > rec_bytes) return ANSLIN_ERR_CORRUPT;
+      for (size_t sg = 0; sg < nseg; ++sg) {
+        const uint8_t *te = rec + 4 * kLanes + kSegTableBytes * sg;
+        uint16_t base, total;
+        std::memcpy(&base, te, 2);
+        std::memcpy(&total, te + 2, 2);
+        uint32_t sum = 0;
+        for (int r = 0; r < kLanes / 2; ++r) sum += uint32_t(base) + te[4 + r];
+        if (sum != total) return ANSLIN_ERR_CORRUPT;
+        const uint64_t staged = (((goff & 15) + 2 * uint64_t(total) + 15) & ~uint64_t(15));
+        if (staged > align16(h.max_seg_bytes) || goff + 2 * uint64_t(total) > rec_bytes) return ANSLIN_ERR_CORRUPT;
+        goff += 2 * uint64_t(total);
+      }
+    }
+  }
   anslin_weight *w = new (std::nothrow) anslin_weight;
   if (!w) return ANSLIN_ERR_INVALID_ARG;
   w->h = h;

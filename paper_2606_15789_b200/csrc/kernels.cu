@@ -32,7 +32,6 @@ using namespace anslin;
 
 namespace {
 
-thread_local int g_launches = 0;
 
 // ------------------------------------------------------------------------------------------------
 // PTX wrappers
@@ -131,7 +130,10 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
       : "memory");
   return done != 0;
 }
-constexpr int kBarEpiGo = 2;   // named barrier: MMA warp -> epilogue warps, "accumulator is complete"
+// named barriers 2 and 3: MMA warp -> epilogue warps, "accumulator of segment si is complete".  The id alternates with the
+// segment: a second arrive on the same id then belongs to segment si + 2, which the MMA warp reaches only after the
+// epilogue warps have drained segment si (tempty), i.e. after all four have passed the barrier for it.
+constexpr int kBarEpiGo = 2;
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
@@ -381,7 +383,7 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     if (is_fp8_path(FMT)) ws = p.w_scale;
     // The MMA warp watches the accumulator's mbarrier and releases us through a named barrier: the four
     // epilogue warps sleep in hardware meanwhile instead of polling next to the decoder warps.
-    named_bar_sync(kBarEpiGo, (kEpiWarps + 1) * 32);
+    named_bar_sync(kBarEpiGo + int(si & 1u), (kEpiWarps + 1) * 32);
     tc_fence_after();
     const uint32_t seg = (t == t_begin ? 0u : 1u);
     uint32_t *part = p.partials + size_t(c * 2u + seg) * p.mpad * kTileN;
@@ -705,7 +707,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
         const uint32_t bar = tfull_s + 8 * (rel & 1u), par = (rel >> 1) & 1u;
         if (block) mbar_wait(bar, par);
         else if (!__all_sync(0xffffffffu, mbar_test(bar, par))) break;
-        named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32);
+        named_bar_arrive(kBarEpiGo + int(rel & 1u), (kEpiWarps + 1) * 32);
         ++rel;
       }
     };
@@ -855,7 +857,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
         __syncwarp();
       }
       mbar_wait(tfull_s + 8 * ab, (si >> 1) & 1u);
-      named_bar_arrive(kBarEpiGo, (kEpiWarps + 1) * 32);
+      named_bar_arrive(kBarEpiGo + int(si & 1u), (kEpiWarps + 1) * 32);
       t += nt;
     }
     (void)UK;
@@ -971,7 +973,6 @@ int launch_fused_y(const TensorMaps &tms, const FusedParams &p, uint32_t grid, s
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if (cudaLaunchKernelEx(&cfg, kern, tms, p) != cudaSuccess) return ANSLIN_ERR_CUDA;
-  ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 
@@ -1006,7 +1007,6 @@ int launch_tmem_y(const TensorMaps &tms, const TmemParams &p, uint32_t grid, siz
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   if (cudaLaunchKernelEx(&cfg, kern, tms, p) != cudaSuccess) return ANSLIN_ERR_CUDA;
-  ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 template <uint32_t FMT, bool PAYLOAD>
@@ -1243,7 +1243,6 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   uint32_t per_sm = uint32_t(occ);
   const uint32_t ctas = std::min<uint32_t>((jobs + kDecWarps - 1) / kDecWarps, uint32_t(sm_budget()) * per_sm);
   kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out), stream_bytes);
-  ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 template <uint32_t FMT, bool PAYLOAD>
@@ -1257,7 +1256,6 @@ int launch_dense(const CUtensorMap &tmw, const CUtensorMap &tmx, DenseParams &p,
   auto kern = dense_gemm_kernel<FMT>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
   kern<<<grid, kDenseThreads, smem, st>>>(tmw, tmx, p);
-  ++g_launches;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 
@@ -1274,10 +1272,11 @@ int anslin_debug_prof(void *host_out, size_t bytes) {
 }
 #endif
 
-int anslin_last_launch_count(void) { return g_launches; }
+// Kernels a GEMM call enqueues, from its shape alone: its problems are cut into blocks of <= 256 batch rows and every
+// launch takes up to eight blocks.
+int anslin_gemm_launches(int64_t row_blocks) { return row_blocks < 1 ? 0 : int((row_blocks + kMaxProblems - 1) / kMaxProblems); }
 
 int anslin_decode(const anslin_weight *w, void *w_out_dev, size_t capacity, void *stream) {
-  g_launches = 0;
   if (!w || !w->dev || !w_out_dev) return ANSLIN_ERR_INVALID_ARG;
   if (reinterpret_cast<uintptr_t>(w_out_dev) & 15) return ANSLIN_ERR_INVALID_ARG;
   const Header &h = w->h;
@@ -1322,7 +1321,6 @@ size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, in
 
 int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m, const void *x_scale_dev,
                 void *y_dev, int64_t ldy, void *workspace_dev, size_t workspace_bytes, void *stream) {
-  g_launches = 0;
   if (!w) return ANSLIN_ERR_INVALID_ARG;
   if (m <= kMaxM)
     return gemm_launch(1, &w, &x_dev, x_dtype, &ldx, &m, &x_scale_dev, &y_dev, &ldy, workspace_dev, workspace_bytes,
@@ -1352,7 +1350,6 @@ int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int
 int anslin_gemm_multi_ex(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
                          const int32_t *m, const void *const *x_scale_dev, void *const *y_dev, uint32_t y_dtype, const int64_t *ldy,
                          void *workspace_dev, size_t workspace_bytes, void *stream) {
-  g_launches = 0;
   if (!weights || n < 1 || !x_dev || !ldx || !m || !y_dev || !ldy) return ANSLIN_ERR_INVALID_ARG;
   const void *no_scales[kMaxProblems] = {nullptr};
   for (int32_t i0 = 0; i0 < n; i0 += kMaxProblems) {   // more than kMaxProblems: consecutive launches on the same stream
@@ -1373,7 +1370,6 @@ int anslin_gemm_multi(const anslin_weight *const *weights, int32_t n, const void
 int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts, const int32_t *rows_per_expert_host,
                         const void *x_dev, uint32_t x_dtype, int64_t ldx, const void *x_scale_dev, void *y_dev, int64_t ldy,
                         void *workspace_dev, size_t workspace_bytes, void *stream) {
-  g_launches = 0;
   if (!experts || n_experts < 1 || !rows_per_expert_host || !x_dev || !y_dev) return ANSLIN_ERR_INVALID_ARG;
   // active experts -> problems of one persistent launch (kMaxProblems per launch)
   const anslin_weight *w[kMaxProblems];
@@ -1422,7 +1418,6 @@ size_t anslin_dense_workspace_bytes(uint32_t n_out, uint32_t k_in, int32_t m) {
 int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32_t k_in, const void *w_scale_dev, float w_scale,
                       const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m, const void *x_scale_dev, void *y_dev,
                       int64_t ldy, void *workspace_dev, size_t workspace_bytes, void *stream) {
-  g_launches = 0;
   if (!w_dev || !x_dev || !y_dev || !workspace_dev) return ANSLIN_ERR_INVALID_ARG;
   if (format > kFormatMax || m < 1 || m > 256) return ANSLIN_ERR_UNSUPPORTED;
   // the int4 slot takes fp16 weights (what AWQ dequantises to): same MMA kind as the fused int4 path

@@ -161,6 +161,34 @@ def test_open_rejects_corrupt_containers():
     assert status(buf[:64].copy()) == 1                         # shorter than a header: INVALID_ARG
 
 
+def test_open_checks_lane_stream_segment_tables():
+    """the per-segment tables of a lane-stream record (u16 base, u16 total, 16 x u8 delta) become shared-memory
+    cursors in the kernels, so anslin_open checks them whenever the host copy includes the records section."""
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(128, 512, seed=36, jitter=True))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, 128, 512, tile_k=256, flags=3, tile_n=32)
+    h = oc.Header.unpack(buf)
+    assert h.flags & 2
+
+    def status(b, nbytes=None):
+        out = ctypes.c_void_p()
+        rc = B.lib().anslin_open(b.ctypes.data, b.size if nbytes is None else nbytes, None, ctypes.byref(out))
+        if rc == 0:
+            B.lib().anslin_close(out)
+        return rc
+
+    assert status(buf) == 0
+    table = h.off_records + 128                    # first tile: 32 states, then the segment table
+    for off, what in ((table, "base"), (table + 2, "total"), (table + 4, "delta[0]"), (table + 19, "delta[15]")):
+        bad = buf.copy(); bad[off] ^= 0x40
+        assert status(bad) == 4, what
+    # the tables of a later tile are looked at as well
+    offs = np.frombuffer(buf[h.off_offsets:h.off_offsets + 4 * (h.n_tiles + 1)].tobytes(), dtype=np.uint32)
+    bad = buf.copy(); bad[h.off_records + 16 * int(offs[5]) + 128 + 7] ^= 0x20
+    assert status(bad) == 4
+    # a host copy that stops before the records (header + tables only) cannot be checked that far: accepted
+    assert status(buf, int(h.off_records)) == 0
+
+
 def test_gemm_entry_points_fail_loudly_without_a_device():
     """No CPU fallback: on a box without a GPU the device entry points return an error status."""
     import torch
