@@ -1086,7 +1086,8 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   // shared-memory design splits such a launch by single k-tiles and finishes sooner.
   uint64_t pairs = 0;
   for (int i = 0; i < n; ++i) pairs += uint64_t(ws[i]->h.n_out / kTileN) * ((ws[i]->h.k_in / ws[i]->h.tile_k + 1) / 2);
-  const bool use_tmem = T >= 2 && pairs * 10 >= uint64_t(sm_budget()) * T * 6;
+  const bool long_tiles = h0.tile_k / unit_k_of(h0.format) >= 32;
+  const bool use_tmem = T >= 2 && !(long_tiles && pairs * 10 < uint64_t(sm_budget()) * T * 6);
   // CTAs: one per SM in total, shared out in proportion to the problems' sizes
   const uint32_t S = uint32_t(sm_budget());
   uint32_t ncta[kMaxProblems], cap[kMaxProblems];
