@@ -591,6 +591,15 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         if (lane == 0) mbar_arrive(full_s + 8 * sa);   // the fourth arrival lets the team's issuer warp multiply this unit step
         PROF(3);
       }
+#ifdef ANSLIN_BOUNDS_CHECK   // debug builds (compute-sanitizer is closed on this pool): every word cursor ended inside its staged buffer
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const uint32_t lo = stage_s + uint32_t(j) * P.stream_bytes;
+        if (s[j].ptr + 2u < lo || s[j].ptr > lo + P.stream_bytes) __trap();
+        if (PAYLOAD && (s[j].x < kL || s[j].x >= 2u * kL)) __trap();   // the end state is L + payload
+        if (!PAYLOAD && s[j].x != kL) __trap();                        // ... or exactly the encoder's start state
+      }
+#endif
     }
     PROF(0);
     // ---- epilogue of this stripe segment: the team reads its own accumulator ----
