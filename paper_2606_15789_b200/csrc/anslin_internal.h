@@ -24,7 +24,6 @@ constexpr uint32_t kL = 1u << kStateLoLog2;
 constexpr uint32_t kM = 1u << kProbBits;
 constexpr int kHeaderBytes = 128;
 constexpr int kTailBytes = 4096; // readable bytes guaranteed after the records section (ring read-ahead)
-constexpr int kSegSteps = 256;   // lane-stream layout: decode steps per record segment
 constexpr int kSegTableBytes = 20; // per segment: u16 base, u16 total words, 16 x u8 (region words - base)
 constexpr int kUnitBytes = 4096; // one operand unit = 128 rows x 32 B (one tcgen05.mma K step)
 

@@ -6,7 +6,8 @@
 // interleaved in decoder read order, so the renormalising lanes of a step read CONSECUTIVE 16-bit
 // words (P:l.256 "renormalization loads are naturally coalesced"): ballot + popc prefix picks the word.
 //
-// A decode step is a ~140-cycle dependent chain (LDS table -> IMAD -> vote -> popc -> LDS word), so
+// A decode step is a dependent chain (LDS table -> IMAD -> renormalise: 74 clk for one lane-stream chain alone on an
+// SM, 86 clk for two interleaved; more with ballot / prefix count of the interleaved-word layout), so
 // throughput comes from independent chains in flight: a warp decodes J tiles at once, their steps
 // interleaved instruction by instruction (J = 2 for 32-row tiles), and many such warps share an SM.
 //
@@ -176,7 +177,7 @@ __device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint3
 }
 
 // ---- lane-stream layout (ANSLIN_FLAG_LANE_STREAMS): every lane reads its own word stream ----------------
-// The record is cut into segments of kSegSteps decode steps; a segment's words are staged whole in shared
+// The record is cut into segments of seg_steps_of(format) decode steps; a segment's words are staged whole in shared
 // memory, lanes 2p and 2p+1 sharing region p (lane 2p walks up from its start, lane 2p+1 down from its end).
 // No ballot, no prefix count, no ring upkeep: a step renormalises with a predicated load at the lane's cursor.
 struct LaneStream {

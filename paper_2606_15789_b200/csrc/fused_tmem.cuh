@@ -7,21 +7,21 @@
 //     registers into 8 TMEM columns with one tcgen05.st — no shared-memory operand slot, no swizzle, no proxy fence
 //     ("writes the decoded value directly into the shared-memory" P:l.254 becomes "into tensor memory");
 //   * every warp runs Alg V.2 (P:l.260-287) on TWO tiles at once (k-tiles kt, kt+1 of its stripe quadrant), their
-//     steps interleaved, so a team hands the tensor core two K slices per unit step;
-//   * there is no central MMA warp: the team meets on a named barrier and ITS OWN warp 0 issues the two
-//     tcgen05.mma (A from TMEM, X slice from shared memory, accumulator in TMEM) and the commit that frees the
-//     A columns and the X ring slot ("ready[2]" flags of P:l.210 -> one mbarrier per ring slot);
-//   * the X slices (pad16(m) rows x 32 bytes, SWIZZLE_32B) arrive by TMA one unit step ahead, in a 2-deep ring
-//     per team, issued by warp 1 of the team (which otherwise only waits for warp 0 at that point);
+//     steps interleaved, so a team hands the tensor core two K slices per unit step; the operand columns are double
+//     buffered, so a decoder warp never waits for the tensor core in steady state;
+//   * one ISSUER warp per team (the paper's consumer warps, P:l.226-247): it sleeps on the team's "operand stored"
+//     mbarrier, issues the two tcgen05.mma of the unit step (A from TMEM, X slice from shared memory, accumulator in
+//     TMEM), commits them to the barrier that frees the operand columns ("ready[2]" flags of P:l.210 -> mbarriers), and
+//     requests the X slices (pad16(m) rows x 32 bytes, SWIZZLE_32B) of the unit step two ahead by TMA into a 3-deep ring;
 //   * nothing in the decode loop waits for HBM: the bf16 sign/mantissa bytes of the NEXT unit travel by cp.async into a
 //     shared-memory double buffer (a register-destination global load shares scoreboards with the loop's LDS and
 //     stalled every unit for an HBM round trip);
 //   * the team reads its own accumulator back (tcgen05.ld: warp q -> lanes 32q..) at the end of a stripe segment;
-//   * split-K: a team is a "virtual CTA" of the stream-K split.  Every contributor of a stripe stores its partial,
-//     raises a flag, waits for the other contributors' flags and then reduces ITS OWN slice of the stripe's outputs,
-//     summing the contributors in team order (bit-reproducible; the reduction is spread over all contributors
-//     instead of falling on one of them).
-// TMEM budget: T teams x (pad16(m) accumulator columns + 16 operand columns) <= 512  ->  T = 5 up to m = 80.
+//   * split-K: a team is a "virtual CTA" of a two-level stream-K split (pairs evenly over the CTAs, then over a CTA's
+//     teams).  Every contributor of a stripe stores its partial, raises a flag, waits for the other contributors' flags
+//     and then reduces ITS OWN slice of the stripe's outputs, summing the contributors in team order (bit-reproducible;
+//     the reduction is spread over all contributors instead of falling on one of them).
+// TMEM budget: T teams x (pad16(m) accumulator columns + 32 operand columns) <= 512  ->  T = 4 up to m = 96.
 #pragma once
 
 constexpr int kTeamWarps = 4;

@@ -1,16 +1,17 @@
-// libanslin device side (sm_100a): decode-only kernel, fused rANS-decode + tcgen05 GEMM kernel,
-// dense tcgen05 comparator, and their C-ABI launchers.
+// libanslin device side (sm_100a): decode-only kernel, the two fused rANS-decode + tcgen05 GEMM kernels, the dense
+// tcgen05 comparator, and their C-ABI launchers.
 //
-// Fused kernel = Alg V.1 (P:l.196-252) re-designed for Blackwell (DESIGN.md §"Kernels"):
-//   * the paper's single producer warp becomes up to 24 decoder warps per CTA (decode is the
-//     bottleneck at small batch, P:l.306), each running Alg V.2 on its own tile;
-//   * the paper's consumer warps become ONE thread issuing tcgen05.mma with the accumulator in
-//     TMEM; the weights are the MMA "A" operand (M = 128 weight rows), the batch is MMA N;
-//   * ready[2] flags (P:l.210) become mbarrier full/empty pairs over a ring of 4 KiB operand
-//     units (128 rows x 32 B = one MMA K step), so a decoder warp hands the tensor core a K slice
-//     every 64 (bf16) decode steps instead of a whole tile ("ring buffer lets decode run several
-//     sub-tiles ahead", P:l.297);
-//   * activations arrive by TMA (cp.async.bulk.tensor) into the same ring slot.
+// Fused kernel = Alg V.1 (P:l.196-252) re-designed for Blackwell:
+//   * fused_tmem_kernel (fused_tmem.cuh): lane-stream containers with 32-row tiles.  Teams of four decoder warps hand the
+//     decoded operand to the tensor core through TENSOR MEMORY (tcgen05.st -> tcgen05.mma with A in TMEM); one issuer warp
+//     per team issues the MMAs and the TMA loads of the X slices; stream-K split over teams.  The path bench.py times.
+//   * fused_gemm_kernel (below): every other container layout, batches above 96 rows, and launches of few, long tile pairs.
+//     The paper's single producer warp becomes up to 16 decoder warps per CTA (decode is the bottleneck at small batch,
+//     P:l.306), the consumer warps become ONE thread issuing tcgen05.mma with the accumulator in TMEM; ready[2] flags
+//     (P:l.210) become mbarrier full/empty pairs over private slots of 4 KiB operand units (128 rows x 32 B = one MMA K
+//     step) in shared memory ("ring buffer lets decode run several sub-tiles ahead", P:l.297); activations arrive by
+//     TMA (cp.async.bulk.tensor) into the same slot.
+//   In both, the weights are the MMA "A" operand (M = 128 weight rows) and the batch is MMA N.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_fp16.h>

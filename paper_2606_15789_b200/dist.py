@@ -1,5 +1,5 @@
 """Multi-GPU plumbing for bench.py: the path shards by independent batches (one replica of the layer and one
-batch per GPU, weak scaling, NO data-path collective — DESIGN.md §10).  torch.distributed is used only for the
+batch per GPU, weak scaling, NO data-path collective — DESIGN.md §10 "Multi-GPU").  torch.distributed is used only for the
 timing contract: a barrier on both sides of the timed region and the MAX over ranks of the measured time."""
 from __future__ import annotations
 
