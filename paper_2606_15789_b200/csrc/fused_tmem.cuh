@@ -105,21 +105,21 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 
-// One operand unit (32 operand bytes per row = 8 registers) of the warp's two tiles.  rv[j]: bf16: the unit's 16 raw
-// (sign | mantissa) bytes of this lane.  sz[j]: int4: this lane's (scale, zero) pair of the unit's quantisation group.
-template <uint32_t FMT, bool PAYLOAD>
-__device__ __forceinline__ void decode_unit_regs(LaneStream (&s)[2], uint32_t tab_s, uint32_t dir, bool last_unit, const uint4 (&rv)[2],
+// Half H (0 / 1) of one operand unit (32 operand bytes per row = 8 registers) of the warp's two tiles: registers
+// r[j][4H .. 4H+3].  rv[j]: bf16: the unit's 16 raw (sign | mantissa) bytes of this lane.  sz[j]: int4: this lane's (scale, zero)
+// pair of the unit's quantisation group.  The unit is cut in two so that its housekeeping (hand-over of the previous unit,
+// the next unit's raw bytes, the operand-free probe) sits between the halves, where its latencies overlap decode steps.
+template <uint32_t FMT, bool PAYLOAD, int H>
+__device__ __forceinline__ void decode_half_regs(LaneStream (&s)[2], uint32_t tab_s, uint32_t dir, bool last_unit, const uint4 (&rv)[2],
                                                  const uint32_t (&sz)[2], uint32_t (&r)[2][8]) {
   static_assert(FMT != ANSLIN_FMT_BF16_PAIR4, "the pair variant runs on the shared-memory operand path");
   if constexpr (FMT == ANSLIN_FMT_BF16) {
-    uint32_t R0[2] = {rv[0].x, rv[1].x}, R1[2] = {rv[0].y, rv[1].y};
+    uint32_t R0[2], R1[2];
+    if (H == 0) { R0[0] = rv[0].x; R0[1] = rv[1].x; R1[0] = rv[0].y; R1[1] = rv[1].y; }
+    else { R0[0] = rv[0].z; R0[1] = rv[1].z; R1[0] = rv[0].w; R1[1] = rv[1].w; }
     uint4 o[2];
     decode8_bf16<LaneWords, 2>(s, tab_s, dir, R0, R1, o);
-#pragma unroll
-    for (int j = 0; j < 2; ++j) { r[j][0] = o[j].x; r[j][1] = o[j].y; r[j][2] = o[j].z; r[j][3] = o[j].w; }
-    R0[0] = rv[0].z; R0[1] = rv[1].z; R1[0] = rv[0].w; R1[1] = rv[1].w;
-    decode8_bf16<LaneWords, 2>(s, tab_s, dir, R0, R1, o);
-    if (PAYLOAD && last_unit) {
+    if (H == 1 && PAYLOAD && last_unit) {
       // raw bytes 14, 15 of the tile's last vector ride in the END state (A4): merge them in now
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
@@ -128,37 +128,33 @@ __device__ __forceinline__ void decode_unit_regs(LaneStream (&s)[2], uint32_t ta
       }
     }
 #pragma unroll
-    for (int j = 0; j < 2; ++j) { r[j][4] = o[j].x; r[j][5] = o[j].y; r[j][6] = o[j].z; r[j][7] = o[j].w; }
+    for (int j = 0; j < 2; ++j) { r[j][4 * H] = o[j].x; r[j][4 * H + 1] = o[j].y; r[j][4 * H + 2] = o[j].z; r[j][4 * H + 3] = o[j].w; }
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
-    uint32_t B0[2], B1[2];
-    decode4<LaneWords, 2>(s, B0, tab_s, dir);
-    decode4<LaneWords, 2>(s, B1, tab_s, dir);
+    uint32_t Bq[2];
+    decode4<LaneWords, 2>(s, Bq, tab_s, dir);
 #pragma unroll
     for (int j = 0; j < 2; ++j) {
       const __half2 szh = *reinterpret_cast<const __half2 *>(&sz[j]);
       const __half2 sc = __half2half2(__low2half(szh));
       const __half2 zoff = __hadd2(__half2half2(__high2half(szh)), __float2half2_rn(1024.f));
 #pragma unroll
-      for (int b = 0; b < 4; ++b) {
-        r[j][b] = awq_dequant2((B0[j] >> (8 * b)) & 0xFFu, zoff, sc);
-        r[j][4 + b] = awq_dequant2((B1[j] >> (8 * b)) & 0xFFu, zoff, sc);
-      }
+      for (int b = 0; b < 4; ++b) r[j][4 * H + b] = awq_dequant2((Bq[j] >> (8 * b)) & 0xFFu, zoff, sc);
     }
   } else if constexpr (FMT == ANSLIN_FMT_FP4_E2M1) {
 #pragma unroll
-    for (int h = 0; h < 4; ++h) {
+    for (int h = 0; h < 2; ++h) {
       uint32_t Bq[2];
       decode4<LaneWords, 2>(s, Bq, tab_s, dir);
 #pragma unroll
-      for (int j = 0; j < 2; ++j) e2m1x8_to_e4m3(Bq[j], r[j][2 * h], r[j][2 * h + 1]);
+      for (int j = 0; j < 2; ++j) e2m1x8_to_e4m3(Bq[j], r[j][4 * H + 2 * h], r[j][4 * H + 2 * h + 1]);
     }
   } else {   // fp8 / int8: the symbol byte is the operand byte
 #pragma unroll
-    for (int h = 0; h < 8; ++h) {
+    for (int h = 0; h < 4; ++h) {
       uint32_t q[2];
       decode4<LaneWords, 2>(s, q, tab_s, dir);
-      r[0][h] = q[0];
-      r[1][h] = q[1];
+      r[0][4 * H + h] = q[0];
+      r[1][4 * H + h] = q[1];
     }
   }
 }
@@ -457,6 +453,19 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   } else {
   uint32_t n = 0, seg_i = 0;
   bool dep_waited = false;
+  // hand-over of a unit step, second part: wait for the warp's tensor-memory stores, then the arrival that (as the fourth of
+  // the team) lets the issuer warp multiply the step.  Deferred to the middle of the next unit so that the store latency
+  // overlaps decode steps; completed before anything waits for the step's MMAs (the segment's epilogue).
+  uint32_t pending_full = 0;
+  auto finish_handover = [&]() {
+    if (pending_full) {
+      tmem_wait_st();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(pending_full);
+      pending_full = 0;
+    }
+  };
 #ifdef ANSLIN_STAGGER_NS
   __nanosleep(team * ANSLIN_STAGGER_NS);   // teams out of phase: one team's hand-over overlaps the others' decoding
 #endif
@@ -570,11 +579,15 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
 #ifdef ANSLIN_SKEL_NO_DECODE   // timing experiment only (wrong results): everything but the rANS steps
 #pragma unroll
         for (int k = 0; k < 8; ++k) { r[0][k] = rv[0].x + k; r[1][k] = rv[1].y ^ k; }
+        finish_handover();
 #else
-        decode_unit_regs<FMT, PAYLOAD>(s, tab_s, dir, last_unit, rv, sz, r);
+        decode_half_regs<FMT, PAYLOAD, 0>(s, tab_s, dir, last_unit, rv, sz, r);
+        // the PREVIOUS unit's tensor-memory stores have had half a unit to land: publish them now, between the halves
+        finish_handover();
+        decode_half_regs<FMT, PAYLOAD, 1>(s, tab_s, dir, last_unit, rv, sz, r);
 #endif
         PROF(1);
-        // ---- hand-over: registers -> tensor memory -> tcgen05.mma ----
+        // ---- hand-over: registers -> tensor memory (-> tcgen05.mma once the stores are published) ----
         if (!slot_free) mbar_wait(done_s + 8 * sa, ((n - 2) >> 1) & 1u);
         PROF(2);
 #ifdef ANSLIN_SKEL_NO_STTM   // timing experiment only (wrong results): how much do the tensor-memory stores cost
@@ -582,13 +595,10 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
 #endif
         tmem_st8(a_t + sa * 2u * kACols + lane_t, r[0]);
         tmem_st8(a_t + sa * 2u * kACols + kACols + lane_t, r[1]);
-        tmem_wait_st();
 #ifdef ANSLIN_SKEL_NO_STTM
         }
 #endif
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(full_s + 8 * sa);   // the fourth arrival lets the team's issuer warp multiply this unit step
+        pending_full = full_s + 8 * sa;
         PROF(3);
       }
 #ifdef ANSLIN_BOUNDS_CHECK   // debug builds (compute-sanitizer is closed on this pool): every word cursor ended inside its staged buffer
@@ -601,6 +611,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
 #endif
     }
+    finish_handover();
     PROF(0);
     // ---- epilogue of this stripe segment: the team reads its own accumulator ----
     TRACE(2);
