@@ -645,12 +645,11 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
       tc_fence_before();   // the next segment's first MMA (after the next team barrier) overwrites the accumulator
       if (!whole) {
-        // the team's partial stores are ordered before the barrier; the one thread that raises the flag then fences at
-        // GPU scope (cumulative over what the barrier made visible to it), as a grid-wide barrier would
+        // the team's partial stores are ordered before the barrier; the release store of the one thread that raises the flag
+        // is cumulative over what the barrier made visible to it (no separate fence: st.release.gpu carries it)
         named_bar_sync(bar_id, kNT);
         if (q == 0 && lane == 0) {
           uint32_t *flag = reinterpret_cast<uint32_t *>(ep.counters) + (v * 2u + seg);
-          __threadfence();
           asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(ep.epoch) : "memory");
         }
         if (seg == 0) { fin_stripe[0] = stripe; fin_valid[0] = true; }
