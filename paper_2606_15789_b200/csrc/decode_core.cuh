@@ -82,7 +82,7 @@ __device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, c
   __syncthreads();
   for (int s = warp; s < 256; s += nwarp) {
     const uint32_t c0 = cum[s], f = cum[s + 1] - c0;
-    for (uint32_t k = lane; k < f; k += 32) tab[c0 + k] = uint32_t(s) | (f << 8) | (k << 20);
+    for (uint32_t k = lane; k < f; k += 32) tab[c0 + k] = uint32_t(s) | (k << 8) | (f << 20);
   }
   __syncthreads();
 }
@@ -149,13 +149,19 @@ __device__ __forceinline__ void stream_upkeep8(Stream (&s)[J], uint32_t ring0, i
   __syncwarp();
 }
 
+// x' = f * (x >> b) + (slot - c) (Alg V.2 l.7, P:l.276) from the table entry e = sym | (slot - c) << 8 | f << 20.  Two shifts
+// and no mask: e >> 8 = f << 12 | (slot - c) carries f * 2^12 too much, which the multiplicand (x >> 12) - 2^12 takes back
+// (all modulo 2^32; the result is < 2^32 as in the plain form).
+__device__ __forceinline__ uint32_t state_update(uint32_t x, uint32_t e) {
+  return (e >> 20) * ((x >> kProbBits) - (1u << kProbBits)) + (e >> 8);
+}
 // One decode step of Alg V.2 for all 32 lanes of one stream; returns the table entry (symbol in bits 7:0).
 __device__ __forceinline__ uint32_t decode_step(Stream &s, uint32_t tab_s, uint32_t lt) {
   uint32_t ea, e;
   asm("mul.lo.u32 %0, %1, 4;" : "=r"(ea) : "r"(s.x));          // shift on the FMA pipe (IMAD.SHL), mask on the ALU,
   asm("and.b32 %0, %0, 0x3FFC;" : "+r"(ea));                   // table base folded into the load's address operand
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea + tab_s));
-  uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
+  uint32_t xn = state_update(s.x, e);
   // renormalisation: the lanes with x < 2^16 read consecutive words, x = (x << 16) | word
   asm volatile(
       "{\n\t.reg .pred p;\n\t.reg .u16 h;\n\t.reg .u32 w, m, r, a;\n\t"
@@ -257,7 +263,7 @@ __device__ __forceinline__ uint32_t lane_step(LaneStream &s, uint32_t tab_s, uin
   asm("mul.lo.u32 %0, %1, 4;" : "=r"(ea) : "r"(s.x));          // shift on the FMA pipe (IMAD.SHL), mask on the ALU,
   asm("and.b32 %0, %0, 0x3FFC;" : "+r"(ea));                   // table base folded into the load's address operand
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e) : "r"(ea + tab_s));
-  uint32_t xn = ((e >> 8) & 0xFFFu) * (s.x >> kProbBits) + (e >> 20);
+  uint32_t xn = state_update(s.x, e);
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
       "setp.lt.u32 p, %0, 65536;\n\t"
@@ -282,8 +288,8 @@ __device__ __forceinline__ void lane_step2(LaneStream &s0, LaneStream &s1, uint3
   asm("and.b32 %0, %0, 0x3FFC;" : "+r"(a1));
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e0) : "r"(a0 + tab_s));
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e1) : "r"(a1 + tab_s));
-  uint32_t x0 = ((e0 >> 8) & 0xFFFu) * (s0.x >> kProbBits) + (e0 >> 20);
-  uint32_t x1 = ((e1 >> 8) & 0xFFFu) * (s1.x >> kProbBits) + (e1 >> 20);
+  uint32_t x0 = state_update(s0.x, e0);
+  uint32_t x1 = state_update(s1.x, e1);
   asm volatile(
       "{\n\t.reg .pred p, q;\n\t"
       "setp.lt.u32 p, %0, 65536;\n\t"
