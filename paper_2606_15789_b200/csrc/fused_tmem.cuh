@@ -384,6 +384,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   const uint32_t acc_t = tmem_base + team * P.tmem_stride, a_t = acc_t + mpad;   // accumulator, then two operand units
   const uint32_t lane_t = (q * 32u) << 16;
   const uint32_t rawbuf_s = smem0 + raw_off + uint32_t(warp) * 2u * kRawBufBytes;  // chain j, vector parity b at j * 1024 + b * 512
+  const uint32_t rawlane_s = rawbuf_s + 16u * uint32_t(lane);                        // ... this lane's 16 bytes of it
   const uint32_t stage_s = smem0 + stage_off + uint32_t(warp) * 2u * P.stream_bytes, tab_s = smem0;
   const uint32_t dir = (lane & 1) ? uint32_t(-2) : 2u;
   const int bar_id = 1 + int(team);
@@ -451,19 +452,28 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
     }
   } else {
-  uint32_t n = 0, seg_i = 0;
+  uint32_t seg_i = 0;
+#ifdef ANSLIN_TRACE
+  uint32_t n = 0;
+#endif
   bool dep_waited = false;
+#ifdef ANSLIN_SKEL_NO_RAW   // timing experiment only (wrong results): how much does the raw-byte path cost
+  constexpr bool kRawOn = false;
+#else
+  constexpr bool kRawOn = kRaw;
+#endif
   // hand-over of a unit step, second part: wait for the warp's tensor-memory stores, then the arrival that (as the fourth of
   // the team) lets the issuer warp multiply the step.  Deferred to the middle of the next unit so that the store latency
   // overlaps decode steps; completed before anything waits for the step's MMAs (the segment's epilogue).
-  uint32_t pending_full = 0;
-  auto finish_handover = [&]() {
-    if (pending_full) {
+  bool pending = false;       // a unit's stores are not yet published
+  uint32_t kpar = 0;          // parity of (unit step / 2): the phase of the operand-free barriers
+  auto finish_handover = [&](uint32_t full_bar) {
+    if (pending) {
       tmem_wait_st();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(pending_full);
-      pending_full = 0;
+      if (lane == 0) mbar_arrive(full_bar);
+      pending = false;
     }
   };
 #ifdef ANSLIN_STAGGER_NS
@@ -499,42 +509,48 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         next_off[0] = offs[next_tile];
         next_off[1] = offs[next_tile + (kn + 1 < KT ? 4u : 0u)];
       }
-#pragma unroll 1
-      for (uint32_t u = 0; u < units; ++u, ++n) {
-        if (u == 1 && has_next) {
+      // One unit of both tiles.  A tile has an even number of units (tmem_eligible), so the parity PAR of a unit step — which
+      // half of the operand columns, which raw buffer, which barriers — is a compile-time constant of each copy of the body.
+      auto unit_body = [&](auto par_c, const uint32_t u) {
+        constexpr uint32_t PAR = decltype(par_c)::value;
+        if constexpr (PAR == 1) {
+          if (u == 1 && has_next) {
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
-            if (lane < 24) prefetch_l2(cbase + off_records + size_t(next_off[j]) * 16 + lane * 128);
-            else if (kRaw) prefetch_l2(cbase + off_raw + size_t(next_tile + 4u * uint32_t(j)) * rtb + (lane - 24) * 128);
-            cur_off[j] = next_off[j];   // the next pair opens without another look at the offset table
+            for (int j = 0; j < 2; ++j) {
+              if (lane < 24) prefetch_l2(cbase + off_records + size_t(next_off[j]) * 16 + lane * 128);
+              else if (kRaw) prefetch_l2(cbase + off_raw + size_t(next_tile + 4u * uint32_t(j)) * rtb + (lane - 24) * 128);
+              cur_off[j] = next_off[j];   // the next pair opens without another look at the offset table
+            }
+          }
+        } else {
+          if (u == 0) PROF(6);
+          if (u % kUnitsPerSeg == 0) {
+            // stage the segment (drains cp.async first and last); at the tile's start its first raw vector rides in the same group
+            if (kRawOn && u == 0) {
+              lane_open_segments<2>(s, stage_s, P.stream_bytes, 0, lane, [&]() {
+#pragma unroll
+                for (int j = 0; j < 2; ++j) { cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes, rawp[j]); rawp[j] += 512; }
+              });
+            } else {
+              lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);
+            }
+          }
+          if (u == 0) PROF(4);
+          if (!dep_waited) {   // everything before this point read the container only
+            grid_dep_wait();
+            dep_waited = true;
           }
         }
-        if (u % kUnitsPerSeg == 0) {
-          // stage the segment (drains cp.async first and last); at the tile's start its first raw vector rides in the same group
-          if (kRaw && u == 0) {
-            lane_open_segments<2>(s, stage_s, P.stream_bytes, 0, lane, [&]() {
-#pragma unroll
-              for (int j = 0; j < 2; ++j) { cp_async16(rawbuf_s + uint32_t(j) * kRawBufBytes + 16u * uint32_t(lane), rawp[j]); rawp[j] += 512; }
-            });
-          } else {
-            lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);
-          }
-        }
-        if (u == 0) PROF(4);
-        if (!dep_waited) {   // everything before this point read the container only
-          grid_dep_wait();
-          dep_waited = true;
-        }
-        const bool last_unit = u + 1 == units;
+        const bool last_unit = PAR == 1 && u + 1 == units;
         uint4 rv[2] = {make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0)};
         uint32_t sz[2] = {0, 0};
-#ifdef ANSLIN_SKEL_NO_RAW   // timing experiment only (wrong results): how much does the raw-byte path cost
-        if (false)
-#endif
-        if constexpr (kRaw) {
-          // this unit's raw vector was copied during the previous unit; fetch the next one into the other half
+        if constexpr (kRawOn) {
+          // this unit's raw vector was copied during the previous unit; fetch the next one into the other buffer.
+          // rawp[j]: at an even unit the next vector, at an odd unit the one before it (advanced by two vectors at a time)
+          PROF(0);
           cp_async_wait_all();
-          const uint32_t rb = rawbuf_s + (u & 1u) * 512u;
+          PROF(7);
+          const uint32_t rb = rawlane_s + PAR * 512u;
           if (PAYLOAD && last_unit) {
             // last vector with the state-payload flag: 7 sub-rows of 32 x 2 bytes (bytes 14, 15 come from the end state)
             __syncwarp();
@@ -542,23 +558,23 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
             for (int j = 0; j < 2; ++j) {
               uint32_t h[7];
 #pragma unroll
-              for (int k = 0; k < 7; ++k) h[k] = lds16(rb + uint32_t(j) * kRawBufBytes + uint32_t(k) * 64u + 2u * uint32_t(lane));
+              for (int k = 0; k < 7; ++k)
+                h[k] = lds16(rawbuf_s + 512u + uint32_t(j) * kRawBufBytes + uint32_t(k) * 64u + 2u * uint32_t(lane));
               rv[j] = make_uint4(h[0] | (h[1] << 16), h[2] | (h[3] << 16), h[4] | (h[5] << 16), h[6]);
             }
           } else {
 #pragma unroll
-            for (int j = 0; j < 2; ++j) rv[j] = lds128(rb + uint32_t(j) * kRawBufBytes + 16u * uint32_t(lane));
+            for (int j = 0; j < 2; ++j) rv[j] = lds128(rb + uint32_t(j) * kRawBufBytes);
           }
           if (!last_unit) {
-            const bool short_vec = PAYLOAD && u + 2 == units;   // the next vector is the payload-shortened one: 448 bytes
+            const bool short_vec = PAYLOAD && PAR == 0 && u + 2 == units;   // the next vector is the payload-shortened one: 448 bytes
             if (!short_vec || lane < 28) {
 #pragma unroll
-              for (int j = 0; j < 2; ++j) cp_async16(rawbuf_s + uint32_t(j) * kRawBufBytes + ((u + 1) & 1u) * 512u + 16u * uint32_t(lane), rawp[j]);
+              for (int j = 0; j < 2; ++j) cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes + (PAR ^ 1u) * 512u, rawp[j] + PAR * 512u);
             }
-#pragma unroll
-            for (int j = 0; j < 2; ++j) rawp[j] += 512;
             cp_async_commit();
           }
+          if constexpr (PAR == 1) { rawp[0] += 1024; rawp[1] += 1024; }
         }
         if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll
@@ -568,38 +584,47 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
                           q * 32u + uint32_t(lane));
           }
         }
-        const uint32_t sa = n & 1u;
-        // have the MMAs of step n-2 read this half of the operand columns?  Asked now, needed after the unit is decoded
-        const bool slot_free = n < 2 || mbar_test(done_s + 8 * sa, ((n - 2) >> 1) & 1u);
+        // have the MMAs that read this half of the operand columns two steps ago finished?  (On fresh barriers the parity
+        // of the "previous" phase passes at once.)  Asked now, needed after the unit is decoded.
+        const bool slot_free = mbar_test(done_s + 8 * PAR, kpar ^ 1u);
         uint32_t r[2][8];
 #ifdef ANSLIN_TRACE
-        if (blockIdx.x == 7 && lane == 0 && n < 48) g_prof[160 * kMaxTeams * 4 * 8 - 4 * 4 * 48 + ((team * 4 + q) * 48 + n)] = gtimer();
+        if (blockIdx.x == 7 && lane == 0 && n + PAR < 48) g_prof[160 * kMaxTeams * 4 * 8 - 4 * 4 * 48 + ((team * 4 + q) * 48 + n + PAR)] = gtimer();
 #endif
         PROF(0);
 #ifdef ANSLIN_SKEL_NO_DECODE   // timing experiment only (wrong results): everything but the rANS steps
 #pragma unroll
         for (int k = 0; k < 8; ++k) { r[0][k] = rv[0].x + k; r[1][k] = rv[1].y ^ k; }
-        finish_handover();
+        finish_handover(full_s + 8 * (PAR ^ 1u));
 #else
         decode_half_regs<FMT, PAYLOAD, 0>(s, tab_s, dir, last_unit, rv, sz, r);
         // the PREVIOUS unit's tensor-memory stores have had half a unit to land: publish them now, between the halves
-        finish_handover();
+        finish_handover(full_s + 8 * (PAR ^ 1u));
         decode_half_regs<FMT, PAYLOAD, 1>(s, tab_s, dir, last_unit, rv, sz, r);
 #endif
         PROF(1);
         // ---- hand-over: registers -> tensor memory (-> tcgen05.mma once the stores are published) ----
-        if (!slot_free) mbar_wait(done_s + 8 * sa, ((n - 2) >> 1) & 1u);
+        if (!slot_free) mbar_wait(done_s + 8 * PAR, kpar ^ 1u);
         PROF(2);
 #ifdef ANSLIN_SKEL_NO_STTM   // timing experiment only (wrong results): how much do the tensor-memory stores cost
         if (r[0][0] == 0x12345678u && r[1][7] == 0x9abcdef0u && r[0][3] == 1u && r[1][2] == 7u) {
 #endif
-        tmem_st8(a_t + sa * 2u * kACols + lane_t, r[0]);
-        tmem_st8(a_t + sa * 2u * kACols + kACols + lane_t, r[1]);
+        tmem_st8(a_t + PAR * 2u * kACols + lane_t, r[0]);
+        tmem_st8(a_t + PAR * 2u * kACols + kACols + lane_t, r[1]);
 #ifdef ANSLIN_SKEL_NO_STTM
         }
 #endif
-        pending_full = full_s + 8 * sa;
+        pending = true;
         PROF(3);
+      };
+#pragma unroll 1
+      for (uint32_t u = 0; u < units; u += 2) {
+        unit_body(std::integral_constant<uint32_t, 0>{}, u);
+        unit_body(std::integral_constant<uint32_t, 1>{}, u + 1);
+        kpar ^= 1u;
+#ifdef ANSLIN_TRACE
+        n += 2;
+#endif
       }
 #ifdef ANSLIN_BOUNDS_CHECK   // debug builds (compute-sanitizer is closed on this pool): every word cursor ended inside its staged buffer
 #pragma unroll
@@ -611,7 +636,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
 #endif
     }
-    finish_handover();
+    finish_handover(full_s + 8);   // a tile ends with an odd unit
     PROF(0);
     // ---- epilogue of this stripe segment: the team reads its own accumulator ----
     TRACE(2);

@@ -985,7 +985,8 @@ uint32_t tmem_teams(uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
   return T;
 }
 bool tmem_eligible(const Header &h) {
-  return (h.flags & ANSLIN_FLAG_LANE_STREAMS) && h.tile_n == 32 && h.format != ANSLIN_FMT_BF16_PAIR4 && h.tile_k / unit_k_of(h.format) >= 2 &&
+  return (h.flags & ANSLIN_FLAG_LANE_STREAMS) && h.tile_n == 32 && h.format != ANSLIN_FMT_BF16_PAIR4 && h.tile_k / unit_k_of(h.format) >= 2 && (h.tile_k / unit_k_of(h.format)) % 2 == 0 &&   // units come in pairs
+        
          uint64_t(h.n_out / kTileN) * ((h.k_in / h.tile_k + 1) / 2) < (1u << 22);   // 32-bit split arithmetic in TeamMap
 }
 
