@@ -42,8 +42,8 @@ __host__ __device__ constexpr size_t tmem_smem_bytes(uint32_t T, uint32_t mpad_m
   return 1024 /*align slack*/ + kTmXOff + size_t(T) * kXDepth * 2 * mpad_max * 32 + (tmem_has_raw(fmt) ? size_t(T) * kTeamWarps * 2 * kRawBufBytes : 0) +
          size_t(T) * kTeamWarps * 2 * stream_bytes + 16;
 }
-// split-K control words of a problem (inside its flag area): u32 flag[2 * teams] | u32 stripe_count[stripes]
-constexpr size_t kTmStripeCntOff = 8 * 160 * kMaxTeams + 256;
+// split-K control words of a problem (its flag area): u32 flag[2 * teams][PK], one word per (partial slot, reader)
+constexpr size_t kTmFlagSlots = 2 * 160 * kMaxTeams;
 
 struct TmemParams {
   Problem prob[kMaxProblems];
@@ -199,21 +199,43 @@ struct TeamMap {
 // partial of.  The contributors of a stripe are the distinct owners of its PK pairs, in pair order; contributor vv's partial
 // slot is its first segment (slot 0) unless the stripe is its second one, which can only be the case for the stripe's first
 // contributor.  Every contributor sums ITS slice of the stripe's outputs over all contributors, in that order.
-// scratch: team-private shared memory, 2 * (PK + 1) words.
+// Flags: a partial slot has one flag word PER READER (flags[slot * PK + reader's index among the contributors]); its writer
+// sets them all to the launch epoch, every reader clears its own as soon as it has seen it, so that a replay of this very
+// launch (CUDA graph: same epoch) starts from "nothing stored" without any reader counting or atomics.
+// scratch: team-private shared memory, 2 * PK words.
 template <uint32_t FMT, bool YB>
 __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &tm, uint32_t PK, int ns, const uint32_t (&stripes)[2], uint32_t v,
                                             uint32_t tid, int bar, uint32_t *scratch) {
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   uint32_t *flags = reinterpret_cast<uint32_t *>(p.counters);
-  // 1. the partial slot of every pair's owner (one pair per thread), then wait for that partial's flag
+  // 1. the partial slot of every pair's owner (one pair per thread)
   for (int sg = 0; sg < ns; ++sg) {
-    uint32_t *list = scratch + sg * (PK + 1);
+    uint32_t *list = scratch + sg * PK;
     const uint32_t p0 = stripes[sg] * PK;
     for (uint32_t k = tid; k < PK; k += kNT) {
       const uint32_t vv = tm.owner(p0 + k), v_first = tm.owner(p0);
-      const uint32_t slot = vv * 2u + ((vv == v_first && tm.first(v_first) < p0) ? 1u : 0u);
-      list[k] = slot;
-      const uint32_t *flag = flags + slot;
+      list[k] = vv * 2u + ((vv == v_first && tm.first(v_first) < p0) ? 1u : 0u);
+    }
+  }
+  named_bar_sync(bar, kNT);
+  // 2. how many contributors, and which one am I (consecutive pairs of one owner share a slot)
+  uint32_t counts[2] = {1, 1}, mine[2] = {0, 0};
+  for (int sg = 0; sg < ns; ++sg) {
+    const uint32_t *list = scratch + sg * PK;
+    uint32_t count = 0, my_index = 0;
+    for (uint32_t k = 0, prev = 0xFFFFFFFFu; k < PK; ++k) {
+      const uint32_t sl = list[k];
+      if (sl != prev) { if ((sl >> 1) == v) my_index = count; ++count; prev = sl; }
+    }
+    counts[sg] = count;
+    mine[sg] = my_index;
+  }
+  // 3. wait for every contributor's flag addressed to me, and take it down
+  for (int sg = 0; sg < ns; ++sg) {
+    const uint32_t *list = scratch + sg * PK;
+    for (uint32_t k = tid; k < PK; k += kNT) {
+      if (k > 0 && list[k] == list[k - 1]) continue;
+      uint32_t *flag = flags + size_t(list[k]) * PK + mine[sg];
       uint32_t val, spins = 0;
       while (true) {
         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(val) : "l"(flag) : "memory");
@@ -221,24 +243,17 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
         __nanosleep(100);
         if (++spins > (1u << 24)) __trap();   // a protocol bug traps instead of hanging the GPU
       }
+      *reinterpret_cast<volatile uint32_t *>(flag) = 0u;
     }
   }
   RTRACE(5);
   named_bar_sync(bar, kNT);
   const size_t slot_words = size_t(p.mpad) * kTileN;
   const uint32_t n_items = p.m * 32u;   // one item = one batch row x 4 output channels
-  uint32_t counts[2] = {0, 0};
   for (int sg = 0; sg < ns; ++sg) {
-    const uint32_t *list = scratch + sg * (PK + 1);
-    // 2. how many contributors, and which one am I (consecutive pairs of one owner share a slot)
-    uint32_t count = 0, my_index = 0;
-    for (uint32_t k = 0, prev = 0xFFFFFFFFu; k < PK; ++k) {
-      const uint32_t sl = list[k];
-      if (sl != prev) { if ((sl >> 1) == v) my_index = count; ++count; prev = sl; }
-    }
-    counts[sg] = count;
-    // 3. my slice of the stripe's items
-    const uint32_t it_begin = my_index * n_items / count, it_end = (my_index + 1) * n_items / count;
+    const uint32_t *list = scratch + sg * PK;
+    // 4. my slice of the stripe's items
+    const uint32_t it_begin = mine[sg] * n_items / counts[sg], it_end = (mine[sg] + 1) * n_items / counts[sg];
     for (uint32_t it = it_begin + tid; it < it_end; it += kNT) {
       const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u;
       const uint32_t *src = p.partials + size_t(mm) * kTileN + r4;
@@ -291,28 +306,6 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
     }
   }
   RTRACE(6);
-  // 4. The last contributor to finish reading a stripe clears its flags and its counter, so that a replay of this very
-  // launch (CUDA graph: same epoch) starts from "nothing stored".  Counter word = epoch tag << 8 | readers done; any other
-  // tag (stale or never written bytes) reads as zero readers.
-  named_bar_sync(bar, kNT);
-  if (tid < uint32_t(ns)) {
-    uint32_t *cnt = reinterpret_cast<uint32_t *>(reinterpret_cast<uint8_t *>(p.counters) + kTmStripeCntOff) + stripes[tid];
-    const uint32_t tag = (p.epoch << 8), count = tid == 0 ? counts[0] : counts[1];
-    uint32_t old = *reinterpret_cast<volatile uint32_t *>(cnt), done;
-    while (true) {
-      done = ((old & 0xFFFFFF00u) == tag ? (old & 0xFFu) : 0u) + 1u;
-      const uint32_t seen = atomicCAS(cnt, old, done == count ? 0u : (tag | done));
-      if (seen == old) break;
-      old = seen;
-    }
-    scratch[tid * (PK + 1) + PK] = done == count ? 1u : 0u;
-  }
-  named_bar_sync(bar, kNT);
-  for (int sg = 0; sg < ns; ++sg) {
-    const uint32_t *list = scratch + sg * (PK + 1);
-    if (list[PK])
-      for (uint32_t k = tid; k < PK; k += kNT) flags[list[k]] = 0u;
-  }
 }
 
 template <uint32_t FMT, bool PAYLOAD, bool YB>
@@ -670,12 +663,13 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
       tc_fence_before();   // the next segment's first MMA (after the next team barrier) overwrites the accumulator
       if (!whole) {
-        // the team's partial stores are ordered before the barrier; the release store of the one thread that raises the flag
-        // is cumulative over what the barrier made visible to it (no separate fence: st.release.gpu carries it)
+        // the team's partial stores are ordered before the barrier; the release store of a thread that raises a flag is
+        // cumulative over what the barrier made visible to it (no separate fence: st.release.gpu carries it)
         named_bar_sync(bar_id, kNT);
-        if (q == 0 && lane == 0) {
-          uint32_t *flag = reinterpret_cast<uint32_t *>(ep.counters) + (v * 2u + seg);
-          asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(ep.epoch) : "memory");
+        {   // one flag per possible reader of this partial (team_reduce)
+          uint32_t *flag = reinterpret_cast<uint32_t *>(ep.counters) + size_t(v * 2u + seg) * PK;
+          for (uint32_t rdr = q * 32u + uint32_t(lane); rdr < PK; rdr += kNT)
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag + rdr), "r"(ep.epoch) : "memory");
         }
         if (seg == 0) { fin_stripe[0] = stripe; fin_valid[0] = true; }
         else { fin_stripe[1] = stripe; fin_valid[1] = true; }

@@ -934,13 +934,17 @@ uint32_t next_epoch() {
   return v;
 }
 
-// bytes of a problem's split-K flag area (two u32 flags per CTA; sized generously by stripes too so that older callers' sizes hold)
-size_t flag_bytes(uint32_t stripes) { return align16(size_t(stripes) * 8 + 256 + 8 * 160 * kMaxTeams); }
+// bytes of a problem's split-K flag area: the shared-memory design keeps two u32 flags per CTA and a u64 counter per stripe,
+// the tensor-memory design one u32 flag per (partial slot of a team, reader) = kTmFlagSlots x pairs per stripe
+size_t flag_bytes(const Header &h) {
+  const size_t stripes = h.n_out / kTileN, pk = (h.k_in / h.tile_k + 1) / 2;
+  return align16(std::max(stripes * 8 + 256 + 8 * 160 * kMaxTeams, kTmFlagSlots * pk * 4));
+}
 struct Workspace { size_t counters_off, partials_off, total; };
 Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
   Workspace w;
   w.counters_off = 0;
-  w.partials_off = flag_bytes(stripes);
+  w.partials_off = align16(size_t(stripes) * 8 + 256 + 8 * 160 * kMaxTeams);   // the dense comparator's flag area
   w.total = w.partials_off + size_t(grid) * 2 * mpad * kTileN * 4;
   return w;
 }
@@ -1100,7 +1104,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
   size_t off = 0;
   uint8_t *wsb = static_cast<uint8_t *>(workspace_dev);
   size_t counters_bytes = 0;
-  for (int i = 0; i < n; ++i) counters_bytes += flag_bytes(ws[i]->h.n_out / kTileN);
+  for (int i = 0; i < n; ++i) counters_bytes += flag_bytes(ws[i]->h);
   size_t part_off = counters_bytes;
   uint32_t cta0 = 0;
   Problem prob[kMaxProblems];
@@ -1118,7 +1122,7 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     q.ncta = ncta[i];
     cta0 += ncta[i];
     q.counters = reinterpret_cast<unsigned long long *>(wsb + off);
-    off += flag_bytes(h.n_out / kTileN);
+    off += flag_bytes(h);
     q.partials = reinterpret_cast<uint32_t *>(wsb + part_off);
     part_off += size_t(ncta[i]) * teams * 2 * q.mpad * kTileN * 4;
     const uint32_t uk = unit_k_of(h.format);
@@ -1206,7 +1210,7 @@ size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_ma
   bool tmem_ok = true;
   for (int i = 0; i < n; ++i) {
     if (!ws[i]) return 0;
-    counters += flag_bytes(ws[i]->h.n_out / kTileN);
+    counters += flag_bytes(ws[i]->h);
     stream_bytes = std::max<uint32_t>(stream_bytes, uint32_t(align16(ws[i]->h.max_seg_bytes)));
     tmem_ok = tmem_ok && tmem_eligible(ws[i]->h);
   }
