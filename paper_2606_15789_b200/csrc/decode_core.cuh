@@ -62,12 +62,20 @@ __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefe
 // Expand the 256 x u16 frequency table of the container into the 4096-entry slot table in shared
 // memory (Alg V.1 l.6 "Copy global decode table T into shared memory", P:l.212).  All threads of
 // the CTA must call; `cum` is 257 u32 of scratch.  Ends with __syncthreads().
-__device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, const uint16_t *freq_g) {
+// Split in two so that a caller can have the table's HBM round trip in flight under other loads: lane l of warp 0 holds
+// frequencies 8l .. 8l+7 (one 16-byte load).
+__device__ __forceinline__ uint4 slot_table_load(const uint16_t *freq_g) {
+  uint4 fr = make_uint4(0, 0, 0, 0);
+  if (threadIdx.x < 32) fr = *reinterpret_cast<const uint4 *>(freq_g + threadIdx.x * 8);   // off_freq is 16-byte aligned
+  return fr;
+}
+__device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, const uint4 fr) {
   const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarp = nthr >> 5;
   if (warp == 0) {  // exclusive prefix sum of 256 frequencies: 8 per lane + warp scan
+    const uint32_t w[4] = {fr.x, fr.y, fr.z, fr.w};
     uint32_t f[8], s = 0;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) { f[i] = freq_g[lane * 8 + i]; s += f[i]; }
+    for (int i = 0; i < 8; ++i) { f[i] = (w[i >> 1] >> (16 * (i & 1))) & 0xFFFFu; s += f[i]; }
     uint32_t inc = s;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -85,6 +93,9 @@ __device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, c
     for (uint32_t k = lane; k < f; k += 32) tab[c0 + k] = uint32_t(s) | (k << 8) | (f << 20);
   }
   __syncthreads();
+}
+__device__ __forceinline__ void build_slot_table(uint32_t *tab, uint32_t *cum, const uint16_t *freq_g) {
+  build_slot_table(tab, cum, slot_table_load(freq_g));
 }
 
 // One lane's view of one tile's compressed stream.

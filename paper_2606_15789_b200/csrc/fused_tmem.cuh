@@ -202,7 +202,7 @@ struct TeamMap {
 // Flags: a partial slot has one flag word PER READER (flags[slot * PK + reader's index among the contributors]); its writer
 // sets them all to the launch epoch, every reader clears its own as soon as it has seen it, so that a replay of this very
 // launch (CUDA graph: same epoch) starts from "nothing stored" without any reader counting or atomics.
-// scratch: team-private shared memory, 2 * PK words.
+// scratch: team-private shared memory, 4 * PK words.
 template <uint32_t FMT, bool YB>
 __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &tm, uint32_t PK, int ns, const uint32_t (&stripes)[2], uint32_t v,
                                             uint32_t tid, int bar, uint32_t *scratch) {
@@ -218,14 +218,21 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
     }
   }
   named_bar_sync(bar, kNT);
-  // 2. how many contributors, and which one am I (consecutive pairs of one owner share a slot)
+  // 2. how many contributors, and which one am I (consecutive pairs of one owner share a slot); thread 0 leaves the
+  //    list without the repeats behind it
   uint32_t counts[2] = {1, 1}, mine[2] = {0, 0};
   for (int sg = 0; sg < ns; ++sg) {
     const uint32_t *list = scratch + sg * PK;
+    uint32_t *ulist = scratch + (2 + sg) * PK;
     uint32_t count = 0, my_index = 0;
     for (uint32_t k = 0, prev = 0xFFFFFFFFu; k < PK; ++k) {
       const uint32_t sl = list[k];
-      if (sl != prev) { if ((sl >> 1) == v) my_index = count; ++count; prev = sl; }
+      if (sl != prev) {
+        if ((sl >> 1) == v) my_index = count;
+        if (tid == 0) ulist[count] = sl;
+        ++count;
+        prev = sl;
+      }
     }
     counts[sg] = count;
     mine[sg] = my_index;
@@ -251,38 +258,10 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
   const size_t slot_words = size_t(p.mpad) * kTileN;
   const uint32_t n_items = p.m * 32u;   // one item = one batch row x 4 output channels
   for (int sg = 0; sg < ns; ++sg) {
-    const uint32_t *list = scratch + sg * PK;
-    // 4. my slice of the stripe's items
-    const uint32_t it_begin = mine[sg] * n_items / counts[sg], it_end = (mine[sg] + 1) * n_items / counts[sg];
-    for (uint32_t it = it_begin + tid; it < it_end; it += kNT) {
-      const uint32_t mm = it >> 5, r4 = (it & 31u) * 4u;
-      const uint32_t *src = p.partials + size_t(mm) * kTileN + r4;
-      uint32_t acc[4];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) acc[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
-      uint32_t prev = 0xFFFFFFFFu;
-      for (uint32_t kb = 0; kb < PK; kb += 8) {
-        uint4 val[8];
-        bool use[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          use[j] = false;
-          if (kb + j < PK) {
-            const uint32_t sl = list[kb + j];
-            use[j] = sl != prev;
-            prev = sl;
-            if (use[j]) val[j] = ldcg128(src + size_t(sl) * slot_words);
-          }
-        }
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {   // fixed team order -> bit-reproducible sums
-          if (use[j]) {
-            acc[0] = acc_add<FMT>(acc[0], val[j].x); acc[1] = acc_add<FMT>(acc[1], val[j].y);
-            acc[2] = acc_add<FMT>(acc[2], val[j].z); acc[3] = acc_add<FMT>(acc[3], val[j].w);
-          }
-        }
-      }
-      const uint32_t n4 = stripes[sg] * kTileN + r4;
+    const uint32_t *ulist = scratch + (2 + sg) * PK;
+    const uint32_t count = counts[sg];
+    auto emit = [&](const uint32_t (&acc)[4], uint32_t it) {
+      const uint32_t mm = it >> 5, n4 = stripes[sg] * kTileN + (it & 31u) * 4u;
       const float xs = kScaled ? p.x_scale[mm] : 1.0f;
       float o[4];
 #pragma unroll
@@ -303,6 +282,40 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
         if ((reinterpret_cast<uintptr_t>(yo) & 15) == 0) *reinterpret_cast<float4 *>(yo) = make_float4(o[0], o[1], o[2], o[3]);
         else { yo[0] = o[0]; yo[1] = o[1]; yo[2] = o[2]; yo[3] = o[3]; }
       }
+    };
+    // 4. my slice of the stripe's items, two items at a time and four contributors at a time: up to eight 16-byte loads in
+    //    flight per thread (the loop is bound by L2 round trips, ~1.5 us each under the launch's tail)
+    const uint32_t it_begin = mine[sg] * n_items / count, it_end = (mine[sg] + 1) * n_items / count;
+    for (uint32_t it = it_begin + tid; it < it_end; it += 2 * kNT) {
+      const bool two = it + kNT < it_end;
+      const uint32_t it1 = two ? it + kNT : it;
+      const uint32_t *src0 = p.partials + size_t(it >> 5) * kTileN + (it & 31u) * 4u;
+      const uint32_t *src1 = p.partials + size_t(it1 >> 5) * kTileN + (it1 & 31u) * 4u;
+      uint32_t acc0[4], acc1[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) acc0[j] = acc1[j] = FMT == ANSLIN_FMT_INT8 ? 0u : __float_as_uint(0.0f);
+      for (uint32_t kb = 0; kb < count; kb += 4) {
+        uint4 v0[4], v1[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          if (kb + j < count) {
+            const size_t so = size_t(ulist[kb + j]) * slot_words;
+            v0[j] = ldcg128(src0 + so);
+            v1[j] = ldcg128(src1 + so);
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {   // fixed team order -> bit-reproducible sums
+          if (kb + j < count) {
+            acc0[0] = acc_add<FMT>(acc0[0], v0[j].x); acc0[1] = acc_add<FMT>(acc0[1], v0[j].y);
+            acc0[2] = acc_add<FMT>(acc0[2], v0[j].z); acc0[3] = acc_add<FMT>(acc0[3], v0[j].w);
+            acc1[0] = acc_add<FMT>(acc1[0], v1[j].x); acc1[1] = acc_add<FMT>(acc1[1], v1[j].y);
+            acc1[2] = acc_add<FMT>(acc1[2], v1[j].z); acc1[3] = acc_add<FMT>(acc1[3], v1[j].w);
+          }
+        }
+      }
+      emit(acc0, it);
+      if (two) emit(acc1, it1);
     }
   }
   RTRACE(6);
@@ -349,7 +362,8 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   const uint32_t v = c * T + (decoder ? team : 0u);
   const uint32_t p_begin = tm.first(v), p_end = decoder ? tm.first(v + 1) : p_begin;
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cbase + pr.cv.off_offsets);
-  // record offsets of this warp's first pair of tiles: in flight while the slot table is built
+  // the frequency table and the record offsets of this warp's first pair of tiles: one HBM round trip for both
+  const uint4 freq_regs = slot_table_load(reinterpret_cast<const uint16_t *>(cbase + pr.cv.off_freq));
   uint32_t cur_off[2] = {0, 0};
   if (p_begin < p_end) {
     const uint32_t s0 = p_begin / PK, k0 = 2u * (p_begin % PK), t0 = (s0 * KT + k0) * 4u + q;
@@ -369,7 +383,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   }
   if (warp == 0) tmem_alloc(smem0 + kTmPtrOff, 512);
   tc_fence_before();
-  build_slot_table(tab, cum, reinterpret_cast<const uint16_t *>(cbase + pr.cv.off_freq));   // ends with __syncthreads()
+  build_slot_table(tab, cum, freq_regs);   // ends with __syncthreads()
   tc_fence_after();
   const uint32_t tmem_base = *tmemptr;
 
