@@ -35,6 +35,7 @@ constexpr uint32_t kNT = 32 * kTeamWarps;                    // threads of a tea
 // shared-memory carve-up, from the 1024-byte aligned base: slot table | prefix scratch | barriers | X rings | raw | staging
 constexpr uint32_t kTmBarOff = 16384 + 1088;                 // 64 bytes of mbarriers per team
 constexpr uint32_t kTmPtrOff = kTmBarOff + 64 * kMaxTeams;
+constexpr uint32_t kTmWarpBarOff = kTmPtrOff + 16;             // one mbarrier per decoder warp: its staged segments have landed
 constexpr uint32_t kTmXOff = 18432;
 constexpr uint32_t kRawBufBytes = 1024;                      // bf16: two 512-byte raw vectors per chain
 __host__ __device__ constexpr bool tmem_has_raw(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16; }
@@ -103,6 +104,55 @@ __device__ __forceinline__ uint32_t lds16(uint32_t a) {
 }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+               : "memory");
+}
+// lane_open_segments (decode_core.cuh) for two records whose staging buffers are small enough to be copied whole without
+// waiting for the segment table (bufbytes <= kTailBytes): ONE bulk copy per record, issued by lane 0 and completed on the
+// warp's mbarrier `bar` (phase `parity`), instead of six 16-byte cp.async per lane and record.
+// extra(): cp.async copies of the caller (first raw vectors), waited for here too.
+template <class Extra>
+__device__ __forceinline__ void lane_open_segments_bulk(LaneStream (&s)[2], uint32_t buf0, uint32_t bufbytes, int seg, int lane, uint32_t bar,
+                                                        uint32_t parity, const Extra &extra) {
+  __syncwarp();   // every lane is done with the words of the previous segments
+  uint32_t hdr[2], delta[2];
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const uint8_t *te = s[j].rec + 4 * kLanes + kSegTableBytes * seg;
+    hdr[j] = *reinterpret_cast<const uint32_t *>(te);   // u16 base | u16 total words
+    delta[j] = lane < kLanes / 2 ? uint32_t(te[4 + lane]) : 0u;
+  }
+  if (lane == 0) {
+    mbar_arrive_expect_tx(bar, 2u * bufbytes);
+#pragma unroll
+    for (int j = 0; j < 2; ++j) bulk_copy_g2s(buf0 + uint32_t(j) * bufbytes, s[j].rec + (s[j].goff & ~15u), bufbytes, bar);
+  }
+  extra();
+  cp_async_commit();
+#pragma unroll
+  for (int j = 0; j < 2; ++j) {
+    const uint32_t base = hdr[j] & 0xFFFFu, total = hdr[j] >> 16, buf = buf0 + uint32_t(j) * bufbytes;
+    const uint32_t size = lane < kLanes / 2 ? base + delta[j] : 0u;   // words of region `lane`
+    uint32_t end = size;
+#pragma unroll
+    for (int d = 1; d < kLanes / 2; d <<= 1) {
+      const uint32_t o = __shfl_up_sync(0xffffffffu, end, d);
+      if (lane >= d) end += o;
+    }
+    const uint32_t start = end - size;
+    const uint32_t start_p = __shfl_sync(0xffffffffu, start, lane >> 1), end_p = __shfl_sync(0xffffffffu, end, lane >> 1);
+    const uint32_t skew = s[j].goff & 15u;
+    // the cursor is clamped into the staged buffer (see lane_open_segments)
+    s[j].ptr = buf + skew + 2u * min((lane & 1) ? end_p - 1u : start_p, (bufbytes - skew) / 2u - 1u);
+    s[j].goff += 2u * total;
+  }
+  cp_async_wait_all();
+  mbar_wait(bar, parity);
+#pragma unroll
+  for (int j = 0; j < 2; ++j) asm volatile("ld.shared.u16 %0, [%1];" : "=r"(s[j].w) : "r"(s[j].ptr) : "memory");
 }
 
 // Half H (0 / 1) of one operand unit (32 operand bytes per row = 8 registers) of the warp's two tiles: registers
@@ -379,6 +429,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   if (threadIdx.x == 0) {
     for (uint32_t i = 0; i < T; ++i)
       for (uint32_t b = 0; b < 8; ++b) mbar_init(bars_s + 64 * i + 8 * b, b >= 6 ? kTeamWarps : 1);
+    for (uint32_t i = 0; i < kTeamWarps * T; ++i) mbar_init(smem0 + kTmWarpBarOff + 8 * i, 1);
     fence_mbar_init();
   }
   if (warp == 0) tmem_alloc(smem0 + kTmPtrOff, 512);
@@ -473,6 +524,8 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   // the team) lets the issuer warp multiply the step.  Deferred to the middle of the next unit so that the store latency
   // overlaps decode steps; completed before anything waits for the step's MMAs (the segment's epilogue).
   bool pending = false;       // a unit's stores are not yet published
+  uint32_t open_par = 0;      // phase of the warp's staging barrier
+  const uint32_t warpbar_s = smem0 + kTmWarpBarOff + 8u * uint32_t(warp);
   uint32_t kpar = 0;          // parity of (unit step / 2): the phase of the operand-free barriers
   auto finish_handover = [&](uint32_t full_bar) {
     if (pending) {
@@ -533,13 +586,17 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
           if (u == 0) PROF(6);
           if (u % kUnitsPerSeg == 0) {
             // stage the segment (drains cp.async first and last); at the tile's start its first raw vector rides in the same group
-            if (kRawOn && u == 0) {
-              lane_open_segments<2>(s, stage_s, P.stream_bytes, 0, lane, [&]() {
+            auto first_raw = [&]() {
+              if (kRawOn && u == 0) {
 #pragma unroll
                 for (int j = 0; j < 2; ++j) { cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes, rawp[j]); rawp[j] += 512; }
-              });
+              }
+            };
+            if (P.stream_bytes <= uint32_t(kTailBytes)) {
+              lane_open_segments_bulk(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane, warpbar_s, open_par, first_raw);
+              open_par ^= 1u;
             } else {
-              lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane);
+              lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane, first_raw);
             }
           }
           if (u == 0) PROF(4);
