@@ -171,9 +171,9 @@ def run_reference(args):
 
 
 # Warp instructions per decoded bf16 symbol in the hot loop of fused_tmem_kernel<bf16> (counted in
-# profiles/r2_sass_decode_loop.md): 13 in the rANS step (IMAD.SHL, LOP3, LDS, SHF x3, LOP3, IMAD, ISETP, @IMAD, @IMAD.IADD,
-# @LDS.U16 + the state shift) and 2.5 in the bf16 merge (PRMT x2, SHF, IMAD.SHL, LOP3 per two weights).
-INSTR_PER_SYMBOL = 15.5
+# profiles/r2_sass_decode_loop.md): 11 in the rANS step (IMAD.SHL, LOP3, LDS, LEA.HI, SHF x2, IMAD, ISETP, @IMAD, @IMAD.IADD,
+# @LDS.U16) and 2.5 in the bf16 merge (PRMT x2, SHF, IMAD.SHL, LOP3 per two weights).
+INSTR_PER_SYMBOL = 13.5
 
 
 def run_other_config(args):
