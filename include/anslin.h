@@ -40,7 +40,8 @@ typedef enum {
   ANSLIN_ERR_UNSUPPORTED = 2,
   ANSLIN_ERR_BUFFER_TOO_SMALL = 3,
   ANSLIN_ERR_CORRUPT = 4,
-  ANSLIN_ERR_CUDA = 5
+  ANSLIN_ERR_CUDA = 5,
+  ANSLIN_ERR_STATIC_LIMIT = 6   /* anslin_gemm_static: the problem needs more scratch than the library's static array holds */
 } anslin_status;
 
 /* Numeric format of W (P:l.80, l.341; BASELINE.json configs 1-5). */
@@ -168,6 +169,22 @@ size_t anslin_gemm_multi_workspace_bytes(const anslin_weight *const *weights, in
 int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m,
                 const void *x_scale_dev, void *y_dev, int64_t ldy, void *workspace_dev,
                 size_t workspace_bytes, void *stream);
+
+/*
+ * anslin_gemm for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc)
+ * and so cannot provide a workspace: the split-K scratch is a static device array inside the library
+ * (ANSLIN_STATIC_WORKSPACE_BYTES, held by every GPU that loads the library until the process exits).  The call allocates
+ * nothing: no cudaMalloc, cudaFree or allocating library routine; it enqueues one cudaMemsetAsync of the flag words and the
+ * launch(es) of anslin_gemm on `stream`.  Arguments, layouts and results are anslin_gemm's.
+ *   Limit: anslin_gemm_workspace_bytes(w, m) <= ANSLIN_STATIC_WORKSPACE_BYTES, else ANSLIN_ERR_STATIC_LIMIT and nothing is
+ *   enqueued (24 MiB covers every shape at m <= 32 for containers the tensor-memory kernel takes; larger batches need
+ *   anslin_gemm with a caller-owned workspace).
+ *   The array is ONE per device and shared by every call: two calls that may overlap on the GPU (different streams, or
+ *   graph branches without an edge between them) race on it and give wrong results; calls on one stream are ordered and safe.
+ */
+#define ANSLIN_STATIC_WORKSPACE_BYTES (24u << 20)
+int anslin_gemm_static(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m,
+                       const void *x_scale_dev, void *y_dev, int64_t ldy, void *stream);
 
 /*
  * n independent fused decode-GEMMs in ONE persistent launch (projections that share an input, e.g.

@@ -25,7 +25,7 @@ EXPORTS = ["anslin_encode_bound", "anslin_encode_host", "anslin_open", "anslin_c
            "anslin_gemm_multi", "anslin_gemm_multi_ex", "anslin_gemm_grouped",
            "anslin_dense_workspace_bytes", "anslin_dense_gemm", "anslin_histogram", "anslin_entropy_bits",
            "anslin_entropy_weighted", "anslin_encode_device_workspace_bytes", "anslin_encode_device_head_bytes",
-           "anslin_encode_device", "anslin_gemm_launches", "anslin_status_string"]
+           "anslin_encode_device", "anslin_gemm_launches", "anslin_status_string", "anslin_gemm_static"]
 
 
 class AnslinError(RuntimeError):
@@ -66,6 +66,7 @@ def lib() -> ctypes.CDLL:
         L.anslin_decode.argtypes = [vp, vp, sz, vp]
         L.anslin_gemm_workspace_bytes.argtypes = [vp, i32]; L.anslin_gemm_workspace_bytes.restype = sz
         L.anslin_gemm.argtypes = [vp, vp, u32, i64, i32, vp, vp, i64, vp, sz, vp]
+        L.anslin_gemm_static.argtypes = [vp, vp, u32, i64, i32, vp, vp, i64, vp]
         L.anslin_gemm_multi_workspace_bytes.argtypes = [ctypes.POINTER(vp), i32, i32]
         L.anslin_gemm_multi_workspace_bytes.restype = sz
         L.anslin_gemm_multi.argtypes = [ctypes.POINTER(vp), i32, ctypes.POINTER(vp), u32, ctypes.POINTER(i64), ctypes.POINTER(i32),
@@ -187,6 +188,16 @@ def anslin_gemm(w: Weight, x_ptr: int, x_dtype: int, ldx: int, m: int, x_scale_p
                 ws_ptr: int, ws_bytes: int, stream: int = 0):
     _check(lib().anslin_gemm(w.handle, ctypes.c_void_p(x_ptr), x_dtype, ldx, m, ctypes.c_void_p(x_scale_ptr or 0),
                              ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(ws_ptr), ws_bytes, ctypes.c_void_p(stream)), "anslin_gemm")
+
+
+STATIC_WORKSPACE_BYTES = 24 << 20
+
+
+def anslin_gemm_static(w: Weight, x_ptr: int, x_dtype: int, ldx: int, m: int, x_scale_ptr: int | None, y_ptr: int, ldy: int,
+                       stream: int = 0):
+    """anslin_gemm on the library's static workspace: allocates nothing (include/anslin.h)."""
+    _check(lib().anslin_gemm_static(w.handle, ctypes.c_void_p(x_ptr), x_dtype, ldx, m, ctypes.c_void_p(x_scale_ptr or 0),
+                                    ctypes.c_void_p(y_ptr), ldy, ctypes.c_void_p(stream)), "anslin_gemm_static")
 
 
 def anslin_gemm_multi_workspace_bytes(weights, m_max: int) -> int:

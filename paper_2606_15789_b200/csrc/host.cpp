@@ -550,6 +550,7 @@ const char *anslin_status_string(int s) {
     case ANSLIN_ERR_BUFFER_TOO_SMALL: return "buffer too small";
     case ANSLIN_ERR_CORRUPT: return "corrupt container";
     case ANSLIN_ERR_CUDA: return "CUDA error";
+    case ANSLIN_ERR_STATIC_LIMIT: return "problem needs more scratch than the static workspace (ANSLIN_STATIC_WORKSPACE_BYTES) holds";
     default: return "unknown status";
   }
 }

@@ -1354,6 +1354,39 @@ int anslin_gemm(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int
   return ANSLIN_OK;
 }
 
+// ---- anslin_gemm without a caller-provided workspace and without any allocation ------------------------------------------
+// The split-K flags and partials live in a file-scope device array (every GPU that loads the library holds these
+// ANSLIN_STATIC_WORKSPACE_BYTES until the process exits).  In host code the array's NAME is only a host-side stand-in for the
+// symbol, never a device address: its address is asked for once per device with cudaGetSymbolAddress, with that device
+// current, and that pointer is what the kernel is given.
+static __device__ __align__(256) unsigned char g_static_workspace[ANSLIN_STATIC_WORKSPACE_BYTES];
+
+int anslin_gemm_static(const anslin_weight *w, const void *x_dev, uint32_t x_dtype, int64_t ldx, int32_t m, const void *x_scale_dev,
+                       void *y_dev, int64_t ldy, void *stream) {
+  if (!w) return ANSLIN_ERR_INVALID_ARG;
+  if (m < 1) return ANSLIN_ERR_INVALID_ARG;
+  // the same size rule as the caller of anslin_gemm follows; beyond the array: refuse before anything is enqueued
+  const size_t need = anslin_gemm_workspace_bytes(w, m);
+  if (need == 0) return ANSLIN_ERR_UNSUPPORTED;
+  if (need > size_t(ANSLIN_STATIC_WORKSPACE_BYTES)) return ANSLIN_ERR_STATIC_LIMIT;
+  constexpr int kMaxDevices = 64;
+  static std::atomic<void *> ptr_of_device[kMaxDevices];   // zero-initialised; a race between two first calls stores the same value twice
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return ANSLIN_ERR_CUDA;
+  void *ptr = ptr_of_device[dev].load(std::memory_order_acquire);
+  if (!ptr) {
+    if (cudaGetSymbolAddress(&ptr, g_static_workspace) != cudaSuccess || !ptr) return ANSLIN_ERR_CUDA;
+    ptr_of_device[dev].store(ptr, std::memory_order_release);
+  }
+  // The array keeps whatever the last call left in it.  The kernels need the split-K flag words to start as "not stored":
+  // their readers take them down and a flag holds a per-launch epoch, but this path does not lean on either: the flag
+  // area (the first bytes of the workspace; the partials behind it are written before they are read) is cleared
+  // on the stream ahead of the launch.  No allocation: a memset node, capturable like the launch itself.
+  const size_t flags = flag_bytes(w->h) * size_t(std::max<int64_t>(1, std::min<int64_t>(kMaxProblems, (int64_t(m) + kMaxM - 1) / kMaxM)));
+  if (cudaMemsetAsync(ptr, 0, std::min(flags, need), static_cast<cudaStream_t>(stream)) != cudaSuccess) return ANSLIN_ERR_CUDA;
+  return anslin_gemm(w, x_dev, x_dtype, ldx, m, x_scale_dev, y_dev, ldy, ptr, size_t(ANSLIN_STATIC_WORKSPACE_BYTES), stream);
+}
+
 int anslin_gemm_multi_ex(const anslin_weight *const *weights, int32_t n, const void *const *x_dev, uint32_t x_dtype, const int64_t *ldx,
                          const int32_t *m, const void *const *x_scale_dev, void *const *y_dev, uint32_t y_dtype, const int64_t *ldy,
                          void *workspace_dev, size_t workspace_bytes, void *stream) {

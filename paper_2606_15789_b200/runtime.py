@@ -70,6 +70,16 @@ class DeviceWeight:
         return y
 
 
+    def gemm_static(self, x: torch.Tensor, x_scale: torch.Tensor | None = None, y: torch.Tensor | None = None,
+                    x_dtype: int | None = None) -> torch.Tensor:
+        """anslin_gemm_static: the same product on the library's static workspace; the call allocates nothing (y given)."""
+        m = x.shape[0]
+        if y is None:
+            y = torch.empty((m, self.n_out), dtype=torch.float32, device=x.device)
+        B.anslin_gemm_static(self.weight, x.data_ptr(), B.X_DTYPE[self.fmt] if x_dtype is None else x_dtype, x.stride(0), m,
+                             None if x_scale is None else x_scale.data_ptr(), y.data_ptr(), y.stride(0), _stream())
+        return y
+
 def encode_on_device(fmt: int, w: torch.Tensor, n_out: int, k_in: int, tile_k: int = 256, flags: int = B.FLAG_LANE_STREAMS,
                      scales: np.ndarray | None = None, zeros: np.ndarray | None = None, group_size: int = 0,
                      w_scale: float = 1.0) -> "DeviceWeight":
