@@ -284,7 +284,7 @@ def config_records(hbm_peak: float, tc_peak: float, sm_mhz: float):
     def record(cfg, mat, n, k, m, fmt_name, cont_bytes, n_sym, flops, tc_ratio, fused_us, dense_us, decode_us, bits, h):
         hbm_us = cont_bytes / (hbm_peak * 1e9) * 1e6
         tc_us = flops / (tc_peak * tc_ratio * 1e12) * 1e6
-        issue_us = n_sym * 13.0 / (148 * 4 * 32 * sm_mhz * 1e6) * 1e6            # 13 warp instructions per rANS step
+        issue_us = n_sym * 11.0 / (148 * 4 * 32 * sm_mhz * 1e6) * 1e6            # 11 warp instructions per rANS step
         recs.append({"config": cfg, "matrix": "%s %dx%d" % (mat, n, k), "m": m, "format": fmt_name, "fused_us": round(fused_us, 1),
                      "tflops": round(flops / fused_us / 1e6, 2), "compressed_gbs": round(cont_bytes / fused_us / 1e3, 1),
                      "bound_hbm_us": round(hbm_us, 1), "bound_tensor_us": round(tc_us, 2), "bound_issue_us": round(issue_us, 1),
@@ -477,18 +477,26 @@ def main():
             traffic, traffic_source = tj.get("fused_gemm_bytes_per_launch_mean"), tj.get("source")
 
     # ---- e2e: the same step through the C ABI with HOST buffers (pinned X in, Y out) inside the timed region
-    # Device->host reads of Y run on a copy stream of their own, behind an event per launch group, so that they
-    # overlap the next group's kernel; a group's next launch waits for the previous read of its Y buffers.
-    copy_stream = torch.cuda.Stream()
+    # Both directions run on copy streams of their own, as a serving loop would have them: the host->device copy of a launch
+    # group's X waits for the group's previous kernel (the last reader of that X buffer) and overlaps the other groups'
+    # kernels; the device->host read of its Y runs behind an event per group and overlaps the next group's kernel; a
+    # group's next launch waits for its X copy and for the previous read of its Y buffers.  Every step still moves all X in
+    # and all Y out inside the timed region.
+    copy_stream, h2d_stream = torch.cuda.Stream(), torch.cuda.Stream()
     y_ready = [torch.cuda.Event() for _ in groups]
     y_read = [torch.cuda.Event() for _ in groups]
+    x_done = [torch.cuda.Event() for _ in groups]
 
     def step_e2e(calls_=None, ys_=None, ys_host_=None):
         calls_, ys_, ys_host_ = calls_ or calls, ys_ or ys, ys_host_ or ys_host
         main = torch.cuda.current_stream()
         for gi, (g, call) in enumerate(zip(groups, calls_)):
-            for o in sorted({x_owner[i] for i in g}):
-                xs_dev[o].view(torch.int16).copy_(xs_host[o], non_blocking=True)
+            h2d_stream.wait_event(y_ready[gi])
+            with torch.cuda.stream(h2d_stream):
+                for o in sorted({x_owner[i] for i in g}):
+                    xs_dev[o].view(torch.int16).copy_(xs_host[o], non_blocking=True)
+                x_done[gi].record(h2d_stream)
+            main.wait_event(x_done[gi])
             main.wait_event(y_read[gi])
             call()
             y_ready[gi].record(main)

@@ -295,8 +295,14 @@ __device__ __forceinline__ void lane_step2(LaneStream &s0, LaneStream &s1, uint3
   uint32_t a0, a1;
   asm("mul.lo.u32 %0, %1, 4;" : "=r"(a0) : "r"(s0.x));
   asm("mul.lo.u32 %0, %1, 4;" : "=r"(a1) : "r"(s1.x));
+#ifdef ANSLIN_SKEL_NOCONFLICT   // timing experiment only (wrong results): the table gather without bank conflicts
+  { const uint32_t l4 = (threadIdx.x & 31u) << 2;
+    asm("lop3.b32 %0, %0, 0x3F80, %1, 0xEA;" : "+r"(a0) : "r"(l4));
+    asm("lop3.b32 %0, %0, 0x3F80, %1, 0xEA;" : "+r"(a1) : "r"(l4)); }
+#else
   asm("and.b32 %0, %0, 0x3FFC;" : "+r"(a0));
   asm("and.b32 %0, %0, 0x3FFC;" : "+r"(a1));
+#endif
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e0) : "r"(a0 + tab_s));
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(e1) : "r"(a1 + tab_s));
   uint32_t x0 = state_update(s0.x, e0);
@@ -309,8 +315,11 @@ __device__ __forceinline__ void lane_step2(LaneStream &s0, LaneStream &s1, uint3
       "@q mad.lo.u32 %3, %3, 65536, %5;\n\t"
       "@p add.u32 %1, %1, %6;\n\t"
       "@q add.u32 %4, %4, %6;\n\t"
+#ifndef ANSLIN_SKEL_NOWORDLOAD   // timing experiment only (wrong results): no look-ahead word loads
       "@p ld.shared.u16 %2, [%1];\n\t"
-      "@q ld.shared.u16 %5, [%4];\n\t}"
+      "@q ld.shared.u16 %5, [%4];\n\t"
+#endif
+      "}"
       : "+r"(x0), "+r"(s0.ptr), "+r"(s0.w), "+r"(x1), "+r"(s1.ptr), "+r"(s1.w)
       : "r"(dir)
       : "memory");
