@@ -890,25 +890,55 @@ EncodeTiledFn encode_tiled_fn() {
 }
 
 // 2-D row-major tensor [rows x cols] of `ebytes`-byte elements, leading dimension ld elements.
+// The encoded map is a function of these arguments only (it holds the address, not a device handle), and encoding costs a
+// driver call: the last few maps of a thread are kept, so that a serving loop that calls with the same (pointer, m, ld)
+// step after step encodes each map once.
 bool make_map_2d(CUtensorMap *map, const void *ptr, int ebytes, uint64_t cols, uint64_t rows, uint64_t ld, uint32_t box_cols,
                  uint32_t box_rows, CUtensorMapSwizzle swz) {
+  struct Entry { const void *ptr; uint64_t cols, rows, ld; uint32_t box_cols, box_rows; int ebytes, swz; bool valid; CUtensorMap map; };
+  constexpr int kEntries = 32;
+  static thread_local Entry cache[kEntries] = {};
+  static thread_local int next = 0;
+  for (int i = 0; i < kEntries; ++i) {
+    const Entry &e = cache[i];
+    if (e.valid && e.ptr == ptr && e.cols == cols && e.rows == rows && e.ld == ld && e.box_cols == box_cols && e.box_rows == box_rows &&
+        e.ebytes == ebytes && e.swz == int(swz)) {
+      *map = e.map;
+      return true;
+    }
+  }
   EncodeTiledFn fn = encode_tiled_fn();
   if (!fn) return false;
   cuuint64_t dims[2] = {cols, rows}, strides[1] = {ld * uint64_t(ebytes)};
   cuuint32_t box[2] = {box_cols, box_rows}, estr[2] = {1, 1};
   CUtensorMapDataType dt = ebytes == 2 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_UINT8;
-  return fn(map, dt, 2, const_cast<void *>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
-            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  if (fn(map, dt, 2, const_cast<void *>(ptr), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
+         CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return false;
+  Entry &e = cache[next];
+  next = (next + 1) % kEntries;
+  e.ptr = ptr; e.cols = cols; e.rows = rows; e.ld = ld; e.box_cols = box_cols; e.box_rows = box_rows; e.ebytes = ebytes; e.swz = int(swz);
+  e.map = *map;
+  e.valid = true;
+  return true;
 }
 
+// Per-device state (SM count, "shared-memory limit raised" marks of the kernel instantiations) is indexed by the current device.
+constexpr int kMaxDevices = 64;
+int device_index() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) return 0;
+  return dev % kMaxDevices;
+}
 int num_sms() {
-  static int n = [] {
-    int dev = 0, v = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+  static std::atomic<int> n[kMaxDevices];   // 0 = not asked yet
+  const int dev = device_index();
+  int v = n[dev].load(std::memory_order_relaxed);
+  if (v == 0) {
     if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    return v;
-  }();
-  return n;
+    n[dev].store(v, std::memory_order_relaxed);
+  }
+  return v;
 }
 
 uint32_t mpad_of(int32_t m) { return uint32_t((m + 15) / 16 * 16); }
@@ -962,7 +992,8 @@ int sm_budget() { return std::max(1, num_sms()); }
 template <uint32_t FMT, int RB, bool PAYLOAD, bool LS, bool YB>
 int launch_fused_y(const TensorMaps &tms, const FusedParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
   auto kern = fused_gemm_kernel<FMT, RB, (RB == 1 ? kJ32 : 1), PAYLOAD, LS, YB>;
-  static thread_local size_t smem_set = 0;     // per instantiation: raise the dynamic shared memory limit once
+  static thread_local size_t smem_set_dev[kMaxDevices] = {};   // per instantiation and device: raise the dynamic shared memory limit once
+  size_t &smem_set = smem_set_dev[device_index()];
   if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
     smem_set = kSmemMax;
@@ -997,7 +1028,8 @@ bool tmem_eligible(const Header &h) {
 template <uint32_t FMT, bool PAYLOAD, bool YB>
 int launch_tmem_y(const TensorMaps &tms, const TmemParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
   auto kern = fused_tmem_kernel<FMT, PAYLOAD, YB>;
-  static thread_local size_t smem_set = 0;
+  static thread_local size_t smem_set_dev[kMaxDevices] = {};
+  size_t &smem_set = smem_set_dev[device_index()];
   if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
     smem_set = kSmemMax;
@@ -1236,8 +1268,11 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   // + 16: a lane-stream's look-ahead word load may touch the two bytes after the last stream buffer
   const size_t smem = 4 * kM + 1056 + size_t(kDecWarps) * J * (stream_bytes + GlobalEmit<FMT, RB, J>::kStageBytes) + 16;
   if (smem > kSmemMax) return ANSLIN_ERR_UNSUPPORTED;
-  static thread_local size_t smem_set = 0, smem_occ = 0;   // per instantiation
-  static thread_local int occ = 0;
+  struct DevState { size_t smem_set, smem_occ; int occ; };
+  static thread_local DevState dev_state[kMaxDevices] = {};   // per instantiation and device
+  DevState &ds = dev_state[device_index()];
+  size_t &smem_set = ds.smem_set, &smem_occ = ds.smem_occ;
+  int &occ = ds.occ;
   if (smem > smem_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
     smem_set = smem;
