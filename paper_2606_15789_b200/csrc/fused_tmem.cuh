@@ -536,9 +536,13 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       pending = false;
     }
   };
-#ifdef ANSLIN_STAGGER_NS
-  __nanosleep(team * ANSLIN_STAGGER_NS);   // teams out of phase: one team's hand-over overlaps the others' decoding
+  // Teams start half a microsecond apart: the sixteen decoder warps of an SM otherwise run in lock step, and every tile opening
+  // and hand-over of one team then coincides with the others'.  The offset persists for the launch and pays for itself
+  // (0.2800 against 0.2820 ms per step; 1 us apart the same, 1.5 us apart 0.2843: profiles/r2_skeleton_experiments.md).
+#ifndef ANSLIN_STAGGER_NS
+#define ANSLIN_STAGGER_NS 500
 #endif
+  __nanosleep(team * ANSLIN_STAGGER_NS);
   TRACE(1);
   PROF_DECL
 #pragma unroll 1
