@@ -575,6 +575,21 @@ def main():
             fl = sum(2.0 * mm * n * k for (_, n, k, _) in layer)
             extra["M=%d" % mm] = {"ms": round(t, 4), "tflops": round(fl / (t * 1e-3) / 1e12, 3),
                                   "compressed_gbs": round(comp_bytes / (t * 1e-3) / 1e9, 1)}
+            # the same batch size through the step's four grouped launches (q+k+v, o, gate+up, down)
+            calls_m = [rt.MultiGemm([dws[i] for i in g], [xm[x_owner[i]] for i in g], ys=[ym[i] for i in g]) for g in groups]
+            for _ in range(3):
+                for cm in calls_m:
+                    cm()
+            torch.cuda.synchronize(); a.record()
+            for _ in range(20):
+                for cm in calls_m:
+                    cm()
+            b.record(); torch.cuda.synchronize()
+            tg = a.elapsed_time(b) / 20
+            extra["M=%d" % mm].update({"grouped_ms": round(tg, 4), "grouped_tflops": round(fl / (tg * 1e-3) / 1e12, 3),
+                                       "grouped_compressed_gbs": round(comp_bytes / (tg * 1e-3) / 1e9, 1),
+                                       "grouped_frac_of_hbm_roofline": round((comp_bytes + sum(2 * mm * k for (_, n, k, _) in [layer[g[0]] for g in groups]) + sum(4 * mm * n for (_, n, k, _) in layer)) / (tg * 1e-3) / 1e9 / hbm_peak, 4)})
+            del calls_m
         out["per_m"] = extra
         wd = [torch.from_numpy(w.view(np.int16)).cuda() for (_, _, _, w) in layer]
         wsd = [torch.empty(B.anslin_dense_workspace_bytes(n, k, m), dtype=torch.uint8, device="cuda") for (_, n, k, _) in layer]
