@@ -410,15 +410,17 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
     if (!whole) {
       __threadfence();
       named_bar_sync(1, kEpiWarps * 32);
-      if (warp == 0 && lane == 0) {
-        // every thread's partial stores are fenced and the warps have met: raise this segment's flag.  The stripe's last
-        // contributor (the CTA that holds its last k-tile, known from the shape alone) sums the partials once it has seen
-        // every flag of the stripe carry this launch's epoch (splitk_fixup): no atomics, no retries under contention, and
-        // stale or uninitialised workspace bytes never match the epoch.
+      if (warp == 0) {
+        // every thread's partial stores are fenced and the warps have met: raise this segment's flags, one word per reader
+        // (flag[(c * 2 + seg) * KT + reader's index among the stripe's contributors]).  The contributors of a stripe are the
+        // CTAs c_first .. c_last that hold its k-tiles (known from the shape alone); EVERY one of them sums its own slice of
+        // the stripe's outputs once it has seen the flags addressed to it carry this launch's epoch (splitk_fixup): no
+        // atomics, no retries under contention, and stale or uninitialised workspace bytes never match the epoch.
         const uint32_t c_first = cta_of_tile(stripe * KT, G, T), c_last = cta_of_tile(stripe * KT + KT - 1, G, T);
-        uint32_t *flag = reinterpret_cast<uint32_t *>(p.counters) + (c * 2u + seg);
-        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag), "r"(p.epoch) : "memory");
-        fin[seg].stripe = stripe; fin[seg].c_first = c_first; fin[seg].c_last = c_last; fin[seg].valid = c == c_last ? 1u : 0u;
+        uint32_t *flag = reinterpret_cast<uint32_t *>(p.counters) + size_t(c * 2u + seg) * KT;
+        for (uint32_t r = uint32_t(lane); r <= c_last - c_first; r += 32)
+          asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(flag + r), "r"(p.epoch) : "memory");
+        if (lane == 0) { fin[seg].stripe = stripe; fin[seg].c_first = c_first; fin[seg].c_last = c_last; fin[seg].valid = 1u; }
       }
     }
     t += nt;
@@ -426,11 +428,12 @@ __device__ __forceinline__ void epilogue_run(const EpiParams &p, uint32_t tmem_b
 }
 
 // Deterministic split-K fix-up by ALL threads of the CTA (call after a CTA-wide barrier that follows
-// epilogue_run): for each stripe recorded in fin[], sum the partials of its contributors in CTA order
-// (bit-reproducible), apply the scales and store Y.  One item = one batch row x 4 output channels;
-// 16-byte loads, up to 8 contributors in flight per thread.
+// epilogue_run): for each stripe recorded in fin[] (every stripe this CTA holds a partial of), sum THIS CTA's slice of the
+// stripe's outputs over the partials of all contributors in CTA order (bit-reproducible), apply the scales and store Y.
+// One item = one batch row x 4 output channels; 16-byte loads, up to 8 contributors in flight per thread.  (One owner CTA
+// summing a whole stripe took ~15 us at the end of every launch.)
 template <uint32_t FMT, bool YB = false>
-__device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *fin, uint32_t KT, uint32_t G, uint32_t T) {
+__device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *fin, uint32_t KT, uint32_t c, uint32_t G, uint32_t T) {   // c: this CTA's index in its problem
   constexpr bool kScaled = FMT == ANSLIN_FMT_INT8 || is_fp8_path(FMT);
   constexpr int kItems = 2;   // items per thread and pass: their loads are all issued before the first add
   for (int seg = 0; seg < 2; ++seg) {
@@ -439,10 +442,11 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
     // contributor cc's partial slot: its first segment (slot 0) unless the stripe is its second one, which can only
     // be the case for the first contributor (every later one starts inside the stripe)
     const uint32_t first_slot = cta_first_tile(c_first, G, T) < stripe * KT ? 1u : 0u;
-    // wait for the other contributors (all CTAs of the persistent grid are resident, and a stripe's contributors have
-    // lower CTA indices than its owner): one flag per thread
+    // wait for the flags the contributors address to this CTA (all CTAs of the persistent grid are resident and raise their
+    // flags before they get here): one flag per thread
+    const uint32_t count = c_last - c_first + 1u, my_index = c - c_first;
     for (uint32_t cc = c_first + threadIdx.x; cc <= c_last; cc += blockDim.x) {
-      const uint32_t *flag = reinterpret_cast<const uint32_t *>(p.counters) + (cc * 2u + (cc == c_first ? first_slot : 0u));
+      const uint32_t *flag = reinterpret_cast<const uint32_t *>(p.counters) + size_t(cc * 2u + (cc == c_first ? first_slot : 0u)) * KT + my_index;
       uint32_t v, spins = 0;
       while (true) {
         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
@@ -455,8 +459,8 @@ __device__ __forceinline__ void splitk_fixup(const EpiParams &p, const FinSeg *f
     }
     __syncthreads();
     const size_t slot_words = size_t(p.mpad) * kTileN;
-    const uint32_t n_items = p.m * 32u;
-    for (uint32_t it0 = threadIdx.x; it0 < n_items; it0 += blockDim.x * kItems) {
+    const uint32_t all_items = p.m * 32u, it_begin = my_index * all_items / count, n_items = (my_index + 1u) * all_items / count;
+    for (uint32_t it0 = it_begin + threadIdx.x; it0 < n_items; it0 += blockDim.x * kItems) {
       uint32_t acc[kItems][4];
 #pragma unroll
       for (int q = 0; q < kItems; ++q)
@@ -774,7 +778,7 @@ __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __gri
   __syncthreads();
   if (warp == mma_warp) tmem_dealloc(tmem_base, P.tmem_cols);
   grid_dep_wait();   // warps that had no work of their own join the fix-up: same rule
-  splitk_fixup<FMT, YB>(ep, fin, KT, G, T);
+  splitk_fixup<FMT, YB>(ep, fin, KT, c, G, T);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -810,6 +814,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   FinSeg *fin = reinterpret_cast<FinSeg *>(smem + bar_off + 16 * kMaxSlots + 48);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t G = gridDim.x, KT = p.KB, T = (p.n_out / kTileN) * KT;
+  grid_dep_launch_dependents();   // programmatic dependent launch: the next kernel's prologue may overlap this one's tail
   if (threadIdx.x == 0) {
     for (uint32_t i = 0; i < p.S; ++i) { mbar_init(full_s + 8 * i, 1); mbar_init(empty_s + 8 * i, 1); }
     for (uint32_t i = 0; i < 2; ++i) { mbar_init(tfull_s + 8 * i, 1); mbar_init(tempty_s + 8 * i, kEpiWarps); fin[i].valid = 0; }
@@ -826,6 +831,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   if (warp == 5) {
     if (lane == 0) {
       uint32_t seq = 0;
+      grid_dep_wait();   // W and X belong to the stream's earlier kernels until they are done; every store of this CTA follows a load
       for (uint32_t t = t_begin; t < t_end; ++t, ++seq) {
         const uint32_t stripe = t / KT, kb = t % KT, slot = seq % p.S, par = (seq / p.S) & 1u;
         mbar_wait(empty_s + 8 * slot, par ^ 1u);
@@ -868,7 +874,7 @@ __global__ void __launch_bounds__(kDenseThreads, 1) dense_gemm_kernel(const __gr
   tc_fence_before();
   __syncthreads();
   if (warp == 0) tmem_dealloc(tmem_base, p.tmem_cols);
-  splitk_fixup<FMT>(ep, fin, KT, G, T);
+  splitk_fixup<FMT>(ep, fin, KT, blockIdx.x, G, T);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -971,10 +977,10 @@ size_t flag_bytes(const Header &h) {
   return align16(std::max(stripes * 8 + 256 + 8 * 160 * kMaxTeams, kTmFlagSlots * pk * 4));
 }
 struct Workspace { size_t counters_off, partials_off, total; };
-Workspace workspace_layout(uint32_t stripes, uint32_t grid, uint32_t mpad) {
+Workspace workspace_layout(uint32_t kb, uint32_t grid, uint32_t mpad) {   // kb: k-blocks per stripe
   Workspace w;
   w.counters_off = 0;
-  w.partials_off = align16(size_t(stripes) * 8 + 256 + 8 * 160 * kMaxTeams);   // the dense comparator's flag area
+  w.partials_off = align16(size_t(grid) * 2 * kb * 4 + 256);   // the dense comparator's flag area: one word per (partial slot, reader)
   w.total = w.partials_off + size_t(grid) * 2 * mpad * kTileN * 4;
   return w;
 }
@@ -1296,8 +1302,23 @@ int launch_decode(const ContainerView &cv, void *out, cudaStream_t st) {
 template <uint32_t FMT>
 int launch_dense(const CUtensorMap &tmw, const CUtensorMap &tmx, DenseParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
   auto kern = dense_gemm_kernel<FMT>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) return ANSLIN_ERR_CUDA;
-  kern<<<grid, kDenseThreads, smem, st>>>(tmw, tmx, p);
+  static thread_local size_t smem_set_dev[kMaxDevices] = {};
+  size_t &smem_set = smem_set_dev[device_index()];
+  if (smem > smem_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
+    smem_set = kSmemMax;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(kDenseThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // the prologue overlaps the predecessor's tail
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, kern, tmw, tmx, p) != cudaSuccess) return ANSLIN_ERR_CUDA;
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 
@@ -1485,9 +1506,8 @@ int anslin_gemm_grouped(const anslin_weight *const *experts, int32_t n_experts, 
 }
 
 size_t anslin_dense_workspace_bytes(uint32_t n_out, uint32_t k_in, int32_t m) {
-  (void)k_in;
   if (m < 1 || m > 256 || n_out % kTileN) return 0;
-  return workspace_layout(n_out / kTileN, uint32_t(std::max(num_sms(), 148)), mpad_of(m)).total;
+  return workspace_layout(k_in / 64 + 1, uint32_t(std::max(num_sms(), 148)), mpad_of(m)).total;   // k-blocks of 64 (2-byte) or 128 (1-byte) elements
 }
 
 int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32_t k_in, const void *w_scale_dev, float w_scale,
@@ -1520,7 +1540,7 @@ int anslin_dense_gemm(uint32_t format, const void *w_dev, uint32_t n_out, uint32
   p.S = uint32_t(std::min<size_t>((kSmemMax - fixed) / p.stage_bytes, 12));
   const size_t smem = fixed + size_t(p.S) * p.stage_bytes;
   const uint32_t stripes = n_out / kTileN, T = stripes * p.KB, grid = grid_of(T, 8);
-  const Workspace ws = workspace_layout(stripes, grid, p.mpad);
+  const Workspace ws = workspace_layout(p.KB, grid, p.mpad);
   if (workspace_bytes < ws.total) return ANSLIN_ERR_BUFFER_TOO_SMALL;
   p.counters = reinterpret_cast<unsigned long long *>(static_cast<uint8_t *>(workspace_dev) + ws.counters_off);
   p.epoch = next_epoch();
