@@ -561,6 +561,7 @@ struct SmemEmit {
 };
 
 #include "fused_tmem.cuh"
+#include "decode_lanes.cuh"
 
 template <uint32_t FMT, int RB, int J, bool PAYLOAD, bool LS, bool YB>
 __global__ void __launch_bounds__(kGemmThreads, 1) fused_gemm_kernel(const __grid_constant__ TensorMaps tms,
@@ -1293,8 +1294,51 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   kern<<<ctas, kDecWarps * 32, smem, st>>>(cv, static_cast<uint8_t *>(out), stream_bytes);
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
+// decode_lanes_kernel (decode_lanes.cuh) where the container allows it: lane streams, 32-row tiles, a unit of 32 bytes of W per
+// row, an even number of units per tile; as many decoder warps (16, 12 or 8) as the staged segments leave room for.
+template <uint32_t FMT, bool PAYLOAD>
+int launch_decode_lanes(const ContainerView &cv, void *out, cudaStream_t st, bool *launched) {
+  *launched = false;
+  if constexpr (decode_lanes_format(FMT)) {
+    if (!(cv.flags & ANSLIN_FLAG_LANE_STREAMS) || cv.tile_n != 32 || cv.units < 2 || cv.units % 2 || cv.n_tiles < 2) return ANSLIN_OK;
+    const uint32_t stream_bytes = uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32)));
+    uint32_t warps = kLaneDecWarps;
+    while (warps >= 8 && decode_lanes_smem(warps, stream_bytes) > kSmemMax) warps -= 4;
+    if (warps < 8) return ANSLIN_OK;
+    const size_t row_bytes = row_bytes_of(FMT, cv.k_in);
+    CUtensorMap tmo;
+    if (!make_map_2d(&tmo, out, 1, row_bytes, cv.n_out, row_bytes, 32, 32, CU_TENSOR_MAP_SWIZZLE_NONE)) return ANSLIN_ERR_CUDA;
+    auto kern = decode_lanes_kernel<FMT, PAYLOAD>;
+    static thread_local size_t smem_set_dev[kMaxDevices] = {};
+    size_t &smem_set = smem_set_dev[device_index()];
+    if (smem_set == 0) {
+      if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(kSmemMax)) != cudaSuccess) return ANSLIN_ERR_CUDA;
+      smem_set = kSmemMax;
+    }
+    const uint32_t jobs = cv.n_tiles / 2;
+    const uint32_t grid = std::min<uint32_t>(uint32_t(sm_budget()), jobs);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(warps * 32);
+    cfg.dynamicSmemBytes = decode_lanes_smem(warps, stream_bytes);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // launch latency and CTA set-up overlap the predecessor's tail
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    *launched = true;
+    if (cudaLaunchKernelEx(&cfg, kern, tmo, cv, stream_bytes) != cudaSuccess) return ANSLIN_ERR_CUDA;
+    return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
+  }
+  return ANSLIN_OK;
+}
+
 template <uint32_t FMT, bool PAYLOAD>
 int launch_decode(const ContainerView &cv, void *out, cudaStream_t st) {
+  bool launched = false;
+  const int rc = launch_decode_lanes<FMT, PAYLOAD>(cv, out, st, &launched);
+  if (rc != ANSLIN_OK || launched) return rc;
   if (cv.flags & ANSLIN_FLAG_LANE_STREAMS) return cv.tile_n == 32 ? launch_decode_t<FMT, 1, PAYLOAD, true>(cv, out, st) : int(ANSLIN_ERR_CORRUPT);
   return cv.tile_n == 32 ? launch_decode_t<FMT, 1, PAYLOAD, false>(cv, out, st) : launch_decode_t<FMT, 4, PAYLOAD, false>(cv, out, st);
 }
