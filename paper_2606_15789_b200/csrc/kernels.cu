@@ -1295,16 +1295,16 @@ int launch_decode_t(const ContainerView &cv, void *out, cudaStream_t st) {
   return cudaGetLastError() == cudaSuccess ? ANSLIN_OK : ANSLIN_ERR_CUDA;
 }
 // decode_lanes_kernel (decode_lanes.cuh) where the container allows it: lane streams, 32-row tiles, a unit of 32 bytes of W per
-// row, an even number of units per tile; as many decoder warps (16, 12 or 8) as the staged segments leave room for.
+// row, an even number of units per tile, staged segments small enough for 16 decoder warps.
 template <uint32_t FMT, bool PAYLOAD>
 int launch_decode_lanes(const ContainerView &cv, void *out, cudaStream_t st, bool *launched) {
   *launched = false;
   if constexpr (decode_lanes_format(FMT)) {
     if (!(cv.flags & ANSLIN_FLAG_LANE_STREAMS) || cv.tile_n != 32 || cv.units < 2 || cv.units % 2 || cv.n_tiles < 2) return ANSLIN_OK;
     const uint32_t stream_bytes = uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32)));
-    uint32_t warps = kLaneDecWarps;
-    while (warps >= 8 && decode_lanes_smem(warps, stream_bytes) > kSmemMax) warps -= 4;
-    if (warps < 8) return ANSLIN_OK;
+    // all 16 decoder warps or the old kernel: with fewer (int8: 4.7 KiB staged per segment) decode_kernel's 2 x 8 warps per SM win
+    const uint32_t warps = kLaneDecWarps;
+    if (decode_lanes_smem(warps, stream_bytes) > kSmemMax) return ANSLIN_OK;
     const size_t row_bytes = row_bytes_of(FMT, cv.k_in);
     CUtensorMap tmo;
     if (!make_map_2d(&tmo, out, 1, row_bytes, cv.n_out, row_bytes, 32, 32, CU_TENSOR_MAP_SWIZZLE_NONE)) return ANSLIN_ERR_CUDA;
