@@ -8,19 +8,25 @@
 //     no per-lane global store instruction, no transposition through shared memory, nothing on the LSU pipe but two STS.128
 //     per lane and unit (a lane-per-row STG.128 costs one L1 wavefront per row: 64 per unit and chain);
 //   * the boxes are double buffered per chain; cp.async.bulk.wait_group.read frees a box two units later.
-// Formats whose unit is 32 bytes of W per row: bf16 (16 weights), int8 / fp8 (32 weights).  Packed 4-bit formats, 128-row tiles
-// and interleaved words stay on decode_kernel.
+// Formats: bf16 (16 weights = 32 bytes per row and unit), int8 / fp8 (32 weights), and the packed 4-bit formats in their stored
+// packing (fp4: 16 bytes per unit; int4: 8, two units per box row).  128-row tiles, interleaved words and the bf16 pair variant
+// stay on decode_kernel.
 #pragma once
 
 constexpr int kLaneDecWarps = 16;
-constexpr uint32_t kOutBoxBytes = 1024;   // 32 rows x 32 bytes
 __host__ __device__ constexpr bool decode_lanes_format(uint32_t fmt) {
-  return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT8 || is_fp8(fmt);
+  return fmt == ANSLIN_FMT_BF16 || fmt == ANSLIN_FMT_INT8 || is_fp8(fmt) || is_packed4(fmt);
 }
-// shared memory from the 1024-byte aligned base: slot table 16 KiB | prefix scratch + warp barriers 2 KiB | per warp: raw 2 KiB |
-// out boxes 4 KiB | two staged segments
-__host__ __device__ constexpr size_t decode_lanes_smem(uint32_t warps, uint32_t stream_bytes) {
-  return 1024 + 18432 + size_t(warps) * (2 * kRawBufBytes + 4 * kOutBoxBytes + 2 * size_t(stream_bytes)) + 16;
+// bytes of row-major W a lane decodes per unit (bf16: 16 weights, int8 / fp8: 32, fp4: 32 codes = 16 bytes, int4: 16 codes = 8 bytes)
+// and bytes per box row: the TMA engine wants at least 16, so an int4 box row holds two units
+__host__ __device__ constexpr uint32_t decode_lanes_unit_bytes(uint32_t fmt) { return fmt == ANSLIN_FMT_INT4_AWQ ? 8u : fmt == ANSLIN_FMT_FP4_E2M1 ? 16u : 32u; }
+__host__ __device__ constexpr uint32_t decode_lanes_box_row(uint32_t fmt) { return is_packed4(fmt) ? 16u : 32u; }
+// shared memory from the 1024-byte aligned base: slot table 16 KiB | prefix scratch + warp barriers 2 KiB | per warp: raw 2 KiB
+// (bf16 only) | four out boxes (two chains, double buffered) | two staged segments
+__host__ __device__ constexpr uint32_t decode_lanes_raw_bytes(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16 ? 2u * kRawBufBytes : 0u; }
+__host__ __device__ constexpr uint32_t decode_lanes_box_bytes(uint32_t fmt) { return 32u * decode_lanes_box_row(fmt); }
+__host__ __device__ constexpr size_t decode_lanes_smem(uint32_t fmt, uint32_t warps, uint32_t stream_bytes) {
+  return 1024 + 18432 + size_t(warps) * (decode_lanes_raw_bytes(fmt) + 4 * decode_lanes_box_bytes(fmt) + 2 * size_t(stream_bytes)) + 16;
 }
 
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, uint32_t src, int c0, int c1) {
@@ -34,6 +40,7 @@ __global__ void __launch_bounds__(kLaneDecWarps * 32, 1) decode_lanes_kernel(con
                                                                              const uint32_t stream_bytes) {
   constexpr bool kRaw = FMT == ANSLIN_FMT_BF16;
   constexpr uint32_t kUnitsPerSeg = seg_steps_of(FMT) / unit_steps32(FMT);
+  constexpr uint32_t kUB = decode_lanes_unit_bytes(FMT);
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t *smem = smem_raw + (smem0 - smem_u32(smem_raw));
@@ -62,9 +69,10 @@ __global__ void __launch_bounds__(kLaneDecWarps * 32, 1) decode_lanes_kernel(con
   build_slot_table(tab, cum, freq_regs);   // ends with __syncthreads()
 
   const uint32_t tab_s = smem0, per_warp0 = smem0 + 18432;
-  const uint32_t rawbuf_s = per_warp0 + uint32_t(warp) * 2u * kRawBufBytes, rawlane_s = rawbuf_s + 16u * uint32_t(lane);
-  const uint32_t out_s = per_warp0 + W * 2u * kRawBufBytes + uint32_t(warp) * 4u * kOutBoxBytes;   // box (chain j, parity b) at (j * 2 + b) KiB
-  const uint32_t stage_s = per_warp0 + W * (2u * kRawBufBytes + 4u * kOutBoxBytes) + uint32_t(warp) * 2u * stream_bytes;
+  constexpr uint32_t kRawBytes = decode_lanes_raw_bytes(FMT), kOutBoxBytes = decode_lanes_box_bytes(FMT);
+  const uint32_t rawbuf_s = per_warp0 + uint32_t(warp) * kRawBytes, rawlane_s = rawbuf_s + 16u * uint32_t(lane);
+  const uint32_t out_s = per_warp0 + W * kRawBytes + uint32_t(warp) * 4u * kOutBoxBytes;   // box (chain j, parity b) at (j * 2 + b) boxes
+  const uint32_t stage_s = per_warp0 + W * (kRawBytes + 4u * kOutBoxBytes) + uint32_t(warp) * 2u * stream_bytes;
   const uint32_t dir = (lane & 1) ? uint32_t(-2) : 2u;
   const size_t rtb = raw_tile_bytes(32, cv.tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0);
   const uint32_t tile_row_bytes = uint32_t(row_bytes_of(FMT, cv.tile_k));
@@ -143,24 +151,49 @@ __global__ void __launch_bounds__(kLaneDecWarps * 32, 1) decode_lanes_kernel(con
         if constexpr (PAR == 1) { rawp[0] += 1024; rawp[1] += 1024; }
       }
       uint32_t r[2][8];
-      decode_half_regs<FMT, PAYLOAD, 0>(s, tab_s, dir, last_unit, rv, sz, r);
-      decode_half_regs<FMT, PAYLOAD, 1>(s, tab_s, dir, last_unit, rv, sz, r);
+      if constexpr (is_packed4(FMT)) {   // the stored packing: one coded byte = two 4-bit codes
+#pragma unroll
+        for (int h = 0; h < int(kUB / 4); ++h) {
+          uint32_t Bq[2];
+          decode4<LaneWords, 2>(s, Bq, tab_s, dir);
+          r[0][h] = Bq[0];
+          r[1][h] = Bq[1];
+        }
+      } else {
+        decode_half_regs<FMT, PAYLOAD, 0>(s, tab_s, dir, last_unit, rv, sz, r);
+        decode_half_regs<FMT, PAYLOAD, 1>(s, tab_s, dir, last_unit, rv, sz, r);
+      }
       // ---- registers -> shared-memory box -> TMA store ----
-      if (lane == 0) bulk_wait_read<1>();   // the stores of two units ago (this parity's boxes) have read their boxes
-      __syncwarp();
+      // box parity: the unit's (one box per unit) or the unit pair's (int4: two units fill one box row)
+      const uint32_t bpar = kUB == 8 ? ((u >> 1) & 1u) : PAR;
+      const bool first_of_box = kUB != 8 || PAR == 0, last_of_box = kUB != 8 || PAR == 1;
+      if (first_of_box) {
+        if (lane == 0) bulk_wait_read<1>();   // the stores that last used this parity's boxes have read them
+        __syncwarp();
+      }
 #pragma unroll
       for (int j = 0; j < 2; ++j) {
-        const uint32_t box = out_s + (uint32_t(j) * 2u + PAR) * kOutBoxBytes + box_lane;
-        const uint4 lo = make_uint4(r[j][0], r[j][1], r[j][2], r[j][3]), hi = make_uint4(r[j][4], r[j][5], r[j][6], r[j][7]);
-        sts128(box + (swap_halves ? 16u : 0u), swap_halves ? hi : lo);
-        sts128(box + (swap_halves ? 0u : 16u), swap_halves ? lo : hi);
+        const uint32_t box0 = out_s + (uint32_t(j) * 2u + bpar) * kOutBoxBytes;
+        if constexpr (kUB == 32) {
+          const uint32_t box = box0 + box_lane;
+          const uint4 lo = make_uint4(r[j][0], r[j][1], r[j][2], r[j][3]), hi = make_uint4(r[j][4], r[j][5], r[j][6], r[j][7]);
+          sts128(box + (swap_halves ? 16u : 0u), swap_halves ? hi : lo);
+          sts128(box + (swap_halves ? 0u : 16u), swap_halves ? lo : hi);
+        } else if constexpr (kUB == 16) {
+          sts128(box0 + uint32_t(lane) * 16u, make_uint4(r[j][0], r[j][1], r[j][2], r[j][3]));
+        } else {
+          asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(box0 + uint32_t(lane) * 16u + PAR * 8u), "r"(r[j][0]), "r"(r[j][1]) : "memory");
+        }
       }
-      fence_proxy_async();   // generic-proxy stores -> visible to the TMA engine's async proxy
-      __syncwarp();
-      if (lane == 0) {
+      if (last_of_box) {
+        fence_proxy_async();   // generic-proxy stores -> visible to the TMA engine's async proxy
+        __syncwarp();
+        if (lane == 0) {
+          const int col = col0 + int((kUB == 8 ? (u & ~1u) : u) * kUB);
 #pragma unroll
-        for (int j = 0; j < 2; ++j) tma_store_2d(&tmo, out_s + (uint32_t(j) * 2u + PAR) * kOutBoxBytes, col0 + int(u * 32u), row0 + 32 * j);
-        bulk_commit();
+          for (int j = 0; j < 2; ++j) tma_store_2d(&tmo, out_s + (uint32_t(j) * 2u + bpar) * kOutBoxBytes, col, row0 + 32 * j);
+          bulk_commit();
+        }
       }
     };
 #pragma unroll 1

@@ -1304,10 +1304,10 @@ int launch_decode_lanes(const ContainerView &cv, void *out, cudaStream_t st, boo
     const uint32_t stream_bytes = uint32_t(align16(std::max<uint32_t>(cv.max_seg_bytes, 32)));
     // all 16 decoder warps or the old kernel: with fewer (int8: 4.7 KiB staged per segment) decode_kernel's 2 x 8 warps per SM win
     const uint32_t warps = kLaneDecWarps;
-    if (decode_lanes_smem(warps, stream_bytes) > kSmemMax) return ANSLIN_OK;
+    if (decode_lanes_smem(FMT, warps, stream_bytes) > kSmemMax) return ANSLIN_OK;
     const size_t row_bytes = row_bytes_of(FMT, cv.k_in);
     CUtensorMap tmo;
-    if (!make_map_2d(&tmo, out, 1, row_bytes, cv.n_out, row_bytes, 32, 32, CU_TENSOR_MAP_SWIZZLE_NONE)) return ANSLIN_ERR_CUDA;
+    if (!make_map_2d(&tmo, out, 1, row_bytes, cv.n_out, row_bytes, decode_lanes_box_row(FMT), 32, CU_TENSOR_MAP_SWIZZLE_NONE)) return ANSLIN_ERR_CUDA;
     auto kern = decode_lanes_kernel<FMT, PAYLOAD>;
     static thread_local size_t smem_set_dev[kMaxDevices] = {};
     size_t &smem_set = smem_set_dev[device_index()];
@@ -1320,7 +1320,7 @@ int launch_decode_lanes(const ContainerView &cv, void *out, cudaStream_t st, boo
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(warps * 32);
-    cfg.dynamicSmemBytes = decode_lanes_smem(warps, stream_bytes);
+    cfg.dynamicSmemBytes = decode_lanes_smem(FMT, warps, stream_bytes);
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // launch latency and CTA set-up overlap the predecessor's tail
