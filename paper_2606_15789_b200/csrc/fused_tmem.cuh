@@ -29,7 +29,7 @@ constexpr int kMaxTeams = 4;
 constexpr int kTmemThreads = 32 * (kTeamWarps + 1) * kMaxTeams;   // 16 decoder warps + one issuer warp per team = 640: up to 96 registers
 constexpr uint32_t kACols = 8;                               // TMEM columns of one operand unit (32 bytes per row)
 constexpr uint32_t kASlotCols = 4 * kACols;                  // per team: two operand units (one per chain), double buffered
-constexpr uint32_t kXDepth = 3;                              // X ring slots per team (each: the two slices of one unit step)
+constexpr uint32_t kXDepth = 3;                              // X ring slots per team (each: the two slices of one unit step); 2 where shared memory is short
 constexpr uint32_t kNT = 32 * kTeamWarps;                    // threads of a team
 
 // shared-memory carve-up, from the 1024-byte aligned base: slot table | prefix scratch | barriers | X rings | raw | staging
@@ -39,8 +39,10 @@ constexpr uint32_t kTmWarpBarOff = kTmPtrOff + 16;             // one mbarrier p
 constexpr uint32_t kTmXOff = 18432;
 constexpr uint32_t kRawBufBytes = 1024;                      // bf16: two 512-byte raw vectors per chain
 __host__ __device__ constexpr bool tmem_has_raw(uint32_t fmt) { return fmt == ANSLIN_FMT_BF16; }
-__host__ __device__ constexpr size_t tmem_smem_bytes(uint32_t T, uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
-  return 1024 /*align slack*/ + kTmXOff + size_t(T) * kXDepth * 2 * mpad_max * 32 + (tmem_has_raw(fmt) ? size_t(T) * kTeamWarps * 2 * kRawBufBytes : 0) +
+// xslices: X slices per ring slot = k-tiles per work item (2, or 1 for the kernel's J = 1)
+__host__ __device__ constexpr size_t tmem_smem_bytes(uint32_t T, uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt, uint32_t xdepth = kXDepth,
+                                                     uint32_t xslices = 2) {
+  return 1024 /*align slack*/ + kTmXOff + size_t(T) * xdepth * xslices * mpad_max * 32 + (tmem_has_raw(fmt) ? size_t(T) * kTeamWarps * 2 * kRawBufBytes : 0) +
          size_t(T) * kTeamWarps * 2 * stream_bytes + 16;
 }
 // split-K control words of a problem (its flag area): u32 flag[2 * teams][PK], one word per (partial slot, reader)
@@ -55,6 +57,7 @@ struct TmemParams {
   uint32_t xslice_bytes;   // max mpad * 32
   uint32_t tmem_stride;    // TMEM columns per team: max mpad + kASlotCols
   uint32_t afmt, bfmt;
+  uint32_t xdepth;         // X ring slots per team: 3, or 2
 };
 
 __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8]) {
@@ -114,26 +117,26 @@ __device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void *src, uin
 // waiting for the segment table (bufbytes <= kTailBytes): ONE bulk copy per record, issued by lane 0 and completed on the
 // warp's mbarrier `bar` (phase `parity`), instead of six 16-byte cp.async per lane and record.
 // extra(): cp.async copies of the caller (first raw vectors), waited for here too.
-template <class Extra>
-__device__ __forceinline__ void lane_open_segments_bulk(LaneStream (&s)[2], uint32_t buf0, uint32_t bufbytes, int seg, int lane, uint32_t bar,
+template <class Extra, int J>
+__device__ __forceinline__ void lane_open_segments_bulk(LaneStream (&s)[J], uint32_t buf0, uint32_t bufbytes, int seg, int lane, uint32_t bar,
                                                         uint32_t parity, const Extra &extra) {
   __syncwarp();   // every lane is done with the words of the previous segments
-  uint32_t hdr[2], delta[2];
+  uint32_t hdr[J], delta[J];
 #pragma unroll
-  for (int j = 0; j < 2; ++j) {
+  for (int j = 0; j < J; ++j) {
     const uint8_t *te = s[j].rec + 4 * kLanes + kSegTableBytes * seg;
     hdr[j] = *reinterpret_cast<const uint32_t *>(te);   // u16 base | u16 total words
     delta[j] = lane < kLanes / 2 ? uint32_t(te[4 + lane]) : 0u;
   }
   if (lane == 0) {
-    mbar_arrive_expect_tx(bar, 2u * bufbytes);
+    mbar_arrive_expect_tx(bar, uint32_t(J) * bufbytes);
 #pragma unroll
-    for (int j = 0; j < 2; ++j) bulk_copy_g2s(buf0 + uint32_t(j) * bufbytes, s[j].rec + (s[j].goff & ~15u), bufbytes, bar);
+    for (int j = 0; j < J; ++j) bulk_copy_g2s(buf0 + uint32_t(j) * bufbytes, s[j].rec + (s[j].goff & ~15u), bufbytes, bar);
   }
   extra();
   cp_async_commit();
 #pragma unroll
-  for (int j = 0; j < 2; ++j) {
+  for (int j = 0; j < J; ++j) {
     const uint32_t base = hdr[j] & 0xFFFFu, total = hdr[j] >> 16, buf = buf0 + uint32_t(j) * bufbytes;
     const uint32_t size = lane < kLanes / 2 ? base + delta[j] : 0u;   // words of region `lane`
     uint32_t end = size;
@@ -152,38 +155,38 @@ __device__ __forceinline__ void lane_open_segments_bulk(LaneStream (&s)[2], uint
   cp_async_wait_all();
   mbar_wait(bar, parity);
 #pragma unroll
-  for (int j = 0; j < 2; ++j) asm volatile("ld.shared.u16 %0, [%1];" : "=r"(s[j].w) : "r"(s[j].ptr) : "memory");
+  for (int j = 0; j < J; ++j) asm volatile("ld.shared.u16 %0, [%1];" : "=r"(s[j].w) : "r"(s[j].ptr) : "memory");
 }
 
 // Half H (0 / 1) of one operand unit (32 operand bytes per row = 8 registers) of the warp's two tiles: registers
 // r[j][4H .. 4H+3].  rv[j]: bf16: the unit's 16 raw (sign | mantissa) bytes of this lane.  sz[j]: int4: this lane's (scale, zero)
 // pair of the unit's quantisation group.  The unit is cut in two so that its housekeeping (hand-over of the previous unit,
 // the next unit's raw bytes, the operand-free probe) sits between the halves, where its latencies overlap decode steps.
-template <uint32_t FMT, bool PAYLOAD, int H>
-__device__ __forceinline__ void decode_half_regs(LaneStream (&s)[2], uint32_t tab_s, uint32_t dir, bool last_unit, const uint4 (&rv)[2],
-                                                 const uint32_t (&sz)[2], uint32_t (&r)[2][8]) {
+template <uint32_t FMT, bool PAYLOAD, int H, int J>
+__device__ __forceinline__ void decode_half_regs(LaneStream (&s)[J], uint32_t tab_s, uint32_t dir, bool last_unit, const uint4 (&rv)[J],
+                                                 const uint32_t (&sz)[J], uint32_t (&r)[J][8]) {
   static_assert(FMT != ANSLIN_FMT_BF16_PAIR4, "the pair variant runs on the shared-memory operand path");
   if constexpr (FMT == ANSLIN_FMT_BF16) {
-    uint32_t R0[2], R1[2];
-    if (H == 0) { R0[0] = rv[0].x; R0[1] = rv[1].x; R1[0] = rv[0].y; R1[1] = rv[1].y; }
-    else { R0[0] = rv[0].z; R0[1] = rv[1].z; R1[0] = rv[0].w; R1[1] = rv[1].w; }
-    uint4 o[2];
-    decode8_bf16<LaneWords, 2>(s, tab_s, dir, R0, R1, o);
+    uint32_t R0[J], R1[J];
+    #pragma unroll
+    for (int j = 0; j < J; ++j) { R0[j] = H == 0 ? rv[j].x : rv[j].z; R1[j] = H == 0 ? rv[j].y : rv[j].w; }
+    uint4 o[J];
+    decode8_bf16<LaneWords, J>(s, tab_s, dir, R0, R1, o);
     if (H == 1 && PAYLOAD && last_unit) {
       // raw bytes 14, 15 of the tile's last vector ride in the END state (A4): merge them in now
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < J; ++j) {
         const uint32_t pl = s[j].x - kL;   // byte 14 | byte 15 << 8, each = mantissa << 1 | sign
         o[j].w |= ((pl >> 1) & 0x7Fu) | ((pl & 1u) << 15) | (((pl >> 9) & 0x7Fu) << 16) | (((pl >> 8) & 1u) << 31);
       }
     }
 #pragma unroll
-    for (int j = 0; j < 2; ++j) { r[j][4 * H] = o[j].x; r[j][4 * H + 1] = o[j].y; r[j][4 * H + 2] = o[j].z; r[j][4 * H + 3] = o[j].w; }
+    for (int j = 0; j < J; ++j) { r[j][4 * H] = o[j].x; r[j][4 * H + 1] = o[j].y; r[j][4 * H + 2] = o[j].z; r[j][4 * H + 3] = o[j].w; }
   } else if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
-    uint32_t Bq[2];
-    decode4<LaneWords, 2>(s, Bq, tab_s, dir);
+    uint32_t Bq[J];
+    decode4<LaneWords, J>(s, Bq, tab_s, dir);
 #pragma unroll
-    for (int j = 0; j < 2; ++j) {
+    for (int j = 0; j < J; ++j) {
       const __half2 szh = *reinterpret_cast<const __half2 *>(&sz[j]);
       const __half2 sc = __half2half2(__low2half(szh));
       const __half2 zoff = __hadd2(__half2half2(__high2half(szh)), __float2half2_rn(1024.f));
@@ -193,18 +196,18 @@ __device__ __forceinline__ void decode_half_regs(LaneStream (&s)[2], uint32_t ta
   } else if constexpr (FMT == ANSLIN_FMT_FP4_E2M1) {
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      uint32_t Bq[2];
-      decode4<LaneWords, 2>(s, Bq, tab_s, dir);
+      uint32_t Bq[J];
+      decode4<LaneWords, J>(s, Bq, tab_s, dir);
 #pragma unroll
-      for (int j = 0; j < 2; ++j) e2m1x8_to_e4m3(Bq[j], r[j][4 * H + 2 * h], r[j][4 * H + 2 * h + 1]);
+      for (int j = 0; j < J; ++j) e2m1x8_to_e4m3(Bq[j], r[j][4 * H + 2 * h], r[j][4 * H + 2 * h + 1]);
     }
   } else {   // fp8 / int8: the symbol byte is the operand byte
 #pragma unroll
     for (int h = 0; h < 4; ++h) {
-      uint32_t q[2];
-      decode4<LaneWords, 2>(s, q, tab_s, dir);
-      r[0][4 * H + h] = q[0];
-      r[1][4 * H + h] = q[1];
+      uint32_t q[J];
+      decode4<LaneWords, J>(s, q, tab_s, dir);
+#pragma unroll
+      for (int j = 0; j < J; ++j) r[j][4 * H + h] = q[j];
     }
   }
 }
@@ -371,7 +374,10 @@ __device__ __forceinline__ void team_reduce(const EpiParams &p, const TeamMap &t
   RTRACE(6);
 }
 
-template <uint32_t FMT, bool PAYLOAD, bool YB>
+// J = 2: a work item is a PAIR of k-tiles of one stripe, a warp interleaves the two (throughput: the default).  J = 1: a work item
+// is ONE k-tile and a warp runs one chain at its latency: for launches with at most one tile per team, whose duration is the
+// sequential length of an item (32 x 1024 int8 tiles of a 13824 x 5120 matrix; a 1024 x 5120 projection on its own).
+template <uint32_t FMT, bool PAYLOAD, bool YB, int J = 2>
 __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __grid_constant__ TensorMaps tms,
                                                                       const __grid_constant__ TmemParams P) {
   using TR = FmtTraits<FMT>;
@@ -401,12 +407,13 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   uint32_t *cum = reinterpret_cast<uint32_t *>(smem + 16384);
   const uint32_t bars_s = smem0 + kTmBarOff;   // per team: done[2] +0, xfull[3] +16, accfull +40, full[2] +48
   volatile uint32_t *tmemptr = reinterpret_cast<volatile uint32_t *>(smem + kTmPtrOff);
-  const uint32_t raw_off = kTmXOff + T * kXDepth * 2u * P.xslice_bytes;
+  const uint32_t XD = P.xdepth;
+  const uint32_t raw_off = kTmXOff + T * XD * uint32_t(J) * P.xslice_bytes;
   const uint32_t stage_off = raw_off + (kRaw ? T * kTeamWarps * 2u * kRawBufBytes : 0u);
 
   // stream-K split over TEAMS (TeamMap): team v owns pairs [first(v), first(v+1)) of the stripe-major sequence of
   // (stripe, k-tile pair) items
-  const uint32_t PK = (KT + 1) / 2, stripes = n_out / kTileN, Ptot = stripes * PK;
+  const uint32_t PK = (KT + J - 1) / J, stripes = n_out / kTileN, Ptot = stripes * PK;   // items per stripe
   const TeamMap tm{G, T, Ptot};
   const bool decoder = uint32_t(warp) < kTeamWarps * T;
   const uint32_t v = c * T + (decoder ? team : 0u);
@@ -414,13 +421,13 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
   const uint32_t *offs = reinterpret_cast<const uint32_t *>(cbase + pr.cv.off_offsets);
   // the frequency table and the record offsets of this warp's first pair of tiles: one HBM round trip for both
   const uint4 freq_regs = slot_table_load(reinterpret_cast<const uint16_t *>(cbase + pr.cv.off_freq));
-  uint32_t cur_off[2] = {0, 0};
+  uint32_t cur_off[J] = {};
   if (p_begin < p_end) {
-    const uint32_t s0 = p_begin / PK, k0 = 2u * (p_begin % PK), t0 = (s0 * KT + k0) * 4u + q;
+    const uint32_t s0 = p_begin / PK, k0 = uint32_t(J) * (p_begin % PK), t0 = (s0 * KT + k0) * 4u + q;
     cur_off[0] = offs[t0];
-    cur_off[1] = offs[t0 + (k0 + 1 < KT ? 4u : 0u)];
+    if constexpr (J == 2) cur_off[1] = offs[t0 + (k0 + 1 < KT ? 4u : 0u)];
 #pragma unroll
-    for (int j = 0; j < 2; ++j) {   // ... and the records themselves (and their raw bytes) on their way into L2
+    for (int j = 0; j < J; ++j) {   // ... and the records themselves (and their raw bytes) on their way into L2
       if (lane < 24) prefetch_l2(cbase + off_records + size_t(cur_off[j]) * 16 + lane * 128);
       else if (tmem_has_raw(FMT))
         prefetch_l2(cbase + off_raw + size_t(t0 + (j && k0 + 1 < KT ? 4u : 0u)) * raw_tile_bytes(32, tile_k, PAYLOAD ? ANSLIN_FLAG_STATE_PAYLOAD : 0) + (lane - 24) * 128);
@@ -463,27 +470,26 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
     const uint32_t it = uint32_t(warp) - kTeamWarps * T, vt = c * T + it;
     const uint32_t pb = tm.first(vt), pe = tm.first(vt + 1), Nt = (pe - pb) * units;
     const uint32_t bt = bars_s + 64 * it, acc = tmem_base + it * P.tmem_stride, at = acc + mpad;
-    const uint32_t xr = smem0 + kTmXOff + it * kXDepth * 2u * P.xslice_bytes;   // ring slot sx, slice j at (sx * 2 + j) * xslice_bytes
+    const uint32_t xr = smem0 + kTmXOff + it * XD * uint32_t(J) * P.xslice_bytes;   // ring slot sx, slice j at (sx * J + j) * xslice_bytes
     const uint64_t bdesc0 = make_smem_desc(xr, 16, 256, kLayoutSW32);
     const uint32_t bdesc_step = P.xslice_bytes >> 4;
     const bool leader = elect_one_sync();
     uint32_t kpx = pb % PK, ux = 0, sxx = 0, nx = 0;   // X request cursor: pair in stripe, unit, ring slot, unit step
     auto request_x = [&]() {   // the two X slices of unit step nx
       if (leader) {
-        const uint32_t ktA = 2u * kpx, bar = bt + 16 + 8 * sxx;
-        const bool hasB = ktA + 1 < KT;
+        const uint32_t ktA = uint32_t(J) * kpx, bar = bt + 16 + 8 * sxx;
+        const bool hasB = J == 2 && ktA + 1 < KT;
         const int kA = int(ktA * tile_k + ux * kUnitK);
         mbar_arrive_expect_tx(bar, hasB ? 2 * xbytes : xbytes);
-        tma_load_2d(xr + (sxx * 2u) * P.xslice_bytes, xmap, kA, 0, bar);
-        if (hasB) tma_load_2d(xr + (sxx * 2u + 1u) * P.xslice_bytes, xmap, kA + int(tile_k), 0, bar);
+        tma_load_2d(xr + (sxx * uint32_t(J)) * P.xslice_bytes, xmap, kA, 0, bar);
+        if (hasB) tma_load_2d(xr + (sxx * uint32_t(J) + 1u) * P.xslice_bytes, xmap, kA + int(tile_k), 0, bar);
       }
       ++nx;
-      if (++sxx == kXDepth) sxx = 0;
+      if (++sxx == XD) sxx = 0;
       if (++ux == units) { ux = 0; if (++kpx == PK) kpx = 0; }
     };
     grid_dep_wait();   // X belongs to the stream's earlier kernels until they are done
-    if (Nt > 0) request_x();
-    if (Nt > 1) request_x();
+    for (uint32_t i = 0; i + 1 < XD && i < Nt; ++i) request_x();   // XD - 1 unit steps ahead
     uint32_t pp = pb, kp = pb % PK, u = 0, sx = 0, xpar = 0;
 #pragma unroll 1
     for (uint32_t n = 0; n < Nt; ++n) {
@@ -491,19 +497,19 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       mbar_wait_relaxed(bt + 48 + 8 * sa, (n >> 1) & 1u, 250);   // all four decoder warps have stored this step's operand columns
       mbar_wait_relaxed(bt + 16 + 8 * sx, xpar, 100);            // its X slices have landed
       tc_fence_after();
-      const bool hasB = 2u * kp + 1 < KT, last_unit = u + 1 == units;
+      const bool hasB = J == 2 && 2u * kp + 1 < KT, last_unit = u + 1 == units;
       const bool seg_first = u == 0 && (pp == pb || kp == 0), seg_last = last_unit && (pp + 1 == pe || kp + 1 == PK);
       if (leader) {
-        const uint64_t bdA = bdesc0 + uint64_t(sx * 2u * bdesc_step);
+        const uint64_t bdA = bdesc0 + uint64_t(sx * uint32_t(J) * bdesc_step);
         umma_ts<TR::kind>(acc, at + sa * 2u * kACols, bdA, idesc, seg_first ? 0u : 1u);
         if (hasB) umma_ts<TR::kind>(acc, at + sa * 2u * kACols + kACols, bdA + bdesc_step, idesc, 1u);
         umma_commit(bt + 8 * sa);
         if (seg_last) umma_commit(bt + 40);
       }
       __syncwarp();
-      if (++sx == kXDepth) { sx = 0; xpar ^= 1u; }
+      if (++sx == XD) { sx = 0; xpar ^= 1u; }
       if (last_unit) { u = 0; ++pp; if (++kp == PK) kp = 0; } else ++u;
-      // the X slices of step n + 2 go to the ring slot last read by the MMAs of step n - 1 (issued one step ago)
+      // the X slices of step n + XD - 1 go to the ring slot last read by the MMAs of step n - 1 (issued one step ago)
       if (nx < Nt) {
         if (n >= 1) mbar_wait_relaxed(bt + 8 * ((n - 1) & 1u), ((n - 1) >> 1) & 1u, 100);
         request_x();
@@ -551,27 +557,27 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
     const bool whole = kp0 == 0 && np == PK;
 #pragma unroll 1
     for (uint32_t i = 0; i < np; ++i) {
-      const uint32_t ktA = 2u * (kp0 + i);
-      const bool hasB = ktA + 1 < KT;
-      LaneStream s[2];
-      uint32_t tile[2];
+      const uint32_t ktA = uint32_t(J) * (kp0 + i);
+      const bool hasB = J == 2 && ktA + 1 < KT;
+      LaneStream s[J];
+      uint32_t tile[J];
       tile[0] = (stripe * KT + ktA) * 4u + q;
-      tile[1] = hasB ? tile[0] + 4u : tile[0];   // odd KT: the second chain re-decodes the first tile; its output is never multiplied
-      const uint8_t *rawp[2] = {nullptr, nullptr};   // this lane's 16 bytes of the NEXT raw vector to fetch
+      if constexpr (J == 2) tile[1] = hasB ? tile[0] + 4u : tile[0];   // odd KT: the second chain re-decodes the first tile; its output is never multiplied
+      const uint8_t *rawp[J] = {};   // this lane's 16 bytes of the NEXT raw vector to fetch
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < J; ++j) {
         const uint8_t *rec = cbase + off_records + size_t(cur_off[j]) * 16;
         lane_open(s[j], rec, int(units / kUnitsPerSeg), lane);
         if (kRaw) rawp[j] = cbase + off_raw + size_t(tile[j]) * rtb + 16 * lane;
       }
       // the records of this warp's next pair: pulled into L2 during the first unit
       const bool has_next = p + i + 1 < p_end;
-      uint32_t next_tile = 0, next_off[2] = {0, 0};
+      uint32_t next_tile = 0, next_off[J] = {};
       if (has_next) {
-        const uint32_t pn = p + i + 1, sn = pn / PK, kn = 2u * (pn % PK);
+        const uint32_t pn = p + i + 1, sn = pn / PK, kn = uint32_t(J) * (pn % PK);
         next_tile = (sn * KT + kn) * 4u + q;
         next_off[0] = offs[next_tile];
-        next_off[1] = offs[next_tile + (kn + 1 < KT ? 4u : 0u)];
+        if constexpr (J == 2) next_off[1] = offs[next_tile + (kn + 1 < KT ? 4u : 0u)];
       }
       // One unit of both tiles.  A tile has an even number of units (tmem_eligible), so the parity PAR of a unit step — which
       // half of the operand columns, which raw buffer, which barriers — is a compile-time constant of each copy of the body.
@@ -580,7 +586,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         if constexpr (PAR == 1) {
           if (u == 1 && has_next) {
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+            for (int j = 0; j < J; ++j) {
               if (lane < 24) prefetch_l2(cbase + off_records + size_t(next_off[j]) * 16 + lane * 128);
               else if (kRaw) prefetch_l2(cbase + off_raw + size_t(next_tile + 4u * uint32_t(j)) * rtb + (lane - 24) * 128);
               cur_off[j] = next_off[j];   // the next pair opens without another look at the offset table
@@ -593,14 +599,14 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
             auto first_raw = [&]() {
               if (kRawOn && u == 0) {
 #pragma unroll
-                for (int j = 0; j < 2; ++j) { cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes, rawp[j]); rawp[j] += 512; }
+                for (int j = 0; j < J; ++j) { cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes, rawp[j]); rawp[j] += 512; }
               }
             };
             if (P.stream_bytes <= uint32_t(kTailBytes)) {
               lane_open_segments_bulk(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane, warpbar_s, open_par, first_raw);
               open_par ^= 1u;
             } else {
-              lane_open_segments<2>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane, first_raw);
+              lane_open_segments<J>(s, stage_s, P.stream_bytes, int(u / kUnitsPerSeg), lane, first_raw);
             }
           }
           if (u == 0) PROF(4);
@@ -610,8 +616,10 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
           }
         }
         const bool last_unit = PAR == 1 && u + 1 == units;
-        uint4 rv[2] = {make_uint4(0, 0, 0, 0), make_uint4(0, 0, 0, 0)};
-        uint32_t sz[2] = {0, 0};
+        uint4 rv[J];
+        uint32_t sz[J];
+#pragma unroll
+        for (int j = 0; j < J; ++j) { rv[j] = make_uint4(0, 0, 0, 0); sz[j] = 0; }
         if constexpr (kRawOn) {
           // this unit's raw vector was copied during the previous unit; fetch the next one into the other buffer.
           // rawp[j]: at an even unit the next vector, at an odd unit the one before it (advanced by two vectors at a time)
@@ -623,7 +631,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
             // last vector with the state-payload flag: 7 sub-rows of 32 x 2 bytes (bytes 14, 15 come from the end state)
             __syncwarp();
 #pragma unroll
-            for (int j = 0; j < 2; ++j) {
+            for (int j = 0; j < J; ++j) {
               uint32_t h[7];
 #pragma unroll
               for (int k = 0; k < 7; ++k)
@@ -632,21 +640,24 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
             }
           } else {
 #pragma unroll
-            for (int j = 0; j < 2; ++j) rv[j] = lds128(rb + uint32_t(j) * kRawBufBytes);
+            for (int j = 0; j < J; ++j) rv[j] = lds128(rb + uint32_t(j) * kRawBufBytes);
           }
           if (!last_unit) {
             const bool short_vec = PAYLOAD && PAR == 0 && u + 2 == units;   // the next vector is the payload-shortened one: 448 bytes
             if (!short_vec || lane < 28) {
 #pragma unroll
-              for (int j = 0; j < 2; ++j) cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes + (PAR ^ 1u) * 512u, rawp[j] + PAR * 512u);
+              for (int j = 0; j < J; ++j) cp_async16(rawlane_s + uint32_t(j) * kRawBufBytes + (PAR ^ 1u) * 512u, rawp[j] + PAR * 512u);
             }
             cp_async_commit();
           }
-          if constexpr (PAR == 1) { rawp[0] += 1024; rawp[1] += 1024; }
+          if constexpr (PAR == 1) {
+#pragma unroll
+            for (int j = 0; j < J; ++j) rawp[j] += 1024;
+          }
         }
         if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
 #pragma unroll
-          for (int j = 0; j < 2; ++j) {
+          for (int j = 0; j < J; ++j) {
             const uint32_t k_elem = (ktA + uint32_t(j)) * tile_k + u * kUnitK;
             sz[j] = __ldg(reinterpret_cast<const uint32_t *>(cbase + off_scales) + size_t(k_elem / qgroup) * n_out + size_t(stripe) * kTileN +
                           q * 32u + uint32_t(lane));
@@ -655,14 +666,14 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         // have the MMAs that read this half of the operand columns two steps ago finished?  (On fresh barriers the parity
         // of the "previous" phase passes at once.)  Asked now, needed after the unit is decoded.
         const bool slot_free = mbar_test(done_s + 8 * PAR, kpar ^ 1u);
-        uint32_t r[2][8];
+        uint32_t r[J][8];
 #ifdef ANSLIN_TRACE
         if (blockIdx.x == 7 && lane == 0 && n + PAR < 48) g_prof[160 * kMaxTeams * 4 * 8 - 4 * 4 * 48 + ((team * 4 + q) * 48 + n + PAR)] = gtimer();
 #endif
         PROF(0);
 #ifdef ANSLIN_SKEL_NO_DECODE   // timing experiment only (wrong results): everything but the rANS steps
 #pragma unroll
-        for (int k = 0; k < 8; ++k) { r[0][k] = rv[0].x + k; r[1][k] = rv[1].y ^ k; }
+        for (int k = 0; k < 8; ++k) { r[0][k] = rv[0].x + k; r[J - 1][k] = rv[J - 1].y ^ k; }
         finish_handover(full_s + 8 * (PAR ^ 1u));
 #else
         decode_half_regs<FMT, PAYLOAD, 0>(s, tab_s, dir, last_unit, rv, sz, r);
@@ -675,10 +686,10 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         if (!slot_free) mbar_wait(done_s + 8 * PAR, kpar ^ 1u);
         PROF(2);
 #ifdef ANSLIN_SKEL_NO_STTM   // timing experiment only (wrong results): how much do the tensor-memory stores cost
-        if (r[0][0] == 0x12345678u && r[1][7] == 0x9abcdef0u && r[0][3] == 1u && r[1][2] == 7u) {
+        if (r[0][0] == 0x12345678u && r[J - 1][7] == 0x9abcdef0u && r[0][3] == 1u && r[J - 1][2] == 7u) {
 #endif
         tmem_st8(a_t + PAR * 2u * kACols + lane_t, r[0]);
-        tmem_st8(a_t + PAR * 2u * kACols + kACols + lane_t, r[1]);
+        if constexpr (J == 2) tmem_st8(a_t + PAR * 2u * kACols + kACols + lane_t, r[J - 1]);
 #ifdef ANSLIN_SKEL_NO_STTM
         }
 #endif
@@ -696,7 +707,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
       }
 #ifdef ANSLIN_BOUNDS_CHECK   // debug builds (compute-sanitizer is closed on this pool): every word cursor ended inside its staged buffer
 #pragma unroll
-      for (int j = 0; j < 2; ++j) {
+      for (int j = 0; j < J; ++j) {
         const uint32_t lo = stage_s + uint32_t(j) * P.stream_bytes;
         if (s[j].ptr + 2u < lo || s[j].ptr > lo + P.stream_bytes) __trap();
         if (PAYLOAD && (s[j].x < kL || s[j].x >= 2u * kL)) __trap();   // the end state is L + payload

@@ -974,7 +974,7 @@ uint32_t next_epoch() {
 // bytes of a problem's split-K flag area: the shared-memory design keeps two u32 flags per CTA and a u64 counter per stripe,
 // the tensor-memory design one u32 flag per (partial slot of a team, reader) = kTmFlagSlots x pairs per stripe
 size_t flag_bytes(const Header &h) {
-  const size_t stripes = h.n_out / kTileN, pk = (h.k_in / h.tile_k + 1) / 2;
+  const size_t stripes = h.n_out / kTileN, pk = h.k_in / h.tile_k;   // items per stripe: k-tile pairs, or single k-tiles (J = 1)
   return align16(std::max(stripes * 8 + 256 + 8 * 160 * kMaxTeams, kTmFlagSlots * pk * 4));
 }
 struct Workspace { size_t counters_off, partials_off, total; };
@@ -1021,20 +1021,26 @@ int launch_fused_y(const TensorMaps &tms, const FusedParams &p, uint32_t grid, s
 
 // Teams per CTA of the TMEM design (fused_tmem.cuh) for the largest padded batch of a launch and the staged segment size:
 // bounded by tensor memory (mpad accumulator + 16 operand columns per team) and by shared memory; 0 = does not fit.
-uint32_t tmem_teams(uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt) {
+uint32_t tmem_teams(uint32_t mpad_max, uint32_t stream_bytes, uint32_t fmt, uint32_t *xdepth = nullptr, uint32_t xslices = 2) {
   uint32_t T = std::min<uint32_t>(kMaxTeams, 512u / (mpad_max + kASlotCols));
-  while (T > 0 && tmem_smem_bytes(T, mpad_max, stream_bytes, fmt) > kSmemMax) --T;
-  return T;
+  for (; T > 0; --T)   // as many teams as tensor memory allows, with a 3-deep X ring if shared memory has room for it, else 2-deep
+    for (uint32_t d = kXDepth; d >= 2; --d)
+      if (tmem_smem_bytes(T, mpad_max, stream_bytes, fmt, d, xslices) <= kSmemMax) {
+        if (xdepth) *xdepth = d;
+        return T;
+      }
+  if (xdepth) *xdepth = kXDepth;
+  return 0;
 }
 bool tmem_eligible(const Header &h) {
   return (h.flags & ANSLIN_FLAG_LANE_STREAMS) && h.tile_n == 32 && h.format != ANSLIN_FMT_BF16_PAIR4 && h.tile_k / unit_k_of(h.format) >= 2 && (h.tile_k / unit_k_of(h.format)) % 2 == 0 &&   // units come in pairs
         
-         uint64_t(h.n_out / kTileN) * ((h.k_in / h.tile_k + 1) / 2) < (1u << 22);   // 32-bit split arithmetic in TeamMap
+         uint64_t(h.n_out / kTileN) * (h.k_in / h.tile_k) < (1u << 22);   // 32-bit split arithmetic in TeamMap
 }
 
-template <uint32_t FMT, bool PAYLOAD, bool YB>
+template <uint32_t FMT, bool PAYLOAD, bool YB, int J = 2>
 int launch_tmem_y(const TensorMaps &tms, const TmemParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
-  auto kern = fused_tmem_kernel<FMT, PAYLOAD, YB>;
+  auto kern = fused_tmem_kernel<FMT, PAYLOAD, YB, J>;
   static thread_local size_t smem_set_dev[kMaxDevices] = {};
   size_t &smem_set = smem_set_dev[device_index()];
   if (smem > smem_set) {
@@ -1057,6 +1063,11 @@ int launch_tmem_y(const TensorMaps &tms, const TmemParams &p, uint32_t grid, siz
 template <uint32_t FMT, bool PAYLOAD>
 int launch_tmem(bool ybf, const TensorMaps &tms, const TmemParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
   return ybf ? launch_tmem_y<FMT, PAYLOAD, true>(tms, p, grid, smem, st) : launch_tmem_y<FMT, PAYLOAD, false>(tms, p, grid, smem, st);
+}
+// one k-tile per work item (fused_tmem_kernel's J = 1): bf16 and int8 only
+template <uint32_t FMT, bool PAYLOAD>
+int launch_tmem_single(bool ybf, const TensorMaps &tms, const TmemParams &p, uint32_t grid, size_t smem, cudaStream_t st) {
+  return ybf ? launch_tmem_y<FMT, PAYLOAD, true, 1>(tms, p, grid, smem, st) : launch_tmem_y<FMT, PAYLOAD, false, 1>(tms, p, grid, smem, st);
 }
 
 // One launch over n <= kMaxProblems independent GEMMs that share format and tile geometry.
@@ -1125,14 +1136,22 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     }
   }
   // which design: decoded operand through tensor memory (fused_tmem.cuh) or through shared-memory operand slots
-  const uint32_t T = (ls && tmem_ok) ? tmem_teams(mpad_max, stream_bytes, h0.format) : 0u;
+  uint32_t xdepth = kXDepth, xdepth1 = kXDepth;
+  uint32_t T = (ls && tmem_ok) ? tmem_teams(mpad_max, stream_bytes, h0.format, &xdepth) : 0u;
+  const uint32_t T1 = (ls && tmem_ok) ? tmem_teams(mpad_max, stream_bytes, h0.format, &xdepth1, 1) : 0u;   // with one X slice per ring slot (J = 1)
   // The tensor-memory design works on pairs of k-tiles of one stripe.  A launch with fewer pairs than 0.6 x teams (few, long
   // tiles: e.g. 32 x 1024 int8 tiles of a 13824 x 5120 matrix) is bound by the sequential length of a tile pair; the
   // shared-memory design splits such a launch by single k-tiles and finishes sooner.
   uint64_t pairs = 0;
   for (int i = 0; i < n; ++i) pairs += uint64_t(ws[i]->h.n_out / kTileN) * ((ws[i]->h.k_in / ws[i]->h.tile_k + 1) / 2);
   const bool long_tiles = h0.tile_k / unit_k_of(h0.format) >= 32;
-  const bool use_tmem = T >= 2 && !(long_tiles && pairs * 10 < uint64_t(sm_budget()) * T * 6);
+  // ... unless no team gets more than one k-tile: then the tensor-memory kernel runs with ONE tile per work item and one chain
+  // per warp (J = 1), and the launch lasts one tile at a chain's latency instead of one pair at two interleaved chains'
+  uint64_t tiles_total = 0;
+  for (int i = 0; i < n; ++i) tiles_total += uint64_t(ws[i]->h.n_out / kTileN) * (ws[i]->h.k_in / ws[i]->h.tile_k);
+  const bool single = T1 >= 2 && (h0.format == ANSLIN_FMT_BF16 || h0.format == ANSLIN_FMT_INT8) && tiles_total <= uint64_t(sm_budget()) * T1;
+  if (single) { T = T1; xdepth = xdepth1; }
+  const bool use_tmem = T >= 2 && (single || !(long_tiles && pairs * 10 < uint64_t(sm_budget()) * T * 6));
   // CTAs: one per SM in total, shared out in proportion to the problems' sizes
   const uint32_t S = uint32_t(sm_budget());
   uint32_t ncta[kMaxProblems], cap[kMaxProblems];
@@ -1183,12 +1202,15 @@ int gemm_launch(int n, const anslin_weight *const *ws, const void *const *xs, ui
     p.xslice_bytes = mpad_max * 32u;
     p.tmem_stride = mpad_max + kASlotCols;
     p.afmt = afmt_of(h0.format); p.bfmt = bfmt_of(h0.format, x_dtype);
-    const size_t smem = tmem_smem_bytes(T, mpad_max, stream_bytes, h0.format);
+    p.xdepth = xdepth;
+    const size_t smem = tmem_smem_bytes(T, mpad_max, stream_bytes, h0.format, xdepth, single ? 1u : 2u);
     switch (h0.format) {
-      case ANSLIN_FMT_BF16: return pay ? launch_tmem<ANSLIN_FMT_BF16, true>(ybf, tms, p, grid, smem, st) : launch_tmem<ANSLIN_FMT_BF16, false>(ybf, tms, p, grid, smem, st);
+      case ANSLIN_FMT_BF16:
+        if (single) return pay ? launch_tmem_single<ANSLIN_FMT_BF16, true>(ybf, tms, p, grid, smem, st) : launch_tmem_single<ANSLIN_FMT_BF16, false>(ybf, tms, p, grid, smem, st);
+        return pay ? launch_tmem<ANSLIN_FMT_BF16, true>(ybf, tms, p, grid, smem, st) : launch_tmem<ANSLIN_FMT_BF16, false>(ybf, tms, p, grid, smem, st);
       case ANSLIN_FMT_FP8_E4M3:
       case ANSLIN_FMT_FP8_E5M2: return launch_tmem<ANSLIN_FMT_FP8_E4M3, false>(ybf, tms, p, grid, smem, st);
-      case ANSLIN_FMT_INT8: return launch_tmem<ANSLIN_FMT_INT8, false>(ybf, tms, p, grid, smem, st);
+      case ANSLIN_FMT_INT8: return single ? launch_tmem_single<ANSLIN_FMT_INT8, false>(ybf, tms, p, grid, smem, st) : launch_tmem<ANSLIN_FMT_INT8, false>(ybf, tms, p, grid, smem, st);
       case ANSLIN_FMT_INT4_AWQ: return launch_tmem<ANSLIN_FMT_INT4_AWQ, false>(ybf, tms, p, grid, smem, st);
       case ANSLIN_FMT_FP4_E2M1: return launch_tmem<ANSLIN_FMT_FP4_E2M1, false>(ybf, tms, p, grid, smem, st);
     }
@@ -1259,7 +1281,7 @@ size_t multi_workspace_bytes(const anslin_weight *const *ws, int n, int32_t m_ma
   size_t rows = mpad_of(m_max);
   if (tmem_ok)
     for (uint32_t mp = 16; mp <= mpad_of(m_max); mp += 16) {
-      const uint32_t T = tmem_teams(mp, stream_bytes, ws[0]->h.format);
+      const uint32_t T = std::max(tmem_teams(mp, stream_bytes, ws[0]->h.format), tmem_teams(mp, stream_bytes, ws[0]->h.format, nullptr, 1));
       if (T >= 2) rows = std::max(rows, size_t(T) * mp);
     }
   const size_t per_launch = size_t(std::max(sm_budget(), 148)) * 2 * rows * kTileN * 4;
