@@ -595,6 +595,25 @@ def test_gemm_bf16_full_size_projection(name, n, k, m, tile):
     dw.close()
 
 
+def test_gemm_bf16_odd_k_tiles_pair_items():
+    """An odd number of k-tiles per stripe on the tensor-memory kernel's PAIR work items (the last pair of a stripe has one
+    tile; more tiles than teams, so the one-tile work items of small launches are not chosen): 4096 x 4864 bf16, 19 k-tiles
+    of 256, M = 20, lane streams + payload; decode bit-exact, GEMM on sampled channels, run-to-run bit equality."""
+    rt = _rt()
+    n, k, m = 4096, 4864, 20
+    w = inputs.f32_to_bf16_bits(inputs.weights_f32(n, k, seed=131, jitter=True))
+    x = inputs.f32_to_bf16_bits(inputs.acts_f32(m, k, seed=132))
+    buf, _ = B.anslin_encode_host(B.FMT_BF16, w, n, k, tile_k=256, flags=3, tile_n=32)
+    dw = rt.DeviceWeight(buf)
+    assert np.array_equal(dw.decode().cpu().numpy().view(np.uint16), w)
+    xd = rt.x_to_device(B.FMT_BF16, x)
+    y = dw.gemm(xd).cpu().numpy()
+    cols = np.sort(np.random.default_rng(133).choice(n, size=768, replace=False))
+    check_gemm(y[:, cols], *og.gemm_bf16(x, w[cols]))
+    assert np.array_equal(y, dw.gemm(xd).cpu().numpy())
+    dw.close()
+
+
 # ------------------------------------------------------------------ BASELINE configs 3-5 at full size
 def _sample_cols(n, seed, count=512):
     return np.sort(np.random.default_rng(seed).choice(n, size=min(n, count), replace=False))
