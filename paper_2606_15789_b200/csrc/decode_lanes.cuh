@@ -201,6 +201,15 @@ __global__ void __launch_bounds__(kLaneDecWarps * 32, 1) decode_lanes_kernel(con
       unit_body(std::integral_constant<uint32_t, 0>{}, u);
       unit_body(std::integral_constant<uint32_t, 1>{}, u + 1);
     }
+#ifdef ANSLIN_BOUNDS_CHECK   // debug builds (compute-sanitizer is closed on this pool): every word cursor ended inside its staged buffer
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      const uint32_t lo = stage_s + uint32_t(j) * stream_bytes;
+      if (s[j].ptr + 2u < lo || s[j].ptr > lo + stream_bytes) __trap();
+      if (PAYLOAD && (s[j].x < kL || s[j].x >= 2u * kL)) __trap();   // the end state is L + payload
+      if (!PAYLOAD && s[j].x != kL) __trap();                        // ... or exactly the encoder's start state
+    }
+#endif
   }
   cp_async_wait_all();
   if (lane == 0) bulk_wait_read<0>();   // the boxes stay valid until the engine has read them
