@@ -411,6 +411,22 @@ __device__ __forceinline__ uint32_t awq_dequant2(uint32_t byte, __half2 zoff, __
   return *reinterpret_cast<const uint32_t *>(&h);
 }
 
+// The same for four packed bytes at once: the nibbles are split once, then every byte costs one PRMT (a selector nibble with
+// bit 3 set replicates the sign bit of the chosen byte, and a nibble byte is <= 0x0F: zero) and one OR before the two half2 ops.
+__device__ __forceinline__ void awq_dequant8(uint32_t Bq, __half2 zoff, __half2 sc, uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3) {
+  const uint32_t lo = Bq & 0x0F0F0F0Fu, hi = (Bq >> 4) & 0x0F0F0F0Fu;
+  uint32_t v0, v1, v2, v3;   // (PTX prmt: __byte_perm does not pass the selector's replicate bits through)
+  asm("prmt.b32 %0, %1, %2, 0x8480;" : "=r"(v0) : "r"(lo), "r"(hi));
+  asm("prmt.b32 %0, %1, %2, 0x9591;" : "=r"(v1) : "r"(lo), "r"(hi));
+  asm("prmt.b32 %0, %1, %2, 0xA6A2;" : "=r"(v2) : "r"(lo), "r"(hi));
+  asm("prmt.b32 %0, %1, %2, 0xB7B3;" : "=r"(v3) : "r"(lo), "r"(hi));
+  v0 |= 0x64006400u; v1 |= 0x64006400u; v2 |= 0x64006400u; v3 |= 0x64006400u;
+  __half2 h0 = __hmul2(__hsub2(*reinterpret_cast<const __half2 *>(&v0), zoff), sc), h1 = __hmul2(__hsub2(*reinterpret_cast<const __half2 *>(&v1), zoff), sc);
+  __half2 h2 = __hmul2(__hsub2(*reinterpret_cast<const __half2 *>(&v2), zoff), sc), h3 = __hmul2(__hsub2(*reinterpret_cast<const __half2 *>(&v3), zoff), sc);
+  o0 = *reinterpret_cast<const uint32_t *>(&h0); o1 = *reinterpret_cast<const uint32_t *>(&h1);
+  o2 = *reinterpret_cast<const uint32_t *>(&h2); o3 = *reinterpret_cast<const uint32_t *>(&h3);
+}
+
 // fp4-e2m1 (s.ee.m: 0, 0.5, 1, 1.5, 2, 3, 4, 6) -> the e4m3 byte of the same value, four codes at a time: the four
 // nibbles of sel[15:0] pick their magnitude byte from an 8-entry table held in two registers (PRMT), the sign
 // nibble-bit picks 0x00 / 0x80.  `mag` = codes & 0x7777..., `sgn` = (codes >> 3) & 0x1111... (upper 16 bits ignored).

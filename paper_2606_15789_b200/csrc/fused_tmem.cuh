@@ -190,8 +190,7 @@ __device__ __forceinline__ void decode_half_regs(LaneStream (&s)[J], uint32_t ta
       const __half2 szh = *reinterpret_cast<const __half2 *>(&sz[j]);
       const __half2 sc = __half2half2(__low2half(szh));
       const __half2 zoff = __hadd2(__half2half2(__high2half(szh)), __float2half2_rn(1024.f));
-#pragma unroll
-      for (int b = 0; b < 4; ++b) r[j][4 * H + b] = awq_dequant2((Bq[j] >> (8 * b)) & 0xFFu, zoff, sc);
+      awq_dequant8(Bq[j], zoff, sc, r[j][4 * H], r[j][4 * H + 1], r[j][4 * H + 2], r[j][4 * H + 3]);
     }
   } else if constexpr (FMT == ANSLIN_FMT_FP4_E2M1) {
 #pragma unroll
@@ -579,6 +578,7 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
         next_off[0] = offs[next_tile];
         if constexpr (J == 2) next_off[1] = offs[next_tile + (kn + 1 < KT ? 4u : 0u)];
       }
+      uint32_t sz_cur[J] = {}, sz_left = 0;   // int4: the current (scale, zero) pairs and the units they still hold for
       // One unit of both tiles.  A tile has an even number of units (tmem_eligible), so the parity PAR of a unit step — which
       // half of the operand columns, which raw buffer, which barriers — is a compile-time constant of each copy of the body.
       auto unit_body = [&](auto par_c, const uint32_t u) {
@@ -656,12 +656,20 @@ __global__ void __launch_bounds__(kTmemThreads, 1) fused_tmem_kernel(const __gri
           }
         }
         if constexpr (FMT == ANSLIN_FMT_INT4_AWQ) {
+          // this lane's (scale, zero) pairs: loaded again only where a tile's k range enters another quantisation group
+          if (sz_left == 0) {
+            sz_left = 0xFFFFFFFFu;
 #pragma unroll
-          for (int j = 0; j < J; ++j) {
-            const uint32_t k_elem = (ktA + uint32_t(j)) * tile_k + u * kUnitK;
-            sz[j] = __ldg(reinterpret_cast<const uint32_t *>(cbase + off_scales) + size_t(k_elem / qgroup) * n_out + size_t(stripe) * kTileN +
-                          q * 32u + uint32_t(lane));
+            for (int j = 0; j < J; ++j) {
+              const uint32_t k_elem = (ktA + uint32_t(j)) * tile_k + u * kUnitK;
+              sz_cur[j] = __ldg(reinterpret_cast<const uint32_t *>(cbase + off_scales) + size_t(k_elem / qgroup) * n_out + size_t(stripe) * kTileN +
+                                q * 32u + uint32_t(lane));
+              sz_left = min(sz_left, (qgroup - k_elem % qgroup) / kUnitK);   // units until chain j's next group (group sizes are multiples of 16)
+            }
           }
+          --sz_left;
+#pragma unroll
+          for (int j = 0; j < J; ++j) sz[j] = sz_cur[j];
         }
         // have the MMAs that read this half of the operand columns two steps ago finished?  (On fresh barriers the parity
         // of the "previous" phase passes at once.)  Asked now, needed after the unit is decoded.
