@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libanslin.so")
 SOURCES = ["kernels.cu", "histogram.cu", "encode_gpu.cu", "host.cpp"]
-HEADERS = ["anslin_internal.h", "decode_core.cuh", "fused_tmem.cuh", os.path.join("..", "..", "include", "anslin.h")]
+HEADERS = ["anslin_internal.h", "decode_core.cuh", "fused_tmem.cuh", "decode_lanes.cuh", os.path.join("..", "..", "include", "anslin.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC,-O3,-pthread", "--use_fast_math", "-Xptxas", "-v"]
 

@@ -9,17 +9,22 @@
 //   * every warp runs Alg V.2 (P:l.260-287) on TWO tiles at once (k-tiles kt, kt+1 of its stripe quadrant), their
 //     steps interleaved, so a team hands the tensor core two K slices per unit step; the operand columns are double
 //     buffered, so a decoder warp never waits for the tensor core in steady state;
+//     (template parameter J = 1: ONE tile per warp and work item, for launches with at most one tile per team);
+//   * a unit's tcgen05.st are published (wait::st, fence, mbarrier arrive) from the middle of the NEXT unit, and the unit loop
+//     is unrolled by two, so that operand half, raw buffer and barrier addresses are immediates;
+//   * staged lane-stream segments arrive by one cp.async.bulk per record on a per-warp mbarrier;
 //   * one ISSUER warp per team (the paper's consumer warps, P:l.226-247): it sleeps on the team's "operand stored"
 //     mbarrier, issues the two tcgen05.mma of the unit step (A from TMEM, X slice from shared memory, accumulator in
 //     TMEM), commits them to the barrier that frees the operand columns ("ready[2]" flags of P:l.210 -> mbarriers), and
-//     requests the X slices (pad16(m) rows x 32 bytes, SWIZZLE_32B) of the unit step two ahead by TMA into a 3-deep ring;
+//     requests the X slices (pad16(m) rows x 32 bytes, SWIZZLE_32B) of the unit step two ahead by TMA into a 3-deep ring
+//     (2-deep, one step ahead, where shared memory is short);
 //   * nothing in the decode loop waits for HBM: the bf16 sign/mantissa bytes of the NEXT unit travel by cp.async into a
 //     shared-memory double buffer (a register-destination global load shares scoreboards with the loop's LDS and
 //     stalled every unit for an HBM round trip);
 //   * the team reads its own accumulator back (tcgen05.ld: warp q -> lanes 32q..) at the end of a stripe segment;
 //   * split-K: a team is a "virtual CTA" of a two-level stream-K split (pairs evenly over the CTAs, then over a CTA's
-//     teams).  Every contributor of a stripe stores its partial, raises a flag, waits for the other contributors' flags
-//     and then reduces ITS OWN slice of the stripe's outputs, summing the contributors in team order (bit-reproducible;
+//     teams).  Every contributor of a stripe stores its partial, raises one flag per reader, waits for the flags addressed
+//     to it and then reduces ITS OWN slice of the stripe's outputs, summing the contributors in team order (bit-reproducible;
 //     the reduction is spread over all contributors instead of falling on one of them).
 // TMEM budget: T teams x (pad16(m) accumulator columns + 32 operand columns) <= 512  ->  T = 4 up to m = 96.
 #pragma once

@@ -1,10 +1,14 @@
-// libanslin device side (sm_100a): decode-only kernel, the two fused rANS-decode + tcgen05 GEMM kernels, the dense
+// libanslin device side (sm_100a): the decode-only kernels, the two fused rANS-decode + tcgen05 GEMM kernels, the dense
 // tcgen05 comparator, and their C-ABI launchers.
+//
+// Decode only (anslin_decode): decode_lanes_kernel (decode_lanes.cuh) for lane-stream containers with 32-row tiles — decoded
+//   rows leave through TMA stores — and decode_kernel (below) for every other layout.
 //
 // Fused kernel = Alg V.1 (P:l.196-252) re-designed for Blackwell:
 //   * fused_tmem_kernel (fused_tmem.cuh): lane-stream containers with 32-row tiles.  Teams of four decoder warps hand the
 //     decoded operand to the tensor core through TENSOR MEMORY (tcgen05.st -> tcgen05.mma with A in TMEM); one issuer warp
-//     per team issues the MMAs and the TMA loads of the X slices; stream-K split over teams.  The path bench.py times.
+//     per team issues the MMAs and the TMA loads of the X slices; stream-K split over teams; a work item is a pair of
+//     k-tiles (two chains per warp) or, in launches with at most one tile per team, a single k-tile.  The path bench.py times.
 //   * fused_gemm_kernel (below): every other container layout, batches above 96 rows, and launches of few, long tile pairs.
 //     The paper's single producer warp becomes up to 16 decoder warps per CTA (decode is the bottleneck at small batch,
 //     P:l.306), the consumer warps become ONE thread issuing tcgen05.mma with the accumulator in TMEM; ready[2] flags
